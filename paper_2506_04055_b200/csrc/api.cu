@@ -1,0 +1,598 @@
+// api.cu -- the C ABI of include/mlp.h: weight blob parsing, buffer management (fixed capacity, grow on
+// overflow: PAPER.md:84-86) and the per-timestep orchestration of the hot path.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/mlp.h"
+#include "common.cuh"
+
+using namespace painn;
+
+namespace {
+
+struct Buf {
+    void* p = nullptr;
+    size_t bytes = 0;
+};
+
+enum Stage { ST_NBR = 0, ST_FWD_NODE, ST_FWD_EDGE, ST_BWD_NODE, ST_BWD_EDGE, ST_FORCE, ST_COUNT };
+const char* kStageNames[ST_COUNT] = {"nbr_build", "fwd_node", "fwd_edge", "bwd_node", "bwd_edge", "force_virial"};
+
+struct LayerBuf {
+    float *hpre, *phi, *sn, *v1, *pq, *zpre, *a;
+};
+
+}  // namespace
+
+struct mlp_model {
+    int n_species = 0, F = 0, K = 0, T = 0, R = 0;
+    double rc = 0, eps = 0;
+    // weights (device, fp32)
+    std::vector<Buf> wbufs;
+    float* Emb = nullptr;
+    LayerW lw[PAINN_MAX_T];
+    float *Wr1 = nullptr, *br1 = nullptr, *wr2 = nullptr, *br2 = nullptr, *Wr1T = nullptr;
+    // capacities
+    long long cap_atoms = 0, cap_edges = 0, cap_cells = 0;
+    std::vector<Buf*> all;
+    // atom-sized
+    Buf b_cell_id, b_wrap, b_perm, b_inv_perm, b_pos_s, b_types_s, b_wrap_s, b_cell_s, b_local, b_row_cnt, b_row_ptr,
+        b_scan_tmp;
+    // cell-sized
+    Buf b_cell_count, b_cell_start, b_cell_fill;
+    // edge-sized
+    Buf b_ej, b_img, b_rev, b_G;
+    // node feature buffers
+    Buf b_S[PAINN_MAX_T + 1], b_V[PAINN_MAX_T + 1];
+    Buf b_hpre[PAINN_MAX_T], b_phi[PAINN_MAX_T], b_sn[PAINN_MAX_T], b_v1[PAINN_MAX_T], b_pq[PAINN_MAX_T],
+        b_zpre[PAINN_MAX_T], b_a[PAINN_MAX_T];
+    Buf b_h, b_rpre, b_rb, b_eatom, b_sb, b_s1b, b_vb, b_v1b, b_ab, b_pqb, b_gb, b_snb, b_phib, b_hb;
+    Buf b_epart, b_wpart;
+    // small
+    Buf b_misc;            // device: [0..7] flags (int), then long long totals, then bbox doubles
+    void* h_misc = nullptr;   // pinned mirror
+    // host staging for mlp_compute_host
+    Buf d_pos, d_types, d_owner, d_out;   // d_out: energy[1] virial[6] forces[3N]
+    cudaStream_t own_stream = nullptr;
+    // last call
+    long long N_last = 0, n_local_last = 0, E_last = 0;
+    Grid grid_last{};
+    mlp_stats stats{};
+    std::string err;
+    // stage timing
+    bool timing = false;
+    std::vector<cudaEvent_t> ev_pool;
+    std::vector<std::pair<int, cudaEvent_t>> marks;
+    long long forced_edge_cap = 0;
+};
+
+namespace {
+
+const char* kNoModel = "mlp: NULL model";
+
+int fail(mlp_model* m, int code, const std::string& msg) {
+    if (m) m->err = msg;
+    return code;
+}
+#define CU(m, call)                                                                                   \
+    do {                                                                                              \
+        cudaError_t e_ = (call);                                                                      \
+        if (e_ != cudaSuccess)                                                                        \
+            return fail(m, e_ == cudaErrorMemoryAllocation ? MLP_ERR_NOMEM : MLP_ERR_CUDA,            \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));                          \
+    } while (0)
+
+int ensure(mlp_model* m, Buf& b, size_t bytes, bool count_regrow = true) {
+    if (bytes <= b.bytes) return MLP_OK;
+    if (b.p) {
+        CU(m, cudaFree(b.p));
+        m->stats.device_bytes -= (long long)b.bytes;
+        b.p = nullptr;
+        b.bytes = 0;
+    }
+    if (bytes == 0) return MLP_OK;
+    CU(m, cudaMalloc(&b.p, bytes));
+    b.bytes = bytes;
+    m->stats.device_bytes += (long long)bytes;
+    (void)count_regrow;
+    return MLP_OK;
+}
+#define ENS(m, b, bytes)                             \
+    do {                                             \
+        int r_ = ensure(m, b, (size_t)(bytes));      \
+        if (r_ != MLP_OK) return r_;                 \
+    } while (0)
+
+template <class T>
+T* P(const Buf& b) { return reinterpret_cast<T*>(b.p); }
+
+int upload(mlp_model* m, const std::vector<float>& h, float** out) {
+    Buf b;
+    ENS(m, b, h.size() * sizeof(float));
+    CU(m, cudaMemcpy(b.p, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice));
+    m->wbufs.push_back(b);
+    *out = (float*)b.p;
+    return MLP_OK;
+}
+std::vector<float> to_f32(const double* p, size_t n) {
+    std::vector<float> v(n);
+    for (size_t i = 0; i < n; i++) v[i] = (float)p[i];
+    return v;
+}
+std::vector<float> transpose(const std::vector<float>& w, int rows, int cols) {   // [rows x cols] -> [cols x rows]
+    std::vector<float> t((size_t)rows * cols);
+    for (int r = 0; r < rows; r++)
+        for (int c = 0; c < cols; c++) t[(size_t)c * rows + r] = w[(size_t)r * cols + c];
+    return t;
+}
+
+int alloc_atoms(mlp_model* m, long long cap) {
+    const size_t F = m->F, R = m->R, n = (size_t)cap;
+    ENS(m, m->b_cell_id, n * 4); ENS(m, m->b_wrap, n * 3); ENS(m, m->b_perm, n * 4); ENS(m, m->b_inv_perm, n * 4);
+    ENS(m, m->b_pos_s, n * 24); ENS(m, m->b_types_s, n * 4); ENS(m, m->b_wrap_s, n * 3); ENS(m, m->b_cell_s, n * 4);
+    ENS(m, m->b_local, n * 4); ENS(m, m->b_row_cnt, n * 4); ENS(m, m->b_row_ptr, (n + 1) * 4);
+    ENS(m, m->b_scan_tmp, (n / 4096 + 2) * 4);
+    for (int t = 0; t <= m->T; t++) { ENS(m, m->b_S[t], n * F * 4); ENS(m, m->b_V[t], n * 3 * F * 4); }
+    for (int t = 0; t < m->T; t++) {
+        ENS(m, m->b_hpre[t], n * F * 4); ENS(m, m->b_phi[t], n * 3 * F * 4); ENS(m, m->b_sn[t], n * 2 * F * 4);
+        ENS(m, m->b_v1[t], n * 3 * F * 4); ENS(m, m->b_pq[t], n * 6 * F * 4); ENS(m, m->b_zpre[t], n * F * 4);
+        ENS(m, m->b_a[t], n * 3 * F * 4);
+    }
+    ENS(m, m->b_h, n * F * 4); ENS(m, m->b_rpre, n * R * 4); ENS(m, m->b_rb, n * R * 4); ENS(m, m->b_eatom, n * 4);
+    ENS(m, m->b_sb, n * F * 4); ENS(m, m->b_s1b, n * F * 4); ENS(m, m->b_vb, n * 3 * F * 4);
+    ENS(m, m->b_v1b, n * 3 * F * 4); ENS(m, m->b_ab, n * 3 * F * 4); ENS(m, m->b_pqb, n * 6 * F * 4);
+    ENS(m, m->b_gb, n * F * 4); ENS(m, m->b_snb, n * 2 * F * 4); ENS(m, m->b_phib, n * 3 * F * 4);
+    ENS(m, m->b_hb, n * F * 4);
+    ENS(m, m->b_epart, (n / 256 + 2) * 8); ENS(m, m->b_wpart, (n / 8 + 2) * 9 * 8);
+    m->cap_atoms = cap;
+    return MLP_OK;
+}
+int alloc_edges(mlp_model* m, long long cap) {
+    const size_t n = (size_t)cap;
+    ENS(m, m->b_ej, n * 16); ENS(m, m->b_img, n); ENS(m, m->b_rev, n * 4); ENS(m, m->b_G, n * 16);
+    m->cap_edges = cap;
+    return MLP_OK;
+}
+int alloc_cells(mlp_model* m, long long cap) {
+    const size_t n = (size_t)cap;
+    ENS(m, m->b_cell_count, (n + 1) * 4); ENS(m, m->b_cell_start, (n + 2) * 4); ENS(m, m->b_cell_fill, (n + 1) * 4);
+    m->cap_cells = cap;
+    return MLP_OK;
+}
+
+void free_buf(Buf& b, mlp_model* m = nullptr) {
+    if (b.p) cudaFree(b.p);
+    if (m) m->stats.device_bytes -= (long long)b.bytes;
+    b.p = nullptr;
+    b.bytes = 0;
+}
+
+// layout of b_misc / h_misc
+struct Misc {
+    int flags[8];
+    long long cell_total;
+    long long edge_total;
+    double bbox[6 + 6 * 256];
+};
+
+void mark(mlp_model* m, cudaStream_t st, int stage) {
+    if (!m->timing) return;
+    size_t k = m->marks.size();
+    if (k >= m->ev_pool.size()) {
+        cudaEvent_t e;
+        cudaEventCreate(&e);
+        m->ev_pool.push_back(e);
+    }
+    cudaEventRecord(m->ev_pool[k], st);
+    m->marks.push_back({stage, m->ev_pool[k]});
+}
+
+}  // namespace
+
+extern "C" {
+
+__attribute__((visibility("default"))) const char* mlp_version(void) { return "painn-b200 0.1.0 sm_100a"; }
+
+__attribute__((visibility("default"))) const char* mlp_last_error(mlp_model* m) { return m ? m->err.c_str() : kNoModel; }
+
+__attribute__((visibility("default"))) int mlp_create(const void* weights, size_t nbytes, int n_species, double cutoff, long long capacity,
+               mlp_model** out) {
+    if (!out) return MLP_ERR_ARG;
+    *out = nullptr;
+    if (!weights || capacity <= 0) return MLP_ERR_ARG;
+    const unsigned char* b = (const unsigned char*)weights;
+    if (nbytes < 48 || memcmp(b, "PNN1", 4) != 0) return MLP_ERR_WEIGHTS;
+    uint32_t h[7];
+    memcpy(h, b + 4, sizeof h);
+    double rc, eps;
+    memcpy(&rc, b + 32, 8);
+    memcpy(&eps, b + 40, 8);
+    if (h[0] != 1) return MLP_ERR_WEIGHTS;
+    const int ns = (int)h[1], F = (int)h[2], K = (int)h[3], T = (int)h[4], R = (int)h[5];
+    if (ns != n_species || rc != cutoff || !(rc > 0)) return MLP_ERR_WEIGHTS;
+    if (!(F == 32 || F == 64 || F == 128) || K < 1 || K > PAINN_MAX_K || T < 1 || T > PAINN_MAX_T || R != F / 2 ||
+        ns < 1)
+        return MLP_ERR_WEIGHTS;
+    size_t per_layer = (size_t)F * F + F + 3 * F * F + 3 * F + 3 * F * K + 3 * F + 2 * (size_t)F * F + 2 * F * F + F +
+                       3 * F * F + 3 * F;
+    size_t n_dbl = (size_t)ns * F + T * per_layer + (size_t)R * F + R + R + 1;
+    if (nbytes != 48 + 8 * n_dbl) return MLP_ERR_WEIGHTS;
+
+    int dev_count = 0;
+    if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0) return MLP_ERR_CUDA;
+
+    mlp_model* m = new (std::nothrow) mlp_model();
+    if (!m) return MLP_ERR_NOMEM;
+    m->n_species = ns; m->F = F; m->K = K; m->T = T; m->R = R; m->rc = rc; m->eps = eps;
+    std::vector<double> w(n_dbl);
+    memcpy(w.data(), b + 48, 8 * n_dbl);
+    const double* p = w.data();
+    int rcode = MLP_OK;
+    auto up = [&](size_t n, float** dst, std::vector<float>* keep = nullptr) {
+        if (rcode != MLP_OK) { p += n; return; }
+        std::vector<float> v = to_f32(p, n);
+        p += n;
+        rcode = upload(m, v, dst);
+        if (keep) *keep = v;
+    };
+    auto upT = [&](const std::vector<float>& v, int rows, int cols, float** dst) {
+        if (rcode != MLP_OK) return;
+        rcode = upload(m, transpose(v, rows, cols), dst);
+    };
+    up((size_t)ns * F, &m->Emb);
+    for (int t = 0; t < T; t++) {
+        LayerW& l = m->lw[t];
+        std::vector<float> Wm1, Wm2, U, V, Wu1, Wu2;
+        float* tmp;
+        up((size_t)F * F, (float**)&l.Wm1, &Wm1); up(F, (float**)&l.bm1);
+        up((size_t)3 * F * F, (float**)&l.Wm2, &Wm2); up(3 * F, (float**)&l.bm2);
+        up((size_t)3 * F * K, (float**)&l.Wf); up(3 * F, (float**)&l.bf);
+        // U and V are consecutive in the blob -> stacked [2F x F] matrix UV = [U ; V]
+        std::vector<float> UV = to_f32(p, (size_t)2 * F * F);
+        p += (size_t)2 * F * F;
+        if (rcode == MLP_OK) rcode = upload(m, UV, &tmp);
+        l.UV = tmp;
+        up((size_t)F * 2 * F, (float**)&l.Wu1, &Wu1); up(F, (float**)&l.bu1);
+        up((size_t)3 * F * F, (float**)&l.Wu2, &Wu2); up(3 * F, (float**)&l.bu2);
+        upT(Wm1, F, F, (float**)&l.Wm1T);
+        upT(Wm2, 3 * F, F, (float**)&l.Wm2T);
+        upT(UV, 2 * F, F, (float**)&l.UVT);
+        upT(Wu1, F, 2 * F, (float**)&l.Wu1T);
+        upT(Wu2, 3 * F, F, (float**)&l.Wu2T);
+    }
+    std::vector<float> Wr1;
+    up((size_t)R * F, &m->Wr1, &Wr1); up(R, &m->br1); up(R, &m->wr2); up(1, &m->br2);
+    upT(Wr1, R, F, &m->Wr1T);
+    if (rcode == MLP_OK) rcode = ensure(m, m->b_misc, sizeof(Misc));
+    if (rcode == MLP_OK && cudaMallocHost(&m->h_misc, sizeof(Misc)) != cudaSuccess) rcode = MLP_ERR_NOMEM;
+    if (rcode == MLP_OK && cudaStreamCreateWithFlags(&m->own_stream, cudaStreamNonBlocking) != cudaSuccess)
+        rcode = MLP_ERR_CUDA;
+    if (rcode == MLP_OK) rcode = alloc_atoms(m, capacity);
+    if (rcode == MLP_OK) rcode = alloc_edges(m, 64 * capacity);
+    if (rcode == MLP_OK) rcode = alloc_cells(m, capacity + 1024);
+    if (rcode != MLP_OK) {
+        mlp_destroy(m);
+        return rcode;
+    }
+    m->stats.atom_capacity = m->cap_atoms;
+    m->stats.edge_capacity = m->cap_edges;
+    *out = m;
+    return MLP_OK;
+}
+
+__attribute__((visibility("default"))) void mlp_destroy(mlp_model* m) {
+    if (!m) return;
+    for (Buf& b : m->wbufs) free_buf(b);
+    Buf* bs[] = {&m->b_cell_id, &m->b_wrap, &m->b_perm, &m->b_inv_perm, &m->b_pos_s, &m->b_types_s, &m->b_wrap_s,
+                 &m->b_cell_s, &m->b_local, &m->b_row_cnt, &m->b_row_ptr, &m->b_scan_tmp, &m->b_cell_count,
+                 &m->b_cell_start, &m->b_cell_fill, &m->b_ej, &m->b_img, &m->b_rev, &m->b_G, &m->b_h, &m->b_rpre,
+                 &m->b_rb, &m->b_eatom, &m->b_sb, &m->b_s1b, &m->b_vb, &m->b_v1b, &m->b_ab, &m->b_pqb, &m->b_gb,
+                 &m->b_snb, &m->b_phib, &m->b_hb, &m->b_epart, &m->b_wpart, &m->b_misc, &m->d_pos, &m->d_types,
+                 &m->d_owner, &m->d_out};
+    for (Buf* b : bs) free_buf(*b);
+    for (int t = 0; t <= PAINN_MAX_T; t++) { free_buf(m->b_S[t]); free_buf(m->b_V[t]); }
+    for (int t = 0; t < PAINN_MAX_T; t++) {
+        free_buf(m->b_hpre[t]); free_buf(m->b_phi[t]); free_buf(m->b_sn[t]); free_buf(m->b_v1[t]);
+        free_buf(m->b_pq[t]); free_buf(m->b_zpre[t]); free_buf(m->b_a[t]);
+    }
+    if (m->h_misc) cudaFreeHost(m->h_misc);
+    if (m->own_stream) cudaStreamDestroy(m->own_stream);
+    for (cudaEvent_t e : m->ev_pool) cudaEventDestroy(e);
+    delete m;
+}
+
+__attribute__((visibility("default"))) int mlp_set_option(mlp_model* m, const char* name, long long value) {
+    if (!m || !name) return MLP_ERR_ARG;
+    if (!strcmp(name, "stage_timing")) { m->timing = value != 0; return MLP_OK; }
+    if (!strcmp(name, "gemm_emulate")) { painn::g_gemm_emulate = (int)value; return MLP_OK; }
+    if (!strcmp(name, "edge_capacity")) {
+        if (value <= 0) return fail(m, MLP_ERR_ARG, "edge_capacity must be > 0");
+        // shrink-or-set (test hook): drop the edge buffers and reallocate at the requested size
+        free_buf(m->b_ej, m); free_buf(m->b_img, m); free_buf(m->b_rev, m); free_buf(m->b_G, m);
+        int r = alloc_edges(m, value);
+        m->stats.edge_capacity = m->cap_edges;
+        return r;
+    }
+    return fail(m, MLP_ERR_ARG, std::string("unknown option ") + name);
+}
+
+__attribute__((visibility("default"))) int mlp_get_stats(mlp_model* m, mlp_stats* out) {
+    if (!m || !out) return MLP_ERR_ARG;
+    *out = m->stats;
+    return MLP_OK;
+}
+
+__attribute__((visibility("default"))) int mlp_get_stage_ms(mlp_model* m, int max_stages, const char** names, float* ms) {
+    if (!m || !names || !ms || max_stages < 0) return -MLP_ERR_ARG;
+    float acc[ST_COUNT] = {0};
+    if (m->marks.size() >= 2) {
+        if (cudaEventSynchronize(m->marks.back().second) != cudaSuccess) return -MLP_ERR_CUDA;
+        for (size_t k = 0; k + 1 < m->marks.size(); k++) {
+            float t = 0;
+            cudaEventElapsedTime(&t, m->marks[k].second, m->marks[k + 1].second);
+            int s = m->marks[k].first;
+            if (s >= 0 && s < ST_COUNT) acc[s] += t;
+        }
+    }
+    int n = max_stages < ST_COUNT ? max_stages : ST_COUNT;
+    for (int k = 0; k < n; k++) { names[k] = kStageNames[k]; ms[k] = acc[k]; }
+    return n;
+}
+
+__attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const double* pos, const int* types, const double* box, long long n_local,
+                long long n_ghost, const int* ghost_owner, double* energy, double* forces, double* virial,
+                void* cuda_stream) {
+    if (!m) return MLP_ERR_ARG;
+    if (!box || n_local < 0 || n_ghost < 0 || !energy || !virial) return fail(m, MLP_ERR_ARG, "bad argument");
+    const long long N = n_local + n_ghost;
+    if (N > 0 && (!pos || !types || !forces)) return fail(m, MLP_ERR_ARG, "NULL atom array");
+    if (N >= (1ll << 31)) return fail(m, MLP_ERR_ARG, "too many atoms");
+    for (int d = 0; d < 3; d++)
+        if (!std::isfinite(box[d]) || !(box[d] > 0)) return fail(m, MLP_ERR_NONFINITE, "box length not finite/positive");
+    const bool periodic = n_ghost == 0;
+    if (periodic)
+        for (int d = 0; d < 3; d++)
+            if (box[d] < 2.0 * m->rc) return fail(m, MLP_ERR_BOX_TOO_SMALL, "periodic box length < 2 * cutoff");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    long long launches = 0;
+    Launch L{st, &launches};
+    m->marks.clear();
+    m->stats.n_calls++;
+    const int F = m->F, K = m->K, T = m->T, R = m->R;
+    const float rcf = (float)m->rc;
+
+    // ---- capacity (atoms): buffers only grow ----
+    if (N > m->cap_atoms) {
+        long long nc = std::max(N, (long long)(1.5 * m->cap_atoms));
+        int r = alloc_atoms(m, nc);
+        if (r != MLP_OK) return r;
+        m->stats.n_regrow++;
+    }
+    Misc* dm = P<Misc>(m->b_misc);
+    Misc* hm = (Misc*)m->h_misc;
+    CU(m, cudaMemsetAsync(dm, 0, sizeof(int) * 8 + 16, st));
+    mark(m, st, ST_NBR);
+
+    // ---- cell grid ----
+    Grid g{};
+    g.periodic = periodic ? 1 : 0;
+    g.rc2 = m->rc * m->rc;
+    double lo[3] = {0, 0, 0}, ext[3] = {box[0], box[1], box[2]};
+    if (!periodic) {
+        nbr_bbox(L, pos, N, dm->bbox);
+        CU(m, cudaMemcpyAsync(hm->bbox, dm->bbox, 6 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CU(m, cudaStreamSynchronize(st));
+        for (int d = 0; d < 3; d++) {
+            if (!(hm->bbox[d] <= hm->bbox[3 + d])) return fail(m, MLP_ERR_NONFINITE, "no finite positions");
+            lo[d] = hm->bbox[d];
+            ext[d] = hm->bbox[3 + d] - hm->bbox[d];
+        }
+    }
+    const double min_side = m->rc * (1.0 + 1e-9);
+    long long ncells = 1;
+    for (int d = 0; d < 3; d++) {
+        long long n = (long long)std::floor(ext[d] / min_side);
+        if (n < 1) n = 1;
+        if (!periodic) n += 1;   // open mode: side = rc(1+1e-9) exactly, last cell partially filled
+        g.n[d] = (int)n;
+        g.origin[d] = lo[d];
+        g.box[d] = box[d];
+        g.inv_side[d] = periodic ? (double)n / ext[d] : 1.0 / min_side;
+        ncells *= n;
+    }
+    // cap the grid (sparse / huge bounding boxes): coarser cells are still correct, only slower
+    const long long max_cells = std::max<long long>(4 * N + 4096, 32768);
+    while (ncells > max_cells) {
+        int dmax = 0;
+        for (int d = 1; d < 3; d++) if (g.n[d] > g.n[dmax]) dmax = d;
+        int nn = (g.n[dmax] + 1) / 2;
+        if (periodic) g.inv_side[dmax] = (double)nn / ext[dmax];
+        else { g.inv_side[dmax] *= 0.5; }
+        g.n[dmax] = nn;
+        ncells = (long long)g.n[0] * g.n[1] * g.n[2];
+    }
+    if (ncells > m->cap_cells) {
+        int r = alloc_cells(m, ncells + ncells / 2);
+        if (r != MLP_OK) return r;
+    }
+    m->grid_last = g;
+    int* cell_count = P<int>(m->b_cell_count);
+    int* cell_start = P<int>(m->b_cell_start);
+    int* cell_fill = P<int>(m->b_cell_fill);
+    CU(m, cudaMemsetAsync(cell_count, 0, (size_t)(ncells + 1) * 4, st));
+    CU(m, cudaMemsetAsync(cell_fill, 0, (size_t)(ncells + 1) * 4, st));
+
+    // ---- a0-a3 neighbour build ----
+    nbr_bin(L, pos, types, N, m->n_species, g, P<int>(m->b_cell_id), P<signed char>(m->b_wrap), cell_count, dm->flags);
+    exclusive_scan(L, cell_count, cell_start, ncells, P<int>(m->b_scan_tmp), &dm->cell_total);
+    nbr_place(L, N, ncells, P<int>(m->b_cell_id), cell_start, cell_fill, P<int>(m->b_perm));
+    nbr_sort_cells(L, ncells, cell_start, P<int>(m->b_perm));
+    nbr_gather(L, N, n_local, P<int>(m->b_perm), pos, types, P<signed char>(m->b_wrap), P<double>(m->b_pos_s),
+               P<int>(m->b_types_s), P<signed char>(m->b_wrap_s), P<int>(m->b_inv_perm), P<float>(m->b_local),
+               P<int>(m->b_cell_id), P<int>(m->b_cell_s));
+    nbr_count(L, N, g, P<double>(m->b_pos_s), P<signed char>(m->b_wrap_s), P<int>(m->b_cell_s), cell_start,
+              P<int>(m->b_row_cnt));
+    exclusive_scan(L, P<int>(m->b_row_cnt), P<int>(m->b_row_ptr), N, P<int>(m->b_scan_tmp), &dm->edge_total);
+    // the one host read of the call: error flags + edge count (overflow check)
+    CU(m, cudaMemcpyAsync(hm, dm, sizeof(int) * 8 + 16, cudaMemcpyDeviceToHost, st));
+    CU(m, cudaStreamSynchronize(st));
+    if (hm->flags[0] & FLAG_NONFINITE) return fail(m, MLP_ERR_NONFINITE, "non-finite (or absurdly far) position");
+    if (hm->flags[0] & FLAG_TYPE_RANGE) return fail(m, MLP_ERR_TYPE_RANGE, "atom type outside 0..n_species-1");
+    const long long E = hm->edge_total;
+    if (E >= (1ll << 31) - 64) return fail(m, MLP_ERR_NOMEM, "more than 2^31 edges");
+    if (E > m->cap_edges) {
+        // enlarge: x1.5, at least the counted need plus head-room ("overflown and nearly filled")
+        long long nc = std::max((long long)(1.5 * m->cap_edges), E + E / 8);
+        free_buf(m->b_ej, m); free_buf(m->b_img, m); free_buf(m->b_rev, m); free_buf(m->b_G, m);
+        int r = alloc_edges(m, nc);
+        if (r != MLP_OK) return r;
+        m->stats.n_regrow++;
+    }
+    float4* ej = P<float4>(m->b_ej);
+    const int* row_ptr = P<int>(m->b_row_ptr);
+    nbr_fill(L, N, g, P<double>(m->b_pos_s), P<signed char>(m->b_wrap_s), P<int>(m->b_cell_s), cell_start, row_ptr,
+             m->cap_edges, ej, P<unsigned char>(m->b_img), dm->flags);
+    nbr_reverse(L, N, row_ptr, ej, P<unsigned char>(m->b_img), P<int>(m->b_rev));
+
+    // ---- forward ----
+    mark(m, st, ST_FWD_NODE);
+    embed(L, N, F, P<int>(m->b_types_s), m->Emb, P<float>(m->b_S[0]), P<float>(m->b_V[0]));
+    float* h = P<float>(m->b_h);
+    for (int t = 0; t < T; t++) {
+        const LayerW& l = m->lw[t];
+        float *S = P<float>(m->b_S[t]), *V = P<float>(m->b_V[t]);
+        float *hpre = P<float>(m->b_hpre[t]), *phi = P<float>(m->b_phi[t]), *sn = P<float>(m->b_sn[t]),
+              *v1 = P<float>(m->b_v1[t]), *pq = P<float>(m->b_pq[t]), *zpre = P<float>(m->b_zpre[t]),
+              *a = P<float>(m->b_a[t]);
+        gemm_nt(L, S, F, l.Wm1, F, hpre, F, N, F, F, l.bm1, false);
+        silu_fwd(L, N * F, hpre, h);
+        gemm_nt(L, h, F, l.Wm2, F, phi, 3 * F, N, 3 * F, F, l.bm2, false);
+        mark(m, st, ST_FWD_EDGE);
+        message_fwd(L, N, F, K, rcf, row_ptr, ej, S, V, phi, l.Wf, l.bf, sn, v1);
+        mark(m, st, ST_FWD_NODE);
+        gemm_nt(L, v1, F, l.UV, F, pq, 2 * F, 3 * N, 2 * F, F, nullptr, false);
+        update_mid(L, N, F, (float)m->eps, pq, sn);
+        gemm_nt(L, sn, 2 * F, l.Wu1, 2 * F, zpre, F, N, F, 2 * F, l.bu1, false);
+        silu_fwd(L, N * F, zpre, h);
+        gemm_nt(L, h, F, l.Wu2, F, a, 3 * F, N, 3 * F, F, l.bu2, false);
+        update_out(L, N, F, sn, v1, pq, a, P<float>(m->b_S[t + 1]), P<float>(m->b_V[t + 1]));
+    }
+    int n_epart = 0, n_wpart = 0;
+    gemm_nt(L, P<float>(m->b_S[T]), F, m->Wr1, F, P<float>(m->b_rpre), R, N, R, F, m->br1, false);
+    readout(L, N, R, P<float>(m->b_rpre), m->wr2, m->br2, P<float>(m->b_local), P<float>(m->b_rb),
+            P<float>(m->b_eatom), P<double>(m->b_epart), &n_epart);
+
+    // ---- backward ----
+    mark(m, st, ST_BWD_NODE);
+    float *sb = P<float>(m->b_sb), *s1b = P<float>(m->b_s1b), *vb = P<float>(m->b_vb), *v1b = P<float>(m->b_v1b);
+    gemm_nt(L, P<float>(m->b_rb), R, m->Wr1T, R, sb, F, N, F, R, nullptr, false);
+    if (N > 0) CU(m, cudaMemsetAsync(vb, 0, (size_t)N * 3 * F * 4, st));
+    for (int t = T - 1; t >= 0; t--) {
+        const LayerW& l = m->lw[t];
+        float *ab = P<float>(m->b_ab), *pqb = P<float>(m->b_pqb), *gb = P<float>(m->b_gb), *snb = P<float>(m->b_snb),
+              *phib = P<float>(m->b_phib), *hb = P<float>(m->b_hb);
+        update_bwd1(L, N, F, sb, vb, P<float>(m->b_pq[t]), P<float>(m->b_a[t]), ab, pqb);
+        gemm_nt(L, ab, 3 * F, l.Wu2T, 3 * F, gb, F, N, F, 3 * F, nullptr, false);
+        mul_dsilu(L, N * F, P<float>(m->b_zpre[t]), gb);
+        gemm_nt(L, gb, F, l.Wu1T, F, snb, 2 * F, N, 2 * F, F, nullptr, false);
+        update_bwd2(L, N, F, sb, vb, snb, P<float>(m->b_sn[t]), P<float>(m->b_pq[t]), pqb, s1b, v1b);
+        gemm_nt(L, pqb, 2 * F, l.UVT, 2 * F, v1b, F, 3 * N, F, 2 * F, nullptr, true);
+        mark(m, st, ST_BWD_EDGE);
+        message_bwd(L, N, F, K, rcf, row_ptr, ej, s1b, v1b, P<float>(m->b_phi[t]), P<float>(m->b_V[t]), l.Wf, l.bf,
+                    phib, vb, P<float4>(m->b_G), t == T - 1);
+        mark(m, st, ST_BWD_NODE);
+        gemm_nt(L, phib, 3 * F, l.Wm2T, 3 * F, hb, F, N, F, 3 * F, nullptr, false);
+        mul_dsilu(L, N * F, P<float>(m->b_hpre[t]), hb);
+        gemm_nt(L, hb, F, l.Wm1T, F, s1b, F, N, F, F, nullptr, true);
+        std::swap(sb, s1b);
+    }
+
+    // ---- forces, ghost fold, virial, energy ----
+    mark(m, st, ST_FORCE);
+    if (N > 0) CU(m, cudaMemsetAsync(forces, 0, (size_t)N * 3 * 8, st));
+    force_final(L, N, n_local, row_ptr, ej, P<int>(m->b_rev), P<float4>(m->b_G), P<int>(m->b_perm), ghost_owner,
+                forces, P<double>(m->b_wpart), &n_wpart);
+    reduce_final(L, P<double>(m->b_epart), n_epart, P<double>(m->b_wpart), n_wpart, energy, virial);
+    mark(m, st, -1);
+    CU(m, cudaGetLastError());
+
+    m->N_last = N; m->n_local_last = n_local; m->E_last = E;
+    m->stats.n_atoms = N; m->stats.n_edges = E; m->stats.atom_capacity = m->cap_atoms;
+    m->stats.edge_capacity = m->cap_edges;
+    for (int d = 0; d < 3; d++) m->stats.n_cells[d] = g.n[d];
+    m->stats.n_launches = launches;
+    return MLP_OK;
+}
+
+__attribute__((visibility("default"))) int mlp_compute_host(mlp_model* m, const double* pos, const int* types, const double* box, long long n_local,
+                     long long n_ghost, const int* ghost_owner, double* energy, double* forces, double* virial) {
+    if (!m) return MLP_ERR_ARG;
+    if (n_local < 0 || n_ghost < 0 || !energy || !virial) return fail(m, MLP_ERR_ARG, "bad argument");
+    const long long N = n_local + n_ghost;
+    if (N > 0 && (!pos || !types || !forces)) return fail(m, MLP_ERR_ARG, "NULL atom array");
+    cudaStream_t st = m->own_stream;
+    ENS(m, m->d_pos, (size_t)N * 24 + 8); ENS(m, m->d_types, (size_t)N * 4 + 8);
+    ENS(m, m->d_out, (size_t)(7 + 3 * N) * 8);
+    if (ghost_owner) ENS(m, m->d_owner, (size_t)n_ghost * 4 + 8);
+    if (N > 0) {
+        CU(m, cudaMemcpyAsync(m->d_pos.p, pos, (size_t)N * 24, cudaMemcpyHostToDevice, st));
+        CU(m, cudaMemcpyAsync(m->d_types.p, types, (size_t)N * 4, cudaMemcpyHostToDevice, st));
+    }
+    if (ghost_owner && n_ghost > 0)
+        CU(m, cudaMemcpyAsync(m->d_owner.p, ghost_owner, (size_t)n_ghost * 4, cudaMemcpyHostToDevice, st));
+    double* dout = P<double>(m->d_out);
+    int r = mlp_compute(m, P<double>(m->d_pos), P<int>(m->d_types), box, n_local, n_ghost,
+                        ghost_owner ? P<int>(m->d_owner) : nullptr, dout, dout + 7, dout + 1, st);
+    if (r != MLP_OK) return r;
+    CU(m, cudaMemcpyAsync(energy, dout, 8, cudaMemcpyDeviceToHost, st));
+    CU(m, cudaMemcpyAsync(virial, dout + 1, 48, cudaMemcpyDeviceToHost, st));
+    if (N > 0) CU(m, cudaMemcpyAsync(forces, dout + 7, (size_t)N * 24, cudaMemcpyDeviceToHost, st));
+    CU(m, cudaStreamSynchronize(st));
+    return MLP_OK;
+}
+
+__attribute__((visibility("default"))) int mlp_get_neighbors(mlp_model* m, long long* n_edges, int* i, int* j, signed char* image3) {
+    if (!m || !n_edges) return MLP_ERR_ARG;
+    *n_edges = m->E_last;
+    if (!i) return MLP_OK;
+    if (!j || !image3) return fail(m, MLP_ERR_ARG, "NULL output");
+    const long long E = m->E_last, N = m->N_last;
+    if (E == 0) return MLP_OK;
+    Buf bi, bj, bm;
+    ENS(m, bi, E * 4); ENS(m, bj, E * 4); ENS(m, bm, E * 3);
+    long long launches = 0;
+    Launch L{m->own_stream, &launches};
+    CU(m, cudaDeviceSynchronize());
+    nbr_export(L, N, P<int>(m->b_row_ptr), P<float4>(m->b_ej), P<unsigned char>(m->b_img), P<int>(m->b_perm),
+               P<signed char>(m->b_wrap_s), P<int>(bi), P<int>(bj), P<signed char>(bm));
+    CU(m, cudaMemcpyAsync(i, bi.p, E * 4, cudaMemcpyDeviceToHost, m->own_stream));
+    CU(m, cudaMemcpyAsync(j, bj.p, E * 4, cudaMemcpyDeviceToHost, m->own_stream));
+    CU(m, cudaMemcpyAsync(image3, bm.p, E * 3, cudaMemcpyDeviceToHost, m->own_stream));
+    CU(m, cudaStreamSynchronize(m->own_stream));
+    free_buf(bi, m); free_buf(bj, m); free_buf(bm, m);
+    return MLP_OK;
+}
+
+__attribute__((visibility("default"))) int mlp_get_layer_state(mlp_model* m, int t, float* out) {
+    if (!m || !out || t < 0 || t > m->T) return MLP_ERR_ARG;
+    const long long N = m->N_last;
+    if (N == 0) return MLP_OK;
+    Buf b;
+    ENS(m, b, (size_t)N * 4 * m->F * 4);
+    long long launches = 0;
+    Launch L{m->own_stream, &launches};
+    CU(m, cudaDeviceSynchronize());
+    unpermute_state(L, N, m->F, P<int>(m->b_perm), P<float>(m->b_S[t]), P<float>(m->b_V[t]), P<float>(b));
+    CU(m, cudaMemcpyAsync(out, b.p, (size_t)N * 4 * m->F * 4, cudaMemcpyDeviceToHost, m->own_stream));
+    CU(m, cudaStreamSynchronize(m->own_stream));
+    free_buf(b, m);
+    return MLP_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,87 @@
+// common.cuh -- shared declarations of the PaiNN hot-path kernels (internal to the CUDA path).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define PAINN_MAX_T 8
+#define PAINN_MAX_K 32
+
+namespace painn {
+
+// Cell grid of one call (host-computed, passed by value to the neighbour kernels).
+struct Grid {
+    double origin[3];   // ghost mode: bounding-box min; periodic mode: 0
+    double box[3];      // periodic box lengths (periodic mode)
+    double inv_side[3]; // 1 / cell side
+    int n[3];           // cells per dimension
+    int periodic;       // 1: periodic (n_ghost == 0), 0: open boundaries
+    double rc2;         // cutoff^2
+};
+
+// error flags written by the device (bit mask in flags[0])
+enum { FLAG_TYPE_RANGE = 1, FLAG_NONFINITE = 2, FLAG_EDGE_OVERFLOW = 4 };
+
+struct LayerW {
+    const float *Wm1, *bm1, *Wm2, *bm2, *Wf, *bf, *UV, *Wu1, *bu1, *Wu2, *bu2;   // [out x in] row-major
+    const float *Wm1T, *Wm2T, *UVT, *Wu1T, *Wu2T;                                // transposes [in x out]
+};
+
+struct Launch {            // per-call launch context
+    cudaStream_t stream;
+    long long* counter;    // kernels launched
+};
+
+// ---- neighbour build (nbr.cu) ----
+void nbr_bin(const Launch& L, const double* pos, const int* types, long long N, int n_species, Grid g,
+             int* cell_id, signed char* wrap, int* cell_count, int* flags);
+void nbr_bbox(const Launch& L, const double* pos, long long N, double* bbox6);
+void exclusive_scan(const Launch& L, const int* in, int* out, long long n, int* block_tmp, long long* total);
+void nbr_place(const Launch& L, long long N, long long ncells, const int* cell_id, const int* cell_start,
+               int* cell_fill, int* perm);
+void nbr_sort_cells(const Launch& L, long long ncells, const int* cell_start, int* perm);
+void nbr_gather(const Launch& L, long long N, long long n_local, const int* perm, const double* pos,
+                const int* types, const signed char* wrap, double* pos_s, int* types_s, signed char* wrap_s,
+                int* inv_perm, float* local_mask, const int* cell_id, int* cell_s);
+void nbr_count(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s,
+               const int* cell_s, const int* cell_start, int* row_cnt);
+void nbr_fill(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s,
+              const int* cell_s, const int* cell_start, const int* row_ptr, long long cap_edges, float4* ej, unsigned char* img,
+              int* flags);
+void nbr_reverse(const Launch& L, long long N, const int* row_ptr, const float4* ej, const unsigned char* img,
+                 int* rev);
+void nbr_export(const Launch& L, long long N, const int* row_ptr, const float4* ej, const unsigned char* img,
+                const int* perm, const signed char* wrap_s, int* out_i, int* out_j, signed char* out_img);
+
+extern int g_gemm_emulate;   // debug knob, see gemm.cu
+// ---- dense node GEMM (gemm.cu):  C[M x N] (+)= A[M x K] . B[N x K]^T + bias ----
+void gemm_nt(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
+             int N, int K, const float* bias, bool accumulate);
+
+// ---- model kernels (painn_fwd.cu / painn_bwd.cu) ----
+void embed(const Launch& L, long long N, int F, const int* types_s, const float* Emb, float* s0, float* v0);
+void silu_fwd(const Launch& L, long long n, const float* x, float* y);
+void mul_dsilu(const Launch& L, long long n, const float* pre, float* g);   // g *= SiLU'(pre)
+void message_fwd(const Launch& L, long long N, int F, int K, float rc, const int* row_ptr, const float4* ej,
+                 const float* s, const float* v, const float* phi, const float* Wf, const float* bf, float* sn,
+                 float* v1);
+void update_mid(const Launch& L, long long N, int F, float eps, const float* pq, float* sn);
+void update_out(const Launch& L, long long N, int F, const float* sn, const float* v1, const float* pq,
+                const float* a, float* s_out, float* v_out);
+void readout(const Launch& L, long long N, int R, const float* rpre, const float* wr2, const float* br2,
+             const float* local_mask, float* rb, float* e_atom, double* e_partial, int* n_partial);
+void update_bwd1(const Launch& L, long long N, int F, const float* sb, const float* vb, const float* pq,
+                 const float* a, float* ab, float* pqb);
+void update_bwd2(const Launch& L, long long N, int F, const float* sb, const float* vb, const float* snb,
+                 const float* sn, const float* pq, float* pqb, float* s1b, float* v1b);
+void message_bwd(const Launch& L, long long N, int F, int K, float rc, const int* row_ptr, const float4* ej,
+                 const float* s1b, const float* v1b, const float* phi, const float* v_in, const float* Wf,
+                 const float* bf, float* phib, float* vb_out, float4* G, bool first);
+void force_final(const Launch& L, long long N, long long n_local, const int* row_ptr, const float4* ej,
+                 const int* rev, const float4* G, const int* perm, const int* ghost_owner, double* forces,
+                 double* w_partial, int* n_partial);
+void reduce_final(const Launch& L, const double* e_partial, int n_e, const double* w_partial, int n_w,
+                  double* energy, double* virial);
+void unpermute_state(const Launch& L, long long N, int F, const int* perm, const float* s, const float* v,
+                     float* out);
+
+}  // namespace painn

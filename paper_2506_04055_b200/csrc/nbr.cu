@@ -1,0 +1,363 @@
+// nbr.cu -- cell-list neighbour build (north_star item 1).
+//
+// Replaces the CPU (LAMMPS) neighbour list + per-step cutoff pruning of PAPER.md:58, 68 with a GPU build:
+//   bin atoms into cells of side >= rc  ->  counting sort by cell (stable: ties by caller index)  ->
+//   per-atom count over the 27-cell stencil  ->  exclusive scan  ->  fill a fixed-capacity CSR
+//   (overflow flag, regrow by the host)  ->  reverse-edge index.
+// The cutoff predicate is evaluated in fp64 with explicit round-to-nearest mul/add (no FMA contraction) on the
+// positions AS GIVEN, so the edge set is bit-identical to the definition (reading A4).
+#include "common.cuh"
+
+namespace painn {
+
+#define KLAUNCH(L) (++*(L).counter)
+
+__device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
+
+// ------------------------------------------------------------------------------------------------ a0 + a1
+__global__ void k_bin(const double* __restrict__ pos, const int* __restrict__ types, long long N, int n_species,
+                      Grid g, int* __restrict__ cell_id, signed char* __restrict__ wrap,
+                      int* __restrict__ cell_count, int* __restrict__ flags) {
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int t = types[i];
+    int bad = 0;
+    if (t < 0 || t >= n_species) bad |= FLAG_TYPE_RANGE;
+    int c[3];
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+        double x = pos[3 * i + d];
+        if (!isfinite(x)) { bad |= FLAG_NONFINITE; x = 0.0; }
+        double w = 0.0, xw;
+        if (g.periodic) {
+            w = floor(x / g.box[d]);
+            xw = x - w * g.box[d];
+            if (fabs(w) > 100.0) { bad |= FLAG_NONFINITE; w = 0.0; xw = 0.0; }
+        } else {
+            xw = x - g.origin[d];
+        }
+        wrap[3 * i + d] = (signed char)(int)w;
+        c[d] = clampi((int)floor(xw * g.inv_side[d]), 0, g.n[d] - 1);
+    }
+    int cell = (c[2] * g.n[1] + c[1]) * g.n[0] + c[0];
+    cell_id[i] = cell;
+    atomicAdd(&cell_count[cell], 1);
+    if (bad) atomicOr(flags, bad);
+}
+
+void nbr_bin(const Launch& L, const double* pos, const int* types, long long N, int n_species, Grid g,
+             int* cell_id, signed char* wrap, int* cell_count, int* flags) {
+    if (N == 0) return;
+    k_bin<<<(unsigned)((N + 255) / 256), 256, 0, L.stream>>>(pos, types, N, n_species, g, cell_id, wrap,
+                                                             cell_count, flags);
+    KLAUNCH(L);
+}
+
+// bounding box (ghost / open mode): bbox6 = {min x,y,z, max x,y,z}; initialised by the kernel's first block
+__global__ void k_bbox(const double* __restrict__ pos, long long N, double* __restrict__ part) {
+    __shared__ double smin[3][256], smax[3][256];
+    double mn[3] = {1e300, 1e300, 1e300}, mx[3] = {-1e300, -1e300, -1e300};
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x)
+        for (int d = 0; d < 3; d++) {
+            double x = pos[3 * i + d];
+            if (isfinite(x)) { mn[d] = fmin(mn[d], x); mx[d] = fmax(mx[d], x); }
+        }
+    for (int d = 0; d < 3; d++) { smin[d][threadIdx.x] = mn[d]; smax[d][threadIdx.x] = mx[d]; }
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+        if (threadIdx.x < s)
+            for (int d = 0; d < 3; d++) {
+                smin[d][threadIdx.x] = fmin(smin[d][threadIdx.x], smin[d][threadIdx.x + s]);
+                smax[d][threadIdx.x] = fmax(smax[d][threadIdx.x], smax[d][threadIdx.x + s]);
+            }
+        __syncthreads();
+    }
+    if (threadIdx.x < 3) {
+        part[6 * blockIdx.x + threadIdx.x] = smin[threadIdx.x][0];
+        part[6 * blockIdx.x + 3 + threadIdx.x] = smax[threadIdx.x][0];
+    }
+}
+__global__ void k_bbox_final(const double* __restrict__ part, int nb, double* __restrict__ bbox6) {
+    int d = threadIdx.x;
+    if (d >= 6) return;
+    double v = part[d];
+    for (int b = 1; b < nb; b++) v = d < 3 ? fmin(v, part[6 * b + d]) : fmax(v, part[6 * b + d]);
+    bbox6[d] = v;
+}
+// bbox6 must have room for 6 + 6*256 doubles (result first, partials after)
+void nbr_bbox(const Launch& L, const double* pos, long long N, double* bbox6) {
+    int nb = (int)((N + 255) / 256);
+    if (nb > 256) nb = 256;
+    if (nb < 1) nb = 1;
+    k_bbox<<<nb, 256, 0, L.stream>>>(pos, N, bbox6 + 6);
+    KLAUNCH(L);
+    k_bbox_final<<<1, 32, 0, L.stream>>>(bbox6 + 6, nb, bbox6);
+    KLAUNCH(L);
+}
+
+// ------------------------------------------------------------------------------------------------ scan
+constexpr int SCAN_T = 1024, SCAN_I = 4, SCAN_B = SCAN_T * SCAN_I;
+
+__device__ __forceinline__ int block_exclusive_scan(int v, int* total) {   // 1024 threads
+    __shared__ int wsum[32];
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int x = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+    if (lane == 31) wsum[w] = x;
+    __syncthreads();
+    if (w == 0) {
+        int s = wsum[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, s, o); if (lane >= o) s += y; }
+        wsum[lane] = s;
+    }
+    __syncthreads();
+    int base = w ? wsum[w - 1] : 0;
+    *total = wsum[31];
+    return base + x - v;
+}
+
+__global__ void __launch_bounds__(SCAN_T) k_scan_block(const int* __restrict__ in, int* __restrict__ out,
+                                                       long long n, int* __restrict__ block_tot) {
+    long long base = (long long)blockIdx.x * SCAN_B + (long long)threadIdx.x * SCAN_I;
+    int v[SCAN_I], s = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_I; k++) { v[k] = (base + k < n) ? in[base + k] : 0; s += v[k]; }
+    int tot;
+    int ex = block_exclusive_scan(s, &tot);
+#pragma unroll
+    for (int k = 0; k < SCAN_I; k++) { if (base + k < n) out[base + k] = ex; ex += v[k]; }
+    if (threadIdx.x == 0) block_tot[blockIdx.x] = tot;
+}
+__global__ void __launch_bounds__(SCAN_T) k_scan_tops(int* __restrict__ block_tot, long long nb,
+                                                      long long* __restrict__ total) {
+    __shared__ long long carry_s;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (long long b0 = 0; b0 < nb; b0 += SCAN_T) {
+        long long b = b0 + threadIdx.x;
+        int v = b < nb ? block_tot[b] : 0;
+        int tot;
+        int ex = block_exclusive_scan(v, &tot);
+        long long carry = carry_s;
+        if (b < nb) block_tot[b] = (int)(carry + ex);
+        __syncthreads();
+        if (threadIdx.x == 0) carry_s = carry + tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *total = carry_s;
+}
+__global__ void k_scan_add(int* __restrict__ out, long long n, const int* __restrict__ block_tot,
+                           const long long* __restrict__ total) {
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i < n) out[i] += block_tot[i / SCAN_B];
+    if (i == n) out[n] = (int)*total;
+}
+// out has n+1 entries; block_tmp needs ceil(n / 4096) ints; *total (device) receives the 64-bit sum
+void exclusive_scan(const Launch& L, const int* in, int* out, long long n, int* block_tmp, long long* total) {
+    long long nb = (n + SCAN_B - 1) / SCAN_B;
+    if (nb < 1) nb = 1;
+    k_scan_block<<<(unsigned)nb, SCAN_T, 0, L.stream>>>(in, out, n, block_tmp);
+    KLAUNCH(L);
+    k_scan_tops<<<1, SCAN_T, 0, L.stream>>>(block_tmp, nb, total);
+    KLAUNCH(L);
+    k_scan_add<<<(unsigned)((n + 1 + 255) / 256), 256, 0, L.stream>>>(out, n, block_tmp, total);
+    KLAUNCH(L);
+}
+
+// ------------------------------------------------------------------------------------------------ a2
+__global__ void k_place(long long N, const int* __restrict__ cell_id, const int* __restrict__ cell_start,
+                        int* __restrict__ cell_fill, int* __restrict__ perm) {
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int c = cell_id[i];
+    int slot = cell_start[c] + atomicAdd(&cell_fill[c], 1);
+    perm[slot] = (int)i;
+}
+void nbr_place(const Launch& L, long long N, long long ncells, const int* cell_id, const int* cell_start,
+               int* cell_fill, int* perm) {
+    if (N == 0) return;
+    k_place<<<(unsigned)((N + 255) / 256), 256, 0, L.stream>>>(N, cell_id, cell_start, cell_fill, perm);
+    KLAUNCH(L);
+}
+// order inside a cell = ascending caller index (makes the sort stable and the whole build deterministic)
+__global__ void k_sort_cells(long long ncells, const int* __restrict__ cell_start, int* __restrict__ perm) {
+    long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (c >= ncells) return;
+    int b = cell_start[c], e = cell_start[c + 1];
+    for (int i = b + 1; i < e; i++) {
+        int v = perm[i], k = i - 1;
+        while (k >= b && perm[k] > v) { perm[k + 1] = perm[k]; k--; }
+        perm[k + 1] = v;
+    }
+}
+void nbr_sort_cells(const Launch& L, long long ncells, const int* cell_start, int* perm) {
+    k_sort_cells<<<(unsigned)((ncells + 127) / 128), 128, 0, L.stream>>>(ncells, cell_start, perm);
+    KLAUNCH(L);
+}
+__global__ void k_gather(long long N, long long n_local, const int* __restrict__ perm,
+                         const double* __restrict__ pos, const int* __restrict__ types,
+                         const signed char* __restrict__ wrap, double* __restrict__ pos_s,
+                         int* __restrict__ types_s, signed char* __restrict__ wrap_s, int* __restrict__ inv_perm,
+                         float* __restrict__ local_mask, const int* __restrict__ cell_id, int* __restrict__ cell_s) {
+    long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (a >= N) return;
+    int i = perm[a];
+    for (int d = 0; d < 3; d++) { pos_s[3 * a + d] = pos[3 * (long long)i + d]; wrap_s[3 * a + d] = wrap[3 * (long long)i + d]; }
+    int t = types[i];
+    types_s[a] = t;
+    inv_perm[i] = (int)a;
+    cell_s[a] = cell_id[i];
+    local_mask[a] = i < n_local ? 1.0f : 0.0f;
+}
+void nbr_gather(const Launch& L, long long N, long long n_local, const int* perm, const double* pos,
+                const int* types, const signed char* wrap, double* pos_s, int* types_s, signed char* wrap_s,
+                int* inv_perm, float* local_mask, const int* cell_id, int* cell_s) {
+    if (N == 0) return;
+    k_gather<<<(unsigned)((N + 255) / 256), 256, 0, L.stream>>>(N, n_local, perm, pos, types, wrap, pos_s, types_s,
+                                                                wrap_s, inv_perm, local_mask, cell_id, cell_s);
+    KLAUNCH(L);
+}
+
+// ------------------------------------------------------------------------------------------------ a3
+// Visit every candidate (b, shift) of sorted atom a in the fixed stencil order (dz, dy, dx ascending, atoms of a
+// cell ascending) and call f(b, code, dx, dy, dz) for those passing  (dx*dx + dy*dy) + dz*dz < rc^2  (strict, fp64,
+// no contraction);  dx = (x_b + S*L) - x_a with S the image relative to the positions as given.
+template <class Fn>
+__device__ __forceinline__ void visit_neighbors(long long a, const Grid& g, const double* __restrict__ pos_s,
+                                                const signed char* __restrict__ wrap_s,
+                                                const int* __restrict__ cell_s,
+                                                const int* __restrict__ cell_start, Fn f) {
+    const double xa = pos_s[3 * a], ya = pos_s[3 * a + 1], za = pos_s[3 * a + 2];
+    const int wa0 = wrap_s[3 * a], wa1 = wrap_s[3 * a + 1], wa2 = wrap_s[3 * a + 2];
+    int c[3];
+    {
+        int cell = cell_s[a];
+        c[0] = cell % g.n[0]; cell /= g.n[0];
+        c[1] = cell % g.n[1];
+        c[2] = cell / g.n[1];
+    }
+    for (int dz = -1; dz <= 1; dz++) {
+        int cz = c[2] + dz, sz = 0;
+        if (cz < 0) { if (!g.periodic) continue; cz += g.n[2]; sz = -1; }
+        else if (cz >= g.n[2]) { if (!g.periodic) continue; cz -= g.n[2]; sz = 1; }
+        for (int dy = -1; dy <= 1; dy++) {
+            int cy = c[1] + dy, sy = 0;
+            if (cy < 0) { if (!g.periodic) continue; cy += g.n[1]; sy = -1; }
+            else if (cy >= g.n[1]) { if (!g.periodic) continue; cy -= g.n[1]; sy = 1; }
+            for (int dx = -1; dx <= 1; dx++) {
+                int cx = c[0] + dx, sx = 0;
+                if (cx < 0) { if (!g.periodic) continue; cx += g.n[0]; sx = -1; }
+                else if (cx >= g.n[0]) { if (!g.periodic) continue; cx -= g.n[0]; sx = 1; }
+                const int cell = (cz * g.n[1] + cy) * g.n[0] + cx;
+                const int code = (sx + 1) * 9 + (sy + 1) * 3 + (sz + 1);
+                const int b0 = cell_start[cell], b1 = cell_start[cell + 1];
+                for (int b = b0; b < b1; b++) {
+                    if (b == a && code == 13) continue;
+                    double Sx = 0.0, Sy = 0.0, Sz = 0.0;
+                    if (g.periodic) {
+                        Sx = (double)(sx - (int)wrap_s[3 * b] + wa0);
+                        Sy = (double)(sy - (int)wrap_s[3 * b + 1] + wa1);
+                        Sz = (double)(sz - (int)wrap_s[3 * b + 2] + wa2);
+                    }
+                    double ex = __dsub_rn(__dadd_rn(pos_s[3 * b], __dmul_rn(Sx, g.box[0])), xa);
+                    double ey = __dsub_rn(__dadd_rn(pos_s[3 * b + 1], __dmul_rn(Sy, g.box[1])), ya);
+                    double ez = __dsub_rn(__dadd_rn(pos_s[3 * b + 2], __dmul_rn(Sz, g.box[2])), za);
+                    double d2 = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
+                    if (d2 < g.rc2) f(b, code, ex, ey, ez);
+                }
+            }
+        }
+    }
+}
+
+__global__ void __launch_bounds__(128) k_count(long long N, Grid g, const double* __restrict__ pos_s,
+                                               const signed char* __restrict__ wrap_s, const int* __restrict__ cell_s,
+                                               const int* __restrict__ cell_start, int* __restrict__ row_cnt) {
+    long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (a >= N) return;
+    int cnt = 0;
+    visit_neighbors(a, g, pos_s, wrap_s, cell_s, cell_start, [&](int, int, double, double, double) { cnt++; });
+    row_cnt[a] = cnt;
+}
+void nbr_count(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s,
+               const int* cell_s, const int* cell_start, int* row_cnt) {
+    if (N == 0) return;
+    k_count<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, pos_s, wrap_s, cell_s, cell_start, row_cnt);
+    KLAUNCH(L);
+}
+
+__global__ void __launch_bounds__(128) k_fill(long long N, Grid g, const double* __restrict__ pos_s,
+                                              const signed char* __restrict__ wrap_s, const int* __restrict__ cell_s,
+                                              const int* __restrict__ cell_start, const int* __restrict__ row_ptr,
+                                              long long cap_edges, float4* __restrict__ ej,
+                                              unsigned char* __restrict__ img, int* __restrict__ flags) {
+    long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (a >= N) return;
+    long long e = row_ptr[a];
+    if ((long long)row_ptr[a + 1] > cap_edges) { atomicOr(flags, FLAG_EDGE_OVERFLOW); return; }
+    visit_neighbors(a, g, pos_s, wrap_s, cell_s, cell_start, [&](int b, int code, double ex, double ey, double ez) {
+        ej[e] = make_float4((float)ex, (float)ey, (float)ez, __int_as_float(b));
+        img[e] = (unsigned char)code;
+        e++;
+    });
+}
+void nbr_fill(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s,
+              const int* cell_s, const int* cell_start, const int* row_ptr, long long cap_edges, float4* ej, unsigned char* img,
+              int* flags) {
+    if (N == 0) return;
+    k_fill<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, pos_s, wrap_s, cell_s, cell_start, row_ptr, cap_edges,
+                                                              ej, img, flags);
+    KLAUNCH(L);
+}
+
+// reverse-edge index: for slot e = (a <- b, code) find the slot of (b <- a, 26 - code) in row b
+__global__ void k_reverse(long long N, const int* __restrict__ row_ptr, const float4* __restrict__ ej,
+                          const unsigned char* __restrict__ img, int* __restrict__ rev) {
+    // one warp per row a
+    long long a = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
+    int lane = threadIdx.x & 31;
+    if (a >= N) return;
+    for (int e = row_ptr[a] + lane; e < row_ptr[a + 1]; e += 32) {
+        int b = __float_as_int(ej[e].w);
+        int want = 26 - (int)img[e];
+        int r = -1;
+        for (int x = row_ptr[b]; x < row_ptr[b + 1]; x++)
+            if (__float_as_int(ej[x].w) == (int)a && (int)img[x] == want) { r = x; break; }
+        rev[e] = r;
+    }
+}
+void nbr_reverse(const Launch& L, long long N, const int* row_ptr, const float4* ej, const unsigned char* img,
+                 int* rev) {
+    if (N == 0) return;
+    k_reverse<<<(unsigned)((N * 32 + 255) / 256), 256, 0, L.stream>>>(N, row_ptr, ej, img, rev);
+    KLAUNCH(L);
+}
+
+// export in caller indices with images relative to the positions as given
+__global__ void k_export(long long N, const int* __restrict__ row_ptr, const float4* __restrict__ ej,
+                         const unsigned char* __restrict__ img, const int* __restrict__ perm,
+                         const signed char* __restrict__ wrap_s, int* __restrict__ out_i, int* __restrict__ out_j,
+                         signed char* __restrict__ out_img) {
+    long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (a >= N) return;
+    for (int e = row_ptr[a]; e < row_ptr[a + 1]; e++) {
+        int b = __float_as_int(ej[e].w);
+        int code = img[e];
+        int s[3] = {code / 9 - 1, (code / 3) % 3 - 1, code % 3 - 1};
+        out_i[e] = perm[a];
+        out_j[e] = perm[b];
+        for (int d = 0; d < 3; d++)
+            out_img[3 * (long long)e + d] = (signed char)(s[d] - (int)wrap_s[3 * (long long)b + d] + (int)wrap_s[3 * a + d]);
+    }
+}
+void nbr_export(const Launch& L, long long N, const int* row_ptr, const float4* ej, const unsigned char* img,
+                const int* perm, const signed char* wrap_s, int* out_i, int* out_j, signed char* out_img) {
+    if (N == 0) return;
+    k_export<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, row_ptr, ej, img, perm, wrap_s, out_i, out_j,
+                                                                out_img);
+    KLAUNCH(L);
+}
+
+}  // namespace painn

@@ -1,0 +1,240 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the fp64 oracle, element by element, on the same
+seeded inputs.  Tolerances are BASELINE.json's (reading A17):
+    |E_gpu - E_or| / n_local <= 1e-4 ;  rms(dF) / rms(F_or) <= 2e-3 ;  max|dF| <= 1e-2 rms(F_or) ;
+    ||dW||_F <= 2e-3 ||W||_F (A16) ;  neighbour sets bit-exact as sorted (i, j, image) lists.
+"""
+import numpy as np
+import pytest
+
+import gen
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+E_TOL, F_RMS_TOL, F_MAX_TOL, W_TOL = 1e-4, 2e-3, 1e-2, 2e-3
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("CUDA device required for -m gpu tests (no CPU fallback exists)")
+    return torch
+
+
+def _blob(model, **kw):
+    return gen.make_weights(model["n_species"], model["F"], model["K"], model["T"], model["rc"],
+                            seed=model["wseed"], **kw)
+
+
+def _gpu_eval(c, blob, capacity=None, edge_capacity=None, host=False, fold=True):
+    import paper_2506_04055_b200 as P
+    torch = _torch()
+    N = len(c["pos"])
+    m = P.Model(blob, c["model"]["n_species"], c["model"]["rc"], capacity or max(N, 1))
+    if edge_capacity:
+        m.set_option("edge_capacity", edge_capacity)
+    go = c.get("ghost_owner") if fold else None
+    if host:
+        e, f, w = m.compute_host(c["pos"], c["types"], c["box"], c["n_local"], c["n_ghost"], go)
+        return m, float(e[0]), f, w
+    dev = torch.device("cuda:0")
+    pos = torch.from_numpy(c["pos"]).to(dev)
+    types = torch.from_numpy(c["types"]).to(dev)
+    god = None if go is None else torch.from_numpy(np.ascontiguousarray(go, np.int32)).to(dev)
+    e, f, w = m.compute(pos, types, c["box"], c["n_local"], c["n_ghost"], god)
+    torch.cuda.synchronize()
+    return m, float(e.cpu()[0]), f.cpu().numpy(), w.cpu().numpy()
+
+
+def _oracle_eval(c, blob, fold=True):
+    return oracle.compute(blob, c["pos"], c["types"], c["box"], c["n_local"], c["n_ghost"],
+                          c.get("ghost_owner") if fold else None)
+
+
+def _check(c, e, f, w, ref, label=""):
+    nl = max(c["n_local"], 1)
+    de = abs(e - ref["energy"]) / nl
+    fr = ref["forces"]
+    rms = np.sqrt((fr ** 2).mean()) if fr.size else 0.0
+    drms = np.sqrt(((f - fr) ** 2).mean()) if fr.size else 0.0
+    dmax = np.abs(f - fr).max() if fr.size else 0.0
+    wn = np.linalg.norm(ref["virial"])
+    dw = np.linalg.norm(w - ref["virial"])
+    msg = (f"{label}: dE/atom={de:.3e} rmsF={rms:.3e} rel_rms_dF={drms / max(rms, 1e-300):.3e} "
+           f"max_dF/rms={dmax / max(rms, 1e-300):.3e} rel_dW={dw / max(wn, 1e-300):.3e}")
+    print(msg)
+    assert np.isfinite(e) and np.isfinite(f).all() and np.isfinite(w).all(), msg
+    assert de <= E_TOL, msg
+    if rms > 0:
+        assert drms <= F_RMS_TOL * rms, msg
+        assert dmax <= F_MAX_TOL * rms, msg
+    if wn > 0:
+        assert dw <= W_TOL * wn, msg
+
+
+def _same_edges(m, c, rc=5.0):
+    gi, gj, gim = m.neighbors()
+    oi, oj, oim = oracle.neighbors(c["pos"], c["box"], rc, periodic=c["n_ghost"] == 0)
+    assert len(gi) == len(oi), (len(gi), len(oi))
+    assert np.array_equal(gi, oi) and np.array_equal(gj, oj) and np.array_equal(gim, oim)
+    return len(gi)
+
+
+# reduced variants of the five BASELINE.json configs: several cells / tiles and ragged tails, oracle in seconds
+SMALL = {
+    1: {},                                                          # 192 atoms, 2 cells per dim
+    2: dict(n_mol=1000, L=31.04),                                   # 3,000 atoms, 6 cells per dim
+    3: dict(n_mol=600, L=26.2),                                     # slab + ghosts (open boundaries)
+    4: dict(ncell=4),                                               # 512 atoms diamond, 28 neighbours
+    5: dict(n_slots=1200, L=32.98),                                 # 5 species, chains + water
+}
+
+
+@pytest.fixture(scope="module", params=[1, 2, 3, 4, 5])
+def case(request):
+    k = request.param
+    c = gen.make_config(k, **SMALL[k])
+    blob = _blob(c["model"])
+    return k, c, blob
+
+
+def test_parity_small_configs(case):
+    k, c, blob = case
+    m, e, f, w = _gpu_eval(c, blob)
+    ne = _same_edges(m, c)
+    ref = _oracle_eval(c, blob)
+    assert ref["n_edges"] == ne
+    _check(c, e, f, w, ref, f"config {k} (reduced, N={len(c['pos'])}, E={ne})")
+    st = m.stats()
+    assert st["n_edges"] == ne and st["n_atoms"] == len(c["pos"]) and st["n_launches"] > 0
+
+
+def test_layer_states_config1():
+    c = gen.make_config(1)
+    blob = _blob(c["model"])
+    m, e, f, w = _gpu_eval(c, blob)
+    ref = oracle.compute(blob, c["pos"], c["types"], c["box"], want_states=True)
+    for t in range(c["model"]["T"] + 1):
+        got = m.layer_state(t, len(c["pos"]))
+        want = ref["states"][t]
+        scale = np.abs(want).max()
+        assert np.abs(got - want).max() <= 2e-4 * max(scale, 1.0), (t, np.abs(got - want).max(), scale)
+
+
+def test_host_entry_point_matches_device():
+    c = gen.make_config(1)
+    blob = _blob(c["model"])
+    _, e1, f1, w1 = _gpu_eval(c, blob)
+    _, e2, f2, w2 = _gpu_eval(c, blob, host=True)
+    assert e1 == e2 and np.array_equal(f1, f2) and np.array_equal(w1, w2)
+
+
+def test_ghost_partial_forces_without_owner_map():
+    c = gen.make_config(3, **SMALL[3])
+    blob = _blob(c["model"])
+    m, e, f, w = _gpu_eval(c, blob, fold=False)
+    ref = _oracle_eval(c, blob, fold=False)
+    _check(c, e, f, w, ref, "slab, no fold")
+    assert np.abs(f[c["n_local"]:]).max() > 0           # ghosts carry partial forces
+
+
+def test_regrow_gives_identical_result():
+    """capacity too small -> enlarge -> recompute; buffers only grow; second call does not regrow."""
+    c = gen.make_config(2, **SMALL[2])
+    blob = _blob(c["model"])
+    _, e0, f0, w0 = _gpu_eval(c, blob)
+    m, e1, f1, w1 = _gpu_eval(c, blob, capacity=100, edge_capacity=1000)
+    st = m.stats()
+    assert st["n_regrow"] >= 2 and st["atom_capacity"] >= len(c["pos"]) and st["edge_capacity"] >= st["n_edges"]
+    assert e0 == e1 and np.array_equal(f0, f1) and np.array_equal(w0, w1)
+    torch = _torch()
+    dev = torch.device("cuda:0")
+    m.compute(torch.from_numpy(c["pos"]).to(dev), torch.from_numpy(c["types"]).to(dev), c["box"])
+    torch.cuda.synchronize()
+    assert m.stats()["n_regrow"] == st["n_regrow"]
+
+
+def test_deterministic_repeat():
+    c = gen.make_config(1)
+    blob = _blob(c["model"])
+    _, e0, f0, w0 = _gpu_eval(c, blob)
+    _, e1, f1, w1 = _gpu_eval(c, blob)
+    assert e0 == e1 and np.array_equal(w0, w1)
+    assert np.abs(f0 - f1).max() <= 1e-12
+
+
+def test_unwrapped_positions_same_physics():
+    """Positions shifted by whole box vectors (reading A13): same E, F, W; images relative to positions as given."""
+    c = gen.make_config(1)
+    blob = _blob(c["model"])
+    _, e0, f0, w0 = _gpu_eval(c, blob)
+    rng = np.random.default_rng(5)
+    c2 = dict(c)
+    c2["pos"] = c["pos"] + rng.integers(-1, 2, size=c["pos"].shape) * c["box"]
+    m, e1, f1, w1 = _gpu_eval(c2, blob)
+    assert abs(e0 - e1) <= 1e-4 * len(f0)
+    assert np.abs(f0 - f1).max() <= 1e-3 * np.sqrt((f0 ** 2).mean())
+    gi, gj, gim = m.neighbors()
+    r = c2["pos"][gj] + gim * c["box"] - c2["pos"][gi]
+    assert ((r ** 2).sum(1) < 25.0).all() and len(gi) == oracle.compute(blob, c["pos"], c["types"], c["box"])["n_edges"]
+
+
+def test_edge_cases():
+    import paper_2506_04055_b200 as P
+    torch = _torch()
+    dev = torch.device("cuda:0")
+    model = dict(n_species=2, F=32, K=16, T=2, rc=5.0, wseed=3)
+    blob = _blob(model)
+    m = P.Model(blob, 2, 5.0, 16)
+    box = [30.0, 30.0, 30.0]
+    # empty system
+    e, f, w = m.compute(torch.empty((0, 3), dtype=torch.float64, device=dev), torch.empty(0, dtype=torch.int32, device=dev), box)
+    torch.cuda.synchronize()
+    assert float(e[0]) == 0.0 and f.shape == (0, 3) and float(w.abs().max()) == 0.0
+    # isolated atoms: no edges, E = sum of single-atom energies, F = 0
+    pos = np.array([[1.0, 1.0, 1.0], [15.0, 15.0, 15.0], [25.0, 8.0, 3.0]])
+    types = np.array([0, 1, 1], np.int32)
+    e, f, w = m.compute(torch.from_numpy(pos).to(dev), torch.from_numpy(types).to(dev), box)
+    torch.cuda.synchronize()
+    ref = oracle.compute(blob, pos, types, np.array(box))
+    assert ref["n_edges"] == 0 and m.stats()["n_edges"] == 0
+    assert abs(float(e[0]) - ref["energy"]) <= 1e-4 * 3 and float(f.abs().max()) == 0.0
+    # dimer
+    pos = np.array([[10.0, 10.0, 10.0], [11.3, 10.4, 9.1]])
+    types = np.array([0, 1], np.int32)
+    e, f, w = m.compute(torch.from_numpy(pos).to(dev), torch.from_numpy(types).to(dev), box)
+    torch.cuda.synchronize()
+    ref = oracle.compute(blob, pos, types, np.array(box))
+    c = dict(n_local=2)
+    _check(c, float(e[0]), f.cpu().numpy(), w.cpu().numpy(), ref, "dimer")
+
+
+def test_error_codes():
+    import paper_2506_04055_b200 as P
+    torch = _torch()
+    dev = torch.device("cuda:0")
+    c = gen.make_config(1)
+    blob = _blob(c["model"])
+    with pytest.raises(P.MLPError) as ei:
+        P.Model(blob, 3, 5.0, 10)
+    assert ei.value.code == 2
+    with pytest.raises(P.MLPError) as ei:
+        P.Model(blob[:-8], 2, 5.0, 10)
+    assert ei.value.code == 2
+    m = P.Model(blob, 2, 5.0, 192)
+    pos = torch.from_numpy(c["pos"]).to(dev)
+    types = torch.from_numpy(c["types"]).to(dev)
+    with pytest.raises(P.MLPError) as ei:
+        m.compute(pos, types, [9.9, 12.42, 12.42])
+    assert ei.value.code == 3
+    bad = types.clone(); bad[7] = 2
+    with pytest.raises(P.MLPError) as ei:
+        m.compute(pos, bad, c["box"])
+    assert ei.value.code == 4
+    badp = pos.clone(); badp[3, 1] = float("nan")
+    with pytest.raises(P.MLPError) as ei:
+        m.compute(badp, types, c["box"])
+    assert ei.value.code == 7
+    e, f, w = m.compute(pos, types, c["box"])     # model still usable after errors
+    torch.cuda.synchronize()
+    assert np.isfinite(float(e[0]))
