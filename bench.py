@@ -1,0 +1,307 @@
+#!/usr/bin/env python
+"""bench.py -- atom-steps/s of the PaiNN E + F + virial hot path (BASELINE.json metric) on synthetic workloads.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl ours|reference]
+
+One "step" = one full mlp_compute (neighbour rebuild + forward + adjoint + force/virial assembly) over the
+whole system.  N > 1 (torchrun): the path does not shard inside one evaluation (BASELINE.json: one GPU, no
+collectives), so every rank evaluates its own replica of the workload ("weak" scaling, no data-path collective);
+value = N * n_local / max-over-ranks time.  Prints ONE JSON line on rank 0.
+--impl reference times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import gen  # noqa: E402
+
+METRIC = "atom-steps/s (E+F+virial) PaiNN F=128 at 1M atoms"
+UNIT = "atom-steps/s"
+# bounded CPU-oracle sample: reduced replica of the same recipe (O(N^2) neighbour search keeps it small)
+CPU_SAMPLE = {5: dict(n_slots=2400, L=41.55), 4: dict(ncell=9), 2: dict(n_mol=2400, L=41.55), 1: {},
+              3: dict(n_mol=1500, L=35.56)}
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm=d["hbm_gbs"], bf16=d["bf16_tflops"], bf16_sus=d["bf16_tflops_sustained"],
+                    sm_max=d.get("sm_max_mhz", 1965.0), src="measured")
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sus=1400.0, sm_max=1965.0, src="fallback")
+
+
+def _workload(k, small=False):
+    over = {}
+    if small:
+        over = CPU_SAMPLE[k]
+    c = gen.make_config(k, **over)
+    m = c["model"]
+    blob = gen.make_weights(m["n_species"], m["F"], m["K"], m["T"], m["rc"], seed=m["wseed"])
+    return c, blob
+
+
+def _cached_workload(k):
+    """Full-size generation takes a minute (pure-numpy rejection sampling); cache it under /tmp per process tree."""
+    path = f"/tmp/painn_b200_cfg{k}.npz"
+    if os.path.exists(path):
+        try:
+            z = np.load(path, allow_pickle=False)
+            c = dict(pos=z["pos"], types=z["types"], box=z["box"], n_local=int(z["n_local"]), n_ghost=int(z["n_ghost"]),
+                     ghost_owner=z["ghost_owner"] if z["ghost_owner"].size else None, name=str(z["name"]),
+                     model=json.loads(str(z["model"])))
+            m = c["model"]
+            return c, gen.make_weights(m["n_species"], m["F"], m["K"], m["T"], m["rc"], seed=m["wseed"])
+        except Exception:
+            pass
+    c, blob = _workload(k)
+    try:
+        tmp = path + f".{os.getpid()}.npz"
+        np.savez(tmp, pos=c["pos"], types=c["types"], box=c["box"], n_local=c["n_local"], n_ghost=c["n_ghost"],
+                 ghost_owner=c["ghost_owner"] if c["ghost_owner"] is not None else np.empty(0, np.int32),
+                 name=c["name"], model=json.dumps(c["model"]))
+        os.replace(tmp, path)
+    except Exception:
+        pass
+    return c, blob
+
+
+def _oracle_time(k, steps, warmup):
+    import oracle
+    c, blob = _workload(k, small=True)
+    ts = []
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        oracle.compute(blob, c["pos"], c["types"], c["box"], c["n_local"], c["n_ghost"], c["ghost_owner"])
+        if it >= warmup:
+            ts.append(time.perf_counter() - t0)
+    t = float(np.mean(ts))
+    return dict(value=c["n_local"] / t, unit=UNIT, cores=oracle.threads(), kind="oracle",
+                sample=f"config {k} recipe reduced to {c['n_local']} local atoms ({len(c['pos'])} total), "
+                       f"{steps} evaluation(s) of {t:.2f} s each, O(N^2) neighbour search included"), t
+
+
+class _ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-i", str(index), "-lms", "100"], stdout=subprocess.PIPE,
+                                      stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except Exception:
+            self.p.kill()
+            out = ""
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    power_w_max=max(pw) if pw else None, samples=len(sm), reasons=sorted(reasons))
+
+
+def _stage_work(stats, model, n_atoms):
+    """Algorithmic work per step of each timed stage: (bound, units, unit-name)."""
+    F, K, T = model["F"], model["K"], model["T"]
+    E, N = stats["n_edges"], n_atoms
+    R = F // 2
+    w = {}
+    # edge stages: filter (2 * 3F * (K+1) flop) + products/segment sums; adjoint evaluates filter and its derivative
+    w["fwd_edge"] = ("alu", T * E * (2.0 * 3 * F * (K + 1) + 2.0 * 8 * F), "flop")
+    w["bwd_edge"] = ("alu", T * E * (2.0 * 2 * 3 * F * (K + 1) + 2.0 * 24 * F), "flop")
+    # node GEMMs (flop), fwd: phi-MLP F->F->3F, U|V (3 comps) F->2F, update MLP 2F->F->3F ; readout F->R
+    fwd = T * N * 2.0 * (F * F + 3 * F * F + 3 * 2 * F * F + 2 * F * F + 3 * F * F) + N * 2.0 * F * R
+    w["fwd_node"] = ("tensor", fwd, "flop")
+    w["bwd_node"] = ("tensor", fwd, "flop")          # transposed GEMMs only (weights are fixed)
+    # neighbour build: read pos (24 B) ~3x, write ej 16 B + img 1 B + rev 4 B per edge
+    w["nbr_build"] = ("hbm", N * 24.0 * 3 + E * 21.0, "B")
+    # force/virial: G read twice (own + reverse) 16 B, ej 16 B, rev 4 B per edge; forces 24 B per atom
+    w["force_virial"] = ("hbm", E * 52.0 + N * 24.0, "B")
+    return w
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config (1-5); 5 = 1M-atom headline")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    k = args.config
+
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        steps = max(1, min(args.steps, 3))
+        warm = min(args.warmup, 1)
+        cb, t = _oracle_time(k, steps, warm)
+        line = dict(impl="reference", metric=METRIC, value=cb["value"], unit=UNIT, n_gpus=args.gpus, steps=steps,
+                    warmup=warm, ms_per_step=t * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None,
+                    dtype="f64", data="synthetic",
+                    config=dict(workload=f"config {k} ({gen.CONFIGS[k]['name']}), bounded CPU sample", sample=cb["sample"]),
+                    cpu_baseline=cb, e2e=dict(value=cb["value"], unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+                    gpu_launches=0)
+        print(json.dumps(line))
+        return 0
+
+    import torch
+    import paper_2506_04055_b200 as P
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    dev = torch.device(f"cuda:{local_rank}")
+    torch.cuda.set_device(dev)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    c, blob = _cached_workload(k)
+    model = c["model"]
+    N, n_local = len(c["pos"]), c["n_local"]
+    m = P.Model(blob, model["n_species"], model["rc"], N)
+    pos = torch.from_numpy(c["pos"]).to(dev)
+    types = torch.from_numpy(c["types"]).to(dev)
+    owner = None if c["ghost_owner"] is None else torch.from_numpy(np.ascontiguousarray(c["ghost_owner"], np.int32)).to(dev)
+    out = (torch.empty(1, dtype=torch.float64, device=dev), torch.empty((N, 3), dtype=torch.float64, device=dev),
+           torch.empty(6, dtype=torch.float64, device=dev))
+    stream = torch.cuda.current_stream(dev)
+
+    def step():
+        m.compute(pos, types, c["box"], n_local, c["n_ghost"], owner, out=out, stream=stream)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize(dev)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    # ---- timed region: device-resident inputs, CUDA events on the launching stream ----
+    sampler = _ClockSampler(local_rank) if rank == 0 else None
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    clocks = sampler.stop() if sampler else None
+    stats = m.stats()
+    launches = stats["n_launches"] * args.steps
+    t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * n_local / (ms_step * 1e-3)
+
+    # ---- per-stage timing (separate pass, not part of `value`) -> roofline of the dominant kernel ----
+    m.set_option("stage_timing", 1)
+    acc = {}
+    reps = max(1, min(args.steps, 5))
+    for _ in range(reps):
+        step()
+        torch.cuda.synchronize(dev)
+        for kname, v in m.stage_ms().items():
+            acc[kname] = acc.get(kname, 0.0) + v / reps
+    m.set_option("stage_timing", 0)
+    peaks = _peaks()
+    work = _stage_work(stats, model, N)
+    dom = max(acc, key=acc.get)
+    bound, units, _ = work[dom]
+    T = model["T"]
+    n_launch = {"fwd_edge": T, "bwd_edge": T}.get(dom, 1)
+    dur_ms = acc[dom] / n_launch
+    if bound == "hbm":
+        achieved, peak, unit = units / n_launch / (dur_ms * 1e-3) / 1e9, peaks["hbm"], "GB/s"
+    elif bound == "tensor":
+        # 3xTF32 / TF32 path: tf32 peak = measured bf16 peak x nominal ratio 1.1/2.25 (B200_PROFILING.md table)
+        achieved, peak, unit = units / n_launch / (dur_ms * 1e-3) / 1e12, peaks["bf16_sus"] * (1.1 / 2.25), "TFLOP/s"
+    else:
+        # plain fp32 ALU: 148 SMs x 128 FMA lanes x 2 flop x max SM clock (B200_PROFILING.md nominal table)
+        achieved, peak, unit = units / n_launch / (dur_ms * 1e-3) / 1e12, 148 * 128 * 2 * peaks["sm_max"] * 1e6 / 1e12, "TFLOP/s"
+    roofline = dict(kernel=dom, bound=bound, achieved=achieved, peak=peak, unit=unit, frac=achieved / peak,
+                    traffic=None, peak_source=peaks["src"], launches_per_step=n_launch, ms_per_launch=dur_ms,
+                    stage_ms={kk: round(v, 4) for kk, v in acc.items()})
+
+    # ---- end to end through the host-buffer entry point (pinned host memory, copies inside the timed region) ----
+    hpos = torch.from_numpy(c["pos"]).pin_memory()
+    htypes = torch.from_numpy(c["types"]).pin_memory()
+    hown = None if c["ghost_owner"] is None else torch.from_numpy(np.ascontiguousarray(c["ghost_owner"], np.int32)).pin_memory().numpy()
+    hout = (torch.empty(1, dtype=torch.float64).pin_memory().numpy(), torch.empty((N, 3), dtype=torch.float64).pin_memory().numpy(),
+            torch.empty(6, dtype=torch.float64).pin_memory().numpy())
+    e2e_steps = max(1, min(args.steps, 5))
+    m.compute_host(hpos.numpy(), htypes.numpy(), c["box"], n_local, c["n_ghost"], hown, out=hout)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        m.compute_host(hpos.numpy(), htypes.numpy(), c["box"], n_local, c["n_ghost"], hown, out=hout)
+    torch.cuda.synchronize(dev)
+    te = (time.perf_counter() - t0) / e2e_steps
+    tt = torch.tensor([te], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    te = float(tt.item())
+    e2e = dict(value=world * n_local / te, unit=UNIT, ms_per_step=te * 1e3,
+               h2d_bytes_per_step=N * 28 + (0 if hown is None else 4 * c["n_ghost"]), d2h_bytes_per_step=N * 24 + 56)
+
+    if rank == 0:
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            cpu, _ = _oracle_time(k, 1, 0)
+        line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
+                    ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
+                    data="synthetic",
+                    config=dict(workload=f"config {k}: {c['name']}, {n_local} local + {c['n_ghost']} ghost atoms, "
+                                         f"{stats['n_edges']} directed edges, PaiNN {model['T']}x{model['F']} K={model['K']} rc={model['rc']}",
+                                l2="working set (tens of GB) far larger than the 126 MB L2; no explicit flush",
+                                multi_gpu="replicas only (one evaluation does not shard; BASELINE.json fixes 1 GPU)",
+                                precision="fp64 cutoff predicate, fp32 edge math and node state, 3xTF32/fp32 GEMMs"),
+                    clocks=clocks, e2e=e2e, gpu_launches=launches, roofline=roofline, cpu_baseline=cpu)
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

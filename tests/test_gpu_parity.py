@@ -12,6 +12,15 @@ import oracle
 pytestmark = pytest.mark.gpu
 
 E_TOL, F_RMS_TOL, F_MAX_TOL, W_TOL = 1e-4, 2e-3, 1e-2, 2e-3
+# fp32 edge geometry (north_star: "fp32 edge math") rounds every r_e component with sigma_r ~ 1.5e-7 A; the energy
+# then random-walks by F_rms * sigma_r per atom, i.e. |dE|/n_local ~ F_rms * sigma_r / sqrt(n_local).  With the
+# un-normalised random weights of the F = 128 models F_rms reaches 1e5, so on REDUCED systems this floor can exceed
+# 1e-4; at the full BASELINE sizes (n_local ~ 1e6) it is below it.  DESIGN.md section 5 derives this.
+SIGMA_R = 1.5e-7
+
+
+def _e_tol(f_rms, n_local):
+    return max(E_TOL, 3.0 * f_rms * SIGMA_R / np.sqrt(max(n_local, 1)))
 
 
 def _torch():
@@ -64,7 +73,7 @@ def _check(c, e, f, w, ref, label=""):
            f"max_dF/rms={dmax / max(rms, 1e-300):.3e} rel_dW={dw / max(wn, 1e-300):.3e}")
     print(msg)
     assert np.isfinite(e) and np.isfinite(f).all() and np.isfinite(w).all(), msg
-    assert de <= E_TOL, msg
+    assert de <= _e_tol(rms, nl), msg
     if rms > 0:
         assert drms <= F_RMS_TOL * rms, msg
         assert dmax <= F_MAX_TOL * rms, msg
