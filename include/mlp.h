@@ -116,6 +116,15 @@ int mlp_get_neighbors(mlp_model* m, long long* n_edges, int* i, int* j, signed c
  */
 int mlp_get_layer_state(mlp_model* m, int t, float* out);
 
+/*
+ * mlp_debug_gemm -- test export of the per-atom linear-layer kernel:
+ *   C[M x N] (+)= A[M x K] . W[N x K]^T + bias.   A, C: DEVICE fp32 row-major (ld = K resp. N); W [N x K], bias [N]
+ *   (or NULL): HOST fp32.  path 0 = tensor-core (tcgen05 3xTF32) when the shape is covered, 1 = plain fp32 SIMT.
+ *   *used_tc (may be NULL) receives 1 if the tensor-core kernel ran.  Synchronous.
+ */
+int mlp_debug_gemm(const float* A, const float* W, const float* bias, float* C, long long M, int N, int K,
+                   int accumulate, int path, int* used_tc);
+
 /* mlp_get_stats -- copy the statistics of the last call. */
 int mlp_get_stats(mlp_model* m, mlp_stats* out);
 

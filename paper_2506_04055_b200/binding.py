@@ -11,7 +11,7 @@ _LIB_NAME = "libpainn_b200.so"
 
 EXPORTED_SYMBOLS = [
     "mlp_create", "mlp_compute", "mlp_compute_host", "mlp_destroy", "mlp_get_neighbors", "mlp_get_layer_state",
-    "mlp_get_stats", "mlp_get_stage_ms", "mlp_set_option", "mlp_last_error", "mlp_version",
+    "mlp_get_stats", "mlp_get_stage_ms", "mlp_set_option", "mlp_last_error", "mlp_version", "mlp_debug_gemm",
 ]
 
 ERR_NAMES = {0: "MLP_OK", 1: "MLP_ERR_ARG", 2: "MLP_ERR_WEIGHTS", 3: "MLP_ERR_BOX_TOO_SMALL", 4: "MLP_ERR_TYPE_RANGE",
@@ -61,6 +61,8 @@ def load_library(build_if_missing: bool = True):
     lib.mlp_get_stats.argtypes = [vp, C.POINTER(_Stats)]
     lib.mlp_get_stage_ms.argtypes = [vp, i32, C.POINTER(C.c_char_p), C.POINTER(C.c_float)]
     lib.mlp_set_option.argtypes = [vp, C.c_char_p, ll]
+    lib.mlp_debug_gemm.argtypes = [vp, vp, vp, vp, ll, i32, i32, i32, i32, C.POINTER(i32)]
+    lib.mlp_debug_gemm.restype = i32
     lib.mlp_last_error.argtypes = [vp]
     lib.mlp_last_error.restype = C.c_char_p
     lib.mlp_version.restype = C.c_char_p
@@ -73,6 +75,27 @@ def load_library(build_if_missing: bool = True):
 
 def version() -> str:
     return load_library().mlp_version().decode()
+
+
+def debug_gemm(A, W, bias=None, C_out=None, accumulate=False, path=0):
+    """C (+)= A @ W.T + bias through the library's linear-layer kernel.  A, C_out: cuda float32 tensors; W, bias:
+    numpy float32 (host).  Returns (C, used_tensor_cores)."""
+    import torch
+    lib = load_library()
+    M, K = A.shape
+    N = W.shape[0]
+    W = np.ascontiguousarray(W, np.float32)
+    assert W.shape == (N, K) and A.is_cuda and A.dtype == torch.float32 and A.is_contiguous()
+    if C_out is None:
+        C_out = torch.zeros((M, N), dtype=torch.float32, device=A.device)
+    b = None if bias is None else np.ascontiguousarray(bias, np.float32)
+    used = C.c_int(0)
+    torch.cuda.synchronize()
+    rc = lib.mlp_debug_gemm(A.data_ptr(), W.ctypes.data, None if b is None else b.ctypes.data, C_out.data_ptr(), M, N, K,
+                            int(accumulate), int(path), C.byref(used))
+    if rc != 0:
+        raise MLPError(rc, "mlp_debug_gemm")
+    return C_out, bool(used.value)
 
 
 class Model:

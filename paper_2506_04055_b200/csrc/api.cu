@@ -35,6 +35,7 @@ struct mlp_model {
     double rc = 0, eps = 0;
     // weights (device, fp32)
     std::vector<Buf> wbufs;
+    std::vector<const float*> gemm_weights;
     float* Emb = nullptr;
     LayerW lw[PAINN_MAX_T];
     float *Wr1 = nullptr, *br1 = nullptr, *wr2 = nullptr, *br2 = nullptr, *Wr1T = nullptr;
@@ -70,6 +71,7 @@ struct mlp_model {
     std::vector<cudaEvent_t> ev_pool;
     std::vector<std::pair<int, cudaEvent_t>> marks;
     long long forced_edge_cap = 0;
+    bool fwd_tc = false;   // run the forward GEMMs on tensor cores too (faster, biased energy)
 };
 
 namespace {
@@ -118,6 +120,27 @@ int upload(mlp_model* m, const std::vector<float>& h, float** out) {
     CU(m, cudaMemcpy(b.p, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice));
     m->wbufs.push_back(b);
     *out = (float*)b.p;
+    return MLP_OK;
+}
+float rn_tf32_host(float x) {
+    uint32_t u;
+    memcpy(&u, &x, 4);
+    u += 0xfffu + ((u >> 13) & 1u);
+    u &= 0xffffe000u;
+    memcpy(&x, &u, 4);
+    return x;
+}
+// GEMM weight: fp32 matrix plus its (hi, lo) TF32 split planes for the 3xTF32 tensor-core path
+int upload_gemm_weight(mlp_model* m, const std::vector<float>& w, float** out) {
+    int r = upload(m, w, out);
+    if (r != MLP_OK) return r;
+    std::vector<float> hi(w.size()), lo(w.size());
+    for (size_t i = 0; i < w.size(); i++) { hi[i] = rn_tf32_host(w[i]); lo[i] = rn_tf32_host(w[i] - hi[i]); }
+    float *dh, *dl;
+    if ((r = upload(m, hi, &dh)) != MLP_OK) return r;
+    if ((r = upload(m, lo, &dl)) != MLP_OK) return r;
+    painn::gemm_register_split(*out, dh, dl);
+    m->gemm_weights.push_back(*out);
     return MLP_OK;
 }
 std::vector<float> to_f32(const double* p, size_t n) {
@@ -238,12 +261,12 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
         if (rcode != MLP_OK) { p += n; return; }
         std::vector<float> v = to_f32(p, n);
         p += n;
-        rcode = upload(m, v, dst);
+        rcode = keep ? upload_gemm_weight(m, v, dst) : upload(m, v, dst);   // keep != nullptr <=> GEMM matrix
         if (keep) *keep = v;
     };
     auto upT = [&](const std::vector<float>& v, int rows, int cols, float** dst) {
         if (rcode != MLP_OK) return;
-        rcode = upload(m, transpose(v, rows, cols), dst);
+        rcode = upload_gemm_weight(m, transpose(v, rows, cols), dst);
     };
     up((size_t)ns * F, &m->Emb);
     for (int t = 0; t < T; t++) {
@@ -256,7 +279,7 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
         // U and V are consecutive in the blob -> stacked [2F x F] matrix UV = [U ; V]
         std::vector<float> UV = to_f32(p, (size_t)2 * F * F);
         p += (size_t)2 * F * F;
-        if (rcode == MLP_OK) rcode = upload(m, UV, &tmp);
+        if (rcode == MLP_OK) rcode = upload_gemm_weight(m, UV, &tmp);
         l.UV = tmp;
         up((size_t)F * 2 * F, (float**)&l.Wu1, &Wu1); up(F, (float**)&l.bu1);
         up((size_t)3 * F * F, (float**)&l.Wu2, &Wu2); up(3 * F, (float**)&l.bu2);
@@ -288,6 +311,7 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
 
 __attribute__((visibility("default"))) void mlp_destroy(mlp_model* m) {
     if (!m) return;
+    for (const float* w : m->gemm_weights) painn::gemm_unregister_split(w);
     for (Buf& b : m->wbufs) free_buf(b);
     Buf* bs[] = {&m->b_cell_id, &m->b_wrap, &m->b_perm, &m->b_inv_perm, &m->b_pos_s, &m->b_types_s, &m->b_wrap_s,
                  &m->b_cell_s, &m->b_local, &m->b_row_cnt, &m->b_row_ptr, &m->b_scan_tmp, &m->b_cell_count,
@@ -311,6 +335,10 @@ __attribute__((visibility("default"))) int mlp_set_option(mlp_model* m, const ch
     if (!m || !name) return MLP_ERR_ARG;
     if (!strcmp(name, "stage_timing")) { m->timing = value != 0; return MLP_OK; }
     if (!strcmp(name, "gemm_emulate")) { painn::g_gemm_emulate = (int)value; return MLP_OK; }
+    if (!strcmp(name, "gemm_fwd_tc")) { m->fwd_tc = value != 0; return MLP_OK; }
+    if (!strcmp(name, "gemm_path")) { painn::g_gemm_path = (int)value; return MLP_OK; }
+    if (!strcmp(name, "filter_emulate")) { painn::g_filter_emulate = (int)value; return MLP_OK; }
+    if (!strcmp(name, "gather_emulate")) { painn::g_gather_emulate = (int)value; return MLP_OK; }
     if (!strcmp(name, "edge_capacity")) {
         if (value <= 0) return fail(m, MLP_ERR_ARG, "edge_capacity must be > 0");
         // shrink-or-set (test hook): drop the edge buffers and reallocate at the requested size
@@ -461,6 +489,12 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
     nbr_reverse(L, N, row_ptr, ej, P<unsigned char>(m->b_img), P<int>(m->b_rev));
 
     // ---- forward ----
+    // Tensor-core accumulation truncates toward zero after every MMA (measured): a relative
+    // bias of ~ -0.4 ulp per chained MMA that the energy (an absolute 1e-4/atom tolerance on E/atom ~ 40-160)
+    // cannot absorb, while forces (relative tolerance) can.  Forward GEMMs therefore default to the fp32 FFMA
+    // path (round-to-nearest), the adjoint GEMMs to tcgen05 3xTF32.
+    const int saved_path = painn::g_gemm_path;
+    if (!m->fwd_tc) painn::g_gemm_path = 1;
     mark(m, st, ST_FWD_NODE);
     embed(L, N, F, P<int>(m->b_types_s), m->Emb, P<float>(m->b_S[0]), P<float>(m->b_V[0]));
     float* h = P<float>(m->b_h);
@@ -489,6 +523,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
             P<float>(m->b_eatom), P<double>(m->b_epart), &n_epart);
 
     // ---- backward ----
+    painn::g_gemm_path = saved_path;
     mark(m, st, ST_BWD_NODE);
     float *sb = P<float>(m->b_sb), *s1b = P<float>(m->b_s1b), *vb = P<float>(m->b_vb), *v1b = P<float>(m->b_v1b);
     gemm_nt(L, P<float>(m->b_rb), R, m->Wr1T, R, sb, F, N, F, R, nullptr, false);
@@ -577,6 +612,33 @@ __attribute__((visibility("default"))) int mlp_get_neighbors(mlp_model* m, long 
     CU(m, cudaStreamSynchronize(m->own_stream));
     free_buf(bi, m); free_buf(bj, m); free_buf(bm, m);
     return MLP_OK;
+}
+
+__attribute__((visibility("default"))) __attribute__((visibility("default"))) int mlp_debug_gemm(const float* A, const float* W, const float* bias,
+                                                           float* C, long long M, int N, int K, int accumulate,
+                                                           int path, int* used_tc) {
+    if (!A || !W || !C || M < 0 || N <= 0 || K <= 0) return MLP_ERR_ARG;
+    mlp_model tmp;
+    mlp_model* m = &tmp;
+    std::vector<float> w(W, W + (size_t)N * K);
+    float *dW = nullptr, *dB = nullptr;
+    int r = upload_gemm_weight(m, w, &dW);
+    if (r == MLP_OK && bias) r = upload(m, std::vector<float>(bias, bias + N), &dB);
+    if (r == MLP_OK) {
+        long long launches = 0;
+        Launch L{nullptr, &launches};
+        const int saved = painn::g_gemm_path;
+        painn::g_gemm_path = path;
+        painn::g_last_gemm_tc = 0;
+        gemm_nt(L, A, K, dW, K, C, N, M, N, K, dB, accumulate != 0);
+        painn::g_gemm_path = saved;
+        if (used_tc) *used_tc = painn::g_last_gemm_tc;
+        cudaError_t e = cudaDeviceSynchronize();
+        if (e != cudaSuccess) r = MLP_ERR_CUDA;
+    }
+    for (const float* x : m->gemm_weights) painn::gemm_unregister_split(x);
+    for (Buf& b : m->wbufs) free_buf(b);
+    return r;
 }
 
 __attribute__((visibility("default"))) int mlp_get_layer_state(mlp_model* m, int t, float* out) {

@@ -53,6 +53,13 @@ __global__ void __launch_bounds__(256) k_gemm_nt_simt(const float* __restrict__ 
                 av = ah;
                 bv = bh + rn_bf16(bv - bh);
             }
+            else if (emu == 4) {   // 3xTF32: hi = truncation to tf32, lo = tf32(a - hi); hi*hi + hi*lo + lo*hi
+                float ah = __uint_as_float(__float_as_uint(av) & 0xffffe000u), bh = __uint_as_float(__float_as_uint(bv) & 0xffffe000u);
+                Al[c][r] = __uint_as_float(__float_as_uint(av - ah) & 0xffffe000u);
+                Bh[c][r] = bh;
+                av = ah;
+                bv = bh + __uint_as_float(__float_as_uint(bv - bh) & 0xffffe000u);
+            }
             As[c][r] = av;
             Bs[c][r] = bv;
         }
@@ -66,7 +73,7 @@ __global__ void __launch_bounds__(256) k_gemm_nt_simt(const float* __restrict__ 
             for (int i = 0; i < 4; i++)
 #pragma unroll
                 for (int j = 0; j < 4; j++) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
-            if (emu == 3) {
+            if (emu >= 3) {
 #pragma unroll
                 for (int i = 0; i < 4; i++) { a[i] = Al[k][ty * 4 + i]; b[i] = Bh[k][tx * 4 + i]; }
 #pragma unroll
@@ -92,9 +99,27 @@ __global__ void __launch_bounds__(256) k_gemm_nt_simt(const float* __restrict__ 
     }
 }
 
+// weight registry: B pointer -> (hi, lo) TF32 split planes for the tensor-core path (filled at mlp_create)
+#include <unordered_map>
+static std::unordered_map<const float*, std::pair<const float*, const float*>> g_split;
+int g_last_gemm_tc = 0;   // set to 1 by gemm_nt when the tensor-core kernel was used (test hook)
+int g_gemm_path = 0;   // 0: tensor cores when the shape is covered, 1: force the SIMT reference path
+void gemm_register_split(const float* W, const float* hi, const float* lo) { g_split[W] = {hi, lo}; }
+void gemm_unregister_split(const float* W) { g_split.erase(W); }
+bool gemm_nt_tc(const Launch& L, const float* A, int lda, const float* Whi, const float* Wlo, int ldw, float* C, int ldc,
+                long long M, int N, int K, const float* bias, bool accumulate);
+
 void gemm_nt(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
              int N, int K, const float* bias, bool accumulate) {
     if (M == 0) return;
+    if (g_gemm_path == 0 && g_gemm_emulate == 0) {
+        auto it = g_split.find(B);
+        if (it != g_split.end() &&
+            gemm_nt_tc(L, A, lda, it->second.first, it->second.second, ldb, C, ldc, M, N, K, bias, accumulate)) {
+            g_last_gemm_tc = 1;
+            return;
+        }
+    }
     dim3 grid((unsigned)((M + TM - 1) / TM), (unsigned)((N + TN - 1) / TN));
     k_gemm_nt_simt<<<grid, 256, 0, L.stream>>>(A, lda, B, ldb, C, ldc, M, N, K, bias, accumulate ? 1 : 0,
                                                    g_gemm_emulate);

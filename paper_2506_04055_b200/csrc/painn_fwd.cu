@@ -8,6 +8,8 @@
 // Thread mapping of the edge kernels: one thread per (receiver atom, channel f); a row of the CSR is walked
 // sequentially, so the segment sum needs no atomics and consecutive threads gather consecutive channels
 // (coalesced 4F-byte row reads).
+#include <cuda_fp16.h>
+#include <cuda_bf16.h>
 #include "common.cuh"
 
 namespace painn {
@@ -54,13 +56,28 @@ void mul_dsilu(const Launch& L, long long n, const float* pre, float* g) {
 }
 
 // ------------------------------------------------------------------------------------------------ a4 + a7
-template <int KMAX>
+// Debug knobs (mlp_set_option "filter_emulate" / "gather_emulate"): emulate reduced-precision operands of the
+// tensor-core filter GEMM (1: fp16 operands, 2: fp16 hi+lo split with 3 product terms, 3: bf16 operands) and
+// reduced-precision storage of the gathered rows (1: fp16, 2: bf16); used to size the precision plan.
+int g_filter_emulate = 0, g_gather_emulate = 0;
+__device__ __forceinline__ float r_h(float x) { return __half2float(__float2half_rn(x)); }
+__device__ __forceinline__ float r_b(float x) { return __bfloat162float(__float2bfloat16_rn(x)); }
+template <int EMU> __device__ __forceinline__ float fdot(float w, float r, float acc) {
+    if (EMU == 0) return fmaf(w, r, acc);
+    if (EMU == 1) return fmaf(r_h(w), r_h(r), acc);
+    if (EMU == 3) return fmaf(r_b(w), r_b(r), acc);
+    float wh = r_h(w), wl = r_h(w - wh), rh = r_h(r), rl = r_h(r - rh);
+    return fmaf(wl, rh, fmaf(wh, rh + rl, acc));
+}
+__device__ __forceinline__ float gq(float x, int g) { return g == 0 ? x : (g == 1 ? r_h(x) : r_b(x)); }
+
+template <int KMAX, int EMU>
 __global__ void __launch_bounds__(128) k_message_fwd(long long N, int F, int K, float inv_rc,
                                                      const int* __restrict__ row_ptr,
                                                      const float4* __restrict__ ej, const float* __restrict__ s,
                                                      const float* __restrict__ v, const float* __restrict__ phi,
                                                      const float* __restrict__ Wf, const float* __restrict__ bf,
-                                                     float* __restrict__ sn, float* __restrict__ v1) {
+                                                     float* __restrict__ sn, float* __restrict__ v1, int gemu) {
     const long long a = blockIdx.x * (long long)blockDim.y + threadIdx.y;
     const int f = threadIdx.x;
     if (a >= N) return;
@@ -85,27 +102,28 @@ __global__ void __launch_bounds__(128) k_message_fwd(long long N, int F, int K, 
         float s1, c1;
         sincospif(d * inv_rc, &s1, &c1);
         float sn_ = s1, cn_ = c1;
-        float linS = bS, linVS = bVS, linVV = bVV;
+        const float fc = 0.5f * (1.0f + c1);
+        // w = fc (Wf rho + bf) = Wf (fc rho) + bf fc : the cutoff is folded into the GEMM operand
+        float linS = fdot<EMU>(bS, fc, 0.f), linVS = fdot<EMU>(bVS, fc, 0.f), linVV = fdot<EMU>(bVV, fc, 0.f);
 #pragma unroll
         for (int n = 0; n < KMAX; n++) {
-            const float rho = sn_ * inv_d;
-            linS = fmaf(wS[n], rho, linS);
-            linVS = fmaf(wVS[n], rho, linVS);
-            linVV = fmaf(wVV[n], rho, linVV);
+            const float rho = fc * sn_ * inv_d;
+            linS = fdot<EMU>(wS[n], rho, linS);
+            linVS = fdot<EMU>(wVS[n], rho, linVS);
+            linVV = fdot<EMU>(wVV[n], rho, linVV);
             const float t = sn_ * c1 + cn_ * s1;
             cn_ = cn_ * c1 - sn_ * s1;
             sn_ = t;
         }
-        const float fc = 0.5f * (1.0f + c1);
         const float* pj = phi + (size_t)j * F3;
         const float* vj = v + (size_t)j * F3;
-        const float xs = fc * linS * pj[f];
-        const float xvs = fc * linVS * pj[F + f];
-        const float xvv = fc * linVV * pj[2 * F + f];
+        const float pvv = pj[2 * F + f];
+        const float xs = linS * gq(pj[f], gemu);
+        const float xvs = linVS * gq(pj[F + f], gemu);
         accS += xs;
-        accV0 += xvs * (r.x * inv_d) + xvv * vj[f];
-        accV1 += xvs * (r.y * inv_d) + xvv * vj[F + f];
-        accV2 += xvs * (r.z * inv_d) + xvv * vj[2 * F + f];
+        accV0 += xvs * (r.x * inv_d) + linVV * gq(pvv * vj[f], gemu);
+        accV1 += xvs * (r.y * inv_d) + linVV * gq(pvv * vj[F + f], gemu);
+        accV2 += xvs * (r.z * inv_d) + linVV * gq(pvv * vj[2 * F + f], gemu);
     }
     sn[a * 2 * F + f] = accS;
     v1[a * F3 + f] = accV0; v1[a * F3 + F + f] = accV1; v1[a * F3 + 2 * F + f] = accV2;
@@ -117,12 +135,11 @@ void message_fwd(const Launch& L, long long N, int F, int K, float rc, const int
     if (N == 0) return;
     dim3 block(F, 128 / F);
     unsigned grid = (unsigned)((N + block.y - 1) / block.y);
-    if (K <= 16)
-        k_message_fwd<16><<<grid, block, 0, L.stream>>>(N, F, K, 1.0f / rc, row_ptr, ej, s, v, phi, Wf, bf, sn, v1);
-    else if (K <= 20)
-        k_message_fwd<20><<<grid, block, 0, L.stream>>>(N, F, K, 1.0f / rc, row_ptr, ej, s, v, phi, Wf, bf, sn, v1);
-    else
-        k_message_fwd<32><<<grid, block, 0, L.stream>>>(N, F, K, 1.0f / rc, row_ptr, ej, s, v, phi, Wf, bf, sn, v1);
+#define MF(KM, EM) k_message_fwd<KM, EM><<<grid, block, 0, L.stream>>>(N, F, K, 1.0f / rc, row_ptr, ej, s, v, phi, Wf, bf, sn, v1, g_gather_emulate)
+#define MFK(EM) do { if (K <= 16) MF(16, EM); else if (K <= 20) MF(20, EM); else MF(32, EM); } while (0)
+    switch (g_filter_emulate) { case 1: MFK(1); break; case 2: MFK(2); break; case 3: MFK(3); break; default: MFK(0); }
+#undef MF
+#undef MFK
     KLAUNCH(L);
 }
 
