@@ -39,6 +39,8 @@ struct mlp_model {
     float* Emb = nullptr;
     LayerW lw[PAINN_MAX_T];
     float *Wr1 = nullptr, *br1 = nullptr, *wr2 = nullptr, *br2 = nullptr, *Wr1T = nullptr;
+    void* filt_img[PAINN_MAX_T] = {};   // tcgen05 A-operand image of (Wf | bf), fp16 hi/lo split (edge_tc.cu)
+    int edge_path = 0;                  // 0: tensor-core edge kernels when F == 128, 1: plain fp32 kernels
     // capacities
     long long cap_atoms = 0, cap_edges = 0, cap_cells = 0;
     std::vector<Buf*> all;
@@ -55,6 +57,7 @@ struct mlp_model {
         b_zpre[PAINN_MAX_T], b_a[PAINN_MAX_T];
     Buf b_h, b_rpre, b_rb, b_eatom, b_sb, b_s1b, b_vb, b_v1b, b_ab, b_pqb, b_gb, b_snb, b_phib, b_hb;
     Buf b_epart, b_wpart;
+    Buf b_Q4, b_Q1;   // gather rows of the tensor-core edge kernels
     // small
     Buf b_misc;            // device: [0..7] flags (int), then long long totals, then bbox doubles
     void* h_misc = nullptr;   // pinned mirror
@@ -172,6 +175,7 @@ int alloc_atoms(mlp_model* m, long long cap) {
     ENS(m, m->b_v1b, n * 3 * F * 4); ENS(m, m->b_ab, n * 3 * F * 4); ENS(m, m->b_pqb, n * 6 * F * 4);
     ENS(m, m->b_gb, n * F * 4); ENS(m, m->b_snb, n * 2 * F * 4); ENS(m, m->b_phib, n * 3 * F * 4);
     ENS(m, m->b_hb, n * F * 4);
+    if (m->F == 128) { ENS(m, m->b_Q4, n * F * 16); ENS(m, m->b_Q1, n * F * 4); }
     ENS(m, m->b_epart, (n / 256 + 2) * 8); ENS(m, m->b_wpart, (n / 8 + 2) * 9 * 8);
     m->cap_atoms = cap;
     return MLP_OK;
@@ -275,6 +279,18 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
         float* tmp;
         up((size_t)F * F, (float**)&l.Wm1, &Wm1); up(F, (float**)&l.bm1);
         up((size_t)3 * F * F, (float**)&l.Wm2, &Wm2); up(3 * F, (float**)&l.bm2);
+        {
+            std::vector<float> Wf_h = to_f32(p, (size_t)3 * F * K), bf_h = to_f32(p + (size_t)3 * F * K, (size_t)3 * F);
+            if (F == 128 && K <= 23 && rcode == MLP_OK) {
+                std::vector<unsigned short> img;
+                edge_build_filter_image(Wf_h.data(), bf_h.data(), K, img);
+                Buf b;
+                rcode = ensure(m, b, img.size() * 2);
+                if (rcode == MLP_OK && cudaMemcpy(b.p, img.data(), img.size() * 2, cudaMemcpyHostToDevice) != cudaSuccess) rcode = MLP_ERR_CUDA;
+                m->wbufs.push_back(b);
+                m->filt_img[t] = b.p;
+            }
+        }
         up((size_t)3 * F * K, (float**)&l.Wf); up(3 * F, (float**)&l.bf);
         // U and V are consecutive in the blob -> stacked [2F x F] matrix UV = [U ; V]
         std::vector<float> UV = to_f32(p, (size_t)2 * F * F);
@@ -317,7 +333,7 @@ __attribute__((visibility("default"))) void mlp_destroy(mlp_model* m) {
                  &m->b_cell_s, &m->b_local, &m->b_row_cnt, &m->b_row_ptr, &m->b_scan_tmp, &m->b_cell_count,
                  &m->b_cell_start, &m->b_cell_fill, &m->b_ej, &m->b_img, &m->b_rev, &m->b_G, &m->b_h, &m->b_rpre,
                  &m->b_rb, &m->b_eatom, &m->b_sb, &m->b_s1b, &m->b_vb, &m->b_v1b, &m->b_ab, &m->b_pqb, &m->b_gb,
-                 &m->b_snb, &m->b_phib, &m->b_hb, &m->b_epart, &m->b_wpart, &m->b_misc, &m->d_pos, &m->d_types,
+                 &m->b_snb, &m->b_phib, &m->b_hb, &m->b_Q4, &m->b_Q1, &m->b_epart, &m->b_wpart, &m->b_misc, &m->d_pos, &m->d_types,
                  &m->d_owner, &m->d_out};
     for (Buf* b : bs) free_buf(*b);
     for (int t = 0; t <= PAINN_MAX_T; t++) { free_buf(m->b_S[t]); free_buf(m->b_V[t]); }
@@ -335,6 +351,7 @@ __attribute__((visibility("default"))) int mlp_set_option(mlp_model* m, const ch
     if (!m || !name) return MLP_ERR_ARG;
     if (!strcmp(name, "stage_timing")) { m->timing = value != 0; return MLP_OK; }
     if (!strcmp(name, "gemm_emulate")) { painn::g_gemm_emulate = (int)value; return MLP_OK; }
+    if (!strcmp(name, "edge_path")) { m->edge_path = (int)value; return MLP_OK; }
     if (!strcmp(name, "gemm_fwd_tc")) { m->fwd_tc = value != 0; return MLP_OK; }
     if (!strcmp(name, "gemm_path")) { painn::g_gemm_path = (int)value; return MLP_OK; }
     if (!strcmp(name, "filter_emulate")) { painn::g_filter_emulate = (int)value; return MLP_OK; }
@@ -508,7 +525,13 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         silu_fwd(L, N * F, hpre, h);
         gemm_nt(L, h, F, l.Wm2, F, phi, 3 * F, N, 3 * F, F, l.bm2, false);
         mark(m, st, ST_FWD_EDGE);
-        message_fwd(L, N, F, K, rcf, row_ptr, ej, S, V, phi, l.Wf, l.bf, sn, v1);
+        bool done = false;
+        if (m->edge_path == 0 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
+            make_gather_rows(L, N, phi, V, P<float>(m->b_Q4), P<float>(m->b_Q1), t > 0);
+            done = message_fwd_tc(L, N, K, rcf, row_ptr, ej, S, V, P<float>(m->b_Q4), P<float>(m->b_Q1), m->filt_img[t], sn,
+                                  v1, t > 0);
+        }
+        if (!done) message_fwd(L, N, F, K, rcf, row_ptr, ej, S, V, phi, l.Wf, l.bf, sn, v1);
         mark(m, st, ST_FWD_NODE);
         gemm_nt(L, v1, F, l.UV, F, pq, 2 * F, 3 * N, 2 * F, F, nullptr, false);
         update_mid(L, N, F, (float)m->eps, pq, sn);

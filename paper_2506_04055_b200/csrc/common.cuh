@@ -3,6 +3,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <vector>
+
 #define PAINN_MAX_T 8
 #define PAINN_MAX_K 32
 
@@ -86,5 +88,12 @@ void reduce_final(const Launch& L, const double* e_partial, int n_e, const doubl
                   double* energy, double* virial);
 void unpermute_state(const Launch& L, long long N, int F, const int* perm, const float* s, const float* v,
                      float* out);
+
+// ---- tensor-core edge kernels (edge_tc.cu), F = 128 ----
+void edge_build_filter_image(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img);
+size_t edge_filter_image_bytes();
+void make_gather_rows(const Launch& L, long long N, const float* phi, const float* v, float* Q4, float* Q1, bool has_v);
+bool message_fwd_tc(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* s,
+                    const float* v, const float* Q4, const float* Q1, const void* A_img, float* sn, float* v1, bool has_v);
 
 }  // namespace painn

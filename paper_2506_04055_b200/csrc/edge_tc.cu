@@ -1,0 +1,355 @@
+// edge_tc.cu -- message pass with the per-edge filter on tensor cores (F = 128 models).
+//
+//   w_e = fc(d_e) (Wf rho(d_e) + bf)  is a [3F x (K+1)] . [(K+1) x edges] GEMM: per 32-edge tile one warp group
+//   computes R_e = fc (1, rho_1..rho_K) on the fly (sincospi + rotation recurrence), writes it as the B operand into
+//   shared memory, one thread issues tcgen05.mma (A = Wf|bf resident in shared memory, M = 128 channels per chunk,
+//   N = 32 edges), and the accumulator D[channel, edge] lands in TMEM with ONE CHANNEL PER LANE.  The four consumer
+//   warps then read their own channel's filter values (tcgen05.ld 32x32b) and run the segment sum over the sorted
+//   CSR rows with plain FMAs: no atomics, no shuffles, coalesced 512 B gathers of the sender rows.
+//
+// Precision: fp16 operands alone miss the force tolerance (measured), so both operands are
+// split x = hi + lo (two fp16 numbers, ~22 bits) and three product terms are accumulated:
+//   hi(W) hi(R)  +  [hi(W) 2^-11][lo(R) 2^11]  +  [lo(W) 2^11][hi(R) 2^-11]           (K dimension 3 x 32 = 96)
+// The two small terms are issued first so the fp32 accumulator (which truncates toward zero after every MMA) sees
+// only two full-magnitude additions.
+#include <cuda_fp16.h>
+
+#include <algorithm>
+#include <cstring>
+#include <vector>
+
+#include "common.cuh"
+#include "tc_common.cuh"
+
+namespace painn {
+
+#define KLAUNCH(L) (++*(L).counter)
+
+namespace etc {
+
+constexpr int F = 128;
+constexpr int NE = 32;                        // edges per tile (MMA N)
+constexpr int KP = 96;                        // 3 terms x 32 basis slots
+constexpr int LBO = 128, SBO = (KP / 8) * 128;          // 1536
+constexpr int A_CHUNK_BYTES = (F / 8) * SBO;            // 24576
+constexpr int B_BYTES = (NE / 8) * SBO;                 // 6144
+constexpr int NTHREADS = 256;
+
+// host: A operand image of one layer (3 chunks), see header comment; W[f][0] = bf, W[f][b] = Wf[f][b-1]
+void build_filter_image(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img) {
+    img.assign(3 * A_CHUNK_BYTES / 2, 0);
+    for (int c = 0; c < 3; c++)
+        for (int r = 0; r < F; r++)
+            for (int b = 0; b <= K; b++) {
+                const float w = b == 0 ? bf[c * F + r] : Wf[(size_t)(c * F + r) * K + (b - 1)];
+                const __half hi = __float2half_rn(w);
+                const float hif = __half2float(hi);
+                const __half t1 = __float2half_rn(hif * (1.0f / 2048.0f));
+                const __half t2 = __float2half_rn((w - hif) * 2048.0f);
+                const __half vals[3] = {hi, t1, t2};
+                for (int t = 0; t < 3; t++) {
+                    const int k = t * 32 + b;
+                    const size_t off = (size_t)c * A_CHUNK_BYTES + (r / 8) * SBO + (k / 8) * LBO + (r % 8) * 16 + (k % 8) * 2;
+                    unsigned short bits;
+                    memcpy(&bits, &vals[t], 2);
+                    img[off / 2] = bits;
+                }
+            }
+}
+
+// gather rows: Q4[j][f] = (phi^s, phi^vs, phi^vv v_x, phi^vv v_y), Q1[j][f] = phi^vv v_z ; layer 0 (v = 0): Q2 = (phi^s, phi^vs)
+__global__ void k_make_gather(long long N, const float* __restrict__ phi, const float* __restrict__ v,
+                              float4* __restrict__ Q4, float* __restrict__ Q1, float2* __restrict__ Q2, int has_v) {
+    long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (idx >= N * F) return;
+    const long long j = idx / F;
+    const int f = (int)(idx - j * F);
+    const float ps = phi[j * 3 * F + f], pvs = phi[j * 3 * F + F + f];
+    if (has_v) {
+        const float pvv = phi[j * 3 * F + 2 * F + f];
+        Q4[idx] = make_float4(ps, pvs, pvv * v[j * 3 * F + f], pvv * v[j * 3 * F + F + f]);
+        Q1[idx] = pvv * v[j * 3 * F + 2 * F + f];
+    } else {
+        Q2[idx] = make_float2(ps, pvs);
+    }
+}
+
+struct FwdParams {
+    long long N;
+    const int* row_ptr;
+    const float4* ej;
+    const float* s;
+    const float* v;
+    const float4* Q4;
+    const float* Q1;
+    const float2* Q2;
+    const uint4* A_img;
+    float* sn;     // s' written with row stride 2F
+    float* v1;
+    float inv_rc;
+    int K;
+    int atoms_per_unit;
+};
+
+template <bool HAS_V>
+__global__ void __launch_bounds__(NTHREADS, 2) k_message_fwd_tc(FwdParams p) {
+    constexpr int NCH = HAS_V ? 3 : 2;
+    constexpr int TCOLS = NCH * NE;                 // TMEM columns per buffer
+    constexpr int TALLOC = HAS_V ? 256 : 128;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+    uint8_t* sA = smem;
+    uint8_t* sB = sA + NCH * A_CHUNK_BYTES;
+    float4* sMeta = (float4*)(sB + 2 * B_BYTES);
+    uint64_t* bars = (uint64_t*)(sMeta + 2 * NE);
+    uint64_t* b_full = bars;          // [2] producer -> MMA      (count 96)
+    uint64_t* t_full = bars + 2;      // [2] MMA commit -> consumers (count 1)
+    uint64_t* t_empty = bars + 4;     // [2] consumers -> producer   (count 4)
+    uint32_t* tmem_slot = (uint32_t*)(bars + 6);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    using namespace tc;
+
+    // ---- one-time setup: filter operand into smem, zero B (padding slots stay zero), barriers, TMEM ----
+    {
+        const uint4* src = p.A_img;
+        uint4* dst = (uint4*)sA;
+        for (int i = tid; i < NCH * A_CHUNK_BYTES / 16; i += NTHREADS) dst[i] = src[i];
+        uint4* zb = (uint4*)sB;
+        for (int i = tid; i < 2 * B_BYTES / 16; i += NTHREADS) zb[i] = make_uint4(0, 0, 0, 0);
+    }
+    if (tid == 0) {
+        for (int b = 0; b < 2; b++) { mbar_init(&b_full[b], 96); mbar_init(&t_full[b], 1); mbar_init(&t_empty[b], 4); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 7) tmem_alloc(tmem_slot, TALLOC);
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    const long long n_units = (p.N + p.atoms_per_unit - 1) / p.atoms_per_unit;
+
+    if (warp < 4) {
+        // ===================== consumers: one channel per thread =====================
+        const int f = tid;
+        const uint32_t lane_base = tmem_base + ((uint32_t)(warp * 32) << 16);
+        uint32_t it = 0;
+        for (long long u = blockIdx.x; u < n_units; u += gridDim.x) {
+            const long long a0 = u * p.atoms_per_unit;
+            const long long a1 = min(p.N, a0 + (long long)p.atoms_per_unit);
+            const int e_begin = p.row_ptr[a0], e_end = p.row_ptr[a1];
+            const int ntiles = (e_end - e_begin + NE - 1) / NE;
+            long long a_cur = a0;
+            int row_end = p.row_ptr[a0 + 1];
+            float accS = p.s[a_cur * F + f];
+            float acc0 = p.v[a_cur * 3 * F + f], acc1 = p.v[a_cur * 3 * F + F + f], acc2 = p.v[a_cur * 3 * F + 2 * F + f];
+            for (int t = 0; t < ntiles; t++, it++) {
+                const int buf = it & 1;
+                mbar_wait(&t_full[buf], (it >> 1) & 1);
+                tc_fence_after();
+                const float4* meta = sMeta + buf * NE;
+#pragma unroll 1
+                for (int g = 0; g < NE / 16; g++) {
+                    uint32_t ws[16], wvs[16], wvv[16];
+                    tmem_ld16_nowait(lane_base + buf * TCOLS + g * 16, ws);
+                    tmem_ld16_nowait(lane_base + buf * TCOLS + NE + g * 16, wvs);
+                    if (HAS_V) tmem_ld16_nowait(lane_base + buf * TCOLS + 2 * NE + g * 16, wvv);
+                    tmem_wait_ld();
+#pragma unroll
+                    for (int h = 0; h < 2; h++) {
+                        float4 m[8], q4[8];
+                        float q1[8];
+                        float2 q2[8];
+#pragma unroll
+                        for (int i = 0; i < 8; i++) {
+                            m[i] = meta[g * 16 + h * 8 + i];
+                            const size_t row = (size_t)__float_as_int(m[i].w) * F + f;
+                            if (HAS_V) { q4[i] = __ldg(p.Q4 + row); q1[i] = __ldg(p.Q1 + row); }
+                            else q2[i] = __ldg(p.Q2 + row);
+                        }
+#pragma unroll
+                        for (int i = 0; i < 8; i++) {
+                            const int E = e_begin + t * NE + g * 16 + h * 8 + i;
+                            if (E < e_end) {
+                                while (E >= row_end) {   // uniform: finish receiver a_cur, start the next row
+                                    p.sn[a_cur * 2 * F + f] = accS;
+                                    p.v1[a_cur * 3 * F + f] = acc0; p.v1[a_cur * 3 * F + F + f] = acc1; p.v1[a_cur * 3 * F + 2 * F + f] = acc2;
+                                    a_cur++;
+                                    row_end = p.row_ptr[a_cur + 1];
+                                    accS = p.s[a_cur * F + f];
+                                    acc0 = p.v[a_cur * 3 * F + f]; acc1 = p.v[a_cur * 3 * F + F + f]; acc2 = p.v[a_cur * 3 * F + 2 * F + f];
+                                }
+                                const int k = h * 8 + i;
+                                const float w_s = __uint_as_float(ws[k]), w_vs = __uint_as_float(wvs[k]);
+                                if (HAS_V) {
+                                    const float w_vv = __uint_as_float(wvv[k]);
+                                    accS = fmaf(w_s, q4[i].x, accS);
+                                    const float tv = w_vs * q4[i].y;
+                                    acc0 = fmaf(tv, m[i].x, fmaf(w_vv, q4[i].z, acc0));
+                                    acc1 = fmaf(tv, m[i].y, fmaf(w_vv, q4[i].w, acc1));
+                                    acc2 = fmaf(tv, m[i].z, fmaf(w_vv, q1[i], acc2));
+                                } else {
+                                    accS = fmaf(w_s, q2[i].x, accS);
+                                    const float tv = w_vs * q2[i].y;
+                                    acc0 = fmaf(tv, m[i].x, acc0);
+                                    acc1 = fmaf(tv, m[i].y, acc1);
+                                    acc2 = fmaf(tv, m[i].z, acc2);
+                                }
+                            }
+                        }
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&t_empty[buf]);
+            }
+            // finish the last receiver with edges, then pass trailing edge-less atoms through (s' = s, v' = v)
+            for (;;) {
+                p.sn[a_cur * 2 * F + f] = accS;
+                p.v1[a_cur * 3 * F + f] = acc0; p.v1[a_cur * 3 * F + F + f] = acc1; p.v1[a_cur * 3 * F + 2 * F + f] = acc2;
+                if (++a_cur >= a1) break;
+                accS = p.s[a_cur * F + f];
+                acc0 = p.v[a_cur * 3 * F + f]; acc1 = p.v[a_cur * 3 * F + F + f]; acc2 = p.v[a_cur * 3 * F + 2 * F + f];
+            }
+        }
+    } else if (warp < 7) {
+        // ===================== producers: B operand R_e = fc (1, rho_1 .. rho_K) split into fp16 hi / lo =====================
+        const int pt = tid - 128, e = pt & 31, h = pt >> 5;   // h: basis slots 8h .. 8h+7 (slot 0 = bias, slot n = rho_n)
+        uint32_t it = 0;
+        for (long long u = blockIdx.x; u < n_units; u += gridDim.x) {
+            const long long a0 = u * p.atoms_per_unit;
+            const long long a1 = min(p.N, a0 + (long long)p.atoms_per_unit);
+            const int e_begin = p.row_ptr[a0], e_end = p.row_ptr[a1];
+            const int ntiles = (e_end - e_begin + NE - 1) / NE;
+            for (int t = 0; t < ntiles; t++, it++) {
+                const int buf = it & 1;
+                const int E = e_begin + t * NE + e;
+                float4 r = make_float4(1.f, 0.f, 0.f, __int_as_float(0));
+                const bool valid = E < e_end;
+                if (valid) r = __ldg(p.ej + E);
+                const float d2 = r.x * r.x + r.y * r.y + r.z * r.z;
+                const float inv_d = rsqrtf(d2);
+                const float x = d2 * inv_d * p.inv_rc;
+                float s1, c1;
+                sincospif(x, &s1, &c1);
+                const float fc = valid ? 0.5f * (1.0f + c1) : 0.0f;
+                const float amp = fc * inv_d;
+                float sn_, cn_;
+                const int n0 = h == 0 ? 1 : 8 * h;
+                if (h == 0) { sn_ = s1; cn_ = c1; } else sincospif((float)n0 * x, &sn_, &cn_);
+                __half2 hi2[4], t1[4], t2[4];
+                float vals[8];
+#pragma unroll
+                for (int i = 0; i < 8; i++) {
+                    const int b = h * 8 + i;
+                    float R;
+                    if (b == 0) R = fc;
+                    else {
+                        R = b <= p.K ? amp * sn_ : 0.0f;
+                        const float tt = sn_ * c1 + cn_ * s1;
+                        cn_ = cn_ * c1 - sn_ * s1;
+                        sn_ = tt;
+                    }
+                    vals[i] = R;
+                }
+#pragma unroll
+                for (int i = 0; i < 4; i++) {
+                    const __half h0 = __float2half_rn(vals[2 * i]), h1 = __float2half_rn(vals[2 * i + 1]);
+                    const float f0 = __half2float(h0), f1 = __half2float(h1);
+                    hi2[i] = __halves2half2(h0, h1);
+                    t1[i] = __halves2half2(__float2half_rn((vals[2 * i] - f0) * 2048.0f), __float2half_rn((vals[2 * i + 1] - f1) * 2048.0f));
+                    t2[i] = __halves2half2(__float2half_rn(f0 * (1.0f / 2048.0f)), __float2half_rn(f1 * (1.0f / 2048.0f)));
+                }
+                mbar_wait(&t_empty[buf], ((it >> 1) & 1) ^ 1);
+                uint8_t* bb = sB + buf * B_BYTES + (e >> 3) * SBO + (e & 7) * 16 + h * LBO;
+                *(uint4*)(bb) = *(uint4*)hi2;                       // term 0: k = b
+                *(uint4*)(bb + 4 * LBO) = *(uint4*)t1;              // term 1: k = 32 + b   (lo(R) 2^11)
+                *(uint4*)(bb + 8 * LBO) = *(uint4*)t2;              // term 2: k = 64 + b   (hi(R) 2^-11)
+                if (h == 0) sMeta[buf * NE + e] = make_float4(r.x * inv_d, r.y * inv_d, r.z * inv_d, r.w);
+                fence_async_smem();
+                mbar_arrive(&b_full[buf]);
+            }
+        }
+    } else {
+        // ===================== MMA issuer =====================
+        if (lane == 0) {
+            const uint32_t idesc = (1u << 4) | ((uint32_t)(NE >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);   // f16 x f16 -> f32
+            const uint32_t a_base = smem_u32(sA), b_base = smem_u32(sB);
+            uint32_t it = 0;
+            for (long long u = blockIdx.x; u < n_units; u += gridDim.x) {
+                const long long a0 = u * p.atoms_per_unit;
+                const long long a1 = min(p.N, a0 + (long long)p.atoms_per_unit);
+                const int e_begin = p.row_ptr[a0], e_end = p.row_ptr[a1];
+                const int ntiles = (e_end - e_begin + NE - 1) / NE;
+                for (int t = 0; t < ntiles; t++, it++) {
+                    const int buf = it & 1;
+                    mbar_wait(&b_full[buf], (it >> 1) & 1);
+                    tc_fence_after();
+#pragma unroll
+                    for (int c = 0; c < NCH; c++) {
+                        const uint32_t d = tmem_base + buf * TCOLS + c * NE;
+#pragma unroll
+                        for (int o = 0; o < 6; o++) {
+                            const int kk = (o + 2) % 6;          // small terms (k-steps 2..5) first, main term last
+                            const uint64_t ad = make_desc_nosw(a_base + c * A_CHUNK_BYTES + kk * 2 * LBO, LBO, SBO);
+                            const uint64_t bd = make_desc_nosw(b_base + buf * B_BYTES + kk * 2 * LBO, LBO, SBO);
+                            umma_f16(d, ad, bd, idesc, o != 0);
+                        }
+                    }
+                    umma_commit(&t_full[buf]);
+                }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 7) tmem_dealloc(tmem_base, TALLOC);
+}
+
+constexpr int fwd_smem_bytes(bool has_v) { return (has_v ? 3 : 2) * A_CHUNK_BYTES + 2 * B_BYTES + 2 * NE * 16 + 64 + 128; }
+
+}  // namespace etc
+
+void edge_build_filter_image(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img) {
+    etc::build_filter_image(Wf, bf, K, img);
+}
+size_t edge_filter_image_bytes() { return 3 * etc::A_CHUNK_BYTES; }
+
+void make_gather_rows(const Launch& L, long long N, const float* phi, const float* v, float* Q4, float* Q1, bool has_v) {
+    if (N == 0) return;
+    etc::k_make_gather<<<(unsigned)((N * etc::F + 255) / 256), 256, 0, L.stream>>>(N, phi, v, (float4*)Q4, Q1, (float2*)Q4,
+                                                                                  has_v ? 1 : 0);
+    KLAUNCH(L);
+}
+
+// F = 128, K <= 23 only.  Q4/Q1 from make_gather_rows (layer 0: Q4 holds float2 rows).
+bool message_fwd_tc(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* s,
+                    const float* v, const float* Q4, const float* Q1, const void* A_img, float* sn, float* v1, bool has_v) {
+    using namespace etc;
+    if (N == 0) return true;
+    if (K > 23) return false;
+    static int n_sm = 0;
+    static bool attr = false;
+    if (!n_sm) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    }
+    if (!attr) {
+        if (cudaFuncSetAttribute(k_message_fwd_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fwd_smem_bytes(true)) != cudaSuccess ||
+            cudaFuncSetAttribute(k_message_fwd_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fwd_smem_bytes(false)) != cudaSuccess)
+            return false;
+        attr = true;
+    }
+    FwdParams p{N, row_ptr, ej, s, v, (const float4*)Q4, Q1, (const float2*)Q4, (const uint4*)A_img, sn, v1, 1.0f / rc, K, 16};
+    const long long n_units = (N + p.atoms_per_unit - 1) / p.atoms_per_unit;
+    const int grid = (int)std::min<long long>(n_units, 2LL * n_sm);
+    if (has_v) k_message_fwd_tc<true><<<grid, NTHREADS, fwd_smem_bytes(true), L.stream>>>(p);
+    else k_message_fwd_tc<false><<<grid, NTHREADS, fwd_smem_bytes(false), L.stream>>>(p);
+    KLAUNCH(L);
+    return true;
+}
+
+}  // namespace painn
