@@ -562,8 +562,15 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         update_bwd2(L, N, F, sb, vb, snb, P<float>(m->b_sn[t]), P<float>(m->b_pq[t]), pqb, s1b, v1b);
         gemm_nt(L, pqb, 2 * F, l.UVT, 2 * F, v1b, F, 3 * N, F, 2 * F, nullptr, true);
         mark(m, st, ST_BWD_EDGE);
-        message_bwd(L, N, F, K, rcf, row_ptr, ej, s1b, v1b, P<float>(m->b_phi[t]), P<float>(m->b_V[t]), l.Wf, l.bf,
-                    phib, vb, P<float4>(m->b_G), t == T - 1);
+        bool done = false;
+        if (m->edge_path == 0 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
+            make_gather_rows_bwd(L, N, s1b, v1b, P<float>(m->b_Q4));
+            done = message_bwd_tc(L, N, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<float>(m->b_phi[t]), P<float>(m->b_V[t]),
+                                  v1b, m->filt_img[t], phib, vb, P<float4>(m->b_G), t == T - 1);
+        }
+        if (!done)
+            message_bwd(L, N, F, K, rcf, row_ptr, ej, s1b, v1b, P<float>(m->b_phi[t]), P<float>(m->b_V[t]), l.Wf, l.bf,
+                        phib, vb, P<float4>(m->b_G), t == T - 1);
         mark(m, st, ST_BWD_NODE);
         gemm_nt(L, phib, 3 * F, l.Wm2T, 3 * F, hb, F, N, F, 3 * F, nullptr, false);
         mul_dsilu(L, N * F, P<float>(m->b_hpre[t]), hb);

@@ -95,5 +95,9 @@ size_t edge_filter_image_bytes();
 void make_gather_rows(const Launch& L, long long N, const float* phi, const float* v, float* Q4, float* Q1, bool has_v);
 bool message_fwd_tc(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* s,
                     const float* v, const float* Q4, const float* Q1, const void* A_img, float* sn, float* v1, bool has_v);
+void make_gather_rows_bwd(const Launch& L, long long N, const float* s1b, const float* v1b, float* Gb);
+bool message_bwd_tc(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
+                    const float* phi, const float* v_in, const float* v1b, const void* A_img, float* phib, float* vb_out,
+                    float4* G, bool first);
 
 }  // namespace painn

@@ -310,6 +310,304 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_message_fwd_tc(FwdParams p) {
 
 constexpr int fwd_smem_bytes(bool has_v) { return (has_v ? 3 : 2) * A_CHUNK_BYTES + 2 * B_BYTES + 2 * NE * 16 + 64 + 128; }
 
+// ================================================================================================ adjoint (a12)
+// One thread per channel again, walking the SENDER's own row (no-atomics gather form, painn_bwd.cu header).
+// Per 16-edge tile the producers emit R_e (rows 0..15 of the B operand) and R'_e = d/dd [fc (1, rho)] (rows 16..31),
+// so one N = 32 MMA per chunk yields both the filter w (columns 0..15) and its derivative w' (columns 16..31).
+// The four per-edge scalars (db, ub_x, ub_y, ub_z) are reduced over the 128 channels with a butterfly
+// transpose-reduce (31 shuffles per 8 edges per warp) + one shared-memory hop across the four warps.
+constexpr int NEB = 16;
+
+// gather rows of the adjoint pass: Gb[i][f] = (sb', vb'_x, vb'_y, vb'_z)
+__global__ void k_make_gather_bwd(long long N, const float* __restrict__ s1b, const float* __restrict__ v1b,
+                                  float4* __restrict__ Gb) {
+    long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (idx >= N * F) return;
+    const long long j = idx / F;
+    const int f = (int)(idx - j * F);
+    Gb[idx] = make_float4(s1b[idx], v1b[j * 3 * F + f], v1b[j * 3 * F + F + f], v1b[j * 3 * F + 2 * F + f]);
+}
+
+struct BwdParams {
+    long long N;
+    const int* row_ptr;
+    const float4* ej;
+    const float4* Gb;
+    const float* phi;
+    const float* v_in;
+    const float* v1b;
+    const uint4* A_img;
+    float* phib;
+    float* vb_out;
+    float4* G;
+    float inv_rc;
+    int K;
+    int atoms_per_unit;
+    int first;
+};
+
+__global__ void __launch_bounds__(NTHREADS, 2) k_message_bwd_tc(BwdParams p) {
+    constexpr int NCH = 3;
+    constexpr int TCOLS = NCH * 2 * NEB;            // 96 TMEM columns per buffer
+    constexpr int TALLOC = 256;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+    uint8_t* sA = smem;
+    uint8_t* sB = sA + NCH * A_CHUNK_BYTES;                  // 2 buffers x (32 rows x 96 halfs) = 2 x 6144
+    float4* sMeta = (float4*)(sB + 2 * B_BYTES);            // [2][16] (u_e, i)
+    float* sInvd = (float*)(sMeta + 2 * NEB);               // [2][16]
+    float* sRed = sInvd + 2 * NEB;                          // [2][4][32]
+    uint64_t* bars = (uint64_t*)(sRed + 2 * 4 * 32);
+    uint64_t* b_full = bars;          // [2] (count 48)
+    uint64_t* t_full = bars + 2;      // [2] (count 1)
+    uint64_t* t_empty = bars + 4;     // [2] (count 4)
+    uint32_t* tmem_slot = (uint32_t*)(bars + 6);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    using namespace tc;
+    {
+        const uint4* src = p.A_img;
+        uint4* dst = (uint4*)sA;
+        for (int i = tid; i < NCH * A_CHUNK_BYTES / 16; i += NTHREADS) dst[i] = src[i];
+        uint4* zb = (uint4*)sB;
+        for (int i = tid; i < 2 * B_BYTES / 16; i += NTHREADS) zb[i] = make_uint4(0, 0, 0, 0);
+    }
+    if (tid == 0) {
+        for (int b = 0; b < 2; b++) { mbar_init(&b_full[b], 48); mbar_init(&t_full[b], 1); mbar_init(&t_empty[b], 4); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 7) tmem_alloc(tmem_slot, TALLOC);
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+    const long long n_units = (p.N + p.atoms_per_unit - 1) / p.atoms_per_unit;
+
+    if (warp < 4) {
+        // ===================== consumers =====================
+        const int f = tid;
+        const uint32_t lane_base = tmem_base + ((uint32_t)(warp * 32) << 16);
+        uint32_t it = 0, hc = 0;    // tile counter, 8-edge half counter (selects the reduction buffer)
+        for (long long u = blockIdx.x; u < n_units; u += gridDim.x) {
+            const long long a0 = u * p.atoms_per_unit;
+            const long long a1 = min(p.N, a0 + (long long)p.atoms_per_unit);
+            const int e_begin = p.row_ptr[a0], e_end = p.row_ptr[a1];
+            const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
+            long long j = a0;
+            int row_end = p.row_ptr[a0 + 1];
+            float phS = p.phi[j * 3 * F + f], phVS = p.phi[j * 3 * F + F + f], phVV = p.phi[j * 3 * F + 2 * F + f];
+            float vj0 = p.v_in[j * 3 * F + f], vj1 = p.v_in[j * 3 * F + F + f], vj2 = p.v_in[j * 3 * F + 2 * F + f];
+            float pbS = 0.f, pbVS = 0.f, Y0 = 0.f, Y1 = 0.f, Y2 = 0.f;
+            auto finish_row = [&]() {
+                p.phib[j * 3 * F + f] = pbS;
+                p.phib[j * 3 * F + F + f] = pbVS;
+                p.phib[j * 3 * F + 2 * F + f] = vj0 * Y0 + vj1 * Y1 + vj2 * Y2;
+                p.vb_out[j * 3 * F + f] = p.v1b[j * 3 * F + f] + phVV * Y0;
+                p.vb_out[j * 3 * F + F + f] = p.v1b[j * 3 * F + F + f] + phVV * Y1;
+                p.vb_out[j * 3 * F + 2 * F + f] = p.v1b[j * 3 * F + 2 * F + f] + phVV * Y2;
+            };
+            auto start_row = [&]() {
+                row_end = p.row_ptr[j + 1];
+                phS = p.phi[j * 3 * F + f]; phVS = p.phi[j * 3 * F + F + f]; phVV = p.phi[j * 3 * F + 2 * F + f];
+                vj0 = p.v_in[j * 3 * F + f]; vj1 = p.v_in[j * 3 * F + F + f]; vj2 = p.v_in[j * 3 * F + 2 * F + f];
+                pbS = pbVS = Y0 = Y1 = Y2 = 0.f;
+            };
+            for (int t = 0; t < ntiles; t++, it++) {
+                const int buf = it & 1;
+                mbar_wait(&t_full[buf], (it >> 1) & 1);
+                tc_fence_after();
+                const float4* meta = sMeta + buf * NEB;
+#pragma unroll 1
+                for (int h = 0; h < 2; h++, hc++) {
+                    uint32_t w[3][8], dw[3][8];
+#pragma unroll
+                    for (int c = 0; c < 3; c++) {
+                        tmem_ld8_nowait(lane_base + buf * TCOLS + c * 2 * NEB + h * 8, w[c]);
+                        tmem_ld8_nowait(lane_base + buf * TCOLS + c * 2 * NEB + NEB + h * 8, dw[c]);
+                    }
+                    float4 m[8], gb[8];
+#pragma unroll
+                    for (int i = 0; i < 8; i++) {
+                        m[i] = meta[h * 8 + i];
+                        gb[i] = __ldg(p.Gb + (size_t)__float_as_int(m[i].w) * F + f);
+                    }
+                    tmem_wait_ld();
+                    float part[32];
+#pragma unroll
+                    for (int i = 0; i < 8; i++) {
+                        const int E = e_begin + t * NEB + h * 8 + i;
+                        float db = 0.f, ub0 = 0.f, ub1 = 0.f, ub2 = 0.f;
+                        if (E < e_end) {
+                            while (E >= row_end) { finish_row(); j++; start_row(); }
+                            const float wS = __uint_as_float(w[0][i]), wVS = __uint_as_float(w[1][i]), wVV = __uint_as_float(w[2][i]);
+                            const float dS = __uint_as_float(dw[0][i]), dVS = __uint_as_float(dw[1][i]), dVV = __uint_as_float(dw[2][i]);
+                            const float sb = gb[i].x, vb0 = gb[i].y, vb1 = gb[i].z, vb2 = gb[i].w;
+                            const float X = vb0 * m[i].x + vb1 * m[i].y + vb2 * m[i].z;
+                            const float Z = vb0 * vj0 + vb1 * vj1 + vb2 * vj2;
+                            pbS = fmaf(wS, sb, pbS);
+                            pbVS = fmaf(wVS, X, pbVS);
+                            Y0 = fmaf(wVV, vb0, Y0); Y1 = fmaf(wVV, vb1, Y1); Y2 = fmaf(wVV, vb2, Y2);
+                            db = phS * sb * dS + phVS * X * dVS + phVV * Z * dVV;
+                            const float tt = wVS * phVS;
+                            ub0 = tt * vb0; ub1 = tt * vb1; ub2 = tt * vb2;
+                        }
+                        part[4 * i] = db; part[4 * i + 1] = ub0; part[4 * i + 2] = ub1; part[4 * i + 3] = ub2;
+                    }
+                    // butterfly transpose-reduce: lane l ends with the warp total of part[l]
+#pragma unroll
+                    for (int o = 16, n = 16; o >= 1; o >>= 1, n >>= 1) {
+                        const bool up = (lane & o) != 0;
+#pragma unroll
+                        for (int k = 0; k < 16; k++) {
+                            if (k < n) {
+                                const float keep = up ? part[k + n] : part[k];
+                                const float send = up ? part[k] : part[k + n];
+                                part[k] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+                            }
+                        }
+                    }
+                    float* red = sRed + (hc & 1) * 128;
+                    red[warp * 32 + lane] = part[0];
+                    asm volatile("bar.sync 1, 128;" ::: "memory");
+                    if (tid < 8) {
+                        const int E = e_begin + t * NEB + h * 8 + tid;
+                        if (E < e_end) {
+                            float db = 0.f, ub0 = 0.f, ub1 = 0.f, ub2 = 0.f;
+#pragma unroll
+                            for (int wq = 0; wq < 4; wq++) {
+                                db += red[wq * 32 + 4 * tid]; ub0 += red[wq * 32 + 4 * tid + 1];
+                                ub1 += red[wq * 32 + 4 * tid + 2]; ub2 += red[wq * 32 + 4 * tid + 3];
+                            }
+                            const float4 mm = meta[h * 8 + tid];
+                            const float inv_d = sInvd[buf * NEB + h * 8 + tid];
+                            const float uu = ub0 * mm.x + ub1 * mm.y + ub2 * mm.z;
+                            float4 g = make_float4(db * mm.x + (ub0 - uu * mm.x) * inv_d, db * mm.y + (ub1 - uu * mm.y) * inv_d,
+                                                   db * mm.z + (ub2 - uu * mm.z) * inv_d, 0.f);
+                            if (!p.first) { const float4 o = p.G[E]; g.x += o.x; g.y += o.y; g.z += o.z; }
+                            p.G[E] = g;
+                        }
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&t_empty[buf]);
+            }
+            for (;;) {
+                finish_row();
+                if (++j >= a1) break;
+                start_row();
+            }
+        }
+    } else if (warp < 6) {
+        // ===================== producers: rows 0..15 R_e, rows 16..31 R'_e =====================
+        const int pt = tid - 128, e = pt & 15, h = pt >> 4;   // h = 0..3 (h == 3 idle)
+        uint32_t it = 0;
+        const float a1c = 3.14159265358979323846f * p.inv_rc;
+        for (long long u = blockIdx.x; u < n_units; u += gridDim.x) {
+            const long long a0 = u * p.atoms_per_unit;
+            const long long a1 = min(p.N, a0 + (long long)p.atoms_per_unit);
+            const int e_begin = p.row_ptr[a0], e_end = p.row_ptr[a1];
+            const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
+            for (int t = 0; t < ntiles; t++, it++) {
+                if (h == 3) continue;
+                const int buf = it & 1;
+                const int E = e_begin + t * NEB + e;
+                float4 r = make_float4(1.f, 0.f, 0.f, __int_as_float(0));
+                const bool valid = E < e_end;
+                if (valid) r = __ldg(p.ej + E);
+                const float d2 = r.x * r.x + r.y * r.y + r.z * r.z;
+                const float inv_d = rsqrtf(d2);
+                const float x = d2 * inv_d * p.inv_rc;
+                float s1, c1;
+                sincospif(x, &s1, &c1);
+                const float fc = valid ? 0.5f * (1.0f + c1) : 0.0f;
+                const float dfc = valid ? -0.5f * a1c * s1 : 0.0f;
+                float sn_, cn_;
+                const int n0 = h == 0 ? 1 : 8 * h;
+                if (h == 0) { sn_ = s1; cn_ = c1; } else sincospif((float)n0 * x, &sn_, &cn_);
+                float vals[8], dvals[8];
+#pragma unroll
+                for (int i = 0; i < 8; i++) {
+                    const int b = h * 8 + i;
+                    if (b == 0) { vals[i] = fc; dvals[i] = dfc; }
+                    else {
+                        const float rho = sn_ * inv_d;
+                        const float drho = ((float)b * a1c * cn_ - rho) * inv_d;
+                        vals[i] = b <= p.K ? fc * rho : 0.0f;
+                        dvals[i] = b <= p.K ? dfc * rho + fc * drho : 0.0f;
+                        const float tt = sn_ * c1 + cn_ * s1;
+                        cn_ = cn_ * c1 - sn_ * s1;
+                        sn_ = tt;
+                    }
+                }
+                __half2 q[6][4];
+#pragma unroll
+                for (int i = 0; i < 4; i++) {
+#pragma unroll
+                    for (int z = 0; z < 2; z++) {
+                        const float v0 = z ? dvals[2 * i] : vals[2 * i], v1 = z ? dvals[2 * i + 1] : vals[2 * i + 1];
+                        const __half h0 = __float2half_rn(v0), h1 = __float2half_rn(v1);
+                        const float f0 = __half2float(h0), f1 = __half2float(h1);
+                        q[3 * z + 0][i] = __halves2half2(h0, h1);
+                        q[3 * z + 1][i] = __halves2half2(__float2half_rn((v0 - f0) * 2048.0f), __float2half_rn((v1 - f1) * 2048.0f));
+                        q[3 * z + 2][i] = __halves2half2(__float2half_rn(f0 * (1.0f / 2048.0f)), __float2half_rn(f1 * (1.0f / 2048.0f)));
+                    }
+                }
+                mbar_wait(&t_empty[buf], ((it >> 1) & 1) ^ 1);
+#pragma unroll
+                for (int z = 0; z < 2; z++) {
+                    const int row = z * NEB + e;
+                    uint8_t* bb = sB + buf * B_BYTES + (row >> 3) * SBO + (row & 7) * 16 + h * LBO;
+                    *(uint4*)(bb) = *(uint4*)q[3 * z + 0];
+                    *(uint4*)(bb + 4 * LBO) = *(uint4*)q[3 * z + 1];
+                    *(uint4*)(bb + 8 * LBO) = *(uint4*)q[3 * z + 2];
+                }
+                if (h == 0) {
+                    sMeta[buf * NEB + e] = make_float4(-r.x * inv_d, -r.y * inv_d, -r.z * inv_d, r.w);   // u_e of edge (i <- j)
+                    sInvd[buf * NEB + e] = inv_d;
+                }
+                fence_async_smem();
+                mbar_arrive(&b_full[buf]);
+            }
+        }
+    } else if (warp == 7) {
+        if (lane == 0) {
+            const uint32_t idesc = (1u << 4) | ((uint32_t)((2 * NEB) >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+            const uint32_t a_base = smem_u32(sA), b_base = smem_u32(sB);
+            uint32_t it = 0;
+            for (long long u = blockIdx.x; u < n_units; u += gridDim.x) {
+                const long long a0 = u * p.atoms_per_unit;
+                const long long a1 = min(p.N, a0 + (long long)p.atoms_per_unit);
+                const int e_begin = p.row_ptr[a0], e_end = p.row_ptr[a1];
+                const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
+                for (int t = 0; t < ntiles; t++, it++) {
+                    const int buf = it & 1;
+                    mbar_wait(&b_full[buf], (it >> 1) & 1);
+                    tc_fence_after();
+#pragma unroll
+                    for (int c = 0; c < NCH; c++) {
+                        const uint32_t d = tmem_base + buf * TCOLS + c * 2 * NEB;
+#pragma unroll
+                        for (int o = 0; o < 6; o++) {
+                            const int kk = (o + 2) % 6;
+                            const uint64_t ad = make_desc_nosw(a_base + c * A_CHUNK_BYTES + kk * 2 * LBO, LBO, SBO);
+                            const uint64_t bd = make_desc_nosw(b_base + buf * B_BYTES + kk * 2 * LBO, LBO, SBO);
+                            umma_f16(d, ad, bd, idesc, o != 0);
+                        }
+                    }
+                    umma_commit(&t_full[buf]);
+                }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 7) tmem_dealloc(tmem_base, TALLOC);
+}
+
+constexpr int bwd_smem_bytes() { return 3 * A_CHUNK_BYTES + 2 * B_BYTES + 2 * NEB * 16 + 2 * NEB * 4 + 2 * 4 * 32 * 4 + 64 + 128; }
+
 }  // namespace etc
 
 void edge_build_filter_image(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img) {
@@ -348,6 +646,39 @@ bool message_fwd_tc(const Launch& L, long long N, int K, float rc, const int* ro
     const int grid = (int)std::min<long long>(n_units, 2LL * n_sm);
     if (has_v) k_message_fwd_tc<true><<<grid, NTHREADS, fwd_smem_bytes(true), L.stream>>>(p);
     else k_message_fwd_tc<false><<<grid, NTHREADS, fwd_smem_bytes(false), L.stream>>>(p);
+    KLAUNCH(L);
+    return true;
+}
+
+void make_gather_rows_bwd(const Launch& L, long long N, const float* s1b, const float* v1b, float* Gb) {
+    if (N == 0) return;
+    etc::k_make_gather_bwd<<<(unsigned)((N * etc::F + 255) / 256), 256, 0, L.stream>>>(N, s1b, v1b, (float4*)Gb);
+    KLAUNCH(L);
+}
+
+bool message_bwd_tc(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
+                    const float* phi, const float* v_in, const float* v1b, const void* A_img, float* phib, float* vb_out,
+                    float4* G, bool first) {
+    using namespace etc;
+    if (N == 0) return true;
+    if (K > 23) return false;
+    static int n_sm = 0;
+    static bool attr = false;
+    if (!n_sm) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    }
+    if (!attr) {
+        if (cudaFuncSetAttribute(k_message_bwd_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, bwd_smem_bytes()) != cudaSuccess)
+            return false;
+        attr = true;
+    }
+    BwdParams p{N, row_ptr, ej, (const float4*)Gb, phi, v_in, v1b, (const uint4*)A_img, phib, vb_out, G, 1.0f / rc, K, 16,
+                first ? 1 : 0};
+    const long long n_units = (N + p.atoms_per_unit - 1) / p.atoms_per_unit;
+    const int grid = (int)std::min<long long>(n_units, 2LL * n_sm);
+    k_message_bwd_tc<<<grid, NTHREADS, bwd_smem_bytes(), L.stream>>>(p);
     KLAUNCH(L);
     return true;
 }
