@@ -130,6 +130,8 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_message_fwd_tc(FwdParams p) {
     const uint32_t tmem_base = *tmem_slot;
 
     const long long n_units = (p.N + p.atoms_per_unit - 1) / p.atoms_per_unit;
+    // register re-partition per warpgroup: consumers (warps 0-3) 168, producer / MMA warps (4-7) 88  (2 CTAs per SM)
+    if (warp < 4) reg_inc<168>(); else reg_dec<88>();
 
     if (warp < 4) {
         // ===================== consumers: one channel per thread =====================
@@ -152,51 +154,48 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_message_fwd_tc(FwdParams p) {
                 const float4* meta = sMeta + buf * NE;
 #pragma unroll 1
                 for (int g = 0; g < NE / 16; g++) {
+                    // 16 sender rows in flight per thread before the first use (the pass is bound by gather latency)
+                    float4 q4[16];
+                    float q1[16];
+                    float2 q2[16];
+#pragma unroll
+                    for (int i = 0; i < 16; i++) {
+                        const size_t row = (size_t)__float_as_int(meta[g * 16 + i].w) * F + f;
+                        if (HAS_V) { q4[i] = __ldg(p.Q4 + row); q1[i] = __ldg(p.Q1 + row); }
+                        else q2[i] = __ldg(p.Q2 + row);
+                    }
                     uint32_t ws[16], wvs[16], wvv[16];
                     tmem_ld16_nowait(lane_base + buf * TCOLS + g * 16, ws);
                     tmem_ld16_nowait(lane_base + buf * TCOLS + NE + g * 16, wvs);
                     if (HAS_V) tmem_ld16_nowait(lane_base + buf * TCOLS + 2 * NE + g * 16, wvv);
                     tmem_wait_ld();
 #pragma unroll
-                    for (int h = 0; h < 2; h++) {
-                        float4 m[8], q4[8];
-                        float q1[8];
-                        float2 q2[8];
-#pragma unroll
-                        for (int i = 0; i < 8; i++) {
-                            m[i] = meta[g * 16 + h * 8 + i];
-                            const size_t row = (size_t)__float_as_int(m[i].w) * F + f;
-                            if (HAS_V) { q4[i] = __ldg(p.Q4 + row); q1[i] = __ldg(p.Q1 + row); }
-                            else q2[i] = __ldg(p.Q2 + row);
-                        }
-#pragma unroll
-                        for (int i = 0; i < 8; i++) {
-                            const int E = e_begin + t * NE + g * 16 + h * 8 + i;
-                            if (E < e_end) {
-                                while (E >= row_end) {   // uniform: finish receiver a_cur, start the next row
-                                    p.sn[a_cur * 2 * F + f] = accS;
-                                    p.v1[a_cur * 3 * F + f] = acc0; p.v1[a_cur * 3 * F + F + f] = acc1; p.v1[a_cur * 3 * F + 2 * F + f] = acc2;
-                                    a_cur++;
-                                    row_end = p.row_ptr[a_cur + 1];
-                                    accS = p.s[a_cur * F + f];
-                                    acc0 = p.v[a_cur * 3 * F + f]; acc1 = p.v[a_cur * 3 * F + F + f]; acc2 = p.v[a_cur * 3 * F + 2 * F + f];
-                                }
-                                const int k = h * 8 + i;
-                                const float w_s = __uint_as_float(ws[k]), w_vs = __uint_as_float(wvs[k]);
-                                if (HAS_V) {
-                                    const float w_vv = __uint_as_float(wvv[k]);
-                                    accS = fmaf(w_s, q4[i].x, accS);
-                                    const float tv = w_vs * q4[i].y;
-                                    acc0 = fmaf(tv, m[i].x, fmaf(w_vv, q4[i].z, acc0));
-                                    acc1 = fmaf(tv, m[i].y, fmaf(w_vv, q4[i].w, acc1));
-                                    acc2 = fmaf(tv, m[i].z, fmaf(w_vv, q1[i], acc2));
-                                } else {
-                                    accS = fmaf(w_s, q2[i].x, accS);
-                                    const float tv = w_vs * q2[i].y;
-                                    acc0 = fmaf(tv, m[i].x, acc0);
-                                    acc1 = fmaf(tv, m[i].y, acc1);
-                                    acc2 = fmaf(tv, m[i].z, acc2);
-                                }
+                    for (int i = 0; i < 16; i++) {
+                        const int E = e_begin + t * NE + g * 16 + i;
+                        if (E < e_end) {
+                            while (E >= row_end) {   // uniform: finish receiver a_cur, start the next row
+                                p.sn[a_cur * 2 * F + f] = accS;
+                                p.v1[a_cur * 3 * F + f] = acc0; p.v1[a_cur * 3 * F + F + f] = acc1; p.v1[a_cur * 3 * F + 2 * F + f] = acc2;
+                                a_cur++;
+                                row_end = p.row_ptr[a_cur + 1];
+                                accS = p.s[a_cur * F + f];
+                                acc0 = p.v[a_cur * 3 * F + f]; acc1 = p.v[a_cur * 3 * F + F + f]; acc2 = p.v[a_cur * 3 * F + 2 * F + f];
+                            }
+                            const float4 m = meta[g * 16 + i];
+                            const float w_s = __uint_as_float(ws[i]), w_vs = __uint_as_float(wvs[i]);
+                            if (HAS_V) {
+                                const float w_vv = __uint_as_float(wvv[i]);
+                                accS = fmaf(w_s, q4[i].x, accS);
+                                const float tv = w_vs * q4[i].y;
+                                acc0 = fmaf(tv, m.x, fmaf(w_vv, q4[i].z, acc0));
+                                acc1 = fmaf(tv, m.y, fmaf(w_vv, q4[i].w, acc1));
+                                acc2 = fmaf(tv, m.z, fmaf(w_vv, q1[i], acc2));
+                            } else {
+                                accS = fmaf(w_s, q2[i].x, accS);
+                                const float tv = w_vs * q2[i].y;
+                                acc0 = fmaf(tv, m.x, acc0);
+                                acc1 = fmaf(tv, m.y, acc1);
+                                acc2 = fmaf(tv, m.z, acc2);
                             }
                         }
                     }
@@ -262,7 +261,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_message_fwd_tc(FwdParams p) {
                     t1[i] = __halves2half2(__float2half_rn((vals[2 * i] - f0) * 2048.0f), __float2half_rn((vals[2 * i + 1] - f1) * 2048.0f));
                     t2[i] = __halves2half2(__float2half_rn(f0 * (1.0f / 2048.0f)), __float2half_rn(f1 * (1.0f / 2048.0f)));
                 }
-                mbar_wait(&t_empty[buf], ((it >> 1) & 1) ^ 1);
+                mbar_wait_relaxed(&t_empty[buf], ((it >> 1) & 1) ^ 1);
                 uint8_t* bb = sB + buf * B_BYTES + (e >> 3) * SBO + (e & 7) * 16 + h * LBO;
                 *(uint4*)(bb) = *(uint4*)hi2;                       // term 0: k = b
                 *(uint4*)(bb + 4 * LBO) = *(uint4*)t1;              // term 1: k = 32 + b   (lo(R) 2^11)
@@ -285,7 +284,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_message_fwd_tc(FwdParams p) {
                 const int ntiles = (e_end - e_begin + NE - 1) / NE;
                 for (int t = 0; t < ntiles; t++, it++) {
                     const int buf = it & 1;
-                    mbar_wait(&b_full[buf], (it >> 1) & 1);
+                    mbar_wait_relaxed(&b_full[buf], (it >> 1) & 1);
                     tc_fence_after();
 #pragma unroll
                     for (int c = 0; c < NCH; c++) {
@@ -360,8 +359,10 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_message_bwd_tc(BwdParams p) {
     uint64_t* bars = (uint64_t*)(sRed + 2 * 4 * 32);
     uint64_t* b_full = bars;          // [2] (count 48)
     uint64_t* t_full = bars + 2;      // [2] (count 1)
-    uint64_t* t_empty = bars + 4;     // [2] (count 4)
-    uint32_t* tmem_slot = (uint32_t*)(bars + 6);
+    uint64_t* t_empty = bars + 4;     // [2] consumers (4) + finisher (1) -> producer
+    uint64_t* r_full = bars + 6;      // [2] per-edge partial sums written (count 4)
+    uint64_t* r_empty = bars + 8;     // [2] finisher done with the reduction buffer (count 1)
+    uint32_t* tmem_slot = (uint32_t*)(bars + 10);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     using namespace tc;
@@ -373,7 +374,10 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_message_bwd_tc(BwdParams p) {
         for (int i = tid; i < 2 * B_BYTES / 16; i += NTHREADS) zb[i] = make_uint4(0, 0, 0, 0);
     }
     if (tid == 0) {
-        for (int b = 0; b < 2; b++) { mbar_init(&b_full[b], 48); mbar_init(&t_full[b], 1); mbar_init(&t_empty[b], 4); }
+        for (int b = 0; b < 2; b++) {
+            mbar_init(&b_full[b], 48); mbar_init(&t_full[b], 1); mbar_init(&t_empty[b], 5);
+            mbar_init(&r_full[b], 4); mbar_init(&r_empty[b], 1);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 7) tmem_alloc(tmem_slot, TALLOC);
@@ -383,6 +387,8 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_message_bwd_tc(BwdParams p) {
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
     const long long n_units = (p.N + p.atoms_per_unit - 1) / p.atoms_per_unit;
+    // register re-partition per warpgroup: consumers (warps 0-3) 168, producer / MMA warps (4-7) 88  (2 CTAs per SM)
+    if (warp < 4) reg_inc<168>(); else reg_dec<88>();
 
     if (warp < 4) {
         // ===================== consumers =====================
@@ -467,27 +473,12 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_message_bwd_tc(BwdParams p) {
                             }
                         }
                     }
+                    // hand the 32 warp totals to the finisher warp (cross-warp sum, g_e, G update) without a CTA barrier
                     float* red = sRed + (hc & 1) * 128;
+                    mbar_wait(&r_empty[hc & 1], ((hc >> 1) & 1) ^ 1);
                     red[warp * 32 + lane] = part[0];
-                    asm volatile("bar.sync 1, 128;" ::: "memory");
-                    if (tid < 8) {
-                        const int E = e_begin + t * NEB + h * 8 + tid;
-                        if (E < e_end) {
-                            float db = 0.f, ub0 = 0.f, ub1 = 0.f, ub2 = 0.f;
-#pragma unroll
-                            for (int wq = 0; wq < 4; wq++) {
-                                db += red[wq * 32 + 4 * tid]; ub0 += red[wq * 32 + 4 * tid + 1];
-                                ub1 += red[wq * 32 + 4 * tid + 2]; ub2 += red[wq * 32 + 4 * tid + 3];
-                            }
-                            const float4 mm = meta[h * 8 + tid];
-                            const float inv_d = sInvd[buf * NEB + h * 8 + tid];
-                            const float uu = ub0 * mm.x + ub1 * mm.y + ub2 * mm.z;
-                            float4 g = make_float4(db * mm.x + (ub0 - uu * mm.x) * inv_d, db * mm.y + (ub1 - uu * mm.y) * inv_d,
-                                                   db * mm.z + (ub2 - uu * mm.z) * inv_d, 0.f);
-                            if (!p.first) { const float4 o = p.G[E]; g.x += o.x; g.y += o.y; g.z += o.z; }
-                            p.G[E] = g;
-                        }
-                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&r_full[hc & 1]);
                 }
                 tc_fence_before();
                 __syncwarp();
@@ -554,7 +545,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_message_bwd_tc(BwdParams p) {
                         q[3 * z + 2][i] = __halves2half2(__float2half_rn(f0 * (1.0f / 2048.0f)), __float2half_rn(f1 * (1.0f / 2048.0f)));
                     }
                 }
-                mbar_wait(&t_empty[buf], ((it >> 1) & 1) ^ 1);
+                mbar_wait_relaxed(&t_empty[buf], ((it >> 1) & 1) ^ 1);
 #pragma unroll
                 for (int z = 0; z < 2; z++) {
                     const int row = z * NEB + e;
@@ -571,6 +562,43 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_message_bwd_tc(BwdParams p) {
                 mbar_arrive(&b_full[buf]);
             }
         }
+    } else if (warp == 6) {
+        // ===================== finisher: sum the four warps' partials, assemble g_e, accumulate G =====================
+        uint32_t it = 0, hc = 0;
+        for (long long u = blockIdx.x; u < n_units; u += gridDim.x) {
+            const long long a0 = u * p.atoms_per_unit;
+            const long long a1 = min(p.N, a0 + (long long)p.atoms_per_unit);
+            const int e_begin = p.row_ptr[a0], e_end = p.row_ptr[a1];
+            const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
+            for (int t = 0; t < ntiles; t++, it++) {
+                const int buf = it & 1;
+                for (int h = 0; h < 2; h++, hc++) {
+                    mbar_wait_relaxed(&r_full[hc & 1], (hc >> 1) & 1);
+                    const float* red = sRed + (hc & 1) * 128;
+                    const int E = e_begin + t * NEB + h * 8 + lane;
+                    if (lane < 8 && E < e_end) {
+                        float db = 0.f, ub0 = 0.f, ub1 = 0.f, ub2 = 0.f;
+#pragma unroll
+                        for (int wq = 0; wq < 4; wq++) {
+                            db += red[wq * 32 + 4 * lane]; ub0 += red[wq * 32 + 4 * lane + 1];
+                            ub1 += red[wq * 32 + 4 * lane + 2]; ub2 += red[wq * 32 + 4 * lane + 3];
+                        }
+                        const float4 mm = sMeta[buf * NEB + h * 8 + lane];
+                        const float inv_d = sInvd[buf * NEB + h * 8 + lane];
+                        const float uu = ub0 * mm.x + ub1 * mm.y + ub2 * mm.z;
+                        float4 g = make_float4(db * mm.x + (ub0 - uu * mm.x) * inv_d, db * mm.y + (ub1 - uu * mm.y) * inv_d,
+                                               db * mm.z + (ub2 - uu * mm.z) * inv_d, 0.f);
+                        if (!p.first) { const float4 o = p.G[E]; g.x += o.x; g.y += o.y; g.z += o.z; }
+                        p.G[E] = g;
+                    }
+                    __syncwarp();
+                    if (lane == 0) {
+                        mbar_arrive(&r_empty[hc & 1]);
+                        if (h == 1) mbar_arrive(&t_empty[buf]);
+                    }
+                }
+            }
+        }
     } else if (warp == 7) {
         if (lane == 0) {
             const uint32_t idesc = (1u << 4) | ((uint32_t)((2 * NEB) >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
@@ -583,7 +611,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_message_bwd_tc(BwdParams p) {
                 const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
                 for (int t = 0; t < ntiles; t++, it++) {
                     const int buf = it & 1;
-                    mbar_wait(&b_full[buf], (it >> 1) & 1);
+                    mbar_wait_relaxed(&b_full[buf], (it >> 1) & 1);
                     tc_fence_after();
 #pragma unroll
                     for (int c = 0; c < NCH; c++) {
@@ -606,7 +634,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_message_bwd_tc(BwdParams p) {
     if (warp == 7) tmem_dealloc(tmem_base, TALLOC);
 }
 
-constexpr int bwd_smem_bytes() { return 3 * A_CHUNK_BYTES + 2 * B_BYTES + 2 * NEB * 16 + 2 * NEB * 4 + 2 * 4 * 32 * 4 + 64 + 128; }
+constexpr int bwd_smem_bytes() { return 3 * A_CHUNK_BYTES + 2 * B_BYTES + 2 * NEB * 16 + 2 * NEB * 4 + 2 * 4 * 32 * 4 + 96 + 128; }
 
 }  // namespace etc
 
