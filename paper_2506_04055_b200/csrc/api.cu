@@ -522,8 +522,12 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
               *v1 = P<float>(m->b_v1[t]), *pq = P<float>(m->b_pq[t]), *zpre = P<float>(m->b_zpre[t]),
               *a = P<float>(m->b_a[t]);
         gemm_nt(L, S, F, l.Wm1, F, hpre, F, N, F, F, l.bm1, false);
-        silu_fwd(L, N * F, hpre, h);
-        gemm_nt(L, h, F, l.Wm2, F, phi, 3 * F, N, 3 * F, F, l.bm2, false);
+        const bool fuse_act = !m->fwd_tc && gemm_act_supported(3 * F, F);   // SiLU applied while loading A
+        if (fuse_act) gemm_nt_act(L, hpre, F, l.Wm2, F, phi, 3 * F, N, 3 * F, F, l.bm2, false, true);
+        else {
+            silu_fwd(L, N * F, hpre, h);
+            gemm_nt(L, h, F, l.Wm2, F, phi, 3 * F, N, 3 * F, F, l.bm2, false);
+        }
         mark(m, st, ST_FWD_EDGE);
         bool done = false;
         if (m->edge_path == 0 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
@@ -536,8 +540,11 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         gemm_nt(L, v1, F, l.UV, F, pq, 2 * F, 3 * N, 2 * F, F, nullptr, false);
         update_mid(L, N, F, (float)m->eps, pq, sn);
         gemm_nt(L, sn, 2 * F, l.Wu1, 2 * F, zpre, F, N, F, 2 * F, l.bu1, false);
-        silu_fwd(L, N * F, zpre, h);
-        gemm_nt(L, h, F, l.Wu2, F, a, 3 * F, N, 3 * F, F, l.bu2, false);
+        if (fuse_act) gemm_nt_act(L, zpre, F, l.Wu2, F, a, 3 * F, N, 3 * F, F, l.bu2, false, true);
+        else {
+            silu_fwd(L, N * F, zpre, h);
+            gemm_nt(L, h, F, l.Wu2, F, a, 3 * F, N, 3 * F, F, l.bu2, false);
+        }
         update_out(L, N, F, sn, v1, pq, a, P<float>(m->b_S[t + 1]), P<float>(m->b_V[t + 1]));
     }
     int n_epart = 0, n_wpart = 0;

@@ -62,6 +62,10 @@ extern int g_filter_emulate, g_gather_emulate;   // debug knobs, see painn_fwd.c
 void gemm_nt(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
              int N, int K, const float* bias, bool accumulate);
 
+void gemm_nt_act(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
+                 int N, int K, const float* bias, bool accumulate, bool act_a);
+bool gemm_act_supported(int N, int K);
+
 // ---- model kernels (painn_fwd.cu / painn_bwd.cu) ----
 void embed(const Launch& L, long long N, int F, const int* types_s, const float* Emb, float* s0, float* v0);
 void silu_fwd(const Launch& L, long long n, const float* x, float* y);

@@ -99,6 +99,83 @@ __global__ void __launch_bounds__(256) k_gemm_nt_simt(const float* __restrict__ 
     }
 }
 
+
+// ------------------------------------------------------------------------------------------------
+// k_sgemm128: fp32 FFMA path of the FORWARD linear layers (round-to-nearest accumulation; B3).
+// 128 x 128 x 8 tiles, 256 threads, 8 x 8 outputs per thread as 2 x 2 strips of 4 (conflict-free LDS.128),
+// operands transposed into shared memory ([k][row]), next tile prefetched into registers during the FMAs.
+// ACT_A: apply SiLU to A while loading (fuses the activation of the two-layer MLPs into the second GEMM).
+__device__ __forceinline__ float silu_g(float x) { return x / (1.0f + __expf(-x)); }
+
+template <bool ACT_A>
+__global__ void __launch_bounds__(256, 2) k_sgemm128(const float* __restrict__ A, int lda, const float* __restrict__ B,
+                                                      int ldb, float* __restrict__ C, int ldc, long long M, int N, int K,
+                                                      const float* __restrict__ bias, int accumulate) {
+    constexpr int BMs = 128, BNs = 128, BKs = 8, PAD = 4;
+    __shared__ __align__(16) float As[2][BKs][BMs + PAD];
+    __shared__ __align__(16) float Bs[2][BKs][BNs + PAD];
+    const int tid = threadIdx.x;
+    const int n0 = blockIdx.x * BNs;                       // N tiles fastest: CTAs sharing an A tile run together
+    const long long m0 = (long long)blockIdx.y * BMs;
+    const int lrow = tid >> 1, lk = (tid & 1) * 4;         // loader: one float4 along K per thread per operand
+    const int tx = tid & 15, ty = tid >> 4;
+    const long long arow = m0 + lrow;
+    const bool a_ok = arow < M;
+    const float* ap = A + (a_ok ? arow : 0) * lda + lk;
+    const float* bp = B + (size_t)(n0 + lrow) * ldb + lk;
+    float acc[8][8];
+#pragma unroll
+    for (int i = 0; i < 8; i++)
+#pragma unroll
+        for (int j = 0; j < 8; j++) acc[i][j] = 0.0f;
+    float4 ra = a_ok ? *(const float4*)ap : make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 rb = *(const float4*)bp;
+    auto stash = [&](int buf) {
+        if (ACT_A) { ra.x = silu_g(ra.x); ra.y = silu_g(ra.y); ra.z = silu_g(ra.z); ra.w = silu_g(ra.w); }
+        As[buf][lk + 0][lrow] = ra.x; As[buf][lk + 1][lrow] = ra.y; As[buf][lk + 2][lrow] = ra.z; As[buf][lk + 3][lrow] = ra.w;
+        Bs[buf][lk + 0][lrow] = rb.x; Bs[buf][lk + 1][lrow] = rb.y; Bs[buf][lk + 2][lrow] = rb.z; Bs[buf][lk + 3][lrow] = rb.w;
+    };
+    stash(0);
+    __syncthreads();
+    const int nk = K / BKs;
+    for (int kb = 0; kb < nk; kb++) {
+        const int cur = kb & 1;
+        if (kb + 1 < nk) {
+            ra = a_ok ? *(const float4*)(ap + (kb + 1) * BKs) : make_float4(0.f, 0.f, 0.f, 0.f);
+            rb = *(const float4*)(bp + (kb + 1) * BKs);
+        }
+#pragma unroll
+        for (int k = 0; k < BKs; k++) {
+            const float4 a0 = *(const float4*)&As[cur][k][ty * 4], a1 = *(const float4*)&As[cur][k][64 + ty * 4];
+            const float4 b0 = *(const float4*)&Bs[cur][k][tx * 4], b1 = *(const float4*)&Bs[cur][k][64 + tx * 4];
+            const float a[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
+            const float b[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+#pragma unroll
+            for (int i = 0; i < 8; i++)
+#pragma unroll
+                for (int j = 0; j < 8; j++) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+        }
+        if (kb + 1 < nk) {
+            stash(cur ^ 1);
+            __syncthreads();
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < 8; i++) {
+        const long long m = m0 + (i < 4 ? ty * 4 + i : 64 + ty * 4 + (i - 4));
+        if (m >= M) continue;
+#pragma unroll
+        for (int jh = 0; jh < 2; jh++) {
+            const int n = n0 + jh * 64 + tx * 4;
+            float4 v = make_float4(acc[i][jh * 4], acc[i][jh * 4 + 1], acc[i][jh * 4 + 2], acc[i][jh * 4 + 3]);
+            if (bias) { const float4 bb = *(const float4*)(bias + n); v.x += bb.x; v.y += bb.y; v.z += bb.z; v.w += bb.w; }
+            float* cp = C + m * ldc + n;
+            if (accumulate) { const float4 o = *(const float4*)cp; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
+            *(float4*)cp = v;
+        }
+    }
+}
+
 // weight registry: B pointer -> (hi, lo) TF32 split planes for the tensor-core path (filled at mlp_create)
 #include <unordered_map>
 static std::unordered_map<const float*, std::pair<const float*, const float*>> g_split;
@@ -109,9 +186,33 @@ void gemm_unregister_split(const float* W) { g_split.erase(W); }
 bool gemm_nt_tc(const Launch& L, const float* A, int lda, const float* Whi, const float* Wlo, int ldw, float* C, int ldc,
                 long long M, int N, int K, const float* bias, bool accumulate);
 
+void gemm_nt_act(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
+                 int N, int K, const float* bias, bool accumulate, bool act_a);
+bool gemm_act_supported(int N, int K) { return g_gemm_emulate == 0 && N % 128 == 0 && K % 8 == 0; }
+
 void gemm_nt(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
              int N, int K, const float* bias, bool accumulate) {
+    gemm_nt_act(L, A, lda, B, ldb, C, ldc, M, N, K, bias, accumulate, false);
+}
+
+// act_a: C = SiLU(A) . B^T + bias  (only the fp32 FFMA path implements it; callers use it on forward GEMMs only)
+void gemm_nt_act(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
+                 int N, int K, const float* bias, bool accumulate, bool act_a) {
     if (M == 0) return;
+    const bool fast_ok = g_gemm_emulate == 0 && N % 128 == 0 && K % 8 == 0 && lda % 4 == 0 && ldb % 4 == 0 &&
+                         ldc % 4 == 0 && ((((uintptr_t)A | (uintptr_t)B | (uintptr_t)C | (uintptr_t)bias) & 15) == 0);
+    if (act_a || (g_gemm_path == 1 && fast_ok)) {
+        if (fast_ok && M / 128 < 65535) {
+            dim3 grid((unsigned)(N / 128), (unsigned)((M + 127) / 128));
+            if (act_a) k_sgemm128<true><<<grid, 256, 0, L.stream>>>(A, lda, B, ldb, C, ldc, M, N, K, bias, accumulate ? 1 : 0);
+            else k_sgemm128<false><<<grid, 256, 0, L.stream>>>(A, lda, B, ldb, C, ldc, M, N, K, bias, accumulate ? 1 : 0);
+            KLAUNCH(L);
+            return;
+        }
+    }
+    if (act_a) {   // shapes the fast kernel does not cover: caller must not request act_a (checked by the caller)
+        return;
+    }
     if (g_gemm_path == 0 && g_gemm_emulate == 0) {
         auto it = g_split.find(B);
         if (it != g_split.end() &&
