@@ -196,6 +196,10 @@ def main():
     model = c["model"]
     N, n_local = len(c["pos"]), c["n_local"]
     m = P.Model(blob, model["n_species"], model["rc"], N)
+    opts = os.environ.get("PAINN_OPTS", "")          # experiment knobs "name=value,..." (mlp_set_option); default: none
+    for kv in filter(None, opts.split(",")):
+        name, val = kv.split("=")
+        m.set_option(name, int(val))
     pos = torch.from_numpy(c["pos"]).to(dev)
     types = torch.from_numpy(c["types"]).to(dev)
     owner = None if c["ghost_owner"] is None else torch.from_numpy(np.ascontiguousarray(c["ghost_owner"], np.int32)).to(dev)
@@ -298,6 +302,7 @@ def main():
                                          f"{stats['n_edges']} directed edges, PaiNN {model['T']}x{model['F']} K={model['K']} rc={model['rc']}",
                                 l2="working set (tens of GB) far larger than the 126 MB L2; no explicit flush",
                                 multi_gpu="replicas only (one evaluation does not shard; BASELINE.json fixes 1 GPU)",
+                                options=opts or "defaults",
                                 precision="fp64 cutoff predicate, fp32 edge math and node state, 3xTF32/fp32 GEMMs"),
                     clocks=clocks, e2e=e2e, gpu_launches=launches, roofline=roofline, cpu_baseline=cpu)
         print(json.dumps(line))

@@ -39,7 +39,8 @@ struct mlp_model {
     float* Emb = nullptr;
     LayerW lw[PAINN_MAX_T];
     float *Wr1 = nullptr, *br1 = nullptr, *wr2 = nullptr, *br2 = nullptr, *Wr1T = nullptr;
-    void* filt_img[PAINN_MAX_T] = {};   // tcgen05 A-operand image of (Wf | bf), fp16 hi/lo split (edge_tc.cu)
+    void* filt_img[PAINN_MAX_T] = {};
+    void* filt_img2[PAINN_MAX_T] = {};  // unscaled hi | lo image (edge_tc2.cu)   // tcgen05 A-operand image of (Wf | bf), fp16 hi/lo split (edge_tc.cu)
     int edge_path = 0;                  // 0: tensor-core edge kernels when F == 128, 1: plain fp32 kernels
     // capacities
     long long cap_atoms = 0, cap_edges = 0, cap_cells = 0;
@@ -65,7 +66,7 @@ struct mlp_model {
     Buf d_pos, d_types, d_owner, d_out;   // d_out: energy[1] virial[6] forces[3N]
     cudaStream_t own_stream = nullptr;
     // last call
-    long long N_last = 0, n_local_last = 0, E_last = 0;
+    long long N_last = 0, n_local_last = 0, E_last = 0 /* padded slots */, E_real_last = 0;
     Grid grid_last{};
     mlp_stats stats{};
     std::string err;
@@ -204,7 +205,8 @@ void free_buf(Buf& b, mlp_model* m = nullptr) {
 struct Misc {
     int flags[8];
     long long cell_total;
-    long long edge_total;
+    long long edge_total;                 // padded CSR slots (rows padded to ROW_PAD)
+    unsigned long long real_edges;        // edges with d < rc
     double bbox[6 + 6 * 256];
 };
 
@@ -289,6 +291,12 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
                 if (rcode == MLP_OK && cudaMemcpy(b.p, img.data(), img.size() * 2, cudaMemcpyHostToDevice) != cudaSuccess) rcode = MLP_ERR_CUDA;
                 m->wbufs.push_back(b);
                 m->filt_img[t] = b.p;
+                edge_build_filter_image2(Wf_h.data(), bf_h.data(), K, img);
+                Buf b2;
+                if (rcode == MLP_OK) rcode = ensure(m, b2, img.size() * 2);
+                if (rcode == MLP_OK && cudaMemcpy(b2.p, img.data(), img.size() * 2, cudaMemcpyHostToDevice) != cudaSuccess) rcode = MLP_ERR_CUDA;
+                m->wbufs.push_back(b2);
+                m->filt_img2[t] = b2.p;
             }
         }
         up((size_t)3 * F * K, (float**)&l.Wf); up(3 * F, (float**)&l.bf);
@@ -421,7 +429,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
     }
     Misc* dm = P<Misc>(m->b_misc);
     Misc* hm = (Misc*)m->h_misc;
-    CU(m, cudaMemsetAsync(dm, 0, sizeof(int) * 8 + 16, st));
+    CU(m, cudaMemsetAsync(dm, 0, sizeof(int) * 8 + 24, st));
     mark(m, st, ST_NBR);
 
     // ---- cell grid ----
@@ -482,10 +490,10 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
                P<int>(m->b_types_s), P<signed char>(m->b_wrap_s), P<int>(m->b_inv_perm), P<float>(m->b_local),
                P<int>(m->b_cell_id), P<int>(m->b_cell_s));
     nbr_count(L, N, g, P<double>(m->b_pos_s), P<signed char>(m->b_wrap_s), P<int>(m->b_cell_s), cell_start,
-              P<int>(m->b_row_cnt));
+              P<int>(m->b_row_cnt), &dm->real_edges);
     exclusive_scan(L, P<int>(m->b_row_cnt), P<int>(m->b_row_ptr), N, P<int>(m->b_scan_tmp), &dm->edge_total);
     // the one host read of the call: error flags + edge count (overflow check)
-    CU(m, cudaMemcpyAsync(hm, dm, sizeof(int) * 8 + 16, cudaMemcpyDeviceToHost, st));
+    CU(m, cudaMemcpyAsync(hm, dm, sizeof(int) * 8 + 24, cudaMemcpyDeviceToHost, st));
     CU(m, cudaStreamSynchronize(st));
     if (hm->flags[0] & FLAG_NONFINITE) return fail(m, MLP_ERR_NONFINITE, "non-finite (or absurdly far) position");
     if (hm->flags[0] & FLAG_TYPE_RANGE) return fail(m, MLP_ERR_TYPE_RANGE, "atom type outside 0..n_species-1");
@@ -502,7 +510,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
     float4* ej = P<float4>(m->b_ej);
     const int* row_ptr = P<int>(m->b_row_ptr);
     nbr_fill(L, N, g, P<double>(m->b_pos_s), P<signed char>(m->b_wrap_s), P<int>(m->b_cell_s), cell_start, row_ptr,
-             m->cap_edges, ej, P<unsigned char>(m->b_img), dm->flags);
+             m->cap_edges, rcf, ej, P<unsigned char>(m->b_img), dm->flags);
     nbr_reverse(L, N, row_ptr, ej, P<unsigned char>(m->b_img), P<int>(m->b_rev));
 
     // ---- forward ----
@@ -530,7 +538,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         }
         mark(m, st, ST_FWD_EDGE);
         bool done = false;
-        if (m->edge_path == 0 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
+        if (m->edge_path != 1 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
             make_gather_rows(L, N, phi, V, P<float>(m->b_Q4), P<float>(m->b_Q1), t > 0);
             done = message_fwd_tc(L, N, K, rcf, row_ptr, ej, S, V, P<float>(m->b_Q4), P<float>(m->b_Q1), m->filt_img[t], sn,
                                   v1, t > 0);
@@ -570,10 +578,14 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         gemm_nt(L, pqb, 2 * F, l.UVT, 2 * F, v1b, F, 3 * N, F, 2 * F, nullptr, true);
         mark(m, st, ST_BWD_EDGE);
         bool done = false;
-        if (m->edge_path == 0 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
+        if (m->edge_path != 1 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
             make_gather_rows_bwd(L, N, s1b, v1b, P<float>(m->b_Q4));
-            done = message_bwd_tc(L, N, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<float>(m->b_phi[t]), P<float>(m->b_V[t]),
-                                  v1b, m->filt_img[t], phib, vb, P<float4>(m->b_G), t == T - 1);
+            if (m->edge_path == 0)
+                done = message_bwd_tc2(L, N, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<float>(m->b_phi[t]),
+                                       P<float>(m->b_V[t]), v1b, m->filt_img2[t], phib, vb, P<float4>(m->b_G), t == T - 1, true);
+            if (!done)
+                done = message_bwd_tc(L, N, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<float>(m->b_phi[t]), P<float>(m->b_V[t]),
+                                      v1b, m->filt_img[t], phib, vb, P<float4>(m->b_G), t == T - 1);
         }
         if (!done)
             message_bwd(L, N, F, K, rcf, row_ptr, ej, s1b, v1b, P<float>(m->b_phi[t]), P<float>(m->b_V[t]), l.Wf, l.bf,
@@ -594,8 +606,8 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
     mark(m, st, -1);
     CU(m, cudaGetLastError());
 
-    m->N_last = N; m->n_local_last = n_local; m->E_last = E;
-    m->stats.n_atoms = N; m->stats.n_edges = E; m->stats.atom_capacity = m->cap_atoms;
+    m->N_last = N; m->n_local_last = n_local; m->E_last = E; m->E_real_last = (long long)hm->real_edges;
+    m->stats.n_atoms = N; m->stats.n_edges = m->E_real_last; m->stats.atom_capacity = m->cap_atoms;
     m->stats.edge_capacity = m->cap_edges;
     for (int d = 0; d < 3; d++) m->stats.n_cells[d] = g.n[d];
     m->stats.n_launches = launches;
@@ -631,7 +643,7 @@ __attribute__((visibility("default"))) int mlp_compute_host(mlp_model* m, const 
 
 __attribute__((visibility("default"))) int mlp_get_neighbors(mlp_model* m, long long* n_edges, int* i, int* j, signed char* image3) {
     if (!m || !n_edges) return MLP_ERR_ARG;
-    *n_edges = m->E_last;
+    *n_edges = m->E_real_last;
     if (!i) return MLP_OK;
     if (!j || !image3) return fail(m, MLP_ERR_ARG, "NULL output");
     const long long E = m->E_last, N = m->N_last;
@@ -643,10 +655,19 @@ __attribute__((visibility("default"))) int mlp_get_neighbors(mlp_model* m, long 
     CU(m, cudaDeviceSynchronize());
     nbr_export(L, N, P<int>(m->b_row_ptr), P<float4>(m->b_ej), P<unsigned char>(m->b_img), P<int>(m->b_perm),
                P<signed char>(m->b_wrap_s), P<int>(bi), P<int>(bj), P<signed char>(bm));
-    CU(m, cudaMemcpyAsync(i, bi.p, E * 4, cudaMemcpyDeviceToHost, m->own_stream));
-    CU(m, cudaMemcpyAsync(j, bj.p, E * 4, cudaMemcpyDeviceToHost, m->own_stream));
-    CU(m, cudaMemcpyAsync(image3, bm.p, E * 3, cudaMemcpyDeviceToHost, m->own_stream));
+    std::vector<int> hi(E), hj(E);
+    std::vector<signed char> him(3 * (size_t)E);
+    CU(m, cudaMemcpyAsync(hi.data(), bi.p, E * 4, cudaMemcpyDeviceToHost, m->own_stream));
+    CU(m, cudaMemcpyAsync(hj.data(), bj.p, E * 4, cudaMemcpyDeviceToHost, m->own_stream));
+    CU(m, cudaMemcpyAsync(him.data(), bm.p, E * 3, cudaMemcpyDeviceToHost, m->own_stream));
     CU(m, cudaStreamSynchronize(m->own_stream));
+    long long k = 0;                                        // drop the padding slots
+    for (long long e = 0; e < E; e++)
+        if (hi[e] >= 0) {
+            i[k] = hi[e]; j[k] = hj[e];
+            image3[3 * k] = him[3 * e]; image3[3 * k + 1] = him[3 * e + 1]; image3[3 * k + 2] = him[3 * e + 2];
+            k++;
+        }
     free_buf(bi, m); free_buf(bj, m); free_buf(bm, m);
     return MLP_OK;
 }

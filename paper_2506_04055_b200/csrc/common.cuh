@@ -7,6 +7,7 @@
 
 #define PAINN_MAX_T 8
 #define PAINN_MAX_K 32
+#define ROW_PAD 8          // CSR rows are padded to a multiple of ROW_PAD slots (dummy edges: sender index < 0)
 
 namespace painn {
 
@@ -45,10 +46,10 @@ void nbr_gather(const Launch& L, long long N, long long n_local, const int* perm
                 const int* types, const signed char* wrap, double* pos_s, int* types_s, signed char* wrap_s,
                 int* inv_perm, float* local_mask, const int* cell_id, int* cell_s);
 void nbr_count(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s,
-               const int* cell_s, const int* cell_start, int* row_cnt);
+               const int* cell_s, const int* cell_start, int* row_cnt, unsigned long long* real_total);
 void nbr_fill(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s,
-              const int* cell_s, const int* cell_start, const int* row_ptr, long long cap_edges, float4* ej, unsigned char* img,
-              int* flags);
+              const int* cell_s, const int* cell_start, const int* row_ptr, long long cap_edges, float rc, float4* ej,
+              unsigned char* img, int* flags);
 void nbr_reverse(const Launch& L, long long N, const int* row_ptr, const float4* ej, const unsigned char* img,
                  int* rev);
 void nbr_export(const Launch& L, long long N, const int* row_ptr, const float4* ej, const unsigned char* img,
@@ -103,5 +104,9 @@ void make_gather_rows_bwd(const Launch& L, long long N, const float* s1b, const 
 bool message_bwd_tc(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
                     const float* phi, const float* v_in, const float* v1b, const void* A_img, float* phib, float* vb_out,
                     float4* G, bool first);
+void edge_build_filter_image2(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img);
+bool message_bwd_tc2(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
+                     const float* phi, const float* v_in, const float* v1b, const void* A_img2, float* phib, float* vb_out,
+                     float4* G, bool first, bool need_sender);
 
 }  // namespace painn

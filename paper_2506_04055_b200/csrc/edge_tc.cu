@@ -96,8 +96,9 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_message_fwd_tc(FwdParams p) {
     constexpr int NCH = HAS_V ? 3 : 2;
     constexpr int TCOLS = NCH * NE;                 // TMEM columns per buffer
     constexpr int TALLOC = HAS_V ? 256 : 128;
-    extern __shared__ uint8_t smem_raw[];
-    uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+    // declared aligned (no run-time pointer rounding: that would hide the shared address space from the compiler
+    // and turn every LDS / STS into a generic LD / ST)
+    extern __shared__ __align__(128) uint8_t smem[];
     uint8_t* sA = smem;
     uint8_t* sB = sA + NCH * A_CHUNK_BYTES;
     float4* sMeta = (float4*)(sB + 2 * B_BYTES);
@@ -228,12 +229,14 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_message_fwd_tc(FwdParams p) {
                 float4 r = make_float4(1.f, 0.f, 0.f, __int_as_float(0));
                 const bool valid = E < e_end;
                 if (valid) r = __ldg(p.ej + E);
+                const bool real = valid && __float_as_int(r.w) >= 0;     // padding slots carry sender index ~self
+                if (valid && !real) r.w = __int_as_float(~__float_as_int(r.w));
                 const float d2 = r.x * r.x + r.y * r.y + r.z * r.z;
                 const float inv_d = rsqrtf(d2);
                 const float x = d2 * inv_d * p.inv_rc;
                 float s1, c1;
                 sincospif(x, &s1, &c1);
-                const float fc = valid ? 0.5f * (1.0f + c1) : 0.0f;
+                const float fc = real ? 0.5f * (1.0f + c1) : 0.0f;
                 const float amp = fc * inv_d;
                 float sn_, cn_;
                 const int n0 = h == 0 ? 1 : 8 * h;
@@ -349,8 +352,9 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_message_bwd_tc(BwdParams p) {
     constexpr int NCH = 3;
     constexpr int TCOLS = NCH * 2 * NEB;            // 96 TMEM columns per buffer
     constexpr int TALLOC = 256;
-    extern __shared__ uint8_t smem_raw[];
-    uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+    // declared aligned (no run-time pointer rounding: that would hide the shared address space from the compiler
+    // and turn every LDS / STS into a generic LD / ST)
+    extern __shared__ __align__(128) uint8_t smem[];
     uint8_t* sA = smem;
     uint8_t* sB = sA + NCH * A_CHUNK_BYTES;                  // 2 buffers x (32 rows x 96 halfs) = 2 x 6144
     float4* sMeta = (float4*)(sB + 2 * B_BYTES);            // [2][16] (u_e, i)
@@ -507,13 +511,15 @@ __global__ void __launch_bounds__(NTHREADS, 2) k_message_bwd_tc(BwdParams p) {
                 float4 r = make_float4(1.f, 0.f, 0.f, __int_as_float(0));
                 const bool valid = E < e_end;
                 if (valid) r = __ldg(p.ej + E);
+                const bool real = valid && __float_as_int(r.w) >= 0;     // padding slots carry sender index ~self
+                if (valid && !real) r.w = __int_as_float(~__float_as_int(r.w));
                 const float d2 = r.x * r.x + r.y * r.y + r.z * r.z;
                 const float inv_d = rsqrtf(d2);
                 const float x = d2 * inv_d * p.inv_rc;
                 float s1, c1;
                 sincospif(x, &s1, &c1);
-                const float fc = valid ? 0.5f * (1.0f + c1) : 0.0f;
-                const float dfc = valid ? -0.5f * a1c * s1 : 0.0f;
+                const float fc = real ? 0.5f * (1.0f + c1) : 0.0f;
+                const float dfc = real ? -0.5f * a1c * s1 : 0.0f;
                 float sn_, cn_;
                 const int n0 = h == 0 ? 1 : 8 * h;
                 if (h == 0) { sn_ = s1; cn_ = c1; } else sincospif((float)n0 * x, &sn_, &cn_);

@@ -63,8 +63,9 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
     k_gemm_3xtf32(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapWhi,
                   const __grid_constant__ CUtensorMap mapWlo, Params p) {
     using S = Smem<BN, STAGES>;
-    extern __shared__ uint8_t smem_raw[];
-    uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    // declared aligned (no run-time pointer rounding: that would hide the shared address space from the compiler
+    // and turn every LDS / STS into a generic LD / ST)
+    extern __shared__ __align__(1024) uint8_t smem[];
     uint64_t* bars = (uint64_t*)(smem + STAGES * S::STAGE);
     uint64_t* full = bars;                   // TMA landed            (count 1 + tx)
     uint64_t* conv = bars + STAGES;          // A converted           (count 128)

@@ -274,24 +274,31 @@ __device__ __forceinline__ void visit_neighbors(long long a, const Grid& g, cons
 
 __global__ void __launch_bounds__(128) k_count(long long N, Grid g, const double* __restrict__ pos_s,
                                                const signed char* __restrict__ wrap_s, const int* __restrict__ cell_s,
-                                               const int* __restrict__ cell_start, int* __restrict__ row_cnt) {
+                                               const int* __restrict__ cell_start, int* __restrict__ row_cnt,
+                                               unsigned long long* __restrict__ real_total) {
     long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (a >= N) return;
     int cnt = 0;
-    visit_neighbors(a, g, pos_s, wrap_s, cell_s, cell_start, [&](int, int, double, double, double) { cnt++; });
-    row_cnt[a] = cnt;
+    if (a < N) {
+        visit_neighbors(a, g, pos_s, wrap_s, cell_s, cell_start, [&](int, int, double, double, double) { cnt++; });
+        // rows are padded to a multiple of 8 slots with zero-weight dummy edges, so that an 8-edge group of the
+        // tensor-core edge kernels never straddles two rows (branch-free inner loops)
+        row_cnt[a] = (cnt + ROW_PAD - 1) & ~(ROW_PAD - 1);
+    }
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(real_total, (unsigned long long)cnt);
 }
 void nbr_count(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s,
-               const int* cell_s, const int* cell_start, int* row_cnt) {
+               const int* cell_s, const int* cell_start, int* row_cnt, unsigned long long* real_total) {
     if (N == 0) return;
-    k_count<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, pos_s, wrap_s, cell_s, cell_start, row_cnt);
+    k_count<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, pos_s, wrap_s, cell_s, cell_start, row_cnt,
+                                                               real_total);
     KLAUNCH(L);
 }
 
 __global__ void __launch_bounds__(128) k_fill(long long N, Grid g, const double* __restrict__ pos_s,
                                               const signed char* __restrict__ wrap_s, const int* __restrict__ cell_s,
                                               const int* __restrict__ cell_start, const int* __restrict__ row_ptr,
-                                              long long cap_edges, float4* __restrict__ ej,
+                                              long long cap_edges, float rc, float4* __restrict__ ej,
                                               unsigned char* __restrict__ img, int* __restrict__ flags) {
     long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (a >= N) return;
@@ -302,13 +309,18 @@ __global__ void __launch_bounds__(128) k_fill(long long N, Grid g, const double*
         img[e] = (unsigned char)code;
         e++;
     });
+    // dummy slots: sender index ~a (negative), |r| = rc; every kernel gives them exactly zero weight
+    for (const long long e1 = row_ptr[a + 1]; e < e1; e++) {
+        ej[e] = make_float4(rc, 0.0f, 0.0f, __int_as_float(~(int)a));
+        img[e] = 255;
+    }
 }
 void nbr_fill(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s,
-              const int* cell_s, const int* cell_start, const int* row_ptr, long long cap_edges, float4* ej, unsigned char* img,
-              int* flags) {
+              const int* cell_s, const int* cell_start, const int* row_ptr, long long cap_edges, float rc, float4* ej,
+              unsigned char* img, int* flags) {
     if (N == 0) return;
     k_fill<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, pos_s, wrap_s, cell_s, cell_start, row_ptr, cap_edges,
-                                                              ej, img, flags);
+                                                              rc, ej, img, flags);
     KLAUNCH(L);
 }
 
@@ -321,6 +333,7 @@ __global__ void k_reverse(long long N, const int* __restrict__ row_ptr, const fl
     if (a >= N) return;
     for (int e = row_ptr[a] + lane; e < row_ptr[a + 1]; e += 32) {
         int b = __float_as_int(ej[e].w);
+        if (b < 0) { rev[e] = e; continue; }          // dummy slot: its own reverse (G[rev] - G = 0)
         int want = 26 - (int)img[e];
         int r = -1;
         for (int x = row_ptr[b]; x < row_ptr[b + 1]; x++)
@@ -344,6 +357,7 @@ __global__ void k_export(long long N, const int* __restrict__ row_ptr, const flo
     if (a >= N) return;
     for (int e = row_ptr[a]; e < row_ptr[a + 1]; e++) {
         int b = __float_as_int(ej[e].w);
+        if (b < 0) { out_i[e] = -1; out_j[e] = -1; continue; }   // dummy slot (compacted away by the host)
         int code = img[e];
         int s[3] = {code / 9 - 1, (code / 3) % 3 - 1, code % 3 - 1};
         out_i[e] = perm[a];

@@ -120,7 +120,9 @@ __global__ void __launch_bounds__(128) k_message_bwd(long long N, int F, int K, 
         const int cn = min(BWD_CHUNK, e1 - c0);
         for (int k = 0; k < cn; k++) {
             const float4 r = ej[c0 + k];
-            const int i = __float_as_int(r.w);
+            const int i_raw = __float_as_int(r.w);
+            const bool dummy = i_raw < 0;                 // padding slot: zero weight, gathers its own row
+            const int i = dummy ? ~i_raw : i_raw;
             const float d2 = r.x * r.x + r.y * r.y + r.z * r.z;
             const float inv_d = rsqrtf(d2);
             const float d = d2 * inv_d;
@@ -129,8 +131,8 @@ __global__ void __launch_bounds__(128) k_message_bwd(long long N, int F, int K, 
             sincospif(d * inv_rc, &s1, &c1);
             float sn_ = s1, cn_ = c1;
             const float a1 = PI_F * inv_rc;
-            const float fc = 0.5f * (1.0f + c1);
-            const float dfc = -0.5f * a1 * s1;
+            const float fc = dummy ? 0.0f : 0.5f * (1.0f + c1);
+            const float dfc = dummy ? 0.0f : -0.5f * a1 * s1;
             // w = Wf (fc rho) + bf fc ;  w' = Wf (fc' rho + fc rho') + bf fc'   (both as GEMM operands)
             float wS_ = fdot<EMU>(bS, fc, 0.f), wVS_ = fdot<EMU>(bVS, fc, 0.f), wVV_ = fdot<EMU>(bVV, fc, 0.f);
             float dwS = fdot<EMU>(bS, dfc, 0.f), dwVS = fdot<EMU>(bVS, dfc, 0.f), dwVV = fdot<EMU>(bVV, dfc, 0.f);

@@ -96,6 +96,7 @@ __global__ void __launch_bounds__(128) k_message_fwd(long long N, int F, int K, 
     for (int e = e0; e < e1; e++) {
         const float4 r = ej[e];
         const int j = __float_as_int(r.w);
+        if (j < 0) continue;                         // padding slot
         const float d2 = r.x * r.x + r.y * r.y + r.z * r.z;
         const float inv_d = rsqrtf(d2);
         const float d = d2 * inv_d;
