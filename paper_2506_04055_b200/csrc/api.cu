@@ -540,8 +540,12 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         bool done = false;
         if (m->edge_path != 1 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
             make_gather_rows(L, N, phi, V, P<float>(m->b_Q4), P<float>(m->b_Q1), t > 0);
-            done = message_fwd_tc(L, N, K, rcf, row_ptr, ej, S, V, P<float>(m->b_Q4), P<float>(m->b_Q1), m->filt_img[t], sn,
-                                  v1, t > 0);
+            if (m->edge_path == 0)
+                done = message_fwd_v3(L, N, K, rcf, row_ptr, ej, S, V, P<float>(m->b_Q4), P<float>(m->b_Q1), m->filt_img[t],
+                                      sn, v1, t > 0);
+            if (!done)
+                done = message_fwd_tc(L, N, K, rcf, row_ptr, ej, S, V, P<float>(m->b_Q4), P<float>(m->b_Q1), m->filt_img[t],
+                                      sn, v1, t > 0);
         }
         if (!done) message_fwd(L, N, F, K, rcf, row_ptr, ej, S, V, phi, l.Wf, l.bf, sn, v1);
         mark(m, st, ST_FWD_NODE);
@@ -581,6 +585,9 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         if (m->edge_path != 1 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
             make_gather_rows_bwd(L, N, s1b, v1b, P<float>(m->b_Q4));
             if (m->edge_path == 0)
+                done = message_bwd_v3(L, N, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<float>(m->b_phi[t]),
+                                      P<float>(m->b_V[t]), v1b, m->filt_img[t], phib, vb, P<float4>(m->b_G), t == T - 1, t == 0);
+            if (!done && m->edge_path == 3)
                 done = message_bwd_tc2(L, N, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<float>(m->b_phi[t]),
                                        P<float>(m->b_V[t]), v1b, m->filt_img2[t], phib, vb, P<float4>(m->b_G), t == T - 1, true);
             if (!done)
@@ -591,6 +598,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
             message_bwd(L, N, F, K, rcf, row_ptr, ej, s1b, v1b, P<float>(m->b_phi[t]), P<float>(m->b_V[t]), l.Wf, l.bf,
                         phib, vb, P<float4>(m->b_G), t == T - 1);
         mark(m, st, ST_BWD_NODE);
+        if (t == 0) break;      // s^0 is the (constant) embedding: its adjoint is never used
         gemm_nt(L, phib, 3 * F, l.Wm2T, 3 * F, hb, F, N, F, 3 * F, nullptr, false);
         mul_dsilu(L, N * F, P<float>(m->b_hpre[t]), hb);
         gemm_nt(L, hb, F, l.Wm1T, F, s1b, F, N, F, F, nullptr, true);

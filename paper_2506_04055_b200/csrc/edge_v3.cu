@@ -1,0 +1,741 @@
+// edge_v3.cu -- third-generation message / adjoint-message kernels (F = 128).
+//
+// Same mathematics and the same tensor-core filter as edge_tc.cu (per-edge filter w_e = fc (Wf rho + bf) as a
+// tcgen05 GEMM with fp16 hi/lo split operands, accumulator D[channel, edge] in TMEM, one channel per lane, CSR
+// segment sums in registers, no atomics).  What changed comes from the ncu captures of the earlier kernels
+// (profiles/r01_edge_ncu.md): they issued 35 (forward) and 104 (adjoint) warp instructions per (edge, 32 channels),
+// sat at 36-50 % issue utilisation with "long scoreboard" as the top stall, and moved 6 TB/s of the >16 TB/s the
+// L2 -> SM path sustains for this access pattern (row gathers of 512 B per warp).  Here
+//   * the gathers are software-pipelined in two register banks of 8 edges: the loads of batch b+1 are in flight
+//     while batch b is consumed (ping-pong, statically unrolled so that ptxas keeps one scoreboard per bank);
+//   * the pipeline runs across tile and unit boundaries (consumers peek at the producers' "operand ready" barrier
+//     of the next tile to fetch its sender indices early);
+//   * rows are padded to 8 slots with zero-weight dummies, so nothing is predicated per edge: one uniform
+//     row-boundary test per 8 edges; the receiver's own rows (residual / phi_j, v_j) are loaded one row ahead;
+//   * the adjoint reduces its four per-edge scalars over the 128 channels through shared memory (one STS.128 per
+//     (edge, channel), 8 LDS.128 + a 16-lane shuffle tree per thread and 8 edges) instead of a 31-shuffle butterfly
+//     plus a finisher warp, and layer 0 (v = 0, embedding constant) runs a 2-chunk variant without sender adjoint.
+#include <cuda_fp16.h>
+
+#include <algorithm>
+#include <cstring>
+#include <vector>
+
+#include "common.cuh"
+#include "tc_common.cuh"
+
+namespace painn {
+
+#define KLAUNCH(L) (++*(L).counter)
+
+namespace ev3 {
+
+using namespace tc;
+
+constexpr int F = 128;
+constexpr int KP = 96;                        // 3 split terms x 32 basis slots (same A image as edge_tc.cu)
+constexpr int LBO = 128, SBO = (KP / 8) * 128;          // 1536
+constexpr int A_CHUNK_BYTES = (F / 8) * SBO;            // 24576
+
+// -------------------------------------------------------------------------------------------------------------
+// producer helper: R_e = fc (1, rho_1..rho_K) [and R'_e = d/dd of it] for basis slots 8h..8h+7 of one edge
+// -------------------------------------------------------------------------------------------------------------
+struct EdgeGeom {
+    float4 r;        // (r_e, sender index bits)
+    float inv_d, s1, c1, x;
+    bool real;
+};
+__device__ __forceinline__ EdgeGeom load_edge(const float4* __restrict__ ej, int E, int e_end, float inv_rc) {
+    EdgeGeom g;
+    g.r = make_float4(1.f, 0.f, 0.f, __int_as_float(0));
+    const bool valid = E < e_end;
+    if (valid) g.r = __ldg(ej + E);
+    g.real = valid && __float_as_int(g.r.w) >= 0;                 // padding slots carry sender index ~self
+    if (valid && !g.real) g.r.w = __int_as_float(~__float_as_int(g.r.w));
+    const float d2 = g.r.x * g.r.x + g.r.y * g.r.y + g.r.z * g.r.z;
+    g.inv_d = rsqrtf(d2);
+    g.x = d2 * g.inv_d * inv_rc;
+    sincospif(g.x, &g.s1, &g.c1);
+    return g;
+}
+// split 8 fp32 values into the three fp16 planes of the B operand: hi, lo * 2^11, hi * 2^-11
+__device__ __forceinline__ void split3(const float (&v)[8], uint4& p0, uint4& p1, uint4& p2) {
+    __half2 a[4], b[4], c[4];
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+        const __half h0 = __float2half_rn(v[2 * i]), h1 = __float2half_rn(v[2 * i + 1]);
+        const float f0 = __half2float(h0), f1 = __half2float(h1);
+        a[i] = __halves2half2(h0, h1);
+        b[i] = __halves2half2(__float2half_rn((v[2 * i] - f0) * 2048.0f), __float2half_rn((v[2 * i + 1] - f1) * 2048.0f));
+        c[i] = __halves2half2(__float2half_rn(f0 * (1.0f / 2048.0f)), __float2half_rn(f1 * (1.0f / 2048.0f)));
+    }
+    p0 = *(uint4*)a; p1 = *(uint4*)b; p2 = *(uint4*)c;
+}
+
+// =============================================================================================================
+// forward message pass
+// =============================================================================================================
+constexpr int NE = 32;                                  // edges per tile (MMA N)
+constexpr int B_BYTES = (NE / 8) * SBO;                 // 6144
+constexpr int FWD_THREADS = 256;
+
+struct FwdParams {
+    long long N;
+    const int* row_ptr;
+    const float4* ej;
+    const float* s;
+    const float* v;
+    const float4* Q4;
+    const float* Q1;
+    const float2* Q2;
+    const uint4* A_img;
+    float* sn;     // s' written with row stride 2F
+    float* v1;
+    float inv_rc;
+    int K;
+    int atoms_per_unit;
+};
+
+constexpr int fwd_smem_bytes(bool has_v) { return (has_v ? 3 : 2) * A_CHUNK_BYTES + 2 * B_BYTES + 2 * NE * 16 + 64 + 128; }
+
+template <bool HAS_V>
+__global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
+    constexpr int NCH = HAS_V ? 3 : 2;
+    constexpr int TCOLS = NCH * NE;                 // TMEM columns per buffer
+    constexpr int TALLOC = HAS_V ? 256 : 128;
+    extern __shared__ __align__(128) uint8_t smem[];
+    uint8_t* sA = smem;
+    uint8_t* sB = sA + NCH * A_CHUNK_BYTES;
+    float4* sMeta = (float4*)(sB + 2 * B_BYTES);   // [2][NE] (u_e, sender index)
+    uint64_t* bars = (uint64_t*)(sMeta + 2 * NE);
+    uint64_t* b_full = bars;          // [2] producers -> MMA (and consumers: sender indices readable)  (count 96)
+    uint64_t* t_full = bars + 2;      // [2] MMA commit -> consumers (count 1)
+    uint64_t* t_empty = bars + 4;     // [2] consumers -> producers  (count 4)
+    uint32_t* tmem_slot = (uint32_t*)(bars + 6);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    {
+        const uint4* src = p.A_img;
+        uint4* dst = (uint4*)sA;
+        for (int i = tid; i < NCH * A_CHUNK_BYTES / 16; i += FWD_THREADS) dst[i] = src[i];
+        uint4* zb = (uint4*)sB;
+        for (int i = tid; i < 2 * B_BYTES / 16; i += FWD_THREADS) zb[i] = make_uint4(0, 0, 0, 0);
+    }
+    if (tid == 0) {
+        for (int b = 0; b < 2; b++) { mbar_init(&b_full[b], 96); mbar_init(&t_full[b], 1); mbar_init(&t_empty[b], 4); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 7) tmem_alloc(tmem_slot, TALLOC);
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    const long long N = p.N;
+    const int apu = p.atoms_per_unit;
+    const int* __restrict__ row_ptr = p.row_ptr;
+    const long long n_units = (N + apu - 1) / apu;
+    if (warp < 4) reg_inc<168>(); else reg_dec<88>();
+
+    if (warp < 4) {
+        // ===================== consumers: one channel per thread =====================
+        const int f = tid;
+        const float4* __restrict__ Q4 = p.Q4 + f;
+        const float* __restrict__ Q1 = p.Q1 + f;
+        const float2* __restrict__ Q2 = p.Q2 + f;
+        const float* __restrict__ s_in = p.s + f;
+        const float* __restrict__ v_in = p.v + f;
+        float* __restrict__ sn = p.sn + f;
+        float* __restrict__ v1 = p.v1 + f;
+        const uint32_t lane_base = tmem_base + ((uint32_t)(warp * 32) << 16);
+        float4 qa4[8], qb4[8];
+        float qa1[8], qb1[8];
+        float2 qa2[8], qb2[8];
+#define FWD_ISSUE(Q4R, Q1R, Q2R, META8)                                                   \
+    {                                                                                     \
+        _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                \
+            const size_t row_ = (size_t)__float_as_int((META8)[i_].w) * F;                \
+            if (HAS_V) { Q4R[i_] = __ldg(Q4 + row_); Q1R[i_] = __ldg(Q1 + row_); }        \
+            else Q2R[i_] = __ldg(Q2 + row_);                                              \
+        }                                                                                 \
+    }
+        uint32_t it = 0;
+        bool pre = false;                 // first batch of tile `it` already in flight (bank a)
+        for (long long u = blockIdx.x; u < n_units; u += gridDim.x) {
+            const long long a0 = u * apu;
+            const int na = (int)min((long long)apu, N - a0);
+            const int rp = __ldg(row_ptr + a0 + min(lane, na));           // lanes 0..na hold the unit's row pointers
+            const int e_begin = __shfl_sync(0xffffffffu, rp, 0), e_end = __shfl_sync(0xffffffffu, rp, na);
+            const int ntiles = (e_end - e_begin + NE - 1) / NE;
+            bool next_has = false;                                        // does the CTA's next unit have a tile?
+            {
+                const long long un = u + gridDim.x;
+                if (un < n_units) {
+                    const long long b0 = un * apu, b1 = min(N, b0 + apu);
+                    next_has = __ldg(row_ptr + b1) > __ldg(row_ptr + b0);
+                }
+            }
+            if (ntiles > 0 && !pre) {
+                mbar_wait(&b_full[it & 1], (it >> 1) & 1);
+                const float4* m0 = sMeta + (it & 1) * NE;
+                FWD_ISSUE(qa4, qa1, qa2, m0);
+            }
+            pre = false;
+            int a_rel = 0;
+            int row_end = __shfl_sync(0xffffffffu, rp, 1);
+            float accS = 0.f, acc0 = 0.f, acc1 = 0.f, acc2 = 0.f;
+            // residual (s_i, v_i) of the current receiver: loaded at row start, added at row end
+            float rs = s_in[(a0 + a_rel) * F], rv0 = 0.f, rv1 = 0.f, rv2 = 0.f;
+            if (HAS_V) { rv0 = v_in[(a0 + a_rel) * 3 * F]; rv1 = v_in[(a0 + a_rel) * 3 * F + F]; rv2 = v_in[(a0 + a_rel) * 3 * F + 2 * F]; }
+            auto store_row = [&]() {
+                const long long a = a0 + a_rel;
+                sn[a * 2 * F] = accS + rs;
+                v1[a * 3 * F] = acc0 + rv0; v1[a * 3 * F + F] = acc1 + rv1; v1[a * 3 * F + 2 * F] = acc2 + rv2;
+            };
+            auto next_row = [&]() {
+                store_row();
+                a_rel++;
+                row_end = __shfl_sync(0xffffffffu, rp, a_rel + 1);
+                accS = acc0 = acc1 = acc2 = 0.f;
+                const long long a = a0 + a_rel;
+                rs = s_in[a * F];
+                if (HAS_V) { rv0 = v_in[a * 3 * F]; rv1 = v_in[a * 3 * F + F]; rv2 = v_in[a * 3 * F + 2 * F]; }
+            };
+#define FWD_COMPUTE(BI, Q4R, Q1R, Q2R)                                                                      \
+    {                                                                                                       \
+        const int E8_ = e_begin + t * NE + (BI) * 8;                                                        \
+        if (E8_ < e_end) {                                                                                  \
+            while (E8_ >= row_end) next_row();                                                              \
+            uint32_t ws[8], wvs[8], wvv[8];                                                                 \
+            tmem_ld8_nowait(lane_base + buf * TCOLS + (BI) * 8, ws);                                        \
+            tmem_ld8_nowait(lane_base + buf * TCOLS + NE + (BI) * 8, wvs);                                  \
+            if (HAS_V) tmem_ld8_nowait(lane_base + buf * TCOLS + 2 * NE + (BI) * 8, wvv);                   \
+            tmem_wait_ld();                                                                                 \
+            _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                              \
+                const float4 m_ = meta[(BI) * 8 + i_];                                                      \
+                const float w_s = __uint_as_float(ws[i_]), w_vs = __uint_as_float(wvs[i_]);                 \
+                if (HAS_V) {                                                                                \
+                    const float w_vv = __uint_as_float(wvv[i_]);                                            \
+                    accS = fmaf(w_s, Q4R[i_].x, accS);                                                      \
+                    const float tv = w_vs * Q4R[i_].y;                                                      \
+                    acc0 = fmaf(tv, m_.x, fmaf(w_vv, Q4R[i_].z, acc0));                                     \
+                    acc1 = fmaf(tv, m_.y, fmaf(w_vv, Q4R[i_].w, acc1));                                     \
+                    acc2 = fmaf(tv, m_.z, fmaf(w_vv, Q1R[i_], acc2));                                       \
+                } else {                                                                                    \
+                    accS = fmaf(w_s, Q2R[i_].x, accS);                                                      \
+                    const float tv = w_vs * Q2R[i_].y;                                                      \
+                    acc0 = fmaf(tv, m_.x, acc0);                                                            \
+                    acc1 = fmaf(tv, m_.y, acc1);                                                            \
+                    acc2 = fmaf(tv, m_.z, acc2);                                                            \
+                }                                                                                           \
+            }                                                                                               \
+        }                                                                                                   \
+    }
+            for (int t = 0; t < ntiles; t++, it++) {
+                const int buf = it & 1;
+                const float4* meta = sMeta + buf * NE;
+                FWD_ISSUE(qb4, qb1, qb2, meta + 8);
+                mbar_wait(&t_full[buf], (it >> 1) & 1);
+                tc_fence_after();
+                FWD_COMPUTE(0, qa4, qa1, qa2);
+                FWD_ISSUE(qa4, qa1, qa2, meta + 16);
+                FWD_COMPUTE(1, qb4, qb1, qb2);
+                FWD_ISSUE(qb4, qb1, qb2, meta + 24);
+                FWD_COMPUTE(2, qa4, qa1, qa2);
+                if (t + 1 < ntiles || next_has) {                  // first batch of the CTA's next tile
+                    mbar_wait(&b_full[buf ^ 1], ((it + 1) >> 1) & 1);
+                    const float4* mn = sMeta + (buf ^ 1) * NE;
+                    FWD_ISSUE(qa4, qa1, qa2, mn);
+                    pre = t + 1 == ntiles;
+                }
+                FWD_COMPUTE(3, qb4, qb1, qb2);
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&t_empty[buf]);
+            }
+            // finish the last receiver with edges, then pass trailing edge-less atoms through (s' = s, v' = v)
+            for (;;) {
+                store_row();
+                if (a_rel + 1 >= na) break;
+                a_rel++;
+                accS = acc0 = acc1 = acc2 = 0.f;
+                const long long a = a0 + a_rel;
+                rs = s_in[a * F];
+                if (HAS_V) { rv0 = v_in[a * 3 * F]; rv1 = v_in[a * 3 * F + F]; rv2 = v_in[a * 3 * F + 2 * F]; }
+            }
+        }
+#undef FWD_ISSUE
+#undef FWD_COMPUTE
+    } else if (warp < 7) {
+        // ===================== producers: B operand R_e = fc (1, rho_1 .. rho_K), three fp16 planes =====================
+        const int pt = tid - 128, e = pt & 31, h = pt >> 5;   // h: basis slots 8h .. 8h+7 (slot 0 = bias, slot n = rho_n)
+        const float inv_rc = p.inv_rc;
+        const int K = p.K;
+        uint32_t it = 0;
+        for (long long u = blockIdx.x; u < n_units; u += gridDim.x) {
+            const long long a0 = u * apu;
+            const long long a1 = min(N, a0 + (long long)apu);
+            const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
+            const int ntiles = (e_end - e_begin + NE - 1) / NE;
+            for (int t = 0; t < ntiles; t++, it++) {
+                const int buf = it & 1;
+                const EdgeGeom g = load_edge(p.ej, e_begin + t * NE + e, e_end, inv_rc);
+                const float fc = g.real ? 0.5f * (1.0f + g.c1) : 0.0f;
+                const float amp = fc * g.inv_d;
+                float sn_, cn_;
+                if (h == 0) { sn_ = g.s1; cn_ = g.c1; } else sincospif((float)(8 * h) * g.x, &sn_, &cn_);
+                float vals[8];
+#pragma unroll
+                for (int i = 0; i < 8; i++) {
+                    const int b = h * 8 + i;
+                    float R;
+                    if (b == 0) R = fc;
+                    else {
+                        R = b <= K ? amp * sn_ : 0.0f;
+                        const float tt = sn_ * g.c1 + cn_ * g.s1;
+                        cn_ = cn_ * g.c1 - sn_ * g.s1;
+                        sn_ = tt;
+                    }
+                    vals[i] = R;
+                }
+                uint4 p0, p1, p2;
+                split3(vals, p0, p1, p2);
+                mbar_wait(&t_empty[buf], ((it >> 1) & 1) ^ 1);
+                uint8_t* bb = sB + buf * B_BYTES + (e >> 3) * SBO + (e & 7) * 16 + h * LBO;
+                *(uint4*)(bb) = p0;                       // term 0: k = b
+                *(uint4*)(bb + 4 * LBO) = p1;             // term 1: k = 32 + b   (lo(R) 2^11)
+                *(uint4*)(bb + 8 * LBO) = p2;             // term 2: k = 64 + b   (hi(R) 2^-11)
+                if (h == 0) sMeta[buf * NE + e] = make_float4(g.r.x * g.inv_d, g.r.y * g.inv_d, g.r.z * g.inv_d, g.r.w);
+                fence_async_smem();
+                mbar_arrive(&b_full[buf]);
+            }
+        }
+    } else {
+        // ===================== MMA issuer =====================
+        if (lane == 0) {
+            const uint32_t idesc = (1u << 4) | ((uint32_t)(NE >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);   // f16 x f16 -> f32
+            const uint32_t a_base = smem_u32(sA), b_base = smem_u32(sB);
+            uint32_t it = 0;
+            for (long long u = blockIdx.x; u < n_units; u += gridDim.x) {
+                const long long a0 = u * apu;
+                const long long a1 = min(N, a0 + (long long)apu);
+                const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
+                const int ntiles = (e_end - e_begin + NE - 1) / NE;
+                for (int t = 0; t < ntiles; t++, it++) {
+                    const int buf = it & 1;
+                    mbar_wait(&b_full[buf], (it >> 1) & 1);
+                    tc_fence_after();
+#pragma unroll
+                    for (int c = 0; c < NCH; c++) {
+                        const uint32_t d = tmem_base + buf * TCOLS + c * NE;
+#pragma unroll
+                        for (int o = 0; o < 6; o++) {
+                            const int kk = (o + 2) % 6;          // small terms (k-steps 2..5) first, main term last
+                            const uint64_t ad = make_desc_nosw(a_base + c * A_CHUNK_BYTES + kk * 2 * LBO, LBO, SBO);
+                            const uint64_t bd = make_desc_nosw(b_base + buf * B_BYTES + kk * 2 * LBO, LBO, SBO);
+                            umma_f16(d, ad, bd, idesc, o != 0);
+                        }
+                    }
+                    umma_commit(&t_full[buf]);
+                }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 7) tmem_dealloc(tmem_base, TALLOC);
+}
+
+
+// =============================================================================================================
+// adjoint message pass (sender-row gather form, painn_bwd.cu header): one 512-thread CTA per SM = two independent
+// 8-warp pipelines ("groups") that share one copy of the filter operand
+// =============================================================================================================
+constexpr int NEB = 16;                                 // edges per tile; B rows 0..15 = R_e, 16..31 = R'_e
+constexpr int BB_BYTES = (2 * NEB / 8) * SBO;           // 6144
+constexpr int BWD_THREADS = 512;
+constexpr int P_BYTES = 8 * F * 16;                     // per-edge partials of one 8-edge batch: [8][128] float4
+constexpr int G_OFF_B = 0, G_OFF_P = 2 * BB_BYTES, G_OFF_META = G_OFF_P + 2 * P_BYTES,
+              G_OFF_INVD = G_OFF_META + 2 * NEB * 16, G_OFF_BAR = G_OFF_INVD + 2 * NEB * 4, GROUP_BYTES = G_OFF_BAR + 128;
+constexpr int bwd_smem_bytes(int nch) { return nch * A_CHUNK_BYTES + 2 * GROUP_BYTES + 128; }
+
+struct BwdParams {
+    long long N;
+    const int* row_ptr;
+    const float4* ej;
+    const float4* Gb;      // gather rows (sb', vb'_x, vb'_y, vb'_z)
+    const float* phi;
+    const float* v_in;
+    const float* v1b;
+    const uint4* A_img;
+    float* phib;
+    float* vb_out;
+    float4* G;
+    float inv_rc;
+    int K;
+    int atoms_per_unit;
+    int first;
+};
+
+// L0: layer 0 -- v_in = 0 and the embedding is constant, so only the geometry gradient G is produced
+// (chunks s and vs of the filter; no phib / vb_out).
+template <bool L0>
+__global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
+    constexpr int NCH = L0 ? 2 : 3;
+    constexpr int TCOLS = NCH * 2 * NEB;            // TMEM columns per accumulator buffer
+    extern __shared__ __align__(128) uint8_t smem[];
+    uint8_t* sA = smem;
+    const int tid = threadIdx.x, grp = tid >> 8, ltid = tid & 255, lwarp = ltid >> 5, lane = tid & 31;
+    uint8_t* gbase = smem + NCH * A_CHUNK_BYTES + grp * GROUP_BYTES;
+    uint8_t* sB = gbase + G_OFF_B;
+    float4* sP = (float4*)(gbase + G_OFF_P);       // [2][8][F]
+    float4* sMeta = (float4*)(gbase + G_OFF_META); // [2][NEB] (u of edge (i <- j), i)
+    float* sInvd = (float*)(gbase + G_OFF_INVD);   // [2][NEB]
+    uint64_t* bars = (uint64_t*)(gbase + G_OFF_BAR);
+    uint64_t* b_full = bars;          // [2] producers -> MMA, consumers (count 48)
+    uint64_t* t_full = bars + 2;      // [2] MMA commit -> consumers (count 1)
+    uint64_t* t_empty = bars + 4;     // [2] consumers -> producers (count 4)
+    uint32_t* tmem_slot = (uint32_t*)(smem + NCH * A_CHUNK_BYTES + 2 * GROUP_BYTES);
+
+    {
+        const uint4* src = p.A_img;
+        uint4* dst = (uint4*)sA;
+        for (int i = tid; i < NCH * A_CHUNK_BYTES / 16; i += BWD_THREADS) dst[i] = src[i];
+        uint4* zb = (uint4*)sB;
+        for (int i = ltid; i < 2 * BB_BYTES / 16; i += 256) zb[i] = make_uint4(0, 0, 0, 0);
+    }
+    if (ltid == 0) {
+        for (int b = 0; b < 2; b++) { mbar_init(&b_full[b], 48); mbar_init(&t_full[b], 1); mbar_init(&t_empty[b], 4); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (tid >> 5 == 15) tmem_alloc(tmem_slot, 512);
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot + grp * 256;
+    const long long N = p.N;
+    const int apu = p.atoms_per_unit;
+    const int* __restrict__ row_ptr = p.row_ptr;
+    const long long n_units = (N + apu - 1) / apu;
+    const long long u0 = (long long)blockIdx.x * 2 + grp, ustride = (long long)gridDim.x * 2;
+    if (lwarp < 4) reg_inc<168>(); else reg_dec<88>();
+
+    if (lwarp < 4) {
+        // ===================== consumers: one channel per thread =====================
+        const int f = ltid;
+        const float4* __restrict__ Gb = p.Gb + f;
+        const float* __restrict__ phi = p.phi + f;
+        const float* __restrict__ v_in = p.v_in + f;
+        const float* __restrict__ v1b = p.v1b + f;
+        float* __restrict__ phib = p.phib + f;
+        float* __restrict__ vb_out = p.vb_out + f;
+        float4* __restrict__ Gout = p.G;
+        const bool first = p.first != 0;
+        const uint32_t lane_base = tmem_base + ((uint32_t)(lwarp * 32) << 16);
+        const int red_e = ltid >> 4, red_sub = ltid & 15;          // reduction role: edge of the batch, 1/16 of the channels
+        float4 ga[8], gb[8];
+#define BWD_ISSUE(GR, META8)                                                                   \
+    {                                                                                          \
+        _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++)                                       \
+            GR[i_] = __ldg(Gb + (size_t)__float_as_int((META8)[i_].w) * F);                    \
+    }
+        uint32_t it = 0, pb = 0;
+        bool pre = false;
+        for (long long u = u0; u < n_units; u += ustride) {
+            const long long a0 = u * apu;
+            const int na = (int)min((long long)apu, N - a0);
+            const int rp = __ldg(row_ptr + a0 + min(lane, na));
+            const int e_begin = __shfl_sync(0xffffffffu, rp, 0), e_end = __shfl_sync(0xffffffffu, rp, na);
+            const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
+            bool next_has = false;
+            {
+                const long long un = u + ustride;
+                if (un < n_units) {
+                    const long long b0 = un * apu, b1 = min(N, b0 + apu);
+                    next_has = __ldg(row_ptr + b1) > __ldg(row_ptr + b0);
+                }
+            }
+            if (ntiles > 0 && !pre) {
+                mbar_wait(&b_full[it & 1], (it >> 1) & 1);
+                const float4* m0 = sMeta + (it & 1) * NEB;
+                BWD_ISSUE(ga, m0);
+            }
+            pre = false;
+            int j_rel = 0;
+            int row_end = __shfl_sync(0xffffffffu, rp, 1);
+            // own rows of sender j (current) and j + 1 (prefetched)
+            float phS, phVS, phVV = 0.f, vj0 = 0.f, vj1 = 0.f, vj2 = 0.f, r0 = 0.f, r1 = 0.f, r2 = 0.f;
+            float nphS = 0.f, nphVS = 0.f, nphVV = 0.f, nvj0 = 0.f, nvj1 = 0.f, nvj2 = 0.f, nr0 = 0.f, nr1 = 0.f, nr2 = 0.f;
+            float pbS = 0.f, pbVS = 0.f, Y0 = 0.f, Y1 = 0.f, Y2 = 0.f;
+            auto load_own = [&](long long j, float& a, float& b, float& c, float& x, float& y, float& z, float& q0, float& q1, float& q2) {
+                a = phi[j * 3 * F]; b = phi[j * 3 * F + F];
+                if (!L0) {
+                    c = phi[j * 3 * F + 2 * F];
+                    x = v_in[j * 3 * F]; y = v_in[j * 3 * F + F]; z = v_in[j * 3 * F + 2 * F];
+                    q0 = v1b[j * 3 * F]; q1 = v1b[j * 3 * F + F]; q2 = v1b[j * 3 * F + 2 * F];
+                }
+            };
+            load_own(a0, phS, phVS, phVV, vj0, vj1, vj2, r0, r1, r2);
+            if (na > 1) load_own(a0 + 1, nphS, nphVS, nphVV, nvj0, nvj1, nvj2, nr0, nr1, nr2);
+            auto store_row = [&]() {
+                if (L0) return;
+                const long long j = a0 + j_rel;
+                phib[j * 3 * F] = pbS;
+                phib[j * 3 * F + F] = pbVS;
+                phib[j * 3 * F + 2 * F] = vj0 * Y0 + vj1 * Y1 + vj2 * Y2;
+                vb_out[j * 3 * F] = r0 + phVV * Y0;
+                vb_out[j * 3 * F + F] = r1 + phVV * Y1;
+                vb_out[j * 3 * F + 2 * F] = r2 + phVV * Y2;
+            };
+            auto next_row = [&]() {
+                store_row();
+                j_rel++;
+                row_end = __shfl_sync(0xffffffffu, rp, j_rel + 1);
+                phS = nphS; phVS = nphVS; phVV = nphVV; vj0 = nvj0; vj1 = nvj1; vj2 = nvj2; r0 = nr0; r1 = nr1; r2 = nr2;
+                pbS = pbVS = Y0 = Y1 = Y2 = 0.f;
+                if (j_rel + 1 < na) load_own(a0 + j_rel + 1, nphS, nphVS, nphVV, nvj0, nvj1, nvj2, nr0, nr1, nr2);
+            };
+#define BWD_COMPUTE(H, GR)                                                                                        \
+    {                                                                                                             \
+        const int E8_ = e_begin + t * NEB + (H) * 8;                                                              \
+        if (E8_ < e_end) {                                                                                        \
+            while (E8_ >= row_end) next_row();                                                                    \
+            /* the lanes that finish edge red_e of this batch fetch its running G early */                        \
+            const int Er_ = E8_ + red_e;                                                                          \
+            float4 gold_ = make_float4(0.f, 0.f, 0.f, 0.f);                                                       \
+            if (red_sub == 0 && !first && Er_ < e_end) gold_ = Gout[Er_];                                         \
+            uint32_t wS_[8], wVS_[8], wVV_[8], dS_[8], dVS_[8], dVV_[8];                                          \
+            tmem_ld8_nowait(lane_base + buf * TCOLS + (H) * 8, wS_);                                              \
+            tmem_ld8_nowait(lane_base + buf * TCOLS + NEB + (H) * 8, dS_);                                        \
+            tmem_ld8_nowait(lane_base + buf * TCOLS + 2 * NEB + (H) * 8, wVS_);                                   \
+            tmem_ld8_nowait(lane_base + buf * TCOLS + 3 * NEB + (H) * 8, dVS_);                                   \
+            if (!L0) {                                                                                            \
+                tmem_ld8_nowait(lane_base + buf * TCOLS + 4 * NEB + (H) * 8, wVV_);                               \
+                tmem_ld8_nowait(lane_base + buf * TCOLS + 5 * NEB + (H) * 8, dVV_);                               \
+            }                                                                                                     \
+            tmem_wait_ld();                                                                                       \
+            float4* pdst_ = sP + pb * 8 * F + f;                                                                  \
+            _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                                    \
+                const float4 m_ = meta[(H) * 8 + i_];                                                             \
+                const float sb_ = GR[i_].x, vb0_ = GR[i_].y, vb1_ = GR[i_].z, vb2_ = GR[i_].w;                    \
+                const float X_ = fmaf(vb0_, m_.x, fmaf(vb1_, m_.y, vb2_ * m_.z));                                 \
+                const float wVSf_ = __uint_as_float(wVS_[i_]);                                                    \
+                float db_ = phS * (sb_ * __uint_as_float(dS_[i_]));                                               \
+                db_ = fmaf(phVS, X_ * __uint_as_float(dVS_[i_]), db_);                                            \
+                if (!L0) {                                                                                        \
+                    const float wVVf_ = __uint_as_float(wVV_[i_]);                                                \
+                    const float Z_ = fmaf(vb0_, vj0, fmaf(vb1_, vj1, vb2_ * vj2));                                \
+                    db_ = fmaf(phVV, Z_ * __uint_as_float(dVV_[i_]), db_);                                        \
+                    pbS = fmaf(__uint_as_float(wS_[i_]), sb_, pbS);                                               \
+                    pbVS = fmaf(wVSf_, X_, pbVS);                                                                 \
+                    Y0 = fmaf(wVVf_, vb0_, Y0); Y1 = fmaf(wVVf_, vb1_, Y1); Y2 = fmaf(wVVf_, vb2_, Y2);           \
+                }                                                                                                 \
+                const float tt_ = wVSf_ * phVS;                                                                   \
+                pdst_[i_ * F] = make_float4(db_, tt_ * vb0_, tt_ * vb1_, tt_ * vb2_);                             \
+            }                                                                                                     \
+            asm volatile("bar.sync %0, 128;" ::"r"(1 + grp) : "memory");                                          \
+            /* sum over the 128 channels: this thread adds 8 of them for edge red_e, then a 16-lane tree */       \
+            const float4* psrc_ = sP + pb * 8 * F + red_e * F + red_sub;                                          \
+            float4 acc_ = psrc_[0];                                                                               \
+            _Pragma("unroll") for (int k_ = 1; k_ < 8; k_++) {                                                    \
+                const float4 x_ = psrc_[16 * k_];                                                                 \
+                acc_.x += x_.x; acc_.y += x_.y; acc_.z += x_.z; acc_.w += x_.w;                                   \
+            }                                                                                                     \
+            _Pragma("unroll") for (int o_ = 8; o_ >= 1; o_ >>= 1) {                                               \
+                acc_.x += __shfl_xor_sync(0xffffffffu, acc_.x, o_); acc_.y += __shfl_xor_sync(0xffffffffu, acc_.y, o_); \
+                acc_.z += __shfl_xor_sync(0xffffffffu, acc_.z, o_); acc_.w += __shfl_xor_sync(0xffffffffu, acc_.w, o_); \
+            }                                                                                                     \
+            if (red_sub == 0 && Er_ < e_end) {                                                                    \
+                const float4 mm_ = meta[(H) * 8 + red_e];                                                         \
+                const float invd_ = invd[(H) * 8 + red_e];                                                        \
+                const float uu_ = acc_.y * mm_.x + acc_.z * mm_.y + acc_.w * mm_.z;                               \
+                Gout[Er_] = make_float4(gold_.x + acc_.x * mm_.x + (acc_.y - uu_ * mm_.x) * invd_,                \
+                                        gold_.y + acc_.x * mm_.y + (acc_.z - uu_ * mm_.y) * invd_,                \
+                                        gold_.z + acc_.x * mm_.z + (acc_.w - uu_ * mm_.z) * invd_, 0.f);          \
+            }                                                                                                     \
+            pb ^= 1;                                                                                              \
+        }                                                                                                         \
+    }
+            for (int t = 0; t < ntiles; t++, it++) {
+                const int buf = it & 1;
+                const float4* meta = sMeta + buf * NEB;
+                const float* invd = sInvd + buf * NEB;
+                BWD_ISSUE(gb, meta + 8);
+                mbar_wait(&t_full[buf], (it >> 1) & 1);
+                tc_fence_after();
+                BWD_COMPUTE(0, ga);
+                if (t + 1 < ntiles || next_has) {
+                    mbar_wait(&b_full[buf ^ 1], ((it + 1) >> 1) & 1);
+                    const float4* mn = sMeta + (buf ^ 1) * NEB;
+                    BWD_ISSUE(ga, mn);
+                    pre = t + 1 == ntiles;
+                }
+                BWD_COMPUTE(1, gb);
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&t_empty[buf]);
+            }
+            for (;;) {
+                store_row();
+                if (j_rel + 1 >= na) break;
+                // trailing edge-less senders: phib = 0, vb_out = v1b
+                j_rel++;
+                phS = nphS; phVS = nphVS; phVV = nphVV; vj0 = nvj0; vj1 = nvj1; vj2 = nvj2; r0 = nr0; r1 = nr1; r2 = nr2;
+                pbS = pbVS = Y0 = Y1 = Y2 = 0.f;
+                if (j_rel + 1 < na) load_own(a0 + j_rel + 1, nphS, nphVS, nphVV, nvj0, nvj1, nvj2, nr0, nr1, nr2);
+            }
+        }
+#undef BWD_ISSUE
+#undef BWD_COMPUTE
+    } else if (lwarp < 6) {
+        // ===================== producers: rows 0..15 R_e, rows 16..31 R'_e =====================
+        const int pt = ltid - 128, e = pt & 15, h = pt >> 4;   // h = 0..3 (h == 3 idle)
+        const float inv_rc = p.inv_rc;
+        const float a1c = 3.14159265358979323846f * inv_rc;
+        const int K = p.K;
+        uint32_t it = 0;
+        if (h < 3)
+        for (long long u = u0; u < n_units; u += ustride) {
+            const long long a0 = u * apu;
+            const long long a1 = min(N, a0 + (long long)apu);
+            const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
+            const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
+            for (int t = 0; t < ntiles; t++, it++) {
+                const int buf = it & 1;
+                const EdgeGeom g = load_edge(p.ej, e_begin + t * NEB + e, e_end, inv_rc);
+                const float fc = g.real ? 0.5f * (1.0f + g.c1) : 0.0f;
+                const float dfc = g.real ? -0.5f * a1c * g.s1 : 0.0f;
+                float sn_, cn_;
+                if (h == 0) { sn_ = g.s1; cn_ = g.c1; } else sincospif((float)(8 * h) * g.x, &sn_, &cn_);
+                float vals[8], dvals[8];
+#pragma unroll
+                for (int i = 0; i < 8; i++) {
+                    const int b = h * 8 + i;
+                    if (b == 0) { vals[i] = fc; dvals[i] = dfc; }
+                    else {
+                        const float rho = sn_ * g.inv_d;
+                        const float drho = ((float)b * a1c * cn_ - rho) * g.inv_d;
+                        vals[i] = b <= K ? fc * rho : 0.0f;
+                        dvals[i] = b <= K ? dfc * rho + fc * drho : 0.0f;
+                        const float tt = sn_ * g.c1 + cn_ * g.s1;
+                        cn_ = cn_ * g.c1 - sn_ * g.s1;
+                        sn_ = tt;
+                    }
+                }
+                uint4 q[6];
+                split3(vals, q[0], q[1], q[2]);
+                split3(dvals, q[3], q[4], q[5]);
+                mbar_wait(&t_empty[buf], ((it >> 1) & 1) ^ 1);
+#pragma unroll
+                for (int z = 0; z < 2; z++) {
+                    const int row = z * NEB + e;
+                    uint8_t* bb = sB + buf * BB_BYTES + (row >> 3) * SBO + (row & 7) * 16 + h * LBO;
+                    *(uint4*)(bb) = q[3 * z + 0];
+                    *(uint4*)(bb + 4 * LBO) = q[3 * z + 1];
+                    *(uint4*)(bb + 8 * LBO) = q[3 * z + 2];
+                }
+                if (h == 0) {
+                    sMeta[buf * NEB + e] = make_float4(-g.r.x * g.inv_d, -g.r.y * g.inv_d, -g.r.z * g.inv_d, g.r.w);   // u_e of edge (i <- j)
+                    sInvd[buf * NEB + e] = g.inv_d;
+                }
+                fence_async_smem();
+                mbar_arrive(&b_full[buf]);
+            }
+        }
+    } else if (lwarp == 7) {
+        // ===================== MMA issuer =====================
+        if (lane == 0) {
+            const uint32_t idesc = (1u << 4) | ((uint32_t)((2 * NEB) >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+            const uint32_t a_base = smem_u32(sA), b_base = smem_u32(sB);
+            uint32_t it = 0;
+            for (long long u = u0; u < n_units; u += ustride) {
+                const long long a0 = u * apu;
+                const long long a1 = min(N, a0 + (long long)apu);
+                const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
+                const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
+                for (int t = 0; t < ntiles; t++, it++) {
+                    const int buf = it & 1;
+                    mbar_wait(&b_full[buf], (it >> 1) & 1);
+                    tc_fence_after();
+#pragma unroll
+                    for (int c = 0; c < NCH; c++) {
+                        const uint32_t d = tmem_base + buf * TCOLS + c * 2 * NEB;
+#pragma unroll
+                        for (int o = 0; o < 6; o++) {
+                            const int kk = (o + 2) % 6;
+                            const uint64_t ad = make_desc_nosw(a_base + c * A_CHUNK_BYTES + kk * 2 * LBO, LBO, SBO);
+                            const uint64_t bd = make_desc_nosw(b_base + buf * BB_BYTES + kk * 2 * LBO, LBO, SBO);
+                            umma_f16(d, ad, bd, idesc, o != 0);
+                        }
+                    }
+                    umma_commit(&t_full[buf]);
+                }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (tid >> 5 == 15) tmem_dealloc(*tmem_slot, 512);
+}
+
+}  // namespace ev3
+
+static int sm_count() {
+    static int n_sm = 0;
+    if (!n_sm) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    }
+    return n_sm;
+}
+
+// F = 128, K <= 23 only.  Q4/Q1 from make_gather_rows (layer 0: Q4 holds float2 rows); A_img from edge_build_filter_image.
+bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* s,
+                    const float* v, const float* Q4, const float* Q1, const void* A_img, float* sn, float* v1, bool has_v) {
+    using namespace ev3;
+    if (N == 0) return true;
+    if (K > 23) return false;
+    static bool attr = false;
+    if (!attr) {
+        if (cudaFuncSetAttribute(k_msg_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fwd_smem_bytes(true)) != cudaSuccess ||
+            cudaFuncSetAttribute(k_msg_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fwd_smem_bytes(false)) != cudaSuccess)
+            return false;
+        attr = true;
+    }
+    FwdParams p{N, row_ptr, ej, s, v, (const float4*)Q4, Q1, (const float2*)Q4, (const uint4*)A_img, sn, v1, 1.0f / rc, K, 16};
+    const long long n_units = (N + p.atoms_per_unit - 1) / p.atoms_per_unit;
+    const int grid = (int)std::min<long long>(n_units, 2LL * sm_count());
+    if (has_v) k_msg_fwd<true><<<grid, FWD_THREADS, fwd_smem_bytes(true), L.stream>>>(p);
+    else k_msg_fwd<false><<<grid, FWD_THREADS, fwd_smem_bytes(false), L.stream>>>(p);
+    KLAUNCH(L);
+    return true;
+}
+
+// layer0: v_in = 0 and no sender adjoint wanted (phib / vb_out untouched)
+bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
+                    const float* phi, const float* v_in, const float* v1b, const void* A_img, float* phib, float* vb_out,
+                    float4* G, bool first, bool layer0) {
+    using namespace ev3;
+    if (N == 0) return true;
+    if (K > 23) return false;
+    static bool attr = false;
+    if (!attr) {
+        if (cudaFuncSetAttribute(k_msg_bwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bwd_smem_bytes(2)) != cudaSuccess ||
+            cudaFuncSetAttribute(k_msg_bwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bwd_smem_bytes(3)) != cudaSuccess)
+            return false;
+        attr = true;
+    }
+    BwdParams p{N, row_ptr, ej, (const float4*)Gb, phi, v_in, v1b, (const uint4*)A_img, phib, vb_out, G, 1.0f / rc, K, 16,
+                first ? 1 : 0};
+    const long long n_units = (N + p.atoms_per_unit - 1) / p.atoms_per_unit;
+    const int grid = (int)std::min<long long>((n_units + 1) / 2, (long long)sm_count());
+    if (layer0) k_msg_bwd<true><<<grid, BWD_THREADS, bwd_smem_bytes(2), L.stream>>>(p);
+    else k_msg_bwd<false><<<grid, BWD_THREADS, bwd_smem_bytes(3), L.stream>>>(p);
+    KLAUNCH(L);
+    return true;
+}
+
+}  // namespace painn
