@@ -301,7 +301,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
                 }
                 uint4 p0, p1, p2;
                 split3(vals, p0, p1, p2);
-                mbar_wait(&t_empty[buf], ((it >> 1) & 1) ^ 1);
+                mbar_wait_sleep(&t_empty[buf], ((it >> 1) & 1) ^ 1, 256);
                 uint8_t* bb = sB + buf * B_BYTES + (e >> 3) * SBO + (e & 7) * 16 + h * LBO;
                 *(uint4*)(bb) = p0;                       // term 0: k = b
                 *(uint4*)(bb + 4 * LBO) = p1;             // term 1: k = 32 + b   (lo(R) 2^11)
@@ -324,7 +324,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
                 const int ntiles = (e_end - e_begin + NE - 1) / NE;
                 for (int t = 0; t < ntiles; t++, it++) {
                     const int buf = it & 1;
-                    mbar_wait(&b_full[buf], (it >> 1) & 1);
+                    mbar_wait_sleep(&b_full[buf], (it >> 1) & 1, 128);
                     tc_fence_after();
 #pragma unroll
                     for (int c = 0; c < NCH; c++) {
@@ -355,7 +355,8 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
 constexpr int NEB = 16;                                 // edges per tile; B rows 0..15 = R_e, 16..31 = R'_e
 constexpr int BB_BYTES = (2 * NEB / 8) * SBO;           // 6144
 constexpr int BWD_THREADS = 512;
-constexpr int P_BYTES = 8 * F * 16;                     // per-edge partials of one 8-edge batch: [8][128] float4
+constexpr int P_ROW = F * 16 + 64;                      // per-edge partials [128] float4, padded: conflict-free transposed reads
+constexpr int P_BYTES = 8 * P_ROW;                      // one 8-edge batch
 constexpr int G_OFF_B = 0, G_OFF_P = 2 * BB_BYTES, G_OFF_META = G_OFF_P + 2 * P_BYTES,
               G_OFF_INVD = G_OFF_META + 2 * NEB * 16, G_OFF_BAR = G_OFF_INVD + 2 * NEB * 4, GROUP_BYTES = G_OFF_BAR + 128;
 constexpr int bwd_smem_bytes(int nch) { return nch * A_CHUNK_BYTES + 2 * GROUP_BYTES + 128; }
@@ -389,13 +390,15 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
     const int tid = threadIdx.x, grp = tid >> 8, ltid = tid & 255, lwarp = ltid >> 5, lane = tid & 31;
     uint8_t* gbase = smem + NCH * A_CHUNK_BYTES + grp * GROUP_BYTES;
     uint8_t* sB = gbase + G_OFF_B;
-    float4* sP = (float4*)(gbase + G_OFF_P);       // [2][8][F]
+    uint8_t* sP = gbase + G_OFF_P;                 // [2][8] rows of P_ROW bytes: (db, ub_x, ub_y, ub_z) per channel
     float4* sMeta = (float4*)(gbase + G_OFF_META); // [2][NEB] (u of edge (i <- j), i)
     float* sInvd = (float*)(gbase + G_OFF_INVD);   // [2][NEB]
     uint64_t* bars = (uint64_t*)(gbase + G_OFF_BAR);
     uint64_t* b_full = bars;          // [2] producers -> MMA, consumers (count 48)
     uint64_t* t_full = bars + 2;      // [2] MMA commit -> consumers (count 1)
-    uint64_t* t_empty = bars + 4;     // [2] consumers -> producers (count 4)
+    uint64_t* t_empty = bars + 4;     // [2] consumers (4) + reducer (1) -> producers
+    uint64_t* p_full = bars + 6;      // [2] consumers -> reducer: partials of one 8-edge batch written (count 4)
+    uint64_t* p_empty = bars + 8;     // [2] reducer -> consumers (count 1)
     uint32_t* tmem_slot = (uint32_t*)(smem + NCH * A_CHUNK_BYTES + 2 * GROUP_BYTES);
 
     {
@@ -406,7 +409,10 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
         for (int i = ltid; i < 2 * BB_BYTES / 16; i += 256) zb[i] = make_uint4(0, 0, 0, 0);
     }
     if (ltid == 0) {
-        for (int b = 0; b < 2; b++) { mbar_init(&b_full[b], 48); mbar_init(&t_full[b], 1); mbar_init(&t_empty[b], 4); }
+        for (int b = 0; b < 2; b++) {
+            mbar_init(&b_full[b], 48); mbar_init(&t_full[b], 1); mbar_init(&t_empty[b], 5);
+            mbar_init(&p_full[b], 4); mbar_init(&p_empty[b], 1);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (tid >> 5 == 15) tmem_alloc(tmem_slot, 512);
@@ -434,14 +440,13 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
         float4* __restrict__ Gout = p.G;
         const bool first = p.first != 0;
         const uint32_t lane_base = tmem_base + ((uint32_t)(lwarp * 32) << 16);
-        const int red_e = ltid >> 4, red_sub = ltid & 15;          // reduction role: edge of the batch, 1/16 of the channels
         float4 ga[8], gb[8];
 #define BWD_ISSUE(GR, META8)                                                                   \
     {                                                                                          \
         _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++)                                       \
             GR[i_] = __ldg(Gb + (size_t)__float_as_int((META8)[i_].w) * F);                    \
     }
-        uint32_t it = 0, pb = 0;
+        uint32_t it = 0, hc = 0;          // tile counter, active 8-edge batch counter (selects the partials buffer)
         bool pre = false;
         for (long long u = u0; u < n_units; u += ustride) {
             const long long a0 = u * apu;
@@ -502,10 +507,6 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
         const int E8_ = e_begin + t * NEB + (H) * 8;                                                              \
         if (E8_ < e_end) {                                                                                        \
             while (E8_ >= row_end) next_row();                                                                    \
-            /* the lanes that finish edge red_e of this batch fetch its running G early */                        \
-            const int Er_ = E8_ + red_e;                                                                          \
-            float4 gold_ = make_float4(0.f, 0.f, 0.f, 0.f);                                                       \
-            if (red_sub == 0 && !first && Er_ < e_end) gold_ = Gout[Er_];                                         \
             uint32_t wS_[8], wVS_[8], wVV_[8], dS_[8], dVS_[8], dVV_[8];                                          \
             tmem_ld8_nowait(lane_base + buf * TCOLS + (H) * 8, wS_);                                              \
             tmem_ld8_nowait(lane_base + buf * TCOLS + NEB + (H) * 8, dS_);                                        \
@@ -515,8 +516,9 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                 tmem_ld8_nowait(lane_base + buf * TCOLS + 4 * NEB + (H) * 8, wVV_);                               \
                 tmem_ld8_nowait(lane_base + buf * TCOLS + 5 * NEB + (H) * 8, dVV_);                               \
             }                                                                                                     \
+            mbar_wait(&p_empty[hc & 1], ((hc >> 1) & 1) ^ 1);           /* partials buffer free again */          \
             tmem_wait_ld();                                                                                       \
-            float4* pdst_ = sP + pb * 8 * F + f;                                                                  \
+            uint8_t* pdst_ = sP + (hc & 1) * P_BYTES + f * 16;                                                    \
             _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                                    \
                 const float4 m_ = meta[(H) * 8 + i_];                                                             \
                 const float sb_ = GR[i_].x, vb0_ = GR[i_].y, vb1_ = GR[i_].z, vb2_ = GR[i_].w;                    \
@@ -533,35 +535,16 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                     Y0 = fmaf(wVVf_, vb0_, Y0); Y1 = fmaf(wVVf_, vb1_, Y1); Y2 = fmaf(wVVf_, vb2_, Y2);           \
                 }                                                                                                 \
                 const float tt_ = wVSf_ * phVS;                                                                   \
-                pdst_[i_ * F] = make_float4(db_, tt_ * vb0_, tt_ * vb1_, tt_ * vb2_);                             \
+                *(float4*)(pdst_ + i_ * P_ROW) = make_float4(db_, tt_ * vb0_, tt_ * vb1_, tt_ * vb2_);            \
             }                                                                                                     \
-            asm volatile("bar.sync %0, 128;" ::"r"(1 + grp) : "memory");                                          \
-            /* sum over the 128 channels: this thread adds 8 of them for edge red_e, then a 16-lane tree */       \
-            const float4* psrc_ = sP + pb * 8 * F + red_e * F + red_sub;                                          \
-            float4 acc_ = psrc_[0];                                                                               \
-            _Pragma("unroll") for (int k_ = 1; k_ < 8; k_++) {                                                    \
-                const float4 x_ = psrc_[16 * k_];                                                                 \
-                acc_.x += x_.x; acc_.y += x_.y; acc_.z += x_.z; acc_.w += x_.w;                                   \
-            }                                                                                                     \
-            _Pragma("unroll") for (int o_ = 8; o_ >= 1; o_ >>= 1) {                                               \
-                acc_.x += __shfl_xor_sync(0xffffffffu, acc_.x, o_); acc_.y += __shfl_xor_sync(0xffffffffu, acc_.y, o_); \
-                acc_.z += __shfl_xor_sync(0xffffffffu, acc_.z, o_); acc_.w += __shfl_xor_sync(0xffffffffu, acc_.w, o_); \
-            }                                                                                                     \
-            if (red_sub == 0 && Er_ < e_end) {                                                                    \
-                const float4 mm_ = meta[(H) * 8 + red_e];                                                         \
-                const float invd_ = invd[(H) * 8 + red_e];                                                        \
-                const float uu_ = acc_.y * mm_.x + acc_.z * mm_.y + acc_.w * mm_.z;                               \
-                Gout[Er_] = make_float4(gold_.x + acc_.x * mm_.x + (acc_.y - uu_ * mm_.x) * invd_,                \
-                                        gold_.y + acc_.x * mm_.y + (acc_.z - uu_ * mm_.y) * invd_,                \
-                                        gold_.z + acc_.x * mm_.z + (acc_.w - uu_ * mm_.z) * invd_, 0.f);          \
-            }                                                                                                     \
-            pb ^= 1;                                                                                              \
+            __syncwarp();                                                                                         \
+            if (lane == 0) mbar_arrive(&p_full[hc & 1]);                /* hand the batch to the reducer warp */  \
+            hc++;                                                                                                 \
         }                                                                                                         \
     }
             for (int t = 0; t < ntiles; t++, it++) {
                 const int buf = it & 1;
                 const float4* meta = sMeta + buf * NEB;
-                const float* invd = sInvd + buf * NEB;
                 BWD_ISSUE(gb, meta + 8);
                 mbar_wait(&t_full[buf], (it >> 1) & 1);
                 tc_fence_after();
@@ -627,7 +610,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                 uint4 q[6];
                 split3(vals, q[0], q[1], q[2]);
                 split3(dvals, q[3], q[4], q[5]);
-                mbar_wait(&t_empty[buf], ((it >> 1) & 1) ^ 1);
+                mbar_wait_sleep(&t_empty[buf], ((it >> 1) & 1) ^ 1, 256);
 #pragma unroll
                 for (int z = 0; z < 2; z++) {
                     const int row = z * NEB + e;
@@ -644,6 +627,55 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                 mbar_arrive(&b_full[buf]);
             }
         }
+    } else if (lwarp == 6) {
+        // ===================== reducer: sum the partials over the 128 channels, assemble g_e, accumulate G =====================
+        // lane = (edge of the batch, quarter of the channels): 32 conflict-free LDS.128 + two shuffle stages per batch
+        const int re = lane >> 2, rsub = lane & 3;
+        float4* __restrict__ Gout = p.G;
+        const bool first = p.first != 0;
+        uint32_t it = 0, hc = 0;
+        for (long long u = u0; u < n_units; u += ustride) {
+            const long long a0 = u * apu;
+            const long long a1 = min(N, a0 + (long long)apu);
+            const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
+            const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
+            for (int t = 0; t < ntiles; t++, it++) {
+                const int buf = it & 1;
+                for (int h = 0; h < 2; h++) {
+                    const int E8 = e_begin + t * NEB + h * 8;
+                    if (E8 >= e_end) continue;
+                    const int E = E8 + re;
+                    float4 gold = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (rsub == 0 && !first) gold = Gout[E];                  // running sum over layers, fetched early
+                    mbar_wait(&p_full[hc & 1], (hc >> 1) & 1);
+                    const uint8_t* src = sP + (hc & 1) * P_BYTES + re * P_ROW + rsub * 16;
+                    float4 acc = *(const float4*)src;
+#pragma unroll
+                    for (int k = 1; k < 32; k++) {
+                        const float4 x = *(const float4*)(src + k * 64);
+                        acc.x += x.x; acc.y += x.y; acc.z += x.z; acc.w += x.w;
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&p_empty[hc & 1]);
+                    hc++;
+#pragma unroll
+                    for (int o = 2; o >= 1; o >>= 1) {
+                        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
+                        acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o); acc.w += __shfl_xor_sync(0xffffffffu, acc.w, o);
+                    }
+                    if (rsub == 0) {
+                        const float4 mm = sMeta[buf * NEB + h * 8 + re];
+                        const float inv_d = sInvd[buf * NEB + h * 8 + re];
+                        const float uu = acc.y * mm.x + acc.z * mm.y + acc.w * mm.z;
+                        Gout[E] = make_float4(gold.x + acc.x * mm.x + (acc.y - uu * mm.x) * inv_d,
+                                              gold.y + acc.x * mm.y + (acc.z - uu * mm.y) * inv_d,
+                                              gold.z + acc.x * mm.z + (acc.w - uu * mm.z) * inv_d, 0.f);
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&t_empty[buf]);
+            }
+        }
     } else if (lwarp == 7) {
         // ===================== MMA issuer =====================
         if (lane == 0) {
@@ -657,7 +689,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                 const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
                 for (int t = 0; t < ntiles; t++, it++) {
                     const int buf = it & 1;
-                    mbar_wait(&b_full[buf], (it >> 1) & 1);
+                    mbar_wait_sleep(&b_full[buf], (it >> 1) & 1, 128);
                     tc_fence_after();
 #pragma unroll
                     for (int c = 0; c < NCH; c++) {
