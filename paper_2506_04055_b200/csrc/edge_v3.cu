@@ -355,10 +355,13 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
 constexpr int NEB = 16;                                 // edges per tile; B rows 0..15 = R_e, 16..31 = R'_e
 constexpr int BB_BYTES = (2 * NEB / 8) * SBO;           // 6144
 constexpr int BWD_THREADS = 512;
-constexpr int P_ROW = F * 16 + 64;                      // per-edge partials [128] float4, padded: conflict-free transposed reads
+constexpr int P_ROW = F * 16;                           // per-edge partials [128] float4; 16-byte chunk c of row e is stored at
+                                                        // chunk c ^ ((e & 1) << 2): conflict-free transposed reads
 constexpr int P_BYTES = 8 * P_ROW;                      // one 8-edge batch
-constexpr int G_OFF_B = 0, G_OFF_P = 2 * BB_BYTES, G_OFF_META = G_OFF_P + 2 * P_BYTES,
-              G_OFF_INVD = G_OFF_META + 2 * NEB * 16, G_OFF_BAR = G_OFF_INVD + 2 * NEB * 4, GROUP_BYTES = G_OFF_BAR + 128;
+constexpr int GW = 16;                                  // gather window (edges in flight per thread)
+constexpr int RING_BYTES = GW * F * 16;                 // 32768
+constexpr int G_OFF_B = 0, G_OFF_P = 2 * BB_BYTES, G_OFF_RING = G_OFF_P + 2 * P_BYTES, G_OFF_META = G_OFF_RING + RING_BYTES,
+              G_OFF_INVD = G_OFF_META + 4 * NEB * 16, G_OFF_BAR = G_OFF_INVD + 4 * NEB * 4, GROUP_BYTES = G_OFF_BAR + 128;
 constexpr int bwd_smem_bytes(int nch) { return nch * A_CHUNK_BYTES + 2 * GROUP_BYTES + 128; }
 
 struct BwdParams {
@@ -391,14 +394,15 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
     uint8_t* gbase = smem + NCH * A_CHUNK_BYTES + grp * GROUP_BYTES;
     uint8_t* sB = gbase + G_OFF_B;
     uint8_t* sP = gbase + G_OFF_P;                 // [2][8] rows of P_ROW bytes: (db, ub_x, ub_y, ub_z) per channel
-    float4* sMeta = (float4*)(gbase + G_OFF_META); // [2][NEB] (u of edge (i <- j), i)
-    float* sInvd = (float*)(gbase + G_OFF_INVD);   // [2][NEB]
+    float4* sMeta = (float4*)(gbase + G_OFF_META); // [4][NEB] (u of edge (i <- j), i): ring of 4 tiles (the reducer lags)
+    float* sInvd = (float*)(gbase + G_OFF_INVD);   // [4][NEB]
     uint64_t* bars = (uint64_t*)(gbase + G_OFF_BAR);
-    uint64_t* b_full = bars;          // [2] producers -> MMA, consumers (count 48)
-    uint64_t* t_full = bars + 2;      // [2] MMA commit -> consumers (count 1)
-    uint64_t* t_empty = bars + 4;     // [2] consumers (4) + reducer (1) -> producers
-    uint64_t* p_full = bars + 6;      // [2] consumers -> reducer: partials of one 8-edge batch written (count 4)
-    uint64_t* p_empty = bars + 8;     // [2] reducer -> consumers (count 1)
+    uint64_t* t_full = bars;          // [2] MMA commit -> consumers (mbarrier, count 1)
+    uint64_t* p_empty = bars + 2;     // [2] reducer -> consumers: partials buffer read (mbarrier, count 1)
+    // named barriers of this group (hardware-blocking waits): [2] each
+    const int NB_TE = 1 + grp * 6;    // consumers (128, arrive) -> producers (64, sync): tile buffer consumed
+    const int NB_BF = NB_TE + 2;      // producers (64, arrive) -> MMA warp (32, sync): B operand written
+    const int NB_PF = NB_TE + 4;      // consumers (128, arrive) -> reducer (32, sync): partials of one batch written
     uint32_t* tmem_slot = (uint32_t*)(smem + NCH * A_CHUNK_BYTES + 2 * GROUP_BYTES);
 
     {
@@ -409,10 +413,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
         for (int i = ltid; i < 2 * BB_BYTES / 16; i += 256) zb[i] = make_uint4(0, 0, 0, 0);
     }
     if (ltid == 0) {
-        for (int b = 0; b < 2; b++) {
-            mbar_init(&b_full[b], 48); mbar_init(&t_full[b], 1); mbar_init(&t_empty[b], 5);
-            mbar_init(&p_full[b], 4); mbar_init(&p_empty[b], 1);
-        }
+        for (int b = 0; b < 2; b++) { mbar_init(&t_full[b], 1); mbar_init(&p_empty[b], 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (tid >> 5 == 15) tmem_alloc(tmem_slot, 512);
@@ -440,34 +441,35 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
         float4* __restrict__ Gout = p.G;
         const bool first = p.first != 0;
         const uint32_t lane_base = tmem_base + ((uint32_t)(lwarp * 32) << 16);
-        float4 ga[8], gb[8];
-#define BWD_ISSUE(GR, META8)                                                                   \
-    {                                                                                          \
-        _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++)                                       \
-            GR[i_] = __ldg(Gb + (size_t)__float_as_int((META8)[i_].w) * F);                    \
-    }
+        // Rolling gather window: the W = 16 next neighbour rows of this thread's channel are always in flight as
+        // cp.async copies into private 16-byte shared-memory slots (one commit group per edge, wait_group W-1 before
+        // an edge is consumed).  ptxas tracks register-landing loads of different pipeline stages on one scoreboard
+        // (measured: the "ping-pong" LDG banks serialised), cp.async groups complete in order by construction.
+        float4* ring = (float4*)(gbase + G_OFF_RING) + f;             // slot s of this thread: ring[s * F]
+        const float4* __restrict__ ejp = p.ej;
         uint32_t it = 0, hc = 0;          // tile counter, active 8-edge batch counter (selects the partials buffer)
-        bool pre = false;
         for (long long u = u0; u < n_units; u += ustride) {
             const long long a0 = u * apu;
             const int na = (int)min((long long)apu, N - a0);
             const int rp = __ldg(row_ptr + a0 + min(lane, na));
             const int e_begin = __shfl_sync(0xffffffffu, rp, 0), e_end = __shfl_sync(0xffffffffu, rp, na);
-            const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
-            bool next_has = false;
-            {
-                const long long un = u + ustride;
-                if (un < n_units) {
-                    const long long b0 = un * apu, b1 = min(N, b0 + apu);
-                    next_has = __ldg(row_ptr + b1) > __ldg(row_ptr + b0);
+            const int n_e = e_end - e_begin;
+            const int ntiles = (n_e + NEB - 1) / NEB;
+            // sender indices of the unit's edges, 32 per register (lane l <-> edge 32 blk + l); padding slots -> own row
+            auto load_idx = [&](int blk) -> int {
+                const int E = e_begin + 32 * blk + lane;
+                const int ix = E < e_end ? __float_as_int(__ldg(ejp + E).w) : 0;
+                return ix < 0 ? ~ix : ix;
+            };
+            int idx0 = load_idx(0), idx1 = load_idx(1);
+            if (ntiles > 0) {
+#pragma unroll
+                for (int i = 0; i < GW; i++) {
+                    const int j = __shfl_sync(0xffffffffu, idx0, i);
+                    if (i < n_e) cp_async16(ring + i * F, Gb + (size_t)j * F);
+                    cp_async_commit();
                 }
             }
-            if (ntiles > 0 && !pre) {
-                mbar_wait(&b_full[it & 1], (it >> 1) & 1);
-                const float4* m0 = sMeta + (it & 1) * NEB;
-                BWD_ISSUE(ga, m0);
-            }
-            pre = false;
             int j_rel = 0;
             int row_end = __shfl_sync(0xffffffffu, rp, 1);
             // own rows of sender j (current) and j + 1 (prefetched)
@@ -502,11 +504,17 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                 pbS = pbVS = Y0 = Y1 = Y2 = 0.f;
                 if (j_rel + 1 < na) load_own(a0 + j_rel + 1, nphS, nphVS, nphVV, nvj0, nvj1, nvj2, nr0, nr1, nr2);
             };
-#define BWD_COMPUTE(H, GR)                                                                                        \
+#define BWD_COMPUTE(H)                                                                                            \
     {                                                                                                             \
-        const int E8_ = e_begin + t * NEB + (H) * 8;                                                              \
+        const int k0_ = t * NEB + (H) * 8;                                                                        \
+        const int E8_ = e_begin + k0_;                                                                            \
         if (E8_ < e_end) {                                                                                        \
             while (E8_ >= row_end) next_row();                                                                    \
+            /* prefetch targets: edges k0 + 16 .. k0 + 23 of the unit, all in index block tb_ */                  \
+            const int tb_ = (k0_ + GW) >> 5, l0_ = (k0_ + GW) & 31;                                               \
+            if (l0_ == 0) { if (tb_ & 1) idx0 = load_idx(tb_ + 1); else idx1 = load_idx(tb_ + 1); }               \
+            const int isel_ = (tb_ & 1) ? idx1 : idx0;                                                            \
+            const bool pf_ = k0_ + GW < n_e;                                                                      \
             uint32_t wS_[8], wVS_[8], wVV_[8], dS_[8], dVS_[8], dVV_[8];                                          \
             tmem_ld8_nowait(lane_base + buf * TCOLS + (H) * 8, wS_);                                              \
             tmem_ld8_nowait(lane_base + buf * TCOLS + NEB + (H) * 8, dS_);                                        \
@@ -518,10 +526,12 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
             }                                                                                                     \
             mbar_wait(&p_empty[hc & 1], ((hc >> 1) & 1) ^ 1);           /* partials buffer free again */          \
             tmem_wait_ld();                                                                                       \
-            uint8_t* pdst_ = sP + (hc & 1) * P_BYTES + f * 16;                                                    \
+            uint8_t* pdst_ = sP + (hc & 1) * P_BYTES;                                                             \
             _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                                    \
                 const float4 m_ = meta[(H) * 8 + i_];                                                             \
-                const float sb_ = GR[i_].x, vb0_ = GR[i_].y, vb1_ = GR[i_].z, vb2_ = GR[i_].w;                    \
+                cp_async_wait<GW - 1>();                                                                          \
+                const float4 g_ = ring[((H) * 8 + i_) * F];                                                       \
+                const float sb_ = g_.x, vb0_ = g_.y, vb1_ = g_.z, vb2_ = g_.w;                                    \
                 const float X_ = fmaf(vb0_, m_.x, fmaf(vb1_, m_.y, vb2_ * m_.z));                                 \
                 const float wVSf_ = __uint_as_float(wVS_[i_]);                                                    \
                 float db_ = phS * (sb_ * __uint_as_float(dS_[i_]));                                               \
@@ -535,31 +545,27 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                     Y0 = fmaf(wVVf_, vb0_, Y0); Y1 = fmaf(wVVf_, vb1_, Y1); Y2 = fmaf(wVVf_, vb2_, Y2);           \
                 }                                                                                                 \
                 const float tt_ = wVSf_ * phVS;                                                                   \
-                *(float4*)(pdst_ + i_ * P_ROW) = make_float4(db_, tt_ * vb0_, tt_ * vb1_, tt_ * vb2_);            \
+                *(float4*)(pdst_ + i_ * P_ROW + ((f ^ ((i_ & 1) << 2)) << 4)) =                                   \
+                    make_float4(db_, tt_ * vb0_, tt_ * vb1_, tt_ * vb2_);                                         \
+                const int jn_ = __shfl_sync(0xffffffffu, isel_, l0_ + i_);                                        \
+                if (pf_) cp_async16(ring + ((H) * 8 + i_) * F, Gb + (size_t)jn_ * F);                             \
+                cp_async_commit();                                                                                \
             }                                                                                                     \
-            __syncwarp();                                                                                         \
-            if (lane == 0) mbar_arrive(&p_full[hc & 1]);                /* hand the batch to the reducer warp */  \
+            bar_arrive(NB_PF + (hc & 1), 160);                          /* hand the batch to the reducer warp */  \
             hc++;                                                                                                 \
         }                                                                                                         \
     }
             for (int t = 0; t < ntiles; t++, it++) {
                 const int buf = it & 1;
-                const float4* meta = sMeta + buf * NEB;
-                BWD_ISSUE(gb, meta + 8);
+                const float4* meta = sMeta + (it & 3) * NEB;
                 mbar_wait(&t_full[buf], (it >> 1) & 1);
                 tc_fence_after();
-                BWD_COMPUTE(0, ga);
-                if (t + 1 < ntiles || next_has) {
-                    mbar_wait(&b_full[buf ^ 1], ((it + 1) >> 1) & 1);
-                    const float4* mn = sMeta + (buf ^ 1) * NEB;
-                    BWD_ISSUE(ga, mn);
-                    pre = t + 1 == ntiles;
-                }
-                BWD_COMPUTE(1, gb);
+                BWD_COMPUTE(0);
+                BWD_COMPUTE(1);
                 tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&t_empty[buf]);
+                bar_arrive(NB_TE + buf, 192);
             }
+            cp_async_wait<0>();           // slots are re-armed by the next unit's prologue
             for (;;) {
                 store_row();
                 if (j_rel + 1 >= na) break;
@@ -570,16 +576,15 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                 if (j_rel + 1 < na) load_own(a0 + j_rel + 1, nphS, nphVS, nphVV, nvj0, nvj1, nvj2, nr0, nr1, nr2);
             }
         }
-#undef BWD_ISSUE
 #undef BWD_COMPUTE
     } else if (lwarp < 6) {
         // ===================== producers: rows 0..15 R_e, rows 16..31 R'_e =====================
-        const int pt = ltid - 128, e = pt & 15, h = pt >> 4;   // h = 0..3 (h == 3 idle)
+        // thread = (edge e, basis slots 8h .. 8h+7); the h == 3 quarter only takes part in the barriers
+        const int pt = ltid - 128, e = pt & 15, h = pt >> 4;
         const float inv_rc = p.inv_rc;
         const float a1c = 3.14159265358979323846f * inv_rc;
         const int K = p.K;
         uint32_t it = 0;
-        if (h < 3)
         for (long long u = u0; u < n_units; u += ustride) {
             const long long a0 = u * apu;
             const long long a1 = min(N, a0 + (long long)apu);
@@ -587,44 +592,54 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
             const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
             for (int t = 0; t < ntiles; t++, it++) {
                 const int buf = it & 1;
-                const EdgeGeom g = load_edge(p.ej, e_begin + t * NEB + e, e_end, inv_rc);
-                const float fc = g.real ? 0.5f * (1.0f + g.c1) : 0.0f;
-                const float dfc = g.real ? -0.5f * a1c * g.s1 : 0.0f;
-                float sn_, cn_;
-                if (h == 0) { sn_ = g.s1; cn_ = g.c1; } else sincospif((float)(8 * h) * g.x, &sn_, &cn_);
-                float vals[8], dvals[8];
+                uint4 q[6];
+                float4 meta_v = make_float4(0.f, 0.f, 0.f, 0.f);
+                float invd_v = 0.f;
+                if (h < 3) {
+                    const EdgeGeom g = load_edge(p.ej, e_begin + t * NEB + e, e_end, inv_rc);
+                    const float fc = g.real ? 0.5f * (1.0f + g.c1) : 0.0f;
+                    const float dfc = g.real ? -0.5f * a1c * g.s1 : 0.0f;
+                    float sn_, cn_;
+                    if (h == 0) { sn_ = g.s1; cn_ = g.c1; } else sincospif((float)(8 * h) * g.x, &sn_, &cn_);
+                    float vals[8], dvals[8];
 #pragma unroll
-                for (int i = 0; i < 8; i++) {
-                    const int b = h * 8 + i;
-                    if (b == 0) { vals[i] = fc; dvals[i] = dfc; }
-                    else {
-                        const float rho = sn_ * g.inv_d;
-                        const float drho = ((float)b * a1c * cn_ - rho) * g.inv_d;
-                        vals[i] = b <= K ? fc * rho : 0.0f;
-                        dvals[i] = b <= K ? dfc * rho + fc * drho : 0.0f;
-                        const float tt = sn_ * g.c1 + cn_ * g.s1;
-                        cn_ = cn_ * g.c1 - sn_ * g.s1;
-                        sn_ = tt;
+                    for (int i = 0; i < 8; i++) {
+                        const int b = h * 8 + i;
+                        if (b == 0) { vals[i] = fc; dvals[i] = dfc; }
+                        else {
+                            const float rho = sn_ * g.inv_d;
+                            const float drho = ((float)b * a1c * cn_ - rho) * g.inv_d;
+                            vals[i] = b <= K ? fc * rho : 0.0f;
+                            dvals[i] = b <= K ? dfc * rho + fc * drho : 0.0f;
+                            const float tt = sn_ * g.c1 + cn_ * g.s1;
+                            cn_ = cn_ * g.c1 - sn_ * g.s1;
+                            sn_ = tt;
+                        }
+                    }
+                    split3(vals, q[0], q[1], q[2]);
+                    split3(dvals, q[3], q[4], q[5]);
+                    meta_v = make_float4(-g.r.x * g.inv_d, -g.r.y * g.inv_d, -g.r.z * g.inv_d, g.r.w);   // u_e of edge (i <- j)
+                    invd_v = g.inv_d;
+                }
+                __syncwarp();
+                if (it >= 2) bar_sync(NB_TE + buf, 192);          // tile it - 2 consumed: B operand / TMEM buffer free
+                if (h < 3) {
+#pragma unroll
+                    for (int z = 0; z < 2; z++) {
+                        const int row = z * NEB + e;
+                        uint8_t* bb = sB + buf * BB_BYTES + (row >> 3) * SBO + (row & 7) * 16 + h * LBO;
+                        *(uint4*)(bb) = q[3 * z + 0];
+                        *(uint4*)(bb + 4 * LBO) = q[3 * z + 1];
+                        *(uint4*)(bb + 8 * LBO) = q[3 * z + 2];
+                    }
+                    if (h == 0) {
+                        sMeta[(it & 3) * NEB + e] = meta_v;
+                        sInvd[(it & 3) * NEB + e] = invd_v;
                     }
                 }
-                uint4 q[6];
-                split3(vals, q[0], q[1], q[2]);
-                split3(dvals, q[3], q[4], q[5]);
-                mbar_wait_sleep(&t_empty[buf], ((it >> 1) & 1) ^ 1, 256);
-#pragma unroll
-                for (int z = 0; z < 2; z++) {
-                    const int row = z * NEB + e;
-                    uint8_t* bb = sB + buf * BB_BYTES + (row >> 3) * SBO + (row & 7) * 16 + h * LBO;
-                    *(uint4*)(bb) = q[3 * z + 0];
-                    *(uint4*)(bb + 4 * LBO) = q[3 * z + 1];
-                    *(uint4*)(bb + 8 * LBO) = q[3 * z + 2];
-                }
-                if (h == 0) {
-                    sMeta[buf * NEB + e] = make_float4(-g.r.x * g.inv_d, -g.r.y * g.inv_d, -g.r.z * g.inv_d, g.r.w);   // u_e of edge (i <- j)
-                    sInvd[buf * NEB + e] = g.inv_d;
-                }
                 fence_async_smem();
-                mbar_arrive(&b_full[buf]);
+                __syncwarp();
+                bar_arrive(NB_BF + buf, 96);
             }
         }
     } else if (lwarp == 6) {
@@ -647,12 +662,16 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                     const int E = E8 + re;
                     float4 gold = make_float4(0.f, 0.f, 0.f, 0.f);
                     if (rsub == 0 && !first) gold = Gout[E];                  // running sum over layers, fetched early
-                    mbar_wait(&p_full[hc & 1], (hc >> 1) & 1);
+                    bar_sync(NB_PF + (hc & 1), 160);
+                    // this lane adds the 32 chunks rsub + 4 k of row re; odd rows walk k in the order k ^ 1 so that the
+                    // two rows served by one quarter-warp hit different banks (the writers' swizzle only permutes which
+                    // channel sits in which chunk, the sum does not care)
                     const uint8_t* src = sP + (hc & 1) * P_BYTES + re * P_ROW + rsub * 16;
-                    float4 acc = *(const float4*)src;
+                    const int odd = re & 1;
+                    float4 acc = *(const float4*)(src + ((0 ^ odd) << 6));
 #pragma unroll
                     for (int k = 1; k < 32; k++) {
-                        const float4 x = *(const float4*)(src + k * 64);
+                        const float4 x = *(const float4*)(src + ((k ^ odd) << 6));
                         acc.x += x.x; acc.y += x.y; acc.z += x.z; acc.w += x.w;
                     }
                     __syncwarp();
@@ -664,33 +683,31 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                         acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o); acc.w += __shfl_xor_sync(0xffffffffu, acc.w, o);
                     }
                     if (rsub == 0) {
-                        const float4 mm = sMeta[buf * NEB + h * 8 + re];
-                        const float inv_d = sInvd[buf * NEB + h * 8 + re];
+                        const float4 mm = sMeta[(it & 3) * NEB + h * 8 + re];
+                        const float inv_d = sInvd[(it & 3) * NEB + h * 8 + re];
                         const float uu = acc.y * mm.x + acc.z * mm.y + acc.w * mm.z;
                         Gout[E] = make_float4(gold.x + acc.x * mm.x + (acc.y - uu * mm.x) * inv_d,
                                               gold.y + acc.x * mm.y + (acc.z - uu * mm.y) * inv_d,
                                               gold.z + acc.x * mm.z + (acc.w - uu * mm.z) * inv_d, 0.f);
                     }
                 }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&t_empty[buf]);
             }
         }
     } else if (lwarp == 7) {
-        // ===================== MMA issuer =====================
-        if (lane == 0) {
-            const uint32_t idesc = (1u << 4) | ((uint32_t)((2 * NEB) >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-            const uint32_t a_base = smem_u32(sA), b_base = smem_u32(sB);
-            uint32_t it = 0;
-            for (long long u = u0; u < n_units; u += ustride) {
-                const long long a0 = u * apu;
-                const long long a1 = min(N, a0 + (long long)apu);
-                const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
-                const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
-                for (int t = 0; t < ntiles; t++, it++) {
-                    const int buf = it & 1;
-                    mbar_wait_sleep(&b_full[buf], (it >> 1) & 1, 128);
-                    tc_fence_after();
+        // ===================== MMA issuer (lane 0; the whole warp waits on the producers' named barrier) =====================
+        const uint32_t idesc = (1u << 4) | ((uint32_t)((2 * NEB) >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+        const uint32_t a_base = smem_u32(sA), b_base = smem_u32(sB);
+        uint32_t it = 0;
+        for (long long u = u0; u < n_units; u += ustride) {
+            const long long a0 = u * apu;
+            const long long a1 = min(N, a0 + (long long)apu);
+            const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
+            const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
+            for (int t = 0; t < ntiles; t++, it++) {
+                const int buf = it & 1;
+                bar_sync(NB_BF + buf, 96);
+                tc_fence_after();
+                if (lane == 0) {
 #pragma unroll
                     for (int c = 0; c < NCH; c++) {
                         const uint32_t d = tmem_base + buf * TCOLS + c * 2 * NEB;
@@ -704,6 +721,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                     }
                     umma_commit(&t_full[buf]);
                 }
+                __syncwarp();
             }
         }
     }
