@@ -355,13 +355,13 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
 constexpr int NEB = 16;                                 // edges per tile; B rows 0..15 = R_e, 16..31 = R'_e
 constexpr int BB_BYTES = (2 * NEB / 8) * SBO;           // 6144
 constexpr int BWD_THREADS = 512;
-constexpr int P_ROW = F * 16;                           // per-edge partials [128] float4; 16-byte chunk c of row e is stored at
-                                                        // chunk c ^ ((e & 1) << 2): conflict-free transposed reads
+constexpr int P_ROW = 3 * F * 4 + 64;                   // per-edge partials: x | y | z planes of 128 floats (+64 B: the two rows
+                                                        // read by one quarter-warp of the reducer fall into different banks)
 constexpr int P_BYTES = 8 * P_ROW;                      // one 8-edge batch
 constexpr int GW = 16;                                  // gather window (edges in flight per thread)
 constexpr int RING_BYTES = GW * F * 16;                 // 32768
 constexpr int G_OFF_B = 0, G_OFF_P = 2 * BB_BYTES, G_OFF_RING = G_OFF_P + 2 * P_BYTES, G_OFF_META = G_OFF_RING + RING_BYTES,
-              G_OFF_INVD = G_OFF_META + 4 * NEB * 16, G_OFF_BAR = G_OFF_INVD + 4 * NEB * 4, GROUP_BYTES = G_OFF_BAR + 128;
+              G_OFF_BAR = G_OFF_META + 4 * NEB * 16, GROUP_BYTES = G_OFF_BAR + 128;
 constexpr int bwd_smem_bytes(int nch) { return nch * A_CHUNK_BYTES + 2 * GROUP_BYTES + 128; }
 
 struct BwdParams {
@@ -394,8 +394,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
     uint8_t* gbase = smem + NCH * A_CHUNK_BYTES + grp * GROUP_BYTES;
     uint8_t* sB = gbase + G_OFF_B;
     uint8_t* sP = gbase + G_OFF_P;                 // [2][8] rows of P_ROW bytes: (db, ub_x, ub_y, ub_z) per channel
-    float4* sMeta = (float4*)(gbase + G_OFF_META); // [4][NEB] (u of edge (i <- j), i): ring of 4 tiles (the reducer lags)
-    float* sInvd = (float*)(gbase + G_OFF_INVD);   // [4][NEB]
+    float4* sMeta = (float4*)(gbase + G_OFF_META); // [4][NEB] (u of edge (i <- j), 1/d): ring of 4 tiles
     uint64_t* bars = (uint64_t*)(gbase + G_OFF_BAR);
     uint64_t* t_full = bars;          // [2] MMA commit -> consumers (mbarrier, count 1)
     uint64_t* p_empty = bars + 2;     // [2] reducer -> consumers: partials buffer read (mbarrier, count 1)
@@ -544,9 +543,13 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                     pbVS = fmaf(wVSf_, X_, pbVS);                                                                 \
                     Y0 = fmaf(wVVf_, vb0_, Y0); Y1 = fmaf(wVVf_, vb1_, Y1); Y2 = fmaf(wVVf_, vb2_, Y2);           \
                 }                                                                                                 \
-                const float tt_ = wVSf_ * phVS;                                                                   \
-                *(float4*)(pdst_ + i_ * P_ROW + ((f ^ ((i_ & 1) << 2)) << 4)) =                                   \
-                    make_float4(db_, tt_ * vb0_, tt_ * vb1_, tt_ * vb2_);                                         \
+                /* this channel's share of g_e = db u + (ub - (ub.u) u) / d, ub = tt vb':  alpha u + beta vb' */  \
+                const float beta_ = wVSf_ * phVS * m_.w;                                                          \
+                const float alpha_ = fmaf(-beta_, X_, db_);                                                       \
+                float* pd_ = (float*)(pdst_ + i_ * P_ROW) + f;          /* three planes of 128 floats per edge */ \
+                pd_[0] = fmaf(alpha_, m_.x, beta_ * vb0_);                                                        \
+                pd_[F] = fmaf(alpha_, m_.y, beta_ * vb1_);                                                        \
+                pd_[2 * F] = fmaf(alpha_, m_.z, beta_ * vb2_);                                                    \
                 const int jn_ = __shfl_sync(0xffffffffu, isel_, l0_ + i_);                                        \
                 if (pf_) cp_async16(ring + ((H) * 8 + i_) * F, Gb + (size_t)jn_ * F);                             \
                 cp_async_commit();                                                                                \
@@ -594,7 +597,6 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                 const int buf = it & 1;
                 uint4 q[6];
                 float4 meta_v = make_float4(0.f, 0.f, 0.f, 0.f);
-                float invd_v = 0.f;
                 if (h < 3) {
                     const EdgeGeom g = load_edge(p.ej, e_begin + t * NEB + e, e_end, inv_rc);
                     const float fc = g.real ? 0.5f * (1.0f + g.c1) : 0.0f;
@@ -618,8 +620,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                     }
                     split3(vals, q[0], q[1], q[2]);
                     split3(dvals, q[3], q[4], q[5]);
-                    meta_v = make_float4(-g.r.x * g.inv_d, -g.r.y * g.inv_d, -g.r.z * g.inv_d, g.r.w);   // u_e of edge (i <- j)
-                    invd_v = g.inv_d;
+                    meta_v = make_float4(-g.r.x * g.inv_d, -g.r.y * g.inv_d, -g.r.z * g.inv_d, g.inv_d);   // u_e of edge (i <- j), 1/d
                 }
                 __syncwarp();
                 if (it >= 2) bar_sync(NB_TE + buf, 192);          // tile it - 2 consumed: B operand / TMEM buffer free
@@ -632,10 +633,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                         *(uint4*)(bb + 4 * LBO) = q[3 * z + 1];
                         *(uint4*)(bb + 8 * LBO) = q[3 * z + 2];
                     }
-                    if (h == 0) {
-                        sMeta[(it & 3) * NEB + e] = meta_v;
-                        sInvd[(it & 3) * NEB + e] = invd_v;
-                    }
+                    if (h == 0) sMeta[(it & 3) * NEB + e] = meta_v;
                 }
                 fence_async_smem();
                 __syncwarp();
@@ -663,33 +661,28 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                     float4 gold = make_float4(0.f, 0.f, 0.f, 0.f);
                     if (rsub == 0 && !first) gold = Gout[E];                  // running sum over layers, fetched early
                     bar_sync(NB_PF + (hc & 1), 160);
-                    // this lane adds the 32 chunks rsub + 4 k of row re; odd rows walk k in the order k ^ 1 so that the
-                    // two rows served by one quarter-warp hit different banks (the writers' swizzle only permutes which
-                    // channel sits in which chunk, the sum does not care)
+                    // this lane adds a quarter (chunks rsub + 4 k) of each of the three 128-float planes of row re
                     const uint8_t* src = sP + (hc & 1) * P_BYTES + re * P_ROW + rsub * 16;
-                    const int odd = re & 1;
-                    float4 acc = *(const float4*)(src + ((0 ^ odd) << 6));
+                    float3 acc = make_float3(0.f, 0.f, 0.f);
 #pragma unroll
-                    for (int k = 1; k < 32; k++) {
-                        const float4 x = *(const float4*)(src + ((k ^ odd) << 6));
-                        acc.x += x.x; acc.y += x.y; acc.z += x.z; acc.w += x.w;
+                    for (int k = 0; k < 8; k++) {
+                        const float4 x = *(const float4*)(src + k * 64);
+                        const float4 y = *(const float4*)(src + F * 4 + k * 64);
+                        const float4 z = *(const float4*)(src + 2 * F * 4 + k * 64);
+                        acc.x += (x.x + x.y) + (x.z + x.w);
+                        acc.y += (y.x + y.y) + (y.z + y.w);
+                        acc.z += (z.x + z.y) + (z.z + z.w);
                     }
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&p_empty[hc & 1]);
                     hc++;
 #pragma unroll
                     for (int o = 2; o >= 1; o >>= 1) {
-                        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
-                        acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o); acc.w += __shfl_xor_sync(0xffffffffu, acc.w, o);
+                        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o);
+                        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
+                        acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o);
                     }
-                    if (rsub == 0) {
-                        const float4 mm = sMeta[(it & 3) * NEB + h * 8 + re];
-                        const float inv_d = sInvd[(it & 3) * NEB + h * 8 + re];
-                        const float uu = acc.y * mm.x + acc.z * mm.y + acc.w * mm.z;
-                        Gout[E] = make_float4(gold.x + acc.x * mm.x + (acc.y - uu * mm.x) * inv_d,
-                                              gold.y + acc.x * mm.y + (acc.z - uu * mm.y) * inv_d,
-                                              gold.z + acc.x * mm.z + (acc.w - uu * mm.z) * inv_d, 0.f);
-                    }
+                    if (rsub == 0) Gout[E] = make_float4(gold.x + acc.x, gold.y + acc.y, gold.z + acc.z, 0.f);
                 }
             }
         }
