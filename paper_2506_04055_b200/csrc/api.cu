@@ -307,6 +307,13 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
         l.UV = tmp;
         up((size_t)F * 2 * F, (float**)&l.Wu1, &Wu1); up(F, (float**)&l.bu1);
         up((size_t)3 * F * F, (float**)&l.Wu2, &Wu2); up(3 * F, (float**)&l.bu2);
+        if (rcode == MLP_OK) {      // integer slices for the exact tensor-core path of the forward GEMMs
+            painn::gemm_register_exact(l.Wm1, Wm1.data(), F, F);
+            painn::gemm_register_exact(l.Wm2, Wm2.data(), 3 * F, F);
+            painn::gemm_register_exact(l.UV, UV.data(), 2 * F, F);
+            painn::gemm_register_exact(l.Wu1, Wu1.data(), F, 2 * F);
+            painn::gemm_register_exact(l.Wu2, Wu2.data(), 3 * F, F);
+        }
         upT(Wm1, F, F, (float**)&l.Wm1T);
         upT(Wm2, 3 * F, F, (float**)&l.Wm2T);
         upT(UV, 2 * F, F, (float**)&l.UVT);
@@ -315,6 +322,7 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
     }
     std::vector<float> Wr1;
     up((size_t)R * F, &m->Wr1, &Wr1); up(R, &m->br1); up(R, &m->wr2); up(1, &m->br2);
+    if (rcode == MLP_OK) painn::gemm_register_exact(m->Wr1, Wr1.data(), R, F);
     upT(Wr1, R, F, &m->Wr1T);
     if (rcode == MLP_OK) rcode = ensure(m, m->b_misc, sizeof(Misc));
     if (rcode == MLP_OK && cudaMallocHost(&m->h_misc, sizeof(Misc)) != cudaSuccess) rcode = MLP_ERR_NOMEM;
@@ -335,7 +343,7 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
 
 __attribute__((visibility("default"))) void mlp_destroy(mlp_model* m) {
     if (!m) return;
-    for (const float* w : m->gemm_weights) painn::gemm_unregister_split(w);
+    for (const float* w : m->gemm_weights) { painn::gemm_unregister_split(w); painn::gemm_unregister_exact(w); }
     for (Buf& b : m->wbufs) free_buf(b);
     Buf* bs[] = {&m->b_cell_id, &m->b_wrap, &m->b_perm, &m->b_inv_perm, &m->b_pos_s, &m->b_types_s, &m->b_wrap_s,
                  &m->b_cell_s, &m->b_local, &m->b_row_cnt, &m->b_row_ptr, &m->b_scan_tmp, &m->b_cell_count,
@@ -362,6 +370,7 @@ __attribute__((visibility("default"))) int mlp_set_option(mlp_model* m, const ch
     if (!strcmp(name, "edge_path")) { m->edge_path = (int)value; return MLP_OK; }
     if (!strcmp(name, "gemm_fwd_tc")) { m->fwd_tc = value != 0; return MLP_OK; }
     if (!strcmp(name, "gemm_path")) { painn::g_gemm_path = (int)value; return MLP_OK; }
+    if (!strcmp(name, "gemm_fwd_exact")) { painn::g_gemm_fwd_exact = (int)value; return MLP_OK; }
     if (!strcmp(name, "filter_emulate")) { painn::g_filter_emulate = (int)value; return MLP_OK; }
     if (!strcmp(name, "gather_emulate")) { painn::g_gather_emulate = (int)value; return MLP_OK; }
     if (!strcmp(name, "edge_capacity")) {
@@ -696,13 +705,18 @@ __attribute__((visibility("default"))) __attribute__((visibility("default"))) in
         const int saved = painn::g_gemm_path;
         painn::g_gemm_path = path;
         painn::g_last_gemm_tc = 0;
-        gemm_nt(L, A, K, dW, K, C, N, M, N, K, dB, accumulate != 0);
+        if (path == 2) {            // exact integer-slice tensor-core kernel (forward path)
+            painn::gemm_register_exact(dW, w.data(), N, K);
+            painn::g_last_gemm_tc = painn::gemm_nt_exact(L, A, K, dW, C, N, M, N, K, dB, accumulate != 0, false) ? 1 : 0;
+            if (!painn::g_last_gemm_tc) r = MLP_ERR_ARG;
+        } else
+            gemm_nt(L, A, K, dW, K, C, N, M, N, K, dB, accumulate != 0);
         painn::g_gemm_path = saved;
         if (used_tc) *used_tc = painn::g_last_gemm_tc;
         cudaError_t e = cudaDeviceSynchronize();
         if (e != cudaSuccess) r = MLP_ERR_CUDA;
     }
-    for (const float* x : m->gemm_weights) painn::gemm_unregister_split(x);
+    for (const float* x : m->gemm_weights) { painn::gemm_unregister_split(x); painn::gemm_unregister_exact(x); }
     for (Buf& b : m->wbufs) free_buf(b);
     return r;
 }

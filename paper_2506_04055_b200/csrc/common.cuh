@@ -55,9 +55,14 @@ void nbr_reverse(const Launch& L, long long N, const int* row_ptr, const float4*
 void nbr_export(const Launch& L, long long N, const int* row_ptr, const float4* ej, const unsigned char* img,
                 const int* perm, const signed char* wrap_s, int* out_i, int* out_j, signed char* out_img);
 
-extern int g_gemm_emulate, g_gemm_path, g_last_gemm_tc;   // debug knobs, see gemm.cu
+extern int g_gemm_emulate, g_gemm_path, g_last_gemm_tc, g_gemm_fwd_exact;   // debug knobs, see gemm.cu
 void gemm_register_split(const float* W, const float* hi, const float* lo);
 void gemm_unregister_split(const float* W);
+// exact integer-slice tensor-core path of the forward GEMMs (gemm_tc.cu): slices of W [N x K] are cut at create
+void gemm_register_exact(const float* Wdev, const float* Whost, int N, int K);
+void gemm_unregister_exact(const float* Wdev);
+bool gemm_nt_exact(const Launch& L, const float* A, int lda, const float* W, float* C, int ldc, long long M, int N, int K,
+                   const float* bias, bool accumulate, bool act_a);
 extern int g_filter_emulate, g_gather_emulate;   // debug knobs, see painn_fwd.cu
 // ---- dense node GEMM (gemm.cu):  C[M x N] (+)= A[M x K] . B[N x K]^T + bias ----
 void gemm_nt(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,

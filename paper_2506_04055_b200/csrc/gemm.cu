@@ -180,7 +180,8 @@ __global__ void __launch_bounds__(256, 2) k_sgemm128(const float* __restrict__ A
 #include <unordered_map>
 static std::unordered_map<const float*, std::pair<const float*, const float*>> g_split;
 int g_last_gemm_tc = 0;   // set to 1 by gemm_nt when the tensor-core kernel was used (test hook)
-int g_gemm_path = 0;   // 0: tensor cores when the shape is covered, 1: force the SIMT reference path
+int g_gemm_path = 0;   // 0: tensor cores when the shape is covered, 1: forward GEMM (round-to-nearest / exact accumulation wanted)
+int g_gemm_fwd_exact = 1;   // forward GEMMs: 1 = exact integer-slice tensor-core kernel when covered, 0 = fp32 FFMA kernel
 void gemm_register_split(const float* W, const float* hi, const float* lo) { g_split[W] = {hi, lo}; }
 void gemm_unregister_split(const float* W) { g_split.erase(W); }
 bool gemm_nt_tc(const Launch& L, const float* A, int lda, const float* Whi, const float* Wlo, int ldw, float* C, int ldc,
@@ -201,6 +202,11 @@ void gemm_nt_act(const Launch& L, const float* A, int lda, const float* B, int l
     if (M == 0) return;
     const bool fast_ok = g_gemm_emulate == 0 && N % 128 == 0 && K % 8 == 0 && lda % 4 == 0 && ldb % 4 == 0 &&
                          ldc % 4 == 0 && ((((uintptr_t)A | (uintptr_t)B | (uintptr_t)C | (uintptr_t)bias) & 15) == 0);
+    if ((act_a || g_gemm_path == 1) && g_gemm_fwd_exact && g_gemm_emulate == 0 &&
+        gemm_nt_exact(L, A, lda, B, C, ldc, M, N, K, bias, accumulate, act_a)) {
+        g_last_gemm_tc = 1;
+        return;
+    }
     if (act_a || (g_gemm_path == 1 && fast_ok)) {
         if (fast_ok && M / 128 < 65535) {
             dim3 grid((unsigned)(N / 128), (unsigned)((M + 127) / 128));

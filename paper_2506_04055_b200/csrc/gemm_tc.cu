@@ -18,7 +18,11 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <cmath>
 #include <cstdio>
+#include <unordered_map>
+#include <vector>
+#include <algorithm>
 
 #include "common.cuh"
 #include "tc_common.cuh"
@@ -220,6 +224,274 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
     }
 }
 
+// =================================================================================================================
+// k_gemm_exact: error-free tensor-core GEMM for the FORWARD linear layers (K = 128 per launch).
+//
+// tcgen05.mma truncates its fp32 accumulator toward zero after every instruction (B3), a systematic bias the
+// energy cannot absorb.  Truncation is harmless when every partial sum is exactly representable, so the operands are
+// cut into INTEGER slices (block floating point per row, Ozaki-style):
+//     x'_mk = x_mk / 2^e_m  in (-1, 1)      x' ~= (s1 + s2 2^-8 + s3 2^-16) / 128 ,   s_i integers in [-128, 128]
+// (weights likewise, sliced once at create: t1, t2, t3 and 2^f_n).  Every slice value is exact in TF32, every product
+// |s t| <= 2^14, a K = 128 chain of up to three slice pairs stays below 2^24: each accumulator holds an exact integer.
+//     y_mn = 2^(e_m + f_n - 14) ( S2 + S3 2^-8 + S4 2^-16 ),   S_g = sum over slice pairs i + j = g of  s_i . t_j
+// (pairs with i + j >= 5 are dropped: relative 2^-22 of row max x column max, unbiased).  Three accumulators per
+// output tile; 24 MMAs (M = 128, N = 64, K = 8) per 32-wide K block.
+// Each output tile walks its K blocks twice: pass 0 streams A through the ring to find the row maxima (exponents
+// e_m), pass 1 streams A (an L2 hit) and the weight slices again, converts A into its three slices in shared memory
+// and runs the MMAs.  Same warp roles and barriers as k_gemm_3xtf32; ACT applies SiLU to A while converting.
+constexpr int XBN = 64, XSTAGES = 2, XPRE = 4;
+constexpr int XW_TILE = XBN * BK * 4;                                   // 8 KB
+constexpr int XSTAGE = 3 * A_TILE_BYTES + 3 * XW_TILE;                  // 72 KB: A slices 1..3 (slice 1 lands as raw A), W slices 1..3
+constexpr int XSMEM = XSTAGES * XSTAGE + XPRE * A_TILE_BYTES + 4 * BM * 4 + 256 + 1024;
+constexpr int XACC = 4 * XBN;                                           // TMEM columns per accumulator set (S2..S5)
+
+struct XParams {
+    float* C;
+    const float* bias;
+    const float* colscale;     // [N] 2^f_n
+    long long M;
+    int N, ldc, accumulate;
+};
+
+__device__ __forceinline__ float silu_x(float x) { return x / (1.0f + __expf(-x)); }
+
+// Work unit = one 128-row block of A with ALL its N tiles: the row exponents are found once per unit (pass 0, on a
+// separate 4-buffer ring that the producer fills one unit ahead), then every N tile streams A (L2 hits) and its weight
+// slices through the 2-stage main ring (pass 1).
+template <bool ACT>
+__global__ void __launch_bounds__(NUM_THREADS, 1)
+    k_gemm_exact(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapW1,
+                 const __grid_constant__ CUtensorMap mapW2, const __grid_constant__ CUtensorMap mapW3, XParams p) {
+    extern __shared__ __align__(1024) uint8_t smem[];
+    uint8_t* pre = smem + XSTAGES * XSTAGE;                          // [XPRE] raw A blocks of the next unit
+    float* rowscale = (float*)(pre + XPRE * A_TILE_BYTES);           // [4][BM]  2^(e_m - 14) of the last four units
+    uint64_t* bars = (uint64_t*)(rowscale + 4 * BM);
+    uint64_t* full = bars;                    // [XSTAGES] TMA landed            (count 1 + tx)
+    uint64_t* conv = full + XSTAGES;          // [XSTAGES] A converted           (count 128)
+    uint64_t* empty = conv + XSTAGES;         // [XSTAGES] MMAs done             (count 1, tcgen05.commit)
+    uint64_t* pfull = empty + XSTAGES;        // [XPRE] pass-0 block landed      (count 1 + tx)
+    uint64_t* pempty = pfull + XPRE;          // [XPRE] pass-0 block scanned     (count 128)
+    uint64_t* tfull = pempty + XPRE;          // [2] accumulators ready          (count 1)
+    uint64_t* tempty = tfull + 2;             // [2] accumulators drained        (count 4)
+    uint32_t* tmem_slot = (uint32_t*)(tempty + 2);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_tiles = p.N / XBN;
+    const long long units = (p.M + BM - 1) / BM;
+    constexpr int kblocks = 128 / BK;         // 4 == XPRE
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < XSTAGES; s++) { mbar_init(&full[s], 1); mbar_init(&conv[s], 128); mbar_init(&empty[s], 1); }
+        for (int s = 0; s < XPRE; s++) { mbar_init(&pfull[s], 1); mbar_init(&pempty[s], 128); }
+        for (int b = 0; b < 2; b++) { mbar_init(&tfull[b], 1); mbar_init(&tempty[b], 4); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) tmem_alloc(tmem_slot, 512);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    if (warp == 0) {
+        // ===================== TMA producer =====================
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0, pphase = 0;
+            auto preload = [&](long long u) {                         // pass-0 blocks of unit u
+                for (int kb = 0; kb < kblocks; kb++) {
+                    mbar_wait(&pempty[kb], pphase ^ 1);
+                    mbar_expect_tx(&pfull[kb], A_TILE_BYTES);
+                    tma_load_2d(pre + kb * A_TILE_BYTES, &mapA, &pfull[kb], kb * BK, (int)u * BM);
+                }
+                pphase ^= 1;
+            };
+            if ((long long)blockIdx.x < units) preload(blockIdx.x);
+            for (long long u = blockIdx.x; u < units; u += gridDim.x) {
+                const int m0 = (int)u * BM;
+                for (int nt = 0; nt < n_tiles; nt++) {
+                    for (int kb = 0; kb < kblocks; kb++) {
+                        mbar_wait(&empty[stage], phase ^ 1);
+                        uint8_t* st = smem + stage * XSTAGE;
+                        mbar_expect_tx(&full[stage], A_TILE_BYTES + 3 * XW_TILE);
+                        tma_load_2d(st, &mapA, &full[stage], kb * BK, m0);
+                        tma_load_2d(st + 3 * A_TILE_BYTES, &mapW1, &full[stage], kb * BK, nt * XBN);
+                        tma_load_2d(st + 3 * A_TILE_BYTES + XW_TILE, &mapW2, &full[stage], kb * BK, nt * XBN);
+                        tma_load_2d(st + 3 * A_TILE_BYTES + 2 * XW_TILE, &mapW3, &full[stage], kb * BK, nt * XBN);
+                        if (++stage == XSTAGES) { stage = 0; phase ^= 1; }
+                    }
+                    if (nt == 0 && u + gridDim.x < units) preload(u + gridDim.x);   // next unit's pass 0, one unit ahead
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer =====================
+        if (lane == 0) {
+            const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(XBN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+            int stage = 0;
+            uint32_t phase = 0;
+            int buf = 0;
+            uint32_t bphase = 0;
+            for (long long u = blockIdx.x; u < units; u += gridDim.x) {
+                for (int nt = 0; nt < n_tiles; nt++) {
+                    mbar_wait(&tempty[buf], bphase ^ 1);
+                    tc_fence_after();
+                    const uint32_t d = tmem_base + buf * XACC;
+                    for (int kb = 0; kb < kblocks; kb++) {
+                        mbar_wait(&conv[stage], phase);
+                        tc_fence_after();
+                        const uint32_t sa = smem_u32(smem + stage * XSTAGE);
+                        uint64_t a[3], w[3];
+#pragma unroll
+                        for (int i = 0; i < 3; i++) {
+                            a[i] = make_desc_sw128(sa + i * A_TILE_BYTES);
+                            w[i] = make_desc_sw128(sa + 3 * A_TILE_BYTES + i * XW_TILE);
+                        }
+#pragma unroll
+                        for (int kk = 0; kk < BK / 8; kk++) {
+                            const uint64_t o = (uint64_t)(kk * 2);   // 32 B along K inside the swizzle row, >> 4
+                            const uint32_t acc = (kb | kk) != 0;
+                            umma_tf32(d, a[0] + o, w[0] + o, idesc, acc);                   // S2: (1,1)
+                            umma_tf32(d + XBN, a[0] + o, w[1] + o, idesc, acc);             // S3: (1,2) (2,1)
+                            umma_tf32(d + XBN, a[1] + o, w[0] + o, idesc, 1);
+                            umma_tf32(d + 2 * XBN, a[0] + o, w[2] + o, idesc, acc);         // S4: (1,3) (2,2) (3,1)
+                            umma_tf32(d + 2 * XBN, a[1] + o, w[1] + o, idesc, 1);
+                            umma_tf32(d + 2 * XBN, a[2] + o, w[0] + o, idesc, 1);
+                            umma_tf32(d + 3 * XBN, a[1] + o, w[2] + o, idesc, acc);         // S5: (2,3) (3,2)
+                            umma_tf32(d + 3 * XBN, a[2] + o, w[1] + o, idesc, 1);
+                        }
+                        umma_commit(&empty[stage]);
+                        if (++stage == XSTAGES) { stage = 0; phase ^= 1; }
+                    }
+                    umma_commit(&tfull[buf]);
+                    if (++buf == 2) { buf = 0; bphase ^= 1; }
+                }
+            }
+        }
+    } else if (warp < EPI_WARP0) {
+        // ===================== converter: row maxima (pass 0), integer slices (pass 1) =====================
+        const int ct = threadIdx.x - CONV_WARP0 * 32;   // 0..127; chunk idx = ct + 128 i lies in row (ct >> 3) + 16 i
+        int stage = 0;
+        uint32_t phase = 0, pphase = 0;
+        uint32_t ucount = 0;
+        const float MAGIC = 12582912.0f;                // 1.5 * 2^23: (t + MAGIC) - MAGIC = round-to-nearest-even integer
+        for (long long u = blockIdx.x; u < units; u += gridDim.x, ucount++) {
+            float mx[8];
+#pragma unroll
+            for (int i = 0; i < 8; i++) mx[i] = 0.f;
+            for (int kb = 0; kb < kblocks; kb++) {
+                mbar_wait(&pfull[kb], pphase);
+                const float4* a = (const float4*)(pre + kb * A_TILE_BYTES);
+#pragma unroll
+                for (int i = 0; i < 8; i++) {
+                    float4 x = a[ct + i * 128];
+                    if (ACT) { x.x = silu_x(x.x); x.y = silu_x(x.y); x.z = silu_x(x.z); x.w = silu_x(x.w); }
+                    mx[i] = fmaxf(mx[i], fmaxf(fmaxf(fabsf(x.x), fabsf(x.y)), fmaxf(fabsf(x.z), fabsf(x.w))));
+                }
+                mbar_arrive(&pempty[kb]);
+            }
+            pphase ^= 1;
+            float q128[8];                               // 128 / 2^e_m
+#pragma unroll
+            for (int i = 0; i < 8; i++) {
+                float m = mx[i];
+                m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));
+                m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
+                m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 4));
+                // 2^e = smallest power of two > m; non-finite / huge rows fall through as garbage / NaN downstream
+                const uint32_t E = (__float_as_uint(m) >> 23) & 0xffu;       // m in [2^(E-127), 2^(E-126))
+                const uint32_t Ec = E < 20u ? 20u : (E > 230u ? 230u : E);   // keep every scale a normal number
+                q128[i] = __uint_as_float((260u - Ec) << 23);                // 2^(126 - E) * 128
+                if ((ct & 7) == 0) rowscale[(ucount & 3) * BM + (ct >> 3) + 16 * i] = __uint_as_float((Ec - 13u) << 23);   // 2^(e - 14)
+            }
+            for (int e = 0; e < n_tiles * kblocks; e++) {
+                mbar_wait(&full[stage], phase);
+                float4* a1 = (float4*)(smem + stage * XSTAGE);
+                float4* a2 = (float4*)(smem + stage * XSTAGE + A_TILE_BYTES);
+                float4* a3 = (float4*)(smem + stage * XSTAGE + 2 * A_TILE_BYTES);
+#pragma unroll
+                for (int i = 0; i < 8; i++) {
+                    const int idx = ct + i * 128;
+                    float4 x = a1[idx];
+                    if (ACT) { x.x = silu_x(x.x); x.y = silu_x(x.y); x.z = silu_x(x.z); x.w = silu_x(x.w); }
+                    float4 s1, s2, s3;
+#define XSLICE(C)                                                            \
+    {                                                                        \
+        const float t1_ = x.C * q128[i];                                     \
+        s1.C = (t1_ + MAGIC) - MAGIC;                                        \
+        const float t2_ = (t1_ - s1.C) * 256.0f;                             \
+        s2.C = (t2_ + MAGIC) - MAGIC;                                        \
+        const float t3_ = (t2_ - s2.C) * 256.0f;                             \
+        s3.C = (t3_ + MAGIC) - MAGIC;                                        \
+    }
+                    XSLICE(x) XSLICE(y) XSLICE(z) XSLICE(w)
+#undef XSLICE
+                    a1[idx] = s1; a2[idx] = s2; a3[idx] = s3;
+                }
+                fence_async_smem();
+                mbar_arrive(&conv[stage]);
+                if (++stage == XSTAGES) { stage = 0; phase ^= 1; }
+            }
+        }
+    } else {
+        // ===================== epilogue =====================
+        const int q = warp & 3;                      // TMEM lane quadrant this warp may access
+        int buf = 0;
+        uint32_t bphase = 0;
+        uint32_t ucount = 0;
+        for (long long u = blockIdx.x; u < units; u += gridDim.x, ucount++) {
+            const long long row = u * BM + q * 32 + lane;
+            for (int nt = 0; nt < n_tiles; nt++) {
+                const int n0 = nt * XBN;
+                mbar_wait(&tfull[buf], bphase);
+                tc_fence_after();
+                const float rs = rowscale[(ucount & 3) * BM + q * 32 + lane];
+                float* crow = p.C + row * p.ldc + n0;
+                const uint32_t tb = tmem_base + ((uint32_t)(q * 32) << 16) + buf * XACC;
+#pragma unroll 1
+                for (int c0 = 0; c0 < XBN; c0 += 16) {
+                    uint32_t r2[16], r3[16], r4[16], r5[16];
+                    float4 o[4];
+                    if (p.accumulate && row < p.M) {
+#pragma unroll
+                        for (int c = 0; c < 4; c++) o[c] = __ldcs((const float4*)(crow + c0) + c);
+                    }
+                    tmem_ld16_nowait(tb + c0, r2);
+                    tmem_ld16_nowait(tb + XBN + c0, r3);
+                    tmem_ld16_nowait(tb + 2 * XBN + c0, r4);
+                    tmem_ld16_nowait(tb + 3 * XBN + c0, r5);
+                    tmem_wait_ld();
+                    if (row < p.M) {
+#pragma unroll
+                        for (int c = 0; c < 16; c += 4) {
+                            const float4 cs = *(const float4*)(p.colscale + n0 + c0 + c);
+                            float v[4];
+#pragma unroll
+                            for (int j = 0; j < 4; j++) {
+                                const float lo = fmaf(__uint_as_float(r5[c + j]), 1.0f / 256.0f, __uint_as_float(r4[c + j]));
+                                v[j] = fmaf(lo, 1.0f / 65536.0f, fmaf(__uint_as_float(r3[c + j]), 1.0f / 256.0f, __uint_as_float(r2[c + j])));
+                            }
+                            float4 y = make_float4(v[0] * (rs * cs.x), v[1] * (rs * cs.y), v[2] * (rs * cs.z), v[3] * (rs * cs.w));
+                            if (p.bias) {
+                                const float4 b = *(const float4*)(p.bias + n0 + c0 + c);
+                                y.x += b.x; y.y += b.y; y.z += b.z; y.w += b.w;
+                            }
+                            if (p.accumulate) { y.x += o[c / 4].x; y.y += o[c / 4].y; y.z += o[c / 4].z; y.w += o[c / 4].w; }
+                            *(float4*)(crow + c0 + c) = y;
+                        }
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&tempty[buf]);
+                if (++buf == 2) { buf = 0; bphase ^= 1; }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc(tmem_base, 512);
+}
+
 // ---- host side: tensor maps through the driver entry point (no link-time dependency on libcuda) ----
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -266,6 +538,92 @@ static bool launch(const Launch& L, const CUtensorMap& a, const CUtensorMap& whi
 }
 
 }  // namespace tc
+
+// ---- exact integer-slice path: weight slices are cut once, at create ----
+struct ExactW {
+    int N, K;
+    float* planes;     // device [K / 128][3][N][128]  integer-valued slices t1, t2, t3
+    float* cs;         // device [K / 128][N]          2^f_n
+};
+static std::unordered_map<const float*, ExactW> g_exact;
+
+void gemm_register_exact(const float* Wdev, const float* Whost, int N, int K) {
+    if (K % 128 != 0 || N % tc::XBN != 0 || g_exact.count(Wdev)) return;
+    const int nc = K / 128;
+    std::vector<float> pl((size_t)nc * 3 * N * 128), cs((size_t)nc * N);
+    for (int c = 0; c < nc; c++)
+        for (int n = 0; n < N; n++) {
+            const float* w = Whost + (size_t)n * K + c * 128;
+            float m = 0.f;
+            for (int k = 0; k < 128; k++) m = std::fmax(m, std::fabs(w[k]));
+            int ex = 0;
+            if (m > 0.f) std::frexp(m, &ex);               // m = f 2^ex, f in [0.5, 1)  ->  |w| < 2^ex
+            ex = std::min(104, std::max(-106, ex));
+            const float q128 = std::ldexp(1.0f, 7 - ex);
+            cs[(size_t)c * N + n] = std::ldexp(1.0f, ex);
+            for (int k = 0; k < 128; k++) {
+                const float t1 = w[k] * q128;
+                const float s1 = std::nearbyint(t1);
+                const float t2 = (t1 - s1) * 256.0f;
+                const float s2 = std::nearbyint(t2);
+                const float s3 = std::nearbyint((t2 - s2) * 256.0f);
+                pl[(((size_t)c * 3 + 0) * N + n) * 128 + k] = s1;
+                pl[(((size_t)c * 3 + 1) * N + n) * 128 + k] = s2;
+                pl[(((size_t)c * 3 + 2) * N + n) * 128 + k] = s3;
+            }
+        }
+    ExactW e{N, K, nullptr, nullptr};
+    if (cudaMalloc(&e.planes, pl.size() * 4) != cudaSuccess) return;
+    if (cudaMalloc(&e.cs, cs.size() * 4) != cudaSuccess) { cudaFree(e.planes); return; }
+    cudaMemcpy(e.planes, pl.data(), pl.size() * 4, cudaMemcpyHostToDevice);
+    cudaMemcpy(e.cs, cs.data(), cs.size() * 4, cudaMemcpyHostToDevice);
+    g_exact[Wdev] = e;
+}
+void gemm_unregister_exact(const float* Wdev) {
+    auto it = g_exact.find(Wdev);
+    if (it == g_exact.end()) return;
+    cudaFree(it->second.planes);
+    cudaFree(it->second.cs);
+    g_exact.erase(it);
+}
+
+// C (+)= act(A) . W^T + bias on tensor cores with exact accumulation (k_gemm_exact).  Returns false when W has no
+// slices registered or the shape is not covered; the caller then uses the fp32 FFMA kernel.
+bool gemm_nt_exact(const Launch& L, const float* A, int lda, const float* W, float* C, int ldc, long long M, int N, int K,
+                   const float* bias, bool accumulate, bool act_a) {
+    using namespace tc;
+    auto it = g_exact.find(W);
+    if (it == g_exact.end() || it->second.N != N || it->second.K != K) return false;
+    if (M <= 0 || (lda % 4) || (ldc % 4) || (((uintptr_t)A | (uintptr_t)C | (uintptr_t)bias) & 15)) return false;
+    static int n_sm = 0;
+    static bool attr = false;
+    if (!n_sm) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    }
+    if (!attr) {
+        if (cudaFuncSetAttribute(k_gemm_exact<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, XSMEM) != cudaSuccess ||
+            cudaFuncSetAttribute(k_gemm_exact<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, XSMEM) != cudaSuccess)
+            return false;
+        attr = true;
+    }
+    const ExactW& e = it->second;
+    const long long units = (M + BM - 1) / BM;
+    const int grid = (int)(units < n_sm ? units : n_sm);
+    for (int c = 0; c < K / 128; c++) {
+        CUtensorMap ma, m1, m2, m3;
+        const float* pl = e.planes + (size_t)c * 3 * N * 128;
+        if (!make_map(&ma, A + c * 128, M, 128, lda, BM) || !make_map(&m1, pl, N, 128, 128, XBN) ||
+            !make_map(&m2, pl + (size_t)N * 128, N, 128, 128, XBN) || !make_map(&m3, pl + (size_t)2 * N * 128, N, 128, 128, XBN))
+            return false;   // (only possible before the first launch: the driver entry point is missing)
+        XParams p{C, c == 0 ? bias : nullptr, e.cs + (size_t)c * N, M, N, ldc, (accumulate || c > 0) ? 1 : 0};
+        if (act_a) k_gemm_exact<true><<<grid, NUM_THREADS, XSMEM, L.stream>>>(ma, m1, m2, m3, p);
+        else k_gemm_exact<false><<<grid, NUM_THREADS, XSMEM, L.stream>>>(ma, m1, m2, m3, p);
+        KLAUNCH(L);
+    }
+    return true;
+}
 
 // Returns false when the shape is not covered (caller falls back to the SIMT path).
 bool gemm_nt_tc(const Launch& L, const float* A, int lda, const float* Whi, const float* Wlo, int ldw, float* C, int ldc,
