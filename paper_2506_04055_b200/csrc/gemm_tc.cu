@@ -16,6 +16,7 @@
 //   warps 6-9   epilogue     : tcgen05.ld 32x32b (one TMEM lane = one output row per thread), + bias (+ C), st.global
 // The accumulator is double-buffered in TMEM (2 x BN columns), so the epilogue of tile t overlaps the MMAs of t+1.
 #include <cuda.h>
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -239,10 +240,12 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
 // Each output tile walks its K blocks twice: pass 0 streams A through the ring to find the row maxima (exponents
 // e_m), pass 1 streams A (an L2 hit) and the weight slices again, converts A into its three slices in shared memory
 // and runs the MMAs.  Same warp roles and barriers as k_gemm_3xtf32; ACT applies SiLU to A while converting.
-constexpr int XBN = 64, XSTAGES = 2, XPRE = 4;
-constexpr int XW_TILE = XBN * BK * 4;                                   // 8 KB
-constexpr int XSTAGE = 3 * A_TILE_BYTES + 3 * XW_TILE;                  // 72 KB: A slices 1..3 (slice 1 lands as raw A), W slices 1..3
-constexpr int XSMEM = XSTAGES * XSTAGE + XPRE * A_TILE_BYTES + 4 * BM * 4 + 256 + 1024;
+constexpr int XBN = 64, XWST = 3, XRAW = 2;
+constexpr int XSL_BLK = BM * 128;                                       // 16 KB: 128 rows x 64 fp16 (one K half of one slice)
+constexpr int XSL = 3 * 2 * XSL_BLK;                                    // 96 KB: A slices [3][2 K halves], resident per unit
+constexpr int XW_TILE = XBN * 128;                                      // 8 KB: 64 rows x 64 fp16
+constexpr int XW_STAGE = 3 * XW_TILE;                                   // 24 KB: the three weight slices of one (N tile, K half)
+constexpr int XSMEM = XSL + XRAW * A_TILE_BYTES + XWST * XW_STAGE + 4 * BM * 4 + 256 + 1024;
 constexpr int XACC = 4 * XBN;                                           // TMEM columns per accumulator set (S2..S5)
 
 struct XParams {
@@ -255,34 +258,38 @@ struct XParams {
 
 __device__ __forceinline__ float silu_x(float x) { return x / (1.0f + __expf(-x)); }
 
-// Work unit = one 128-row block of A with ALL its N tiles: the row exponents are found once per unit (pass 0, on a
-// separate 4-buffer ring that the producer fills one unit ahead), then every N tile streams A (L2 hits) and its weight
-// slices through the 2-stage main ring (pass 1).
+// Work unit = one 128-row block of A with ALL its N tiles.  The raw fp32 blocks of A stream twice through a small
+// ring (pass 0: row maxima -> exponents; pass 1: conversion, an L2 hit); the fp16 integer slices of the whole block
+// (K = 128) then stay resident while the N tiles run, fed by a 3-stage ring of weight slices.
 template <bool ACT>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
     k_gemm_exact(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapW1,
                  const __grid_constant__ CUtensorMap mapW2, const __grid_constant__ CUtensorMap mapW3, XParams p) {
     extern __shared__ __align__(1024) uint8_t smem[];
-    uint8_t* pre = smem + XSTAGES * XSTAGE;                          // [XPRE] raw A blocks of the next unit
-    float* rowscale = (float*)(pre + XPRE * A_TILE_BYTES);           // [4][BM]  2^(e_m - 14) of the last four units
+    uint8_t* sl = smem;                                               // A slices
+    uint8_t* raw = sl + XSL;                                          // [XRAW] raw A blocks (128 rows x 32 fp32, SWIZZLE_128B)
+    uint8_t* wst = raw + XRAW * A_TILE_BYTES;                         // [XWST] weight-slice stages
+    float* rowscale = (float*)(wst + XWST * XW_STAGE);                // [4][BM]  2^(e_m - 14) of the last four units
     uint64_t* bars = (uint64_t*)(rowscale + 4 * BM);
-    uint64_t* full = bars;                    // [XSTAGES] TMA landed            (count 1 + tx)
-    uint64_t* conv = full + XSTAGES;          // [XSTAGES] A converted           (count 128)
-    uint64_t* empty = conv + XSTAGES;         // [XSTAGES] MMAs done             (count 1, tcgen05.commit)
-    uint64_t* pfull = empty + XSTAGES;        // [XPRE] pass-0 block landed      (count 1 + tx)
-    uint64_t* pempty = pfull + XPRE;          // [XPRE] pass-0 block scanned     (count 128)
-    uint64_t* tfull = pempty + XPRE;          // [2] accumulators ready          (count 1)
-    uint64_t* tempty = tfull + 2;             // [2] accumulators drained        (count 4)
+    uint64_t* rfull = bars;                   // [XRAW] raw block landed          (count 1 + tx)
+    uint64_t* rempty = rfull + XRAW;          // [XRAW] raw block consumed        (count 128)
+    uint64_t* wfull = rempty + XRAW;          // [XWST] weight slices landed      (count 1 + tx)
+    uint64_t* wempty = wfull + XWST;          // [XWST] MMAs of the stage done    (count 1, tcgen05.commit)
+    uint64_t* sl_ready = wempty + XWST;       // [1] A slices of the unit written (count 128)
+    uint64_t* sl_free = sl_ready + 1;         // [1] all MMAs of the unit done    (count 1, tcgen05.commit)
+    uint64_t* tfull = sl_free + 1;            // [2] accumulators ready           (count 1)
+    uint64_t* tempty = tfull + 2;             // [2] accumulators drained         (count 4)
     uint32_t* tmem_slot = (uint32_t*)(tempty + 2);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_tiles = p.N / XBN;
     const long long units = (p.M + BM - 1) / BM;
-    constexpr int kblocks = 128 / BK;         // 4 == XPRE
+    constexpr int kblocks = 128 / BK;         // 4 raw blocks per pass
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < XSTAGES; s++) { mbar_init(&full[s], 1); mbar_init(&conv[s], 128); mbar_init(&empty[s], 1); }
-        for (int s = 0; s < XPRE; s++) { mbar_init(&pfull[s], 1); mbar_init(&pempty[s], 128); }
+        for (int s = 0; s < XRAW; s++) { mbar_init(&rfull[s], 1); mbar_init(&rempty[s], 128); }
+        for (int s = 0; s < XWST; s++) { mbar_init(&wfull[s], 1); mbar_init(&wempty[s], 1); }
+        mbar_init(sl_ready, 128); mbar_init(sl_free, 1);
         for (int b = 0; b < 2; b++) { mbar_init(&tfull[b], 1); mbar_init(&tempty[b], 4); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -293,144 +300,166 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
     const uint32_t tmem_base = *tmem_slot;
 
     if (warp == 0) {
-        // ===================== TMA producer =====================
         if (lane == 0) {
-            int stage = 0;
-            uint32_t phase = 0, pphase = 0;
-            auto preload = [&](long long u) {                         // pass-0 blocks of unit u
-                for (int kb = 0; kb < kblocks; kb++) {
-                    mbar_wait(&pempty[kb], pphase ^ 1);
-                    mbar_expect_tx(&pfull[kb], A_TILE_BYTES);
-                    tma_load_2d(pre + kb * A_TILE_BYTES, &mapA, &pfull[kb], kb * BK, (int)u * BM);
-                }
-                pphase ^= 1;
-            };
-            if ((long long)blockIdx.x < units) preload(blockIdx.x);
-            for (long long u = blockIdx.x; u < units; u += gridDim.x) {
-                const int m0 = (int)u * BM;
-                for (int nt = 0; nt < n_tiles; nt++) {
-                    for (int kb = 0; kb < kblocks; kb++) {
-                        mbar_wait(&empty[stage], phase ^ 1);
-                        uint8_t* st = smem + stage * XSTAGE;
-                        mbar_expect_tx(&full[stage], A_TILE_BYTES + 3 * XW_TILE);
-                        tma_load_2d(st, &mapA, &full[stage], kb * BK, m0);
-                        tma_load_2d(st + 3 * A_TILE_BYTES, &mapW1, &full[stage], kb * BK, nt * XBN);
-                        tma_load_2d(st + 3 * A_TILE_BYTES + XW_TILE, &mapW2, &full[stage], kb * BK, nt * XBN);
-                        tma_load_2d(st + 3 * A_TILE_BYTES + 2 * XW_TILE, &mapW3, &full[stage], kb * BK, nt * XBN);
-                        if (++stage == XSTAGES) { stage = 0; phase ^= 1; }
+            // ===================== TMA producer 1: weight slices =====================
+            int ws = 0;
+            uint32_t wphase = 0;
+            for (long long u = blockIdx.x; u < units; u += gridDim.x)
+                for (int nt = 0; nt < n_tiles; nt++)
+                    for (int kh = 0; kh < 2; kh++) {
+                        mbar_wait(&wempty[ws], wphase ^ 1);
+                        uint8_t* st = wst + ws * XW_STAGE;
+                        mbar_expect_tx(&wfull[ws], XW_STAGE);
+                        tma_load_2d(st, &mapW1, &wfull[ws], kh * 64, nt * XBN);
+                        tma_load_2d(st + XW_TILE, &mapW2, &wfull[ws], kh * 64, nt * XBN);
+                        tma_load_2d(st + 2 * XW_TILE, &mapW3, &wfull[ws], kh * 64, nt * XBN);
+                        if (++ws == XWST) { ws = 0; wphase ^= 1; }
                     }
-                    if (nt == 0 && u + gridDim.x < units) preload(u + gridDim.x);   // next unit's pass 0, one unit ahead
+        } else if (lane == 1) {
+            // ===================== TMA producer 2: raw A blocks, twice per unit =====================
+            int rs = 0;
+            uint32_t rphase = 0;
+            for (long long u = blockIdx.x; u < units; u += gridDim.x)
+                for (int e = 0; e < 2 * kblocks; e++) {
+                    mbar_wait(&rempty[rs], rphase ^ 1);
+                    mbar_expect_tx(&rfull[rs], A_TILE_BYTES);
+                    tma_load_2d(raw + rs * A_TILE_BYTES, &mapA, &rfull[rs], (e & (kblocks - 1)) * BK, (int)u * BM);
+                    if (++rs == XRAW) { rs = 0; rphase ^= 1; }
                 }
-            }
         }
     } else if (warp == 1) {
         // ===================== MMA issuer =====================
         if (lane == 0) {
-            const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(XBN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
-            int stage = 0;
-            uint32_t phase = 0;
+            const uint32_t idesc = (1u << 4) | ((uint32_t)(XBN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);   // f16 x f16 -> f32
+            const uint32_t sl_base = smem_u32(sl);
+            int ws = 0;
+            uint32_t wphase = 0, uphase = 0;
             int buf = 0;
             uint32_t bphase = 0;
             for (long long u = blockIdx.x; u < units; u += gridDim.x) {
+                mbar_wait(sl_ready, uphase);
+                tc_fence_after();
                 for (int nt = 0; nt < n_tiles; nt++) {
                     mbar_wait(&tempty[buf], bphase ^ 1);
                     tc_fence_after();
                     const uint32_t d = tmem_base + buf * XACC;
-                    for (int kb = 0; kb < kblocks; kb++) {
-                        mbar_wait(&conv[stage], phase);
+                    for (int kh = 0; kh < 2; kh++) {
+                        mbar_wait(&wfull[ws], wphase);
                         tc_fence_after();
-                        const uint32_t sa = smem_u32(smem + stage * XSTAGE);
+                        const uint32_t sw = smem_u32(wst + ws * XW_STAGE);
                         uint64_t a[3], w[3];
 #pragma unroll
                         for (int i = 0; i < 3; i++) {
-                            a[i] = make_desc_sw128(sa + i * A_TILE_BYTES);
-                            w[i] = make_desc_sw128(sa + 3 * A_TILE_BYTES + i * XW_TILE);
+                            a[i] = make_desc_sw128(sl_base + (i * 2 + kh) * XSL_BLK);
+                            w[i] = make_desc_sw128(sw + i * XW_TILE);
                         }
 #pragma unroll
-                        for (int kk = 0; kk < BK / 8; kk++) {
-                            const uint64_t o = (uint64_t)(kk * 2);   // 32 B along K inside the swizzle row, >> 4
-                            const uint32_t acc = (kb | kk) != 0;
-                            umma_tf32(d, a[0] + o, w[0] + o, idesc, acc);                   // S2: (1,1)
-                            umma_tf32(d + XBN, a[0] + o, w[1] + o, idesc, acc);             // S3: (1,2) (2,1)
-                            umma_tf32(d + XBN, a[1] + o, w[0] + o, idesc, 1);
-                            umma_tf32(d + 2 * XBN, a[0] + o, w[2] + o, idesc, acc);         // S4: (1,3) (2,2) (3,1)
-                            umma_tf32(d + 2 * XBN, a[1] + o, w[1] + o, idesc, 1);
-                            umma_tf32(d + 2 * XBN, a[2] + o, w[0] + o, idesc, 1);
-                            umma_tf32(d + 3 * XBN, a[1] + o, w[2] + o, idesc, acc);         // S5: (2,3) (3,2)
-                            umma_tf32(d + 3 * XBN, a[2] + o, w[1] + o, idesc, 1);
+                        for (int kk = 0; kk < 4; kk++) {             // 16 fp16 = 32 B along K per MMA
+                            const uint64_t o = (uint64_t)(kk * 2);
+                            const uint32_t acc = (kh | kk) != 0;
+                            umma_f16(d, a[0] + o, w[0] + o, idesc, acc);                   // S2: (1,1)
+                            umma_f16(d + XBN, a[0] + o, w[1] + o, idesc, acc);             // S3: (1,2) (2,1)
+                            umma_f16(d + XBN, a[1] + o, w[0] + o, idesc, 1);
+                            umma_f16(d + 2 * XBN, a[0] + o, w[2] + o, idesc, acc);         // S4: (1,3) (2,2) (3,1)
+                            umma_f16(d + 2 * XBN, a[1] + o, w[1] + o, idesc, 1);
+                            umma_f16(d + 2 * XBN, a[2] + o, w[0] + o, idesc, 1);
+                            umma_f16(d + 3 * XBN, a[1] + o, w[2] + o, idesc, acc);         // S5: (2,3) (3,2)
+                            umma_f16(d + 3 * XBN, a[2] + o, w[1] + o, idesc, 1);
                         }
-                        umma_commit(&empty[stage]);
-                        if (++stage == XSTAGES) { stage = 0; phase ^= 1; }
+                        umma_commit(&wempty[ws]);
+                        if (++ws == XWST) { ws = 0; wphase ^= 1; }
                     }
                     umma_commit(&tfull[buf]);
                     if (++buf == 2) { buf = 0; bphase ^= 1; }
                 }
+                umma_commit(sl_free);
+                uphase ^= 1;
             }
         }
     } else if (warp < EPI_WARP0) {
-        // ===================== converter: row maxima (pass 0), integer slices (pass 1) =====================
-        const int ct = threadIdx.x - CONV_WARP0 * 32;   // 0..127; chunk idx = ct + 128 i lies in row (ct >> 3) + 16 i
-        int stage = 0;
-        uint32_t phase = 0, pphase = 0;
+        // ===================== converter: row maxima (pass 0), fp16 integer slices (pass 1) =====================
+        // thread ct handles the 32-byte chunk PAIRS id = ct + 128 i (i < 4): row r = id >> 2 = (ct >> 2) + 32 i, physical
+        // pair pp = ct & 3.  SWIZZLE_128B stores logical 16-byte chunk c of row r at chunk c ^ (r & 7), so the pair holds
+        // the 8 consecutive K values of logical pair pp ^ ((r & 7) >> 1), the two halves swapped when r is odd.
+        const int ct = threadIdx.x - CONV_WARP0 * 32;
+        const int pp = ct & 3, r0 = ct >> 2;
+        int rs = 0;
+        uint32_t rphase = 0, uphase = 0;
         uint32_t ucount = 0;
         const float MAGIC = 12582912.0f;                // 1.5 * 2^23: (t + MAGIC) - MAGIC = round-to-nearest-even integer
         for (long long u = blockIdx.x; u < units; u += gridDim.x, ucount++) {
-            float mx[8];
+            float mx[4];
 #pragma unroll
-            for (int i = 0; i < 8; i++) mx[i] = 0.f;
+            for (int i = 0; i < 4; i++) mx[i] = 0.f;
             for (int kb = 0; kb < kblocks; kb++) {
-                mbar_wait(&pfull[kb], pphase);
-                const float4* a = (const float4*)(pre + kb * A_TILE_BYTES);
+                mbar_wait(&rfull[rs], rphase);
+                const float4* a = (const float4*)(raw + rs * A_TILE_BYTES);
 #pragma unroll
-                for (int i = 0; i < 8; i++) {
-                    float4 x = a[ct + i * 128];
-                    if (ACT) { x.x = silu_x(x.x); x.y = silu_x(x.y); x.z = silu_x(x.z); x.w = silu_x(x.w); }
-                    mx[i] = fmaxf(mx[i], fmaxf(fmaxf(fabsf(x.x), fabsf(x.y)), fmaxf(fabsf(x.z), fabsf(x.w))));
+                for (int i = 0; i < 4; i++) {
+#pragma unroll
+                    for (int h = 0; h < 2; h++) {
+                        float4 x = a[(ct + i * 128) * 2 + h];
+                        if (ACT) { x.x = silu_x(x.x); x.y = silu_x(x.y); x.z = silu_x(x.z); x.w = silu_x(x.w); }
+                        mx[i] = fmaxf(mx[i], fmaxf(fmaxf(fabsf(x.x), fabsf(x.y)), fmaxf(fabsf(x.z), fabsf(x.w))));
+                    }
                 }
-                mbar_arrive(&pempty[kb]);
+                mbar_arrive(&rempty[rs]);
+                if (++rs == XRAW) { rs = 0; rphase ^= 1; }
             }
-            pphase ^= 1;
-            float q128[8];                               // 128 / 2^e_m
+            float q128[4];                               // 128 / 2^e_m
 #pragma unroll
-            for (int i = 0; i < 8; i++) {
+            for (int i = 0; i < 4; i++) {
                 float m = mx[i];
                 m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));
                 m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
-                m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 4));
                 // 2^e = smallest power of two > m; non-finite / huge rows fall through as garbage / NaN downstream
                 const uint32_t E = (__float_as_uint(m) >> 23) & 0xffu;       // m in [2^(E-127), 2^(E-126))
                 const uint32_t Ec = E < 20u ? 20u : (E > 230u ? 230u : E);   // keep every scale a normal number
                 q128[i] = __uint_as_float((260u - Ec) << 23);                // 2^(126 - E) * 128
-                if ((ct & 7) == 0) rowscale[(ucount & 3) * BM + (ct >> 3) + 16 * i] = __uint_as_float((Ec - 13u) << 23);   // 2^(e - 14)
+                if (pp == 0) rowscale[(ucount & 3) * BM + r0 + 32 * i] = __uint_as_float((Ec - 13u) << 23);   // 2^(e - 14)
             }
-            for (int e = 0; e < n_tiles * kblocks; e++) {
-                mbar_wait(&full[stage], phase);
-                float4* a1 = (float4*)(smem + stage * XSTAGE);
-                float4* a2 = (float4*)(smem + stage * XSTAGE + A_TILE_BYTES);
-                float4* a3 = (float4*)(smem + stage * XSTAGE + 2 * A_TILE_BYTES);
+            mbar_wait(sl_free, uphase ^ 1);              // the previous unit's MMAs no longer read the slices
+            uphase ^= 1;
+            for (int kb = 0; kb < kblocks; kb++) {
+                mbar_wait(&rfull[rs], rphase);
+                const float4* a = (const float4*)(raw + rs * A_TILE_BYTES);
+                const int kh = kb >> 1;
 #pragma unroll
-                for (int i = 0; i < 8; i++) {
-                    const int idx = ct + i * 128;
-                    float4 x = a1[idx];
-                    if (ACT) { x.x = silu_x(x.x); x.y = silu_x(x.y); x.z = silu_x(x.z); x.w = silu_x(x.w); }
-                    float4 s1, s2, s3;
-#define XSLICE(C)                                                            \
-    {                                                                        \
-        const float t1_ = x.C * q128[i];                                     \
-        s1.C = (t1_ + MAGIC) - MAGIC;                                        \
-        const float t2_ = (t1_ - s1.C) * 256.0f;                             \
-        s2.C = (t2_ + MAGIC) - MAGIC;                                        \
-        const float t3_ = (t2_ - s2.C) * 256.0f;                             \
-        s3.C = (t3_ + MAGIC) - MAGIC;                                        \
-    }
-                    XSLICE(x) XSLICE(y) XSLICE(z) XSLICE(w)
-#undef XSLICE
-                    a1[idx] = s1; a2[idx] = s2; a3[idx] = s3;
+                for (int i = 0; i < 4; i++) {
+                    const int r = r0 + 32 * i;
+                    float4 lo = a[(ct + i * 128) * 2], hi = a[(ct + i * 128) * 2 + 1];
+                    if (r & 1) { const float4 t = lo; lo = hi; hi = t; }
+                    float x[8] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
+                    float s1[8], s2[8], s3[8];
+#pragma unroll
+                    for (int j = 0; j < 8; j++) {
+                        const float xv = ACT ? silu_x(x[j]) : x[j];
+                        const float t1 = xv * q128[i];
+                        s1[j] = (t1 + MAGIC) - MAGIC;
+                        const float t2 = (t1 - s1[j]) * 256.0f;
+                        s2[j] = (t2 + MAGIC) - MAGIC;
+                        const float t3 = (t2 - s2[j]) * 256.0f;
+                        s3[j] = (t3 + MAGIC) - MAGIC;
+                    }
+                    // logical fp16 chunk of this (row, 8 K values) inside the 64-wide K half, and its swizzled position
+                    const int c16 = ((kb & 1) * 4 + (pp ^ ((r & 7) >> 1))) ^ (r & 7);
+                    uint8_t* dst = sl + kh * XSL_BLK + r * 128 + c16 * 16;
+                    __half2 h1[4], h2[4], h3[4];
+#pragma unroll
+                    for (int j = 0; j < 4; j++) {
+                        h1[j] = __floats2half2_rn(s1[2 * j], s1[2 * j + 1]);
+                        h2[j] = __floats2half2_rn(s2[2 * j], s2[2 * j + 1]);
+                        h3[j] = __floats2half2_rn(s3[2 * j], s3[2 * j + 1]);
+                    }
+                    *(uint4*)(dst) = *(uint4*)h1;
+                    *(uint4*)(dst + 2 * XSL_BLK) = *(uint4*)h2;
+                    *(uint4*)(dst + 4 * XSL_BLK) = *(uint4*)h3;
                 }
-                fence_async_smem();
-                mbar_arrive(&conv[stage]);
-                if (++stage == XSTAGES) { stage = 0; phase ^= 1; }
+                mbar_arrive(&rempty[rs]);
+                if (++rs == XRAW) { rs = 0; rphase ^= 1; }
             }
+            fence_async_smem();
+            mbar_arrive(sl_ready);
         }
     } else {
         // ===================== epilogue =====================
@@ -520,6 +549,18 @@ static bool make_map(CUtensorMap* map, const float* ptr, long long rows, int col
                CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// fp16 weight-slice plane [rows x 128], box = 64 halfs (128 B, one swizzle row) x box_rows
+static bool make_map16(CUtensorMap* map, const __half* ptr, int rows, int box_rows) {
+    EncodeTiledFn enc = get_encode();
+    if (!enc) return false;
+    cuuint64_t dims[2] = {128, (cuuint64_t)rows};
+    cuuint64_t strides[1] = {128 * 2};
+    cuuint32_t box[2] = {64, (cuuint32_t)box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, (void*)ptr, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 template <int BN, int STAGES>
 static bool launch(const Launch& L, const CUtensorMap& a, const CUtensorMap& whi, const CUtensorMap& wlo, Params p,
                    int n_sm) {
@@ -542,7 +583,7 @@ static bool launch(const Launch& L, const CUtensorMap& a, const CUtensorMap& whi
 // ---- exact integer-slice path: weight slices are cut once, at create ----
 struct ExactW {
     int N, K;
-    float* planes;     // device [K / 128][3][N][128]  integer-valued slices t1, t2, t3
+    __half* planes;    // device [K / 128][3][N][128]  integer-valued fp16 slices t1, t2, t3
     float* cs;         // device [K / 128][N]          2^f_n
 };
 static std::unordered_map<const float*, ExactW> g_exact;
@@ -550,7 +591,8 @@ static std::unordered_map<const float*, ExactW> g_exact;
 void gemm_register_exact(const float* Wdev, const float* Whost, int N, int K) {
     if (K % 128 != 0 || N % tc::XBN != 0 || g_exact.count(Wdev)) return;
     const int nc = K / 128;
-    std::vector<float> pl((size_t)nc * 3 * N * 128), cs((size_t)nc * N);
+    std::vector<__half> pl((size_t)nc * 3 * N * 128);
+    std::vector<float> cs((size_t)nc * N);
     for (int c = 0; c < nc; c++)
         for (int n = 0; n < N; n++) {
             const float* w = Whost + (size_t)n * K + c * 128;
@@ -567,15 +609,15 @@ void gemm_register_exact(const float* Wdev, const float* Whost, int N, int K) {
                 const float t2 = (t1 - s1) * 256.0f;
                 const float s2 = std::nearbyint(t2);
                 const float s3 = std::nearbyint((t2 - s2) * 256.0f);
-                pl[(((size_t)c * 3 + 0) * N + n) * 128 + k] = s1;
-                pl[(((size_t)c * 3 + 1) * N + n) * 128 + k] = s2;
-                pl[(((size_t)c * 3 + 2) * N + n) * 128 + k] = s3;
+                pl[(((size_t)c * 3 + 0) * N + n) * 128 + k] = __float2half_rn(s1);      // |s| <= 128: exact in fp16
+                pl[(((size_t)c * 3 + 1) * N + n) * 128 + k] = __float2half_rn(s2);
+                pl[(((size_t)c * 3 + 2) * N + n) * 128 + k] = __float2half_rn(s3);
             }
         }
     ExactW e{N, K, nullptr, nullptr};
-    if (cudaMalloc(&e.planes, pl.size() * 4) != cudaSuccess) return;
+    if (cudaMalloc(&e.planes, pl.size() * 2) != cudaSuccess) return;
     if (cudaMalloc(&e.cs, cs.size() * 4) != cudaSuccess) { cudaFree(e.planes); return; }
-    cudaMemcpy(e.planes, pl.data(), pl.size() * 4, cudaMemcpyHostToDevice);
+    cudaMemcpy(e.planes, pl.data(), pl.size() * 2, cudaMemcpyHostToDevice);
     cudaMemcpy(e.cs, cs.data(), cs.size() * 4, cudaMemcpyHostToDevice);
     g_exact[Wdev] = e;
 }
@@ -613,9 +655,9 @@ bool gemm_nt_exact(const Launch& L, const float* A, int lda, const float* W, flo
     const int grid = (int)(units < n_sm ? units : n_sm);
     for (int c = 0; c < K / 128; c++) {
         CUtensorMap ma, m1, m2, m3;
-        const float* pl = e.planes + (size_t)c * 3 * N * 128;
-        if (!make_map(&ma, A + c * 128, M, 128, lda, BM) || !make_map(&m1, pl, N, 128, 128, XBN) ||
-            !make_map(&m2, pl + (size_t)N * 128, N, 128, 128, XBN) || !make_map(&m3, pl + (size_t)2 * N * 128, N, 128, 128, XBN))
+        const __half* pl = e.planes + (size_t)c * 3 * N * 128;
+        if (!make_map(&ma, A + c * 128, M, 128, lda, BM) || !make_map16(&m1, pl, N, XBN) ||
+            !make_map16(&m2, pl + (size_t)N * 128, N, XBN) || !make_map16(&m3, pl + (size_t)2 * N * 128, N, XBN))
             return false;   // (only possible before the first launch: the driver entry point is missing)
         XParams p{C, c == 0 ? bias : nullptr, e.cs + (size_t)c * N, M, N, ldc, (accumulate || c > 0) ? 1 : 0};
         if (act_a) k_gemm_exact<true><<<grid, NUM_THREADS, XSMEM, L.stream>>>(ma, m1, m2, m3, p);
