@@ -240,12 +240,13 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
 // Each output tile walks its K blocks twice: pass 0 streams A through the ring to find the row maxima (exponents
 // e_m), pass 1 streams A (an L2 hit) and the weight slices again, converts A into its three slices in shared memory
 // and runs the MMAs.  Same warp roles and barriers as k_gemm_3xtf32; ACT applies SiLU to A while converting.
-constexpr int XBN = 64, XWST = 3, XRAW = 2;
+constexpr int XBN = 64, XWST = 3, XRAW = 3;
 constexpr int XSL_BLK = BM * 128;                                       // 16 KB: 128 rows x 64 fp16 (one K half of one slice)
 constexpr int XSL = 3 * 2 * XSL_BLK;                                    // 96 KB: A slices [3][2 K halves], resident per unit
 constexpr int XW_TILE = XBN * 128;                                      // 8 KB: 64 rows x 64 fp16
 constexpr int XW_STAGE = 3 * XW_TILE;                                   // 24 KB: the three weight slices of one (N tile, K half)
-constexpr int XSMEM = XSL + XRAW * A_TILE_BYTES + XWST * XW_STAGE + 4 * BM * 4 + 256 + 1024;
+constexpr int XNMAX = 512;                                              // widest N (column scale and bias are staged in shared memory)
+constexpr int XSMEM = XSL + XRAW * A_TILE_BYTES + XWST * XW_STAGE + 4 * BM * 4 + 2 * XNMAX * 4 + 256 + 1024;
 constexpr int XACC = 4 * XBN;                                           // TMEM columns per accumulator set (S2..S5)
 
 struct XParams {
@@ -270,7 +271,9 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
     uint8_t* raw = sl + XSL;                                          // [XRAW] raw A blocks (128 rows x 32 fp32, SWIZZLE_128B)
     uint8_t* wst = raw + XRAW * A_TILE_BYTES;                         // [XWST] weight-slice stages
     float* rowscale = (float*)(wst + XWST * XW_STAGE);                // [4][BM]  2^(e_m - 14) of the last four units
-    uint64_t* bars = (uint64_t*)(rowscale + 4 * BM);
+    float* s_cs = rowscale + 4 * BM;                                  // [N] column scales 2^f_n
+    float* s_bias = s_cs + XNMAX;                                     // [N] bias (zeros when absent)
+    uint64_t* bars = (uint64_t*)(s_bias + XNMAX);
     uint64_t* rfull = bars;                   // [XRAW] raw block landed          (count 1 + tx)
     uint64_t* rempty = rfull + XRAW;          // [XRAW] raw block consumed        (count 128)
     uint64_t* wfull = rempty + XRAW;          // [XWST] weight slices landed      (count 1 + tx)
@@ -294,6 +297,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 1) tmem_alloc(tmem_slot, 512);
+    for (int i = threadIdx.x; i < p.N; i += NUM_THREADS) { s_cs[i] = p.colscale[i]; s_bias[i] = p.bias ? p.bias[i] : 0.0f; }
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -321,6 +325,11 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
             uint32_t rphase = 0;
             for (long long u = blockIdx.x; u < units; u += gridDim.x)
                 for (int e = 0; e < 2 * kblocks; e++) {
+                    // pull the next unit's rows into L2 while this unit is processed (its pass 0 is then an L2 hit too)
+                    if (e < kblocks && u + gridDim.x < units)
+                        asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global [%0, {%1, %2}];" ::"l"(&mapA), "r"(e * BK),
+                                     "r"((int)(u + gridDim.x) * BM)
+                                     : "memory");
                     mbar_wait(&rempty[rs], rphase ^ 1);
                     mbar_expect_tx(&rfull[rs], A_TILE_BYTES);
                     tma_load_2d(raw + rs * A_TILE_BYTES, &mapA, &rfull[rs], (e & (kblocks - 1)) * BK, (int)u * BM);
@@ -492,7 +501,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
                     if (row < p.M) {
 #pragma unroll
                         for (int c = 0; c < 16; c += 4) {
-                            const float4 cs = *(const float4*)(p.colscale + n0 + c0 + c);
+                            const float4 cs = *(const float4*)(s_cs + n0 + c0 + c);
                             float v[4];
 #pragma unroll
                             for (int j = 0; j < 4; j++) {
@@ -500,8 +509,8 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
                                 v[j] = fmaf(lo, 1.0f / 65536.0f, fmaf(__uint_as_float(r3[c + j]), 1.0f / 256.0f, __uint_as_float(r2[c + j])));
                             }
                             float4 y = make_float4(v[0] * (rs * cs.x), v[1] * (rs * cs.y), v[2] * (rs * cs.z), v[3] * (rs * cs.w));
-                            if (p.bias) {
-                                const float4 b = *(const float4*)(p.bias + n0 + c0 + c);
+                            {
+                                const float4 b = *(const float4*)(s_bias + n0 + c0 + c);
                                 y.x += b.x; y.y += b.y; y.z += b.z; y.w += b.w;
                             }
                             if (p.accumulate) { y.x += o[c / 4].x; y.y += o[c / 4].y; y.z += o[c / 4].z; y.w += o[c / 4].w; }
@@ -636,7 +645,7 @@ bool gemm_nt_exact(const Launch& L, const float* A, int lda, const float* W, flo
     using namespace tc;
     auto it = g_exact.find(W);
     if (it == g_exact.end() || it->second.N != N || it->second.K != K) return false;
-    if (M <= 0 || (lda % 4) || (ldc % 4) || (((uintptr_t)A | (uintptr_t)C | (uintptr_t)bias) & 15)) return false;
+    if (M <= 0 || N > XNMAX || (lda % 4) || (ldc % 4) || (((uintptr_t)A | (uintptr_t)C | (uintptr_t)bias) & 15)) return false;
     static int n_sm = 0;
     static bool attr = false;
     if (!n_sm) {
