@@ -76,6 +76,7 @@ struct mlp_model {
     std::vector<std::pair<int, cudaEvent_t>> marks;
     long long forced_edge_cap = 0;
     bool fwd_tc = false;   // run the forward GEMMs on tensor cores too (faster, biased energy)
+    bool bwd_exact = false;   // adjoint GEMMs through the exact integer-slice kernel instead of 3xTF32
 };
 
 namespace {
@@ -272,7 +273,9 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
     };
     auto upT = [&](const std::vector<float>& v, int rows, int cols, float** dst) {
         if (rcode != MLP_OK) return;
-        rcode = upload_gemm_weight(m, transpose(v, rows, cols), dst);
+        const std::vector<float> t = transpose(v, rows, cols);          // [cols x rows]
+        rcode = upload_gemm_weight(m, t, dst);
+        if (rcode == MLP_OK) painn::gemm_register_exact(*dst, t.data(), cols, rows);
     };
     up((size_t)ns * F, &m->Emb);
     for (int t = 0; t < T; t++) {
@@ -369,6 +372,7 @@ __attribute__((visibility("default"))) int mlp_set_option(mlp_model* m, const ch
     if (!strcmp(name, "gemm_emulate")) { painn::g_gemm_emulate = (int)value; return MLP_OK; }
     if (!strcmp(name, "edge_path")) { m->edge_path = (int)value; return MLP_OK; }
     if (!strcmp(name, "gemm_fwd_tc")) { m->fwd_tc = value != 0; return MLP_OK; }
+    if (!strcmp(name, "gemm_bwd_exact")) { m->bwd_exact = value != 0; return MLP_OK; }
     if (!strcmp(name, "gemm_path")) { painn::g_gemm_path = (int)value; return MLP_OK; }
     if (!strcmp(name, "gemm_fwd_exact")) { painn::g_gemm_fwd_exact = (int)value; return MLP_OK; }
     if (!strcmp(name, "filter_emulate")) { painn::g_filter_emulate = (int)value; return MLP_OK; }
@@ -574,7 +578,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
             P<float>(m->b_eatom), P<double>(m->b_epart), &n_epart);
 
     // ---- backward ----
-    painn::g_gemm_path = saved_path;
+    painn::g_gemm_path = m->bwd_exact ? 1 : saved_path;
     mark(m, st, ST_BWD_NODE);
     float *sb = P<float>(m->b_sb), *s1b = P<float>(m->b_s1b), *vb = P<float>(m->b_vb), *v1b = P<float>(m->b_v1b);
     gemm_nt(L, P<float>(m->b_rb), R, m->Wr1T, R, sb, F, N, F, R, nullptr, false);
@@ -614,6 +618,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         std::swap(sb, s1b);
     }
 
+    painn::g_gemm_path = saved_path;
     // ---- forces, ghost fold, virial, energy ----
     mark(m, st, ST_FORCE);
     if (N > 0) CU(m, cudaMemsetAsync(forces, 0, (size_t)N * 3 * 8, st));

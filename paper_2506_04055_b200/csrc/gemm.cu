@@ -202,7 +202,10 @@ void gemm_nt_act(const Launch& L, const float* A, int lda, const float* B, int l
     if (M == 0) return;
     const bool fast_ok = g_gemm_emulate == 0 && N % 128 == 0 && K % 8 == 0 && lda % 4 == 0 && ldb % 4 == 0 &&
                          ldc % 4 == 0 && ((((uintptr_t)A | (uintptr_t)B | (uintptr_t)C | (uintptr_t)bias) & 15) == 0);
-    if ((act_a || g_gemm_path == 1) && g_gemm_fwd_exact && g_gemm_emulate == 0 &&
+    static int fwd_call = 0;                                   // debug: g_gemm_fwd_exact >= 2 is a bit mask over the
+    const int call_type = (act_a || g_gemm_path == 1) ? (fwd_call++ % 16) % 5 : 0;   // forward GEMM types 0..4 (bits 1..5)
+    const bool want_exact = g_gemm_fwd_exact == 1 || (g_gemm_fwd_exact >= 2 && ((g_gemm_fwd_exact >> (1 + call_type)) & 1));
+    if ((act_a || g_gemm_path == 1) && want_exact && g_gemm_emulate == 0 &&
         gemm_nt_exact(L, A, lda, B, C, ldc, M, N, K, bias, accumulate, act_a)) {
         g_last_gemm_tc = 1;
         return;

@@ -241,6 +241,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
 // e_m), pass 1 streams A (an L2 hit) and the weight slices again, converts A into its three slices in shared memory
 // and runs the MMAs.  Same warp roles and barriers as k_gemm_3xtf32; ACT applies SiLU to A while converting.
 constexpr int XBN = 64, XWST = 3, XRAW = 3;
+constexpr int XTHREADS = NUM_THREADS + 32;                              // + warp 10: second TMA producer (raw A blocks)
 constexpr int XSL_BLK = BM * 128;                                       // 16 KB: 128 rows x 64 fp16 (one K half of one slice)
 constexpr int XSL = 3 * 2 * XSL_BLK;                                    // 96 KB: A slices [3][2 K halves], resident per unit
 constexpr int XW_TILE = XBN * 128;                                      // 8 KB: 64 rows x 64 fp16
@@ -263,7 +264,7 @@ __device__ __forceinline__ float silu_x(float x) { return x / (1.0f + __expf(-x)
 // ring (pass 0: row maxima -> exponents; pass 1: conversion, an L2 hit); the fp16 integer slices of the whole block
 // (K = 128) then stay resident while the N tiles run, fed by a 3-stage ring of weight slices.
 template <bool ACT>
-__global__ void __launch_bounds__(NUM_THREADS, 1)
+__global__ void __launch_bounds__(XTHREADS, 1)
     k_gemm_exact(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapW1,
                  const __grid_constant__ CUtensorMap mapW2, const __grid_constant__ CUtensorMap mapW3, XParams p) {
     extern __shared__ __align__(1024) uint8_t smem[];
@@ -297,7 +298,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 1) tmem_alloc(tmem_slot, 512);
-    for (int i = threadIdx.x; i < p.N; i += NUM_THREADS) { s_cs[i] = p.colscale[i]; s_bias[i] = p.bias ? p.bias[i] : 0.0f; }
+    for (int i = threadIdx.x; i < p.N; i += XTHREADS) { s_cs[i] = p.colscale[i]; s_bias[i] = p.bias ? p.bias[i] : 0.0f; }
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -319,7 +320,12 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
                         tma_load_2d(st + 2 * XW_TILE, &mapW3, &wfull[ws], kh * 64, nt * XBN);
                         if (++ws == XWST) { ws = 0; wphase ^= 1; }
                     }
-        } else if (lane == 1) {
+        }
+    } else if (warp == 10) {
+        // The two TMA producers must not share a warp: UTMALDG / SYNCS run on the warp's uniform datapath, and two
+        // divergent spinning lanes of one warp clobbered each other's uniform registers (measured: ~2 % of the pass-0
+        // blocks landed with wrong coordinates).
+        if (lane == 0) {
             // ===================== TMA producer 2: raw A blocks, twice per unit =====================
             int rs = 0;
             uint32_t rphase = 0;
@@ -412,6 +418,11 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
                         mx[i] = fmaxf(mx[i], fmaxf(fmaxf(fabsf(x.x), fabsf(x.y)), fmaxf(fabsf(x.z), fabsf(x.w))));
                     }
                 }
+                // Release to the TMA producer.  The refill is an ASYNC-proxy write to bytes this thread has just read through
+                // the generic proxy: without a proxy fence the two are not ordered even across the mbarrier (measured: ~2 %
+                // of the rows saw part of the next block in pass 0 and got a different, still valid, exponent run to run).
+                asm volatile("" ::"f"(mx[0]), "f"(mx[1]), "f"(mx[2]), "f"(mx[3]) : "memory");
+                fence_async_smem();
                 mbar_arrive(&rempty[rs]);
                 if (++rs == XRAW) { rs = 0; rphase ^= 1; }
             }
@@ -464,13 +475,14 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
                     *(uint4*)(dst + 2 * XSL_BLK) = *(uint4*)h2;
                     *(uint4*)(dst + 4 * XSL_BLK) = *(uint4*)h3;
                 }
+                fence_async_smem();                      // same cross-proxy release as in pass 0
                 mbar_arrive(&rempty[rs]);
                 if (++rs == XRAW) { rs = 0; rphase ^= 1; }
             }
             fence_async_smem();
             mbar_arrive(sl_ready);
         }
-    } else {
+    } else if (warp < 10) {
         // ===================== epilogue =====================
         const int q = warp & 3;                      // TMEM lane quadrant this warp may access
         int buf = 0;
@@ -669,8 +681,8 @@ bool gemm_nt_exact(const Launch& L, const float* A, int lda, const float* W, flo
             !make_map16(&m2, pl + (size_t)N * 128, N, XBN) || !make_map16(&m3, pl + (size_t)2 * N * 128, N, XBN))
             return false;   // (only possible before the first launch: the driver entry point is missing)
         XParams p{C, c == 0 ? bias : nullptr, e.cs + (size_t)c * N, M, N, ldc, (accumulate || c > 0) ? 1 : 0};
-        if (act_a) k_gemm_exact<true><<<grid, NUM_THREADS, XSMEM, L.stream>>>(ma, m1, m2, m3, p);
-        else k_gemm_exact<false><<<grid, NUM_THREADS, XSMEM, L.stream>>>(ma, m1, m2, m3, p);
+        if (act_a) k_gemm_exact<true><<<grid, XTHREADS, XSMEM, L.stream>>>(ma, m1, m2, m3, p);
+        else k_gemm_exact<false><<<grid, XTHREADS, XSMEM, L.stream>>>(ma, m1, m2, m3, p);
         KLAUNCH(L);
     }
     return true;
