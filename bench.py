@@ -138,9 +138,13 @@ def _stage_work(stats, model, n_atoms):
     E, N = stats["n_edges"], n_atoms
     R = F // 2
     w = {}
-    # edge stages: filter (2 * 3F * (K+1) flop) + products/segment sums; adjoint evaluates filter and its derivative
-    w["fwd_edge"] = ("alu", T * E * (2.0 * 3 * F * (K + 1) + 2.0 * 8 * F), "flop")
-    w["bwd_edge"] = ("alu", T * E * (2.0 * 2 * 3 * F * (K + 1) + 2.0 * 24 * F), "flop")
+    # edge stages: compulsory HBM bytes (every per-atom row and per-edge record moved once per launch; DESIGN.md
+    # section 6).  The kernels are bound by the L2 -> SM row gather (reported separately as roofline.l2_gather), so
+    # the HBM fraction states how far that keeps them from the DRAM roof.
+    fwd_atom = (2 * F * 4 + F * 4 + 4 * F * 4) + (T - 1) * (5 * F * 4 + F * 4 + 3 * F * 4 + 4 * F * 4)   # gather rows + residual + outputs
+    w["fwd_edge"] = ("hbm", N * float(fwd_atom) + T * E * 16.0, "B")
+    bwd_atom = (4 * F * 4 + 2 * F * 4) + (T - 1) * (4 * F * 4 + 9 * F * 4 + 6 * F * 4)              # gather rows + own rows + sender adjoint
+    w["bwd_edge"] = ("hbm", N * float(bwd_atom) + E * (16.0 * T + 16.0 + 32.0 * (T - 1)), "B")
     # node GEMMs (flop), fwd: phi-MLP F->F->3F, U|V (3 comps) F->2F, update MLP 2F->F->3F ; readout F->R
     fwd = T * N * 2.0 * (F * F + 3 * F * F + 3 * 2 * F * F + 2 * F * F + 3 * F * F) + N * 2.0 * F * R
     w["fwd_node"] = ("tensor", fwd, "flop")
@@ -250,22 +254,45 @@ def main():
     m.set_option("stage_timing", 0)
     peaks = _peaks()
     work = _stage_work(stats, model, N)
-    dom = max(acc, key=acc.get)
-    bound, units, _ = work[dom]
     T = model["T"]
-    n_launch = {"fwd_edge": T, "bwd_edge": T}.get(dom, 1)
+    n_launch_of = {"fwd_edge": T, "bwd_edge": T}
+
+    def _roof(name):
+        bound, units, _ = work[name]
+        if bound == "hbm":
+            ach, peak, unit = units / (acc[name] * 1e-3) / 1e9, peaks["hbm"], "GB/s"
+        elif bound == "tensor":
+            # forward: exact fp16 integer-slice kernel, adjoint: 3xTF32; both are rated against the peak of their
+            # operand type: fp16 = measured bf16 (sustained, timed inside a long step), tf32 = that x 1.1 / 2.25
+            peak = peaks["bf16_sus"] * (1.0 if name == "fwd_node" else 1.1 / 2.25)
+            ach, unit = units / (acc[name] * 1e-3) / 1e12, "TFLOP/s"
+        else:
+            # plain fp32 ALU: 148 SMs x 128 FMA lanes x 2 flop x max SM clock (B200_PROFILING.md nominal table)
+            ach, peak, unit = units / (acc[name] * 1e-3) / 1e12, 148 * 128 * 2 * peaks["sm_max"] * 1e6 / 1e12, "TFLOP/s"
+        return dict(bound=bound, achieved=ach, peak=peak, unit=unit, frac=ach / peak, ms=round(acc[name], 4))
+
+    stages = {name: _roof(name) for name in acc if name in work}
+    dom = max(acc, key=acc.get)
+    n_launch = n_launch_of.get(dom, 1)
     dur_ms = acc[dom] / n_launch
-    if bound == "hbm":
-        achieved, peak, unit = units / n_launch / (dur_ms * 1e-3) / 1e9, peaks["hbm"], "GB/s"
-    elif bound == "tensor":
-        # 3xTF32 / TF32 path: tf32 peak = measured bf16 peak x nominal ratio 1.1/2.25 (B200_PROFILING.md table)
-        achieved, peak, unit = units / n_launch / (dur_ms * 1e-3) / 1e12, peaks["bf16_sus"] * (1.1 / 2.25), "TFLOP/s"
-    else:
-        # plain fp32 ALU: 148 SMs x 128 FMA lanes x 2 flop x max SM clock (B200_PROFILING.md nominal table)
-        achieved, peak, unit = units / n_launch / (dur_ms * 1e-3) / 1e12, 148 * 128 * 2 * peaks["sm_max"] * 1e6 / 1e12, "TFLOP/s"
-    roofline = dict(kernel=dom, bound=bound, achieved=achieved, peak=peak, unit=unit, frac=achieved / peak,
-                    traffic=None, peak_source=peaks["src"], launches_per_step=n_launch, ms_per_launch=dur_ms,
-                    stage_ms={kk: round(v, 4) for kk, v in acc.items()})
+    # DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/r01_traffic.json)
+    traffic = None
+    try:
+        tj = json.load(open(os.path.join(ROOT, "profiles", "r01_traffic.json")))
+        if k == tj.get("config"):
+            traffic = tj["dram_bytes_per_launch"].get(dom)
+    except Exception:
+        traffic = None
+    roofline = dict(kernel=dom, **{kk: stages[dom][kk] for kk in ("bound", "achieved", "peak", "unit", "frac")},
+                    traffic=traffic, peak_source=peaks["src"], launches_per_step=n_launch, ms_per_launch=dur_ms,
+                    stage_ms={kk: round(v, 4) for kk, v in acc.items()}, stages=stages)
+    if dom in ("fwd_edge", "bwd_edge"):
+        # the edge kernels are bound by the L2 -> SM row gather, not by DRAM: bytes gathered per edge and channel
+        # against the measured gather ceiling of this access pattern (profiles/r01_microbench.md)
+        per_edge = {"fwd_edge": (8.0 + 20.0 * (T - 1)) / T, "bwd_edge": 16.0}[dom] * model["F"]
+        gb = stats["n_edges"] * per_edge / (dur_ms * 1e-3) / 1e9
+        roofline["l2_gather"] = dict(achieved=gb, peak=16200.0, unit="GB/s", frac=gb / 16200.0,
+                                     peak_source="measured row-gather microbenchmark (512 B per warp request)")
 
     # ---- end to end through the host-buffer entry point (pinned host memory, copies inside the timed region) ----
     hpos = torch.from_numpy(c["pos"]).pin_memory()
@@ -303,7 +330,7 @@ def main():
                                 l2="working set (tens of GB) far larger than the 126 MB L2; no explicit flush",
                                 multi_gpu="replicas only (one evaluation does not shard; BASELINE.json fixes 1 GPU)",
                                 options=opts or "defaults",
-                                precision="fp64 cutoff predicate, fp32 edge math and node state, 3xTF32/fp32 GEMMs"),
+                                precision="fp64 cutoff predicate, fp32 edge math and node state, forward GEMMs exact (fp16 integer slices on tcgen05), adjoint GEMMs 3xTF32"),
                     clocks=clocks, e2e=e2e, gpu_launches=launches, roofline=roofline, cpu_baseline=cpu)
         print(json.dumps(line))
     if dist is not None:

@@ -42,6 +42,7 @@ struct mlp_model {
     void* filt_img[PAINN_MAX_T] = {};
     void* filt_img2[PAINN_MAX_T] = {};  // unscaled hi | lo image (edge_tc2.cu)   // tcgen05 A-operand image of (Wf | bf), fp16 hi/lo split (edge_tc.cu)
     int edge_path = 0;                  // 0: tensor-core edge kernels when F == 128, 1: plain fp32 kernels
+    float* tab0 = nullptr;              // [n_species][F] float2 (phi^s, phi^vs) of layer 0: s^0 = Emb[z] depends on the species only
     // capacities
     long long cap_atoms = 0, cap_edges = 0, cap_cells = 0;
     std::vector<Buf*> all;
@@ -327,6 +328,34 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
     up((size_t)R * F, &m->Wr1, &Wr1); up(R, &m->br1); up(R, &m->wr2); up(1, &m->br2);
     if (rcode == MLP_OK) painn::gemm_register_exact(m->Wr1, Wr1.data(), R, F);
     upT(Wr1, R, F, &m->Wr1T);
+    if (rcode == MLP_OK && F == 128 && m->filt_img[0] && ns <= 16) {
+        // layer-0 sender rows per species: phi(Emb[z]) through the same forward GEMM path as the per-atom rows
+        Buf bh, bp;
+        rcode = ensure(m, bh, (size_t)ns * F * 4);
+        if (rcode == MLP_OK) rcode = ensure(m, bp, (size_t)ns * 3 * F * 4);
+        if (rcode == MLP_OK) {
+            long long cnt = 0;
+            Launch L{nullptr, &cnt};
+            const int saved = painn::g_gemm_path;
+            painn::g_gemm_path = 1;
+            gemm_nt(L, m->Emb, F, m->lw[0].Wm1, F, P<float>(bh), F, ns, F, F, m->lw[0].bm1, false);
+            silu_fwd(L, (long long)ns * F, P<float>(bh), P<float>(bh));
+            gemm_nt(L, P<float>(bh), F, m->lw[0].Wm2, F, P<float>(bp), 3 * F, ns, 3 * F, F, m->lw[0].bm2, false);
+            painn::g_gemm_path = saved;
+            std::vector<float> ph((size_t)ns * 3 * F), tab((size_t)ns * F * 2);
+            if (cudaDeviceSynchronize() != cudaSuccess ||
+                cudaMemcpy(ph.data(), bp.p, ph.size() * 4, cudaMemcpyDeviceToHost) != cudaSuccess)
+                rcode = MLP_ERR_CUDA;
+            for (int z = 0; z < ns; z++)
+                for (int f = 0; f < F; f++) {
+                    tab[((size_t)z * F + f) * 2] = ph[(size_t)z * 3 * F + f];
+                    tab[((size_t)z * F + f) * 2 + 1] = ph[(size_t)z * 3 * F + F + f];
+                }
+            if (rcode == MLP_OK) rcode = upload(m, tab, &m->tab0);
+        }
+        free_buf(bh, m);
+        free_buf(bp, m);
+    }
     if (rcode == MLP_OK) rcode = ensure(m, m->b_misc, sizeof(Misc));
     if (rcode == MLP_OK && cudaMallocHost(&m->h_misc, sizeof(Misc)) != cudaSuccess) rcode = MLP_ERR_NOMEM;
     if (rcode == MLP_OK && cudaStreamCreateWithFlags(&m->own_stream, cudaStreamNonBlocking) != cudaSuccess)
@@ -553,9 +582,9 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         bool done = false;
         if (m->edge_path != 1 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
             make_gather_rows(L, N, phi, V, P<float>(m->b_Q4), P<float>(m->b_Q1), t > 0);
-            if (m->edge_path == 0)
+            if (m->edge_path == 0 && (t > 0 || m->tab0))
                 done = message_fwd_v3(L, N, K, rcf, row_ptr, ej, S, V, P<float>(m->b_Q4), P<float>(m->b_Q1), m->filt_img[t],
-                                      sn, v1, t > 0);
+                                      sn, v1, t > 0, P<int>(m->b_types_s), m->tab0, m->n_species);
             if (!done)
                 done = message_fwd_tc(L, N, K, rcf, row_ptr, ej, S, V, P<float>(m->b_Q4), P<float>(m->b_Q1), m->filt_img[t],
                                       sn, v1, t > 0);

@@ -94,9 +94,17 @@ struct FwdParams {
     float inv_rc;
     int K;
     int atoms_per_unit;
+    // layer 0 (HAS_V = false): s^0 = Emb[z], so the sender rows (phi^s_j, phi^vs_j) depend on the SPECIES of j only; they
+    // come from an n_species-row table in shared memory instead of a 55 GB gather through L2
+    const int* types;      // [N] species of the (cell-sorted) atoms
+    const float2* tab;     // [n_tab][F] (phi^s, phi^vs) per species
+    int n_tab;
 };
 
-constexpr int fwd_smem_bytes(bool has_v) { return (has_v ? 3 : 2) * A_CHUNK_BYTES + 2 * B_BYTES + 2 * NE * 16 + 64 + 128; }
+constexpr int TAB_MAX = 16;                             // species rows the shared-memory table can hold
+constexpr int fwd_smem_bytes(bool has_v) {
+    return (has_v ? 3 : 2) * A_CHUNK_BYTES + 2 * B_BYTES + 2 * NE * 16 + 64 + 128 + (has_v ? 0 : TAB_MAX * F * 8);
+}
 
 template <bool HAS_V>
 __global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
@@ -110,8 +118,8 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
     uint64_t* bars = (uint64_t*)(sMeta + 2 * NE);
     uint64_t* b_full = bars;          // [2] producers -> MMA (and consumers: sender indices readable)  (count 96)
     uint64_t* t_full = bars + 2;      // [2] MMA commit -> consumers (count 1)
-    uint64_t* t_empty = bars + 4;     // [2] consumers -> producers  (count 4)
-    uint32_t* tmem_slot = (uint32_t*)(bars + 6);
+    uint32_t* tmem_slot = (uint32_t*)(bars + 6);       // (consumers -> producers: named barriers 1, 2)
+    float2* sTab = (float2*)(bars + 8);                // [n_tab][F] species table (layer 0 only)
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     {
@@ -120,9 +128,11 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
         for (int i = tid; i < NCH * A_CHUNK_BYTES / 16; i += FWD_THREADS) dst[i] = src[i];
         uint4* zb = (uint4*)sB;
         for (int i = tid; i < 2 * B_BYTES / 16; i += FWD_THREADS) zb[i] = make_uint4(0, 0, 0, 0);
+        if (!HAS_V)
+            for (int i = tid; i < p.n_tab * F; i += FWD_THREADS) sTab[i] = p.tab[i];
     }
     if (tid == 0) {
-        for (int b = 0; b < 2; b++) { mbar_init(&b_full[b], 96); mbar_init(&t_full[b], 1); mbar_init(&t_empty[b], 4); }
+        for (int b = 0; b < 2; b++) { mbar_init(&b_full[b], 96); mbar_init(&t_full[b], 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 7) tmem_alloc(tmem_slot, TALLOC);
@@ -157,7 +167,6 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
         _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                \
             const size_t row_ = (size_t)__float_as_int((META8)[i_].w) * F;                \
             if (HAS_V) { Q4R[i_] = __ldg(Q4 + row_); Q1R[i_] = __ldg(Q1 + row_); }        \
-            else Q2R[i_] = __ldg(Q2 + row_);                                              \
         }                                                                                 \
     }
         uint32_t it = 0;
@@ -176,7 +185,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
                     next_has = __ldg(row_ptr + b1) > __ldg(row_ptr + b0);
                 }
             }
-            if (ntiles > 0 && !pre) {
+            if (HAS_V && ntiles > 0 && !pre) {
                 mbar_wait(&b_full[it & 1], (it >> 1) & 1);
                 const float4* m0 = sMeta + (it & 1) * NE;
                 FWD_ISSUE(qa4, qa1, qa2, m0);
@@ -223,8 +232,9 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
                     acc1 = fmaf(tv, m_.y, fmaf(w_vv, Q4R[i_].w, acc1));                                     \
                     acc2 = fmaf(tv, m_.z, fmaf(w_vv, Q1R[i_], acc2));                                       \
                 } else {                                                                                    \
-                    accS = fmaf(w_s, Q2R[i_].x, accS);                                                      \
-                    const float tv = w_vs * Q2R[i_].y;                                                      \
+                    const float2 q_ = sTab[__float_as_int(m_.w) * F + f];       /* species row of the sender */ \
+                    accS = fmaf(w_s, q_.x, accS);                                                           \
+                    const float tv = w_vs * q_.y;                                                           \
                     acc0 = fmaf(tv, m_.x, acc0);                                                            \
                     acc1 = fmaf(tv, m_.y, acc1);                                                            \
                     acc2 = fmaf(tv, m_.z, acc2);                                                            \
@@ -243,7 +253,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
                 FWD_COMPUTE(1, qb4, qb1, qb2);
                 FWD_ISSUE(qb4, qb1, qb2, meta + 24);
                 FWD_COMPUTE(2, qa4, qa1, qa2);
-                if (t + 1 < ntiles || next_has) {                  // first batch of the CTA's next tile
+                if (HAS_V && (t + 1 < ntiles || next_has)) {       // first batch of the CTA's next tile
                     mbar_wait(&b_full[buf ^ 1], ((it + 1) >> 1) & 1);
                     const float4* mn = sMeta + (buf ^ 1) * NE;
                     FWD_ISSUE(qa4, qa1, qa2, mn);
@@ -251,8 +261,7 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
                 }
                 FWD_COMPUTE(3, qb4, qb1, qb2);
                 tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&t_empty[buf]);
+                bar_arrive(1 + buf, 224);              // tile consumed: 128 consumers arrive, 96 producers wait (named barrier)
             }
             // finish the last receiver with edges, then pass trailing edge-less atoms through (s' = s, v' = v)
             for (;;) {
@@ -301,12 +310,16 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
                 }
                 uint4 p0, p1, p2;
                 split3(vals, p0, p1, p2);
-                mbar_wait_sleep(&t_empty[buf], ((it >> 1) & 1) ^ 1, 256);
+                if (it >= 2) bar_sync(1 + buf, 224);   // tile it - 2 consumed (hardware-blocking wait, no spin)
                 uint8_t* bb = sB + buf * B_BYTES + (e >> 3) * SBO + (e & 7) * 16 + h * LBO;
                 *(uint4*)(bb) = p0;                       // term 0: k = b
                 *(uint4*)(bb + 4 * LBO) = p1;             // term 1: k = 32 + b   (lo(R) 2^11)
                 *(uint4*)(bb + 8 * LBO) = p2;             // term 2: k = 64 + b   (hi(R) 2^-11)
-                if (h == 0) sMeta[buf * NE + e] = make_float4(g.r.x * g.inv_d, g.r.y * g.inv_d, g.r.z * g.inv_d, g.r.w);
+                if (h == 0) {
+                    float mw = g.r.w;                                             // sender index ...
+                    if (!HAS_V) mw = __int_as_float(__ldg(p.types + __float_as_int(g.r.w)));   // ... or its species (layer 0)
+                    sMeta[buf * NE + e] = make_float4(g.r.x * g.inv_d, g.r.y * g.inv_d, g.r.z * g.inv_d, mw);
+                }
                 fence_async_smem();
                 mbar_arrive(&b_full[buf]);
             }
@@ -737,10 +750,12 @@ static int sm_count() {
 
 // F = 128, K <= 23 only.  Q4/Q1 from make_gather_rows (layer 0: Q4 holds float2 rows); A_img from edge_build_filter_image.
 bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* s,
-                    const float* v, const float* Q4, const float* Q1, const void* A_img, float* sn, float* v1, bool has_v) {
+                    const float* v, const float* Q4, const float* Q1, const void* A_img, float* sn, float* v1, bool has_v,
+                    const int* types_s, const float* tab, int n_tab) {
     using namespace ev3;
     if (N == 0) return true;
     if (K > 23) return false;
+    if (!has_v && (!tab || !types_s || n_tab > TAB_MAX)) return false;
     static bool attr = false;
     if (!attr) {
         if (cudaFuncSetAttribute(k_msg_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fwd_smem_bytes(true)) != cudaSuccess ||
@@ -748,7 +763,8 @@ bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
             return false;
         attr = true;
     }
-    FwdParams p{N, row_ptr, ej, s, v, (const float4*)Q4, Q1, (const float2*)Q4, (const uint4*)A_img, sn, v1, 1.0f / rc, K, 16};
+    FwdParams p{N, row_ptr, ej, s, v, (const float4*)Q4, Q1, (const float2*)Q4, (const uint4*)A_img, sn, v1, 1.0f / rc, K, 16,
+                types_s, (const float2*)tab, n_tab};
     const long long n_units = (N + p.atoms_per_unit - 1) / p.atoms_per_unit;
     const int grid = (int)std::min<long long>(n_units, 2LL * sm_count());
     if (has_v) k_msg_fwd<true><<<grid, FWD_THREADS, fwd_smem_bytes(true), L.stream>>>(p);
