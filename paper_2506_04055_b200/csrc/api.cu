@@ -571,17 +571,22 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         float *hpre = P<float>(m->b_hpre[t]), *phi = P<float>(m->b_phi[t]), *sn = P<float>(m->b_sn[t]),
               *v1 = P<float>(m->b_v1[t]), *pq = P<float>(m->b_pq[t]), *zpre = P<float>(m->b_zpre[t]),
               *a = P<float>(m->b_a[t]);
-        gemm_nt(L, S, F, l.Wm1, F, hpre, F, N, F, F, l.bm1, false);
+        // layer 0: s^0 = Emb[z], so phi(s^0) is a per-species table (built at create); no per-atom phi-MLP, no gather rows
+        const bool l0_table = t == 0 && m->edge_path == 0 && m->tab0 && K <= 23 && m->filt_img[0] &&
+                              g_filter_emulate == 0 && g_gather_emulate == 0;
         const bool fuse_act = !m->fwd_tc && gemm_act_supported(3 * F, F);   // SiLU applied while loading A
-        if (fuse_act) gemm_nt_act(L, hpre, F, l.Wm2, F, phi, 3 * F, N, 3 * F, F, l.bm2, false, true);
-        else {
-            silu_fwd(L, N * F, hpre, h);
-            gemm_nt(L, h, F, l.Wm2, F, phi, 3 * F, N, 3 * F, F, l.bm2, false);
+        if (!l0_table) {
+            gemm_nt(L, S, F, l.Wm1, F, hpre, F, N, F, F, l.bm1, false);
+            if (fuse_act) gemm_nt_act(L, hpre, F, l.Wm2, F, phi, 3 * F, N, 3 * F, F, l.bm2, false, true);
+            else {
+                silu_fwd(L, N * F, hpre, h);
+                gemm_nt(L, h, F, l.Wm2, F, phi, 3 * F, N, 3 * F, F, l.bm2, false);
+            }
         }
         mark(m, st, ST_FWD_EDGE);
         bool done = false;
         if (m->edge_path != 1 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
-            make_gather_rows(L, N, phi, V, P<float>(m->b_Q4), P<float>(m->b_Q1), t > 0);
+            if (!l0_table) make_gather_rows(L, N, phi, V, P<float>(m->b_Q4), P<float>(m->b_Q1), t > 0);
             if (m->edge_path == 0 && (t > 0 || m->tab0))
                 done = message_fwd_v3(L, N, K, rcf, row_ptr, ej, S, V, P<float>(m->b_Q4), P<float>(m->b_Q1), m->filt_img[t],
                                       sn, v1, t > 0, P<int>(m->b_types_s), m->tab0, m->n_species);
@@ -626,7 +631,10 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         bool done = false;
         if (m->edge_path != 1 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
             make_gather_rows_bwd(L, N, s1b, v1b, P<float>(m->b_Q4));
-            if (m->edge_path == 0)
+            if (t == 0 && m->edge_path == 0 && m->tab0 && K <= 23)
+                done = message_bwd0_v3(L, N, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<int>(m->b_types_s), m->tab0, m->n_species,
+                                       P<int>(m->b_rev), m->filt_img[0], P<float4>(m->b_G), t == T - 1);
+            if (!done && m->edge_path == 0)
                 done = message_bwd_v3(L, N, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<float>(m->b_phi[t]),
                                       P<float>(m->b_V[t]), v1b, m->filt_img[t], phib, vb, P<float4>(m->b_G), t == T - 1, t == 0);
             if (!done && m->edge_path == 3)

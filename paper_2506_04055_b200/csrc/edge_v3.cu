@@ -736,6 +736,275 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
     if (tid >> 5 == 15) tmem_dealloc(*tmem_slot, 512);
 }
 
+// =============================================================================================================
+// layer-0 adjoint: only the geometry gradient is wanted (the embedding is constant) and the sender rows
+// (phi^s_j, phi^vs_j) depend on the species of j only.  The pass therefore walks the RECEIVER's row with the
+// receiver's own (sb'_i, vb'_i) in registers and looks the sender up in the species table: no neighbour-row gather
+// at all.  g of edge (i <- j) is produced at the slot of i's row; G is indexed by the slot of the sender's row
+// (force_final: F_a = sum_x G[rev x] - G[x]), so the reducer scatters through the reverse-edge index.
+// =============================================================================================================
+struct Bwd0Params {
+    long long N;
+    const int* row_ptr;
+    const float4* ej;
+    const float4* Gb;      // (sb', vb'_x, vb'_y, vb'_z) per atom and channel
+    const int* types;
+    const float2* tab;     // [n_tab][F] (phi^s, phi^vs) per species
+    const int* rev;
+    const uint4* A_img;
+    float4* G;
+    float inv_rc;
+    int K;
+    int atoms_per_unit;
+    int first;
+    int n_tab;
+};
+constexpr int G0_OFF_SPEC = G_OFF_BAR + 128, G0_OFF_TAB = G0_OFF_SPEC + 4 * NEB * 4, GROUP0_BYTES = G0_OFF_TAB;
+constexpr int bwd0_smem_bytes() { return 2 * A_CHUNK_BYTES + 2 * GROUP0_BYTES + TAB_MAX * F * 8 + 128; }
+
+__global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p) {
+    constexpr int NCH = 2;
+    constexpr int TCOLS = NCH * 2 * NEB;
+    extern __shared__ __align__(128) uint8_t smem[];
+    uint8_t* sA = smem;
+    const int tid = threadIdx.x, grp = tid >> 8, ltid = tid & 255, lwarp = ltid >> 5, lane = tid & 31;
+    uint8_t* gbase = smem + NCH * A_CHUNK_BYTES + grp * GROUP0_BYTES;
+    uint8_t* sB = gbase + G_OFF_B;
+    uint8_t* sP = gbase + G_OFF_P;
+    float4* sMeta = (float4*)(gbase + G_OFF_META);  // [4][NEB] (u_e, 1/d_e)
+    int* sSpec = (int*)(gbase + G0_OFF_SPEC);       // [4][NEB] species of the sender
+    uint64_t* bars = (uint64_t*)(gbase + G_OFF_BAR);
+    uint64_t* t_full = bars;
+    uint64_t* p_empty = bars + 2;
+    const int NB_TE = 1 + grp * 6, NB_BF = NB_TE + 2, NB_PF = NB_TE + 4;
+    float2* sTab = (float2*)(smem + NCH * A_CHUNK_BYTES + 2 * GROUP0_BYTES);
+    uint32_t* tmem_slot = (uint32_t*)(sTab + TAB_MAX * F);
+    {
+        const uint4* src = p.A_img;
+        uint4* dst = (uint4*)sA;
+        for (int i = tid; i < NCH * A_CHUNK_BYTES / 16; i += BWD_THREADS) dst[i] = src[i];
+        uint4* zb = (uint4*)sB;
+        for (int i = ltid; i < 2 * BB_BYTES / 16; i += 256) zb[i] = make_uint4(0, 0, 0, 0);
+        for (int i = tid; i < p.n_tab * F; i += BWD_THREADS) sTab[i] = p.tab[i];
+    }
+    if (ltid == 0) {
+        for (int b = 0; b < 2; b++) { mbar_init(&t_full[b], 1); mbar_init(&p_empty[b], 1); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (tid >> 5 == 15) tmem_alloc(tmem_slot, 512);
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot + grp * 256;
+    const long long N = p.N;
+    const int apu = p.atoms_per_unit;
+    const int* __restrict__ row_ptr = p.row_ptr;
+    const long long n_units = (N + apu - 1) / apu;
+    const long long u0 = (long long)blockIdx.x * 2 + grp, ustride = (long long)gridDim.x * 2;
+    if (lwarp < 4) reg_inc<168>(); else reg_dec<88>();
+
+    if (lwarp < 4) {
+        // ===================== consumers: one channel per thread, receiver rows =====================
+        const int f = ltid;
+        const float4* __restrict__ Gb = p.Gb + f;
+        const uint32_t lane_base = tmem_base + ((uint32_t)(lwarp * 32) << 16);
+        uint32_t it = 0, hc = 0;
+        for (long long u = u0; u < n_units; u += ustride) {
+            const long long a0 = u * apu;
+            const int na = (int)min((long long)apu, N - a0);
+            const int rp = __ldg(row_ptr + a0 + min(lane, na));
+            const int e_begin = __shfl_sync(0xffffffffu, rp, 0), e_end = __shfl_sync(0xffffffffu, rp, na);
+            const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
+            int i_rel = 0;
+            int row_end = __shfl_sync(0xffffffffu, rp, 1);
+            float4 own = Gb[a0 * F], nown = na > 1 ? Gb[(a0 + 1) * F] : own;      // (sb', vb') of receiver i, i + 1
+            for (int t = 0; t < ntiles; t++, it++) {
+                const int buf = it & 1;
+                const float4* meta = sMeta + (it & 3) * NEB;
+                const int* spec = sSpec + (it & 3) * NEB;
+                mbar_wait(&t_full[buf], (it >> 1) & 1);
+                tc_fence_after();
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    const int E8 = e_begin + t * NEB + h * 8;
+                    if (E8 < e_end) {
+                        while (E8 >= row_end) {
+                            i_rel++;
+                            row_end = __shfl_sync(0xffffffffu, rp, i_rel + 1);
+                            own = nown;
+                            if (i_rel + 1 < na) nown = Gb[(a0 + i_rel + 1) * F];
+                        }
+                        uint32_t dS[8], wVS[8], dVS[8];
+                        tmem_ld8_nowait(lane_base + buf * TCOLS + NEB + h * 8, dS);
+                        tmem_ld8_nowait(lane_base + buf * TCOLS + 2 * NEB + h * 8, wVS);
+                        tmem_ld8_nowait(lane_base + buf * TCOLS + 3 * NEB + h * 8, dVS);
+                        mbar_wait(&p_empty[hc & 1], ((hc >> 1) & 1) ^ 1);
+                        tmem_wait_ld();
+                        uint8_t* pdst = sP + (hc & 1) * P_BYTES;
+#pragma unroll
+                        for (int i = 0; i < 8; i++) {
+                            const float4 m = meta[h * 8 + i];
+                            const float2 ph = sTab[spec[h * 8 + i] * F + f];
+                            const float X = fmaf(own.y, m.x, fmaf(own.z, m.y, own.w * m.z));
+                            float db = ph.x * (own.x * __uint_as_float(dS[i]));
+                            db = fmaf(ph.y, X * __uint_as_float(dVS[i]), db);
+                            const float beta = __uint_as_float(wVS[i]) * ph.y * m.w;
+                            const float alpha = fmaf(-beta, X, db);
+                            float* pd = (float*)(pdst + i * P_ROW) + f;
+                            pd[0] = fmaf(alpha, m.x, beta * own.y);
+                            pd[F] = fmaf(alpha, m.y, beta * own.z);
+                            pd[2 * F] = fmaf(alpha, m.z, beta * own.w);
+                        }
+                        bar_arrive(NB_PF + (hc & 1), 160);
+                        hc++;
+                    }
+                }
+                tc_fence_before();
+                bar_arrive(NB_TE + buf, 192);
+            }
+        }
+    } else if (lwarp < 6) {
+        // ===================== producers: rows 0..15 R_e, rows 16..31 R'_e; meta (u_e, 1/d), species =====================
+        const int pt = ltid - 128, e = pt & 15, h = pt >> 4;
+        const float inv_rc = p.inv_rc;
+        const float a1c = 3.14159265358979323846f * inv_rc;
+        const int K = p.K;
+        uint32_t it = 0;
+        for (long long u = u0; u < n_units; u += ustride) {
+            const long long a0 = u * apu;
+            const long long a1 = min(N, a0 + (long long)apu);
+            const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
+            const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
+            for (int t = 0; t < ntiles; t++, it++) {
+                const int buf = it & 1;
+                uint4 q[6];
+                float4 meta_v = make_float4(0.f, 0.f, 0.f, 0.f);
+                int spec_v = 0;
+                if (h < 3) {
+                    const EdgeGeom g = load_edge(p.ej, e_begin + t * NEB + e, e_end, inv_rc);
+                    if (h == 0) spec_v = __ldg(p.types + __float_as_int(g.r.w));
+                    const float fc = g.real ? 0.5f * (1.0f + g.c1) : 0.0f;
+                    const float dfc = g.real ? -0.5f * a1c * g.s1 : 0.0f;
+                    float sn_, cn_;
+                    if (h == 0) { sn_ = g.s1; cn_ = g.c1; } else sincospif((float)(8 * h) * g.x, &sn_, &cn_);
+                    float vals[8], dvals[8];
+#pragma unroll
+                    for (int i = 0; i < 8; i++) {
+                        const int b = h * 8 + i;
+                        if (b == 0) { vals[i] = fc; dvals[i] = dfc; }
+                        else {
+                            const float rho = sn_ * g.inv_d;
+                            const float drho = ((float)b * a1c * cn_ - rho) * g.inv_d;
+                            vals[i] = b <= K ? fc * rho : 0.0f;
+                            dvals[i] = b <= K ? dfc * rho + fc * drho : 0.0f;
+                            const float tt = sn_ * g.c1 + cn_ * g.s1;
+                            cn_ = cn_ * g.c1 - sn_ * g.s1;
+                            sn_ = tt;
+                        }
+                    }
+                    split3(vals, q[0], q[1], q[2]);
+                    split3(dvals, q[3], q[4], q[5]);
+                    meta_v = make_float4(g.r.x * g.inv_d, g.r.y * g.inv_d, g.r.z * g.inv_d, g.inv_d);
+                }
+                __syncwarp();
+                if (it >= 2) bar_sync(NB_TE + buf, 192);
+                if (h < 3) {
+#pragma unroll
+                    for (int z = 0; z < 2; z++) {
+                        const int row = z * NEB + e;
+                        uint8_t* bb = sB + buf * BB_BYTES + (row >> 3) * SBO + (row & 7) * 16 + h * LBO;
+                        *(uint4*)(bb) = q[3 * z + 0];
+                        *(uint4*)(bb + 4 * LBO) = q[3 * z + 1];
+                        *(uint4*)(bb + 8 * LBO) = q[3 * z + 2];
+                    }
+                    if (h == 0) { sMeta[(it & 3) * NEB + e] = meta_v; sSpec[(it & 3) * NEB + e] = spec_v; }
+                }
+                fence_async_smem();
+                __syncwarp();
+                bar_arrive(NB_BF + buf, 96);
+            }
+        }
+    } else if (lwarp == 6) {
+        // ===================== reducer: channel sums, scatter into the sender-row slot =====================
+        const int re = lane >> 2, rsub = lane & 3;
+        float4* __restrict__ Gout = p.G;
+        const bool first = p.first != 0;
+        uint32_t hc = 0;
+        for (long long u = u0; u < n_units; u += ustride) {
+            const long long a0 = u * apu;
+            const long long a1 = min(N, a0 + (long long)apu);
+            const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
+            const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
+            for (int t = 0; t < ntiles; t++) {
+                for (int h = 0; h < 2; h++) {
+                    const int E8 = e_begin + t * NEB + h * 8;
+                    if (E8 >= e_end) continue;
+                    const int tgt = __ldg(p.rev + E8 + re);
+                    float4 gold = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (rsub == 0 && !first) gold = Gout[tgt];
+                    bar_sync(NB_PF + (hc & 1), 160);
+                    const uint8_t* src = sP + (hc & 1) * P_BYTES + re * P_ROW + rsub * 16;
+                    float3 acc = make_float3(0.f, 0.f, 0.f);
+#pragma unroll
+                    for (int k = 0; k < 8; k++) {
+                        const float4 x = *(const float4*)(src + k * 64);
+                        const float4 y = *(const float4*)(src + F * 4 + k * 64);
+                        const float4 z = *(const float4*)(src + 2 * F * 4 + k * 64);
+                        acc.x += (x.x + x.y) + (x.z + x.w);
+                        acc.y += (y.x + y.y) + (y.z + y.w);
+                        acc.z += (z.x + z.y) + (z.z + z.w);
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&p_empty[hc & 1]);
+                    hc++;
+#pragma unroll
+                    for (int o = 2; o >= 1; o >>= 1) {
+                        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o);
+                        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
+                        acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o);
+                    }
+                    if (rsub == 0) Gout[tgt] = make_float4(gold.x + acc.x, gold.y + acc.y, gold.z + acc.z, 0.f);
+                }
+            }
+        }
+    } else if (lwarp == 7) {
+        // ===================== MMA issuer =====================
+        const uint32_t idesc = (1u << 4) | ((uint32_t)((2 * NEB) >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+        const uint32_t a_base = smem_u32(sA), b_base = smem_u32(sB);
+        uint32_t it = 0;
+        for (long long u = u0; u < n_units; u += ustride) {
+            const long long a0 = u * apu;
+            const long long a1 = min(N, a0 + (long long)apu);
+            const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
+            const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
+            for (int t = 0; t < ntiles; t++, it++) {
+                const int buf = it & 1;
+                bar_sync(NB_BF + buf, 96);
+                tc_fence_after();
+                if (lane == 0) {
+#pragma unroll
+                    for (int c = 0; c < NCH; c++) {
+                        const uint32_t d = tmem_base + buf * TCOLS + c * 2 * NEB;
+#pragma unroll
+                        for (int o = 0; o < 6; o++) {
+                            const int kk = (o + 2) % 6;
+                            const uint64_t ad = make_desc_nosw(a_base + c * A_CHUNK_BYTES + kk * 2 * LBO, LBO, SBO);
+                            const uint64_t bd = make_desc_nosw(b_base + buf * BB_BYTES + kk * 2 * LBO, LBO, SBO);
+                            umma_f16(d, ad, bd, idesc, o != 0);
+                        }
+                    }
+                    umma_commit(&t_full[buf]);
+                }
+                __syncwarp();
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (tid >> 5 == 15) tmem_dealloc(*tmem_slot, 512);
+}
+
 }  // namespace ev3
 
 static int sm_count() {
@@ -793,6 +1062,26 @@ bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
     const int grid = (int)std::min<long long>((n_units + 1) / 2, (long long)sm_count());
     if (layer0) k_msg_bwd<true><<<grid, BWD_THREADS, bwd_smem_bytes(2), L.stream>>>(p);
     else k_msg_bwd<false><<<grid, BWD_THREADS, bwd_smem_bytes(3), L.stream>>>(p);
+    KLAUNCH(L);
+    return true;
+}
+
+// layer-0 adjoint through the species table (see k_msg_bwd0); G indexed as everywhere else (slot of the sender's row)
+bool message_bwd0_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
+                     const int* types_s, const float* tab, int n_tab, const int* rev, const void* A_img, float4* G, bool first) {
+    using namespace ev3;
+    if (N == 0) return true;
+    if (K > 23 || !tab || n_tab > TAB_MAX) return false;
+    static bool attr = false;
+    if (!attr) {
+        if (cudaFuncSetAttribute(k_msg_bwd0, cudaFuncAttributeMaxDynamicSharedMemorySize, bwd0_smem_bytes()) != cudaSuccess) return false;
+        attr = true;
+    }
+    Bwd0Params p{N, row_ptr, ej, (const float4*)Gb, types_s, (const float2*)tab, rev, (const uint4*)A_img, G, 1.0f / rc, K, 16,
+                 first ? 1 : 0, n_tab};
+    const long long n_units = (N + p.atoms_per_unit - 1) / p.atoms_per_unit;
+    const int grid = (int)std::min<long long>((n_units + 1) / 2, (long long)sm_count());
+    k_msg_bwd0<<<grid, BWD_THREADS, bwd0_smem_bytes(), L.stream>>>(p);
     KLAUNCH(L);
     return true;
 }
