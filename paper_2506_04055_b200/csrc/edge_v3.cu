@@ -479,7 +479,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                 for (int i = 0; i < GW; i++) {
                     const int j = __shfl_sync(0xffffffffu, idx0, i);
                     if (i < n_e) cp_async16(ring + i * F, Gb + (size_t)j * F);
-                    cp_async_commit();
+                    if ((i & 7) == 7) cp_async_commit();            // one commit group per 8-edge batch
                 }
             }
             int j_rel = 0;
@@ -538,10 +538,10 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
             }                                                                                                     \
             mbar_wait(&p_empty[hc & 1], ((hc >> 1) & 1) ^ 1);           /* partials buffer free again */          \
             tmem_wait_ld();                                                                                       \
+            cp_async_wait<1>();              /* this batch's rows have landed; the next batch's stay in flight */ \
             uint8_t* pdst_ = sP + (hc & 1) * P_BYTES;                                                             \
             _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                                    \
                 const float4 m_ = meta[(H) * 8 + i_];                                                             \
-                cp_async_wait<GW - 1>();                                                                          \
                 const float4 g_ = ring[((H) * 8 + i_) * F];                                                       \
                 const float sb_ = g_.x, vb0_ = g_.y, vb1_ = g_.z, vb2_ = g_.w;                                    \
                 const float X_ = fmaf(vb0_, m_.x, fmaf(vb1_, m_.y, vb2_ * m_.z));                                 \
@@ -563,10 +563,13 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                 pd_[0] = fmaf(alpha_, m_.x, beta_ * vb0_);                                                        \
                 pd_[F] = fmaf(alpha_, m_.y, beta_ * vb1_);                                                        \
                 pd_[2 * F] = fmaf(alpha_, m_.z, beta_ * vb2_);                                                    \
+            }                                                                                                     \
+            /* re-arm the 8 slots with the rows of edges k0 + 16 .. k0 + 23 (one commit group, also when empty) */ \
+            _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                                    \
                 const int jn_ = __shfl_sync(0xffffffffu, isel_, l0_ + i_);                                        \
                 if (pf_) cp_async16(ring + ((H) * 8 + i_) * F, Gb + (size_t)jn_ * F);                             \
-                cp_async_commit();                                                                                \
             }                                                                                                     \
+            cp_async_commit();                                                                                    \
             bar_arrive(NB_PF + (hc & 1), 160);                          /* hand the batch to the reducer warp */  \
             hc++;                                                                                                 \
         }                                                                                                         \
