@@ -66,6 +66,8 @@ struct mlp_model {
     // host staging for mlp_compute_host
     Buf d_pos, d_types, d_owner, d_out;   // d_out: energy[1] virial[6] forces[3N]
     cudaStream_t own_stream = nullptr;
+    cudaStream_t side_stream = nullptr;            // reverse-edge index is built beside the forward pass
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     // last call
     long long N_last = 0, n_local_last = 0, E_last = 0 /* padded slots */, E_real_last = 0;
     Grid grid_last{};
@@ -358,7 +360,10 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
     }
     if (rcode == MLP_OK) rcode = ensure(m, m->b_misc, sizeof(Misc));
     if (rcode == MLP_OK && cudaMallocHost(&m->h_misc, sizeof(Misc)) != cudaSuccess) rcode = MLP_ERR_NOMEM;
-    if (rcode == MLP_OK && cudaStreamCreateWithFlags(&m->own_stream, cudaStreamNonBlocking) != cudaSuccess)
+    if (rcode == MLP_OK && (cudaStreamCreateWithFlags(&m->own_stream, cudaStreamNonBlocking) != cudaSuccess ||
+                            cudaStreamCreateWithFlags(&m->side_stream, cudaStreamNonBlocking) != cudaSuccess ||
+                            cudaEventCreateWithFlags(&m->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+                            cudaEventCreateWithFlags(&m->ev_join, cudaEventDisableTiming) != cudaSuccess))
         rcode = MLP_ERR_CUDA;
     if (rcode == MLP_OK) rcode = alloc_atoms(m, capacity);
     if (rcode == MLP_OK) rcode = alloc_edges(m, 64 * capacity);
@@ -391,6 +396,9 @@ __attribute__((visibility("default"))) void mlp_destroy(mlp_model* m) {
     }
     if (m->h_misc) cudaFreeHost(m->h_misc);
     if (m->own_stream) cudaStreamDestroy(m->own_stream);
+    if (m->side_stream) cudaStreamDestroy(m->side_stream);
+    if (m->ev_fork) cudaEventDestroy(m->ev_fork);
+    if (m->ev_join) cudaEventDestroy(m->ev_join);
     for (cudaEvent_t e : m->ev_pool) cudaEventDestroy(e);
     delete m;
 }
@@ -553,7 +561,15 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
     const int* row_ptr = P<int>(m->b_row_ptr);
     nbr_fill(L, N, g, P<double>(m->b_pos_s), P<signed char>(m->b_wrap_s), P<int>(m->b_cell_s), cell_start, row_ptr,
              m->cap_edges, rcf, ej, P<unsigned char>(m->b_img), dm->flags);
-    nbr_reverse(L, N, row_ptr, ej, P<unsigned char>(m->b_img), P<int>(m->b_rev));
+    // the reverse-edge index is needed by the layer-0 adjoint and the force assembly only: build it on a side stream,
+    // overlapped with the forward pass (its warps fit beside the GEMM / element-wise kernels)
+    {
+        Launch Ls{m->side_stream, &launches};
+        CU(m, cudaEventRecord(m->ev_fork, st));
+        CU(m, cudaStreamWaitEvent(m->side_stream, m->ev_fork, 0));
+        nbr_reverse(Ls, N, row_ptr, ej, P<unsigned char>(m->b_img), P<int>(m->b_rev));
+        CU(m, cudaEventRecord(m->ev_join, m->side_stream));
+    }
 
     // ---- forward ----
     // Tensor-core accumulation truncates toward zero after every MMA (measured): a relative
@@ -612,6 +628,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
             P<float>(m->b_eatom), P<double>(m->b_epart), &n_epart);
 
     // ---- backward ----
+    CU(m, cudaStreamWaitEvent(st, m->ev_join, 0));          // reverse-edge index ready
     painn::g_gemm_path = m->bwd_exact ? 1 : saved_path;
     mark(m, st, ST_BWD_NODE);
     float *sb = P<float>(m->b_sb), *s1b = P<float>(m->b_s1b), *vb = P<float>(m->b_vb), *v1b = P<float>(m->b_v1b);
