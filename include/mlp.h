@@ -136,7 +136,14 @@ int mlp_get_stats(mlp_model* m, mlp_stats* out);
 int mlp_get_stage_ms(mlp_model* m, int max_stages, const char** names, float* ms);
 
 /* mlp_set_option -- integer knobs: "stage_timing" (0/1), "edge_capacity" (force an initial edge capacity,
- * used by the regrow tests).  Unknown names return MLP_ERR_ARG. */
+ * test hook for the overflow / regrow path of PAPER.md:84-86), and experiment switches that select between
+ * implementations of the same arithmetic (defaults are the shipped path; DESIGN.md sections 5-7b):
+ *   "edge_path"       0 gen-3 tensor-core edge kernels (F = 128, K <= 23), 1 plain fp32 kernels, 2 / 3 earlier generations
+ *   "gemm_fwd_exact"  1 forward GEMMs on tcgen05 with exact integer slices, 0 fp32 FFMA kernel
+ *   "gemm_bwd_exact"  0 adjoint GEMMs 3xTF32, 1 exact integer slices
+ *   "gemm_fwd_tc"     1 forward GEMMs 3xTF32 (biased energy, B3)
+ *   "gemm_emulate", "filter_emulate", "gather_emulate", "gemm_path"  operand-precision emulation (measurements of section 5)
+ * Unknown names return MLP_ERR_ARG. */
 int mlp_set_option(mlp_model* m, const char* name, long long value);
 
 /* mlp_last_error -- text of the last error on this model (static string when m == NULL). */
