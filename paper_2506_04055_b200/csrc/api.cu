@@ -639,8 +639,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         float *ab = P<float>(m->b_ab), *pqb = P<float>(m->b_pqb), *gb = P<float>(m->b_gb), *snb = P<float>(m->b_snb),
               *phib = P<float>(m->b_phib), *hb = P<float>(m->b_hb);
         update_bwd1(L, N, F, sb, vb, P<float>(m->b_pq[t]), P<float>(m->b_a[t]), ab, pqb);
-        gemm_nt(L, ab, 3 * F, l.Wu2T, 3 * F, gb, F, N, F, 3 * F, nullptr, false);
-        mul_dsilu(L, N * F, P<float>(m->b_zpre[t]), gb);
+        gemm_nt_dsilu(L, ab, 3 * F, l.Wu2T, 3 * F, gb, F, N, F, 3 * F, P<float>(m->b_zpre[t]));
         gemm_nt(L, gb, F, l.Wu1T, F, snb, 2 * F, N, 2 * F, F, nullptr, false);
         update_bwd2(L, N, F, sb, vb, snb, P<float>(m->b_sn[t]), P<float>(m->b_pq[t]), pqb, s1b, v1b);
         gemm_nt(L, pqb, 2 * F, l.UVT, 2 * F, v1b, F, 3 * N, F, 2 * F, nullptr, true);
@@ -666,8 +665,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
                         phib, vb, P<float4>(m->b_G), t == T - 1);
         mark(m, st, ST_BWD_NODE);
         if (t == 0) break;      // s^0 is the (constant) embedding: its adjoint is never used
-        gemm_nt(L, phib, 3 * F, l.Wm2T, 3 * F, hb, F, N, F, 3 * F, nullptr, false);
-        mul_dsilu(L, N * F, P<float>(m->b_hpre[t]), hb);
+        gemm_nt_dsilu(L, phib, 3 * F, l.Wm2T, 3 * F, hb, F, N, F, 3 * F, P<float>(m->b_hpre[t]));
         gemm_nt(L, hb, F, l.Wm1T, F, s1b, F, N, F, F, nullptr, true);
         std::swap(sb, s1b);
     }

@@ -71,6 +71,8 @@ void gemm_nt(const Launch& L, const float* A, int lda, const float* B, int ldb, 
 void gemm_nt_act(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
                  int N, int K, const float* bias, bool accumulate, bool act_a);
 bool gemm_act_supported(int N, int K);
+void gemm_nt_dsilu(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
+                   int N, int K, const float* pre);
 
 // ---- model kernels (painn_fwd.cu / painn_bwd.cu) ----
 void embed(const Launch& L, long long N, int F, const int* types_s, const float* Emb, float* s0, float* v0);

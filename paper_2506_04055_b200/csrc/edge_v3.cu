@@ -59,15 +59,16 @@ __device__ __forceinline__ EdgeGeom load_edge(const float4* __restrict__ ej, int
     return g;
 }
 // split 8 fp32 values into the three fp16 planes of the B operand: hi, lo * 2^11, hi * 2^-11
+// (packed conversions: one F2FP per pair; the 2^-11 plane is an exact exponent shift done in half2)
 __device__ __forceinline__ void split3(const float (&v)[8], uint4& p0, uint4& p1, uint4& p2) {
     __half2 a[4], b[4], c[4];
+    const __half2 k = __floats2half2_rn(1.0f / 2048.0f, 1.0f / 2048.0f);
 #pragma unroll
     for (int i = 0; i < 4; i++) {
-        const __half h0 = __float2half_rn(v[2 * i]), h1 = __float2half_rn(v[2 * i + 1]);
-        const float f0 = __half2float(h0), f1 = __half2float(h1);
-        a[i] = __halves2half2(h0, h1);
-        b[i] = __halves2half2(__float2half_rn((v[2 * i] - f0) * 2048.0f), __float2half_rn((v[2 * i + 1] - f1) * 2048.0f));
-        c[i] = __halves2half2(__float2half_rn(f0 * (1.0f / 2048.0f)), __float2half_rn(f1 * (1.0f / 2048.0f)));
+        a[i] = __floats2half2_rn(v[2 * i], v[2 * i + 1]);
+        const float2 f = __half22float2(a[i]);
+        b[i] = __floats2half2_rn((v[2 * i] - f.x) * 2048.0f, (v[2 * i + 1] - f.y) * 2048.0f);
+        c[i] = __hmul2(a[i], k);
     }
     p0 = *(uint4*)a; p1 = *(uint4*)b; p2 = *(uint4*)c;
 }

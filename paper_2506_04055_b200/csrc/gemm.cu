@@ -185,7 +185,8 @@ int g_gemm_fwd_exact = 1;   // forward GEMMs: 1 = exact integer-slice tensor-cor
 void gemm_register_split(const float* W, const float* hi, const float* lo) { g_split[W] = {hi, lo}; }
 void gemm_unregister_split(const float* W) { g_split.erase(W); }
 bool gemm_nt_tc(const Launch& L, const float* A, int lda, const float* Whi, const float* Wlo, int ldw, float* C, int ldc,
-                long long M, int N, int K, const float* bias, bool accumulate);
+                long long M, int N, int K, const float* bias, bool accumulate, const float* dsilu_pre = nullptr, int ld_pre = 0);
+void mul_dsilu(const Launch& L, long long n, const float* pre, float* g);
 
 void gemm_nt_act(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
                  int N, int K, const float* bias, bool accumulate, bool act_a);
@@ -194,6 +195,23 @@ bool gemm_act_supported(int N, int K) { return g_gemm_emulate == 0 && N % 128 ==
 void gemm_nt(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
              int N, int K, const float* bias, bool accumulate) {
     gemm_nt_act(L, A, lda, B, ldb, C, ldc, M, N, K, bias, accumulate, false);
+}
+
+// C = (A . B^T) * SiLU'(pre)   (pre: [M x N] contiguous): adjoint of a SiLU layer; fused into the 3xTF32 epilogue when
+// that kernel covers the shape, otherwise GEMM followed by the element-wise kernel
+void gemm_nt_dsilu(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
+                   int N, int K, const float* pre) {
+    if (M == 0) return;
+    if (g_gemm_path == 0 && g_gemm_emulate == 0 && ldc == N) {
+        auto it = g_split.find(B);
+        if (it != g_split.end() &&
+            gemm_nt_tc(L, A, lda, it->second.first, it->second.second, ldb, C, ldc, M, N, K, nullptr, false, pre, N)) {
+            g_last_gemm_tc = 1;
+            return;
+        }
+    }
+    gemm_nt(L, A, lda, B, ldb, C, ldc, M, N, K, nullptr, false);
+    mul_dsilu(L, M * N, pre, C);
 }
 
 // act_a: C = SiLU(A) . B^T + bias  (only the fp32 FFMA path implements it; callers use it on forward GEMMs only)

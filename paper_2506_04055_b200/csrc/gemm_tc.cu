@@ -54,7 +54,13 @@ struct Params {
     const float* bias;
     long long M;
     int N, K, ldc, accumulate;
+    const float* dsilu_pre;    // optional [M x N] (row stride ld_pre): C = (A W^T + bias) * SiLU'(pre), fused adjoint of the activation
+    int ld_pre;
 };
+__device__ __forceinline__ float dsilu_x(float x) {
+    const float sg = 1.0f / (1.0f + __expf(-x));
+    return sg * (1.0f + x * (1.0f - sg));
+}
 
 template <int BN, int STAGES>
 struct Smem {
@@ -196,6 +202,9 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
                 if (p.accumulate && row < p.M) {
 #pragma unroll
                     for (int c = 0; c < 8; c++) o[c] = __ldcs((const float4*)(crow + c0) + c);
+                } else if (p.dsilu_pre && row < p.M) {     // (never combined with accumulate)
+#pragma unroll
+                    for (int c = 0; c < 8; c++) o[c] = __ldcs((const float4*)(p.dsilu_pre + row * p.ld_pre + n0 + c0) + c);
                 }
                 tmem_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + buf * BN + c0, r);
                 if (row < p.M) {
@@ -208,6 +217,9 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
                             v.x += b.x; v.y += b.y; v.z += b.z; v.w += b.w;
                         }
                         if (p.accumulate) { v.x += o[c / 4].x; v.y += o[c / 4].y; v.z += o[c / 4].z; v.w += o[c / 4].w; }
+                        else if (p.dsilu_pre) {
+                            v.x *= dsilu_x(o[c / 4].x); v.y *= dsilu_x(o[c / 4].y); v.z *= dsilu_x(o[c / 4].z); v.w *= dsilu_x(o[c / 4].w);
+                        }
                         *(float4*)(crow + c0 + c) = v;
                     }
                 }
@@ -690,8 +702,9 @@ bool gemm_nt_exact(const Launch& L, const float* A, int lda, const float* W, flo
 
 // Returns false when the shape is not covered (caller falls back to the SIMT path).
 bool gemm_nt_tc(const Launch& L, const float* A, int lda, const float* Whi, const float* Wlo, int ldw, float* C, int ldc,
-                long long M, int N, int K, const float* bias, bool accumulate) {
+                long long M, int N, int K, const float* bias, bool accumulate, const float* dsilu_pre, int ld_pre) {
     using namespace tc;
+    if (dsilu_pre && (accumulate || (ld_pre % 4) || ((uintptr_t)dsilu_pre & 15))) return false;
     if (M <= 0 || K % BK != 0 || K < BK || (lda % 4) || (ldw % 4) || (ldc % 4)) return false;
     if (((uintptr_t)A | (uintptr_t)Whi | (uintptr_t)Wlo | (uintptr_t)C) & 15) return false;
     const int BN = (N % 128 == 0) ? 128 : (N % 64 == 0 ? 64 : 0);
@@ -705,7 +718,7 @@ bool gemm_nt_tc(const Launch& L, const float* A, int lda, const float* Whi, cons
     CUtensorMap ma, mh, ml;
     if (!make_map(&ma, A, M, K, lda, BM) || !make_map(&mh, Whi, N, K, ldw, BN) || !make_map(&ml, Wlo, N, K, ldw, BN))
         return false;
-    Params p{C, bias, M, N, K, ldc, accumulate ? 1 : 0};
+    Params p{C, bias, M, N, K, ldc, accumulate ? 1 : 0, dsilu_pre, ld_pre};
     if (BN == 128) return launch<128, 3>(L, ma, mh, ml, p, n_sm);
     return launch<64, 4>(L, ma, mh, ml, p, n_sm);
 }
