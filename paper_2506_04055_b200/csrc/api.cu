@@ -40,6 +40,7 @@ struct mlp_model {
     LayerW lw[PAINN_MAX_T];
     float *Wr1 = nullptr, *br1 = nullptr, *wr2 = nullptr, *br2 = nullptr, *Wr1T = nullptr;
     void* filt_img[PAINN_MAX_T] = {};
+    void* filt_rows[PAINN_MAX_T] = {};  // same numbers as plain rows [3][F][96] fp16 (TMEM-resident A operand)
     void* filt_img2[PAINN_MAX_T] = {};  // unscaled hi | lo image (edge_tc2.cu)   // tcgen05 A-operand image of (Wf | bf), fp16 hi/lo split (edge_tc.cu)
     int edge_path = 0;                  // 0: tensor-core edge kernels when F == 128, 1: plain fp32 kernels
     float* tab0 = nullptr;              // [n_species][F] float2 (phi^s, phi^vs) of layer 0: s^0 = Emb[z] depends on the species only
@@ -297,6 +298,12 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
                 if (rcode == MLP_OK && cudaMemcpy(b.p, img.data(), img.size() * 2, cudaMemcpyHostToDevice) != cudaSuccess) rcode = MLP_ERR_CUDA;
                 m->wbufs.push_back(b);
                 m->filt_img[t] = b.p;
+                edge_build_filter_rows(Wf_h.data(), bf_h.data(), K, img);
+                Buf b3;
+                if (rcode == MLP_OK) rcode = ensure(m, b3, img.size() * 2);
+                if (rcode == MLP_OK && cudaMemcpy(b3.p, img.data(), img.size() * 2, cudaMemcpyHostToDevice) != cudaSuccess) rcode = MLP_ERR_CUDA;
+                m->wbufs.push_back(b3);
+                m->filt_rows[t] = b3.p;
                 edge_build_filter_image2(Wf_h.data(), bf_h.data(), K, img);
                 Buf b2;
                 if (rcode == MLP_OK) rcode = ensure(m, b2, img.size() * 2);
@@ -649,7 +656,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
             make_gather_rows_bwd(L, N, s1b, v1b, P<float>(m->b_Q4));
             if (t == 0 && m->edge_path == 0 && m->tab0 && K <= 23)
                 done = message_bwd0_v3(L, N, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<int>(m->b_types_s), m->tab0, m->n_species,
-                                       P<int>(m->b_rev), m->filt_img[0], P<float4>(m->b_G), t == T - 1);
+                                       P<int>(m->b_rev), m->filt_rows[0], P<float4>(m->b_G), t == T - 1);
             if (!done && m->edge_path == 0)
                 done = message_bwd_v3(L, N, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<float>(m->b_phi[t]),
                                       P<float>(m->b_V[t]), v1b, m->filt_img[t], phib, vb, P<float4>(m->b_G), t == T - 1, t == 0);

@@ -124,6 +124,7 @@ bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
                     const float* phi, const float* v_in, const float* v1b, const void* A_img, float* phib, float* vb_out,
                     float4* G, bool first, bool layer0);
 
+void edge_build_filter_rows(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img);
 bool message_bwd0_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
                      const int* types_s, const float* tab, int n_tab, const int* rev, const void* A_img, float4* G, bool first);
 

@@ -747,6 +747,27 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
 // at all.  g of edge (i <- j) is produced at the slot of i's row; G is indexed by the slot of the sender's row
 // (force_final: F_a = sum_x G[rev x] - G[x]), so the reducer scatters through the reverse-edge index.
 // =============================================================================================================
+// tcgen05.st: 16 consecutive 32-bit columns of this thread's TMEM lane
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
+        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]),
+        "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+        : "memory");
+}
+// A operand from TMEM (lane = row, 8 columns = 16 fp16 along K), B from shared memory
+__device__ __forceinline__ void umma_f16_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n"
+        "}\n" ::"r"(tmem_d),
+        "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(acc)
+        : "memory");
+}
+
 struct Bwd0Params {
     long long N;
     const int* row_ptr;
@@ -755,7 +776,7 @@ struct Bwd0Params {
     const int* types;
     const float2* tab;     // [n_tab][F] (phi^s, phi^vs) per species
     const int* rev;
-    const uint4* A_img;
+    const uint4* A_img;    // [2 chunks][128 rows][96 fp16] row-major (k = term * 32 + basis slot): TMEM-resident A operand
     float4* G;
     float inv_rc;
     int K;
@@ -764,15 +785,15 @@ struct Bwd0Params {
     int n_tab;
 };
 constexpr int G0_OFF_SPEC = G_OFF_BAR + 128, G0_OFF_TAB = G0_OFF_SPEC + 4 * NEB * 4, GROUP0_BYTES = G0_OFF_TAB;
-constexpr int bwd0_smem_bytes() { return 2 * A_CHUNK_BYTES + 2 * GROUP0_BYTES + TAB_MAX * F * 8 + 128; }
+constexpr int bwd0_smem_bytes() { return 2 * GROUP0_BYTES + TAB_MAX * F * 8 + 128; }
+constexpr int BWD0_TMEM_A = 128;                        // TMEM columns 128..223: the filter operand (2 chunks x 48 columns)
 
 __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p) {
     constexpr int NCH = 2;
     constexpr int TCOLS = NCH * 2 * NEB;
     extern __shared__ __align__(128) uint8_t smem[];
-    uint8_t* sA = smem;
     const int tid = threadIdx.x, grp = tid >> 8, ltid = tid & 255, lwarp = ltid >> 5, lane = tid & 31;
-    uint8_t* gbase = smem + NCH * A_CHUNK_BYTES + grp * GROUP0_BYTES;
+    uint8_t* gbase = smem + grp * GROUP0_BYTES;
     uint8_t* sB = gbase + G_OFF_B;
     uint8_t* sP = gbase + G_OFF_P;
     float4* sMeta = (float4*)(gbase + G_OFF_META);  // [4][NEB] (u_e, 1/d_e)
@@ -781,12 +802,9 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
     uint64_t* t_full = bars;
     uint64_t* p_empty = bars + 2;
     const int NB_TE = 1 + grp * 6, NB_BF = NB_TE + 2, NB_PF = NB_TE + 4;
-    float2* sTab = (float2*)(smem + NCH * A_CHUNK_BYTES + 2 * GROUP0_BYTES);
+    float2* sTab = (float2*)(smem + 2 * GROUP0_BYTES);
     uint32_t* tmem_slot = (uint32_t*)(sTab + TAB_MAX * F);
     {
-        const uint4* src = p.A_img;
-        uint4* dst = (uint4*)sA;
-        for (int i = tid; i < NCH * A_CHUNK_BYTES / 16; i += BWD_THREADS) dst[i] = src[i];
         uint4* zb = (uint4*)sB;
         for (int i = ltid; i < 2 * BB_BYTES / 16; i += 256) zb[i] = make_uint4(0, 0, 0, 0);
         for (int i = tid; i < p.n_tab * F; i += BWD_THREADS) sTab[i] = p.tab[i];
@@ -800,7 +818,29 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
+    // filter operand into TMEM (lane = channel row, 48 columns = 96 fp16 per chunk): the MMAs then read only the small B
+    // operand from shared memory -- the 72 KB image and its re-read by every MMA (ncu: 35 % of the shared-memory data
+    // pipe next to an LSU pipe that was 82 % busy) are gone
+    if (tid < 128) {
+        const uint32_t abase = *tmem_slot + BWD0_TMEM_A + ((uint32_t)((tid >> 5) * 32) << 16);
+#pragma unroll
+        for (int c = 0; c < NCH; c++) {
+            const uint4* src = p.A_img + ((size_t)c * 128 + tid) * 12;       // 96 fp16 = 12 x 16 B
+#pragma unroll
+            for (int j = 0; j < 3; j++) {
+                uint32_t r[16];
+#pragma unroll
+                for (int q = 0; q < 4; q++) { const uint4 v = src[j * 4 + q]; r[4 * q] = v.x; r[4 * q + 1] = v.y; r[4 * q + 2] = v.z; r[4 * q + 3] = v.w; }
+                tmem_st16(abase + c * 48 + j * 16, r);
+            }
+        }
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
     const uint32_t tmem_base = *tmem_slot + grp * 256;
+    const uint32_t tmem_A = *tmem_slot + BWD0_TMEM_A;
     const long long N = p.N;
     const int apu = p.atoms_per_unit;
     const int* __restrict__ row_ptr = p.row_ptr;
@@ -975,7 +1015,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
     } else if (lwarp == 7) {
         // ===================== MMA issuer =====================
         const uint32_t idesc = (1u << 4) | ((uint32_t)((2 * NEB) >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-        const uint32_t a_base = smem_u32(sA), b_base = smem_u32(sB);
+        const uint32_t b_base = smem_u32(sB);
         uint32_t it = 0;
         for (long long u = u0; u < n_units; u += ustride) {
             const long long a0 = u * apu;
@@ -993,9 +1033,8 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
 #pragma unroll
                         for (int o = 0; o < 6; o++) {
                             const int kk = (o + 2) % 6;
-                            const uint64_t ad = make_desc_nosw(a_base + c * A_CHUNK_BYTES + kk * 2 * LBO, LBO, SBO);
                             const uint64_t bd = make_desc_nosw(b_base + buf * BB_BYTES + kk * 2 * LBO, LBO, SBO);
-                            umma_f16(d, ad, bd, idesc, o != 0);
+                            umma_f16_ts(d, tmem_A + c * 48 + kk * 8, bd, idesc, o != 0);
                         }
                     }
                     umma_commit(&t_full[buf]);
@@ -1010,6 +1049,25 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
 }
 
 }  // namespace ev3
+
+// host: filter operand of one layer as plain rows [3 chunks][128 channels][96 fp16], k = term * 32 + basis slot, terms
+// (hi, hi 2^-11, lo 2^11) of (bf | Wf) -- the TMEM-resident A operand of k_msg_bwd0 (same numbers as edge_build_filter_image)
+void edge_build_filter_rows(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img) {
+    img.assign((size_t)3 * ev3::F * ev3::KP, 0);
+    for (int c = 0; c < 3; c++)
+        for (int r = 0; r < ev3::F; r++)
+            for (int b = 0; b <= K; b++) {
+                const float w = b == 0 ? bf[c * ev3::F + r] : Wf[(size_t)(c * ev3::F + r) * K + (b - 1)];
+                const __half hi = __float2half_rn(w);
+                const float hif = __half2float(hi);
+                const __half vals[3] = {hi, __float2half_rn(hif * (1.0f / 2048.0f)), __float2half_rn((w - hif) * 2048.0f)};
+                for (int t = 0; t < 3; t++) {
+                    unsigned short bits;
+                    memcpy(&bits, &vals[t], 2);
+                    img[((size_t)c * ev3::F + r) * ev3::KP + t * 32 + b] = bits;
+                }
+            }
+}
 
 static int sm_count() {
     static int n_sm = 0;
