@@ -659,7 +659,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
                                        P<int>(m->b_rev), m->filt_rows[0], P<float4>(m->b_G), t == T - 1);
             if (!done && m->edge_path == 0)
                 done = message_bwd_v3(L, N, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<float>(m->b_phi[t]),
-                                      P<float>(m->b_V[t]), v1b, m->filt_img[t], phib, vb, P<float4>(m->b_G), t == T - 1, t == 0);
+                                      P<float>(m->b_V[t]), v1b, m->filt_img[t], m->filt_rows[t], phib, vb, P<float4>(m->b_G), t == T - 1, t == 0);
             if (!done && m->edge_path == 3)
                 done = message_bwd_tc2(L, N, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<float>(m->b_phi[t]),
                                        P<float>(m->b_V[t]), v1b, m->filt_img2[t], phib, vb, P<float4>(m->b_G), t == T - 1, true);

@@ -121,8 +121,8 @@ bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
                     const float* v, const float* Q4, const float* Q1, const void* A_img, float* sn, float* v1, bool has_v,
                     const int* types_s = nullptr, const float* tab = nullptr, int n_tab = 0);
 bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
-                    const float* phi, const float* v_in, const float* v1b, const void* A_img, float* phib, float* vb_out,
-                    float4* G, bool first, bool layer0);
+                    const float* phi, const float* v_in, const float* v1b, const void* A_img, const void* A_rows, float* phib,
+                    float* vb_out, float4* G, bool first, bool layer0);
 
 void edge_build_filter_rows(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img);
 bool message_bwd0_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,

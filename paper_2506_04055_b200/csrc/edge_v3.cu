@@ -376,7 +376,28 @@ constexpr int GW = 16;                                  // gather window (edges 
 constexpr int RING_BYTES = GW * F * 16;                 // 32768
 constexpr int G_OFF_B = 0, G_OFF_P = 2 * BB_BYTES, G_OFF_RING = G_OFF_P + 2 * P_BYTES, G_OFF_META = G_OFF_RING + RING_BYTES,
               G_OFF_BAR = G_OFF_META + 4 * NEB * 16, GROUP_BYTES = G_OFF_BAR + 128;
-constexpr int bwd_smem_bytes(int nch) { return nch * A_CHUNK_BYTES + 2 * GROUP_BYTES + 128; }
+constexpr int bwd_smem_bytes(int nch) { return (nch - 2) * A_CHUNK_BYTES + 2 * GROUP_BYTES + 128; }
+
+// tcgen05.st: 16 consecutive 32-bit columns of this thread's TMEM lane
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
+        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]),
+        "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+        : "memory");
+}
+// A operand from TMEM (lane = row, 8 columns = 16 fp16 along K), B from shared memory
+__device__ __forceinline__ void umma_f16_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n"
+        "}\n" ::"r"(tmem_d),
+        "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(acc)
+        : "memory");
+}
 
 struct BwdParams {
     long long N;
@@ -386,7 +407,8 @@ struct BwdParams {
     const float* phi;
     const float* v_in;
     const float* v1b;
-    const uint4* A_img;
+    const uint4* A_img;    // chunk vv of the no-swizzle K-major image (shared-memory A operand)
+    const uint4* A_rows;   // [3][128][96] fp16 rows: chunks s, vs become TMEM-resident A operands
     float* phib;
     float* vb_out;
     float4* G;
@@ -405,7 +427,8 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
     extern __shared__ __align__(128) uint8_t smem[];
     uint8_t* sA = smem;
     const int tid = threadIdx.x, grp = tid >> 8, ltid = tid & 255, lwarp = ltid >> 5, lane = tid & 31;
-    uint8_t* gbase = smem + NCH * A_CHUNK_BYTES + grp * GROUP_BYTES;
+    constexpr int NSM = NCH - 2;                    // chunks kept in shared memory (vv); s and vs live in TMEM
+    uint8_t* gbase = smem + NSM * A_CHUNK_BYTES + grp * GROUP_BYTES;
     uint8_t* sB = gbase + G_OFF_B;
     uint8_t* sP = gbase + G_OFF_P;                 // [2][8] rows of P_ROW bytes: (db, ub_x, ub_y, ub_z) per channel
     float4* sMeta = (float4*)(gbase + G_OFF_META); // [4][NEB] (u of edge (i <- j), 1/d): ring of 4 tiles
@@ -416,12 +439,12 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
     const int NB_TE = 1 + grp * 6;    // consumers (128, arrive) -> producers (64, sync): tile buffer consumed
     const int NB_BF = NB_TE + 2;      // producers (64, arrive) -> MMA warp (32, sync): B operand written
     const int NB_PF = NB_TE + 4;      // consumers (128, arrive) -> reducer (32, sync): partials of one batch written
-    uint32_t* tmem_slot = (uint32_t*)(smem + NCH * A_CHUNK_BYTES + 2 * GROUP_BYTES);
+    uint32_t* tmem_slot = (uint32_t*)(smem + NSM * A_CHUNK_BYTES + 2 * GROUP_BYTES);
 
     {
-        const uint4* src = p.A_img;
+        const uint4* src = p.A_img + 2 * (A_CHUNK_BYTES / 16);
         uint4* dst = (uint4*)sA;
-        for (int i = tid; i < NCH * A_CHUNK_BYTES / 16; i += BWD_THREADS) dst[i] = src[i];
+        for (int i = tid; i < NSM * A_CHUNK_BYTES / 16; i += BWD_THREADS) dst[i] = src[i];
         uint4* zb = (uint4*)sB;
         for (int i = ltid; i < 2 * BB_BYTES / 16; i += 256) zb[i] = make_uint4(0, 0, 0, 0);
     }
@@ -434,7 +457,28 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
+    // chunks s and vs of the filter operand into TMEM (lane = channel row, 48 columns = 96 fp16 each): columns 192..239
+    // and 448..495, the gaps behind the two groups' accumulators (2 x 96 columns each)
+    if (tid < 128) {
+#pragma unroll
+        for (int c = 0; c < 2; c++) {
+            const uint32_t abase = *tmem_slot + 192 + c * 256 + ((uint32_t)((tid >> 5) * 32) << 16);
+            const uint4* src = p.A_rows + ((size_t)c * 128 + tid) * 12;
+#pragma unroll
+            for (int j = 0; j < 3; j++) {
+                uint32_t r[16];
+#pragma unroll
+                for (int q = 0; q < 4; q++) { const uint4 v = src[j * 4 + q]; r[4 * q] = v.x; r[4 * q + 1] = v.y; r[4 * q + 2] = v.z; r[4 * q + 3] = v.w; }
+                tmem_st16(abase + j * 16, r);
+            }
+        }
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
     const uint32_t tmem_base = *tmem_slot + grp * 256;
+    const uint32_t tmem_A = *tmem_slot + 192;
     const long long N = p.N;
     const int apu = p.atoms_per_unit;
     const int* __restrict__ row_ptr = p.row_ptr;
@@ -724,9 +768,9 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
 #pragma unroll
                         for (int o = 0; o < 6; o++) {
                             const int kk = (o + 2) % 6;
-                            const uint64_t ad = make_desc_nosw(a_base + c * A_CHUNK_BYTES + kk * 2 * LBO, LBO, SBO);
                             const uint64_t bd = make_desc_nosw(b_base + buf * BB_BYTES + kk * 2 * LBO, LBO, SBO);
-                            umma_f16(d, ad, bd, idesc, o != 0);
+                            if (c < 2) umma_f16_ts(d, tmem_A + c * 256 + kk * 8, bd, idesc, o != 0);
+                            else umma_f16(d, make_desc_nosw(a_base + kk * 2 * LBO, LBO, SBO), bd, idesc, o != 0);
                         }
                     }
                     umma_commit(&t_full[buf]);
@@ -747,27 +791,6 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
 // at all.  g of edge (i <- j) is produced at the slot of i's row; G is indexed by the slot of the sender's row
 // (force_final: F_a = sum_x G[rev x] - G[x]), so the reducer scatters through the reverse-edge index.
 // =============================================================================================================
-// tcgen05.st: 16 consecutive 32-bit columns of this thread's TMEM lane
-__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {
-    asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
-        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
-        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]),
-        "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
-        : "memory");
-}
-// A operand from TMEM (lane = row, 8 columns = 16 fp16 along K), B from shared memory
-__device__ __forceinline__ void umma_f16_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "setp.ne.b32 p, %4, 0;\n"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n"
-        "}\n" ::"r"(tmem_d),
-        "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(acc)
-        : "memory");
-}
-
 struct Bwd0Params {
     long long N;
     const int* row_ptr;
@@ -1106,8 +1129,8 @@ bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
 
 // layer0: v_in = 0 and no sender adjoint wanted (phib / vb_out untouched)
 bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
-                    const float* phi, const float* v_in, const float* v1b, const void* A_img, float* phib, float* vb_out,
-                    float4* G, bool first, bool layer0) {
+                    const float* phi, const float* v_in, const float* v1b, const void* A_img, const void* A_rows, float* phib,
+                    float* vb_out, float4* G, bool first, bool layer0) {
     using namespace ev3;
     if (N == 0) return true;
     if (K > 23) return false;
@@ -1118,8 +1141,8 @@ bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
             return false;
         attr = true;
     }
-    BwdParams p{N, row_ptr, ej, (const float4*)Gb, phi, v_in, v1b, (const uint4*)A_img, phib, vb_out, G, 1.0f / rc, K, 16,
-                first ? 1 : 0};
+    BwdParams p{N, row_ptr, ej, (const float4*)Gb, phi, v_in, v1b, (const uint4*)A_img, (const uint4*)A_rows, phib, vb_out, G,
+                1.0f / rc, K, 16, first ? 1 : 0};
     const long long n_units = (N + p.atoms_per_unit - 1) / p.atoms_per_unit;
     const int grid = (int)std::min<long long>((n_units + 1) / 2, (long long)sm_count());
     if (layer0) k_msg_bwd<true><<<grid, BWD_THREADS, bwd_smem_bytes(2), L.stream>>>(p);
