@@ -252,15 +252,14 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
 // Each output tile walks its K blocks twice: pass 0 streams A through the ring to find the row maxima (exponents
 // e_m), pass 1 streams A (an L2 hit) and the weight slices again, converts A into its three slices in shared memory
 // and runs the MMAs.  Same warp roles and barriers as k_gemm_3xtf32; ACT applies SiLU to A while converting.
-constexpr int XBN = 64, XWST = 3, XRAW = 3;
+constexpr int XBN = 32, XWST = 4, XRAW = 3;
 constexpr int XTHREADS = NUM_THREADS + 32;                              // + warp 10: second TMA producer (raw A blocks)
-constexpr int XSL_BLK = BM * 128;                                       // 16 KB: 128 rows x 64 fp16 (one K half of one slice)
-constexpr int XSL = 3 * 2 * XSL_BLK;                                    // 96 KB: A slices [3][2 K halves], resident per unit
-constexpr int XW_TILE = XBN * 128;                                      // 8 KB: 64 rows x 64 fp16
-constexpr int XW_STAGE = 3 * XW_TILE;                                   // 24 KB: the three weight slices of one (N tile, K half)
+constexpr int XW_TILE = XBN * 128;                                      // 4 KB: 32 rows x 64 fp16 (one slice, one K half)
+constexpr int XW_STAGE = 3 * 2 * XW_TILE;                               // 24 KB: the three weight slices of one N tile, K = 128
 constexpr int XNMAX = 512;                                              // widest N (column scale and bias are staged in shared memory)
-constexpr int XSMEM = XSL + XRAW * A_TILE_BYTES + XWST * XW_STAGE + 4 * BM * 4 + 2 * XNMAX * 4 + 256 + 1024;
-constexpr int XACC = 4 * XBN;                                           // TMEM columns per accumulator set (S2..S5)
+constexpr int XSMEM = XRAW * A_TILE_BYTES + XWST * XW_STAGE + 4 * BM * 4 + 2 * XNMAX * 4 + 256 + 1024;
+constexpr int XTM_A = 0;                                                // TMEM columns 0..191: A slices [3][64 columns = 128 fp16]
+constexpr int XTM_ACC = 192, XACC = 4 * XBN;                            // TMEM columns 192..447: 2 accumulator sets (S2..S5 x 32)
 
 struct XParams {
     float* C;
@@ -271,17 +270,36 @@ struct XParams {
 };
 
 __device__ __forceinline__ float silu_x(float x) { return x / (1.0f + __expf(-x)); }
+__device__ __forceinline__ void tmem_st16x(uint32_t taddr, const uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
+        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]),
+        "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+        : "memory");
+}
+__device__ __forceinline__ void umma_f16_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n"
+        "}\n" ::"r"(tmem_d),
+        "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(acc)
+        : "memory");
+}
 
 // Work unit = one 128-row block of A with ALL its N tiles.  The raw fp32 blocks of A stream twice through a small
-// ring (pass 0: row maxima -> exponents; pass 1: conversion, an L2 hit); the fp16 integer slices of the whole block
-// (K = 128) then stay resident while the N tiles run, fed by a 3-stage ring of weight slices.
+// ring (pass 0: row maxima -> exponents; pass 1: conversion, an L2 hit).  The fp16 integer slices of the whole block
+// (K = 128) are written straight into TENSOR MEMORY (one row per lane, tcgen05.st) and stay there while the N tiles
+// run: the MMAs take A from TMEM and only the small weight-slice tiles from shared memory (with A in shared memory the
+// kernel was bound by re-reading 4 KB of A for every N = 64 MMA: 85 cycles per MMA instead of 32).
 template <bool ACT>
 __global__ void __launch_bounds__(XTHREADS, 1)
     k_gemm_exact(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapW1,
                  const __grid_constant__ CUtensorMap mapW2, const __grid_constant__ CUtensorMap mapW3, XParams p) {
     extern __shared__ __align__(1024) uint8_t smem[];
-    uint8_t* sl = smem;                                               // A slices
-    uint8_t* raw = sl + XSL;                                          // [XRAW] raw A blocks (128 rows x 32 fp32, SWIZZLE_128B)
+    uint8_t* raw = smem;                                              // [XRAW] raw A blocks (128 rows x 32 fp32, SWIZZLE_128B)
     uint8_t* wst = raw + XRAW * A_TILE_BYTES;                         // [XWST] weight-slice stages
     float* rowscale = (float*)(wst + XWST * XW_STAGE);                // [4][BM]  2^(e_m - 14) of the last four units
     float* s_cs = rowscale + 4 * BM;                                  // [N] column scales 2^f_n
@@ -322,16 +340,18 @@ __global__ void __launch_bounds__(XTHREADS, 1)
             int ws = 0;
             uint32_t wphase = 0;
             for (long long u = blockIdx.x; u < units; u += gridDim.x)
-                for (int nt = 0; nt < n_tiles; nt++)
+                for (int nt = 0; nt < n_tiles; nt++) {
+                    mbar_wait(&wempty[ws], wphase ^ 1);
+                    uint8_t* st = wst + ws * XW_STAGE;
+                    mbar_expect_tx(&wfull[ws], XW_STAGE);
+#pragma unroll
                     for (int kh = 0; kh < 2; kh++) {
-                        mbar_wait(&wempty[ws], wphase ^ 1);
-                        uint8_t* st = wst + ws * XW_STAGE;
-                        mbar_expect_tx(&wfull[ws], XW_STAGE);
-                        tma_load_2d(st, &mapW1, &wfull[ws], kh * 64, nt * XBN);
-                        tma_load_2d(st + XW_TILE, &mapW2, &wfull[ws], kh * 64, nt * XBN);
-                        tma_load_2d(st + 2 * XW_TILE, &mapW3, &wfull[ws], kh * 64, nt * XBN);
-                        if (++ws == XWST) { ws = 0; wphase ^= 1; }
+                        tma_load_2d(st + (0 * 2 + kh) * XW_TILE, &mapW1, &wfull[ws], kh * 64, nt * XBN);
+                        tma_load_2d(st + (1 * 2 + kh) * XW_TILE, &mapW2, &wfull[ws], kh * 64, nt * XBN);
+                        tma_load_2d(st + (2 * 2 + kh) * XW_TILE, &mapW3, &wfull[ws], kh * 64, nt * XBN);
                     }
+                    if (++ws == XWST) { ws = 0; wphase ^= 1; }
+                }
         }
     } else if (warp == 10) {
         // The two TMA producers must not share a warp: UTMALDG / SYNCS run on the warp's uniform datapath, and two
@@ -355,10 +375,10 @@ __global__ void __launch_bounds__(XTHREADS, 1)
                 }
         }
     } else if (warp == 1) {
-        // ===================== MMA issuer =====================
-        if (lane == 0) {
+        // ===================== MMA issuer: the warp stays converged, one elected lane issues =====================
+        {
             const uint32_t idesc = (1u << 4) | ((uint32_t)(XBN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);   // f16 x f16 -> f32
-            const uint32_t sl_base = smem_u32(sl);
+            const uint32_t ta = tmem_base + XTM_A;
             int ws = 0;
             uint32_t wphase = 0, uphase = 0;
             int buf = 0;
@@ -368,130 +388,116 @@ __global__ void __launch_bounds__(XTHREADS, 1)
                 tc_fence_after();
                 for (int nt = 0; nt < n_tiles; nt++) {
                     mbar_wait(&tempty[buf], bphase ^ 1);
+                    mbar_wait(&wfull[ws], wphase);
                     tc_fence_after();
-                    const uint32_t d = tmem_base + buf * XACC;
-                    for (int kh = 0; kh < 2; kh++) {
-                        mbar_wait(&wfull[ws], wphase);
-                        tc_fence_after();
-                        const uint32_t sw = smem_u32(wst + ws * XW_STAGE);
-                        uint64_t a[3], w[3];
+                    const uint32_t d = tmem_base + XTM_ACC + buf * XACC;
+                    const uint32_t sw = smem_u32(wst + ws * XW_STAGE);
+                    if (elect_one()) {
 #pragma unroll
-                        for (int i = 0; i < 3; i++) {
-                            a[i] = make_desc_sw128(sl_base + (i * 2 + kh) * XSL_BLK);
-                            w[i] = make_desc_sw128(sw + i * XW_TILE);
-                        }
+                        for (int kh = 0; kh < 2; kh++) {
+                            uint64_t w[3];
 #pragma unroll
-                        for (int kk = 0; kk < 4; kk++) {             // 16 fp16 = 32 B along K per MMA
-                            const uint64_t o = (uint64_t)(kk * 2);
-                            const uint32_t acc = (kh | kk) != 0;
-                            umma_f16(d, a[0] + o, w[0] + o, idesc, acc);                   // S2: (1,1)
-                            umma_f16(d + XBN, a[0] + o, w[1] + o, idesc, acc);             // S3: (1,2) (2,1)
-                            umma_f16(d + XBN, a[1] + o, w[0] + o, idesc, 1);
-                            umma_f16(d + 2 * XBN, a[0] + o, w[2] + o, idesc, acc);         // S4: (1,3) (2,2) (3,1)
-                            umma_f16(d + 2 * XBN, a[1] + o, w[1] + o, idesc, 1);
-                            umma_f16(d + 2 * XBN, a[2] + o, w[0] + o, idesc, 1);
-                            umma_f16(d + 3 * XBN, a[1] + o, w[2] + o, idesc, acc);         // S5: (2,3) (3,2)
-                            umma_f16(d + 3 * XBN, a[2] + o, w[1] + o, idesc, 1);
+                            for (int i = 0; i < 3; i++) w[i] = make_desc_sw128(sw + (i * 2 + kh) * XW_TILE);
+#pragma unroll
+                            for (int kk = 0; kk < 4; kk++) {             // 16 fp16 along K = 8 TMEM columns of A, 32 B of a W row
+                                const uint64_t o = (uint64_t)(kk * 2);
+                                const uint32_t a0 = ta + kh * 32 + kk * 8, a1 = a0 + 64, a2 = a0 + 128;
+                                const uint32_t acc = (kh | kk) != 0;
+                                // S2: (1,1)   S3: (1,2) (2,1)   S4: (1,3) (2,2) (3,1)   S5: (2,3) (3,2)
+                                umma_f16_ts(d, a0, w[0] + o, idesc, acc);
+                                umma_f16_ts(d + XBN, a0, w[1] + o, idesc, acc);
+                                umma_f16_ts(d + 2 * XBN, a0, w[2] + o, idesc, acc);
+                                umma_f16_ts(d + 3 * XBN, a1, w[2] + o, idesc, acc);
+                                umma_f16_ts(d + XBN, a1, w[0] + o, idesc, 1);
+                                umma_f16_ts(d + 2 * XBN, a1, w[1] + o, idesc, 1);
+                                umma_f16_ts(d + 3 * XBN, a2, w[1] + o, idesc, 1);
+                                umma_f16_ts(d + 2 * XBN, a2, w[0] + o, idesc, 1);
+                            }
                         }
                         umma_commit(&wempty[ws]);
-                        if (++ws == XWST) { ws = 0; wphase ^= 1; }
+                        umma_commit(&tfull[buf]);
+                        if (nt == n_tiles - 1) umma_commit(sl_free);
                     }
-                    umma_commit(&tfull[buf]);
+                    __syncwarp();
+                    if (++ws == XWST) { ws = 0; wphase ^= 1; }
                     if (++buf == 2) { buf = 0; bphase ^= 1; }
                 }
-                umma_commit(sl_free);
                 uphase ^= 1;
             }
         }
     } else if (warp < EPI_WARP0) {
-        // ===================== converter: row maxima (pass 0), fp16 integer slices (pass 1) =====================
-        // thread ct handles the 32-byte chunk PAIRS id = ct + 128 i (i < 4): row r = id >> 2 = (ct >> 2) + 32 i, physical
-        // pair pp = ct & 3.  SWIZZLE_128B stores logical 16-byte chunk c of row r at chunk c ^ (r & 7), so the pair holds
-        // the 8 consecutive K values of logical pair pp ^ ((r & 7) >> 1), the two halves swapped when r is odd.
-        const int ct = threadIdx.x - CONV_WARP0 * 32;
-        const int pp = ct & 3, r0 = ct >> 2;
+        // ===================== converter: one row per thread (= TMEM lane) =====================
+        // SWIZZLE_128B stores logical 16-byte chunk c of row r at chunk c ^ (r & 7): reading the chunks in logical order is
+        // conflict-free for the 8 consecutive rows of a quarter-warp.
+        const int row = (warp & 3) * 32 + lane;
+        const uint32_t trow = tmem_base + XTM_A + ((uint32_t)((warp & 3) * 32) << 16);
+        const int rx = row & 7;
         int rs = 0;
         uint32_t rphase = 0, uphase = 0;
         uint32_t ucount = 0;
         const float MAGIC = 12582912.0f;                // 1.5 * 2^23: (t + MAGIC) - MAGIC = round-to-nearest-even integer
         for (long long u = blockIdx.x; u < units; u += gridDim.x, ucount++) {
-            float mx[4];
-#pragma unroll
-            for (int i = 0; i < 4; i++) mx[i] = 0.f;
+            float mx = 0.f;
             for (int kb = 0; kb < kblocks; kb++) {
                 mbar_wait(&rfull[rs], rphase);
-                const float4* a = (const float4*)(raw + rs * A_TILE_BYTES);
+                const float4* a = (const float4*)(raw + rs * A_TILE_BYTES + row * 128);
 #pragma unroll
-                for (int i = 0; i < 4; i++) {
-#pragma unroll
-                    for (int h = 0; h < 2; h++) {
-                        float4 x = a[(ct + i * 128) * 2 + h];
-                        if (ACT) { x.x = silu_x(x.x); x.y = silu_x(x.y); x.z = silu_x(x.z); x.w = silu_x(x.w); }
-                        mx[i] = fmaxf(mx[i], fmaxf(fmaxf(fabsf(x.x), fabsf(x.y)), fmaxf(fabsf(x.z), fabsf(x.w))));
-                    }
+                for (int c = 0; c < 8; c++) {
+                    float4 x = a[c ^ rx];
+                    if (ACT) { x.x = silu_x(x.x); x.y = silu_x(x.y); x.z = silu_x(x.z); x.w = silu_x(x.w); }
+                    mx = fmaxf(mx, fmaxf(fmaxf(fabsf(x.x), fabsf(x.y)), fmaxf(fabsf(x.z), fabsf(x.w))));
                 }
                 // Release to the TMA producer.  The refill is an ASYNC-proxy write to bytes this thread has just read through
                 // the generic proxy: without a proxy fence the two are not ordered even across the mbarrier (measured: ~2 %
                 // of the rows saw part of the next block in pass 0 and got a different, still valid, exponent run to run).
-                asm volatile("" ::"f"(mx[0]), "f"(mx[1]), "f"(mx[2]), "f"(mx[3]) : "memory");
+                asm volatile("" ::"f"(mx) : "memory");
                 fence_async_smem();
                 mbar_arrive(&rempty[rs]);
                 if (++rs == XRAW) { rs = 0; rphase ^= 1; }
             }
-            float q128[4];                               // 128 / 2^e_m
-#pragma unroll
-            for (int i = 0; i < 4; i++) {
-                float m = mx[i];
-                m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));
-                m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
-                // 2^e = smallest power of two > m; non-finite / huge rows fall through as garbage / NaN downstream
-                const uint32_t E = (__float_as_uint(m) >> 23) & 0xffu;       // m in [2^(E-127), 2^(E-126))
-                const uint32_t Ec = E < 20u ? 20u : (E > 230u ? 230u : E);   // keep every scale a normal number
-                q128[i] = __uint_as_float((260u - Ec) << 23);                // 2^(126 - E) * 128
-                if (pp == 0) rowscale[(ucount & 3) * BM + r0 + 32 * i] = __uint_as_float((Ec - 13u) << 23);   // 2^(e - 14)
-            }
+            // 2^e = smallest power of two > max |x|; non-finite / huge rows fall through as garbage / NaN downstream
+            const uint32_t E = (__float_as_uint(mx) >> 23) & 0xffu;      // mx in [2^(E-127), 2^(E-126))
+            const uint32_t Ec = E < 20u ? 20u : (E > 230u ? 230u : E);   // keep every scale a normal number
+            const float q128 = __uint_as_float((260u - Ec) << 23);       // 128 / 2^e
+            rowscale[(ucount & 3) * BM + row] = __uint_as_float((Ec - 13u) << 23);   // 2^(e - 14)
             mbar_wait(sl_free, uphase ^ 1);              // the previous unit's MMAs no longer read the slices
             uphase ^= 1;
+            tc_fence_after();
             for (int kb = 0; kb < kblocks; kb++) {
                 mbar_wait(&rfull[rs], rphase);
-                const float4* a = (const float4*)(raw + rs * A_TILE_BYTES);
-                const int kh = kb >> 1;
+                const float4* a = (const float4*)(raw + rs * A_TILE_BYTES + row * 128);
+                uint32_t h1[16], h2[16], h3[16];          // 32 K values x 3 slices, two fp16 per TMEM column
 #pragma unroll
-                for (int i = 0; i < 4; i++) {
-                    const int r = r0 + 32 * i;
-                    float4 lo = a[(ct + i * 128) * 2], hi = a[(ct + i * 128) * 2 + 1];
-                    if (r & 1) { const float4 t = lo; lo = hi; hi = t; }
-                    float x[8] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
-                    float s1[8], s2[8], s3[8];
+                for (int c = 0; c < 8; c++) {
+                    const float4 v = a[c ^ rx];
+                    const float x[4] = {v.x, v.y, v.z, v.w};
+                    float s1[4], s2[4], s3[4];
 #pragma unroll
-                    for (int j = 0; j < 8; j++) {
+                    for (int j = 0; j < 4; j++) {
                         const float xv = ACT ? silu_x(x[j]) : x[j];
-                        const float t1 = xv * q128[i];
+                        const float t1 = xv * q128;
                         s1[j] = (t1 + MAGIC) - MAGIC;
                         const float t2 = (t1 - s1[j]) * 256.0f;
                         s2[j] = (t2 + MAGIC) - MAGIC;
                         const float t3 = (t2 - s2[j]) * 256.0f;
                         s3[j] = (t3 + MAGIC) - MAGIC;
                     }
-                    // logical fp16 chunk of this (row, 8 K values) inside the 64-wide K half, and its swizzled position
-                    const int c16 = ((kb & 1) * 4 + (pp ^ ((r & 7) >> 1))) ^ (r & 7);
-                    uint8_t* dst = sl + kh * XSL_BLK + r * 128 + c16 * 16;
-                    __half2 h1[4], h2[4], h3[4];
 #pragma unroll
-                    for (int j = 0; j < 4; j++) {
-                        h1[j] = __floats2half2_rn(s1[2 * j], s1[2 * j + 1]);
-                        h2[j] = __floats2half2_rn(s2[2 * j], s2[2 * j + 1]);
-                        h3[j] = __floats2half2_rn(s3[2 * j], s3[2 * j + 1]);
+                    for (int j = 0; j < 2; j++) {
+                        __half2 p1 = __floats2half2_rn(s1[2 * j], s1[2 * j + 1]), p2 = __floats2half2_rn(s2[2 * j], s2[2 * j + 1]),
+                                p3 = __floats2half2_rn(s3[2 * j], s3[2 * j + 1]);
+                        h1[2 * c + j] = *(uint32_t*)&p1; h2[2 * c + j] = *(uint32_t*)&p2; h3[2 * c + j] = *(uint32_t*)&p3;
                     }
-                    *(uint4*)(dst) = *(uint4*)h1;
-                    *(uint4*)(dst + 2 * XSL_BLK) = *(uint4*)h2;
-                    *(uint4*)(dst + 4 * XSL_BLK) = *(uint4*)h3;
                 }
-                fence_async_smem();                      // same cross-proxy release as in pass 0
+                fence_async_smem();                      // cross-proxy release of the raw block (see pass 0)
                 mbar_arrive(&rempty[rs]);
                 if (++rs == XRAW) { rs = 0; rphase ^= 1; }
+                tmem_st16x(trow + kb * 16, h1);
+                tmem_st16x(trow + 64 + kb * 16, h2);
+                tmem_st16x(trow + 128 + kb * 16, h3);
             }
-            fence_async_smem();
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            tc_fence_before();
             mbar_arrive(sl_ready);
         }
     } else if (warp < 10) {
@@ -508,8 +514,8 @@ __global__ void __launch_bounds__(XTHREADS, 1)
                 tc_fence_after();
                 const float rs = rowscale[(ucount & 3) * BM + q * 32 + lane];
                 float* crow = p.C + row * p.ldc + n0;
-                const uint32_t tb = tmem_base + ((uint32_t)(q * 32) << 16) + buf * XACC;
-#pragma unroll 1
+                const uint32_t tb = tmem_base + XTM_ACC + ((uint32_t)(q * 32) << 16) + buf * XACC;
+#pragma unroll
                 for (int c0 = 0; c0 < XBN; c0 += 16) {
                     uint32_t r2[16], r3[16], r4[16], r5[16];
                     float4 o[4];
@@ -522,6 +528,11 @@ __global__ void __launch_bounds__(XTHREADS, 1)
                     tmem_ld16_nowait(tb + 2 * XBN + c0, r4);
                     tmem_ld16_nowait(tb + 3 * XBN + c0, r5);
                     tmem_wait_ld();
+                    if (c0 + 16 == XBN) {                // last read of this accumulator set: hand it back before the stores
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(&tempty[buf]);
+                    }
                     if (row < p.M) {
 #pragma unroll
                         for (int c = 0; c < 16; c += 4) {
@@ -542,9 +553,6 @@ __global__ void __launch_bounds__(XTHREADS, 1)
                         }
                     }
                 }
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&tempty[buf]);
                 if (++buf == 2) { buf = 0; bphase ^= 1; }
             }
         }
