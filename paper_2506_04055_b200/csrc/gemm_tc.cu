@@ -125,8 +125,8 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
             }
         }
     } else if (warp == 1) {
-        // ===================== MMA issuer =====================
-        if (lane == 0) {
+        // ===================== MMA issuer: converged warp, one elected lane issues =====================
+        {
             const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
             int stage = 0;
             uint32_t phase = 0;
@@ -140,20 +140,23 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
                     mbar_wait(&conv[stage], phase);
                     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                     const uint32_t sa = smem_u32(smem + stage * S::STAGE);
-                    const uint64_t a_hi = make_desc_sw128(sa), a_lo = make_desc_sw128(sa + A_TILE_BYTES);
-                    const uint64_t w_hi = make_desc_sw128(sa + 2 * A_TILE_BYTES),
-                                   w_lo = make_desc_sw128(sa + 2 * A_TILE_BYTES + S::B_TILE);
+                    if (elect_one()) {
+                        const uint64_t a_hi = make_desc_sw128(sa), a_lo = make_desc_sw128(sa + A_TILE_BYTES);
+                        const uint64_t w_hi = make_desc_sw128(sa + 2 * A_TILE_BYTES),
+                                       w_lo = make_desc_sw128(sa + 2 * A_TILE_BYTES + S::B_TILE);
 #pragma unroll
-                    for (int kk = 0; kk < BK / 8; kk++) {
-                        const uint64_t o = (uint64_t)(kk * 2);   // 32 B along K inside the swizzle row, >> 4
-                        umma_tf32(d, a_lo + o, w_hi + o, idesc, (kb | kk) != 0);
-                        umma_tf32(d, a_hi + o, w_lo + o, idesc, 1);
-                        umma_tf32(d, a_hi + o, w_hi + o, idesc, 1);
+                        for (int kk = 0; kk < BK / 8; kk++) {
+                            const uint64_t o = (uint64_t)(kk * 2);   // 32 B along K inside the swizzle row, >> 4
+                            umma_tf32(d, a_lo + o, w_hi + o, idesc, (kb | kk) != 0);
+                            umma_tf32(d, a_hi + o, w_lo + o, idesc, 1);
+                            umma_tf32(d, a_hi + o, w_hi + o, idesc, 1);
+                        }
+                        umma_commit(&empty[stage]);
+                        if (kb == kblocks - 1) umma_commit(&tfull[buf]);
                     }
-                    umma_commit(&empty[stage]);
+                    __syncwarp();
                     if (++stage == STAGES) { stage = 0; phase ^= 1; }
                 }
-                umma_commit(&tfull[buf]);
                 if (++buf == 2) { buf = 0; bphase ^= 1; }
             }
         }
