@@ -326,8 +326,8 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
             }
         }
     } else {
-        // ===================== MMA issuer =====================
-        if (lane == 0) {
+        // ===================== MMA issuer: the warp stays converged, one elected lane issues (descriptors in uniform registers) =====================
+        {
             const uint32_t idesc = (1u << 4) | ((uint32_t)(NE >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);   // f16 x f16 -> f32
             const uint32_t a_base = smem_u32(sA), b_base = smem_u32(sB);
             uint32_t it = 0;
@@ -340,18 +340,21 @@ __global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
                     const int buf = it & 1;
                     mbar_wait_sleep(&b_full[buf], (it >> 1) & 1, 128);
                     tc_fence_after();
+                    if (elect_one()) {
 #pragma unroll
-                    for (int c = 0; c < NCH; c++) {
-                        const uint32_t d = tmem_base + buf * TCOLS + c * NE;
+                        for (int c = 0; c < NCH; c++) {
+                            const uint32_t d = tmem_base + buf * TCOLS + c * NE;
 #pragma unroll
-                        for (int o = 0; o < 6; o++) {
-                            const int kk = (o + 2) % 6;          // small terms (k-steps 2..5) first, main term last
-                            const uint64_t ad = make_desc_nosw(a_base + c * A_CHUNK_BYTES + kk * 2 * LBO, LBO, SBO);
-                            const uint64_t bd = make_desc_nosw(b_base + buf * B_BYTES + kk * 2 * LBO, LBO, SBO);
-                            umma_f16(d, ad, bd, idesc, o != 0);
+                            for (int o = 0; o < 6; o++) {
+                                const int kk = (o + 2) % 6;          // small terms (k-steps 2..5) first, main term last
+                                const uint64_t ad = make_desc_nosw(a_base + c * A_CHUNK_BYTES + kk * 2 * LBO, LBO, SBO);
+                                const uint64_t bd = make_desc_nosw(b_base + buf * B_BYTES + kk * 2 * LBO, LBO, SBO);
+                                umma_f16(d, ad, bd, idesc, o != 0);
+                            }
                         }
+                        umma_commit(&t_full[buf]);
                     }
-                    umma_commit(&t_full[buf]);
+                    __syncwarp();
                 }
             }
         }
@@ -761,7 +764,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                 const int buf = it & 1;
                 bar_sync(NB_BF + buf, 96);
                 tc_fence_after();
-                if (lane == 0) {
+                if (elect_one()) {
 #pragma unroll
                     for (int c = 0; c < NCH; c++) {
                         const uint32_t d = tmem_base + buf * TCOLS + c * 2 * NEB;
@@ -1049,7 +1052,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
                 const int buf = it & 1;
                 bar_sync(NB_BF + buf, 96);
                 tc_fence_after();
-                if (lane == 0) {
+                if (elect_one()) {
 #pragma unroll
                     for (int c = 0; c < NCH; c++) {
                         const uint32_t d = tmem_base + buf * TCOLS + c * 2 * NEB;
