@@ -32,24 +32,46 @@ SMALL_MODEL = dict(n_species=2, F=8, K=6, T=2, rc=5.0, wseed=11)
 
 
 # ------------------------------------------------------------------ finite differences
-def test_forces_match_finite_differences_config1(cfg1):
-    """All 576 coordinates of config 1, |dF| <= 1e-6 (BASELINE.json).  4th-order central stencil at
-    h = 1e-4 A (reading A21: the K = 16 basis makes the 2-point truncation term ~1e-6 itself)."""
-    c = cfg1
-    ref = oracle.compute(c["blob"], c["pos"], c["types"], c["box"])
-    h = 1e-4
-    F_fd = np.zeros_like(ref["forces"])
-
-    def E(p):
-        return oracle.compute(c["blob"], p, c["types"], c["box"])["energy"]
-
-    for a in range(c["pos"].shape[0]):
+def _fd_rows(args):
+    """Worker of the finite-difference pin: 4th-order central differences of the oracle energy for a range of atoms.
+    Runs in its own process with one OpenMP thread (a 192-atom evaluation does not scale over threads; eight
+    single-threaded workers are ~3x faster than eight OpenMP threads on one evaluation at a time)."""
+    blob, pos, types, box, lo, hi, h = args
+    import oracle as orc
+    out = np.zeros((hi - lo, 3))
+    for a in range(lo, hi):
         for d in range(3):
             e = []
             for k in (1, -1, 2, -2):
-                p = c["pos"].copy(); p[a, d] += k * h
-                e.append(E(p))
-            F_fd[a, d] = -(8 * (e[0] - e[1]) - (e[2] - e[3])) / (12 * h)
+                p = pos.copy(); p[a, d] += k * h
+                e.append(orc.compute(blob, p, types, box)["energy"])
+            out[a - lo, d] = -(8 * (e[0] - e[1]) - (e[2] - e[3])) / (12 * h)
+    return lo, out
+
+
+def _fd_init():
+    import os
+    os.environ["OMP_NUM_THREADS"] = "1"
+
+
+def test_forces_match_finite_differences_config1(cfg1):
+    """All 576 coordinates of config 1, |dF| <= 1e-6 (BASELINE.json).  4th-order central stencil at
+    h = 1e-4 A (reading A21: the K = 16 basis makes the 2-point truncation term ~1e-6 itself)."""
+    import multiprocessing as mp
+    import os
+    from concurrent.futures import ProcessPoolExecutor
+    c = cfg1
+    ref = oracle.compute(c["blob"], c["pos"], c["types"], c["box"])
+    h = 1e-4
+    n = c["pos"].shape[0]
+    nw = max(1, min(os.cpu_count() or 1, 16))
+    bounds = np.linspace(0, n, 4 * nw + 1).astype(int)
+    jobs = [(c["blob"], c["pos"], c["types"], c["box"], int(bounds[i]), int(bounds[i + 1]), h)
+            for i in range(len(bounds) - 1) if bounds[i + 1] > bounds[i]]
+    F_fd = np.zeros_like(ref["forces"])
+    with ProcessPoolExecutor(max_workers=nw, mp_context=mp.get_context("spawn"), initializer=_fd_init) as ex:
+        for lo, out in ex.map(_fd_rows, jobs):
+            F_fd[lo:lo + len(out)] = out
     err = np.abs(F_fd - ref["forces"]).max()
     assert err <= 1e-6, err
 
