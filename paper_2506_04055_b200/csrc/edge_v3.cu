@@ -375,6 +375,7 @@ constexpr int BWD_THREADS = 512;
 constexpr int P_ROW = 3 * F * 4 + 64;                   // per-edge partials: x | y | z planes of 128 floats (+64 B: the two rows
                                                         // read by one quarter-warp of the reducer fall into different banks)
 constexpr int P_BYTES = 8 * P_ROW;                      // one 8-edge batch
+constexpr int BWD_PD = 3;                               // consumer loop: shared-memory loads run this many edges ahead
 constexpr int GW = 16;                                  // gather window (edges in flight per thread)
 constexpr int RING_BYTES = GW * F * 16;                 // 32768
 constexpr int G_OFF_B = 0, G_OFF_P = 2 * BB_BYTES, G_OFF_RING = G_OFF_P + 2 * P_BYTES, G_OFF_META = G_OFF_RING + RING_BYTES,
@@ -516,16 +517,18 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
             const int n_e = e_end - e_begin;
             const int ntiles = (n_e + NEB - 1) / NEB;
             // sender indices of the unit's edges, 32 per register (lane l <-> edge 32 blk + l); padding slots -> own row
+            // (returned raw: padding slots carry ~own row; the sign is folded after the shuffle, so that nothing
+            // waits for the load where it is issued)
             auto load_idx = [&](int blk) -> int {
                 const int E = e_begin + 32 * blk + lane;
-                const int ix = E < e_end ? __float_as_int(__ldg(ejp + E).w) : 0;
-                return ix < 0 ? ~ix : ix;
+                return E < e_end ? __float_as_int(__ldg(ejp + E).w) : 0;
             };
             int idx0 = load_idx(0), idx1 = load_idx(1);
             if (ntiles > 0) {
 #pragma unroll
                 for (int i = 0; i < GW; i++) {
-                    const int j = __shfl_sync(0xffffffffu, idx0, i);
+                    int j = __shfl_sync(0xffffffffu, idx0, i);
+                    j = j < 0 ? ~j : j;
                     if (i < n_e) cp_async16(ring + i * F, Gb + (size_t)j * F);
                     if ((i & 7) == 7) cp_async_commit();            // one commit group per 8-edge batch
                 }
@@ -588,9 +591,21 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
             tmem_wait_ld();                                                                                       \
             cp_async_wait<1>();              /* this batch's rows have landed; the next batch's stay in flight */ \
             uint8_t* pdst_ = sP + (hc & 1) * P_BYTES;                                                             \
+            /* the loads of edge i + BWD_PD are issued before the partials of edge i are stored: ptxas cannot */  \
+            /* prove that the stores to sP do not alias the ring, and would otherwise expose the full LDS     */  \
+            /* latency once per edge (measured: 25 % of the consumers' time)                                  */  \
+            float4 mq_[8], gq_[8];                                                                                \
+            _Pragma("unroll") for (int i_ = 0; i_ < BWD_PD; i_++) {                                               \
+                mq_[i_] = meta[(H) * 8 + i_];                                                                     \
+                gq_[i_] = ring[((H) * 8 + i_) * F];                                                               \
+            }                                                                                                     \
             _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                                    \
-                const float4 m_ = meta[(H) * 8 + i_];                                                             \
-                const float4 g_ = ring[((H) * 8 + i_) * F];                                                       \
+                if (i_ + BWD_PD < 8) {                                                                            \
+                    mq_[i_ + BWD_PD] = meta[(H) * 8 + i_ + BWD_PD];                                               \
+                    gq_[i_ + BWD_PD] = ring[((H) * 8 + i_ + BWD_PD) * F];                                         \
+                }                                                                                                 \
+                const float4 m_ = mq_[i_];                                                                        \
+                const float4 g_ = gq_[i_];                                                                        \
                 const float sb_ = g_.x, vb0_ = g_.y, vb1_ = g_.z, vb2_ = g_.w;                                    \
                 const float X_ = fmaf(vb0_, m_.x, fmaf(vb1_, m_.y, vb2_ * m_.z));                                 \
                 const float wVSf_ = __uint_as_float(wVS_[i_]);                                                    \
@@ -614,7 +629,8 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
             }                                                                                                     \
             /* re-arm the 8 slots with the rows of edges k0 + 16 .. k0 + 23 (one commit group, also when empty) */ \
             _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                                    \
-                const int jn_ = __shfl_sync(0xffffffffu, isel_, l0_ + i_);                                        \
+                int jn_ = __shfl_sync(0xffffffffu, isel_, l0_ + i_);                                              \
+                jn_ = jn_ < 0 ? ~jn_ : jn_;                                                                       \
                 if (pf_) cp_async16(ring + ((H) * 8 + i_) * F, Gb + (size_t)jn_ * F);                             \
             }                                                                                                     \
             cp_async_commit();                                                                                    \
@@ -912,10 +928,18 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
                         mbar_wait(&p_empty[hc & 1], ((hc >> 1) & 1) ^ 1);
                         tmem_wait_ld();
                         uint8_t* pdst = sP + (hc & 1) * P_BYTES;
+                        // all shared-memory reads of the batch before its first store (see BWD_PD in k_msg_bwd)
+                        float4 mq[8];
+                        float2 pq[8];
 #pragma unroll
                         for (int i = 0; i < 8; i++) {
-                            const float4 m = meta[h * 8 + i];
-                            const float2 ph = sTab[spec[h * 8 + i] * F + f];
+                            mq[i] = meta[h * 8 + i];
+                            pq[i] = sTab[spec[h * 8 + i] * F + f];
+                        }
+#pragma unroll
+                        for (int i = 0; i < 8; i++) {
+                            const float4 m = mq[i];
+                            const float2 ph = pq[i];
                             const float X = fmaf(own.y, m.x, fmaf(own.z, m.y, own.w * m.z));
                             float db = ph.x * (own.x * __uint_as_float(dS[i]));
                             db = fmaf(ph.y, X * __uint_as_float(dVS[i]), db);
@@ -997,22 +1021,41 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
         }
     } else if (lwarp == 6) {
         // ===================== reducer: channel sums, scatter into the sender-row slot =====================
+        // The scatter target rev[E] and the running sum G[rev[E]] (a random 16-byte row, usually from DRAM) are two
+        // dependent global loads per batch: issued where they are needed, their latencies (~1.5 us per batch) were the
+        // bound of the whole kernel (measured: consumers 46 % of their time waiting for the partials buffer).  The
+        // reducer therefore runs them ahead: rev in coalesced 32-edge blocks (one register per lane, two blocks in
+        // flight, the target of a batch taken by shuffle), G of batch b + 1 while batch b is reduced.  The loop is
+        // unrolled over two blocks so that every register choice is static (a select between a landed and a pending
+        // register would wait for both).
         const int re = lane >> 2, rsub = lane & 3;
         float4* __restrict__ Gout = p.G;
-        const bool first = p.first != 0;
+        const bool want_old = p.first == 0 && rsub == 0;
+        const int* __restrict__ rev = p.rev;
         uint32_t hc = 0;
         for (long long u = u0; u < n_units; u += ustride) {
             const long long a0 = u * apu;
             const long long a1 = min(N, a0 + (long long)apu);
             const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
-            const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
-            for (int t = 0; t < ntiles; t++) {
-                for (int h = 0; h < 2; h++) {
-                    const int E8 = e_begin + t * NEB + h * 8;
-                    if (E8 >= e_end) continue;
-                    const int tgt = __ldg(p.rev + E8 + re);
-                    float4 gold = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (rsub == 0 && !first) gold = Gout[tgt];
+            const int nb = (e_end - e_begin + 7) >> 3;                 // 8-edge batches of the unit (rows are padded to 8)
+            auto ld_blk = [&](int blk) -> int {
+                const int E = e_begin + 32 * blk + lane;
+                return E < e_end ? __ldg(rev + E) : 0;
+            };
+            int rA = ld_blk(0), rB = ld_blk(1);
+            int tcur = __shfl_sync(0xffffffffu, rA, re);
+            float4 gc = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (want_old && nb > 0) gc = Gout[tcur];
+            for (int b0 = 0; b0 < nb; b0 += 8) {
+#pragma unroll
+                for (int i = 0; i < 8; i++) {
+                    const int b = b0 + i;
+                    if (b >= nb) break;
+                    if (i == 0 && b0 > 0) rB = ld_blk((b0 >> 2) + 1);
+                    if (i == 4) rA = ld_blk((b0 >> 2) + 2);
+                    const int tnext = __shfl_sync(0xffffffffu, (((i + 1) >> 2) & 1) ? rB : rA, ((i + 1) & 3) * 8 + re);
+                    float4 gn = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (want_old && b + 1 < nb) gn = Gout[tnext];
                     bar_sync(NB_PF + (hc & 1), 160);
                     const uint8_t* src = sP + (hc & 1) * P_BYTES + re * P_ROW + rsub * 16;
                     float3 acc = make_float3(0.f, 0.f, 0.f);
@@ -1034,7 +1077,9 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
                         acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
                         acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o);
                     }
-                    if (rsub == 0) Gout[tgt] = make_float4(gold.x + acc.x, gold.y + acc.y, gold.z + acc.z, 0.f);
+                    if (rsub == 0) Gout[tcur] = make_float4(gc.x + acc.x, gc.y + acc.y, gc.z + acc.z, 0.f);
+                    tcur = tnext;
+                    gc = gn;
                 }
             }
         }
