@@ -567,14 +567,15 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
     float4* ej = P<float4>(m->b_ej);
     const int* row_ptr = P<int>(m->b_row_ptr);
     nbr_fill(L, N, g, P<double>(m->b_pos_s), P<signed char>(m->b_wrap_s), P<int>(m->b_cell_s), cell_start, row_ptr,
-             m->cap_edges, rcf, ej, P<unsigned char>(m->b_img), dm->flags);
+             m->cap_edges, rcf, ej, P<unsigned char>(m->b_img), P<int>(m->b_G), dm->flags);
     // the reverse-edge index is needed by the layer-0 adjoint and the force assembly only: build it on a side stream,
-    // overlapped with the forward pass (its warps fit beside the GEMM / element-wise kernels)
+    // overlapped with the forward pass (its warps fit beside the GEMM / element-wise kernels).  Its compact search
+    // keys live in the G buffer, which nothing touches before the adjoint pass (joined below before it starts)
     {
         Launch Ls{m->side_stream, &launches};
         CU(m, cudaEventRecord(m->ev_fork, st));
         CU(m, cudaStreamWaitEvent(m->side_stream, m->ev_fork, 0));
-        nbr_reverse(Ls, N, row_ptr, ej, P<unsigned char>(m->b_img), P<int>(m->b_rev));
+        nbr_reverse(Ls, N, row_ptr, ej, P<unsigned char>(m->b_img), P<int>(m->b_G), P<int>(m->b_rev));
         CU(m, cudaEventRecord(m->ev_join, m->side_stream));
     }
 

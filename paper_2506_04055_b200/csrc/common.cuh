@@ -49,9 +49,9 @@ void nbr_count(const Launch& L, long long N, Grid g, const double* pos_s, const 
                const int* cell_s, const int* cell_start, int* row_cnt, unsigned long long* real_total);
 void nbr_fill(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s,
               const int* cell_s, const int* cell_start, const int* row_ptr, long long cap_edges, float rc, float4* ej,
-              unsigned char* img, int* flags);
+              unsigned char* img, int* key, int* flags);
 void nbr_reverse(const Launch& L, long long N, const int* row_ptr, const float4* ej, const unsigned char* img,
-                 int* rev);
+                 const int* key, int* rev);
 void nbr_export(const Launch& L, long long N, const int* row_ptr, const float4* ej, const unsigned char* img,
                 const int* perm, const signed char* wrap_s, int* out_i, int* out_j, signed char* out_img);
 

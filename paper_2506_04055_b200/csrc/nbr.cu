@@ -299,7 +299,8 @@ __global__ void __launch_bounds__(128) k_fill(long long N, Grid g, const double*
                                               const signed char* __restrict__ wrap_s, const int* __restrict__ cell_s,
                                               const int* __restrict__ cell_start, const int* __restrict__ row_ptr,
                                               long long cap_edges, float rc, float4* __restrict__ ej,
-                                              unsigned char* __restrict__ img, int* __restrict__ flags) {
+                                              unsigned char* __restrict__ img, int* __restrict__ key,
+                                              int* __restrict__ flags) {
     long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (a >= N) return;
     long long e = row_ptr[a];
@@ -307,20 +308,23 @@ __global__ void __launch_bounds__(128) k_fill(long long N, Grid g, const double*
     visit_neighbors(a, g, pos_s, wrap_s, cell_s, cell_start, [&](int b, int code, double ex, double ey, double ez) {
         ej[e] = make_float4((float)ex, (float)ey, (float)ez, __int_as_float(b));
         img[e] = (unsigned char)code;
+        if (key) key[e] = (b << 5) | code;        // compact search key of the reverse-edge pass (N < 2^26)
         e++;
     });
     // dummy slots: sender index ~a (negative), |r| = rc; every kernel gives them exactly zero weight
     for (const long long e1 = row_ptr[a + 1]; e < e1; e++) {
         ej[e] = make_float4(rc, 0.0f, 0.0f, __int_as_float(~(int)a));
         img[e] = 255;
+        if (key) key[e] = -1;
     }
 }
 void nbr_fill(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s,
               const int* cell_s, const int* cell_start, const int* row_ptr, long long cap_edges, float rc, float4* ej,
-              unsigned char* img, int* flags) {
+              unsigned char* img, int* key, int* flags) {
     if (N == 0) return;
+    if (N >= (1ll << 26)) key = nullptr;
     k_fill<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, pos_s, wrap_s, cell_s, cell_start, row_ptr, cap_edges,
-                                                              rc, ej, img, flags);
+                                                              rc, ej, img, key, flags);
     KLAUNCH(L);
 }
 
@@ -341,9 +345,44 @@ __global__ void k_reverse(long long N, const int* __restrict__ row_ptr, const fl
         rev[e] = r;
     }
 }
+// The same search on the compact keys (sender << 5 | image code) written by k_fill: rows start at multiples of 8 slots,
+// so 8 candidates are two aligned 16-byte loads (the float4 records cost a 32-byte sector per two candidates: 4x the
+// L2 traffic, which is what bounds this pass).
+__global__ void k_reverse_keys(long long N, const int* __restrict__ row_ptr, const int* __restrict__ key,
+                               int* __restrict__ rev) {
+    long long a = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
+    int lane = threadIdx.x & 31;
+    if (a >= N) return;
+    for (int e = row_ptr[a] + lane; e < row_ptr[a + 1]; e += 32) {
+        const int k = key[e];
+        if (k < 0) { rev[e] = e; continue; }          // dummy slot: its own reverse (G[rev] - G = 0)
+        const int b = k >> 5;
+        const int want = ((int)a << 5) | (26 - (k & 31));
+        int r = -1;
+        const int x1 = row_ptr[b + 1];
+        for (int x = row_ptr[b]; x < x1 && r < 0; x += 8) {
+            const int4 q0 = *(const int4*)(key + x), q1 = *(const int4*)(key + x + 4);
+            if (q0.x == want) r = x;
+            else if (q0.y == want) r = x + 1;
+            else if (q0.z == want) r = x + 2;
+            else if (q0.w == want) r = x + 3;
+            else if (q1.x == want) r = x + 4;
+            else if (q1.y == want) r = x + 5;
+            else if (q1.z == want) r = x + 6;
+            else if (q1.w == want) r = x + 7;
+        }
+        rev[e] = r;
+    }
+}
+// key: the array nbr_fill wrote (nullptr, or N >= 2^26: search the float4 records)
 void nbr_reverse(const Launch& L, long long N, const int* row_ptr, const float4* ej, const unsigned char* img,
-                 int* rev) {
+                 const int* key, int* rev) {
     if (N == 0) return;
+    if (key && N < (1ll << 26)) {
+        k_reverse_keys<<<(unsigned)((N * 32 + 255) / 256), 256, 0, L.stream>>>(N, row_ptr, key, rev);
+        KLAUNCH(L);
+        return;
+    }
     k_reverse<<<(unsigned)((N * 32 + 255) / 256), 256, 0, L.stream>>>(N, row_ptr, ej, img, rev);
     KLAUNCH(L);
 }
