@@ -38,6 +38,7 @@ constexpr int BM = 128, BK = 32;                       // 32 fp32 = 128 B = one 
 constexpr int NUM_THREADS = 320;                       // 10 warps
 constexpr int CONV_WARP0 = 2, EPI_WARP0 = 6;
 constexpr int A_TILE_BYTES = BM * BK * 4;              // 16 KB
+constexpr int EPI_LD = 36;                             // staging row stride in floats: 16-byte rows of a quarter-warp fall into distinct banks
 
 // K-major, SWIZZLE_128B shared-memory matrix descriptor: rows of 128 B, 8-row groups 1024 B apart
 __device__ __forceinline__ uint64_t make_desc_sw128(uint32_t saddr) {
@@ -66,7 +67,8 @@ template <int BN, int STAGES>
 struct Smem {
     static constexpr int B_TILE = BN * BK * 4;
     static constexpr int STAGE = 2 * A_TILE_BYTES + 2 * B_TILE;
-    static constexpr int BYTES = STAGES * STAGE + 1024 /*align*/ + 256 /*barriers*/;
+    static constexpr int EPI = 4 * 32 * EPI_LD * 4;     // epilogue staging: one [32 rows][32 columns (+4)] fp32 tile per warp
+    static constexpr int BYTES = STAGES * STAGE + 1024 /*align*/ + 256 /*barriers*/ + EPI;
 };
 
 template <int BN, int STAGES>
@@ -120,6 +122,15 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
                     tma_load_2d(st, &mapA, &full[stage], kb * BK, m0);
                     tma_load_2d(st + 2 * A_TILE_BYTES, &mapWhi, &full[stage], kb * BK, n0);
                     tma_load_2d(st + 2 * A_TILE_BYTES + S::B_TILE, &mapWlo, &full[stage], kb * BK, n0);
+                    // the same block of this CTA's next unit goes to L2 now: only STAGES blocks (48 KB) can be in
+                    // flight to shared memory, too few to cover the DRAM latency at full bandwidth
+                    if (t + gridDim.x < total) {
+                        const int m1 = (int)((t + gridDim.x) / n_tiles) * BM;
+                        if (m1 != m0)
+                            asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global [%0, {%1, %2}];" ::"l"(&mapA), "r"(kb * BK),
+                                         "r"(m1)
+                                         : "memory");
+                    }
                     if (++stage == STAGES) { stage = 0; phase ^= 1; }
                 }
             }
@@ -186,7 +197,13 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
         }
     } else {
         // ===================== epilogue =====================
+        // tcgen05.ld hands every thread one ROW of the tile; global accesses in that layout touch 32 different lines per
+        // instruction (32 LSU wavefronts each, measured: the LSU data pipe was the busiest unit of this kernel).  Each
+        // warp therefore turns its 32 x 32 chunk through a private shared-memory tile and does all global traffic
+        // (residual / SiLU' argument loads, stores) with a quarter-warp per 128-byte row segment.
         const int q = warp & 3;                      // TMEM lane quadrant this warp may access
+        float* stg = (float*)(smem + STAGES * S::STAGE + 256) + q * 32 * EPI_LD;
+        const int sub = lane >> 3, c4 = (lane & 7) * 4;          // coalesced phase: row i * 4 + sub, columns c4 .. c4 + 3
         int buf = 0;
         uint32_t bphase = 0;
         for (long long t = blockIdx.x; t < total; t += gridDim.x) {
@@ -194,38 +211,43 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
             const int n0 = (int)(t % n_tiles) * BN;
             mbar_wait(&tfull[buf], bphase);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const long long row = m0 + q * 32 + lane;
-            float* crow = p.C + row * p.ldc + n0;
+            const long long row0 = m0 + q * 32 + sub;
 #pragma unroll 1
             for (int c0 = 0; c0 < BN; c0 += 32) {
                 uint32_t r[32];
                 float4 o[8];
-                // accumulate: issue all residual loads of this 32-column chunk BEFORE waiting on TMEM, so they are
-                // in flight together (a load -> add -> store chain per float4 serialises on DRAM latency)
-                if (p.accumulate && row < p.M) {
+                // issue all residual loads of this chunk BEFORE waiting on TMEM, so they are in flight together
+                if (p.accumulate) {
 #pragma unroll
-                    for (int c = 0; c < 8; c++) o[c] = __ldcs((const float4*)(crow + c0) + c);
-                } else if (p.dsilu_pre && row < p.M) {     // (never combined with accumulate)
+                    for (int i = 0; i < 8; i++)
+                        if (row0 + 4 * i < p.M) o[i] = __ldcs((const float4*)(p.C + (row0 + 4 * i) * p.ldc + n0 + c0 + c4));
+                } else if (p.dsilu_pre) {     // (never combined with accumulate)
 #pragma unroll
-                    for (int c = 0; c < 8; c++) o[c] = __ldcs((const float4*)(p.dsilu_pre + row * p.ld_pre + n0 + c0) + c);
+                    for (int i = 0; i < 8; i++)
+                        if (row0 + 4 * i < p.M)
+                            o[i] = __ldcs((const float4*)(p.dsilu_pre + (row0 + 4 * i) * p.ld_pre + n0 + c0 + c4));
                 }
+                float4 b4 = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (p.bias) b4 = *(const float4*)(p.bias + n0 + c0 + c4);
                 tmem_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + buf * BN + c0, r);
-                if (row < p.M) {
 #pragma unroll
-                    for (int c = 0; c < 32; c += 4) {
-                        float4 v = make_float4(__uint_as_float(r[c]), __uint_as_float(r[c + 1]), __uint_as_float(r[c + 2]),
-                                               __uint_as_float(r[c + 3]));
-                        if (p.bias) {
-                            const float4 b = *(const float4*)(p.bias + n0 + c0 + c);
-                            v.x += b.x; v.y += b.y; v.z += b.z; v.w += b.w;
-                        }
-                        if (p.accumulate) { v.x += o[c / 4].x; v.y += o[c / 4].y; v.z += o[c / 4].z; v.w += o[c / 4].w; }
+                for (int c = 0; c < 8; c++)
+                    *(float4*)(stg + lane * EPI_LD + 4 * c) = make_float4(__uint_as_float(r[4 * c]), __uint_as_float(r[4 * c + 1]),
+                                                                          __uint_as_float(r[4 * c + 2]), __uint_as_float(r[4 * c + 3]));
+                __syncwarp();
+#pragma unroll
+                for (int i = 0; i < 8; i++) {
+                    float4 v = *(const float4*)(stg + (4 * i + sub) * EPI_LD + c4);
+                    v.x += b4.x; v.y += b4.y; v.z += b4.z; v.w += b4.w;
+                    if (row0 + 4 * i < p.M) {
+                        if (p.accumulate) { v.x += o[i].x; v.y += o[i].y; v.z += o[i].z; v.w += o[i].w; }
                         else if (p.dsilu_pre) {
-                            v.x *= dsilu_x(o[c / 4].x); v.y *= dsilu_x(o[c / 4].y); v.z *= dsilu_x(o[c / 4].z); v.w *= dsilu_x(o[c / 4].w);
+                            v.x *= dsilu_x(o[i].x); v.y *= dsilu_x(o[i].y); v.z *= dsilu_x(o[i].z); v.w *= dsilu_x(o[i].w);
                         }
-                        *(float4*)(crow + c0 + c) = v;
+                        *(float4*)(p.C + (row0 + 4 * i) * p.ldc + n0 + c0 + c4) = v;
                     }
                 }
+                __syncwarp();
             }
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             __syncwarp();
@@ -260,7 +282,7 @@ constexpr int XTHREADS = NUM_THREADS + 32;                              // + war
 constexpr int XW_TILE = XBN * 128;                                      // 4 KB: 32 rows x 64 fp16 (one slice, one K half)
 constexpr int XW_STAGE = 3 * 2 * XW_TILE;                               // 24 KB: the three weight slices of one N tile, K = 128
 constexpr int XNMAX = 512;                                              // widest N (column scale and bias are staged in shared memory)
-constexpr int XSMEM = XRAW * A_TILE_BYTES + XWST * XW_STAGE + 4 * BM * 4 + 2 * XNMAX * 4 + 256 + 1024;
+constexpr int XSMEM = XRAW * A_TILE_BYTES + XWST * XW_STAGE + 4 * BM * 4 + 2 * XNMAX * 4 + 256 + 4 * 32 * EPI_LD * 4 + 1024;
 constexpr int XTM_A = 0;                                                // TMEM columns 0..191: A slices [3][64 columns = 128 fp16]
 constexpr int XTM_ACC = 192, XACC = 4 * XBN;                            // TMEM columns 192..447: 2 accumulator sets (S2..S5 x 32)
 
@@ -505,27 +527,31 @@ __global__ void __launch_bounds__(XTHREADS, 1)
         }
     } else if (warp < 10) {
         // ===================== epilogue =====================
+        // combine and scale in the TMEM layout (thread = row), then turn the 32 x 32 tile through a private shared-memory
+        // tile so that the residual loads and the stores are coalesced (see k_gemm_3xtf32)
         const int q = warp & 3;                      // TMEM lane quadrant this warp may access
+        float* stg = (float*)((uint8_t*)bars + 256) + q * 32 * EPI_LD;
+        const int sub = lane >> 3, c4 = (lane & 7) * 4;
         int buf = 0;
         uint32_t bphase = 0;
         uint32_t ucount = 0;
         for (long long u = blockIdx.x; u < units; u += gridDim.x, ucount++) {
-            const long long row = u * BM + q * 32 + lane;
+            const long long row0 = u * BM + q * 32 + sub;
             for (int nt = 0; nt < n_tiles; nt++) {
                 const int n0 = nt * XBN;
+                float4 o[8];
+                if (p.accumulate) {
+#pragma unroll
+                    for (int i = 0; i < 8; i++)
+                        if (row0 + 4 * i < p.M) o[i] = __ldcs((const float4*)(p.C + (row0 + 4 * i) * p.ldc + n0 + c4));
+                }
                 mbar_wait(&tfull[buf], bphase);
                 tc_fence_after();
                 const float rs = rowscale[(ucount & 3) * BM + q * 32 + lane];
-                float* crow = p.C + row * p.ldc + n0;
                 const uint32_t tb = tmem_base + XTM_ACC + ((uint32_t)(q * 32) << 16) + buf * XACC;
 #pragma unroll
                 for (int c0 = 0; c0 < XBN; c0 += 16) {
                     uint32_t r2[16], r3[16], r4[16], r5[16];
-                    float4 o[4];
-                    if (p.accumulate && row < p.M) {
-#pragma unroll
-                        for (int c = 0; c < 4; c++) o[c] = __ldcs((const float4*)(crow + c0) + c);
-                    }
                     tmem_ld16_nowait(tb + c0, r2);
                     tmem_ld16_nowait(tb + XBN + c0, r3);
                     tmem_ld16_nowait(tb + 2 * XBN + c0, r4);
@@ -536,26 +562,31 @@ __global__ void __launch_bounds__(XTHREADS, 1)
                         __syncwarp();
                         if (lane == 0) mbar_arrive(&tempty[buf]);
                     }
-                    if (row < p.M) {
 #pragma unroll
-                        for (int c = 0; c < 16; c += 4) {
-                            const float4 cs = *(const float4*)(s_cs + n0 + c0 + c);
-                            float v[4];
+                    for (int c = 0; c < 16; c += 4) {
+                        const float4 cs = *(const float4*)(s_cs + n0 + c0 + c);
+                        float v[4];
 #pragma unroll
-                            for (int j = 0; j < 4; j++) {
-                                const float lo = fmaf(__uint_as_float(r5[c + j]), 1.0f / 256.0f, __uint_as_float(r4[c + j]));
-                                v[j] = fmaf(lo, 1.0f / 65536.0f, fmaf(__uint_as_float(r3[c + j]), 1.0f / 256.0f, __uint_as_float(r2[c + j])));
-                            }
-                            float4 y = make_float4(v[0] * (rs * cs.x), v[1] * (rs * cs.y), v[2] * (rs * cs.z), v[3] * (rs * cs.w));
-                            {
-                                const float4 b = *(const float4*)(s_bias + n0 + c0 + c);
-                                y.x += b.x; y.y += b.y; y.z += b.z; y.w += b.w;
-                            }
-                            if (p.accumulate) { y.x += o[c / 4].x; y.y += o[c / 4].y; y.z += o[c / 4].z; y.w += o[c / 4].w; }
-                            *(float4*)(crow + c0 + c) = y;
+                        for (int j = 0; j < 4; j++) {
+                            const float lo = fmaf(__uint_as_float(r5[c + j]), 1.0f / 256.0f, __uint_as_float(r4[c + j]));
+                            v[j] = fmaf(lo, 1.0f / 65536.0f, fmaf(__uint_as_float(r3[c + j]), 1.0f / 256.0f, __uint_as_float(r2[c + j])));
                         }
+                        float4 y = make_float4(v[0] * (rs * cs.x), v[1] * (rs * cs.y), v[2] * (rs * cs.z), v[3] * (rs * cs.w));
+                        const float4 b = *(const float4*)(s_bias + n0 + c0 + c);
+                        y.x += b.x; y.y += b.y; y.z += b.z; y.w += b.w;
+                        *(float4*)(stg + lane * EPI_LD + c0 + c) = y;
                     }
                 }
+                __syncwarp();
+#pragma unroll
+                for (int i = 0; i < 8; i++) {
+                    float4 y = *(const float4*)(stg + (4 * i + sub) * EPI_LD + c4);
+                    if (row0 + 4 * i < p.M) {
+                        if (p.accumulate) { y.x += o[i].x; y.y += o[i].y; y.z += o[i].z; y.w += o[i].w; }
+                        *(float4*)(p.C + (row0 + 4 * i) * p.ldc + n0 + c4) = y;
+                    }
+                }
+                __syncwarp();
                 if (++buf == 2) { buf = 0; bphase ^= 1; }
             }
         }
