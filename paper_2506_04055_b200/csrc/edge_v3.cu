@@ -526,18 +526,20 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
             const int n_e = e_end - e_begin;
             const int ntiles = (n_e + NEB - 1) / NEB;
             // sender indices of the unit's edges, 32 per register (lane l <-> edge 32 blk + l); padding slots -> own row
-            // (returned raw: padding slots carry ~own row; the sign is folded after the shuffle, so that nothing
-            // waits for the load where it is issued)
+            // (returned raw: padding slots carry ~own row; the sign is folded one batch after the load was issued, so
+            // that nothing waits for the load where it is issued)
             auto load_idx = [&](int blk) -> int {
                 const int E = e_begin + 32 * blk + lane;
                 return E < e_end ? __float_as_int(__ldg(ejp + E).w) : 0;
             };
             int idx0 = load_idx(0), idx1 = load_idx(1);
+            idx0 ^= idx0 >> 31;
+            idx1 ^= idx1 >> 31;
+            int idxn = 0;
             if (ntiles > 0) {
 #pragma unroll
                 for (int i = 0; i < GW; i++) {
-                    int j = __shfl_sync(0xffffffffu, idx0, i);
-                    j = j < 0 ? ~j : j;
+                    const int j = __shfl_sync(0xffffffffu, idx0, i);
                     if (i < n_e) cp_async16(ring + i * F, Gb + (size_t)j * F);
                     if ((i & 7) == 7) cp_async_commit();            // one commit group per 8-edge batch
                 }
@@ -584,7 +586,10 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
             while (E8_ >= row_end) next_row();                                                                    \
             /* prefetch targets: edges k0 + 16 .. k0 + 23 of the unit, all in index block tb_ */                  \
             const int tb_ = (k0_ + GW) >> 5, l0_ = (k0_ + GW) & 31;                                               \
-            if (l0_ == 0) { if (tb_ & 1) idx0 = load_idx(tb_ + 1); else idx1 = load_idx(tb_ + 1); }               \
+            /* the next index block lands in its own register and is folded into idx0 / idx1 one batch later: */ \
+            /* the select below then never reads a register with a load in flight                              */ \
+            if (l0_ == 0) idxn = load_idx(tb_ + 1);                                                               \
+            if (l0_ == 8) { if (tb_ & 1) idx0 = idxn ^ (idxn >> 31); else idx1 = idxn ^ (idxn >> 31); }           \
             const int isel_ = (tb_ & 1) ? idx1 : idx0;                                                            \
             const bool pf_ = k0_ + GW < n_e;                                                                      \
             uint32_t wS_[8], wVS_[8], wVV_[8], dS_[8], dVS_[8], dVV_[8];                                          \
@@ -638,8 +643,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
             }                                                                                                     \
             /* re-arm the 8 slots with the rows of edges k0 + 16 .. k0 + 23 (one commit group, also when empty) */ \
             _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                                    \
-                int jn_ = __shfl_sync(0xffffffffu, isel_, l0_ + i_);                                              \
-                jn_ = jn_ < 0 ? ~jn_ : jn_;                                                                       \
+                const int jn_ = __shfl_sync(0xffffffffu, isel_, l0_ + i_);                                        \
                 if (pf_) cp_async16(ring + ((H) * 8 + i_) * F, Gb + (size_t)jn_ * F);                             \
             }                                                                                                     \
             cp_async_commit();                                                                                    \
