@@ -391,6 +391,16 @@ constexpr int G_OFF_B = 0, G_OFF_P = 2 * BB_BYTES, G_OFF_RING = G_OFF_P + 2 * P_
               G_OFF_BAR = G_OFF_META + 4 * NEB * 16, GROUP_BYTES = G_OFF_BAR + 128;
 constexpr int bwd_smem_bytes(int nch) { return (nch - 2) * A_CHUNK_BYTES + 2 * GROUP_BYTES + 128; }
 
+// two fp32 additions in one instruction (register pairs as they come out of a 16-byte shared-memory load): the reducer
+// warps sit on the critical path of their pipeline and are bound by instruction issue
+__device__ __forceinline__ unsigned long long fadd2(unsigned long long a, unsigned long long b) {
+    unsigned long long d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ float hsum2(unsigned long long a) {
+    return __uint_as_float((uint32_t)a) + __uint_as_float((uint32_t)(a >> 32));
+}
 // tcgen05.st: 16 consecutive 32-bit columns of this thread's TMEM lane
 __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {
     asm volatile(
@@ -759,16 +769,17 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                     bar_sync(NB_PF + (hc & 1), 160);
                     // this lane adds a quarter (chunks rsub + 4 k) of each of the three 128-float planes of row re
                     const uint8_t* src = sP + (hc & 1) * P_BYTES + re * P_ROW + rsub * 16;
-                    float3 acc = make_float3(0.f, 0.f, 0.f);
+                    unsigned long long ax = 0ull, ay = 0ull, az = 0ull;      // packed (+0.f, +0.f)
 #pragma unroll
                     for (int k = 0; k < 8; k++) {
-                        const float4 x = *(const float4*)(src + k * 64);
-                        const float4 y = *(const float4*)(src + F * 4 + k * 64);
-                        const float4 z = *(const float4*)(src + 2 * F * 4 + k * 64);
-                        acc.x += (x.x + x.y) + (x.z + x.w);
-                        acc.y += (y.x + y.y) + (y.z + y.w);
-                        acc.z += (z.x + z.y) + (z.z + z.w);
+                        const ulonglong2 x = *(const ulonglong2*)(src + k * 64);
+                        const ulonglong2 y = *(const ulonglong2*)(src + F * 4 + k * 64);
+                        const ulonglong2 z = *(const ulonglong2*)(src + 2 * F * 4 + k * 64);
+                        ax = fadd2(ax, fadd2(x.x, x.y));
+                        ay = fadd2(ay, fadd2(y.x, y.y));
+                        az = fadd2(az, fadd2(z.x, z.y));
                     }
+                    float3 acc = make_float3(hsum2(ax), hsum2(ay), hsum2(az));
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&p_empty[hc & 1]);
                     hc++;
@@ -1077,16 +1088,17 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
                     if (want_old && b + 1 < nb) gn = Gout[tnext];
                     bar_sync(NB_PF + (hc & 1), 160);
                     const uint8_t* src = sP + (hc & 1) * P_BYTES + re * P_ROW + rsub * 16;
-                    float3 acc = make_float3(0.f, 0.f, 0.f);
+                    unsigned long long ax = 0ull, ay = 0ull, az = 0ull;      // packed (+0.f, +0.f)
 #pragma unroll
                     for (int k = 0; k < 8; k++) {
-                        const float4 x = *(const float4*)(src + k * 64);
-                        const float4 y = *(const float4*)(src + F * 4 + k * 64);
-                        const float4 z = *(const float4*)(src + 2 * F * 4 + k * 64);
-                        acc.x += (x.x + x.y) + (x.z + x.w);
-                        acc.y += (y.x + y.y) + (y.z + y.w);
-                        acc.z += (z.x + z.y) + (z.z + z.w);
+                        const ulonglong2 x = *(const ulonglong2*)(src + k * 64);
+                        const ulonglong2 y = *(const ulonglong2*)(src + F * 4 + k * 64);
+                        const ulonglong2 z = *(const ulonglong2*)(src + 2 * F * 4 + k * 64);
+                        ax = fadd2(ax, fadd2(x.x, x.y));
+                        ay = fadd2(ay, fadd2(y.x, y.y));
+                        az = fadd2(az, fadd2(z.x, z.y));
                     }
+                    float3 acc = make_float3(hsum2(ax), hsum2(ay), hsum2(az));
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&p_empty[hc & 1]);
                     hc++;
