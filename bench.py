@@ -28,7 +28,7 @@ import gen  # noqa: E402
 METRIC = "atom-steps/s (E+F+virial) PaiNN F=128 at 1M atoms"
 UNIT = "atom-steps/s"
 # bounded CPU-oracle sample: reduced replica of the same recipe (O(N^2) neighbour search keeps it small)
-CPU_SAMPLE = {5: dict(n_slots=3000, L=44.77), 4: dict(ncell=9), 2: dict(n_mol=2400, L=41.55), 1: {},
+CPU_SAMPLE = {5: dict(n_slots=6000, L=56.41), 4: dict(ncell=9), 2: dict(n_mol=2400, L=41.55), 1: {},
               3: dict(n_mol=1500, L=35.56)}
 
 
