@@ -59,7 +59,7 @@ struct Params {
     int ld_pre;
 };
 __device__ __forceinline__ float dsilu_x(float x) {
-    const float sg = 1.0f / (1.0f + __expf(-x));
+    const float sg = __fdividef(1.0f, 1.0f + __expf(-x));     // adjoint only: 2 ulp (forces carry a relative tolerance)
     return sg * (1.0f + x * (1.0f - sg));
 }
 
