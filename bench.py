@@ -156,6 +156,21 @@ def _stage_work(stats, model, n_atoms):
     return w
 
 
+def _max_over_ranks(x, dist, device):
+    """Time of the job = the slowest rank's (contract: MAX over ranks); dist is torch.distributed or None (one rank)."""
+    import torch
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def _job_value(world, n_local, seconds_per_step):
+    """Whole-job throughput of `world` independent replicas ("replicas only"): every rank evaluates
+    its own n_local atoms per step, nothing is exchanged on the data path."""
+    return world * n_local / seconds_per_step
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -235,12 +250,9 @@ def main():
     clocks = sampler.stop() if sampler else None
     stats = m.stats()
     launches = stats["n_launches"] * args.steps
-    t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total = float(t.item())
+    ms_total = _max_over_ranks(ms_total, dist, dev)
     ms_step = ms_total / args.steps
-    value = world * n_local / (ms_step * 1e-3)
+    value = _job_value(world, n_local, ms_step * 1e-3)
 
     # ---- per-stage timing (separate pass, not part of `value`) -> roofline of the dominant kernel ----
     m.set_option("stage_timing", 1)
@@ -308,11 +320,8 @@ def main():
         m.compute_host(hpos.numpy(), htypes.numpy(), c["box"], n_local, c["n_ghost"], hown, out=hout)
     torch.cuda.synchronize(dev)
     te = (time.perf_counter() - t0) / e2e_steps
-    tt = torch.tensor([te], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    te = float(tt.item())
-    e2e = dict(value=world * n_local / te, unit=UNIT, ms_per_step=te * 1e3,
+    te = _max_over_ranks(te, dist, dev)
+    e2e = dict(value=_job_value(world, n_local, te), unit=UNIT, ms_per_step=te * 1e3,
                h2d_bytes_per_step=N * 28 + (0 if hown is None else 4 * c["n_ghost"]), d2h_bytes_per_step=N * 24 + 56)
 
     if rank == 0:

@@ -389,3 +389,31 @@ def test_unwrapped_positions_need_wider_image_range():
     a = set(zip(i0.tolist(), j0.tolist(), map(tuple, S0.tolist())))
     b = set(zip(i1.tolist(), j1.tolist(), map(tuple, (S1 + (w[j1] - w[i1])).astype(int).tolist())))
     assert a == b
+
+
+def test_oracle_reproduces_golden_config1():
+    """Regression guard for the oracle itself (tests/golden/oracle_config1.txt, written by tests/golden/make_golden.py from
+    oracle/ only): a change of its arithmetic has to be deliberate -- re-run the script and justify it in the commit."""
+    import importlib.util
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(here, "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mg)
+    c, r = mg.evaluate()
+    want = {}
+    for line in open(os.path.join(here, "oracle_config1.txt")):
+        if line.startswith("#"):
+            continue
+        k, *v = line.split()
+        if k == "force":
+            want.setdefault("force", {})[int(v[0])] = np.array([float(x) for x in v[1:]])
+        else:
+            want[k] = np.array([float(x) for x in v])
+    assert len(c["pos"]) == int(want["n_atoms"][0]) and int(r["n_edges"]) == int(want["n_edges"][0])
+    # fp64 results depend on the BLAS summation order (thread count): 1e-10 relative, far below any tolerance of the path
+    assert abs(float(r["energy"]) - want["energy"][0]) <= 1e-10 * abs(want["energy"][0])
+    assert np.abs(np.asarray(r["virial"]).ravel() - want["virial"]).max() <= 1e-9 * np.abs(want["virial"]).max()
+    frms = np.sqrt((r["forces"] ** 2).mean())
+    for a, f in want["force"].items():
+        assert np.abs(r["forces"][a] - f).max() <= 1e-9 * frms
