@@ -139,6 +139,8 @@ int mlp_get_stage_ms(mlp_model* m, int max_stages, const char** names, float* ms
  * test hook for the overflow / regrow path of PAPER.md:84-86), and experiment switches that select between
  * implementations of the same arithmetic (defaults are the shipped path; DESIGN.md sections 5-7b):
  *   "edge_path"       0 gen-3 tensor-core edge kernels (F = 128, K <= 23), 1 plain fp32 kernels, 2 / 3 earlier generations
+ *   "l0_collapse"     1 layer-0 adjoint with the channel contraction hoisted into two GEMMs (n_species (K+1) <= 128),
+ *                     0 per-edge channel sums (k_msg_bwd0)
  *   "gemm_fwd_exact"  1 forward GEMMs on tcgen05 with exact integer slices, 0 fp32 FFMA kernel
  *   "gemm_bwd_exact"  0 adjoint GEMMs 3xTF32, 1 exact integer slices
  *   "gemm_fwd_tc"     1 forward GEMMs 3xTF32 (biased energy, B3)

@@ -44,6 +44,9 @@ struct mlp_model {
     void* filt_img2[PAINN_MAX_T] = {};  // unscaled hi | lo image (edge_tc2.cu)   // tcgen05 A-operand image of (Wf | bf), fp16 hi/lo split (edge_tc.cu)
     int edge_path = 0;                  // 0: tensor-core edge kernels when F == 128, 1: plain fp32 kernels
     float* tab0 = nullptr;              // [n_species][F] float2 (phi^s, phi^vs) of layer 0: s^0 = Emb[z] depends on the species only
+    float *Wl0s = nullptr, *Wl0v = nullptr;   // [np0][F]: layer-0 adjoint with the channels contracted first (edge_l0.cu)
+    int np0 = 0;                        // columns of those GEMMs: n_species (K + 1) rounded up to 128
+    int l0_collapse = 1;                // option: use them (0: k_msg_bwd0)
     // capacities
     long long cap_atoms = 0, cap_edges = 0, cap_cells = 0;
     std::vector<Buf*> all;
@@ -282,6 +285,7 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
         if (rcode == MLP_OK) painn::gemm_register_exact(*dst, t.data(), cols, rows);
     };
     up((size_t)ns * F, &m->Emb);
+    std::vector<float> Wf0_h, bf0_h;          // layer-0 filter weights (for the collapsed layer-0 adjoint)
     for (int t = 0; t < T; t++) {
         LayerW& l = m->lw[t];
         std::vector<float> Wm1, Wm2, U, V, Wu1, Wu2;
@@ -290,6 +294,7 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
         up((size_t)3 * F * F, (float**)&l.Wm2, &Wm2); up(3 * F, (float**)&l.bm2);
         {
             std::vector<float> Wf_h = to_f32(p, (size_t)3 * F * K), bf_h = to_f32(p + (size_t)3 * F * K, (size_t)3 * F);
+            if (t == 0) { Wf0_h = Wf_h; bf0_h = bf_h; }
             if (F == 128 && K <= 23 && rcode == MLP_OK) {
                 std::vector<unsigned short> img;
                 edge_build_filter_image(Wf_h.data(), bf_h.data(), K, img);
@@ -361,6 +366,23 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
                     tab[((size_t)z * F + f) * 2 + 1] = ph[(size_t)z * 3 * F + F + f];
                 }
             if (rcode == MLP_OK) rcode = upload(m, tab, &m->tab0);
+            // layer-0 adjoint, channels contracted first (edge_l0.cu): rows n = z (K + 1) + k,
+            //   Wl0s[n][c] = Wf^s[c][k] phi^s_z[c],  Wl0v[n][c] = Wf^vs[c][k] phi^vs_z[c]   (k = 0: the bias bf)
+            const int KP1 = K + 1, np0 = ((ns * KP1 + 127) / 128) * 128;
+            if (rcode == MLP_OK && K <= 23 && !Wf0_h.empty()) {
+                std::vector<float> ws((size_t)np0 * F, 0.f), wv((size_t)np0 * F, 0.f);
+                for (int z = 0; z < ns; z++)
+                    for (int k = 0; k < KP1; k++)
+                        for (int c = 0; c < F; c++) {
+                            const float fs = k == 0 ? bf0_h[c] : Wf0_h[(size_t)c * K + (k - 1)];
+                            const float fv = k == 0 ? bf0_h[F + c] : Wf0_h[(size_t)(F + c) * K + (k - 1)];
+                            ws[((size_t)z * KP1 + k) * F + c] = fs * tab[((size_t)z * F + c) * 2];
+                            wv[((size_t)z * KP1 + k) * F + c] = fv * tab[((size_t)z * F + c) * 2 + 1];
+                        }
+                rcode = upload_gemm_weight(m, ws, &m->Wl0s);
+                if (rcode == MLP_OK) rcode = upload_gemm_weight(m, wv, &m->Wl0v);
+                if (rcode == MLP_OK) m->np0 = np0;
+            }
         }
         free_buf(bh, m);
         free_buf(bp, m);
@@ -415,6 +437,7 @@ __attribute__((visibility("default"))) int mlp_set_option(mlp_model* m, const ch
     if (!strcmp(name, "stage_timing")) { m->timing = value != 0; return MLP_OK; }
     if (!strcmp(name, "gemm_emulate")) { painn::g_gemm_emulate = (int)value; return MLP_OK; }
     if (!strcmp(name, "edge_path")) { m->edge_path = (int)value; return MLP_OK; }
+    if (!strcmp(name, "l0_collapse")) { m->l0_collapse = (int)value; return MLP_OK; }
     if (!strcmp(name, "gemm_fwd_tc")) { m->fwd_tc = value != 0; return MLP_OK; }
     if (!strcmp(name, "gemm_bwd_exact")) { m->bwd_exact = value != 0; return MLP_OK; }
     if (!strcmp(name, "gemm_path")) { painn::g_gemm_path = (int)value; return MLP_OK; }
@@ -653,7 +676,19 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         gemm_nt(L, pqb, 2 * F, l.UVT, 2 * F, v1b, F, 3 * N, F, 2 * F, nullptr, true);
         mark(m, st, ST_BWD_EDGE);
         bool done = false;
-        if (m->edge_path != 1 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
+        if (t == 0 && m->edge_path == 0 && m->l0_collapse && m->Wl0s && m->np0 == 128 && g_filter_emulate == 0 &&
+            g_gather_emulate == 0) {
+            // layer 0: contract the channels per (receiver, sender species) with two GEMMs, then O(K) work per edge.
+            // B -> the gather-row buffer ([3N][128] floats of its [N][128] float4), C -> the (unused at layer 0) phib buffer
+            float *Bv = P<float>(m->b_Q4), *Cs = phib;
+            mark(m, st, ST_BWD_NODE);
+            gemm_nt(L, v1b, F, m->Wl0v, F, Bv, m->np0, 3 * N, m->np0, F, nullptr, false);
+            gemm_nt(L, s1b, F, m->Wl0s, F, Cs, m->np0, N, m->np0, F, nullptr, false);
+            mark(m, st, ST_BWD_EDGE);
+            done = message_bwd0_collapsed(L, N, K, rcf, row_ptr, ej, P<int>(m->b_types_s), m->n_species, P<int>(m->b_rev), Bv,
+                                          Cs, m->np0, P<float4>(m->b_G), t == T - 1);
+        }
+        if (!done && m->edge_path != 1 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
             make_gather_rows_bwd(L, N, s1b, v1b, P<float>(m->b_Q4));
             if (t == 0 && m->edge_path == 0 && m->tab0 && K <= 23)
                 done = message_bwd0_v3(L, N, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<int>(m->b_types_s), m->tab0, m->n_species,
