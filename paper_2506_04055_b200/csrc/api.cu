@@ -45,6 +45,7 @@ struct mlp_model {
     int edge_path = 0;                  // 0: tensor-core edge kernels when F == 128, 1: plain fp32 kernels
     float* tab0 = nullptr;              // [n_species][F] float2 (phi^s, phi^vs) of layer 0: s^0 = Emb[z] depends on the species only
     float *Wl0s = nullptr, *Wl0v = nullptr;   // [np0][F]: layer-0 adjoint with the channels contracted first (edge_l0.cu)
+    float *Wl0sT = nullptr, *Wl0vT = nullptr; // [F][np0]: their transposes, the forward counterpart
     int np0 = 0;                        // columns of those GEMMs: n_species (K + 1) rounded up to 128
     int l0_collapse = 1;                // option: use them (0: k_msg_bwd0)
     // capacities
@@ -381,6 +382,11 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
                         }
                 rcode = upload_gemm_weight(m, ws, &m->Wl0s);
                 if (rcode == MLP_OK) rcode = upload_gemm_weight(m, wv, &m->Wl0v);
+                const std::vector<float> wsT = transpose(ws, np0, F), wvT = transpose(wv, np0, F);
+                if (rcode == MLP_OK) rcode = upload_gemm_weight(m, wsT, &m->Wl0sT);
+                if (rcode == MLP_OK) painn::gemm_register_exact(m->Wl0sT, wsT.data(), F, np0);
+                if (rcode == MLP_OK) rcode = upload_gemm_weight(m, wvT, &m->Wl0vT);
+                if (rcode == MLP_OK) painn::gemm_register_exact(m->Wl0vT, wvT.data(), F, np0);
                 if (rcode == MLP_OK) m->np0 = np0;
             }
         }
@@ -632,7 +638,18 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         }
         mark(m, st, ST_FWD_EDGE);
         bool done = false;
-        if (m->edge_path != 1 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
+        if (l0_table && m->l0_collapse && m->Wl0sT && m->np0 == 128) {
+            // layer 0: per-(receiver, species) radial sums (O(K) per edge), then two GEMMs (edge_l0.cu).  The sums live in
+            // the gather-row buffers, which layer 0 does not use: Q1 [N][128], Q4 [3N][128] floats
+            float *As = P<float>(m->b_Q1), *Av = P<float>(m->b_Q4);
+            if (message_fwd0_collapsed_accum(L, N, K, rcf, row_ptr, ej, P<int>(m->b_types_s), m->n_species, S, F, sn, 2 * F, As, Av,
+                                             m->np0)) {
+                gemm_nt(L, As, m->np0, m->Wl0sT, m->np0, sn, 2 * F, N, F, m->np0, nullptr, true);
+                gemm_nt(L, Av, m->np0, m->Wl0vT, m->np0, v1, F, 3 * N, F, m->np0, nullptr, false);
+                done = true;
+            }
+        }
+        if (!done && m->edge_path != 1 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
             if (!l0_table) make_gather_rows(L, N, phi, V, P<float>(m->b_Q4), P<float>(m->b_Q1), t > 0);
             if (m->edge_path == 0 && (t > 0 || m->tab0))
                 done = message_fwd_v3(L, N, K, rcf, row_ptr, ej, S, V, P<float>(m->b_Q4), P<float>(m->b_Q1), m->filt_img[t],

@@ -127,7 +127,10 @@ bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
 void edge_build_filter_rows(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img);
 bool message_bwd0_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
                      const int* types_s, const float* tab, int n_tab, const int* rev, const void* A_img, float4* G, bool first);
-// ---- layer-0 adjoint with the channels contracted first (edge_l0.cu) ----
+// ---- layer 0 with the channels contracted outside the edge loop (edge_l0.cu) ----
+bool message_fwd0_collapsed_accum(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej,
+                                  const int* types_s, int n_species, const float* s_in, int F, float* sn, int ldsn, float* As,
+                                  float* Av, int NP);
 bool message_bwd0_collapsed(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej,
                             const int* types_s, int n_species, const int* rev, const float* Bv, const float* Cs, int NP,
                             float4* G, bool first);

@@ -93,7 +93,105 @@ __global__ void __launch_bounds__(WARPS * 32) k_l0_bwd(long long N, const int* _
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Forward counterpart.  With s^0_j = Emb[z_j] and v^0 = 0 the layer-0 message is
+//     ds_i[c] = sum_z phi^s_z[c]  sum_k Wf^s[c][k]  Rs_iz[k] ,      Rs_iz[k] = sum_{j in N(i), z_j = z} R_k(d_ij)
+//     dv_i[c] = sum_z phi^vs_z[c] sum_k Wf^vs[c][k] Q_iz[k]  ,      Q_iz[k]  = sum_{j in N(i), z_j = z} R_k(d_ij) u_ij
+// i.e. an O(K) accumulation per edge into per-(receiver, species) radial sums, then two GEMMs against [F x n_species
+// (K + 1)] matrices.  One warp per receiver, lane = radial slot k (each lane owns its column of the accumulators: no
+// atomics, fixed summation order, bit-reproducible); the edges of the row are prepared 32 at a time by lane = edge.
+// Writes As [N][NP] = Rs, Av [3N][NP] = Q (row 3 i + component) and copies s_i into the s' half of sn (ldsn floats per
+// row), to which the first GEMM accumulates.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int RLD = 25;            // row stride of the per-edge radial values (odd: conflict-free both ways)
+__global__ void __launch_bounds__(WARPS * 32) k_l0_fwd(long long N, const int* __restrict__ row_ptr, const float4* __restrict__ ej,
+                                                      const int* __restrict__ types, const float* __restrict__ s_in, int F,
+                                                      float* __restrict__ sn, int ldsn, float* __restrict__ As,
+                                                      float* __restrict__ Av, int NP, int n_used, int K, float inv_rc) {
+    extern __shared__ float4 sm[];       // [WARPS][n_used] accumulators | [WARPS][32] (u, species offset) | [WARPS][32][RLD] R_k
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float4* acc = sm + warp * n_used;
+    float4* rec = sm + WARPS * n_used + warp * 32;
+    float* Rb = (float*)(sm + WARPS * (n_used + 32)) + warp * 32 * RLD;
+    const int KP1 = K + 1;
+    for (long long i = (long long)blockIdx.x * WARPS + warp; i < N; i += (long long)gridDim.x * WARPS) {
+        const int e0 = __ldg(row_ptr + i), e1 = __ldg(row_ptr + i + 1);
+        for (int n = lane; n < n_used; n += 32) acc[n] = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int c = lane * 4; c < F; c += 128) *(float4*)(sn + i * ldsn + c) = __ldg((const float4*)(s_in + i * F + c));
+        for (int eb = e0; eb < e1; eb += 32) {
+            // lane = edge: geometry and all K + 1 radial values of up to 32 edges (one sincospi + rotation recurrence per
+            // 8 slots, as the producers of the tensor-core kernels do)
+            const int E = eb + lane;
+            float4 r = make_float4(1.f, 0.f, 0.f, __int_as_float(-1));
+            if (E < e1) r = __ldg(ej + E);
+            const int jb = __float_as_int(r.w);
+            const float d2 = r.x * r.x + r.y * r.y + r.z * r.z;
+            const float inv_d = rsqrtf(d2);
+            const float x = d2 * inv_d * inv_rc;
+            float s1, c1;
+            sincospif(x, &s1, &c1);
+            const float fc = jb >= 0 ? 0.5f * (1.0f + c1) : 0.0f;                  // padding slots: zero weight
+            const int z = jb >= 0 ? __ldg(types + jb) : 0;
+            __syncwarp();
+            rec[lane] = make_float4(r.x * inv_d, r.y * inv_d, r.z * inv_d, __int_as_float(z * KP1));
+            float* rb = Rb + lane * RLD;
+            rb[0] = fc;
+            const float amp = fc * inv_d;
+            float sn_ = s1, cn_ = c1;
+            for (int b = 1; b <= K; b++) {
+                if ((b & 7) == 0) sincospif((float)b * x, &sn_, &cn_);
+                rb[b] = amp * sn_;
+                const float tt = fmaf(sn_, c1, cn_ * s1);
+                cn_ = fmaf(cn_, c1, -sn_ * s1);
+                sn_ = tt;
+            }
+            __syncwarp();
+            // lane = radial slot: walk the edges in order (each lane owns its column of the accumulators)
+            const int ne = min(32, e1 - eb);
+            if (lane < KP1) {
+                for (int e = 0; e < ne; e++) {
+                    const float4 u = rec[e];
+                    const float R = Rb[e * RLD + lane];
+                    float4* q = acc + __float_as_int(u.w) + lane;
+                    float4 v = *q;
+                    v.x += R; v.y = fmaf(R, u.x, v.y); v.z = fmaf(R, u.y, v.z); v.w = fmaf(R, u.z, v.w);
+                    *q = v;
+                }
+            }
+        }
+        __syncwarp();
+        for (int n = lane; n < NP; n += 32) {
+            const float4 v = n < n_used ? acc[n] : make_float4(0.f, 0.f, 0.f, 0.f);
+            As[i * NP + n] = v.x;
+            Av[(3 * i) * NP + n] = v.y; Av[(3 * i + 1) * NP + n] = v.z; Av[(3 * i + 2) * NP + n] = v.w;
+        }
+        __syncwarp();
+    }
+}
+
 }  // namespace el0
+
+bool message_fwd0_collapsed_accum(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej,
+                                  const int* types_s, int n_species, const float* s_in, int F, float* sn, int ldsn, float* As,
+                                  float* Av, int NP) {
+    using namespace el0;
+    if (N == 0) return true;
+    const int n_used = n_species * (K + 1);
+    if (K + 1 > KMAX1 || n_used > NP || (F % 4) || (ldsn % 4)) return false;
+    const size_t smem = (size_t)WARPS * (n_used + 32) * sizeof(float4) + (size_t)WARPS * 32 * RLD * sizeof(float);
+    if (smem > 48 * 1024) return false;
+    static int n_sm = 0;
+    if (!n_sm) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    }
+    const long long want = (N + WARPS - 1) / WARPS;
+    const int grid = (int)(want < (long long)n_sm * 8 ? want : (long long)n_sm * 8);
+    k_l0_fwd<<<grid, WARPS * 32, smem, L.stream>>>(N, row_ptr, ej, types_s, s_in, F, sn, ldsn, As, Av, NP, n_used, K, 1.0f / rc);
+    KLAUNCH(L);
+    return true;
+}
 
 // Bv: [3N][NP] (row 3 i + component), Cs: [N][NP]; columns n = species (K + 1) + k, n < n_species (K + 1) <= NP
 bool message_bwd0_collapsed(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej,
