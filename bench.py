@@ -132,19 +132,29 @@ class _ClockSampler:
                     power_w_max=max(pw) if pw else None, samples=len(sm), reasons=sorted(reasons))
 
 
-def _stage_work(stats, model, n_atoms):
-    """Algorithmic work per step of each timed stage: (bound, units, unit-name)."""
+def _stage_work(stats, model, n_atoms, layer0_split=False):
+    """Algorithmic work per step of each timed stage: (bound, units, unit-name).
+    layer0_split: the collapsed layer-0 passes are timed as their own stage ("layer0"); fwd_edge / bwd_edge then hold
+    the T - 1 launches of layers >= 1 only."""
     F, K, T = model["F"], model["K"], model["T"]
     E, N = stats["n_edges"], n_atoms
     R = F // 2
     w = {}
+    if layer0_split:
+        NP = 128                                       # columns of the per-(receiver, species) radial sums
+        # forward: s in, radial sums written and read by the GEMMs, s' / v1 out, one edge record per edge;
+        # adjoint: s1b / v1b in, contracted vectors written and read, edge record + reverse index + G read-modify-write
+        l0 = N * (F * 4.0 + 2 * 4 * NP * 4.0 + 4 * F * 4.0) + E * 16.0 \
+            + N * (4 * F * 4.0 + 2 * 4 * NP * 4.0) + E * (16.0 + 4.0 + 32.0)
+        w["layer0"] = ("hbm", l0, "B")
     # edge stages: compulsory HBM bytes (every per-atom row and per-edge record moved once per launch; DESIGN.md
     # section 6).  The kernels are bound by the L2 -> SM row gather (reported separately as roofline.l2_gather), so
     # the HBM fraction states how far that keeps them from the DRAM roof.
-    fwd_atom = (2 * F * 4 + F * 4 + 4 * F * 4) + (T - 1) * (5 * F * 4 + F * 4 + 3 * F * 4 + 4 * F * 4)   # gather rows + residual + outputs
-    w["fwd_edge"] = ("hbm", N * float(fwd_atom) + T * E * 16.0, "B")
-    bwd_atom = (4 * F * 4 + 2 * F * 4) + (T - 1) * (4 * F * 4 + 9 * F * 4 + 6 * F * 4)              # gather rows + own rows + sender adjoint
-    w["bwd_edge"] = ("hbm", N * float(bwd_atom) + E * (16.0 * T + 16.0 + 32.0 * (T - 1)), "B")
+    f0 = 0 if layer0_split else 1                      # layer-0 terms of the per-edge kernels (species-table kernels)
+    fwd_atom = f0 * (2 * F * 4 + F * 4 + 4 * F * 4) + (T - 1) * (5 * F * 4 + F * 4 + 3 * F * 4 + 4 * F * 4)   # gather rows + residual + outputs
+    w["fwd_edge"] = ("hbm", N * float(fwd_atom) + (T - 1 + f0) * E * 16.0, "B")
+    bwd_atom = f0 * (4 * F * 4 + 2 * F * 4) + (T - 1) * (4 * F * 4 + 9 * F * 4 + 6 * F * 4)              # gather rows + own rows + sender adjoint
+    w["bwd_edge"] = ("hbm", N * float(bwd_atom) + E * (16.0 * (T - 1 + f0) + f0 * 16.0 + 32.0 * (T - 1)), "B")
     # node GEMMs (flop), fwd: phi-MLP F->F->3F, U|V (3 comps) F->2F, update MLP 2F->F->3F ; readout F->R
     fwd = T * N * 2.0 * (F * F + 3 * F * F + 3 * 2 * F * F + 2 * F * F + 3 * F * F) + N * 2.0 * F * R
     w["fwd_node"] = ("tensor", fwd, "flop")
@@ -265,9 +275,10 @@ def main():
             acc[kname] = acc.get(kname, 0.0) + v / reps
     m.set_option("stage_timing", 0)
     peaks = _peaks()
-    work = _stage_work(stats, model, N)
+    split = acc.get("layer0", 0.0) > 0.0             # collapsed layer-0 passes timed as their own stage
+    work = _stage_work(stats, model, N, layer0_split=split)
     T = model["T"]
-    n_launch_of = {"fwd_edge": T, "bwd_edge": T}
+    n_launch_of = {"fwd_edge": T - 1, "bwd_edge": T - 1} if split else {"fwd_edge": T, "bwd_edge": T}
 
     def _roof(name):
         bound, units, _ = work[name]
@@ -301,7 +312,7 @@ def main():
     if dom in ("fwd_edge", "bwd_edge"):
         # the edge kernels are bound by the L2 -> SM row gather, not by DRAM: bytes gathered per edge and channel
         # against the measured gather ceiling of this access pattern (profiles/r01_microbench.md)
-        per_edge = {"fwd_edge": (8.0 + 20.0 * (T - 1)) / T, "bwd_edge": 16.0}[dom] * model["F"]
+        per_edge = {"fwd_edge": 20.0 if split else (8.0 + 20.0 * (T - 1)) / T, "bwd_edge": 16.0}[dom] * model["F"]
         gb = stats["n_edges"] * per_edge / (dur_ms * 1e-3) / 1e9
         roofline["l2_gather"] = dict(achieved=gb, peak=16200.0, unit="GB/s", frac=gb / 16200.0,
                                      peak_source="measured row-gather microbenchmark (512 B per warp request)")

@@ -21,8 +21,9 @@ struct Buf {
     size_t bytes = 0;
 };
 
-enum Stage { ST_NBR = 0, ST_FWD_NODE, ST_FWD_EDGE, ST_BWD_NODE, ST_BWD_EDGE, ST_FORCE, ST_COUNT };
-const char* kStageNames[ST_COUNT] = {"nbr_build", "fwd_node", "fwd_edge", "bwd_node", "bwd_edge", "force_virial"};
+enum Stage { ST_NBR = 0, ST_FWD_NODE, ST_FWD_EDGE, ST_BWD_NODE, ST_BWD_EDGE, ST_FORCE, ST_L0, ST_COUNT };
+// "layer0": both collapsed layer-0 message passes with their GEMMs (edge_l0.cu); fwd_edge / bwd_edge then hold layers >= 1
+const char* kStageNames[ST_COUNT] = {"nbr_build", "fwd_node", "fwd_edge", "bwd_node", "bwd_edge", "force_virial", "layer0"};
 
 struct LayerBuf {
     float *hpre, *phi, *sn, *v1, *pq, *zpre, *a;
@@ -642,6 +643,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
             // layer 0: per-(receiver, species) radial sums (O(K) per edge), then two GEMMs (edge_l0.cu).  The sums live in
             // the gather-row buffers, which layer 0 does not use: Q1 [N][128], Q4 [3N][128] floats
             float *As = P<float>(m->b_Q1), *Av = P<float>(m->b_Q4);
+            mark(m, st, ST_L0);
             if (message_fwd0_collapsed_accum(L, N, K, rcf, row_ptr, ej, P<int>(m->b_types_s), m->n_species, S, F, sn, 2 * F, As, Av,
                                              m->np0)) {
                 gemm_nt(L, As, m->np0, m->Wl0sT, m->np0, sn, 2 * F, N, F, m->np0, nullptr, true);
@@ -698,10 +700,9 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
             // layer 0: contract the channels per (receiver, sender species) with two GEMMs, then O(K) work per edge.
             // B -> the gather-row buffer ([3N][128] floats of its [N][128] float4), C -> the (unused at layer 0) phib buffer
             float *Bv = P<float>(m->b_Q4), *Cs = phib;
-            mark(m, st, ST_BWD_NODE);
+            mark(m, st, ST_L0);
             gemm_nt(L, v1b, F, m->Wl0v, F, Bv, m->np0, 3 * N, m->np0, F, nullptr, false);
             gemm_nt(L, s1b, F, m->Wl0s, F, Cs, m->np0, N, m->np0, F, nullptr, false);
-            mark(m, st, ST_BWD_EDGE);
             done = message_bwd0_collapsed(L, N, K, rcf, row_ptr, ej, P<int>(m->b_types_s), m->n_species, P<int>(m->b_rev), Bv,
                                           Cs, m->np0, P<float4>(m->b_G), t == T - 1);
         }
