@@ -691,8 +691,9 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         update_bwd1(L, N, F, sb, vb, P<float>(m->b_pq[t]), P<float>(m->b_a[t]), ab, pqb);
         gemm_nt_dsilu(L, ab, 3 * F, l.Wu2T, 3 * F, gb, F, N, F, 3 * F, P<float>(m->b_zpre[t]));
         gemm_nt(L, gb, F, l.Wu1T, F, snb, 2 * F, N, 2 * F, F, nullptr, false);
-        update_bwd2(L, N, F, sb, vb, snb, P<float>(m->b_sn[t]), P<float>(m->b_pq[t]), pqb, s1b, v1b);
-        gemm_nt(L, pqb, 2 * F, l.UVT, 2 * F, v1b, F, 3 * N, F, 2 * F, nullptr, true);
+        // vb'_1 = vb + (U^T pb + V^T qb): the GEMM takes vb as the residual of its epilogue (no copy into v1b first)
+        update_bwd2(L, N, F, sb, vb, snb, P<float>(m->b_sn[t]), P<float>(m->b_pq[t]), pqb, s1b, nullptr);
+        gemm_nt_resid(L, pqb, 2 * F, l.UVT, 2 * F, v1b, F, 3 * N, F, 2 * F, vb);
         mark(m, st, ST_BWD_EDGE);
         bool done = false;
         if (t == 0 && m->edge_path == 0 && m->l0_collapse && m->Wl0s && m->np0 == 128 && g_filter_emulate == 0 &&

@@ -70,6 +70,8 @@ void gemm_nt(const Launch& L, const float* A, int lda, const float* B, int ldb, 
 
 void gemm_nt_act(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
                  int N, int K, const float* bias, bool accumulate, bool act_a);
+void gemm_nt_resid(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
+                   int N, int K, const float* resid);
 bool gemm_act_supported(int N, int K);
 void gemm_nt_dsilu(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
                    int N, int K, const float* pre);

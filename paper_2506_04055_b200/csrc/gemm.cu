@@ -185,7 +185,8 @@ int g_gemm_fwd_exact = 1;   // forward GEMMs: 1 = exact integer-slice tensor-cor
 void gemm_register_split(const float* W, const float* hi, const float* lo) { g_split[W] = {hi, lo}; }
 void gemm_unregister_split(const float* W) { g_split.erase(W); }
 bool gemm_nt_tc(const Launch& L, const float* A, int lda, const float* Whi, const float* Wlo, int ldw, float* C, int ldc,
-                long long M, int N, int K, const float* bias, bool accumulate, const float* dsilu_pre = nullptr, int ld_pre = 0);
+                long long M, int N, int K, const float* bias, bool accumulate, const float* dsilu_pre = nullptr, int ld_pre = 0,
+                const float* resid = nullptr);
 void mul_dsilu(const Launch& L, long long n, const float* pre, float* g);
 
 void gemm_nt_act(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
@@ -212,6 +213,23 @@ void gemm_nt_dsilu(const Launch& L, const float* A, int lda, const float* B, int
     }
     gemm_nt(L, A, lda, B, ldb, C, ldc, M, N, K, nullptr, false);
     mul_dsilu(L, M * N, pre, C);
+}
+
+// C = resid + A . B^T  (resid: [M x N], row stride ldc, may not overlap C): the adjoint GEMMs that add to a term held in
+// another buffer read it in the epilogue instead of having it copied into C first
+void gemm_nt_resid(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
+                   int N, int K, const float* resid) {
+    if (M == 0) return;
+    if (g_gemm_path == 0 && g_gemm_emulate == 0) {
+        auto it = g_split.find(B);
+        if (it != g_split.end() &&
+            gemm_nt_tc(L, A, lda, it->second.first, it->second.second, ldb, C, ldc, M, N, K, nullptr, false, nullptr, 0, resid)) {
+            g_last_gemm_tc = 1;
+            return;
+        }
+    }
+    cudaMemcpy2DAsync(C, (size_t)ldc * 4, resid, (size_t)ldc * 4, (size_t)N * 4, (size_t)M, cudaMemcpyDeviceToDevice, L.stream);
+    gemm_nt(L, A, lda, B, ldb, C, ldc, M, N, K, nullptr, true);
 }
 
 // act_a: C = SiLU(A) . B^T + bias  (only the fp32 FFMA path implements it; callers use it on forward GEMMs only)

@@ -57,6 +57,7 @@ struct Params {
     int N, K, ldc, accumulate;
     const float* dsilu_pre;    // optional [M x N] (row stride ld_pre): C = (A W^T + bias) * SiLU'(pre), fused adjoint of the activation
     int ld_pre;
+    const float* resid;        // accumulate: the term added to A W^T (row stride ldc); C itself for an in-place accumulation
 };
 __device__ __forceinline__ float dsilu_x(float x) {
     const float sg = __fdividef(1.0f, 1.0f + __expf(-x));     // adjoint only: 2 ulp (forces carry a relative tolerance)
@@ -220,7 +221,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
                 if (p.accumulate) {
 #pragma unroll
                     for (int i = 0; i < 8; i++)
-                        if (row0 + 4 * i < p.M) o[i] = __ldcs((const float4*)(p.C + (row0 + 4 * i) * p.ldc + n0 + c0 + c4));
+                        if (row0 + 4 * i < p.M) o[i] = __ldcs((const float4*)(p.resid + (row0 + 4 * i) * p.ldc + n0 + c0 + c4));
                 } else if (p.dsilu_pre) {     // (never combined with accumulate)
 #pragma unroll
                     for (int i = 0; i < 8; i++)
@@ -746,7 +747,8 @@ bool gemm_nt_exact(const Launch& L, const float* A, int lda, const float* W, flo
 
 // Returns false when the shape is not covered (caller falls back to the SIMT path).
 bool gemm_nt_tc(const Launch& L, const float* A, int lda, const float* Whi, const float* Wlo, int ldw, float* C, int ldc,
-                long long M, int N, int K, const float* bias, bool accumulate, const float* dsilu_pre, int ld_pre) {
+                long long M, int N, int K, const float* bias, bool accumulate, const float* dsilu_pre, int ld_pre,
+                const float* resid) {
     using namespace tc;
     if (dsilu_pre && (accumulate || (ld_pre % 4) || ((uintptr_t)dsilu_pre & 15))) return false;
     if (M <= 0 || K % BK != 0 || K < BK || (lda % 4) || (ldw % 4) || (ldc % 4)) return false;
@@ -762,7 +764,8 @@ bool gemm_nt_tc(const Launch& L, const float* A, int lda, const float* Whi, cons
     CUtensorMap ma, mh, ml;
     if (!make_map(&ma, A, M, K, lda, BM) || !make_map(&mh, Whi, N, K, ldw, BN) || !make_map(&ml, Wlo, N, K, ldw, BN))
         return false;
-    Params p{C, bias, M, N, K, ldc, accumulate ? 1 : 0, dsilu_pre, ld_pre};
+    if (resid && (((uintptr_t)resid & 15) || dsilu_pre)) return false;
+    Params p{C, bias, M, N, K, ldc, (accumulate || resid) ? 1 : 0, dsilu_pre, ld_pre, resid ? resid : C};
     if (BN == 128) return launch<128, 3>(L, ma, mh, ml, p, n_sm);
     return launch<64, 4>(L, ma, mh, ml, p, n_sm);
 }

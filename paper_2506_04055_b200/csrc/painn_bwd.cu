@@ -64,7 +64,7 @@ __global__ void k_update_bwd2(long long N, int F, const float* __restrict__ sb, 
 #pragma unroll
     for (int c = 0; c < 3; c++) {
         pqb[a * 6 * F + c * 2 * F + F + f] += nb_over_n * pq[a * 6 * F + c * 2 * F + F + f];
-        v1b[a * 3 * F + c * F + f] = vb[a * 3 * F + c * F + f];
+        if (v1b) v1b[a * 3 * F + c * F + f] = vb[a * 3 * F + c * F + f];   // nullptr: the U|V adjoint GEMM reads vb as its residual
     }
     s1b[idx] = sb[idx] + snb[a * 2 * F + f];
 }
