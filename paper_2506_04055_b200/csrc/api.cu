@@ -48,6 +48,7 @@ struct mlp_model {
     float *Wl0s = nullptr, *Wl0v = nullptr;   // [np0][F]: layer-0 adjoint with the channels contracted first (edge_l0.cu)
     float *Wl0sT = nullptr, *Wl0vT = nullptr; // [F][np0]: their transposes, the forward counterpart
     int np0 = 0;                        // columns of those GEMMs: n_species (K + 1) rounded up to 128
+    int fwd_groups = 1;                 // option: forward edge kernel as one 512-thread CTA per SM, filter chunks s, vs in TMEM (0: k_msg_fwd)
     int l0_collapse = 1;                // option: use them (0: k_msg_bwd0)
     // capacities
     long long cap_atoms = 0, cap_edges = 0, cap_cells = 0;
@@ -445,6 +446,7 @@ __attribute__((visibility("default"))) int mlp_set_option(mlp_model* m, const ch
     if (!strcmp(name, "gemm_emulate")) { painn::g_gemm_emulate = (int)value; return MLP_OK; }
     if (!strcmp(name, "edge_path")) { m->edge_path = (int)value; return MLP_OK; }
     if (!strcmp(name, "l0_collapse")) { m->l0_collapse = (int)value; return MLP_OK; }
+    if (!strcmp(name, "fwd_groups")) { m->fwd_groups = (int)value; return MLP_OK; }
     if (!strcmp(name, "gemm_fwd_tc")) { m->fwd_tc = value != 0; return MLP_OK; }
     if (!strcmp(name, "gemm_bwd_exact")) { m->bwd_exact = value != 0; return MLP_OK; }
     if (!strcmp(name, "gemm_path")) { painn::g_gemm_path = (int)value; return MLP_OK; }
@@ -655,7 +657,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
             if (!l0_table) make_gather_rows(L, N, phi, V, P<float>(m->b_Q4), P<float>(m->b_Q1), t > 0);
             if (m->edge_path == 0 && (t > 0 || m->tab0))
                 done = message_fwd_v3(L, N, K, rcf, row_ptr, ej, S, V, P<float>(m->b_Q4), P<float>(m->b_Q1), m->filt_img[t],
-                                      sn, v1, t > 0, P<int>(m->b_types_s), m->tab0, m->n_species);
+                                      m->filt_rows[t], sn, v1, t > 0, P<int>(m->b_types_s), m->tab0, m->n_species, m->fwd_groups != 0);
             if (!done)
                 done = message_fwd_tc(L, N, K, rcf, row_ptr, ej, S, V, P<float>(m->b_Q4), P<float>(m->b_Q1), m->filt_img[t],
                                       sn, v1, t > 0);

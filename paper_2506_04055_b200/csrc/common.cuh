@@ -120,8 +120,8 @@ bool message_bwd_tc2(const Launch& L, long long N, int K, float rc, const int* r
 
 // ---- generation-3 edge kernels (edge_v3.cu), F = 128: software-pipelined gathers, shared-memory channel reduction ----
 bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* s,
-                    const float* v, const float* Q4, const float* Q1, const void* A_img, float* sn, float* v1, bool has_v,
-                    const int* types_s = nullptr, const float* tab = nullptr, int n_tab = 0);
+                    const float* v, const float* Q4, const float* Q1, const void* A_img, const void* A_rows, float* sn, float* v1,
+                    bool has_v, const int* types_s, const float* tab, int n_tab, bool grouped);
 bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
                     const float* phi, const float* v_in, const float* v1b, const void* A_img, const void* A_rows, float* phib,
                     float* vb_out, float4* G, bool first, bool layer0);

@@ -96,6 +96,7 @@ struct FwdParams {
     const float* Q1;
     const float2* Q2;
     const uint4* A_img;
+    const uint4* A_rows;   // [3][128][96] fp16 rows of the same operand (grouped kernel: TMEM-resident chunks s, vs)
     float* sn;     // s' written with row stride 2F
     float* v1;
     float inv_rc;
@@ -421,6 +422,304 @@ __device__ __forceinline__ void umma_f16_ts(uint32_t tmem_d, uint32_t tmem_a, ui
         "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(acc)
         : "memory");
 }
+
+// =============================================================================================================
+// forward message pass, grouped form: one 512-thread CTA per SM = two independent 8-warp pipelines ("groups", as in the
+// adjoint kernel below) that share ONE copy of the filter operand, chunks s and vs of which are TMEM-resident (A-from-
+// TMEM MMA).  ncu on k_msg_fwd: the tensor core re-reads the 72 KB shared-memory image for every 32-edge tile (33 % of the
+// L1 data stage, l1tex__data_pipe_tc_wavefronts) and collides with the consumers' loads on the data banks (arbitration
+// conflicts in 23 % of the cycles, LSU wavefronts 74 %): the kernel is bound by the L1 data stage, not by L2 or DRAM.
+// =============================================================================================================
+constexpr int FWDG_THREADS = 512;
+constexpr int FWDG_GROUP_BYTES = ((2 * B_BYTES + 2 * NE * 16 + 64) + 127) / 128 * 128;
+constexpr int fwdg_smem_bytes(bool has_v) {
+    return (has_v ? 1 : 0) * A_CHUNK_BYTES + 2 * FWDG_GROUP_BYTES + 128 + (has_v ? 0 : TAB_MAX * F * 8);
+}
+template <bool HAS_V>
+__global__ void __launch_bounds__(FWDG_THREADS, 1) k_msg_fwd_g(const FwdParams p) {
+    constexpr int NCH = HAS_V ? 3 : 2;
+    constexpr int TCOLS = NCH * NE;                 // TMEM columns per buffer
+    extern __shared__ __align__(128) uint8_t smem[];
+    constexpr int NSM = NCH - 2;                    // chunks kept in shared memory (vv); s and vs live in TMEM
+    uint8_t* sA = smem;
+    const int tid = threadIdx.x, grp = tid >> 8, ltid = tid & 255, lwarp = ltid >> 5, lane = tid & 31;
+    uint8_t* gbase = smem + NSM * A_CHUNK_BYTES + grp * FWDG_GROUP_BYTES;
+    uint8_t* sB = gbase;
+    float4* sMeta = (float4*)(sB + 2 * B_BYTES);   // [2][NE] (u_e, sender index)
+    uint64_t* bars = (uint64_t*)(sMeta + 2 * NE);
+    uint64_t* b_full = bars;          // [2] producers -> MMA (and consumers: sender indices readable)  (count 96)
+    uint64_t* t_full = bars + 2;      // [2] MMA commit -> consumers (count 1)
+    const int NB = 1 + grp * 2;       // named barriers NB + buf of this group (consumers -> producers: tile consumed)
+    uint32_t* tmem_slot = (uint32_t*)(smem + NSM * A_CHUNK_BYTES + 2 * FWDG_GROUP_BYTES);
+    float2* sTab = (float2*)(tmem_slot + 32);          // [n_tab][F] species table (layer 0 only), shared by both groups
+
+    {
+        const uint4* src = p.A_img + 2 * (A_CHUNK_BYTES / 16);        // chunk vv of the shared-memory image
+        uint4* dst = (uint4*)sA;
+        for (int i = tid; i < NSM * A_CHUNK_BYTES / 16; i += FWDG_THREADS) dst[i] = src[i];
+        uint4* zb = (uint4*)sB;
+        for (int i = ltid; i < 2 * B_BYTES / 16; i += 256) zb[i] = make_uint4(0, 0, 0, 0);
+        if (!HAS_V)
+            for (int i = tid; i < p.n_tab * F; i += FWDG_THREADS) sTab[i] = p.tab[i];
+    }
+    if (ltid == 0) {
+        for (int b = 0; b < 2; b++) { mbar_init(&b_full[b], 96); mbar_init(&t_full[b], 1); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (tid >> 5 == 15) tmem_alloc(tmem_slot, 512);
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    // chunks s and vs of the filter operand into TMEM (lane = channel row, 48 columns = 96 fp16 each): columns 192..239
+    // and 448..495, the gaps behind the two groups' accumulators (2 buffers x TCOLS <= 192 columns each)
+    if (tid < 128) {
+#pragma unroll
+        for (int c = 0; c < 2; c++) {
+            const uint32_t abase = *tmem_slot + 192 + c * 256 + ((uint32_t)((tid >> 5) * 32) << 16);
+            const uint4* src = p.A_rows + ((size_t)c * 128 + tid) * 12;
+#pragma unroll
+            for (int j = 0; j < 3; j++) {
+                uint32_t r[16];
+#pragma unroll
+                for (int q = 0; q < 4; q++) { const uint4 v = src[j * 4 + q]; r[4 * q] = v.x; r[4 * q + 1] = v.y; r[4 * q + 2] = v.z; r[4 * q + 3] = v.w; }
+                tmem_st16(abase + j * 16, r);
+            }
+        }
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot + grp * 256;
+    const uint32_t tmem_A = *tmem_slot + 192;
+
+    const long long N = p.N;
+    const int apu = p.atoms_per_unit;
+    const int* __restrict__ row_ptr = p.row_ptr;
+    const long long n_units = (N + apu - 1) / apu;
+    const long long u0 = (long long)blockIdx.x * 2 + grp, ustride = (long long)gridDim.x * 2;
+    if (lwarp < 4) reg_inc<168>(); else reg_dec<88>();
+
+    if (lwarp < 4) {
+        // ===================== consumers: one channel per thread =====================
+        const int f = ltid;
+        const float4* __restrict__ Q4 = p.Q4 + f;
+        const float* __restrict__ Q1 = p.Q1 + f;
+        const float2* __restrict__ Q2 = p.Q2 + f;
+        const float* __restrict__ s_in = p.s + f;
+        const float* __restrict__ v_in = p.v + f;
+        float* __restrict__ sn = p.sn + f;
+        float* __restrict__ v1 = p.v1 + f;
+        const uint32_t lane_base = tmem_base + ((uint32_t)(lwarp * 32) << 16);
+        float4 qa4[8], qb4[8];
+        float qa1[8], qb1[8];
+        float2 qa2[8], qb2[8];
+#define FWD_ISSUE(Q4R, Q1R, Q2R, META8)                                                   \
+    {                                                                                     \
+        _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                \
+            const size_t row_ = (size_t)__float_as_int((META8)[i_].w) * F;                \
+            if (HAS_V) { Q4R[i_] = __ldg(Q4 + row_); Q1R[i_] = __ldg(Q1 + row_); }        \
+        }                                                                                 \
+    }
+        uint32_t it = 0;
+        bool pre = false;                 // first batch of tile `it` already in flight (bank a)
+        for (long long u = u0; u < n_units; u += ustride) {
+            const long long a0 = u * apu;
+            const int na = (int)min((long long)apu, N - a0);
+            const int rp = __ldg(row_ptr + a0 + min(lane, na));           // lanes 0..na hold the unit's row pointers
+            const int e_begin = __shfl_sync(0xffffffffu, rp, 0), e_end = __shfl_sync(0xffffffffu, rp, na);
+            const int ntiles = (e_end - e_begin + NE - 1) / NE;
+            bool next_has = false;                                        // does the CTA's next unit have a tile?
+            {
+                const long long un = u + ustride;
+                if (un < n_units) {
+                    const long long b0 = un * apu, b1 = min(N, b0 + apu);
+                    next_has = __ldg(row_ptr + b1) > __ldg(row_ptr + b0);
+                }
+            }
+            if (HAS_V && ntiles > 0 && !pre) {
+                mbar_wait(&b_full[it & 1], (it >> 1) & 1);
+                const float4* m0 = sMeta + (it & 1) * NE;
+                FWD_ISSUE(qa4, qa1, qa2, m0);
+            }
+            pre = false;
+            int a_rel = 0;
+            int row_end = __shfl_sync(0xffffffffu, rp, 1);
+            float accS = 0.f, acc0 = 0.f, acc1 = 0.f, acc2 = 0.f;
+            // residual (s_i, v_i) of the current receiver: loaded at row start, added at row end
+            float rs = s_in[(a0 + a_rel) * F], rv0 = 0.f, rv1 = 0.f, rv2 = 0.f;
+            if (HAS_V) { rv0 = v_in[(a0 + a_rel) * 3 * F]; rv1 = v_in[(a0 + a_rel) * 3 * F + F]; rv2 = v_in[(a0 + a_rel) * 3 * F + 2 * F]; }
+            auto store_row = [&]() {
+                const long long a = a0 + a_rel;
+                sn[a * 2 * F] = accS + rs;
+                v1[a * 3 * F] = acc0 + rv0; v1[a * 3 * F + F] = acc1 + rv1; v1[a * 3 * F + 2 * F] = acc2 + rv2;
+            };
+            auto next_row = [&]() {
+                store_row();
+                a_rel++;
+                row_end = __shfl_sync(0xffffffffu, rp, a_rel + 1);
+                accS = acc0 = acc1 = acc2 = 0.f;
+                const long long a = a0 + a_rel;
+                rs = s_in[a * F];
+                if (HAS_V) { rv0 = v_in[a * 3 * F]; rv1 = v_in[a * 3 * F + F]; rv2 = v_in[a * 3 * F + 2 * F]; }
+            };
+#define FWD_COMPUTE(BI, Q4R, Q1R, Q2R)                                                                      \
+    {                                                                                                       \
+        const int E8_ = e_begin + t * NE + (BI) * 8;                                                        \
+        if (E8_ < e_end) {                                                                                  \
+            while (E8_ >= row_end) next_row();                                                              \
+            uint32_t ws[8], wvs[8], wvv[8];                                                                 \
+            tmem_ld8_nowait(lane_base + buf * TCOLS + (BI) * 8, ws);                                        \
+            tmem_ld8_nowait(lane_base + buf * TCOLS + NE + (BI) * 8, wvs);                                  \
+            if (HAS_V) tmem_ld8_nowait(lane_base + buf * TCOLS + 2 * NE + (BI) * 8, wvv);                   \
+            tmem_wait_ld();                                                                                 \
+            _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                              \
+                const float4 m_ = meta[(BI) * 8 + i_];                                                      \
+                const float w_s = __uint_as_float(ws[i_]), w_vs = __uint_as_float(wvs[i_]);                 \
+                if (HAS_V) {                                                                                \
+                    const float w_vv = __uint_as_float(wvv[i_]);                                            \
+                    accS = fmaf(w_s, Q4R[i_].x, accS);                                                      \
+                    const float tv = w_vs * Q4R[i_].y;                                                      \
+                    acc0 = fmaf(tv, m_.x, fmaf(w_vv, Q4R[i_].z, acc0));                                     \
+                    acc1 = fmaf(tv, m_.y, fmaf(w_vv, Q4R[i_].w, acc1));                                     \
+                    acc2 = fmaf(tv, m_.z, fmaf(w_vv, Q1R[i_], acc2));                                       \
+                } else {                                                                                    \
+                    const float2 q_ = sTab[__float_as_int(m_.w) * F + f];       /* species row of the sender */ \
+                    accS = fmaf(w_s, q_.x, accS);                                                           \
+                    const float tv = w_vs * q_.y;                                                           \
+                    acc0 = fmaf(tv, m_.x, acc0);                                                            \
+                    acc1 = fmaf(tv, m_.y, acc1);                                                            \
+                    acc2 = fmaf(tv, m_.z, acc2);                                                            \
+                }                                                                                           \
+            }                                                                                               \
+        }                                                                                                   \
+    }
+            for (int t = 0; t < ntiles; t++, it++) {
+                const int buf = it & 1;
+                const float4* meta = sMeta + buf * NE;
+                FWD_ISSUE(qb4, qb1, qb2, meta + 8);
+                mbar_wait(&t_full[buf], (it >> 1) & 1);
+                tc_fence_after();
+                FWD_COMPUTE(0, qa4, qa1, qa2);
+                FWD_ISSUE(qa4, qa1, qa2, meta + 16);
+                FWD_COMPUTE(1, qb4, qb1, qb2);
+                FWD_ISSUE(qb4, qb1, qb2, meta + 24);
+                FWD_COMPUTE(2, qa4, qa1, qa2);
+                if (HAS_V && (t + 1 < ntiles || next_has)) {       // first batch of the CTA's next tile
+                    mbar_wait(&b_full[buf ^ 1], ((it + 1) >> 1) & 1);
+                    const float4* mn = sMeta + (buf ^ 1) * NE;
+                    FWD_ISSUE(qa4, qa1, qa2, mn);
+                    pre = t + 1 == ntiles;
+                }
+                FWD_COMPUTE(3, qb4, qb1, qb2);
+                tc_fence_before();
+                bar_arrive(NB + buf, 224);              // tile consumed: 128 consumers arrive, 96 producers wait (named barrier)
+            }
+            // finish the last receiver with edges, then pass trailing edge-less atoms through (s' = s, v' = v)
+            for (;;) {
+                store_row();
+                if (a_rel + 1 >= na) break;
+                a_rel++;
+                accS = acc0 = acc1 = acc2 = 0.f;
+                const long long a = a0 + a_rel;
+                rs = s_in[a * F];
+                if (HAS_V) { rv0 = v_in[a * 3 * F]; rv1 = v_in[a * 3 * F + F]; rv2 = v_in[a * 3 * F + 2 * F]; }
+            }
+        }
+#undef FWD_ISSUE
+#undef FWD_COMPUTE
+    } else if (lwarp < 7) {
+        // ===================== producers: B operand R_e = fc (1, rho_1 .. rho_K), three fp16 planes =====================
+        const int pt = ltid - 128, e = pt & 31, h = pt >> 5;   // h: basis slots 8h .. 8h+7 (slot 0 = bias, slot n = rho_n)
+        const float inv_rc = p.inv_rc;
+        const int K = p.K;
+        uint32_t it = 0;
+        for (long long u = u0; u < n_units; u += ustride) {
+            const long long a0 = u * apu;
+            const long long a1 = min(N, a0 + (long long)apu);
+            const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
+            const int ntiles = (e_end - e_begin + NE - 1) / NE;
+            float4 raw_n = load_edge_raw(p.ej, e_begin + e, e_end);
+            for (int t = 0; t < ntiles; t++, it++) {
+                const int buf = it & 1;
+                const float4 raw = raw_n;
+                if (t + 1 < ntiles) raw_n = load_edge_raw(p.ej, e_begin + (t + 1) * NE + e, e_end);
+                const EdgeGeom g = edge_geom(raw, e_begin + t * NE + e, e_end, inv_rc);
+                const float fc = g.real ? 0.5f * (1.0f + g.c1) : 0.0f;
+                const float amp = fc * g.inv_d;
+                float sn_, cn_;
+                if (h == 0) { sn_ = g.s1; cn_ = g.c1; } else sincospif((float)(8 * h) * g.x, &sn_, &cn_);
+                float vals[8];
+#pragma unroll
+                for (int i = 0; i < 8; i++) {
+                    const int b = h * 8 + i;
+                    float R;
+                    if (b == 0) R = fc;
+                    else {
+                        R = b <= K ? amp * sn_ : 0.0f;
+                        const float tt = sn_ * g.c1 + cn_ * g.s1;
+                        cn_ = cn_ * g.c1 - sn_ * g.s1;
+                        sn_ = tt;
+                    }
+                    vals[i] = R;
+                }
+                uint4 p0, p1, p2;
+                split3(vals, p0, p1, p2);
+                if (it >= 2) bar_sync(NB + buf, 224);   // tile it - 2 consumed (hardware-blocking wait, no spin)
+                uint8_t* bb = sB + buf * B_BYTES + (e >> 3) * SBO + (e & 7) * 16 + h * LBO;
+                *(uint4*)(bb) = p0;                       // term 0: k = b
+                *(uint4*)(bb + 4 * LBO) = p1;             // term 1: k = 32 + b   (lo(R) 2^11)
+                *(uint4*)(bb + 8 * LBO) = p2;             // term 2: k = 64 + b   (hi(R) 2^-11)
+                if (h == 0) {
+                    float mw = g.r.w;                                             // sender index ...
+                    if (!HAS_V) mw = __int_as_float(__ldg(p.types + __float_as_int(g.r.w)));   // ... or its species (layer 0)
+                    sMeta[buf * NE + e] = make_float4(g.r.x * g.inv_d, g.r.y * g.inv_d, g.r.z * g.inv_d, mw);
+                }
+                fence_async_smem();
+                mbar_arrive(&b_full[buf]);
+            }
+        }
+    } else {
+        // ===================== MMA issuer: the warp stays converged, one elected lane issues (descriptors in uniform registers) =====================
+        {
+            const uint32_t idesc = (1u << 4) | ((uint32_t)(NE >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);   // f16 x f16 -> f32
+            const uint32_t a_base = smem_u32(sA), b_base = smem_u32(sB);
+            uint32_t it = 0;
+            for (long long u = u0; u < n_units; u += ustride) {
+                const long long a0 = u * apu;
+                const long long a1 = min(N, a0 + (long long)apu);
+                const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
+                const int ntiles = (e_end - e_begin + NE - 1) / NE;
+                for (int t = 0; t < ntiles; t++, it++) {
+                    const int buf = it & 1;
+                    mbar_wait_sleep(&b_full[buf], (it >> 1) & 1, 128);
+                    tc_fence_after();
+                    if (elect_one()) {
+#pragma unroll
+                        for (int c = 0; c < NCH; c++) {
+                            const uint32_t d = tmem_base + buf * TCOLS + c * NE;
+#pragma unroll
+                            for (int o = 0; o < 6; o++) {
+                                const int kk = (o + 2) % 6;          // small terms (k-steps 2..5) first, main term last
+                                const uint64_t bd = make_desc_nosw(b_base + buf * B_BYTES + kk * 2 * LBO, LBO, SBO);
+                                if (c < 2) umma_f16_ts(d, tmem_A + c * 256 + kk * 8, bd, idesc, o != 0);
+                                else umma_f16(d, make_desc_nosw(a_base + kk * 2 * LBO, LBO, SBO), bd, idesc, o != 0);
+                            }
+                        }
+                        umma_commit(&t_full[buf]);
+                    }
+                    __syncwarp();
+                }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (tid >> 5 == 15) tmem_dealloc(*tmem_slot, 512);
+}
+
+
 
 struct BwdParams {
     long long N;
@@ -1183,8 +1482,8 @@ static int sm_count() {
 
 // F = 128, K <= 23 only.  Q4/Q1 from make_gather_rows (layer 0: Q4 holds float2 rows); A_img from edge_build_filter_image.
 bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* s,
-                    const float* v, const float* Q4, const float* Q1, const void* A_img, float* sn, float* v1, bool has_v,
-                    const int* types_s, const float* tab, int n_tab) {
+                    const float* v, const float* Q4, const float* Q1, const void* A_img, const void* A_rows, float* sn, float* v1,
+                    bool has_v, const int* types_s, const float* tab, int n_tab, bool grouped) {
     using namespace ev3;
     if (N == 0) return true;
     if (K > 23) return false;
@@ -1192,16 +1491,25 @@ bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
     static bool attr = false;
     if (!attr) {
         if (cudaFuncSetAttribute(k_msg_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fwd_smem_bytes(true)) != cudaSuccess ||
-            cudaFuncSetAttribute(k_msg_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fwd_smem_bytes(false)) != cudaSuccess)
+            cudaFuncSetAttribute(k_msg_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fwd_smem_bytes(false)) != cudaSuccess ||
+            cudaFuncSetAttribute(k_msg_fwd_g<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fwdg_smem_bytes(true)) != cudaSuccess ||
+            cudaFuncSetAttribute(k_msg_fwd_g<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fwdg_smem_bytes(false)) != cudaSuccess)
             return false;
         attr = true;
     }
-    FwdParams p{N, row_ptr, ej, s, v, (const float4*)Q4, Q1, (const float2*)Q4, (const uint4*)A_img, sn, v1, 1.0f / rc, K, 16,
-                types_s, (const float2*)tab, n_tab};
+    FwdParams p{N, row_ptr, ej, s, v, (const float4*)Q4, Q1, (const float2*)Q4, (const uint4*)A_img, (const uint4*)A_rows, sn, v1,
+                1.0f / rc, K, 16, types_s, (const float2*)tab, n_tab};
     const long long n_units = (N + p.atoms_per_unit - 1) / p.atoms_per_unit;
-    const int grid = (int)std::min<long long>(n_units, 2LL * sm_count());
-    if (has_v) k_msg_fwd<true><<<grid, FWD_THREADS, fwd_smem_bytes(true), L.stream>>>(p);
-    else k_msg_fwd<false><<<grid, FWD_THREADS, fwd_smem_bytes(false), L.stream>>>(p);
+    if (grouped && A_rows) {
+        // one CTA per SM, two 8-warp pipelines sharing the TMEM-resident filter operand
+        const int grid = (int)std::min<long long>((n_units + 1) / 2, (long long)sm_count());
+        if (has_v) k_msg_fwd_g<true><<<grid, FWDG_THREADS, fwdg_smem_bytes(true), L.stream>>>(p);
+        else k_msg_fwd_g<false><<<grid, FWDG_THREADS, fwdg_smem_bytes(false), L.stream>>>(p);
+    } else {
+        const int grid = (int)std::min<long long>(n_units, 2LL * sm_count());
+        if (has_v) k_msg_fwd<true><<<grid, FWD_THREADS, fwd_smem_bytes(true), L.stream>>>(p);
+        else k_msg_fwd<false><<<grid, FWD_THREADS, fwd_smem_bytes(false), L.stream>>>(p);
+    }
     KLAUNCH(L);
     return true;
 }
