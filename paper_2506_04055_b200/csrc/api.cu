@@ -65,7 +65,7 @@ struct mlp_model {
     Buf b_hpre[PAINN_MAX_T], b_phi[PAINN_MAX_T], b_sn[PAINN_MAX_T], b_v1[PAINN_MAX_T], b_pq[PAINN_MAX_T],
         b_zpre[PAINN_MAX_T], b_a[PAINN_MAX_T];
     Buf b_h, b_rpre, b_rb, b_eatom, b_sb, b_s1b, b_vb, b_v1b, b_ab, b_pqb, b_gb, b_snb, b_phib, b_hb;
-    Buf b_epart, b_wpart;
+    Buf b_epart, b_wpart, b_red;        // b_red: 128 x 10 doubles, first stage of the final reduction
     Buf b_Q4, b_Q1;   // gather rows of the tensor-core edge kernels
     // small
     Buf b_misc;            // device: [0..7] flags (int), then long long totals, then bbox doubles
@@ -189,6 +189,7 @@ int alloc_atoms(mlp_model* m, long long cap) {
     ENS(m, m->b_hb, n * F * 4);
     if (m->F == 128) { ENS(m, m->b_Q4, n * F * 16); ENS(m, m->b_Q1, n * F * 4); }
     ENS(m, m->b_epart, (n / 256 + 2) * 8); ENS(m, m->b_wpart, (n / 8 + 2) * 9 * 8);
+    ENS(m, m->b_red, 128 * 10 * 8);
     m->cap_atoms = cap;
     return MLP_OK;
 }
@@ -423,7 +424,7 @@ __attribute__((visibility("default"))) void mlp_destroy(mlp_model* m) {
                  &m->b_cell_s, &m->b_local, &m->b_row_cnt, &m->b_row_ptr, &m->b_scan_tmp, &m->b_cell_count,
                  &m->b_cell_start, &m->b_cell_fill, &m->b_ej, &m->b_img, &m->b_rev, &m->b_G, &m->b_h, &m->b_rpre,
                  &m->b_rb, &m->b_eatom, &m->b_sb, &m->b_s1b, &m->b_vb, &m->b_v1b, &m->b_ab, &m->b_pqb, &m->b_gb,
-                 &m->b_snb, &m->b_phib, &m->b_hb, &m->b_Q4, &m->b_Q1, &m->b_epart, &m->b_wpart, &m->b_misc, &m->d_pos, &m->d_types,
+                 &m->b_snb, &m->b_phib, &m->b_hb, &m->b_Q4, &m->b_Q1, &m->b_epart, &m->b_wpart, &m->b_red, &m->b_misc, &m->d_pos, &m->d_types,
                  &m->d_owner, &m->d_out};
     for (Buf* b : bs) free_buf(*b);
     for (int t = 0; t <= PAINN_MAX_T; t++) { free_buf(m->b_S[t]); free_buf(m->b_V[t]); }
@@ -740,7 +741,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
     if (N > 0) CU(m, cudaMemsetAsync(forces, 0, (size_t)N * 3 * 8, st));
     force_final(L, N, n_local, row_ptr, ej, P<int>(m->b_rev), P<float4>(m->b_G), P<int>(m->b_perm), ghost_owner,
                 forces, P<double>(m->b_wpart), &n_wpart);
-    reduce_final(L, P<double>(m->b_epart), n_epart, P<double>(m->b_wpart), n_wpart, energy, virial);
+    reduce_final(L, P<double>(m->b_epart), n_epart, P<double>(m->b_wpart), n_wpart, P<double>(m->b_red), energy, virial);
     mark(m, st, -1);
     CU(m, cudaGetLastError());
 

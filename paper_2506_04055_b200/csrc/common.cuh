@@ -99,7 +99,7 @@ void force_final(const Launch& L, long long N, long long n_local, const int* row
                  const int* rev, const float4* G, const int* perm, const int* ghost_owner, double* forces,
                  double* w_partial, int* n_partial);
 void reduce_final(const Launch& L, const double* e_partial, int n_e, const double* w_partial, int n_w,
-                  double* energy, double* virial);
+                  double* scratch, double* energy, double* virial);
 void unpermute_state(const Launch& L, long long N, int F, const int* perm, const float* s, const float* v,
                      float* out);
 

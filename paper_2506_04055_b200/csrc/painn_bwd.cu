@@ -52,26 +52,37 @@ void update_bwd1(const Launch& L, long long N, int F, const float* sb, const flo
     KLAUNCH(L);
 }
 // qb[c] += nb o q[c] / n ;  sb' = sb + ds ;  vb'[c] = vb[c]  (the U^T pb + V^T qb GEMM accumulates on top)
+// four channels per thread (16-byte accesses: the scalar form moved 4.6 TB/s, launch-list of profiles/r01_launches_cfg5.md)
 __global__ void k_update_bwd2(long long N, int F, const float* __restrict__ sb, const float* __restrict__ vb,
                               const float* __restrict__ snb, const float* __restrict__ sn,
                               const float* __restrict__ pq, float* __restrict__ pqb, float* __restrict__ s1b,
                               float* __restrict__ v1b) {
+    const int F4 = F >> 2;
     long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (idx >= N * F) return;
-    long long a = idx / F;
-    int f = (int)(idx - a * F);
-    const float nb_over_n = snb[a * 2 * F + F + f] / sn[a * 2 * F + F + f];
+    if (idx >= N * F4) return;
+    long long a = idx / F4;
+    int f = (int)(idx - a * F4) * 4;
+    const float4 nb = *(const float4*)(snb + a * 2 * F + F + f), nn = *(const float4*)(sn + a * 2 * F + F + f);
+    const float4 r = make_float4(nb.x / nn.x, nb.y / nn.y, nb.z / nn.z, nb.w / nn.w);
+    float4 q[3], qb[3];
 #pragma unroll
     for (int c = 0; c < 3; c++) {
-        pqb[a * 6 * F + c * 2 * F + F + f] += nb_over_n * pq[a * 6 * F + c * 2 * F + F + f];
-        if (v1b) v1b[a * 3 * F + c * F + f] = vb[a * 3 * F + c * F + f];   // nullptr: the U|V adjoint GEMM reads vb as its residual
+        q[c] = *(const float4*)(pq + a * 6 * F + c * 2 * F + F + f);
+        qb[c] = *(const float4*)(pqb + a * 6 * F + c * 2 * F + F + f);
     }
-    s1b[idx] = sb[idx] + snb[a * 2 * F + f];
+    const float4 s0 = *(const float4*)(sb + a * F + f), s1 = *(const float4*)(snb + a * 2 * F + f);
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        qb[c].x += r.x * q[c].x; qb[c].y += r.y * q[c].y; qb[c].z += r.z * q[c].z; qb[c].w += r.w * q[c].w;
+        *(float4*)(pqb + a * 6 * F + c * 2 * F + F + f) = qb[c];
+        if (v1b) *(float4*)(v1b + a * 3 * F + c * F + f) = *(const float4*)(vb + a * 3 * F + c * F + f);   // nullptr: the U|V adjoint GEMM reads vb as its residual
+    }
+    *(float4*)(s1b + a * F + f) = make_float4(s0.x + s1.x, s0.y + s1.y, s0.z + s1.z, s0.w + s1.w);
 }
 void update_bwd2(const Launch& L, long long N, int F, const float* sb, const float* vb, const float* snb,
                  const float* sn, const float* pq, float* pqb, float* s1b, float* v1b) {
     if (N == 0) return;
-    k_update_bwd2<<<(unsigned)((N * F + 255) / 256), 256, 0, L.stream>>>(N, F, sb, vb, snb, sn, pq, pqb, s1b, v1b);
+    k_update_bwd2<<<(unsigned)((N * (F / 4) + 255) / 256), 256, 0, L.stream>>>(N, F, sb, vb, snb, sn, pq, pqb, s1b, v1b);
     KLAUNCH(L);
 }
 
@@ -286,8 +297,41 @@ __global__ void __launch_bounds__(256) k_reduce_final(const double* __restrict__
         virial[5] = 0.5 * (red[5][0] + red[7][0]);
     }
 }
+// first stage for large systems: block b folds its contiguous share of both partial lists into scratch[b][0..9] (flat,
+// coalesced reads of the [n_w][9] list: with 288 = 32 x 9 threads every thread stays on one component)
+constexpr int RED_BLOCKS = 128, RED_THREADS = 288;
+__global__ void __launch_bounds__(RED_THREADS) k_reduce_stage1(const double* __restrict__ e_partial, int n_e,
+                                                               const double* __restrict__ w_partial, int n_w,
+                                                               double* __restrict__ scratch) {
+    __shared__ double red[RED_THREADS];
+    __shared__ double rede[RED_THREADS];
+    const int t = threadIdx.x, b = blockIdx.x;
+    const long long cw = (n_w + RED_BLOCKS - 1) / RED_BLOCKS, w0 = b * cw * 9, w1 = min((long long)n_w, (b + 1) * cw) * 9;
+    double acc = 0.0, ae = 0.0;
+    for (long long j = w0 + t; j < w1; j += RED_THREADS) acc += w_partial[j];
+    const int ce = (n_e + RED_BLOCKS - 1) / RED_BLOCKS, e1 = min(n_e, (b + 1) * ce);
+    for (int j = b * ce + t; j < e1; j += RED_THREADS) ae += e_partial[j];
+    red[t] = acc; rede[t] = ae;
+    __syncthreads();
+    if (t < 9) {
+        double x = 0.0;
+        for (int i = 0; i < RED_THREADS / 9; i++) x += red[t + 9 * i];
+        scratch[b * 9 + t] = x;
+    } else if (t == 32) {
+        double x = 0.0;
+        for (int i = 0; i < RED_THREADS; i++) x += rede[i];
+        scratch[RED_BLOCKS * 9 + b] = x;
+    }
+}
+// scratch: RED_BLOCKS x 10 doubles (used when n_w is large; the single-block pass alone took 0.35 ms at 1M atoms)
 void reduce_final(const Launch& L, const double* e_partial, int n_e, const double* w_partial, int n_w,
-                  double* energy, double* virial) {
+                  double* scratch, double* energy, double* virial) {
+    if (scratch && n_w > 8192) {
+        k_reduce_stage1<<<RED_BLOCKS, RED_THREADS, 0, L.stream>>>(e_partial, n_e, w_partial, n_w, scratch);
+        KLAUNCH(L);
+        e_partial = scratch + RED_BLOCKS * 9; n_e = RED_BLOCKS;
+        w_partial = scratch; n_w = RED_BLOCKS;
+    }
     k_reduce_final<<<1, 256, 0, L.stream>>>(e_partial, n_e, w_partial, n_w, energy, virial);
     KLAUNCH(L);
 }
