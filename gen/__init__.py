@@ -8,5 +8,5 @@ BASELINE.json ``configs`` and are restated in DESIGN.md §4.
 from .weights import make_weights, blob_layout, parse_blob, BLOB_MAGIC, HEADER_BYTES  # noqa: F401
 from .systems import (  # noqa: F401
     CONFIGS, make_config, water_box, diamond, slab_with_ghosts, peptide_water,
-    periodic_ghosts, replicate, extract_cluster,
+    periodic_ghosts, replicate, extract_cluster, random_gas,
 )

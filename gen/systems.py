@@ -252,6 +252,28 @@ def extract_cluster(pos, box, center, r_local, r_total):
     return il, ig, pos[center] + d[idx]
 
 
+def random_gas(n, box, dmin, seed, n_species=2, empty_frac=0.0):
+    """n uniform points in an orthorhombic periodic box with no pair closer than dmin (draw, drop the later atom of every
+    close pair, redraw the missing ones); `empty_frac` keeps the top of the box in z empty.  Row-length stress input
+    for the neighbour list and the edge kernels: far from the paper's liquids on both sides (isolated atoms at low
+    density, rows of > 100 neighbours at high density)."""
+    rng = np.random.default_rng(seed)
+    box = np.asarray(box, float)
+    hi = box * np.array([1.0, 1.0, 1.0 - empty_frac])
+    pos = np.empty((0, 3))
+    for _ in range(200):
+        pos = np.vstack([pos, rng.uniform(0.0, 1.0, (n - len(pos), 3)) * hi])
+        pairs = cKDTree(pos, boxsize=box).query_pairs(dmin, output_type="ndarray")
+        if len(pairs) == 0:
+            break
+        keep = np.ones(len(pos), bool)
+        keep[pairs[:, 1]] = False                      # i < j in every pair: the earlier atom stays
+        pos = pos[keep]
+    assert len(pos) == n, "random_gas: density too high for dmin"
+    types = rng.integers(0, n_species, n).astype(np.int32)
+    return np.ascontiguousarray(pos), types, box
+
+
 def make_config(k, **over):
     """Build BASELINE.json config k (1..5).  Size overrides (n_mol, L, ncell, n_slots, ...) give the reduced
     variants the CPU tests use.  Returns a dict: pos, types, box, n_local, n_ghost, ghost_owner, model."""

@@ -60,7 +60,7 @@ def _oracle_eval(c, blob, fold=True):
                           c.get("ghost_owner") if fold else None)
 
 
-def _check(c, e, f, w, ref, label=""):
+def _check(c, e, f, w, ref, label="", e_rel=0.0):
     nl = max(c["n_local"], 1)
     de = abs(e - ref["energy"]) / nl
     fr = ref["forces"]
@@ -73,7 +73,7 @@ def _check(c, e, f, w, ref, label=""):
            f"max_dF/rms={dmax / max(rms, 1e-300):.3e} rel_dW={dw / max(wn, 1e-300):.3e}")
     print(msg)
     assert np.isfinite(e) and np.isfinite(f).all() and np.isfinite(w).all(), msg
-    assert de <= _e_tol(rms, nl), msg
+    assert de <= max(_e_tol(rms, nl), e_rel * abs(ref["energy"]) / nl), msg
     if rms > 0:
         assert drms <= F_RMS_TOL * rms, msg
         assert dmax <= F_MAX_TOL * rms, msg
@@ -216,6 +216,38 @@ def test_edge_cases():
     ref = oracle.compute(blob, pos, types, np.array(box))
     c = dict(n_local=2)
     _check(c, float(e[0]), f.cpu().numpy(), w.cpu().numpy(), ref, "dimer")
+
+
+# row-length stress of the F = 128 tensor-core path (the reduced configs all have 28 or ~52 neighbours per atom):
+# (n, box, dmin, empty_frac, edge_capacity) -> isolated atoms and empty rows; rows of > 100 neighbours with more than
+# 64 N edges (regrow of the edge buffers); half-empty non-cubic box; sizes below one 16-atom work unit
+STRESS = {
+    "dilute": (1500, (48.0, 52.0, 56.0), 1.0, 0.0, None),            # ~ 5 neighbours, many atoms with none
+    "dense": (1200, (21.0, 22.0, 23.0), 1.1, 0.0, None),             # ~ 59 neighbours
+    "very_dense": (900, (14.0, 15.0, 16.0), 0.9, 0.0, 20000),        # ~ 140 neighbours, starts far too small: regrow
+    "half_empty": (1000, (20.0, 20.0, 42.0), 1.2, 0.5, None),
+    "single_atom": (1, (20.0, 20.0, 20.0), 1.0, 0.0, None),
+    "seventeen": (17, (11.0, 12.0, 13.0), 1.5, 0.0, None),
+}
+
+
+@pytest.mark.parametrize("name", list(STRESS))
+def test_row_length_stress_tensor_core_path(name):
+    n, box, dmin, empty, ecap = STRESS[name]
+    pos, types, box = gen.random_gas(n, box, dmin, seed=len(name) + n, n_species=3, empty_frac=empty)
+    model = dict(n_species=3, F=128, K=20, T=3, rc=5.0, wseed=77)
+    blob = _blob(model)
+    c = dict(pos=pos, types=types, box=box, n_local=n, n_ghost=0, model=model)
+    m, e, f, w = _gpu_eval(c, blob, edge_capacity=ecap)
+    ne = _same_edges(m, c)
+    ref = _oracle_eval(c, blob)
+    assert ref["n_edges"] == ne
+    if ecap:
+        assert m.stats()["n_regrow"] >= 1 and ne > ecap
+    # at 140 neighbours per atom the un-normalised model explodes (|E| / atom = 4e6, F_rms = 2.6e9): there the absolute
+    # energy tolerance means nothing; measured: relative energy error 1.0e-5 beside a relative force error of 1.9e-5
+    # (= 3.2 sigma of the fp32-geometry floor of DESIGN.md B1), bound used: 3e-5 relative
+    _check(c, e, f, w, ref, f"stress {name} (N={n}, E={ne}, {ne / n:.1f} neighbours per atom)", e_rel=3e-5)
 
 
 def test_error_codes():
