@@ -454,6 +454,12 @@ __attribute__((visibility("default"))) int mlp_set_option(mlp_model* m, const ch
     if (!strcmp(name, "gemm_fwd_exact")) { painn::g_gemm_fwd_exact = (int)value; return MLP_OK; }
     if (!strcmp(name, "filter_emulate")) { painn::g_filter_emulate = (int)value; return MLP_OK; }
     if (!strcmp(name, "gather_emulate")) { painn::g_gather_emulate = (int)value; return MLP_OK; }
+    if (!strcmp(name, "atoms_per_unit")) {
+        if (value < 0 || value > 31) return fail(m, MLP_ERR_ARG, "atoms_per_unit must be 1..31 (one row pointer per lane) or 0");
+        painn::g_atoms_per_unit = value ? (int)value : 16;
+        painn::g_atoms_per_unit_fwd = value ? (int)value : 12;
+        return MLP_OK;
+    }
     if (!strcmp(name, "edge_capacity")) {
         if (value <= 0) return fail(m, MLP_ERR_ARG, "edge_capacity must be > 0");
         // shrink-or-set (test hook): drop the edge buffers and reallocate at the requested size

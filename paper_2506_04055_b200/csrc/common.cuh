@@ -64,6 +64,7 @@ void gemm_unregister_exact(const float* Wdev);
 bool gemm_nt_exact(const Launch& L, const float* A, int lda, const float* W, float* C, int ldc, long long M, int N, int K,
                    const float* bias, bool accumulate, bool act_a);
 extern int g_filter_emulate, g_gather_emulate;   // debug knobs, see painn_fwd.cu
+extern int g_atoms_per_unit, g_atoms_per_unit_fwd;   // work-unit sizes of the gen-3 edge kernels (1..31), see edge_v3.cu
 // ---- dense node GEMM (gemm.cu):  C[M x N] (+)= A[M x K] . B[N x K]^T + bias ----
 void gemm_nt(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
              int N, int K, const float* bias, bool accumulate);

@@ -28,6 +28,11 @@ namespace painn {
 
 #define KLAUNCH(L) (++*(L).counter)
 
+// consecutive cell-sorted atoms per work unit (mlp_set_option "atoms_per_unit" sets both, 1..31: one row pointer per lane).
+// Sweep at config 5 (profiles/r01_microbench.md): the adjoint kernels are flat from 6 to 31, the forward kernel is 3-4 %
+// faster at 10-12 than at 16 and 3 % slower at 28-31.
+int g_atoms_per_unit = 16, g_atoms_per_unit_fwd = 12;
+
 namespace ev3 {
 
 using namespace tc;
@@ -1498,7 +1503,7 @@ bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
         attr = true;
     }
     FwdParams p{N, row_ptr, ej, s, v, (const float4*)Q4, Q1, (const float2*)Q4, (const uint4*)A_img, (const uint4*)A_rows, sn, v1,
-                1.0f / rc, K, 16, types_s, (const float2*)tab, n_tab};
+                1.0f / rc, K, g_atoms_per_unit_fwd, types_s, (const float2*)tab, n_tab};
     const long long n_units = (N + p.atoms_per_unit - 1) / p.atoms_per_unit;
     if (grouped && A_rows) {
         // one CTA per SM, two 8-warp pipelines sharing the TMEM-resident filter operand
@@ -1529,7 +1534,7 @@ bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
         attr = true;
     }
     BwdParams p{N, row_ptr, ej, (const float4*)Gb, phi, v_in, v1b, (const uint4*)A_img, (const uint4*)A_rows, phib, vb_out, G,
-                1.0f / rc, K, 16, first ? 1 : 0};
+                1.0f / rc, K, g_atoms_per_unit, first ? 1 : 0};
     const long long n_units = (N + p.atoms_per_unit - 1) / p.atoms_per_unit;
     const int grid = (int)std::min<long long>((n_units + 1) / 2, (long long)sm_count());
     if (layer0) k_msg_bwd<true><<<grid, BWD_THREADS, bwd_smem_bytes(2), L.stream>>>(p);
@@ -1549,7 +1554,7 @@ bool message_bwd0_v3(const Launch& L, long long N, int K, float rc, const int* r
         if (cudaFuncSetAttribute(k_msg_bwd0, cudaFuncAttributeMaxDynamicSharedMemorySize, bwd0_smem_bytes()) != cudaSuccess) return false;
         attr = true;
     }
-    Bwd0Params p{N, row_ptr, ej, (const float4*)Gb, types_s, (const float2*)tab, rev, (const uint4*)A_img, G, 1.0f / rc, K, 16,
+    Bwd0Params p{N, row_ptr, ej, (const float4*)Gb, types_s, (const float2*)tab, rev, (const uint4*)A_img, G, 1.0f / rc, K, g_atoms_per_unit,
                  first ? 1 : 0, n_tab};
     const long long n_units = (N + p.atoms_per_unit - 1) / p.atoms_per_unit;
     const int grid = (int)std::min<long long>((n_units + 1) / 2, (long long)sm_count());

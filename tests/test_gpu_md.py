@@ -25,7 +25,7 @@ def test_paper_shapes_four_layers(F):
 
 
 @pytest.mark.parametrize("opts", [dict(edge_path=1), dict(edge_path=2), dict(gemm_fwd_exact=0), dict(gemm_bwd_exact=1),
-                                  dict(l0_collapse=0), dict(fwd_groups=0)])
+                                  dict(l0_collapse=0), dict(fwd_groups=0), dict(atoms_per_unit=5), dict(atoms_per_unit=31)])
 def test_alternative_kernel_paths_match_oracle(opts):
     """Every switch of mlp_set_option selects another implementation of the same arithmetic; each must meet the same
     tolerances (the plain fp32 edge kernels, the first-generation tensor-core edge kernels, the fp32 FFMA forward GEMM, the
@@ -42,6 +42,7 @@ def test_alternative_kernel_paths_match_oracle(opts):
         torch.cuda.synchronize()
         e, f, w = float(e[0]), f.cpu().numpy(), w.cpu().numpy()
         m.set_option("gemm_bwd_exact", 0)
+        m.set_option("atoms_per_unit", 0)                  # process-wide knobs: back to the defaults
     ref = _oracle_eval(c, blob)
     _check(c, e, f, w, ref, f"config 5 recipe reduced, options {opts}")
 
