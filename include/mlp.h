@@ -144,6 +144,8 @@ int mlp_get_stage_ms(mlp_model* m, int max_stages, const char** names, float* ms
  *   "gemm_fwd_exact"  1 forward GEMMs on tcgen05 with exact integer slices, 0 fp32 FFMA kernel
  *   "gemm_bwd_exact"  0 adjoint GEMMs 3xTF32, 1 exact integer slices
  *   "gemm_fwd_tc"     1 forward GEMMs 3xTF32 (biased energy, B3)
+ *   "cell_strip"      order of the cells (hence of the sorted atoms): y cut into strips of this many cells, inside a strip
+ *                     (z, y, x); default 6, 0 = plain (z, y, x).  Keeps three z planes of gathered rows inside L2
  *   "atoms_per_unit"  1..31 consecutive cell-sorted atoms per work unit of the tensor-core edge kernels (default 12 forward,
  *                     16 adjoint; setting it sets both, 0 restores the defaults)
  *   "gemm_emulate", "filter_emulate", "gather_emulate", "gemm_path"  operand-precision emulation (measurements of section 5)

@@ -43,6 +43,7 @@ struct mlp_model {
     void* filt_img[PAINN_MAX_T] = {};
     void* filt_rows[PAINN_MAX_T] = {};  // same numbers as plain rows [3][F][96] fp16 (TMEM-resident A operand)
     void* filt_img2[PAINN_MAX_T] = {};  // unscaled hi | lo image (edge_tc2.cu)   // tcgen05 A-operand image of (Wf | bf), fp16 hi/lo split (edge_tc.cu)
+    int cell_strip = 6;                 // y-strip width of the cell order in cells (0: plain z, y, x order)
     int edge_path = 0;                  // 0: tensor-core edge kernels when F == 128, 1: plain fp32 kernels
     float* tab0 = nullptr;              // [n_species][F] float2 (phi^s, phi^vs) of layer 0: s^0 = Emb[z] depends on the species only
     float *Wl0s = nullptr, *Wl0v = nullptr;   // [np0][F]: layer-0 adjoint with the channels contracted first (edge_l0.cu)
@@ -446,6 +447,11 @@ __attribute__((visibility("default"))) int mlp_set_option(mlp_model* m, const ch
     if (!strcmp(name, "stage_timing")) { m->timing = value != 0; return MLP_OK; }
     if (!strcmp(name, "gemm_emulate")) { painn::g_gemm_emulate = (int)value; return MLP_OK; }
     if (!strcmp(name, "edge_path")) { m->edge_path = (int)value; return MLP_OK; }
+    if (!strcmp(name, "cell_strip")) {
+        if (value < 0) return fail(m, MLP_ERR_ARG, "cell_strip must be >= 0");
+        m->cell_strip = (int)value;
+        return MLP_OK;
+    }
     if (!strcmp(name, "l0_collapse")) { m->l0_collapse = (int)value; return MLP_OK; }
     if (!strcmp(name, "fwd_groups")) { m->fwd_groups = (int)value; return MLP_OK; }
     if (!strcmp(name, "gemm_fwd_tc")) { m->fwd_tc = value != 0; return MLP_OK; }
@@ -570,6 +576,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         int r = alloc_cells(m, ncells + ncells / 2);
         if (r != MLP_OK) return r;
     }
+    g.strip = m->cell_strip > 0 && m->cell_strip < g.n[1] ? m->cell_strip : std::max(g.n[1], 1);
     m->grid_last = g;
     int* cell_count = P<int>(m->b_cell_count);
     int* cell_start = P<int>(m->b_cell_start);

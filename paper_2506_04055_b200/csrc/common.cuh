@@ -19,7 +19,26 @@ struct Grid {
     int n[3];           // cells per dimension
     int periodic;       // 1: periodic (n_ghost == 0), 0: open boundaries
     double rc2;         // cutoff^2
+    int strip;          // cell order: y is cut into strips of this many cells; inside a strip z, y, x (x fastest).
+                        // strip >= n[1] is the plain (z, y, x) order.  DESIGN.md section 6 (L2 working set of the gathers)
 };
+
+// Linear index of cell (cx, cy, cz) and its inverse.  With strips of B cells in y the atoms of three consecutive z planes of
+// a strip are 3 n[0] B cells apart instead of 3 n[0] n[1]: the rows the edge kernels gather stay L2-resident between planes.
+__host__ __device__ __forceinline__ int cell_encode(const Grid& g, int cx, int cy, int cz) {
+    const int B = g.strip, sy = cy / B, y0 = sy * B;
+    const int w = g.n[1] - y0 < B ? g.n[1] - y0 : B;
+    return (y0 * g.n[2] + cz * w + (cy - y0)) * g.n[0] + cx;
+}
+__host__ __device__ __forceinline__ void cell_decode(const Grid& g, int cell, int (&c)[3]) {
+    const int B = g.strip, per_strip = B * g.n[2] * g.n[0];
+    const int sy = cell / per_strip, y0 = sy * B;
+    const int w = g.n[1] - y0 < B ? g.n[1] - y0 : B;
+    int rem = cell - sy * per_strip;
+    c[0] = rem % g.n[0]; rem /= g.n[0];
+    c[1] = y0 + rem % w;
+    c[2] = rem / w;
+}
 
 // error flags written by the device (bit mask in flags[0])
 enum { FLAG_TYPE_RANGE = 1, FLAG_NONFINITE = 2, FLAG_EDGE_OVERFLOW = 4 };

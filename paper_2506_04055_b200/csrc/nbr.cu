@@ -39,7 +39,7 @@ __global__ void k_bin(const double* __restrict__ pos, const int* __restrict__ ty
         wrap[3 * i + d] = (signed char)(int)w;
         c[d] = clampi((int)floor(xw * g.inv_side[d]), 0, g.n[d] - 1);
     }
-    int cell = (c[2] * g.n[1] + c[1]) * g.n[0] + c[0];
+    int cell = cell_encode(g, c[0], c[1], c[2]);
     cell_id[i] = cell;
     atomicAdd(&cell_count[cell], 1);
     if (bad) atomicOr(flags, bad);
@@ -232,12 +232,7 @@ __device__ __forceinline__ void visit_neighbors(long long a, const Grid& g, cons
     const double xa = pos_s[3 * a], ya = pos_s[3 * a + 1], za = pos_s[3 * a + 2];
     const int wa0 = wrap_s[3 * a], wa1 = wrap_s[3 * a + 1], wa2 = wrap_s[3 * a + 2];
     int c[3];
-    {
-        int cell = cell_s[a];
-        c[0] = cell % g.n[0]; cell /= g.n[0];
-        c[1] = cell % g.n[1];
-        c[2] = cell / g.n[1];
-    }
+    cell_decode(g, cell_s[a], c);
     for (int dz = -1; dz <= 1; dz++) {
         int cz = c[2] + dz, sz = 0;
         if (cz < 0) { if (!g.periodic) continue; cz += g.n[2]; sz = -1; }
@@ -250,7 +245,7 @@ __device__ __forceinline__ void visit_neighbors(long long a, const Grid& g, cons
                 int cx = c[0] + dx, sx = 0;
                 if (cx < 0) { if (!g.periodic) continue; cx += g.n[0]; sx = -1; }
                 else if (cx >= g.n[0]) { if (!g.periodic) continue; cx -= g.n[0]; sx = 1; }
-                const int cell = (cz * g.n[1] + cy) * g.n[0] + cx;
+                const int cell = cell_encode(g, cx, cy, cz);
                 const int code = (sx + 1) * 9 + (sy + 1) * 3 + (sz + 1);
                 const int b0 = cell_start[cell], b1 = cell_start[cell + 1];
                 for (int b = b0; b < b1; b++) {

@@ -25,7 +25,7 @@ def test_paper_shapes_four_layers(F):
 
 
 @pytest.mark.parametrize("opts", [dict(edge_path=1), dict(edge_path=2), dict(gemm_fwd_exact=0), dict(gemm_bwd_exact=1),
-                                  dict(l0_collapse=0), dict(fwd_groups=0), dict(atoms_per_unit=5), dict(atoms_per_unit=31)])
+                                  dict(l0_collapse=0), dict(fwd_groups=0), dict(atoms_per_unit=5), dict(atoms_per_unit=31), dict(cell_strip=0), dict(cell_strip=1), dict(cell_strip=4)])
 def test_alternative_kernel_paths_match_oracle(opts):
     """Every switch of mlp_set_option selects another implementation of the same arithmetic; each must meet the same
     tolerances (the plain fp32 edge kernels, the first-generation tensor-core edge kernels, the fp32 FFMA forward GEMM, the
