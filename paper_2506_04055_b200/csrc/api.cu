@@ -40,16 +40,17 @@ struct mlp_model {
     float* Emb = nullptr;
     LayerW lw[PAINN_MAX_T];
     float *Wr1 = nullptr, *br1 = nullptr, *wr2 = nullptr, *br2 = nullptr, *Wr1T = nullptr;
-    void* filt_img[PAINN_MAX_T] = {};
+    GemmRegistry reg;                   // tensor-core operands of the GEMM weights (split planes, exact slices)
+    void* filt_img[PAINN_MAX_T] = {};   // tcgen05 A-operand image of (bf | Wf), four fp16 planes (edge_v3.cu), K-major shared-memory layout
     void* filt_rows[PAINN_MAX_T] = {};  // same numbers as plain rows [3][F][96] fp16 (TMEM-resident A operand)
-    void* filt_img2[PAINN_MAX_T] = {};  // unscaled hi | lo image (edge_tc2.cu)   // tcgen05 A-operand image of (Wf | bf), fp16 hi/lo split (edge_tc.cu)
     int cell_strip = 6;                 // y-strip width of the cell order in cells (0: plain z, y, x order)
     int edge_path = 0;                  // 0: tensor-core edge kernels when F == 128, 1: plain fp32 kernels
+    int apu_fwd = 12, apu_bwd = 16;     // atoms per work unit of the tensor-core edge kernels (option atoms_per_unit)
+    int gemm_fwd_exact = 1;             // forward GEMMs: 1 exact integer-slice tcgen05 kernel, 0 fp32 FFMA kernel
     float* tab0 = nullptr;              // [n_species][F] float2 (phi^s, phi^vs) of layer 0: s^0 = Emb[z] depends on the species only
     float *Wl0s = nullptr, *Wl0v = nullptr;   // [np0][F]: layer-0 adjoint with the channels contracted first (edge_l0.cu)
     float *Wl0sT = nullptr, *Wl0vT = nullptr; // [F][np0]: their transposes, the forward counterpart
     int np0 = 0;                        // columns of those GEMMs: n_species (K + 1) rounded up to 128
-    int fwd_groups = 1;                 // option: forward edge kernel as one 512-thread CTA per SM, filter chunks s, vs in TMEM (0: k_msg_fwd)
     int l0_collapse = 1;                // option: use them (0: k_msg_bwd0)
     // capacities
     long long cap_atoms = 0, cap_edges = 0, cap_cells = 0;
@@ -108,13 +109,13 @@ int fail(mlp_model* m, int code, const std::string& msg) {
 
 int ensure(mlp_model* m, Buf& b, size_t bytes, bool count_regrow = true) {
     if (bytes <= b.bytes) return MLP_OK;
+    // contents are never carried over, so the old buffer goes first (peak memory = the larger of the two, not the sum)
     if (b.p) {
-        CU(m, cudaFree(b.p));
+        cudaFree(b.p);
         m->stats.device_bytes -= (long long)b.bytes;
         b.p = nullptr;
         b.bytes = 0;
     }
-    if (bytes == 0) return MLP_OK;
     CU(m, cudaMalloc(&b.p, bytes));
     b.bytes = bytes;
     m->stats.device_bytes += (long long)bytes;
@@ -129,6 +130,13 @@ int ensure(mlp_model* m, Buf& b, size_t bytes, bool count_regrow = true) {
 
 template <class T>
 T* P(const Buf& b) { return reinterpret_cast<T*>(b.p); }
+
+void free_buf(Buf& b, mlp_model* m);
+struct TmpBuf : Buf {             // scratch of the debug exports: released on every return path
+    mlp_model* m;
+    explicit TmpBuf(mlp_model* m_) : m(m_) {}
+    ~TmpBuf() { free_buf(*this, m); }
+};
 
 int upload(mlp_model* m, const std::vector<float>& h, float** out) {
     Buf b;
@@ -155,7 +163,7 @@ int upload_gemm_weight(mlp_model* m, const std::vector<float>& w, float** out) {
     float *dh, *dl;
     if ((r = upload(m, hi, &dh)) != MLP_OK) return r;
     if ((r = upload(m, lo, &dl)) != MLP_OK) return r;
-    painn::gemm_register_split(*out, dh, dl);
+    painn::gemm_register_split(m->reg, *out, dh, dl);
     m->gemm_weights.push_back(*out);
     return MLP_OK;
 }
@@ -171,12 +179,15 @@ std::vector<float> transpose(const std::vector<float>& w, int rows, int cols) { 
     return t;
 }
 
+// The three alloc_* functions zero their capacity first and set it only when every buffer is in place: a failed
+// cudaMalloc half-way leaves capacity 0, so the next call reallocates instead of running kernels on freed pointers.
 int alloc_atoms(mlp_model* m, long long cap) {
     const size_t F = m->F, R = m->R, n = (size_t)cap;
+    m->cap_atoms = 0;
     ENS(m, m->b_cell_id, n * 4); ENS(m, m->b_wrap, n * 3); ENS(m, m->b_perm, n * 4); ENS(m, m->b_inv_perm, n * 4);
     ENS(m, m->b_pos_s, n * 24); ENS(m, m->b_types_s, n * 4); ENS(m, m->b_wrap_s, n * 3); ENS(m, m->b_cell_s, n * 4);
     ENS(m, m->b_local, n * 4); ENS(m, m->b_row_cnt, n * 4); ENS(m, m->b_row_ptr, (n + 1) * 4);
-    ENS(m, m->b_scan_tmp, (n / 4096 + 2) * 4);
+    ENS(m, m->b_scan_tmp, (std::max<size_t>(n, (size_t)m->cap_cells) / 4096 + 2) * 4);   // exclusive_scan over atoms and over cells
     for (int t = 0; t <= m->T; t++) { ENS(m, m->b_S[t], n * F * 4); ENS(m, m->b_V[t], n * 3 * F * 4); }
     for (int t = 0; t < m->T; t++) {
         ENS(m, m->b_hpre[t], n * F * 4); ENS(m, m->b_phi[t], n * 3 * F * 4); ENS(m, m->b_sn[t], n * 2 * F * 4);
@@ -196,18 +207,21 @@ int alloc_atoms(mlp_model* m, long long cap) {
 }
 int alloc_edges(mlp_model* m, long long cap) {
     const size_t n = (size_t)cap;
+    m->cap_edges = 0;
     ENS(m, m->b_ej, n * 16); ENS(m, m->b_img, n); ENS(m, m->b_rev, n * 4); ENS(m, m->b_G, n * 16);
     m->cap_edges = cap;
     return MLP_OK;
 }
 int alloc_cells(mlp_model* m, long long cap) {
     const size_t n = (size_t)cap;
+    m->cap_cells = 0;
     ENS(m, m->b_cell_count, (n + 1) * 4); ENS(m, m->b_cell_start, (n + 2) * 4); ENS(m, m->b_cell_fill, (n + 1) * 4);
+    ENS(m, m->b_scan_tmp, (std::max<size_t>(n, (size_t)m->cap_atoms) / 4096 + 2) * 4);   // the cell scan uses it too
     m->cap_cells = cap;
     return MLP_OK;
 }
 
-void free_buf(Buf& b, mlp_model* m = nullptr) {
+void free_buf(Buf& b, mlp_model* m) {
     if (b.p) cudaFree(b.p);
     if (m) m->stats.device_bytes -= (long long)b.bytes;
     b.p = nullptr;
@@ -287,7 +301,7 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
         if (rcode != MLP_OK) return;
         const std::vector<float> t = transpose(v, rows, cols);          // [cols x rows]
         rcode = upload_gemm_weight(m, t, dst);
-        if (rcode == MLP_OK) painn::gemm_register_exact(*dst, t.data(), cols, rows);
+        if (rcode == MLP_OK) painn::gemm_register_exact(m->reg, *dst, t.data(), cols, rows);
     };
     up((size_t)ns * F, &m->Emb);
     std::vector<float> Wf0_h, bf0_h;          // layer-0 filter weights (for the collapsed layer-0 adjoint)
@@ -314,12 +328,6 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
                 if (rcode == MLP_OK && cudaMemcpy(b3.p, img.data(), img.size() * 2, cudaMemcpyHostToDevice) != cudaSuccess) rcode = MLP_ERR_CUDA;
                 m->wbufs.push_back(b3);
                 m->filt_rows[t] = b3.p;
-                edge_build_filter_image2(Wf_h.data(), bf_h.data(), K, img);
-                Buf b2;
-                if (rcode == MLP_OK) rcode = ensure(m, b2, img.size() * 2);
-                if (rcode == MLP_OK && cudaMemcpy(b2.p, img.data(), img.size() * 2, cudaMemcpyHostToDevice) != cudaSuccess) rcode = MLP_ERR_CUDA;
-                m->wbufs.push_back(b2);
-                m->filt_img2[t] = b2.p;
             }
         }
         up((size_t)3 * F * K, (float**)&l.Wf); up(3 * F, (float**)&l.bf);
@@ -331,11 +339,11 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
         up((size_t)F * 2 * F, (float**)&l.Wu1, &Wu1); up(F, (float**)&l.bu1);
         up((size_t)3 * F * F, (float**)&l.Wu2, &Wu2); up(3 * F, (float**)&l.bu2);
         if (rcode == MLP_OK) {      // integer slices for the exact tensor-core path of the forward GEMMs
-            painn::gemm_register_exact(l.Wm1, Wm1.data(), F, F);
-            painn::gemm_register_exact(l.Wm2, Wm2.data(), 3 * F, F);
-            painn::gemm_register_exact(l.UV, UV.data(), 2 * F, F);
-            painn::gemm_register_exact(l.Wu1, Wu1.data(), F, 2 * F);
-            painn::gemm_register_exact(l.Wu2, Wu2.data(), 3 * F, F);
+            painn::gemm_register_exact(m->reg, l.Wm1, Wm1.data(), F, F);
+            painn::gemm_register_exact(m->reg, l.Wm2, Wm2.data(), 3 * F, F);
+            painn::gemm_register_exact(m->reg, l.UV, UV.data(), 2 * F, F);
+            painn::gemm_register_exact(m->reg, l.Wu1, Wu1.data(), F, 2 * F);
+            painn::gemm_register_exact(m->reg, l.Wu2, Wu2.data(), 3 * F, F);
         }
         upT(Wm1, F, F, (float**)&l.Wm1T);
         upT(Wm2, 3 * F, F, (float**)&l.Wm2T);
@@ -345,7 +353,7 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
     }
     std::vector<float> Wr1;
     up((size_t)R * F, &m->Wr1, &Wr1); up(R, &m->br1); up(R, &m->wr2); up(1, &m->br2);
-    if (rcode == MLP_OK) painn::gemm_register_exact(m->Wr1, Wr1.data(), R, F);
+    if (rcode == MLP_OK) painn::gemm_register_exact(m->reg, m->Wr1, Wr1.data(), R, F);
     upT(Wr1, R, F, &m->Wr1T);
     if (rcode == MLP_OK && F == 128 && m->filt_img[0] && ns <= 16) {
         // layer-0 sender rows per species: phi(Emb[z]) through the same forward GEMM path as the per-atom rows
@@ -355,12 +363,11 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
         if (rcode == MLP_OK) {
             long long cnt = 0;
             Launch L{nullptr, &cnt};
-            const int saved = painn::g_gemm_path;
-            painn::g_gemm_path = 1;
+            L.reg = &m->reg;
+            L.gemm_path = 1;                  // the same forward GEMM kernels as the per-atom rows of the other layers
             gemm_nt(L, m->Emb, F, m->lw[0].Wm1, F, P<float>(bh), F, ns, F, F, m->lw[0].bm1, false);
             silu_fwd(L, (long long)ns * F, P<float>(bh), P<float>(bh));
             gemm_nt(L, P<float>(bh), F, m->lw[0].Wm2, F, P<float>(bp), 3 * F, ns, 3 * F, F, m->lw[0].bm2, false);
-            painn::g_gemm_path = saved;
             std::vector<float> ph((size_t)ns * 3 * F), tab((size_t)ns * F * 2);
             if (cudaDeviceSynchronize() != cudaSuccess ||
                 cudaMemcpy(ph.data(), bp.p, ph.size() * 4, cudaMemcpyDeviceToHost) != cudaSuccess)
@@ -388,9 +395,9 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
                 if (rcode == MLP_OK) rcode = upload_gemm_weight(m, wv, &m->Wl0v);
                 const std::vector<float> wsT = transpose(ws, np0, F), wvT = transpose(wv, np0, F);
                 if (rcode == MLP_OK) rcode = upload_gemm_weight(m, wsT, &m->Wl0sT);
-                if (rcode == MLP_OK) painn::gemm_register_exact(m->Wl0sT, wsT.data(), F, np0);
+                if (rcode == MLP_OK) painn::gemm_register_exact(m->reg, m->Wl0sT, wsT.data(), F, np0);
                 if (rcode == MLP_OK) rcode = upload_gemm_weight(m, wvT, &m->Wl0vT);
-                if (rcode == MLP_OK) painn::gemm_register_exact(m->Wl0vT, wvT.data(), F, np0);
+                if (rcode == MLP_OK) painn::gemm_register_exact(m->reg, m->Wl0vT, wvT.data(), F, np0);
                 if (rcode == MLP_OK) m->np0 = np0;
             }
         }
@@ -419,19 +426,19 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
 
 __attribute__((visibility("default"))) void mlp_destroy(mlp_model* m) {
     if (!m) return;
-    for (const float* w : m->gemm_weights) { painn::gemm_unregister_split(w); painn::gemm_unregister_exact(w); }
-    for (Buf& b : m->wbufs) free_buf(b);
+    painn::gemm_registry_free(m->reg);
+    for (Buf& b : m->wbufs) free_buf(b, nullptr);
     Buf* bs[] = {&m->b_cell_id, &m->b_wrap, &m->b_perm, &m->b_inv_perm, &m->b_pos_s, &m->b_types_s, &m->b_wrap_s,
                  &m->b_cell_s, &m->b_local, &m->b_row_cnt, &m->b_row_ptr, &m->b_scan_tmp, &m->b_cell_count,
                  &m->b_cell_start, &m->b_cell_fill, &m->b_ej, &m->b_img, &m->b_rev, &m->b_G, &m->b_h, &m->b_rpre,
                  &m->b_rb, &m->b_eatom, &m->b_sb, &m->b_s1b, &m->b_vb, &m->b_v1b, &m->b_ab, &m->b_pqb, &m->b_gb,
                  &m->b_snb, &m->b_phib, &m->b_hb, &m->b_Q4, &m->b_Q1, &m->b_epart, &m->b_wpart, &m->b_red, &m->b_misc, &m->d_pos, &m->d_types,
                  &m->d_owner, &m->d_out};
-    for (Buf* b : bs) free_buf(*b);
-    for (int t = 0; t <= PAINN_MAX_T; t++) { free_buf(m->b_S[t]); free_buf(m->b_V[t]); }
+    for (Buf* b : bs) free_buf(*b, nullptr);
+    for (int t = 0; t <= PAINN_MAX_T; t++) { free_buf(m->b_S[t], nullptr); free_buf(m->b_V[t], nullptr); }
     for (int t = 0; t < PAINN_MAX_T; t++) {
-        free_buf(m->b_hpre[t]); free_buf(m->b_phi[t]); free_buf(m->b_sn[t]); free_buf(m->b_v1[t]);
-        free_buf(m->b_pq[t]); free_buf(m->b_zpre[t]); free_buf(m->b_a[t]);
+        free_buf(m->b_hpre[t], nullptr); free_buf(m->b_phi[t], nullptr); free_buf(m->b_sn[t], nullptr); free_buf(m->b_v1[t], nullptr);
+        free_buf(m->b_pq[t], nullptr); free_buf(m->b_zpre[t], nullptr); free_buf(m->b_a[t], nullptr);
     }
     if (m->h_misc) cudaFreeHost(m->h_misc);
     if (m->own_stream) cudaStreamDestroy(m->own_stream);
@@ -445,7 +452,6 @@ __attribute__((visibility("default"))) void mlp_destroy(mlp_model* m) {
 __attribute__((visibility("default"))) int mlp_set_option(mlp_model* m, const char* name, long long value) {
     if (!m || !name) return MLP_ERR_ARG;
     if (!strcmp(name, "stage_timing")) { m->timing = value != 0; return MLP_OK; }
-    if (!strcmp(name, "gemm_emulate")) { painn::g_gemm_emulate = (int)value; return MLP_OK; }
     if (!strcmp(name, "edge_path")) { m->edge_path = (int)value; return MLP_OK; }
     if (!strcmp(name, "cell_strip")) {
         if (value < 0) return fail(m, MLP_ERR_ARG, "cell_strip must be >= 0");
@@ -453,17 +459,13 @@ __attribute__((visibility("default"))) int mlp_set_option(mlp_model* m, const ch
         return MLP_OK;
     }
     if (!strcmp(name, "l0_collapse")) { m->l0_collapse = (int)value; return MLP_OK; }
-    if (!strcmp(name, "fwd_groups")) { m->fwd_groups = (int)value; return MLP_OK; }
     if (!strcmp(name, "gemm_fwd_tc")) { m->fwd_tc = value != 0; return MLP_OK; }
     if (!strcmp(name, "gemm_bwd_exact")) { m->bwd_exact = value != 0; return MLP_OK; }
-    if (!strcmp(name, "gemm_path")) { painn::g_gemm_path = (int)value; return MLP_OK; }
-    if (!strcmp(name, "gemm_fwd_exact")) { painn::g_gemm_fwd_exact = (int)value; return MLP_OK; }
-    if (!strcmp(name, "filter_emulate")) { painn::g_filter_emulate = (int)value; return MLP_OK; }
-    if (!strcmp(name, "gather_emulate")) { painn::g_gather_emulate = (int)value; return MLP_OK; }
+    if (!strcmp(name, "gemm_fwd_exact")) { m->gemm_fwd_exact = value != 0; return MLP_OK; }
     if (!strcmp(name, "atoms_per_unit")) {
         if (value < 0 || value > 31) return fail(m, MLP_ERR_ARG, "atoms_per_unit must be 1..31 (one row pointer per lane) or 0");
-        painn::g_atoms_per_unit = value ? (int)value : 16;
-        painn::g_atoms_per_unit_fwd = value ? (int)value : 12;
+        m->apu_bwd = value ? (int)value : 16;
+        m->apu_fwd = value ? (int)value : 12;
         return MLP_OK;
     }
     if (!strcmp(name, "edge_capacity")) {
@@ -517,6 +519,10 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
     cudaStream_t st = (cudaStream_t)cuda_stream;
     long long launches = 0;
     Launch L{st, &launches};
+    L.reg = &m->reg;
+    L.fwd_exact = m->gemm_fwd_exact;
+    L.apu_fwd = m->apu_fwd;
+    L.apu_bwd = m->apu_bwd;
     m->marks.clear();
     m->stats.n_calls++;
     const int F = m->F, K = m->K, T = m->T, R = m->R;
@@ -585,7 +591,8 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
     CU(m, cudaMemsetAsync(cell_fill, 0, (size_t)(ncells + 1) * 4, st));
 
     // ---- a0-a3 neighbour build ----
-    nbr_bin(L, pos, types, N, m->n_species, g, P<int>(m->b_cell_id), P<signed char>(m->b_wrap), cell_count, dm->flags);
+    nbr_bin(L, pos, types, N, m->n_species, g, P<int>(m->b_cell_id), P<signed char>(m->b_wrap), cell_count, dm->flags, n_local,
+            ghost_owner);
     exclusive_scan(L, cell_count, cell_start, ncells, P<int>(m->b_scan_tmp), &dm->cell_total);
     nbr_place(L, N, ncells, P<int>(m->b_cell_id), cell_start, cell_fill, P<int>(m->b_perm));
     nbr_sort_cells(L, ncells, cell_start, P<int>(m->b_perm));
@@ -600,6 +607,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
     CU(m, cudaStreamSynchronize(st));
     if (hm->flags[0] & FLAG_NONFINITE) return fail(m, MLP_ERR_NONFINITE, "non-finite (or absurdly far) position");
     if (hm->flags[0] & FLAG_TYPE_RANGE) return fail(m, MLP_ERR_TYPE_RANGE, "atom type outside 0..n_species-1");
+    if (hm->flags[0] & FLAG_OWNER_RANGE) return fail(m, MLP_ERR_ARG, "ghost_owner entry outside 0..n_local-1");
     const long long E = hm->edge_total;
     if (E >= (1ll << 31) - 64) return fail(m, MLP_ERR_NOMEM, "more than 2^31 edges");
     if (E > m->cap_edges) {
@@ -621,17 +629,19 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         Launch Ls{m->side_stream, &launches};
         CU(m, cudaEventRecord(m->ev_fork, st));
         CU(m, cudaStreamWaitEvent(m->side_stream, m->ev_fork, 0));
-        nbr_reverse(Ls, N, row_ptr, ej, P<unsigned char>(m->b_img), P<int>(m->b_G), P<int>(m->b_rev));
+        nbr_reverse(Ls, N, row_ptr, ej, P<unsigned char>(m->b_img), P<int>(m->b_G), P<int>(m->b_rev), &dm->flags[1]);
         CU(m, cudaEventRecord(m->ev_join, m->side_stream));
     }
 
     // ---- forward ----
-    // Tensor-core accumulation truncates toward zero after every MMA (measured): a relative
-    // bias of ~ -0.4 ulp per chained MMA that the energy (an absolute 1e-4/atom tolerance on E/atom ~ 40-160)
-    // cannot absorb, while forces (relative tolerance) can.  Forward GEMMs therefore default to the fp32 FFMA
-    // path (round-to-nearest), the adjoint GEMMs to tcgen05 3xTF32.
-    const int saved_path = painn::g_gemm_path;
-    if (!m->fwd_tc) painn::g_gemm_path = 1;
+    // Tensor-core accumulation truncates toward zero after every MMA (measured, B3): a relative bias of
+    // ~ -0.4 ulp per chained MMA that the energy (an absolute 1e-4/atom tolerance on E/atom ~ 40-160) cannot absorb,
+    // while forces (relative tolerance) can.  Forward GEMMs (launch context Lf) therefore run the exact integer-slice
+    // tcgen05 kernel (fp32 FFMA kernel where it does not cover the shape), the adjoint GEMMs (Lb) tcgen05 3xTF32.
+    Launch Lf = L, Lb = L;
+    Lf.gemm_path = m->fwd_tc ? 0 : 1;
+    Lb.gemm_path = m->bwd_exact ? 1 : 0;
+    const bool tc_edges = m->edge_path == 0 && F == 128 && K <= 23 && m->filt_img[0] != nullptr;
     mark(m, st, ST_FWD_NODE);
     embed(L, N, F, P<int>(m->b_types_s), m->Emb, P<float>(m->b_S[0]), P<float>(m->b_V[0]));
     float* h = P<float>(m->b_h);
@@ -642,15 +652,14 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
               *v1 = P<float>(m->b_v1[t]), *pq = P<float>(m->b_pq[t]), *zpre = P<float>(m->b_zpre[t]),
               *a = P<float>(m->b_a[t]);
         // layer 0: s^0 = Emb[z], so phi(s^0) is a per-species table (built at create); no per-atom phi-MLP, no gather rows
-        const bool l0_table = t == 0 && m->edge_path == 0 && m->tab0 && K <= 23 && m->filt_img[0] &&
-                              g_filter_emulate == 0 && g_gather_emulate == 0;
+        const bool l0_table = t == 0 && tc_edges && m->tab0;
         const bool fuse_act = !m->fwd_tc && gemm_act_supported(3 * F, F);   // SiLU applied while loading A
         if (!l0_table) {
-            gemm_nt(L, S, F, l.Wm1, F, hpre, F, N, F, F, l.bm1, false);
-            if (fuse_act) gemm_nt_act(L, hpre, F, l.Wm2, F, phi, 3 * F, N, 3 * F, F, l.bm2, false, true);
+            gemm_nt(Lf, S, F, l.Wm1, F, hpre, F, N, F, F, l.bm1, false);
+            if (fuse_act) gemm_nt_act(Lf, hpre, F, l.Wm2, F, phi, 3 * F, N, 3 * F, F, l.bm2, false, true);
             else {
                 silu_fwd(L, N * F, hpre, h);
-                gemm_nt(L, h, F, l.Wm2, F, phi, 3 * F, N, 3 * F, F, l.bm2, false);
+                gemm_nt(Lf, h, F, l.Wm2, F, phi, 3 * F, N, 3 * F, F, l.bm2, false);
             }
         }
         mark(m, st, ST_FWD_EDGE);
@@ -662,93 +671,86 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
             mark(m, st, ST_L0);
             if (message_fwd0_collapsed_accum(L, N, K, rcf, row_ptr, ej, P<int>(m->b_types_s), m->n_species, S, F, sn, 2 * F, As, Av,
                                              m->np0)) {
-                gemm_nt(L, As, m->np0, m->Wl0sT, m->np0, sn, 2 * F, N, F, m->np0, nullptr, true);
-                gemm_nt(L, Av, m->np0, m->Wl0vT, m->np0, v1, F, 3 * N, F, m->np0, nullptr, false);
+                gemm_nt(Lf, As, m->np0, m->Wl0sT, m->np0, sn, 2 * F, N, F, m->np0, nullptr, true);
+                gemm_nt(Lf, Av, m->np0, m->Wl0vT, m->np0, v1, F, 3 * N, F, m->np0, nullptr, false);
                 done = true;
             }
         }
-        if (!done && m->edge_path != 1 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
+        if (!done && tc_edges && (t > 0 || l0_table)) {
             if (!l0_table) make_gather_rows(L, N, phi, V, P<float>(m->b_Q4), P<float>(m->b_Q1), t > 0);
-            if (m->edge_path == 0 && (t > 0 || m->tab0))
-                done = message_fwd_v3(L, N, K, rcf, row_ptr, ej, S, V, P<float>(m->b_Q4), P<float>(m->b_Q1), m->filt_img[t],
-                                      m->filt_rows[t], sn, v1, t > 0, P<int>(m->b_types_s), m->tab0, m->n_species, m->fwd_groups != 0);
-            if (!done)
-                done = message_fwd_tc(L, N, K, rcf, row_ptr, ej, S, V, P<float>(m->b_Q4), P<float>(m->b_Q1), m->filt_img[t],
-                                      sn, v1, t > 0);
+            done = message_fwd_v3(L, N, K, rcf, row_ptr, ej, S, V, P<float>(m->b_Q4), P<float>(m->b_Q1), m->filt_img[t],
+                                  m->filt_rows[t], sn, v1, t > 0, P<int>(m->b_types_s), m->tab0, m->n_species);
         }
-        if (!done) message_fwd(L, N, F, K, rcf, row_ptr, ej, S, V, phi, l.Wf, l.bf, sn, v1);
+        if (!done) {
+            if (l0_table) return fail(m, MLP_ERR_CUDA, "layer-0 table path unavailable");   // (phi was not computed)
+            message_fwd(L, N, F, K, rcf, row_ptr, ej, S, V, phi, l.Wf, l.bf, sn, v1);
+        }
         mark(m, st, ST_FWD_NODE);
-        gemm_nt(L, v1, F, l.UV, F, pq, 2 * F, 3 * N, 2 * F, F, nullptr, false);
+        gemm_nt(Lf, v1, F, l.UV, F, pq, 2 * F, 3 * N, 2 * F, F, nullptr, false);
         update_mid(L, N, F, (float)m->eps, pq, sn);
-        gemm_nt(L, sn, 2 * F, l.Wu1, 2 * F, zpre, F, N, F, 2 * F, l.bu1, false);
-        if (fuse_act) gemm_nt_act(L, zpre, F, l.Wu2, F, a, 3 * F, N, 3 * F, F, l.bu2, false, true);
+        gemm_nt(Lf, sn, 2 * F, l.Wu1, 2 * F, zpre, F, N, F, 2 * F, l.bu1, false);
+        if (fuse_act) gemm_nt_act(Lf, zpre, F, l.Wu2, F, a, 3 * F, N, 3 * F, F, l.bu2, false, true);
         else {
             silu_fwd(L, N * F, zpre, h);
-            gemm_nt(L, h, F, l.Wu2, F, a, 3 * F, N, 3 * F, F, l.bu2, false);
+            gemm_nt(Lf, h, F, l.Wu2, F, a, 3 * F, N, 3 * F, F, l.bu2, false);
         }
         update_out(L, N, F, sn, v1, pq, a, P<float>(m->b_S[t + 1]), P<float>(m->b_V[t + 1]));
     }
     int n_epart = 0, n_wpart = 0;
-    gemm_nt(L, P<float>(m->b_S[T]), F, m->Wr1, F, P<float>(m->b_rpre), R, N, R, F, m->br1, false);
+    gemm_nt(Lf, P<float>(m->b_S[T]), F, m->Wr1, F, P<float>(m->b_rpre), R, N, R, F, m->br1, false);
     readout(L, N, R, P<float>(m->b_rpre), m->wr2, m->br2, P<float>(m->b_local), P<float>(m->b_rb),
             P<float>(m->b_eatom), P<double>(m->b_epart), &n_epart);
 
     // ---- backward ----
     CU(m, cudaStreamWaitEvent(st, m->ev_join, 0));          // reverse-edge index ready
-    painn::g_gemm_path = m->bwd_exact ? 1 : saved_path;
     mark(m, st, ST_BWD_NODE);
     float *sb = P<float>(m->b_sb), *s1b = P<float>(m->b_s1b), *vb = P<float>(m->b_vb), *v1b = P<float>(m->b_v1b);
-    gemm_nt(L, P<float>(m->b_rb), R, m->Wr1T, R, sb, F, N, F, R, nullptr, false);
+    gemm_nt(Lb, P<float>(m->b_rb), R, m->Wr1T, R, sb, F, N, F, R, nullptr, false);
     if (N > 0) CU(m, cudaMemsetAsync(vb, 0, (size_t)N * 3 * F * 4, st));
     for (int t = T - 1; t >= 0; t--) {
         const LayerW& l = m->lw[t];
         float *ab = P<float>(m->b_ab), *pqb = P<float>(m->b_pqb), *gb = P<float>(m->b_gb), *snb = P<float>(m->b_snb),
               *phib = P<float>(m->b_phib), *hb = P<float>(m->b_hb);
         update_bwd1(L, N, F, sb, vb, P<float>(m->b_pq[t]), P<float>(m->b_a[t]), ab, pqb);
-        gemm_nt_dsilu(L, ab, 3 * F, l.Wu2T, 3 * F, gb, F, N, F, 3 * F, P<float>(m->b_zpre[t]));
-        gemm_nt(L, gb, F, l.Wu1T, F, snb, 2 * F, N, 2 * F, F, nullptr, false);
+        gemm_nt_dsilu(Lb, ab, 3 * F, l.Wu2T, 3 * F, gb, F, N, F, 3 * F, P<float>(m->b_zpre[t]));
+        gemm_nt(Lb, gb, F, l.Wu1T, F, snb, 2 * F, N, 2 * F, F, nullptr, false);
         // vb'_1 = vb + (U^T pb + V^T qb): the GEMM takes vb as the residual of its epilogue (no copy into v1b first)
         update_bwd2(L, N, F, sb, vb, snb, P<float>(m->b_sn[t]), P<float>(m->b_pq[t]), pqb, s1b, nullptr);
-        gemm_nt_resid(L, pqb, 2 * F, l.UVT, 2 * F, v1b, F, 3 * N, F, 2 * F, vb);
+        gemm_nt_resid(Lb, pqb, 2 * F, l.UVT, 2 * F, v1b, F, 3 * N, F, 2 * F, vb);
         mark(m, st, ST_BWD_EDGE);
         bool done = false;
-        if (t == 0 && m->edge_path == 0 && m->l0_collapse && m->Wl0s && m->np0 == 128 && g_filter_emulate == 0 &&
-            g_gather_emulate == 0) {
+        const bool l0_table = t == 0 && tc_edges && m->tab0;
+        if (l0_table && m->l0_collapse && m->Wl0s && m->np0 == 128) {
             // layer 0: contract the channels per (receiver, sender species) with two GEMMs, then O(K) work per edge.
             // B -> the gather-row buffer ([3N][128] floats of its [N][128] float4), C -> the (unused at layer 0) phib buffer
             float *Bv = P<float>(m->b_Q4), *Cs = phib;
             mark(m, st, ST_L0);
-            gemm_nt(L, v1b, F, m->Wl0v, F, Bv, m->np0, 3 * N, m->np0, F, nullptr, false);
-            gemm_nt(L, s1b, F, m->Wl0s, F, Cs, m->np0, N, m->np0, F, nullptr, false);
+            gemm_nt(Lb, v1b, F, m->Wl0v, F, Bv, m->np0, 3 * N, m->np0, F, nullptr, false);
+            gemm_nt(Lb, s1b, F, m->Wl0s, F, Cs, m->np0, N, m->np0, F, nullptr, false);
             done = message_bwd0_collapsed(L, N, K, rcf, row_ptr, ej, P<int>(m->b_types_s), m->n_species, P<int>(m->b_rev), Bv,
                                           Cs, m->np0, P<float4>(m->b_G), t == T - 1);
         }
-        if (!done && m->edge_path != 1 && m->filt_img[t] && g_filter_emulate == 0 && g_gather_emulate == 0) {
+        if (!done && tc_edges) {
             make_gather_rows_bwd(L, N, s1b, v1b, P<float>(m->b_Q4));
-            if (t == 0 && m->edge_path == 0 && m->tab0 && K <= 23)
+            if (l0_table)
                 done = message_bwd0_v3(L, N, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<int>(m->b_types_s), m->tab0, m->n_species,
                                        P<int>(m->b_rev), m->filt_rows[0], P<float4>(m->b_G), t == T - 1);
-            if (!done && m->edge_path == 0)
+            if (!done)
                 done = message_bwd_v3(L, N, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<float>(m->b_phi[t]),
                                       P<float>(m->b_V[t]), v1b, m->filt_img[t], m->filt_rows[t], phib, vb, P<float4>(m->b_G), t == T - 1, t == 0);
-            if (!done && m->edge_path == 3)
-                done = message_bwd_tc2(L, N, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<float>(m->b_phi[t]),
-                                       P<float>(m->b_V[t]), v1b, m->filt_img2[t], phib, vb, P<float4>(m->b_G), t == T - 1, true);
-            if (!done)
-                done = message_bwd_tc(L, N, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<float>(m->b_phi[t]), P<float>(m->b_V[t]),
-                                      v1b, m->filt_img[t], phib, vb, P<float4>(m->b_G), t == T - 1);
         }
-        if (!done)
+        if (!done) {
+            if (l0_table) return fail(m, MLP_ERR_CUDA, "layer-0 table path unavailable");
             message_bwd(L, N, F, K, rcf, row_ptr, ej, s1b, v1b, P<float>(m->b_phi[t]), P<float>(m->b_V[t]), l.Wf, l.bf,
                         phib, vb, P<float4>(m->b_G), t == T - 1);
+        }
         mark(m, st, ST_BWD_NODE);
         if (t == 0) break;      // s^0 is the (constant) embedding: its adjoint is never used
-        gemm_nt_dsilu(L, phib, 3 * F, l.Wm2T, 3 * F, hb, F, N, F, 3 * F, P<float>(m->b_hpre[t]));
-        gemm_nt(L, hb, F, l.Wm1T, F, s1b, F, N, F, F, nullptr, true);
+        gemm_nt_dsilu(Lb, phib, 3 * F, l.Wm2T, 3 * F, hb, F, N, F, 3 * F, P<float>(m->b_hpre[t]));
+        gemm_nt(Lb, hb, F, l.Wm1T, F, s1b, F, N, F, F, nullptr, true);
         std::swap(sb, s1b);
     }
 
-    painn::g_gemm_path = saved_path;
     // ---- forces, ghost fold, virial, energy ----
     mark(m, st, ST_FORCE);
     if (N > 0) CU(m, cudaMemsetAsync(forces, 0, (size_t)N * 3 * 8, st));
@@ -800,7 +802,7 @@ __attribute__((visibility("default"))) int mlp_get_neighbors(mlp_model* m, long 
     if (!j || !image3) return fail(m, MLP_ERR_ARG, "NULL output");
     const long long E = m->E_last, N = m->N_last;
     if (E == 0) return MLP_OK;
-    Buf bi, bj, bm;
+    TmpBuf bi(m), bj(m), bm(m);
     ENS(m, bi, E * 4); ENS(m, bj, E * 4); ENS(m, bm, E * 3);
     long long launches = 0;
     Launch L{m->own_stream, &launches};
@@ -820,11 +822,10 @@ __attribute__((visibility("default"))) int mlp_get_neighbors(mlp_model* m, long 
             image3[3 * k] = him[3 * e]; image3[3 * k + 1] = him[3 * e + 1]; image3[3 * k + 2] = him[3 * e + 2];
             k++;
         }
-    free_buf(bi, m); free_buf(bj, m); free_buf(bm, m);
     return MLP_OK;
 }
 
-__attribute__((visibility("default"))) __attribute__((visibility("default"))) int mlp_debug_gemm(const float* A, const float* W, const float* bias,
+__attribute__((visibility("default"))) int mlp_debug_gemm(const float* A, const float* W, const float* bias,
                                                            float* C, long long M, int N, int K, int accumulate,
                                                            int path, int* used_tc) {
     if (!A || !W || !C || M < 0 || N <= 0 || K <= 0) return MLP_ERR_ARG;
@@ -836,23 +837,24 @@ __attribute__((visibility("default"))) __attribute__((visibility("default"))) in
     if (r == MLP_OK && bias) r = upload(m, std::vector<float>(bias, bias + N), &dB);
     if (r == MLP_OK) {
         long long launches = 0;
+        int used = 0;
         Launch L{nullptr, &launches};
-        const int saved = painn::g_gemm_path;
-        painn::g_gemm_path = path;
-        painn::g_last_gemm_tc = 0;
-        if (path == 2) {            // exact integer-slice tensor-core kernel (forward path)
-            painn::gemm_register_exact(dW, w.data(), N, K);
-            painn::g_last_gemm_tc = painn::gemm_nt_exact(L, A, K, dW, C, N, M, N, K, dB, accumulate != 0, false) ? 1 : 0;
-            if (!painn::g_last_gemm_tc) r = MLP_ERR_ARG;
+        L.reg = &m->reg;
+        L.used_tc = &used;
+        L.gemm_path = path == 0 ? 0 : 1;             // 0: 3xTF32 (adjoint path), 1: fp32 FFMA, 2: exact integer slices
+        L.fwd_exact = path == 2 ? 1 : 0;
+        if (path == 2) {
+            painn::gemm_register_exact(m->reg, dW, w.data(), N, K);
+            if (!painn::gemm_nt_exact(L, A, K, dW, C, N, M, N, K, dB, accumulate != 0, false)) r = MLP_ERR_ARG;
+            else used = 1;
         } else
             gemm_nt(L, A, K, dW, K, C, N, M, N, K, dB, accumulate != 0);
-        painn::g_gemm_path = saved;
-        if (used_tc) *used_tc = painn::g_last_gemm_tc;
+        if (used_tc) *used_tc = used;
         cudaError_t e = cudaDeviceSynchronize();
         if (e != cudaSuccess) r = MLP_ERR_CUDA;
     }
-    for (const float* x : m->gemm_weights) { painn::gemm_unregister_split(x); painn::gemm_unregister_exact(x); }
-    for (Buf& b : m->wbufs) free_buf(b);
+    painn::gemm_registry_free(m->reg);
+    for (Buf& b : m->wbufs) free_buf(b, nullptr);
     return r;
 }
 
@@ -860,7 +862,7 @@ __attribute__((visibility("default"))) int mlp_get_layer_state(mlp_model* m, int
     if (!m || !out || t < 0 || t > m->T) return MLP_ERR_ARG;
     const long long N = m->N_last;
     if (N == 0) return MLP_OK;
-    Buf b;
+    TmpBuf b(m);
     ENS(m, b, (size_t)N * 4 * m->F * 4);
     long long launches = 0;
     Launch L{m->own_stream, &launches};
@@ -868,7 +870,6 @@ __attribute__((visibility("default"))) int mlp_get_layer_state(mlp_model* m, int
     unpermute_state(L, N, m->F, P<int>(m->b_perm), P<float>(m->b_S[t]), P<float>(m->b_V[t]), P<float>(b));
     CU(m, cudaMemcpyAsync(out, b.p, (size_t)N * 4 * m->F * 4, cudaMemcpyDeviceToHost, m->own_stream));
     CU(m, cudaStreamSynchronize(m->own_stream));
-    free_buf(b, m);
     return MLP_OK;
 }
 

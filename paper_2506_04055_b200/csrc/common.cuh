@@ -3,6 +3,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <unordered_map>
+#include <utility>
 #include <vector>
 
 #define PAINN_MAX_T 8
@@ -41,21 +43,37 @@ __host__ __device__ __forceinline__ void cell_decode(const Grid& g, int cell, in
 }
 
 // error flags written by the device (bit mask in flags[0])
-enum { FLAG_TYPE_RANGE = 1, FLAG_NONFINITE = 2, FLAG_EDGE_OVERFLOW = 4 };
+enum { FLAG_TYPE_RANGE = 1, FLAG_NONFINITE = 2, FLAG_EDGE_OVERFLOW = 4, FLAG_OWNER_RANGE = 8 };
 
 struct LayerW {
     const float *Wm1, *bm1, *Wm2, *bm2, *Wf, *bf, *UV, *Wu1, *bu1, *Wu2, *bu2;   // [out x in] row-major
     const float *Wm1T, *Wm2T, *UVT, *Wu1T, *Wu2T;                                // transposes [in x out]
 };
 
-struct Launch {            // per-call launch context
+// Tensor-core operands of the GEMM weights, cut once at mlp_create and owned by the model (gemm.cu / gemm_tc.cu).
+struct ExactW {
+    int N, K;
+    void* planes;          // device [K / 128][3][N][128] integer-valued fp16 slices
+    float* cs;             // device [K / 128][N] column scales
+};
+struct GemmRegistry {
+    std::unordered_map<const float*, std::pair<const float*, const float*>> split;   // W -> (hi, lo) TF32 planes
+    std::unordered_map<const float*, ExactW> exact;                                   // W -> exact slices
+};
+
+struct Launch {            // per-call launch context: everything a kernel launcher may depend on besides its arguments
     cudaStream_t stream;
     long long* counter;    // kernels launched
+    const GemmRegistry* reg = nullptr;
+    int gemm_path = 0;     // 0: adjoint GEMMs (tcgen05 3xTF32 when the shape is covered), 1: forward GEMMs (exact accumulation)
+    int fwd_exact = 1;     // forward GEMMs: 1 exact integer-slice tcgen05 kernel when covered, 0 fp32 FFMA kernel
+    int* used_tc = nullptr;   // set to 1 when a tensor-core GEMM kernel ran (test hook of mlp_debug_gemm)
+    int apu_fwd = 12, apu_bwd = 16;   // consecutive cell-sorted atoms per work unit of the tensor-core edge kernels (1..31)
 };
 
 // ---- neighbour build (nbr.cu) ----
 void nbr_bin(const Launch& L, const double* pos, const int* types, long long N, int n_species, Grid g,
-             int* cell_id, signed char* wrap, int* cell_count, int* flags);
+             int* cell_id, signed char* wrap, int* cell_count, int* flags, long long n_local, const int* ghost_owner);
 void nbr_bbox(const Launch& L, const double* pos, long long N, double* bbox6);
 void exclusive_scan(const Launch& L, const int* in, int* out, long long n, int* block_tmp, long long* total);
 void nbr_place(const Launch& L, long long N, long long ncells, const int* cell_id, const int* cell_start,
@@ -70,20 +88,16 @@ void nbr_fill(const Launch& L, long long N, Grid g, const double* pos_s, const s
               const int* cell_s, const int* cell_start, const int* row_ptr, long long cap_edges, float rc, float4* ej,
               unsigned char* img, int* key, int* flags);
 void nbr_reverse(const Launch& L, long long N, const int* row_ptr, const float4* ej, const unsigned char* img,
-                 const int* key, int* rev);
+                 const int* key, int* rev, int* miss);
 void nbr_export(const Launch& L, long long N, const int* row_ptr, const float4* ej, const unsigned char* img,
                 const int* perm, const signed char* wrap_s, int* out_i, int* out_j, signed char* out_img);
 
-extern int g_gemm_emulate, g_gemm_path, g_last_gemm_tc, g_gemm_fwd_exact;   // debug knobs, see gemm.cu
-void gemm_register_split(const float* W, const float* hi, const float* lo);
-void gemm_unregister_split(const float* W);
+void gemm_register_split(GemmRegistry& reg, const float* W, const float* hi, const float* lo);
 // exact integer-slice tensor-core path of the forward GEMMs (gemm_tc.cu): slices of W [N x K] are cut at create
-void gemm_register_exact(const float* Wdev, const float* Whost, int N, int K);
-void gemm_unregister_exact(const float* Wdev);
+void gemm_register_exact(GemmRegistry& reg, const float* Wdev, const float* Whost, int N, int K);
+void gemm_registry_free(GemmRegistry& reg);
 bool gemm_nt_exact(const Launch& L, const float* A, int lda, const float* W, float* C, int ldc, long long M, int N, int K,
                    const float* bias, bool accumulate, bool act_a);
-extern int g_filter_emulate, g_gather_emulate;   // debug knobs, see painn_fwd.cu
-extern int g_atoms_per_unit, g_atoms_per_unit_fwd;   // work-unit sizes of the gen-3 edge kernels (1..31), see edge_v3.cu
 // ---- dense node GEMM (gemm.cu):  C[M x N] (+)= A[M x K] . B[N x K]^T + bias ----
 void gemm_nt(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
              int N, int K, const float* bias, bool accumulate);
@@ -123,25 +137,13 @@ void reduce_final(const Launch& L, const double* e_partial, int n_e, const doubl
 void unpermute_state(const Launch& L, long long N, int F, const int* perm, const float* s, const float* v,
                      float* out);
 
-// ---- tensor-core edge kernels (edge_tc.cu), F = 128 ----
+// ---- tensor-core edge kernels (edge_v3.cu), F = 128: per-edge filter on tcgen05, software-pipelined gathers ----
 void edge_build_filter_image(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img);
-size_t edge_filter_image_bytes();
 void make_gather_rows(const Launch& L, long long N, const float* phi, const float* v, float* Q4, float* Q1, bool has_v);
-bool message_fwd_tc(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* s,
-                    const float* v, const float* Q4, const float* Q1, const void* A_img, float* sn, float* v1, bool has_v);
 void make_gather_rows_bwd(const Launch& L, long long N, const float* s1b, const float* v1b, float* Gb);
-bool message_bwd_tc(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
-                    const float* phi, const float* v_in, const float* v1b, const void* A_img, float* phib, float* vb_out,
-                    float4* G, bool first);
-void edge_build_filter_image2(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img);
-bool message_bwd_tc2(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
-                     const float* phi, const float* v_in, const float* v1b, const void* A_img2, float* phib, float* vb_out,
-                     float4* G, bool first, bool need_sender);
-
-// ---- generation-3 edge kernels (edge_v3.cu), F = 128: software-pipelined gathers, shared-memory channel reduction ----
 bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* s,
                     const float* v, const float* Q4, const float* Q1, const void* A_img, const void* A_rows, float* sn, float* v1,
-                    bool has_v, const int* types_s, const float* tab, int n_tab, bool grouped);
+                    bool has_v, const int* types_s, const float* tab, int n_tab);
 bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
                     const float* phi, const float* v_in, const float* v1b, const void* A_img, const void* A_rows, float* phib,
                     float* vb_out, float4* G, bool first, bool layer0);

@@ -1,20 +1,28 @@
-// edge_v3.cu -- third-generation message / adjoint-message kernels (F = 128).
+// edge_v3.cu -- message / adjoint-message kernels of the F = 128 models.
 //
-// Same mathematics and the same tensor-core filter as edge_tc.cu (per-edge filter w_e = fc (Wf rho + bf) as a
-// tcgen05 GEMM with fp16 hi/lo split operands, accumulator D[channel, edge] in TMEM, one channel per lane, CSR
-// segment sums in registers, no atomics).  What changed comes from the ncu captures of the earlier kernels
-// (profiles/r01_edge_ncu.md): they issued 35 (forward) and 104 (adjoint) warp instructions per (edge, 32 channels),
-// sat at 36-50 % issue utilisation with "long scoreboard" as the top stall, and moved 6 TB/s of the >16 TB/s the
-// L2 -> SM path sustains for this access pattern (row gathers of 512 B per warp).  Here
-//   * the gathers are software-pipelined in two register banks of 8 edges: the loads of batch b+1 are in flight
-//     while batch b is consumed (ping-pong, statically unrolled so that ptxas keeps one scoreboard per bank);
-//   * the pipeline runs across tile and unit boundaries (consumers peek at the producers' "operand ready" barrier
-//     of the next tile to fetch its sender indices early);
+//   w_e = fc(d_e) (Wf rho(d_e) + bf)  is a [3F x (K+1)] . [(K+1) x edges] GEMM: per tile of edges the producer warps
+//   compute R_e = fc (1, rho_1..rho_K) on the fly (sincospi + rotation recurrence) and write it as the B operand into
+//   shared memory, one elected thread issues tcgen05.mma (A = (bf | Wf), resident in TMEM / shared memory, M = 128
+//   channels per chunk), and the accumulator D[channel, edge] lands in TMEM with ONE CHANNEL PER LANE.  The consumer
+//   warps read their own channel's filter values (tcgen05.ld 32x32b) and run the CSR segment sum in registers: no
+//   atomics, coalesced 512 B gathers of the sender rows.
+//
+// Precision: fp16 operands alone miss the force tolerance, so both operands are split
+// x = hi + r (hi = RN_fp16(x), r the exact remainder) and FOUR product terms are accumulated along K = 4 x 24 = 96:
+//   r(W) r(R)  +  [hi(W) 2^-6][r(R) 2^6]  +  [r(W) 2^6][hi(R) 2^-6]  +  hi(W) hi(R)
+// (split4 / filter_planes; K + 1 <= 24 basis slots per term).  The small terms come first in K and the MMAs are issued
+// in ascending K, so the fp32 accumulator (which truncates toward zero after every MMA, B3) sees only two
+// full-magnitude additions.  Round 1 used three terms with 2^+-11 scales on 32-slot terms: same MMA count, but the
+// hi 2^-11 planes were fp16 subnormals for most operands and the r r term was missing -- 3.6x the per-atom energy noise
+// of the plain fp32 kernels (B1).
+//
+// Kernel structure (from the ncu captures, profiles/r01_edge_ncu.md):
+//   * gathers are software-pipelined: two register banks of 8 edges (forward), a 16-row cp.async window per thread
+//     (adjoint); the pipeline runs across tile and unit boundaries;
 //   * rows are padded to 8 slots with zero-weight dummies, so nothing is predicated per edge: one uniform
 //     row-boundary test per 8 edges; the receiver's own rows (residual / phi_j, v_j) are loaded one row ahead;
-//   * the adjoint reduces its four per-edge scalars over the 128 channels through shared memory (one STS.128 per
-//     (edge, channel), 8 LDS.128 + a 16-lane shuffle tree per thread and 8 edges) instead of a 31-shuffle butterfly
-//     plus a finisher warp, and layer 0 (v = 0, embedding constant) runs a 2-chunk variant without sender adjoint.
+//   * the adjoint reduces its per-edge sums over the 128 channels through shared-memory planes and a reducer warp;
+//   * one 512-thread CTA per SM = two independent 8-warp pipelines sharing one copy of the filter operand.
 #include <cuda_fp16.h>
 
 #include <algorithm>
@@ -28,17 +36,12 @@ namespace painn {
 
 #define KLAUNCH(L) (++*(L).counter)
 
-// consecutive cell-sorted atoms per work unit (mlp_set_option "atoms_per_unit" sets both, 1..31: one row pointer per lane).
-// Sweep at config 5 (profiles/r01_microbench.md): the adjoint kernels are flat from 6 to 31, the forward kernel is 3-4 %
-// faster at 10-12 than at 16 and 3 % slower at 28-31.
-int g_atoms_per_unit = 16, g_atoms_per_unit_fwd = 12;
-
 namespace ev3 {
 
 using namespace tc;
 
 constexpr int F = 128;
-constexpr int KP = 96;                        // 3 split terms x 32 basis slots (same A image as edge_tc.cu)
+constexpr int KP = 96;                        // 4 split terms x 24 basis slots
 constexpr int LBO = 128, SBO = (KP / 8) * 128;          // 1536
 constexpr int A_CHUNK_BYTES = (F / 8) * SBO;            // 24576
 
@@ -69,27 +72,37 @@ __device__ __forceinline__ EdgeGeom edge_geom(const float4 raw, int E, int e_end
     sincospif(g.x, &g.s1, &g.c1);
     return g;
 }
-// split 8 fp32 values into the three fp16 planes of the B operand: hi, lo * 2^11, hi * 2^-11
-// (packed conversions: one F2FP per pair; the 2^-11 plane is an exact exponent shift done in half2)
-__device__ __forceinline__ void split3(const float (&v)[8], uint4& p0, uint4& p1, uint4& p2) {
-    __half2 a[4], b[4], c[4];
-    const __half2 k = __floats2half2_rn(1.0f / 2048.0f, 1.0f / 2048.0f);
+// Split 8 fp32 values x = hi + r (hi = RN_fp16(x), r exact in fp32) into the four fp16 planes of the B operand, one per
+// product term of (A_hi + A_lo)(B_hi + B_lo) (edge_build_filter_rows holds the matching A planes):
+//   term 0 (ll): r            term 1 (hl): r * 2^6  (against A_hi * 2^-6)
+//   term 2 (lh): hi * 2^-6    (against A_lo * 2^6)             term 3 (hh): hi
+// The 2^+-6 scales keep both factors of the cross terms inside fp16's normal range for the magnitudes that occur
+// (|R| ~ 1e-3 .. 1, |W| ~ 1e-3 .. 2): with the earlier 2^+-11 scales hi * 2^-11 was a subnormal for |R| < 0.125 and the
+// cross term lost most of its bits (B1).  What falls below the normal range only costs 2^-25 absolute times
+// the other factor.  Packed conversions: one F2FP per pair; the 2^-6 plane is an exact exponent shift done in half2.
+__device__ __forceinline__ void split4(const float (&v)[8], uint4& p_ll, uint4& p_hl, uint4& p_lh, uint4& p_hh) {
+    __half2 a[4], b[4], c[4], d[4];
+    const __half2 k = __floats2half2_rn(1.0f / 64.0f, 1.0f / 64.0f);
 #pragma unroll
     for (int i = 0; i < 4; i++) {
         a[i] = __floats2half2_rn(v[2 * i], v[2 * i + 1]);
         const float2 f = __half22float2(a[i]);
-        b[i] = __floats2half2_rn((v[2 * i] - f.x) * 2048.0f, (v[2 * i + 1] - f.y) * 2048.0f);
+        const float r0 = v[2 * i] - f.x, r1 = v[2 * i + 1] - f.y;
+        b[i] = __floats2half2_rn(r0 * 64.0f, r1 * 64.0f);
         c[i] = __hmul2(a[i], k);
+        d[i] = __floats2half2_rn(r0, r1);
     }
-    p0 = *(uint4*)a; p1 = *(uint4*)b; p2 = *(uint4*)c;
+    p_hh = *(uint4*)a; p_hl = *(uint4*)b; p_lh = *(uint4*)c; p_ll = *(uint4*)d;
 }
+// byte offset of the 8-slot group h (basis slots 8h .. 8h+7) of product term t inside a B (or A) row block: K index
+// 24 t + 8 h + i, 12 groups of 8 = 96 = KP
+__device__ __forceinline__ int kgrp_off(int t, int h) { return (3 * t + h) * 128; }
 
 // =============================================================================================================
 // forward message pass
 // =============================================================================================================
 constexpr int NE = 32;                                  // edges per tile (MMA N)
 constexpr int B_BYTES = (NE / 8) * SBO;                 // 6144
-constexpr int FWD_THREADS = 256;
 
 struct FwdParams {
     long long N;
@@ -115,270 +128,6 @@ struct FwdParams {
 };
 
 constexpr int TAB_MAX = 16;                             // species rows the shared-memory table can hold
-constexpr int fwd_smem_bytes(bool has_v) {
-    return (has_v ? 3 : 2) * A_CHUNK_BYTES + 2 * B_BYTES + 2 * NE * 16 + 64 + 128 + (has_v ? 0 : TAB_MAX * F * 8);
-}
-
-template <bool HAS_V>
-__global__ void __launch_bounds__(FWD_THREADS, 2) k_msg_fwd(const FwdParams p) {
-    constexpr int NCH = HAS_V ? 3 : 2;
-    constexpr int TCOLS = NCH * NE;                 // TMEM columns per buffer
-    constexpr int TALLOC = HAS_V ? 256 : 128;
-    extern __shared__ __align__(128) uint8_t smem[];
-    uint8_t* sA = smem;
-    uint8_t* sB = sA + NCH * A_CHUNK_BYTES;
-    float4* sMeta = (float4*)(sB + 2 * B_BYTES);   // [2][NE] (u_e, sender index)
-    uint64_t* bars = (uint64_t*)(sMeta + 2 * NE);
-    uint64_t* b_full = bars;          // [2] producers -> MMA (and consumers: sender indices readable)  (count 96)
-    uint64_t* t_full = bars + 2;      // [2] MMA commit -> consumers (count 1)
-    uint32_t* tmem_slot = (uint32_t*)(bars + 6);       // (consumers -> producers: named barriers 1, 2)
-    float2* sTab = (float2*)(bars + 8);                // [n_tab][F] species table (layer 0 only)
-
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    {
-        const uint4* src = p.A_img;
-        uint4* dst = (uint4*)sA;
-        for (int i = tid; i < NCH * A_CHUNK_BYTES / 16; i += FWD_THREADS) dst[i] = src[i];
-        uint4* zb = (uint4*)sB;
-        for (int i = tid; i < 2 * B_BYTES / 16; i += FWD_THREADS) zb[i] = make_uint4(0, 0, 0, 0);
-        if (!HAS_V)
-            for (int i = tid; i < p.n_tab * F; i += FWD_THREADS) sTab[i] = p.tab[i];
-    }
-    if (tid == 0) {
-        for (int b = 0; b < 2; b++) { mbar_init(&b_full[b], 96); mbar_init(&t_full[b], 1); }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    if (warp == 7) tmem_alloc(tmem_slot, TALLOC);
-    fence_async_smem();
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
-    const uint32_t tmem_base = *tmem_slot;
-
-    const long long N = p.N;
-    const int apu = p.atoms_per_unit;
-    const int* __restrict__ row_ptr = p.row_ptr;
-    const long long n_units = (N + apu - 1) / apu;
-    if (warp < 4) reg_inc<168>(); else reg_dec<88>();
-
-    if (warp < 4) {
-        // ===================== consumers: one channel per thread =====================
-        const int f = tid;
-        const float4* __restrict__ Q4 = p.Q4 + f;
-        const float* __restrict__ Q1 = p.Q1 + f;
-        const float2* __restrict__ Q2 = p.Q2 + f;
-        const float* __restrict__ s_in = p.s + f;
-        const float* __restrict__ v_in = p.v + f;
-        float* __restrict__ sn = p.sn + f;
-        float* __restrict__ v1 = p.v1 + f;
-        const uint32_t lane_base = tmem_base + ((uint32_t)(warp * 32) << 16);
-        float4 qa4[8], qb4[8];
-        float qa1[8], qb1[8];
-        float2 qa2[8], qb2[8];
-#define FWD_ISSUE(Q4R, Q1R, Q2R, META8)                                                   \
-    {                                                                                     \
-        _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                \
-            const size_t row_ = (size_t)__float_as_int((META8)[i_].w) * F;                \
-            if (HAS_V) { Q4R[i_] = __ldg(Q4 + row_); Q1R[i_] = __ldg(Q1 + row_); }        \
-        }                                                                                 \
-    }
-        uint32_t it = 0;
-        bool pre = false;                 // first batch of tile `it` already in flight (bank a)
-        for (long long u = blockIdx.x; u < n_units; u += gridDim.x) {
-            const long long a0 = u * apu;
-            const int na = (int)min((long long)apu, N - a0);
-            const int rp = __ldg(row_ptr + a0 + min(lane, na));           // lanes 0..na hold the unit's row pointers
-            const int e_begin = __shfl_sync(0xffffffffu, rp, 0), e_end = __shfl_sync(0xffffffffu, rp, na);
-            const int ntiles = (e_end - e_begin + NE - 1) / NE;
-            bool next_has = false;                                        // does the CTA's next unit have a tile?
-            {
-                const long long un = u + gridDim.x;
-                if (un < n_units) {
-                    const long long b0 = un * apu, b1 = min(N, b0 + apu);
-                    next_has = __ldg(row_ptr + b1) > __ldg(row_ptr + b0);
-                }
-            }
-            if (HAS_V && ntiles > 0 && !pre) {
-                mbar_wait(&b_full[it & 1], (it >> 1) & 1);
-                const float4* m0 = sMeta + (it & 1) * NE;
-                FWD_ISSUE(qa4, qa1, qa2, m0);
-            }
-            pre = false;
-            int a_rel = 0;
-            int row_end = __shfl_sync(0xffffffffu, rp, 1);
-            float accS = 0.f, acc0 = 0.f, acc1 = 0.f, acc2 = 0.f;
-            // residual (s_i, v_i) of the current receiver: loaded at row start, added at row end
-            float rs = s_in[(a0 + a_rel) * F], rv0 = 0.f, rv1 = 0.f, rv2 = 0.f;
-            if (HAS_V) { rv0 = v_in[(a0 + a_rel) * 3 * F]; rv1 = v_in[(a0 + a_rel) * 3 * F + F]; rv2 = v_in[(a0 + a_rel) * 3 * F + 2 * F]; }
-            auto store_row = [&]() {
-                const long long a = a0 + a_rel;
-                sn[a * 2 * F] = accS + rs;
-                v1[a * 3 * F] = acc0 + rv0; v1[a * 3 * F + F] = acc1 + rv1; v1[a * 3 * F + 2 * F] = acc2 + rv2;
-            };
-            auto next_row = [&]() {
-                store_row();
-                a_rel++;
-                row_end = __shfl_sync(0xffffffffu, rp, a_rel + 1);
-                accS = acc0 = acc1 = acc2 = 0.f;
-                const long long a = a0 + a_rel;
-                rs = s_in[a * F];
-                if (HAS_V) { rv0 = v_in[a * 3 * F]; rv1 = v_in[a * 3 * F + F]; rv2 = v_in[a * 3 * F + 2 * F]; }
-            };
-#define FWD_COMPUTE(BI, Q4R, Q1R, Q2R)                                                                      \
-    {                                                                                                       \
-        const int E8_ = e_begin + t * NE + (BI) * 8;                                                        \
-        if (E8_ < e_end) {                                                                                  \
-            while (E8_ >= row_end) next_row();                                                              \
-            uint32_t ws[8], wvs[8], wvv[8];                                                                 \
-            tmem_ld8_nowait(lane_base + buf * TCOLS + (BI) * 8, ws);                                        \
-            tmem_ld8_nowait(lane_base + buf * TCOLS + NE + (BI) * 8, wvs);                                  \
-            if (HAS_V) tmem_ld8_nowait(lane_base + buf * TCOLS + 2 * NE + (BI) * 8, wvv);                   \
-            tmem_wait_ld();                                                                                 \
-            _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                              \
-                const float4 m_ = meta[(BI) * 8 + i_];                                                      \
-                const float w_s = __uint_as_float(ws[i_]), w_vs = __uint_as_float(wvs[i_]);                 \
-                if (HAS_V) {                                                                                \
-                    const float w_vv = __uint_as_float(wvv[i_]);                                            \
-                    accS = fmaf(w_s, Q4R[i_].x, accS);                                                      \
-                    const float tv = w_vs * Q4R[i_].y;                                                      \
-                    acc0 = fmaf(tv, m_.x, fmaf(w_vv, Q4R[i_].z, acc0));                                     \
-                    acc1 = fmaf(tv, m_.y, fmaf(w_vv, Q4R[i_].w, acc1));                                     \
-                    acc2 = fmaf(tv, m_.z, fmaf(w_vv, Q1R[i_], acc2));                                       \
-                } else {                                                                                    \
-                    const float2 q_ = sTab[__float_as_int(m_.w) * F + f];       /* species row of the sender */ \
-                    accS = fmaf(w_s, q_.x, accS);                                                           \
-                    const float tv = w_vs * q_.y;                                                           \
-                    acc0 = fmaf(tv, m_.x, acc0);                                                            \
-                    acc1 = fmaf(tv, m_.y, acc1);                                                            \
-                    acc2 = fmaf(tv, m_.z, acc2);                                                            \
-                }                                                                                           \
-            }                                                                                               \
-        }                                                                                                   \
-    }
-            for (int t = 0; t < ntiles; t++, it++) {
-                const int buf = it & 1;
-                const float4* meta = sMeta + buf * NE;
-                FWD_ISSUE(qb4, qb1, qb2, meta + 8);
-                mbar_wait(&t_full[buf], (it >> 1) & 1);
-                tc_fence_after();
-                FWD_COMPUTE(0, qa4, qa1, qa2);
-                FWD_ISSUE(qa4, qa1, qa2, meta + 16);
-                FWD_COMPUTE(1, qb4, qb1, qb2);
-                FWD_ISSUE(qb4, qb1, qb2, meta + 24);
-                FWD_COMPUTE(2, qa4, qa1, qa2);
-                if (HAS_V && (t + 1 < ntiles || next_has)) {       // first batch of the CTA's next tile
-                    mbar_wait(&b_full[buf ^ 1], ((it + 1) >> 1) & 1);
-                    const float4* mn = sMeta + (buf ^ 1) * NE;
-                    FWD_ISSUE(qa4, qa1, qa2, mn);
-                    pre = t + 1 == ntiles;
-                }
-                FWD_COMPUTE(3, qb4, qb1, qb2);
-                tc_fence_before();
-                bar_arrive(1 + buf, 224);              // tile consumed: 128 consumers arrive, 96 producers wait (named barrier)
-            }
-            // finish the last receiver with edges, then pass trailing edge-less atoms through (s' = s, v' = v)
-            for (;;) {
-                store_row();
-                if (a_rel + 1 >= na) break;
-                a_rel++;
-                accS = acc0 = acc1 = acc2 = 0.f;
-                const long long a = a0 + a_rel;
-                rs = s_in[a * F];
-                if (HAS_V) { rv0 = v_in[a * 3 * F]; rv1 = v_in[a * 3 * F + F]; rv2 = v_in[a * 3 * F + 2 * F]; }
-            }
-        }
-#undef FWD_ISSUE
-#undef FWD_COMPUTE
-    } else if (warp < 7) {
-        // ===================== producers: B operand R_e = fc (1, rho_1 .. rho_K), three fp16 planes =====================
-        const int pt = tid - 128, e = pt & 31, h = pt >> 5;   // h: basis slots 8h .. 8h+7 (slot 0 = bias, slot n = rho_n)
-        const float inv_rc = p.inv_rc;
-        const int K = p.K;
-        uint32_t it = 0;
-        for (long long u = blockIdx.x; u < n_units; u += gridDim.x) {
-            const long long a0 = u * apu;
-            const long long a1 = min(N, a0 + (long long)apu);
-            const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
-            const int ntiles = (e_end - e_begin + NE - 1) / NE;
-            float4 raw_n = load_edge_raw(p.ej, e_begin + e, e_end);
-            for (int t = 0; t < ntiles; t++, it++) {
-                const int buf = it & 1;
-                const float4 raw = raw_n;
-                if (t + 1 < ntiles) raw_n = load_edge_raw(p.ej, e_begin + (t + 1) * NE + e, e_end);
-                const EdgeGeom g = edge_geom(raw, e_begin + t * NE + e, e_end, inv_rc);
-                const float fc = g.real ? 0.5f * (1.0f + g.c1) : 0.0f;
-                const float amp = fc * g.inv_d;
-                float sn_, cn_;
-                if (h == 0) { sn_ = g.s1; cn_ = g.c1; } else sincospif((float)(8 * h) * g.x, &sn_, &cn_);
-                float vals[8];
-#pragma unroll
-                for (int i = 0; i < 8; i++) {
-                    const int b = h * 8 + i;
-                    float R;
-                    if (b == 0) R = fc;
-                    else {
-                        R = b <= K ? amp * sn_ : 0.0f;
-                        const float tt = sn_ * g.c1 + cn_ * g.s1;
-                        cn_ = cn_ * g.c1 - sn_ * g.s1;
-                        sn_ = tt;
-                    }
-                    vals[i] = R;
-                }
-                uint4 p0, p1, p2;
-                split3(vals, p0, p1, p2);
-                if (it >= 2) bar_sync(1 + buf, 224);   // tile it - 2 consumed (hardware-blocking wait, no spin)
-                uint8_t* bb = sB + buf * B_BYTES + (e >> 3) * SBO + (e & 7) * 16 + h * LBO;
-                *(uint4*)(bb) = p0;                       // term 0: k = b
-                *(uint4*)(bb + 4 * LBO) = p1;             // term 1: k = 32 + b   (lo(R) 2^11)
-                *(uint4*)(bb + 8 * LBO) = p2;             // term 2: k = 64 + b   (hi(R) 2^-11)
-                if (h == 0) {
-                    float mw = g.r.w;                                             // sender index ...
-                    if (!HAS_V) mw = __int_as_float(__ldg(p.types + __float_as_int(g.r.w)));   // ... or its species (layer 0)
-                    sMeta[buf * NE + e] = make_float4(g.r.x * g.inv_d, g.r.y * g.inv_d, g.r.z * g.inv_d, mw);
-                }
-                fence_async_smem();
-                mbar_arrive(&b_full[buf]);
-            }
-        }
-    } else {
-        // ===================== MMA issuer: the warp stays converged, one elected lane issues (descriptors in uniform registers) =====================
-        {
-            const uint32_t idesc = (1u << 4) | ((uint32_t)(NE >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);   // f16 x f16 -> f32
-            const uint32_t a_base = smem_u32(sA), b_base = smem_u32(sB);
-            uint32_t it = 0;
-            for (long long u = blockIdx.x; u < n_units; u += gridDim.x) {
-                const long long a0 = u * apu;
-                const long long a1 = min(N, a0 + (long long)apu);
-                const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
-                const int ntiles = (e_end - e_begin + NE - 1) / NE;
-                for (int t = 0; t < ntiles; t++, it++) {
-                    const int buf = it & 1;
-                    mbar_wait_sleep(&b_full[buf], (it >> 1) & 1, 128);
-                    tc_fence_after();
-                    if (elect_one()) {
-#pragma unroll
-                        for (int c = 0; c < NCH; c++) {
-                            const uint32_t d = tmem_base + buf * TCOLS + c * NE;
-#pragma unroll
-                            for (int o = 0; o < 6; o++) {
-                                const int kk = (o + 2) % 6;          // small terms (k-steps 2..5) first, main term last
-                                const uint64_t ad = make_desc_nosw(a_base + c * A_CHUNK_BYTES + kk * 2 * LBO, LBO, SBO);
-                                const uint64_t bd = make_desc_nosw(b_base + buf * B_BYTES + kk * 2 * LBO, LBO, SBO);
-                                umma_f16(d, ad, bd, idesc, o != 0);
-                            }
-                        }
-                        umma_commit(&t_full[buf]);
-                    }
-                    __syncwarp();
-                }
-            }
-        }
-    }
-    tc_fence_before();
-    __syncthreads();
-    if (warp == 7) tmem_dealloc(tmem_base, TALLOC);
-}
-
 
 // =============================================================================================================
 // adjoint message pass (sender-row gather form, painn_bwd.cu header): one 512-thread CTA per SM = two independent
@@ -669,13 +418,14 @@ __global__ void __launch_bounds__(FWDG_THREADS, 1) k_msg_fwd_g(const FwdParams p
                     }
                     vals[i] = R;
                 }
-                uint4 p0, p1, p2;
-                split3(vals, p0, p1, p2);
+                uint4 p0, p1, p2, p3;
+                split4(vals, p0, p1, p2, p3);
                 if (it >= 2) bar_sync(NB + buf, 224);   // tile it - 2 consumed (hardware-blocking wait, no spin)
-                uint8_t* bb = sB + buf * B_BYTES + (e >> 3) * SBO + (e & 7) * 16 + h * LBO;
-                *(uint4*)(bb) = p0;                       // term 0: k = b
-                *(uint4*)(bb + 4 * LBO) = p1;             // term 1: k = 32 + b   (lo(R) 2^11)
-                *(uint4*)(bb + 8 * LBO) = p2;             // term 2: k = 64 + b   (hi(R) 2^-11)
+                uint8_t* bb = sB + buf * B_BYTES + (e >> 3) * SBO + (e & 7) * 16;
+                *(uint4*)(bb + kgrp_off(0, h)) = p0;      // term 0: k = b        lo(R)
+                *(uint4*)(bb + kgrp_off(1, h)) = p1;      // term 1: k = 24 + b   lo(R) 2^6
+                *(uint4*)(bb + kgrp_off(2, h)) = p2;      // term 2: k = 48 + b   hi(R) 2^-6
+                *(uint4*)(bb + kgrp_off(3, h)) = p3;      // term 3: k = 72 + b   hi(R)
                 if (h == 0) {
                     float mw = g.r.w;                                             // sender index ...
                     if (!HAS_V) mw = __int_as_float(__ldg(p.types + __float_as_int(g.r.w)));   // ... or its species (layer 0)
@@ -706,7 +456,7 @@ __global__ void __launch_bounds__(FWDG_THREADS, 1) k_msg_fwd_g(const FwdParams p
                             const uint32_t d = tmem_base + buf * TCOLS + c * NE;
 #pragma unroll
                             for (int o = 0; o < 6; o++) {
-                                const int kk = (o + 2) % 6;          // small terms (k-steps 2..5) first, main term last
+                                const int kk = o;                    // ascending K: the small terms (ll, hl, lh) first, the main term (hh) last
                                 const uint64_t bd = make_desc_nosw(b_base + buf * B_BYTES + kk * 2 * LBO, LBO, SBO);
                                 if (c < 2) umma_f16_ts(d, tmem_A + c * 256 + kk * 8, bd, idesc, o != 0);
                                 else umma_f16(d, make_desc_nosw(a_base + kk * 2 * LBO, LBO, SBO), bd, idesc, o != 0);
@@ -1003,7 +753,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
             float4 raw_n = load_edge_raw(p.ej, e_begin + e, h < 3 ? e_end : 0);
             for (int t = 0; t < ntiles; t++, it++) {
                 const int buf = it & 1;
-                uint4 q[6];
+                uint4 q[8];
                 float4 meta_v = make_float4(0.f, 0.f, 0.f, 0.f);
                 const float4 raw = raw_n;
                 if (t + 1 < ntiles) raw_n = load_edge_raw(p.ej, e_begin + (t + 1) * NEB + e, h < 3 ? e_end : 0);
@@ -1028,8 +778,8 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                             sn_ = tt;
                         }
                     }
-                    split3(vals, q[0], q[1], q[2]);
-                    split3(dvals, q[3], q[4], q[5]);
+                    split4(vals, q[0], q[1], q[2], q[3]);
+                    split4(dvals, q[4], q[5], q[6], q[7]);
                     meta_v = make_float4(-g.r.x * g.inv_d, -g.r.y * g.inv_d, -g.r.z * g.inv_d, g.inv_d);   // u_e of edge (i <- j), 1/d
                 }
                 __syncwarp();
@@ -1038,10 +788,9 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
 #pragma unroll
                     for (int z = 0; z < 2; z++) {
                         const int row = z * NEB + e;
-                        uint8_t* bb = sB + buf * BB_BYTES + (row >> 3) * SBO + (row & 7) * 16 + h * LBO;
-                        *(uint4*)(bb) = q[3 * z + 0];
-                        *(uint4*)(bb + 4 * LBO) = q[3 * z + 1];
-                        *(uint4*)(bb + 8 * LBO) = q[3 * z + 2];
+                        uint8_t* bb = sB + buf * BB_BYTES + (row >> 3) * SBO + (row & 7) * 16;
+#pragma unroll
+                        for (int tm = 0; tm < 4; tm++) *(uint4*)(bb + kgrp_off(tm, h)) = q[4 * z + tm];
                     }
                     if (h == 0) sMeta[(it & 3) * NEB + e] = meta_v;
                 }
@@ -1117,7 +866,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                         const uint32_t d = tmem_base + buf * TCOLS + c * 2 * NEB;
 #pragma unroll
                         for (int o = 0; o < 6; o++) {
-                            const int kk = (o + 2) % 6;
+                            const int kk = o;
                             const uint64_t bd = make_desc_nosw(b_base + buf * BB_BYTES + kk * 2 * LBO, LBO, SBO);
                             if (c < 2) umma_f16_ts(d, tmem_A + c * 256 + kk * 8, bd, idesc, o != 0);
                             else umma_f16(d, make_desc_nosw(a_base + kk * 2 * LBO, LBO, SBO), bd, idesc, o != 0);
@@ -1149,7 +898,7 @@ struct Bwd0Params {
     const int* types;
     const float2* tab;     // [n_tab][F] (phi^s, phi^vs) per species
     const int* rev;
-    const uint4* A_img;    // [2 chunks][128 rows][96 fp16] row-major (k = term * 32 + basis slot): TMEM-resident A operand
+    const uint4* A_img;    // [2 chunks][128 rows][96 fp16] row-major (k = 24 term + basis slot): TMEM-resident A operand
     float4* G;
     float inv_rc;
     int K;
@@ -1304,7 +1053,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
             float4 raw_n = load_edge_raw(p.ej, e_begin + e, h < 3 ? e_end : 0);
             for (int t = 0; t < ntiles; t++, it++) {
                 const int buf = it & 1;
-                uint4 q[6];
+                uint4 q[8];
                 float4 meta_v = make_float4(0.f, 0.f, 0.f, 0.f);
                 const float4 raw = raw_n;
                 if (t + 1 < ntiles) raw_n = load_edge_raw(p.ej, e_begin + (t + 1) * NEB + e, h < 3 ? e_end : 0);
@@ -1331,8 +1080,8 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
                             sn_ = tt;
                         }
                     }
-                    split3(vals, q[0], q[1], q[2]);
-                    split3(dvals, q[3], q[4], q[5]);
+                    split4(vals, q[0], q[1], q[2], q[3]);
+                    split4(dvals, q[4], q[5], q[6], q[7]);
                     meta_v = make_float4(g.r.x * g.inv_d, g.r.y * g.inv_d, g.r.z * g.inv_d, g.inv_d);
                 }
                 __syncwarp();
@@ -1341,10 +1090,9 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
 #pragma unroll
                     for (int z = 0; z < 2; z++) {
                         const int row = z * NEB + e;
-                        uint8_t* bb = sB + buf * BB_BYTES + (row >> 3) * SBO + (row & 7) * 16 + h * LBO;
-                        *(uint4*)(bb) = q[3 * z + 0];
-                        *(uint4*)(bb + 4 * LBO) = q[3 * z + 1];
-                        *(uint4*)(bb + 8 * LBO) = q[3 * z + 2];
+                        uint8_t* bb = sB + buf * BB_BYTES + (row >> 3) * SBO + (row & 7) * 16;
+#pragma unroll
+                        for (int tm = 0; tm < 4; tm++) *(uint4*)(bb + kgrp_off(tm, h)) = q[4 * z + tm];
                     }
                     if (h == 0) { sMeta[(it & 3) * NEB + e] = meta_v; sSpec[(it & 3) * NEB + e] = spec_v; }
                 }
@@ -1438,7 +1186,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
                         const uint32_t d = tmem_base + buf * TCOLS + c * 2 * NEB;
 #pragma unroll
                         for (int o = 0; o < 6; o++) {
-                            const int kk = (o + 2) % 6;
+                            const int kk = o;
                             const uint64_t bd = make_desc_nosw(b_base + buf * BB_BYTES + kk * 2 * LBO, LBO, SBO);
                             umma_f16_ts(d, tmem_A + c * 48 + kk * 8, bd, idesc, o != 0);
                         }
@@ -1456,21 +1204,79 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
 
 }  // namespace ev3
 
-// host: filter operand of one layer as plain rows [3 chunks][128 channels][96 fp16], k = term * 32 + basis slot, terms
-// (hi, hi 2^-11, lo 2^11) of (bf | Wf) -- the TMEM-resident A operand of k_msg_bwd0 (same numbers as edge_build_filter_image)
+// gather rows: Q4[j][f] = (phi^s, phi^vs, phi^vv v_x, phi^vv v_y), Q1[j][f] = phi^vv v_z ; layer 0 (v = 0): Q2 = (phi^s, phi^vs)
+__global__ void k_make_gather(long long N, const float* __restrict__ phi, const float* __restrict__ v,
+                              float4* __restrict__ Q4, float* __restrict__ Q1, float2* __restrict__ Q2, int has_v) {
+    constexpr int F = ev3::F;
+    long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (idx >= N * F) return;
+    const long long j = idx / F;
+    const int f = (int)(idx - j * F);
+    const float ps = phi[j * 3 * F + f], pvs = phi[j * 3 * F + F + f];
+    if (has_v) {
+        const float pvv = phi[j * 3 * F + 2 * F + f];
+        Q4[idx] = make_float4(ps, pvs, pvv * v[j * 3 * F + f], pvv * v[j * 3 * F + F + f]);
+        Q1[idx] = pvv * v[j * 3 * F + 2 * F + f];
+    } else {
+        Q2[idx] = make_float2(ps, pvs);
+    }
+}
+// gather rows of the adjoint pass: Gb[i][f] = (sb', vb'_x, vb'_y, vb'_z)
+__global__ void k_make_gather_bwd(long long N, const float* __restrict__ s1b, const float* __restrict__ v1b,
+                                  float4* __restrict__ Gb) {
+    constexpr int F = ev3::F;
+    long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (idx >= N * F) return;
+    const long long j = idx / F;
+    const int f = (int)(idx - j * F);
+    Gb[idx] = make_float4(s1b[idx], v1b[j * 3 * F + f], v1b[j * 3 * F + F + f], v1b[j * 3 * F + 2 * F + f]);
+}
+void make_gather_rows(const Launch& L, long long N, const float* phi, const float* v, float* Q4, float* Q1, bool has_v) {
+    if (N == 0) return;
+    k_make_gather<<<(unsigned)((N * ev3::F + 255) / 256), 256, 0, L.stream>>>(N, phi, v, (float4*)Q4, Q1, (float2*)Q4, has_v ? 1 : 0);
+    KLAUNCH(L);
+}
+void make_gather_rows_bwd(const Launch& L, long long N, const float* s1b, const float* v1b, float* Gb) {
+    if (N == 0) return;
+    k_make_gather_bwd<<<(unsigned)((N * ev3::F + 255) / 256), 256, 0, L.stream>>>(N, s1b, v1b, (float4*)Gb);
+    KLAUNCH(L);
+}
+
+// host: the four fp16 planes of one filter weight w = hi + r (same split as split4() of the B operand; the term order
+// (ll, hl, lh, hh) pairs plane t of A with plane t of B):  r | hi 2^-6 | r 2^6 | hi
+static void filter_planes(float w, unsigned short (&bits)[4]) {
+    const __half hi = __float2half_rn(w);
+    const float hif = __half2float(hi), r = w - hif;
+    const __half vals[4] = {__float2half_rn(r), __float2half_rn(hif * (1.0f / 64.0f)), __float2half_rn(r * 64.0f), hi};
+    for (int t = 0; t < 4; t++) memcpy(&bits[t], &vals[t], 2);
+}
+// host: filter operand (bf | Wf) of one layer as plain rows [3 chunks][128 channels][96 fp16], k = 24 term + basis slot
+// (basis slot 0 = the bias bf) -- the TMEM-resident A operand
 void edge_build_filter_rows(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img) {
     img.assign((size_t)3 * ev3::F * ev3::KP, 0);
     for (int c = 0; c < 3; c++)
         for (int r = 0; r < ev3::F; r++)
             for (int b = 0; b <= K; b++) {
                 const float w = b == 0 ? bf[c * ev3::F + r] : Wf[(size_t)(c * ev3::F + r) * K + (b - 1)];
-                const __half hi = __float2half_rn(w);
-                const float hif = __half2float(hi);
-                const __half vals[3] = {hi, __float2half_rn(hif * (1.0f / 2048.0f)), __float2half_rn((w - hif) * 2048.0f)};
-                for (int t = 0; t < 3; t++) {
-                    unsigned short bits;
-                    memcpy(&bits, &vals[t], 2);
-                    img[((size_t)c * ev3::F + r) * ev3::KP + t * 32 + b] = bits;
+                unsigned short bits[4];
+                filter_planes(w, bits);
+                for (int t = 0; t < 4; t++) img[((size_t)c * ev3::F + r) * ev3::KP + t * 24 + b] = bits[t];
+            }
+}
+// host: the same numbers as the K-major no-swizzle shared-memory image of the A operand (3 chunks of A_CHUNK_BYTES)
+void edge_build_filter_image(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img) {
+    using namespace ev3;
+    img.assign(3 * A_CHUNK_BYTES / 2, 0);
+    for (int c = 0; c < 3; c++)
+        for (int r = 0; r < F; r++)
+            for (int b = 0; b <= K; b++) {
+                const float w = b == 0 ? bf[c * F + r] : Wf[(size_t)(c * F + r) * K + (b - 1)];
+                unsigned short bits[4];
+                filter_planes(w, bits);
+                for (int t = 0; t < 4; t++) {
+                    const int k = t * 24 + b;
+                    const size_t off = (size_t)c * A_CHUNK_BYTES + (r / 8) * SBO + (k / 8) * LBO + (r % 8) * 16 + (k % 8) * 2;
+                    img[off / 2] = bits[t];
                 }
             }
 }
@@ -1485,36 +1291,29 @@ static int sm_count() {
     return n_sm;
 }
 
-// F = 128, K <= 23 only.  Q4/Q1 from make_gather_rows (layer 0: Q4 holds float2 rows); A_img from edge_build_filter_image.
+// F = 128, K <= 23 only.  Q4/Q1 from make_gather_rows; A_img / A_rows from edge_build_filter_image / _rows.  has_v = false:
+// layer 0 through the species table.
 bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* s,
                     const float* v, const float* Q4, const float* Q1, const void* A_img, const void* A_rows, float* sn, float* v1,
-                    bool has_v, const int* types_s, const float* tab, int n_tab, bool grouped) {
+                    bool has_v, const int* types_s, const float* tab, int n_tab) {
     using namespace ev3;
     if (N == 0) return true;
-    if (K > 23) return false;
+    if (K > 23 || !A_rows || !A_img) return false;
     if (!has_v && (!tab || !types_s || n_tab > TAB_MAX)) return false;
     static bool attr = false;
     if (!attr) {
-        if (cudaFuncSetAttribute(k_msg_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fwd_smem_bytes(true)) != cudaSuccess ||
-            cudaFuncSetAttribute(k_msg_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fwd_smem_bytes(false)) != cudaSuccess ||
-            cudaFuncSetAttribute(k_msg_fwd_g<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fwdg_smem_bytes(true)) != cudaSuccess ||
+        if (cudaFuncSetAttribute(k_msg_fwd_g<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fwdg_smem_bytes(true)) != cudaSuccess ||
             cudaFuncSetAttribute(k_msg_fwd_g<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fwdg_smem_bytes(false)) != cudaSuccess)
             return false;
         attr = true;
     }
     FwdParams p{N, row_ptr, ej, s, v, (const float4*)Q4, Q1, (const float2*)Q4, (const uint4*)A_img, (const uint4*)A_rows, sn, v1,
-                1.0f / rc, K, g_atoms_per_unit_fwd, types_s, (const float2*)tab, n_tab};
+                1.0f / rc, K, L.apu_fwd, types_s, (const float2*)tab, n_tab};
     const long long n_units = (N + p.atoms_per_unit - 1) / p.atoms_per_unit;
-    if (grouped && A_rows) {
-        // one CTA per SM, two 8-warp pipelines sharing the TMEM-resident filter operand
-        const int grid = (int)std::min<long long>((n_units + 1) / 2, (long long)sm_count());
-        if (has_v) k_msg_fwd_g<true><<<grid, FWDG_THREADS, fwdg_smem_bytes(true), L.stream>>>(p);
-        else k_msg_fwd_g<false><<<grid, FWDG_THREADS, fwdg_smem_bytes(false), L.stream>>>(p);
-    } else {
-        const int grid = (int)std::min<long long>(n_units, 2LL * sm_count());
-        if (has_v) k_msg_fwd<true><<<grid, FWD_THREADS, fwd_smem_bytes(true), L.stream>>>(p);
-        else k_msg_fwd<false><<<grid, FWD_THREADS, fwd_smem_bytes(false), L.stream>>>(p);
-    }
+    // one CTA per SM, two 8-warp pipelines sharing the TMEM-resident filter operand
+    const int grid = (int)std::min<long long>((n_units + 1) / 2, (long long)sm_count());
+    if (has_v) k_msg_fwd_g<true><<<grid, FWDG_THREADS, fwdg_smem_bytes(true), L.stream>>>(p);
+    else k_msg_fwd_g<false><<<grid, FWDG_THREADS, fwdg_smem_bytes(false), L.stream>>>(p);
     KLAUNCH(L);
     return true;
 }
@@ -1525,7 +1324,7 @@ bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
                     float* vb_out, float4* G, bool first, bool layer0) {
     using namespace ev3;
     if (N == 0) return true;
-    if (K > 23) return false;
+    if (K > 23 || !A_rows || !A_img) return false;
     static bool attr = false;
     if (!attr) {
         if (cudaFuncSetAttribute(k_msg_bwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bwd_smem_bytes(2)) != cudaSuccess ||
@@ -1534,7 +1333,7 @@ bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
         attr = true;
     }
     BwdParams p{N, row_ptr, ej, (const float4*)Gb, phi, v_in, v1b, (const uint4*)A_img, (const uint4*)A_rows, phib, vb_out, G,
-                1.0f / rc, K, g_atoms_per_unit, first ? 1 : 0};
+                1.0f / rc, K, L.apu_bwd, first ? 1 : 0};
     const long long n_units = (N + p.atoms_per_unit - 1) / p.atoms_per_unit;
     const int grid = (int)std::min<long long>((n_units + 1) / 2, (long long)sm_count());
     if (layer0) k_msg_bwd<true><<<grid, BWD_THREADS, bwd_smem_bytes(2), L.stream>>>(p);
@@ -1554,7 +1353,7 @@ bool message_bwd0_v3(const Launch& L, long long N, int K, float rc, const int* r
         if (cudaFuncSetAttribute(k_msg_bwd0, cudaFuncAttributeMaxDynamicSharedMemorySize, bwd0_smem_bytes()) != cudaSuccess) return false;
         attr = true;
     }
-    Bwd0Params p{N, row_ptr, ej, (const float4*)Gb, types_s, (const float2*)tab, rev, (const uint4*)A_img, G, 1.0f / rc, K, g_atoms_per_unit,
+    Bwd0Params p{N, row_ptr, ej, (const float4*)Gb, types_s, (const float2*)tab, rev, (const uint4*)A_img, G, 1.0f / rc, K, L.apu_bwd,
                  first ? 1 : 0, n_tab};
     const long long n_units = (N + p.atoms_per_unit - 1) / p.atoms_per_unit;
     const int grid = (int)std::min<long long>((n_units + 1) / 2, (long long)sm_count());

@@ -2,8 +2,8 @@
 // (phi-MLP, U/V, update-MLP, readout and their transposed adjoints;
 //  weights are fixed, so there are no weight-gradient GEMMs.)
 //
-// gemm_nt_simt: plain fp32 shared-memory-tiled reference path (kept as the numerical reference of the tcgen05
-// path and for shapes the tensor-core kernel does not cover).
+// k_gemm_nt_simt: plain fp32 shared-memory-tiled path for the shapes the tensor-core kernels do not cover (F = 32, 64
+// models, readout of width 16 / 32).
 #include "common.cuh"
 
 namespace painn {
@@ -12,27 +12,11 @@ namespace painn {
 
 constexpr int TM = 64, TN = 64, TK = 16;
 
-// operand-precision emulation (debug knob "gemm_emulate"): 0 fp32, 1 tf32 (RN), 2 bf16 (RN), 3 bf16 hi+lo split
-// with the three leading product terms (a_hi b_hi + a_hi b_lo + a_lo b_hi).  Used to size the precision plan of
-// the tensor-core path against the parity tolerances before/while it is being written.
-int g_gemm_emulate = 0;
-
-__device__ __forceinline__ float rn_tf32(float x) {
-    uint32_t u = __float_as_uint(x);
-    u += 0xfffu + ((u >> 13) & 1u);
-    return __uint_as_float(u & 0xffffe000u);
-}
-__device__ __forceinline__ float rn_bf16(float x) {
-    uint32_t u = __float_as_uint(x);
-    u += 0x7fffu + ((u >> 16) & 1u);
-    return __uint_as_float(u & 0xffff0000u);
-}
-
 __global__ void __launch_bounds__(256) k_gemm_nt_simt(const float* __restrict__ A, int lda,
                                                       const float* __restrict__ B, int ldb, float* __restrict__ C,
                                                       int ldc, long long M, int N, int K,
-                                                      const float* __restrict__ bias, int accumulate, int emu) {
-    __shared__ float As[TK][TM + 4], Bs[TK][TN + 4], Al[TK][TM + 4], Bh[TK][TN + 4];
+                                                      const float* __restrict__ bias, int accumulate) {
+    __shared__ float As[TK][TM + 4], Bs[TK][TN + 4];
     const long long m0 = (long long)blockIdx.x * TM;
     const int n0 = blockIdx.y * TN;
     const int tx = threadIdx.x % 16, ty = threadIdx.x / 16;
@@ -41,27 +25,9 @@ __global__ void __launch_bounds__(256) k_gemm_nt_simt(const float* __restrict__ 
         for (int idx = threadIdx.x; idx < TM * TK; idx += 256) {
             int r = idx / TK, c = idx % TK;
             long long m = m0 + r;
-            float av = (m < M && k0 + c < K) ? A[m * lda + k0 + c] : 0.0f;
+            As[c][r] = (m < M && k0 + c < K) ? A[m * lda + k0 + c] : 0.0f;
             int n = n0 + r;
-            float bv = (n < N && k0 + c < K) ? B[(size_t)n * ldb + k0 + c] : 0.0f;
-            if (emu == 1) { av = rn_tf32(av); bv = rn_tf32(bv); }
-            else if (emu == 2) { av = rn_bf16(av); bv = rn_bf16(bv); }
-            else if (emu == 3) {
-                float ah = rn_bf16(av), bh = rn_bf16(bv);
-                Al[c][r] = rn_bf16(av - ah);
-                Bh[c][r] = bh;
-                av = ah;
-                bv = bh + rn_bf16(bv - bh);
-            }
-            else if (emu == 4) {   // 3xTF32: hi = truncation to tf32, lo = tf32(a - hi); hi*hi + hi*lo + lo*hi
-                float ah = __uint_as_float(__float_as_uint(av) & 0xffffe000u), bh = __uint_as_float(__float_as_uint(bv) & 0xffffe000u);
-                Al[c][r] = __uint_as_float(__float_as_uint(av - ah) & 0xffffe000u);
-                Bh[c][r] = bh;
-                av = ah;
-                bv = bh + __uint_as_float(__float_as_uint(bv - bh) & 0xffffe000u);
-            }
-            As[c][r] = av;
-            Bs[c][r] = bv;
+            Bs[c][r] = (n < N && k0 + c < K) ? B[(size_t)n * ldb + k0 + c] : 0.0f;
         }
         __syncthreads();
 #pragma unroll
@@ -73,14 +39,6 @@ __global__ void __launch_bounds__(256) k_gemm_nt_simt(const float* __restrict__ 
             for (int i = 0; i < 4; i++)
 #pragma unroll
                 for (int j = 0; j < 4; j++) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
-            if (emu >= 3) {
-#pragma unroll
-                for (int i = 0; i < 4; i++) { a[i] = Al[k][ty * 4 + i]; b[i] = Bh[k][tx * 4 + i]; }
-#pragma unroll
-                for (int i = 0; i < 4; i++)
-#pragma unroll
-                    for (int j = 0; j < 4; j++) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
-            }
         }
         __syncthreads();
     }
@@ -176,22 +134,25 @@ __global__ void __launch_bounds__(256, 2) k_sgemm128(const float* __restrict__ A
     }
 }
 
-// weight registry: B pointer -> (hi, lo) TF32 split planes for the tensor-core path (filled at mlp_create)
-#include <unordered_map>
-static std::unordered_map<const float*, std::pair<const float*, const float*>> g_split;
-int g_last_gemm_tc = 0;   // set to 1 by gemm_nt when the tensor-core kernel was used (test hook)
-int g_gemm_path = 0;   // 0: tensor cores when the shape is covered, 1: forward GEMM (round-to-nearest / exact accumulation wanted)
-int g_gemm_fwd_exact = 1;   // forward GEMMs: 1 = exact integer-slice tensor-core kernel when covered, 0 = fp32 FFMA kernel
-void gemm_register_split(const float* W, const float* hi, const float* lo) { g_split[W] = {hi, lo}; }
-void gemm_unregister_split(const float* W) { g_split.erase(W); }
+// Weight registry (per model, common.cuh::GemmRegistry): weight pointer -> (hi, lo) TF32 split planes of the 3xTF32
+// kernel and -> fp16 integer slices of the exact kernel; filled at mlp_create, read-only afterwards.  Which path a
+// call takes comes with the Launch context (gemm_path / fwd_exact), never from process-wide state.
+void gemm_register_split(GemmRegistry& reg, const float* W, const float* hi, const float* lo) { reg.split[W] = {hi, lo}; }
 bool gemm_nt_tc(const Launch& L, const float* A, int lda, const float* Whi, const float* Wlo, int ldw, float* C, int ldc,
                 long long M, int N, int K, const float* bias, bool accumulate, const float* dsilu_pre = nullptr, int ld_pre = 0,
                 const float* resid = nullptr);
 void mul_dsilu(const Launch& L, long long n, const float* pre, float* g);
 
-void gemm_nt_act(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
-                 int N, int K, const float* bias, bool accumulate, bool act_a);
-bool gemm_act_supported(int N, int K) { return g_gemm_emulate == 0 && N % 128 == 0 && K % 8 == 0; }
+static bool split_of(const Launch& L, const float* B, const float** hi, const float** lo) {
+    if (!L.reg) return false;
+    auto it = L.reg->split.find(B);
+    if (it == L.reg->split.end()) return false;
+    *hi = it->second.first; *lo = it->second.second;
+    return true;
+}
+static void used_tc(const Launch& L) { if (L.used_tc) *L.used_tc = 1; }
+
+bool gemm_act_supported(int N, int K) { return N % 128 == 0 && K % 8 == 0; }
 
 void gemm_nt(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
              int N, int K, const float* bias, bool accumulate) {
@@ -203,13 +164,11 @@ void gemm_nt(const Launch& L, const float* A, int lda, const float* B, int ldb, 
 void gemm_nt_dsilu(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
                    int N, int K, const float* pre) {
     if (M == 0) return;
-    if (g_gemm_path == 0 && g_gemm_emulate == 0 && ldc == N) {
-        auto it = g_split.find(B);
-        if (it != g_split.end() &&
-            gemm_nt_tc(L, A, lda, it->second.first, it->second.second, ldb, C, ldc, M, N, K, nullptr, false, pre, N)) {
-            g_last_gemm_tc = 1;
-            return;
-        }
+    const float *hi, *lo;
+    if (L.gemm_path == 0 && ldc == N && split_of(L, B, &hi, &lo) &&
+        gemm_nt_tc(L, A, lda, hi, lo, ldb, C, ldc, M, N, K, nullptr, false, pre, N)) {
+        used_tc(L);
+        return;
     }
     gemm_nt(L, A, lda, B, ldb, C, ldc, M, N, K, nullptr, false);
     mul_dsilu(L, M * N, pre, C);
@@ -220,55 +179,42 @@ void gemm_nt_dsilu(const Launch& L, const float* A, int lda, const float* B, int
 void gemm_nt_resid(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
                    int N, int K, const float* resid) {
     if (M == 0) return;
-    if (g_gemm_path == 0 && g_gemm_emulate == 0) {
-        auto it = g_split.find(B);
-        if (it != g_split.end() &&
-            gemm_nt_tc(L, A, lda, it->second.first, it->second.second, ldb, C, ldc, M, N, K, nullptr, false, nullptr, 0, resid)) {
-            g_last_gemm_tc = 1;
-            return;
-        }
+    const float *hi, *lo;
+    if (L.gemm_path == 0 && split_of(L, B, &hi, &lo) &&
+        gemm_nt_tc(L, A, lda, hi, lo, ldb, C, ldc, M, N, K, nullptr, false, nullptr, 0, resid)) {
+        used_tc(L);
+        return;
     }
     cudaMemcpy2DAsync(C, (size_t)ldc * 4, resid, (size_t)ldc * 4, (size_t)N * 4, (size_t)M, cudaMemcpyDeviceToDevice, L.stream);
     gemm_nt(L, A, lda, B, ldb, C, ldc, M, N, K, nullptr, true);
 }
 
-// act_a: C = SiLU(A) . B^T + bias  (only the fp32 FFMA path implements it; callers use it on forward GEMMs only)
+// act_a: C = SiLU(A) . B^T + bias  (forward GEMMs only: the exact tensor-core kernel or the fp32 FFMA kernel)
 void gemm_nt_act(const Launch& L, const float* A, int lda, const float* B, int ldb, float* C, int ldc, long long M,
                  int N, int K, const float* bias, bool accumulate, bool act_a) {
     if (M == 0) return;
-    const bool fast_ok = g_gemm_emulate == 0 && N % 128 == 0 && K % 8 == 0 && lda % 4 == 0 && ldb % 4 == 0 &&
+    const bool fast_ok = N % 128 == 0 && K % 8 == 0 && lda % 4 == 0 && ldb % 4 == 0 &&
                          ldc % 4 == 0 && ((((uintptr_t)A | (uintptr_t)B | (uintptr_t)C | (uintptr_t)bias) & 15) == 0);
-    static int fwd_call = 0;                                   // debug: g_gemm_fwd_exact >= 2 is a bit mask over the
-    const int call_type = (act_a || g_gemm_path == 1) ? (fwd_call++ % 16) % 5 : 0;   // forward GEMM types 0..4 (bits 1..5)
-    const bool want_exact = g_gemm_fwd_exact == 1 || (g_gemm_fwd_exact >= 2 && ((g_gemm_fwd_exact >> (1 + call_type)) & 1));
-    if ((act_a || g_gemm_path == 1) && want_exact && g_gemm_emulate == 0 &&
-        gemm_nt_exact(L, A, lda, B, C, ldc, M, N, K, bias, accumulate, act_a)) {
-        g_last_gemm_tc = 1;
+    const bool fwd = act_a || L.gemm_path == 1;      // round-to-nearest / exact accumulation wanted (B3)
+    if (fwd && L.fwd_exact && gemm_nt_exact(L, A, lda, B, C, ldc, M, N, K, bias, accumulate, act_a)) {
+        used_tc(L);
         return;
     }
-    if (act_a || (g_gemm_path == 1 && fast_ok)) {
-        if (fast_ok && M / 128 < 65535) {
-            dim3 grid((unsigned)(N / 128), (unsigned)((M + 127) / 128));
-            if (act_a) k_sgemm128<true><<<grid, 256, 0, L.stream>>>(A, lda, B, ldb, C, ldc, M, N, K, bias, accumulate ? 1 : 0);
-            else k_sgemm128<false><<<grid, 256, 0, L.stream>>>(A, lda, B, ldb, C, ldc, M, N, K, bias, accumulate ? 1 : 0);
-            KLAUNCH(L);
-            return;
-        }
-    }
-    if (act_a) {   // shapes the fast kernel does not cover: caller must not request act_a (checked by the caller)
+    if (fwd && fast_ok && M / 128 < 65535) {
+        dim3 grid((unsigned)(N / 128), (unsigned)((M + 127) / 128));
+        if (act_a) k_sgemm128<true><<<grid, 256, 0, L.stream>>>(A, lda, B, ldb, C, ldc, M, N, K, bias, accumulate ? 1 : 0);
+        else k_sgemm128<false><<<grid, 256, 0, L.stream>>>(A, lda, B, ldb, C, ldc, M, N, K, bias, accumulate ? 1 : 0);
+        KLAUNCH(L);
         return;
     }
-    if (g_gemm_path == 0 && g_gemm_emulate == 0) {
-        auto it = g_split.find(B);
-        if (it != g_split.end() &&
-            gemm_nt_tc(L, A, lda, it->second.first, it->second.second, ldb, C, ldc, M, N, K, bias, accumulate)) {
-            g_last_gemm_tc = 1;
-            return;
-        }
+    if (act_a) return;   // shapes neither kernel covers: callers check gemm_act_supported() before asking for act_a
+    const float *hi, *lo;
+    if (L.gemm_path == 0 && split_of(L, B, &hi, &lo) && gemm_nt_tc(L, A, lda, hi, lo, ldb, C, ldc, M, N, K, bias, accumulate)) {
+        used_tc(L);
+        return;
     }
     dim3 grid((unsigned)((M + TM - 1) / TM), (unsigned)((N + TN - 1) / TN));
-    k_gemm_nt_simt<<<grid, 256, 0, L.stream>>>(A, lda, B, ldb, C, ldc, M, N, K, bias, accumulate ? 1 : 0,
-                                                   g_gemm_emulate);
+    k_gemm_nt_simt<<<grid, 256, 0, L.stream>>>(A, lda, B, ldb, C, ldc, M, N, K, bias, accumulate ? 1 : 0);
     KLAUNCH(L);
 }
 

@@ -659,15 +659,10 @@ static bool launch(const Launch& L, const CUtensorMap& a, const CUtensorMap& whi
 }  // namespace tc
 
 // ---- exact integer-slice path: weight slices are cut once, at create ----
-struct ExactW {
-    int N, K;
-    __half* planes;    // device [K / 128][3][N][128]  integer-valued fp16 slices t1, t2, t3
-    float* cs;         // device [K / 128][N]          2^f_n
-};
-static std::unordered_map<const float*, ExactW> g_exact;
-
-void gemm_register_exact(const float* Wdev, const float* Whost, int N, int K) {
-    if (K % 128 != 0 || N % tc::XBN != 0 || g_exact.count(Wdev)) return;
+// (ExactW in common.cuh: planes = device [K / 128][3][N][128] integer-valued fp16 slices t1, t2, t3; cs = device
+//  [K / 128][N] column scales 2^f_n.)  The registry belongs to the model.
+void gemm_register_exact(GemmRegistry& reg, const float* Wdev, const float* Whost, int N, int K) {
+    if (K % 128 != 0 || N % tc::XBN != 0 || reg.exact.count(Wdev)) return;
     const int nc = K / 128;
     std::vector<__half> pl((size_t)nc * 3 * N * 128);
     std::vector<float> cs((size_t)nc * N);
@@ -697,14 +692,12 @@ void gemm_register_exact(const float* Wdev, const float* Whost, int N, int K) {
     if (cudaMalloc(&e.cs, cs.size() * 4) != cudaSuccess) { cudaFree(e.planes); return; }
     cudaMemcpy(e.planes, pl.data(), pl.size() * 2, cudaMemcpyHostToDevice);
     cudaMemcpy(e.cs, cs.data(), cs.size() * 4, cudaMemcpyHostToDevice);
-    g_exact[Wdev] = e;
+    reg.exact[Wdev] = e;
 }
-void gemm_unregister_exact(const float* Wdev) {
-    auto it = g_exact.find(Wdev);
-    if (it == g_exact.end()) return;
-    cudaFree(it->second.planes);
-    cudaFree(it->second.cs);
-    g_exact.erase(it);
+void gemm_registry_free(GemmRegistry& reg) {
+    for (auto& kv : reg.exact) { cudaFree(kv.second.planes); cudaFree(kv.second.cs); }
+    reg.exact.clear();
+    reg.split.clear();
 }
 
 // C (+)= act(A) . W^T + bias on tensor cores with exact accumulation (k_gemm_exact).  Returns false when W has no
@@ -712,8 +705,9 @@ void gemm_unregister_exact(const float* Wdev) {
 bool gemm_nt_exact(const Launch& L, const float* A, int lda, const float* W, float* C, int ldc, long long M, int N, int K,
                    const float* bias, bool accumulate, bool act_a) {
     using namespace tc;
-    auto it = g_exact.find(W);
-    if (it == g_exact.end() || it->second.N != N || it->second.K != K) return false;
+    if (!L.reg) return false;
+    auto it = L.reg->exact.find(W);
+    if (it == L.reg->exact.end() || it->second.N != N || it->second.K != K) return false;
     if (M <= 0 || N > XNMAX || (lda % 4) || (ldc % 4) || (((uintptr_t)A | (uintptr_t)C | (uintptr_t)bias) & 15)) return false;
     static int n_sm = 0;
     static bool attr = false;
@@ -733,7 +727,7 @@ bool gemm_nt_exact(const Launch& L, const float* A, int lda, const float* W, flo
     const int grid = (int)(units < n_sm ? units : n_sm);
     for (int c = 0; c < K / 128; c++) {
         CUtensorMap ma, m1, m2, m3;
-        const __half* pl = e.planes + (size_t)c * 3 * N * 128;
+        const __half* pl = (const __half*)e.planes + (size_t)c * 3 * N * 128;
         if (!make_map(&ma, A + c * 128, M, 128, lda, BM) || !make_map16(&m1, pl, N, XBN) ||
             !make_map16(&m2, pl + (size_t)N * 128, N, XBN) || !make_map16(&m3, pl + (size_t)2 * N * 128, N, XBN))
             return false;   // (only possible before the first launch: the driver entry point is missing)

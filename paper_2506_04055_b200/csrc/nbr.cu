@@ -17,12 +17,17 @@ __device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? l
 // ------------------------------------------------------------------------------------------------ a0 + a1
 __global__ void k_bin(const double* __restrict__ pos, const int* __restrict__ types, long long N, int n_species,
                       Grid g, int* __restrict__ cell_id, signed char* __restrict__ wrap,
-                      int* __restrict__ cell_count, int* __restrict__ flags) {
+                      int* __restrict__ cell_count, int* __restrict__ flags, long long n_local,
+                      const int* __restrict__ ghost_owner) {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= N) return;
     int t = types[i];
     int bad = 0;
     if (t < 0 || t >= n_species) bad |= FLAG_TYPE_RANGE;
+    if (ghost_owner != nullptr && i >= n_local) {        // the fold adds onto forces[owner]: it must be a local row
+        const int o = ghost_owner[i - n_local];
+        if (o < 0 || o >= n_local) bad |= FLAG_OWNER_RANGE;
+    }
     int c[3];
 #pragma unroll
     for (int d = 0; d < 3; d++) {
@@ -46,10 +51,10 @@ __global__ void k_bin(const double* __restrict__ pos, const int* __restrict__ ty
 }
 
 void nbr_bin(const Launch& L, const double* pos, const int* types, long long N, int n_species, Grid g,
-             int* cell_id, signed char* wrap, int* cell_count, int* flags) {
+             int* cell_id, signed char* wrap, int* cell_count, int* flags, long long n_local, const int* ghost_owner) {
     if (N == 0) return;
     k_bin<<<(unsigned)((N + 255) / 256), 256, 0, L.stream>>>(pos, types, N, n_species, g, cell_id, wrap,
-                                                             cell_count, flags);
+                                                             cell_count, flags, n_local, ghost_owner);
     KLAUNCH(L);
 }
 
@@ -325,7 +330,7 @@ void nbr_fill(const Launch& L, long long N, Grid g, const double* pos_s, const s
 
 // reverse-edge index: for slot e = (a <- b, code) find the slot of (b <- a, 26 - code) in row b
 __global__ void k_reverse(long long N, const int* __restrict__ row_ptr, const float4* __restrict__ ej,
-                          const unsigned char* __restrict__ img, int* __restrict__ rev) {
+                          const unsigned char* __restrict__ img, int* __restrict__ rev, int* __restrict__ miss) {
     // one warp per row a
     long long a = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
     int lane = threadIdx.x & 31;
@@ -337,14 +342,18 @@ __global__ void k_reverse(long long N, const int* __restrict__ row_ptr, const fl
         int r = -1;
         for (int x = row_ptr[b]; x < row_ptr[b + 1]; x++)
             if (__float_as_int(ej[x].w) == (int)a && (int)img[x] == want) { r = x; break; }
+        if (r < 0) { r = e; atomicAdd(miss, 1); }     // see k_reverse_keys
         rev[e] = r;
     }
 }
 // The same search on the compact keys (sender << 5 | image code) written by k_fill: rows start at multiples of 8 slots,
 // so 8 candidates are two aligned 16-byte loads (the float4 records cost a 32-byte sector per two candidates: 4x the
 // L2 traffic, which is what bounds this pass).
+// A pair whose d^2 sits within an ulp of rc^2 can pass the fp64 predicate in one direction only when an image shift is
+// involved (fl(fl(x_b + S L) - x_a) is not the exact negation of fl(fl(x_a - S L) - x_b)): such a slot has no reverse.
+// It maps to itself (G[rev] - G = 0: no force from an edge whose weight fc(rc) is zero anyway) and is counted in *miss.
 __global__ void k_reverse_keys(long long N, const int* __restrict__ row_ptr, const int* __restrict__ key,
-                               int* __restrict__ rev) {
+                               int* __restrict__ rev, int* __restrict__ miss) {
     long long a = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
     int lane = threadIdx.x & 31;
     if (a >= N) return;
@@ -366,19 +375,20 @@ __global__ void k_reverse_keys(long long N, const int* __restrict__ row_ptr, con
             else if (q1.z == want) r = x + 6;
             else if (q1.w == want) r = x + 7;
         }
+        if (r < 0) { r = e; atomicAdd(miss, 1); }
         rev[e] = r;
     }
 }
 // key: the array nbr_fill wrote (nullptr, or N >= 2^26: search the float4 records)
 void nbr_reverse(const Launch& L, long long N, const int* row_ptr, const float4* ej, const unsigned char* img,
-                 const int* key, int* rev) {
+                 const int* key, int* rev, int* miss) {
     if (N == 0) return;
     if (key && N < (1ll << 26)) {
-        k_reverse_keys<<<(unsigned)((N * 32 + 255) / 256), 256, 0, L.stream>>>(N, row_ptr, key, rev);
+        k_reverse_keys<<<(unsigned)((N * 32 + 255) / 256), 256, 0, L.stream>>>(N, row_ptr, key, rev, miss);
         KLAUNCH(L);
         return;
     }
-    k_reverse<<<(unsigned)((N * 32 + 255) / 256), 256, 0, L.stream>>>(N, row_ptr, ej, img, rev);
+    k_reverse<<<(unsigned)((N * 32 + 255) / 256), 256, 0, L.stream>>>(N, row_ptr, ej, img, rev, miss);
     KLAUNCH(L);
 }
 

@@ -88,19 +88,7 @@ void update_bwd2(const Launch& L, long long N, int F, const float* sb, const flo
 
 // ------------------------------------------------------------------------------------------------ a12
 constexpr int BWD_CHUNK = 32;
-extern int g_filter_emulate, g_gather_emulate;
-__device__ __forceinline__ float r_h(float x) { return __half2float(__float2half_rn(x)); }
-__device__ __forceinline__ float r_b(float x) { return __bfloat162float(__float2bfloat16_rn(x)); }
-template <int EMU> __device__ __forceinline__ float fdot(float w, float r, float acc) {
-    if (EMU == 0) return fmaf(w, r, acc);
-    if (EMU == 1) return fmaf(r_h(w), r_h(r), acc);
-    if (EMU == 3) return fmaf(r_b(w), r_b(r), acc);
-    float wh = r_h(w), wl = r_h(w - wh), rh = r_h(r), rl = r_h(r - rh);
-    return fmaf(wl, rh, fmaf(wh, rh + rl, acc));
-}
-__device__ __forceinline__ float gq(float x, int g) { return g == 0 ? x : (g == 1 ? r_h(x) : r_b(x)); }
-
-template <int KMAX, int EMU>
+template <int KMAX>
 __global__ void __launch_bounds__(128) k_message_bwd(long long N, int F, int K, float inv_rc,
                                                      const int* __restrict__ row_ptr,
                                                      const float4* __restrict__ ej,
@@ -108,7 +96,7 @@ __global__ void __launch_bounds__(128) k_message_bwd(long long N, int F, int K, 
                                                      const float* __restrict__ phi, const float* __restrict__ v_in,
                                                      const float* __restrict__ Wf, const float* __restrict__ bf,
                                                      float* __restrict__ phib, float* __restrict__ vb_out,
-                                                     float4* __restrict__ G, int first, int gemu) {
+                                                     float4* __restrict__ G, int first) {
     __shared__ float red[4][BWD_CHUNK][4];
     const long long j = blockIdx.x;
     const int f = threadIdx.x;
@@ -145,22 +133,22 @@ __global__ void __launch_bounds__(128) k_message_bwd(long long N, int F, int K, 
             const float fc = dummy ? 0.0f : 0.5f * (1.0f + c1);
             const float dfc = dummy ? 0.0f : -0.5f * a1 * s1;
             // w = Wf (fc rho) + bf fc ;  w' = Wf (fc' rho + fc rho') + bf fc'   (both as GEMM operands)
-            float wS_ = fdot<EMU>(bS, fc, 0.f), wVS_ = fdot<EMU>(bVS, fc, 0.f), wVV_ = fdot<EMU>(bVV, fc, 0.f);
-            float dwS = fdot<EMU>(bS, dfc, 0.f), dwVS = fdot<EMU>(bVS, dfc, 0.f), dwVV = fdot<EMU>(bVV, dfc, 0.f);
+            float wS_ = fmaf(bS, fc, 0.f), wVS_ = fmaf(bVS, fc, 0.f), wVV_ = fmaf(bVV, fc, 0.f);
+            float dwS = fmaf(bS, dfc, 0.f), dwVS = fmaf(bVS, dfc, 0.f), dwVV = fmaf(bVV, dfc, 0.f);
 #pragma unroll
             for (int n = 0; n < KMAX; n++) {
                 const float rho = sn_ * inv_d;
                 const float drho = ((float)(n + 1) * a1 * cn_ - rho) * inv_d;   // (n pi/rc) cos/d - sin/d^2
                 const float r0 = fc * rho, r1 = dfc * rho + fc * drho;
-                wS_ = fdot<EMU>(wS[n], r0, wS_); wVS_ = fdot<EMU>(wVS[n], r0, wVS_); wVV_ = fdot<EMU>(wVV[n], r0, wVV_);
-                dwS = fdot<EMU>(wS[n], r1, dwS); dwVS = fdot<EMU>(wVS[n], r1, dwVS); dwVV = fdot<EMU>(wVV[n], r1, dwVV);
+                wS_ = fmaf(wS[n], r0, wS_); wVS_ = fmaf(wVS[n], r0, wVS_); wVV_ = fmaf(wVV[n], r0, wVV_);
+                dwS = fmaf(wS[n], r1, dwS); dwVS = fmaf(wVS[n], r1, dwVS); dwVV = fmaf(wVV[n], r1, dwVV);
                 const float t = sn_ * c1 + cn_ * s1;
                 cn_ = cn_ * c1 - sn_ * s1;
                 sn_ = t;
             }
-            const float sbi = gq(s1b[(size_t)i * F + f], gemu);
-            const float vb0 = gq(v1b[(size_t)i * F3 + f], gemu), vb1 = gq(v1b[(size_t)i * F3 + F + f], gemu),
-                        vb2 = gq(v1b[(size_t)i * F3 + 2 * F + f], gemu);
+            const float sbi = s1b[(size_t)i * F + f];
+            const float vb0 = v1b[(size_t)i * F3 + f], vb1 = v1b[(size_t)i * F3 + F + f],
+                        vb2 = v1b[(size_t)i * F3 + 2 * F + f];
             const float X = vb0 * ux + vb1 * uy + vb2 * uz;
             const float Z = vb0 * vj0 + vb1 * vj1 + vb2 * vj2;
             pbS += wS_ * sbi;
@@ -207,11 +195,9 @@ void message_bwd(const Launch& L, long long N, int F, int K, float rc, const int
                  const float* bf, float* phib, float* vb_out, float4* G, bool first) {
     if (N == 0) return;
     unsigned grid = (unsigned)N;
-#define MB(KM, EM) k_message_bwd<KM, EM><<<grid, F, 0, L.stream>>>(N, F, K, 1.0f / rc, row_ptr, ej, s1b, v1b, phi, v_in, Wf, bf, phib, vb_out, G, first ? 1 : 0, g_gather_emulate)
-#define MBK(EM) do { if (K <= 16) MB(16, EM); else if (K <= 20) MB(20, EM); else MB(32, EM); } while (0)
-    switch (g_filter_emulate) { case 1: MBK(1); break; case 2: MBK(2); break; case 3: MBK(3); break; default: MBK(0); }
+#define MB(KM) k_message_bwd<KM><<<grid, F, 0, L.stream>>>(N, F, K, 1.0f / rc, row_ptr, ej, s1b, v1b, phi, v_in, Wf, bf, phib, vb_out, G, first ? 1 : 0)
+    if (K <= 16) MB(16); else if (K <= 20) MB(20); else MB(32);
 #undef MB
-#undef MBK
     KLAUNCH(L);
 }
 

@@ -58,28 +58,13 @@ void mul_dsilu(const Launch& L, long long n, const float* pre, float* g) {
 }
 
 // ------------------------------------------------------------------------------------------------ a4 + a7
-// Debug knobs (mlp_set_option "filter_emulate" / "gather_emulate"): emulate reduced-precision operands of the
-// tensor-core filter GEMM (1: fp16 operands, 2: fp16 hi+lo split with 3 product terms, 3: bf16 operands) and
-// reduced-precision storage of the gathered rows (1: fp16, 2: bf16); used to size the precision plan.
-int g_filter_emulate = 0, g_gather_emulate = 0;
-__device__ __forceinline__ float r_h(float x) { return __half2float(__float2half_rn(x)); }
-__device__ __forceinline__ float r_b(float x) { return __bfloat162float(__float2bfloat16_rn(x)); }
-template <int EMU> __device__ __forceinline__ float fdot(float w, float r, float acc) {
-    if (EMU == 0) return fmaf(w, r, acc);
-    if (EMU == 1) return fmaf(r_h(w), r_h(r), acc);
-    if (EMU == 3) return fmaf(r_b(w), r_b(r), acc);
-    float wh = r_h(w), wl = r_h(w - wh), rh = r_h(r), rl = r_h(r - rh);
-    return fmaf(wl, rh, fmaf(wh, rh + rl, acc));
-}
-__device__ __forceinline__ float gq(float x, int g) { return g == 0 ? x : (g == 1 ? r_h(x) : r_b(x)); }
-
-template <int KMAX, int EMU>
+template <int KMAX>
 __global__ void __launch_bounds__(128) k_message_fwd(long long N, int F, int K, float inv_rc,
                                                      const int* __restrict__ row_ptr,
                                                      const float4* __restrict__ ej, const float* __restrict__ s,
                                                      const float* __restrict__ v, const float* __restrict__ phi,
                                                      const float* __restrict__ Wf, const float* __restrict__ bf,
-                                                     float* __restrict__ sn, float* __restrict__ v1, int gemu) {
+                                                     float* __restrict__ sn, float* __restrict__ v1) {
     const long long a = blockIdx.x * (long long)blockDim.y + threadIdx.y;
     const int f = threadIdx.x;
     if (a >= N) return;
@@ -107,13 +92,13 @@ __global__ void __launch_bounds__(128) k_message_fwd(long long N, int F, int K, 
         float sn_ = s1, cn_ = c1;
         const float fc = 0.5f * (1.0f + c1);
         // w = fc (Wf rho + bf) = Wf (fc rho) + bf fc : the cutoff is folded into the GEMM operand
-        float linS = fdot<EMU>(bS, fc, 0.f), linVS = fdot<EMU>(bVS, fc, 0.f), linVV = fdot<EMU>(bVV, fc, 0.f);
+        float linS = fmaf(bS, fc, 0.f), linVS = fmaf(bVS, fc, 0.f), linVV = fmaf(bVV, fc, 0.f);
 #pragma unroll
         for (int n = 0; n < KMAX; n++) {
             const float rho = fc * sn_ * inv_d;
-            linS = fdot<EMU>(wS[n], rho, linS);
-            linVS = fdot<EMU>(wVS[n], rho, linVS);
-            linVV = fdot<EMU>(wVV[n], rho, linVV);
+            linS = fmaf(wS[n], rho, linS);
+            linVS = fmaf(wVS[n], rho, linVS);
+            linVV = fmaf(wVV[n], rho, linVV);
             const float t = sn_ * c1 + cn_ * s1;
             cn_ = cn_ * c1 - sn_ * s1;
             sn_ = t;
@@ -121,12 +106,12 @@ __global__ void __launch_bounds__(128) k_message_fwd(long long N, int F, int K, 
         const float* pj = phi + (size_t)j * F3;
         const float* vj = v + (size_t)j * F3;
         const float pvv = pj[2 * F + f];
-        const float xs = linS * gq(pj[f], gemu);
-        const float xvs = linVS * gq(pj[F + f], gemu);
+        const float xs = linS * pj[f];
+        const float xvs = linVS * pj[F + f];
         accS += xs;
-        accV0 += xvs * (r.x * inv_d) + linVV * gq(pvv * vj[f], gemu);
-        accV1 += xvs * (r.y * inv_d) + linVV * gq(pvv * vj[F + f], gemu);
-        accV2 += xvs * (r.z * inv_d) + linVV * gq(pvv * vj[2 * F + f], gemu);
+        accV0 += xvs * (r.x * inv_d) + linVV * pvv * vj[f];
+        accV1 += xvs * (r.y * inv_d) + linVV * pvv * vj[F + f];
+        accV2 += xvs * (r.z * inv_d) + linVV * pvv * vj[2 * F + f];
     }
     sn[a * 2 * F + f] = accS;
     v1[a * F3 + f] = accV0; v1[a * F3 + F + f] = accV1; v1[a * F3 + 2 * F + f] = accV2;
@@ -138,11 +123,9 @@ void message_fwd(const Launch& L, long long N, int F, int K, float rc, const int
     if (N == 0) return;
     dim3 block(F, 128 / F);
     unsigned grid = (unsigned)((N + block.y - 1) / block.y);
-#define MF(KM, EM) k_message_fwd<KM, EM><<<grid, block, 0, L.stream>>>(N, F, K, 1.0f / rc, row_ptr, ej, s, v, phi, Wf, bf, sn, v1, g_gather_emulate)
-#define MFK(EM) do { if (K <= 16) MF(16, EM); else if (K <= 20) MF(20, EM); else MF(32, EM); } while (0)
-    switch (g_filter_emulate) { case 1: MFK(1); break; case 2: MFK(2); break; case 3: MFK(3); break; default: MFK(0); }
+#define MF(KM) k_message_fwd<KM><<<grid, block, 0, L.stream>>>(N, F, K, 1.0f / rc, row_ptr, ej, s, v, phi, Wf, bf, sn, v1)
+    if (K <= 16) MF(16); else if (K <= 20) MF(20); else MF(32);
 #undef MF
-#undef MFK
     KLAUNCH(L);
 }
 

@@ -24,12 +24,12 @@ def test_paper_shapes_four_layers(F):
     _check(c, e, f, w, ref, f"config 2 recipe, PaiNN 4 x {F} (N={len(c['pos'])}, E={ne})")
 
 
-@pytest.mark.parametrize("opts", [dict(edge_path=1), dict(edge_path=2), dict(gemm_fwd_exact=0), dict(gemm_bwd_exact=1),
-                                  dict(l0_collapse=0), dict(fwd_groups=0), dict(atoms_per_unit=5), dict(atoms_per_unit=31), dict(cell_strip=0), dict(cell_strip=1), dict(cell_strip=4)])
+@pytest.mark.parametrize("opts", [dict(edge_path=1), dict(gemm_fwd_exact=0), dict(gemm_bwd_exact=1),
+                                  dict(l0_collapse=0), dict(atoms_per_unit=5), dict(atoms_per_unit=31), dict(cell_strip=0), dict(cell_strip=1), dict(cell_strip=4)])
 def test_alternative_kernel_paths_match_oracle(opts):
     """Every switch of mlp_set_option selects another implementation of the same arithmetic; each must meet the same
-    tolerances (the plain fp32 edge kernels, the first-generation tensor-core edge kernels, the fp32 FFMA forward GEMM, the
-    exact-slice adjoint GEMM)."""
+    tolerances (the plain fp32 edge kernels, the fp32 FFMA forward GEMM, the exact-slice adjoint GEMM, the per-edge layer-0
+    kernels, other work-unit sizes and cell orders).  Options belong to the model they are set on."""
     import paper_2506_04055_b200 as P
     torch = _torch()
     c = gen.make_config(5, n_slots=1200, L=32.98)
@@ -41,8 +41,6 @@ def test_alternative_kernel_paths_match_oracle(opts):
         e, f, w = m.compute(torch.from_numpy(c["pos"]).to(dev), torch.from_numpy(c["types"]).to(dev), c["box"])
         torch.cuda.synchronize()
         e, f, w = float(e[0]), f.cpu().numpy(), w.cpu().numpy()
-        m.set_option("gemm_bwd_exact", 0)
-        m.set_option("atoms_per_unit", 0)                  # process-wide knobs: back to the defaults
     ref = _oracle_eval(c, blob)
     _check(c, e, f, w, ref, f"config 5 recipe reduced, options {opts}")
 

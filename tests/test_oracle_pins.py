@@ -77,9 +77,10 @@ def test_forces_match_finite_differences_config1(cfg1):
 
 
 # ------------------------------------------------------------------ dense autograd restatement
-def _dense_energy_torch(arrs, hdr, pos, types, box, n_local, periodic):
+def _dense_energy_torch(arrs, hdr, pos, types, box, n_local, periodic, states=None):
     """Independent restatement of SURVEY.md §8(c) Forward with dense masked pair tensors (no edge lists,
-    no hand adjoint).  pos: torch fp64 [N,3] requiring grad; box torch [3]."""
+    no hand adjoint).  pos: torch fp64 [N,3] requiring grad; box torch [3].  `states` (a list) receives the layer
+    states (s [N,F], v [N,3,F]) after the embedding and after every layer."""
     import torch
     F, K, T, rc, eps = hdr["F"], hdr["K"], hdr["T"], hdr["rc"], hdr["eps"]
     N = pos.shape[0]
@@ -103,6 +104,8 @@ def _dense_energy_torch(arrs, hdr, pos, types, box, n_local, periodic):
     silu = torch.nn.functional.silu
     s = W["Emb"][torch.as_tensor(types, dtype=torch.long)]                                  # [N,F]
     v = torch.zeros(N, 3, F, dtype=torch.float64)
+    if states is not None:
+        states.append((s, v))
     for t in range(T):
         p_ = f"L{t}."
         phi = silu(s @ W[p_ + "Wm1"].T + W[p_ + "bm1"]) @ W[p_ + "Wm2"].T + W[p_ + "bm2"]  # [N,3F]
@@ -120,6 +123,8 @@ def _dense_energy_torch(arrs, hdr, pos, types, box, n_local, periodic):
         avv, asv, ass = a[:, :F], a[:, F:2 * F], a[:, 2 * F:]
         v = v1 + avv[:, None, :] * p
         s = s1 + asv * D + ass
+        if states is not None:
+            states.append((s, v))
     Ei = silu(s @ W["Wr1"].T + W["br1"]) @ W["wr2"] + W["br2"]
     return Ei[:n_local].sum(), Ei
 
@@ -139,6 +144,29 @@ def test_dense_autograd_restatement(periodic):
     assert abs(E.item() - r["energy"]) <= 1e-10 * max(1, abs(r["energy"]))
     np.testing.assert_allclose(Ei.detach().numpy(), r["atom_energy"], rtol=0, atol=1e-10)
     np.testing.assert_allclose(-gP.numpy(), r["forces"], rtol=0, atol=1e-9)
+
+
+@pytest.mark.parametrize("periodic", [True, False])
+def test_state_dump_matches_dense_restatement(periodic):
+    """Pin of the oracle's `state_dump` export (the reference of every layer-state assertion of the GPU tests):
+    [(T+1) x N x 4F] = (s | v_x | v_y | v_z) after the embedding and after each layer, against the per-layer s, v of the
+    dense restatement.  A wrong stride, layer offset or component order fails here."""
+    import torch
+    pos, types, box = _small_water()
+    blob = _blob(SMALL_MODEL)
+    hdr, arrs = gen.parse_blob(blob)
+    N, F, T = len(pos), hdr["F"], hdr["T"]
+    n_local = N if periodic else N - 9
+    r = oracle.compute(blob, pos, types, box, n_local=n_local, n_ghost=N - n_local, periodic=periodic, want_states=True)
+    st = []
+    _dense_energy_torch(arrs, hdr, torch.tensor(pos, dtype=torch.float64), types, torch.tensor(box), n_local, periodic, st)
+    assert r["states"].shape == (T + 1, N, 4 * F) and len(st) == T + 1
+    for t, (s_t, v_t) in enumerate(st):
+        np.testing.assert_allclose(r["states"][t, :, :F], s_t.numpy(), rtol=0, atol=1e-10)
+        for c in range(3):
+            np.testing.assert_allclose(r["states"][t, :, (1 + c) * F:(2 + c) * F], v_t[:, c, :].numpy(), rtol=0, atol=1e-10)
+    assert np.abs(r["states"][0, :, F:]).max() == 0.0            # v^0 = 0
+    assert np.abs(r["states"][T, :, F:]).max() > 0.0             # and the vector channels are not all zero later
 
 
 def test_dense_autograd_virial_open_mode():
@@ -389,6 +417,26 @@ def test_unwrapped_positions_need_wider_image_range():
     a = set(zip(i0.tolist(), j0.tolist(), map(tuple, S0.tolist())))
     b = set(zip(i1.tolist(), j1.tolist(), map(tuple, (S1 + (w[j1] - w[i1])).astype(int).tolist())))
     assert a == b
+
+
+def test_block_decomposition_of_the_fullsize_goldens_is_exact(cfg1, tmp_path):
+    """tests/golden/make_golden_fullsize.py sums the oracle over blocks of local atoms with a T * rc halo of ghosts
+    (PAPER.md:58, 64-66).  On config 1 (box 12.42 A < halo: up to 27 + images of an atom inside one block's halo) the
+    2 x 2 x 2 block sum must reproduce the periodic whole-system oracle: E, the virial and every force."""
+    import importlib.util
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "make_golden_fullsize.py")
+    spec = importlib.util.spec_from_file_location("make_golden_fullsize", path)
+    G = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(G)
+    E, W6, F = G.run(1, 2, 10.0, 8, str(tmp_path / "g.json"), log=lambda s: None)     # T rc = 10 A for the 2-layer model
+    ref = oracle.compute(cfg1["blob"], cfg1["pos"], cfg1["types"], cfg1["box"])
+    assert abs(E - ref["energy"]) <= 1e-10 * abs(ref["energy"])
+    np.testing.assert_allclose(W6, ref["virial"], rtol=0, atol=1e-9 * np.abs(ref["virial"]).max())
+    np.testing.assert_allclose(F, ref["forces"], rtol=0, atol=1e-9 * np.abs(ref["forces"]).max())
+    import json
+    doc = json.load(open(tmp_path / "g.json"))
+    assert doc["energy"] == E and len(doc["sample_idx"]) == 8 and doc["meta"]["blocks"] == [2, 2, 2]
 
 
 def test_oracle_reproduces_golden_config1():
