@@ -54,6 +54,10 @@ typedef struct mlp_stats {
     long long n_calls;        /* mlp_compute calls since mlp_create                                      */
     long long n_launches;     /* kernels launched by the last call                                       */
     long long device_bytes;   /* device memory currently held by the model                               */
+    long long n_list_rebuilds;  /* calls that built the neighbour list from scratch (PAPER.md:68 skin)     */
+    long long n_list_reuses;    /* calls served by the kept rc + skin list (re-filtered at rc)              */
+    long long n_graph_replays;  /* of those, calls replayed from the captured CUDA graph                    */
+    long long n_reached;        /* atoms kept by the T-hop pruning of a ghost-mode graph (else n_atoms)     */
 } mlp_stats;
 
 /*

@@ -27,7 +27,9 @@ class MLPError(RuntimeError):
 class _Stats(C.Structure):
     _fields_ = [("n_atoms", C.c_longlong), ("n_edges", C.c_longlong), ("atom_capacity", C.c_longlong),
                 ("edge_capacity", C.c_longlong), ("n_cells", C.c_longlong * 3), ("n_regrow", C.c_longlong),
-                ("n_calls", C.c_longlong), ("n_launches", C.c_longlong), ("device_bytes", C.c_longlong)]
+                ("n_calls", C.c_longlong), ("n_launches", C.c_longlong), ("device_bytes", C.c_longlong),
+                ("n_list_rebuilds", C.c_longlong), ("n_list_reuses", C.c_longlong), ("n_graph_replays", C.c_longlong),
+                ("n_reached", C.c_longlong)]
 
 
 _lib = None

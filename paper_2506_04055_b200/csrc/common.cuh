@@ -43,7 +43,28 @@ __host__ __device__ __forceinline__ void cell_decode(const Grid& g, int cell, in
 }
 
 // error flags written by the device (bit mask in flags[0])
-enum { FLAG_TYPE_RANGE = 1, FLAG_NONFINITE = 2, FLAG_EDGE_OVERFLOW = 4, FLAG_OWNER_RANGE = 8 };
+enum { FLAG_TYPE_RANGE = 1, FLAG_NONFINITE = 2, FLAG_EDGE_OVERFLOW = 4, FLAG_OWNER_RANGE = 8, FLAG_REBUILD = 16 };
+#define LEVEL_NONE 255     // hop level of an atom no local atom reaches within T hops
+
+// Cell-sorted search structure of one neighbour build and the optional relabelling into the final atom order.
+struct NbrSearch {
+    const double* pos;          // [N][3] positions as given, cell-sorted
+    const signed char* wrap;    // [N][3] wrap counts
+    const int* cell;            // [N] cell of each atom
+    const int* cell_start;      // [n_cells + 1]
+    const int* new_of_old;      // final index of cell-sorted atom b (< 0: dropped), or nullptr = identity
+    const int* old_of_new;      // cell-sorted index of final row a, or nullptr = identity
+    double cut2;                // (list cutoff)^2: rc^2, or (rc + skin)^2 for the superset list
+};
+// Where a CSR slot is written (nbr.cu::emit_edge)
+struct EdgeOut {
+    float4* ej;                 // (r_e fp32, sender index bits)
+    unsigned char* img;         // image code, 255 = padding slot
+    int* key;                   // (sender << 5 | code) search key of the reverse pass, or nullptr
+    float2* xph;                // compensated phase d / rc as (hi, lo), or nullptr
+    double inv_rc;
+    float rc;
+};
 
 struct LayerW {
     const float *Wm1, *bm1, *Wm2, *bm2, *Wf, *bf, *UV, *Wu1, *bu1, *Wu2, *bu2;   // [out x in] row-major
@@ -82,11 +103,27 @@ void nbr_sort_cells(const Launch& L, long long ncells, const int* cell_start, in
 void nbr_gather(const Launch& L, long long N, long long n_local, const int* perm, const double* pos,
                 const int* types, const signed char* wrap, double* pos_s, int* types_s, signed char* wrap_s,
                 int* inv_perm, float* local_mask, const int* cell_id, int* cell_s);
-void nbr_count(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s,
-               const int* cell_s, const int* cell_start, int* row_cnt, unsigned long long* real_total);
-void nbr_fill(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s,
-              const int* cell_s, const int* cell_start, const int* row_ptr, long long cap_edges, float rc, float4* ej,
-              unsigned char* img, int* key, int* flags);
+void nbr_count(const Launch& L, long long N, Grid g, const NbrSearch& S, const int* n_rows_p, int* row_cnt,
+               unsigned long long* real_total);
+void nbr_fill(const Launch& L, long long N, Grid g, const NbrSearch& S, const int* n_rows_p, const int* row_ptr,
+              long long cap_edges, EdgeOut o, int* flags);
+void nbr_levels(const Launch& L, long long N, Grid g, const NbrSearch& S, const float* local_mask, unsigned char* level, int T);
+void nbr_level_sort(const Launch& L, long long N, const unsigned char* level, int T, int* hist, long long* prefix,
+                    int* new_of_old, int* old_of_new);
+void nbr_regather(const Launch& L, long long N, const int* old_of_new, const double* posC, const int* typesC,
+                  const signed char* wrapC, const int* permC, const float* localC, double* pos_s, int* types_s,
+                  signed char* wrap_s, int* perm, int* inv_perm, float* local_mask);
+void nbr_sup_count(const Launch& L, long long N, Grid g, const NbrSearch& S, const int* n_rows_p, int* row_cnt,
+                   unsigned long long* padded_total);
+void nbr_sup_fill(const Launch& L, long long N, Grid g, const NbrSearch& S, const int* n_rows_p, const int* sup_ptr, int* sup_j,
+                  unsigned char* sup_code);
+void nbr_refilter_count(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s, const int* sup_ptr,
+                        const int* sup_j, const unsigned char* sup_code, int* row_cnt, unsigned long long* real_total);
+void nbr_refilter_fill(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s, const int* sup_ptr,
+                       const int* sup_j, const unsigned char* sup_code, const int* row_ptr, long long cap_edges, EdgeOut o, int* flags);
+void nbr_reuse_prep(const Launch& L, long long N, const int* perm, const double* pos, const int* types, const double* pos_ref_s,
+                    const signed char* wrap_ref_s, const int* types_s, Grid g, double half_skin2, double* pos_s, signed char* wrap_s,
+                    int* flags);
 void nbr_reverse(const Launch& L, long long N, const int* row_ptr, const float4* ej, const unsigned char* img,
                  const int* key, int* rev, int* miss);
 void nbr_export(const Launch& L, long long N, const int* row_ptr, const float4* ej, const unsigned char* img,
@@ -143,7 +180,7 @@ void make_gather_rows(const Launch& L, long long N, const float* phi, const floa
 void make_gather_rows_bwd(const Launch& L, long long N, const float* s1b, const float* v1b, float* Gb);
 bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* s,
                     const float* v, const float* Q4, const float* Q1, const void* A_img, const void* A_rows, float* sn, float* v1,
-                    bool has_v, const int* types_s, const float* tab, int n_tab);
+                    bool has_v, const int* types_s, const float* tab, int n_tab, const float2* xph);
 bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
                     const float* phi, const float* v_in, const float* v1b, const void* A_img, const void* A_rows, float* phib,
                     float* vb_out, float4* G, bool first, bool layer0);
@@ -154,7 +191,7 @@ bool message_bwd0_v3(const Launch& L, long long N, int K, float rc, const int* r
 // ---- layer 0 with the channels contracted outside the edge loop (edge_l0.cu) ----
 bool message_fwd0_collapsed_accum(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej,
                                   const int* types_s, int n_species, const float* s_in, int F, float* sn, int ldsn, float* As,
-                                  float* Av, int NP);
+                                  float* Av, int NP, const float2* xph);
 bool message_bwd0_collapsed(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej,
                             const int* types_s, int n_species, const int* rev, const float* Bv, const float* Cs, int NP,
                             float4* G, bool first);

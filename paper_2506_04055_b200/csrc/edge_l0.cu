@@ -103,11 +103,13 @@ __global__ void __launch_bounds__(WARPS * 32) k_l0_bwd(long long N, const int* _
 // Writes As [N][NP] = Rs, Av [3N][NP] = Q (row 3 i + component) and copies s_i into the s' half of sn (ldsn floats per
 // row), to which the first GEMM accumulates.
 // ---------------------------------------------------------------------------------------------------------------
+constexpr float PI_F = 3.14159265358979323846f;
 constexpr int RLD = 25;            // row stride of the per-edge radial values (odd: conflict-free both ways)
 __global__ void __launch_bounds__(WARPS * 32) k_l0_fwd(long long N, const int* __restrict__ row_ptr, const float4* __restrict__ ej,
                                                       const int* __restrict__ types, const float* __restrict__ s_in, int F,
                                                       float* __restrict__ sn, int ldsn, float* __restrict__ As,
-                                                      float* __restrict__ Av, int NP, int n_used, int K, float inv_rc) {
+                                                      float* __restrict__ Av, int NP, int n_used, int K, float inv_rc,
+                                                      const float2* __restrict__ xph) {
     extern __shared__ float4 sm[];       // [WARPS][n_used] accumulators | [WARPS][32] (u, species offset) | [WARPS][32][RLD] R_k
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     float4* acc = sm + warp * n_used;
@@ -126,10 +128,12 @@ __global__ void __launch_bounds__(WARPS * 32) k_l0_fwd(long long N, const int* _
             if (E < e1) r = __ldg(ej + E);
             const int jb = __float_as_int(r.w);
             const float d2 = r.x * r.x + r.y * r.y + r.z * r.z;
-            const float inv_d = rsqrtf(d2);
-            const float x = d2 * inv_d * inv_rc;
+            const float inv_d = 1.0f / sqrtf(d2);                 // IEEE: rsqrtf's 2 ulp would go straight into u and rho
+            float x = d2 * inv_d * inv_rc, xl = 0.f;
+            if (xph != nullptr && E < e1) { const float2 xp = __ldg(xph + E); x = xp.x; xl = xp.y * PI_F; }   // compensated phase (nbr.cu)
             float s1, c1;
             sincospif(x, &s1, &c1);
+            { const float t = fmaf(xl, c1, s1); c1 = fmaf(-xl, s1, c1); s1 = t; }
             const float fc = jb >= 0 ? 0.5f * (1.0f + c1) : 0.0f;                  // padding slots: zero weight
             const int z = jb >= 0 ? __ldg(types + jb) : 0;
             __syncwarp();
@@ -139,7 +143,12 @@ __global__ void __launch_bounds__(WARPS * 32) k_l0_fwd(long long N, const int* _
             const float amp = fc * inv_d;
             float sn_ = s1, cn_ = c1;
             for (int b = 1; b <= K; b++) {
-                if ((b & 7) == 0) sincospif((float)b * x, &sn_, &cn_);
+                if ((b & 7) == 0) {
+                    sincospif((float)b * x, &sn_, &cn_);
+                    const float t = fmaf((float)b * xl, cn_, sn_);
+                    cn_ = fmaf(-(float)b * xl, sn_, cn_);
+                    sn_ = t;
+                }
                 rb[b] = amp * sn_;
                 const float tt = fmaf(sn_, c1, cn_ * s1);
                 cn_ = fmaf(cn_, c1, -sn_ * s1);
@@ -173,7 +182,7 @@ __global__ void __launch_bounds__(WARPS * 32) k_l0_fwd(long long N, const int* _
 
 bool message_fwd0_collapsed_accum(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej,
                                   const int* types_s, int n_species, const float* s_in, int F, float* sn, int ldsn, float* As,
-                                  float* Av, int NP) {
+                                  float* Av, int NP, const float2* xph) {
     using namespace el0;
     if (N == 0) return true;
     const int n_used = n_species * (K + 1);
@@ -188,7 +197,7 @@ bool message_fwd0_collapsed_accum(const Launch& L, long long N, int K, float rc,
     }
     const long long want = (N + WARPS - 1) / WARPS;
     const int grid = (int)(want < (long long)n_sm * 8 ? want : (long long)n_sm * 8);
-    k_l0_fwd<<<grid, WARPS * 32, smem, L.stream>>>(N, row_ptr, ej, types_s, s_in, F, sn, ldsn, As, Av, NP, n_used, K, 1.0f / rc);
+    k_l0_fwd<<<grid, WARPS * 32, smem, L.stream>>>(N, row_ptr, ej, types_s, s_in, F, sn, ldsn, As, Av, NP, n_used, K, 1.0f / rc, xph);
     KLAUNCH(L);
     return true;
 }

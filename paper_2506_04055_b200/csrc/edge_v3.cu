@@ -51,6 +51,7 @@ constexpr int A_CHUNK_BYTES = (F / 8) * SBO;            // 24576
 struct EdgeGeom {
     float4 r;        // (r_e, sender index bits)
     float inv_d, s1, c1, x;
+    float xl;        // pi * x_lo of the compensated phase (0 without it)
     bool real;
 };
 // The record of the NEXT tile's edge is fetched while the current tile is evaluated (load_edge_raw / edge_geom): a
@@ -60,16 +61,29 @@ __device__ __forceinline__ float4 load_edge_raw(const float4* __restrict__ ej, i
     if (E < e_end) r = __ldg(ej + E);
     return r;
 }
-__device__ __forceinline__ EdgeGeom edge_geom(const float4 raw, int E, int e_end, float inv_rc) {
+// xp = (x_hi, x_lo) of nbr.cu::phase_pair, or x_hi < 0: no compensated phase, x from the fp32 record
+__device__ __forceinline__ float2 load_phase(const float2* __restrict__ xph, int E, int e_end) {
+    float2 x = make_float2(-1.f, 0.f);
+    if (xph != nullptr && E < e_end) x = __ldg(xph + E);
+    return x;
+}
+template <bool ACC = false>
+__device__ __forceinline__ EdgeGeom edge_geom(const float4 raw, int E, int e_end, float inv_rc,
+                                              const float2 xp = make_float2(-1.f, 0.f)) {
     EdgeGeom g;
     g.r = raw;
     const bool valid = E < e_end;
     g.real = valid && __float_as_int(g.r.w) >= 0;                 // padding slots carry sender index ~self
     if (valid && !g.real) g.r.w = __int_as_float(~__float_as_int(g.r.w));
     const float d2 = g.r.x * g.r.x + g.r.y * g.r.y + g.r.z * g.r.z;
-    g.inv_d = rsqrtf(d2);
+    g.inv_d = ACC ? 1.0f / sqrtf(d2) : rsqrtf(d2);        // forward (energy) path: IEEE, rsqrtf's 2 ulp go straight into u and rho
     g.x = d2 * g.inv_d * inv_rc;
+    g.xl = 0.f;
+    if (xp.x >= 0.f) { g.x = xp.x; g.xl = xp.y * 3.14159265358979323846f; }
     sincospif(g.x, &g.s1, &g.c1);
+    const float ts = fmaf(g.xl, g.c1, g.s1);                      // sin(pi (x_hi + x_lo)) to first order in x_lo
+    g.c1 = fmaf(-g.xl, g.s1, g.c1);
+    g.s1 = ts;
     return g;
 }
 // Split 8 fp32 values x = hi + r (hi = RN_fp16(x), r exact in fp32) into the four fp16 planes of the B operand, one per
@@ -125,6 +139,7 @@ struct FwdParams {
     const int* types;      // [N] species of the (cell-sorted) atoms
     const float2* tab;     // [n_tab][F] (phi^s, phi^vs) per species
     int n_tab;
+    const float2* xph;     // [edges] compensated phase x = d / rc as (hi, lo) from the fp64 neighbour build, or nullptr
 };
 
 constexpr int TAB_MAX = 16;                             // species rows the shared-memory table can hold
@@ -395,15 +410,27 @@ __global__ void __launch_bounds__(FWDG_THREADS, 1) k_msg_fwd_g(const FwdParams p
             const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
             const int ntiles = (e_end - e_begin + NE - 1) / NE;
             float4 raw_n = load_edge_raw(p.ej, e_begin + e, e_end);
+            float2 xp_n = load_phase(p.xph, e_begin + e, e_end);
             for (int t = 0; t < ntiles; t++, it++) {
                 const int buf = it & 1;
                 const float4 raw = raw_n;
-                if (t + 1 < ntiles) raw_n = load_edge_raw(p.ej, e_begin + (t + 1) * NE + e, e_end);
-                const EdgeGeom g = edge_geom(raw, e_begin + t * NE + e, e_end, inv_rc);
+                const float2 xp = xp_n;
+                if (t + 1 < ntiles) {
+                    raw_n = load_edge_raw(p.ej, e_begin + (t + 1) * NE + e, e_end);
+                    xp_n = load_phase(p.xph, e_begin + (t + 1) * NE + e, e_end);
+                }
+                const EdgeGeom g = edge_geom<true>(raw, e_begin + t * NE + e, e_end, inv_rc, xp);
                 const float fc = g.real ? 0.5f * (1.0f + g.c1) : 0.0f;
                 const float amp = fc * g.inv_d;
                 float sn_, cn_;
-                if (h == 0) { sn_ = g.s1; cn_ = g.c1; } else sincospif((float)(8 * h) * g.x, &sn_, &cn_);
+                if (h == 0) { sn_ = g.s1; cn_ = g.c1; }
+                else {
+                    sincospif((float)(8 * h) * g.x, &sn_, &cn_);
+                    const float dl = (float)(8 * h) * g.xl;              // first-order phase correction (pi x_lo)
+                    const float ts = fmaf(dl, cn_, sn_);
+                    cn_ = fmaf(-dl, sn_, cn_);
+                    sn_ = ts;
+                }
                 float vals[8];
 #pragma unroll
                 for (int i = 0; i < 8; i++) {
@@ -1295,7 +1322,7 @@ static int sm_count() {
 // layer 0 through the species table.
 bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* s,
                     const float* v, const float* Q4, const float* Q1, const void* A_img, const void* A_rows, float* sn, float* v1,
-                    bool has_v, const int* types_s, const float* tab, int n_tab) {
+                    bool has_v, const int* types_s, const float* tab, int n_tab, const float2* xph) {
     using namespace ev3;
     if (N == 0) return true;
     if (K > 23 || !A_rows || !A_img) return false;
@@ -1308,7 +1335,7 @@ bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
         attr = true;
     }
     FwdParams p{N, row_ptr, ej, s, v, (const float4*)Q4, Q1, (const float2*)Q4, (const uint4*)A_img, (const uint4*)A_rows, sn, v1,
-                1.0f / rc, K, L.apu_fwd, types_s, (const float2*)tab, n_tab};
+                1.0f / rc, K, L.apu_fwd, types_s, (const float2*)tab, n_tab, xph};
     const long long n_units = (N + p.atoms_per_unit - 1) / p.atoms_per_unit;
     // one CTA per SM, two 8-warp pipelines sharing the TMEM-resident filter operand
     const int grid = (int)std::min<long long>((n_units + 1) / 2, (long long)sm_count());

@@ -284,8 +284,8 @@ constexpr int XW_TILE = XBN * 128;                                      // 4 KB:
 constexpr int XW_STAGE = 3 * 2 * XW_TILE;                               // 24 KB: the three weight slices of one N tile, K = 128
 constexpr int XNMAX = 512;                                              // widest N (column scale and bias are staged in shared memory)
 constexpr int XSMEM = XRAW * A_TILE_BYTES + XWST * XW_STAGE + 4 * BM * 4 + 2 * XNMAX * 4 + 256 + 4 * 32 * EPI_LD * 4 + 1024;
-constexpr int XTM_A = 0;                                                // TMEM columns 0..191: A slices [3][64 columns = 128 fp16]
-constexpr int XTM_ACC = 192, XACC = 4 * XBN;                            // TMEM columns 192..447: 2 accumulator sets (S2..S5 x 32)
+constexpr int XTM_A = 0;                                                // TMEM columns 0..255: A slices [4][64 columns = 128 fp16]
+constexpr int XTM_ACC = 256, XACC = 4 * XBN;                            // TMEM columns 256..511: 2 accumulator sets (S2..S5 x 32)
 
 struct XParams {
     float* C;
@@ -429,9 +429,9 @@ __global__ void __launch_bounds__(XTHREADS, 1)
 #pragma unroll
                             for (int kk = 0; kk < 4; kk++) {             // 16 fp16 along K = 8 TMEM columns of A, 32 B of a W row
                                 const uint64_t o = (uint64_t)(kk * 2);
-                                const uint32_t a0 = ta + kh * 32 + kk * 8, a1 = a0 + 64, a2 = a0 + 128;
+                                const uint32_t a0 = ta + kh * 32 + kk * 8, a1 = a0 + 64, a2 = a0 + 128, a3 = a0 + 192;
                                 const uint32_t acc = (kh | kk) != 0;
-                                // S2: (1,1)   S3: (1,2) (2,1)   S4: (1,3) (2,2) (3,1)   S5: (2,3) (3,2)
+                                // S2: (1,1)   S3: (1,2) (2,1)   S4: (1,3) (2,2) (3,1)   S5: (2,3) (3,2) (4,1)
                                 umma_f16_ts(d, a0, w[0] + o, idesc, acc);
                                 umma_f16_ts(d + XBN, a0, w[1] + o, idesc, acc);
                                 umma_f16_ts(d + 2 * XBN, a0, w[2] + o, idesc, acc);
@@ -440,6 +440,7 @@ __global__ void __launch_bounds__(XTHREADS, 1)
                                 umma_f16_ts(d + 2 * XBN, a1, w[1] + o, idesc, 1);
                                 umma_f16_ts(d + 3 * XBN, a2, w[1] + o, idesc, 1);
                                 umma_f16_ts(d + 2 * XBN, a2, w[0] + o, idesc, 1);
+                                umma_f16_ts(d + 3 * XBN, a3, w[0] + o, idesc, 1);
                             }
                         }
                         umma_commit(&wempty[ws]);
@@ -494,12 +495,12 @@ __global__ void __launch_bounds__(XTHREADS, 1)
             for (int kb = 0; kb < kblocks; kb++) {
                 mbar_wait(&rfull[rs], rphase);
                 const float4* a = (const float4*)(raw + rs * A_TILE_BYTES + row * 128);
-                uint32_t h1[16], h2[16], h3[16];          // 32 K values x 3 slices, two fp16 per TMEM column
+                uint32_t h1[16], h2[16], h3[16], h4[16];   // 32 K values x 4 slices, two fp16 per TMEM column
 #pragma unroll
                 for (int c = 0; c < 8; c++) {
                     const float4 v = a[c ^ rx];
                     const float x[4] = {v.x, v.y, v.z, v.w};
-                    float s1[4], s2[4], s3[4];
+                    float s1[4], s2[4], s3[4], s4[4];
 #pragma unroll
                     for (int j = 0; j < 4; j++) {
                         const float xv = ACT ? silu_x(x[j]) : x[j];
@@ -509,12 +510,15 @@ __global__ void __launch_bounds__(XTHREADS, 1)
                         s2[j] = (t2 + MAGIC) - MAGIC;
                         const float t3 = (t2 - s2[j]) * 256.0f;
                         s3[j] = (t3 + MAGIC) - MAGIC;
+                        const float t4 = (t3 - s3[j]) * 256.0f;
+                        s4[j] = (t4 + MAGIC) - MAGIC;
                     }
 #pragma unroll
                     for (int j = 0; j < 2; j++) {
                         __half2 p1 = __floats2half2_rn(s1[2 * j], s1[2 * j + 1]), p2 = __floats2half2_rn(s2[2 * j], s2[2 * j + 1]),
-                                p3 = __floats2half2_rn(s3[2 * j], s3[2 * j + 1]);
+                                p3 = __floats2half2_rn(s3[2 * j], s3[2 * j + 1]), p4 = __floats2half2_rn(s4[2 * j], s4[2 * j + 1]);
                         h1[2 * c + j] = *(uint32_t*)&p1; h2[2 * c + j] = *(uint32_t*)&p2; h3[2 * c + j] = *(uint32_t*)&p3;
+                        h4[2 * c + j] = *(uint32_t*)&p4;
                     }
                 }
                 fence_async_smem();                      // cross-proxy release of the raw block (see pass 0)
@@ -523,6 +527,7 @@ __global__ void __launch_bounds__(XTHREADS, 1)
                 tmem_st16x(trow + kb * 16, h1);
                 tmem_st16x(trow + 64 + kb * 16, h2);
                 tmem_st16x(trow + 128 + kb * 16, h3);
+                tmem_st16x(trow + 192 + kb * 16, h4);
             }
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             tc_fence_before();

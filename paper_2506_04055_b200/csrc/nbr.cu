@@ -226,18 +226,18 @@ void nbr_gather(const Launch& L, long long N, long long n_local, const int* perm
 }
 
 // ------------------------------------------------------------------------------------------------ a3
-// Visit every candidate (b, shift) of sorted atom a in the fixed stencil order (dz, dy, dx ascending, atoms of a
-// cell ascending) and call f(b, code, dx, dy, dz) for those passing  (dx*dx + dy*dy) + dz*dz < rc^2  (strict, fp64,
+// Visit every candidate (b, shift) of cell-sorted atom a in the fixed stencil order (dz, dy, dx ascending, atoms of a
+// cell ascending) and call f(b, code, dx, dy, dz) for those passing  (dx*dx + dy*dy) + dz*dz < cut2  (strict, fp64,
 // no contraction);  dx = (x_b + S*L) - x_a with S the image relative to the positions as given.
 template <class Fn>
-__device__ __forceinline__ void visit_neighbors(long long a, const Grid& g, const double* __restrict__ pos_s,
-                                                const signed char* __restrict__ wrap_s,
-                                                const int* __restrict__ cell_s,
-                                                const int* __restrict__ cell_start, Fn f) {
+__device__ __forceinline__ void visit_neighbors(long long a, const Grid& g, const NbrSearch& S, Fn f) {
+    const double* __restrict__ pos_s = S.pos;
+    const signed char* __restrict__ wrap_s = S.wrap;
+    const int* __restrict__ cell_start = S.cell_start;
     const double xa = pos_s[3 * a], ya = pos_s[3 * a + 1], za = pos_s[3 * a + 2];
     const int wa0 = wrap_s[3 * a], wa1 = wrap_s[3 * a + 1], wa2 = wrap_s[3 * a + 2];
     int c[3];
-    cell_decode(g, cell_s[a], c);
+    cell_decode(g, S.cell[a], c);
     for (int dz = -1; dz <= 1; dz++) {
         int cz = c[2] + dz, sz = 0;
         if (cz < 0) { if (!g.periodic) continue; cz += g.n[2]; sz = -1; }
@@ -265,21 +265,55 @@ __device__ __forceinline__ void visit_neighbors(long long a, const Grid& g, cons
                     double ey = __dsub_rn(__dadd_rn(pos_s[3 * b + 1], __dmul_rn(Sy, g.box[1])), ya);
                     double ez = __dsub_rn(__dadd_rn(pos_s[3 * b + 2], __dmul_rn(Sz, g.box[2])), za);
                     double d2 = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
-                    if (d2 < g.rc2) f(b, code, ex, ey, ez);
+                    if (d2 < S.cut2) f(b, code, ex, ey, ez);
                 }
             }
         }
     }
 }
+// final row a -> cell-sorted index; cell-sorted neighbour b -> final index (< 0: dropped by the pruning)
+__device__ __forceinline__ long long row_old(const NbrSearch& S, long long a) { return S.old_of_new ? S.old_of_new[a] : a; }
+__device__ __forceinline__ int idx_new(const NbrSearch& S, int b) { return S.new_of_old ? S.new_of_old[b] : b; }
 
-__global__ void __launch_bounds__(128) k_count(long long N, Grid g, const double* __restrict__ pos_s,
-                                               const signed char* __restrict__ wrap_s, const int* __restrict__ cell_s,
-                                               const int* __restrict__ cell_start, int* __restrict__ row_cnt,
-                                               unsigned long long* __restrict__ real_total) {
+// x = d / rc as an fp32 pair (x_hi + x_lo, from the fp64 difference the predicate already holds).  The radial basis
+// sin(n pi d / rc) turns a relative error eps of d into a phase error n pi x eps: with d computed from the fp32-rounded
+// r_e (eps ~ 1e-7) that is 4e-6 at n = 20 -- 60 fp32 ulps, the largest single error of the layer-1 features (DESIGN.md
+// B1).  The forward edge kernels take the phase from this pair: sincospi(x_hi), first-order correction with x_lo.
+__device__ __forceinline__ float2 phase_pair(double ex, double ey, double ez, double inv_rc) {
+    // d = sqrt(d2) without a double-precision square root: fp32 root + one Newton step in fp64 (error ~1e-15 relative)
+    const double d2 = ex * ex + ey * ey + ez * ez;
+    const float dh = sqrtf((float)d2);
+    const double dhd = (double)dh;
+    const double d = dhd + fma(-dhd, dhd, d2) * (double)(0.5f / dh);
+    const double x = d * inv_rc;
+    const float xh = (float)x;
+    return make_float2(xh, (float)(x - (double)xh));
+}
+// one CSR slot (a <- b): fp32 record, image code, search key of the reverse pass, compensated phase
+__device__ __forceinline__ void emit_edge(const EdgeOut& o, long long e, int b, int code, double ex, double ey, double ez) {
+    o.ej[e] = make_float4((float)ex, (float)ey, (float)ez, __int_as_float(b));
+    o.img[e] = (unsigned char)code;
+    if (o.key) o.key[e] = (b << 5) | code;        // compact search key of the reverse-edge pass (N < 2^26)
+    if (o.xph) o.xph[e] = phase_pair(ex, ey, ez, o.inv_rc);
+}
+// dummy slots: sender index ~a (negative), |r| = rc; every kernel gives them exactly zero weight
+__device__ __forceinline__ void emit_padding(const EdgeOut& o, long long e, long long e1, long long a) {
+    for (; e < e1; e++) {
+        o.ej[e] = make_float4(o.rc, 0.0f, 0.0f, __int_as_float(~(int)a));
+        o.img[e] = 255;
+        if (o.key) o.key[e] = -1;
+        if (o.xph) o.xph[e] = make_float2(1.0f, 0.0f);
+    }
+}
+
+// rows: final order; n_rows_p (device, may be null = N): rows >= *n_rows_p are unreached atoms and stay empty
+__global__ void __launch_bounds__(128) k_count(long long N, Grid g, NbrSearch S, const int* __restrict__ n_rows_p,
+                                               int* __restrict__ row_cnt, unsigned long long* __restrict__ real_total) {
     long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     int cnt = 0;
     if (a < N) {
-        visit_neighbors(a, g, pos_s, wrap_s, cell_s, cell_start, [&](int, int, double, double, double) { cnt++; });
+        if (n_rows_p == nullptr || a < *n_rows_p)
+            visit_neighbors(row_old(S, a), g, S, [&](int b, int, double, double, double) { cnt += idx_new(S, b) >= 0; });
         // rows are padded to a multiple of 8 slots with zero-weight dummy edges, so that an 8-edge group of the
         // tensor-core edge kernels never straddles two rows (branch-free inner loops)
         row_cnt[a] = (cnt + ROW_PAD - 1) & ~(ROW_PAD - 1);
@@ -287,44 +321,296 @@ __global__ void __launch_bounds__(128) k_count(long long N, Grid g, const double
     for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
     if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(real_total, (unsigned long long)cnt);
 }
-void nbr_count(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s,
-               const int* cell_s, const int* cell_start, int* row_cnt, unsigned long long* real_total) {
+void nbr_count(const Launch& L, long long N, Grid g, const NbrSearch& S, const int* n_rows_p, int* row_cnt,
+               unsigned long long* real_total) {
     if (N == 0) return;
-    k_count<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, pos_s, wrap_s, cell_s, cell_start, row_cnt,
-                                                               real_total);
+    k_count<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, S, n_rows_p, row_cnt, real_total);
     KLAUNCH(L);
 }
 
-__global__ void __launch_bounds__(128) k_fill(long long N, Grid g, const double* __restrict__ pos_s,
-                                              const signed char* __restrict__ wrap_s, const int* __restrict__ cell_s,
-                                              const int* __restrict__ cell_start, const int* __restrict__ row_ptr,
-                                              long long cap_edges, float rc, float4* __restrict__ ej,
-                                              unsigned char* __restrict__ img, int* __restrict__ key,
+__global__ void __launch_bounds__(128) k_fill(long long N, Grid g, NbrSearch S, const int* __restrict__ n_rows_p,
+                                              const int* __restrict__ row_ptr, long long cap_edges, EdgeOut o,
                                               int* __restrict__ flags) {
     long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (a >= N) return;
     long long e = row_ptr[a];
     if ((long long)row_ptr[a + 1] > cap_edges) { atomicOr(flags, FLAG_EDGE_OVERFLOW); return; }
-    visit_neighbors(a, g, pos_s, wrap_s, cell_s, cell_start, [&](int b, int code, double ex, double ey, double ez) {
-        ej[e] = make_float4((float)ex, (float)ey, (float)ez, __int_as_float(b));
-        img[e] = (unsigned char)code;
-        if (key) key[e] = (b << 5) | code;        // compact search key of the reverse-edge pass (N < 2^26)
-        e++;
-    });
-    // dummy slots: sender index ~a (negative), |r| = rc; every kernel gives them exactly zero weight
-    for (const long long e1 = row_ptr[a + 1]; e < e1; e++) {
-        ej[e] = make_float4(rc, 0.0f, 0.0f, __int_as_float(~(int)a));
-        img[e] = 255;
-        if (key) key[e] = -1;
+    if (n_rows_p == nullptr || a < *n_rows_p)
+        visit_neighbors(row_old(S, a), g, S, [&](int b, int code, double ex, double ey, double ez) {
+            const int bn = idx_new(S, b);
+            if (bn < 0) return;
+            emit_edge(o, e, bn, code, ex, ey, ez);
+            e++;
+        });
+    emit_padding(o, e, row_ptr[a + 1], a);
+}
+void nbr_fill(const Launch& L, long long N, Grid g, const NbrSearch& S, const int* n_rows_p, const int* row_ptr,
+              long long cap_edges, EdgeOut o, int* flags) {
+    if (N == 0) return;
+    if (N >= (1ll << 26)) o.key = nullptr;
+    k_fill<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, S, n_rows_p, row_ptr, cap_edges, o, flags);
+    KLAUNCH(L);
+}
+
+// ------------------------------------------------------------------------------------------------ T-hop pruning
+// "T rounds of pseudo-messages from local atoms; atoms never reached are dropped" (Fig. 1e): level 0 = local atoms,
+// level t = atoms with a neighbour of level t - 1 (breadth-first over the cutoff graph; with a Verlet skin over the
+// list-cutoff graph, a superset, so the levels are lower bounds for every step the list serves).  Cell-sorted indices.
+__global__ void k_level_init(long long N, const float* __restrict__ local_mask, unsigned char* __restrict__ level) {
+    long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (a < N) level[a] = local_mask[a] != 0.0f ? 0 : LEVEL_NONE;
+}
+__global__ void __launch_bounds__(128) k_level_round(long long N, Grid g, NbrSearch S, unsigned char* __restrict__ level, int t) {
+    long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (a >= N || level[a] != LEVEL_NONE) return;
+    bool hit = false;
+    // (a level written in this round equals t, never t - 1: reading while others write is harmless)
+    visit_neighbors(a, g, S, [&](int b, int, double, double, double) { hit |= level[b] == t - 1; });
+    if (hit) level[a] = (unsigned char)t;
+}
+void nbr_levels(const Launch& L, long long N, Grid g, const NbrSearch& S, const float* local_mask, unsigned char* level, int T) {
+    if (N == 0) return;
+    k_level_init<<<(unsigned)((N + 255) / 256), 256, 0, L.stream>>>(N, local_mask, level);
+    KLAUNCH(L);
+    for (int t = 1; t <= T; t++) {
+        k_level_round<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, S, level, t);
+        KLAUNCH(L);
     }
 }
-void nbr_fill(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s,
-              const int* cell_s, const int* cell_start, const int* row_ptr, long long cap_edges, float rc, float4* ej,
-              unsigned char* img, int* key, int* flags) {
+// Stable partition of the cell-sorted atoms by level (buckets 0..T, then the unreached): final index = atoms of lower
+// levels first, cell order kept inside a level.  Every layer's receivers are then a PREFIX of the atom arrays and the
+// kernels of the model run unchanged on a shorter N.  Three passes: per-block histogram, bucket-major offsets, placement.
+constexpr int LVB = 256;                                // atoms per block
+__device__ __forceinline__ int level_bucket(unsigned char lv, int T) { return lv <= T ? lv : T + 1; }
+__global__ void __launch_bounds__(LVB) k_level_hist(long long N, const unsigned char* __restrict__ level, int T, int* __restrict__ hist) {
+    __shared__ int h[PAINN_MAX_T + 2];
+    if (threadIdx.x < T + 2) h[threadIdx.x] = 0;
+    __syncthreads();
+    long long a = blockIdx.x * (long long)LVB + threadIdx.x;
+    if (a < N) atomicAdd(&h[level_bucket(level[a], T)], 1);
+    __syncthreads();
+    if (threadIdx.x < T + 2) hist[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = h[threadIdx.x];   // bucket-major
+}
+// exclusive scan over the bucket-major table (one block); prefix[k] = atoms with bucket < k (k = 0..T+2)
+__global__ void __launch_bounds__(SCAN_T) k_level_offsets(int* __restrict__ hist, long long n, int nb, int T,
+                                                          long long* __restrict__ prefix) {
+    __shared__ long long carry_s;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (long long b0 = 0; b0 < n; b0 += SCAN_T) {
+        long long b = b0 + threadIdx.x;
+        int v = b < n ? hist[b] : 0;
+        int tot;
+        int ex = block_exclusive_scan(v, &tot);
+        long long carry = carry_s;
+        if (b < n) {
+            hist[b] = (int)(carry + ex);
+            if (b % nb == 0) prefix[b / nb] = carry + ex;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) carry_s = carry + tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) prefix[T + 2] = carry_s;
+}
+__global__ void __launch_bounds__(LVB) k_level_place(long long N, const unsigned char* __restrict__ level, int T,
+                                                     const int* __restrict__ base, long long n_reach_src_unused,
+                                                     const long long* __restrict__ prefix, int* __restrict__ new_of_old,
+                                                     int* __restrict__ old_of_new) {
+    __shared__ int wcnt[LVB / 32][PAINN_MAX_T + 2];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    long long a = blockIdx.x * (long long)LVB + threadIdx.x;
+    const int k = a < N ? level_bucket(level[a], T) : -1;
+    for (int i = lane; i < T + 2; i += 32) wcnt[warp][i] = 0;
+    __syncwarp();
+    const unsigned peers = __match_any_sync(0xffffffffu, k);
+    const int rank_in_warp = __popc(peers & ((1u << lane) - 1u));
+    if (k >= 0 && rank_in_warp == 0) wcnt[warp][k] = __popc(peers);
+    __syncthreads();
+    if (k >= 0) {
+        int before = 0;
+        for (int w = 0; w < warp; w++) before += wcnt[w][k];
+        const int idx = base[(size_t)k * gridDim.x + blockIdx.x] + before + rank_in_warp;
+        old_of_new[idx] = (int)a;
+        new_of_old[a] = k <= T ? idx : -1 - idx;      // unreached atoms keep a slot at the end (outputs stay defined), flagged < 0
+    }
+    (void)n_reach_src_unused; (void)prefix;
+}
+// hist: scratch of (T + 2) * ceil(N / 256) ints; prefix: T + 3 long long (device)
+void nbr_level_sort(const Launch& L, long long N, const unsigned char* level, int T, int* hist, long long* prefix,
+                    int* new_of_old, int* old_of_new) {
     if (N == 0) return;
-    if (N >= (1ll << 26)) key = nullptr;
-    k_fill<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, pos_s, wrap_s, cell_s, cell_start, row_ptr, cap_edges,
-                                                              rc, ej, img, key, flags);
+    const int nb = (int)((N + LVB - 1) / LVB);
+    k_level_hist<<<nb, LVB, 0, L.stream>>>(N, level, T, hist);
+    KLAUNCH(L);
+    k_level_offsets<<<1, SCAN_T, 0, L.stream>>>(hist, (long long)nb * (T + 2), nb, T, prefix);
+    KLAUNCH(L);
+    k_level_place<<<nb, LVB, 0, L.stream>>>(N, level, T, hist, 0, prefix, new_of_old, old_of_new);
+    KLAUNCH(L);
+}
+// per-atom arrays from the cell-sorted order into the final (level-major) order
+__global__ void k_regather(long long N, const int* __restrict__ old_of_new, const double* __restrict__ posC,
+                           const int* __restrict__ typesC, const signed char* __restrict__ wrapC, const int* __restrict__ permC,
+                           const float* __restrict__ localC, double* __restrict__ pos_s, int* __restrict__ types_s,
+                           signed char* __restrict__ wrap_s, int* __restrict__ perm, int* __restrict__ inv_perm,
+                           float* __restrict__ local_mask) {
+    long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (a >= N) return;
+    const int o = old_of_new[a];
+    for (int d = 0; d < 3; d++) { pos_s[3 * a + d] = posC[3 * (long long)o + d]; wrap_s[3 * a + d] = wrapC[3 * (long long)o + d]; }
+    types_s[a] = typesC[o];
+    const int i = permC[o];
+    perm[a] = i;
+    inv_perm[i] = (int)a;
+    local_mask[a] = localC[o];
+}
+void nbr_regather(const Launch& L, long long N, const int* old_of_new, const double* posC, const int* typesC,
+                  const signed char* wrapC, const int* permC, const float* localC, double* pos_s, int* types_s,
+                  signed char* wrap_s, int* perm, int* inv_perm, float* local_mask) {
+    if (N == 0) return;
+    k_regather<<<(unsigned)((N + 255) / 256), 256, 0, L.stream>>>(N, old_of_new, posC, typesC, wrapC, permC, localC, pos_s, types_s,
+                                                                  wrap_s, perm, inv_perm, local_mask);
+    KLAUNCH(L);
+}
+
+// ------------------------------------------------------------------------------------------------ Verlet skin
+// Superset list at rc + skin, final indices, unpadded rows: sup_j, sup_code.  While no atom has moved by more than
+// skin / 2 since it was built, every pair within rc is in it, and a step only re-filters it (the per-step "drop edges
+// longer than the cutoff" of PAPER.md:68) instead of binning, sorting and scanning 27 cells.
+__global__ void __launch_bounds__(128) k_sup_count(long long N, Grid g, NbrSearch S, const int* __restrict__ n_rows_p,
+                                                   int* __restrict__ row_cnt, unsigned long long* __restrict__ padded_total) {
+    long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    int cnt = 0;
+    if (a < N) {
+        if (n_rows_p == nullptr || a < *n_rows_p)
+            visit_neighbors(row_old(S, a), g, S, [&](int b, int, double, double, double) { cnt += idx_new(S, b) >= 0; });
+        row_cnt[a] = cnt;
+        cnt = (cnt + ROW_PAD - 1) & ~(ROW_PAD - 1);       // bound of the padded row of any step this list serves
+    }
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(padded_total, (unsigned long long)cnt);
+}
+__global__ void __launch_bounds__(128) k_sup_fill(long long N, Grid g, NbrSearch S, const int* __restrict__ n_rows_p,
+                                                  const int* __restrict__ sup_ptr, int* __restrict__ sup_j,
+                                                  unsigned char* __restrict__ sup_code) {
+    long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (a >= N || (n_rows_p != nullptr && a >= *n_rows_p)) return;
+    long long e = sup_ptr[a];
+    visit_neighbors(row_old(S, a), g, S, [&](int b, int code, double, double, double) {
+        const int bn = idx_new(S, b);
+        if (bn < 0) return;
+        sup_j[e] = bn;
+        sup_code[e] = (unsigned char)code;
+        e++;
+    });
+}
+void nbr_sup_count(const Launch& L, long long N, Grid g, const NbrSearch& S, const int* n_rows_p, int* row_cnt,
+                   unsigned long long* padded_total) {
+    if (N == 0) return;
+    k_sup_count<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, S, n_rows_p, row_cnt, padded_total);
+    KLAUNCH(L);
+}
+void nbr_sup_fill(const Launch& L, long long N, Grid g, const NbrSearch& S, const int* n_rows_p, const int* sup_ptr, int* sup_j,
+                  unsigned char* sup_code) {
+    if (N == 0) return;
+    k_sup_fill<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, S, n_rows_p, sup_ptr, sup_j, sup_code);
+    KLAUNCH(L);
+}
+// candidates of row a from the superset list, tested with the SAME fp64 expression as visit_neighbors on the current
+// positions as given (pos_s / wrap_s in final order, refreshed by k_reuse_prep): identical edge sets, bit for bit
+template <class Fn>
+__device__ __forceinline__ void visit_superset(long long a, const Grid& g, const double* __restrict__ pos_s,
+                                               const signed char* __restrict__ wrap_s, const int* __restrict__ sup_ptr,
+                                               const int* __restrict__ sup_j, const unsigned char* __restrict__ sup_code, Fn f) {
+    const double xa = pos_s[3 * a], ya = pos_s[3 * a + 1], za = pos_s[3 * a + 2];
+    const int wa0 = wrap_s[3 * a], wa1 = wrap_s[3 * a + 1], wa2 = wrap_s[3 * a + 2];
+    for (int x = sup_ptr[a], x1 = sup_ptr[a + 1]; x < x1; x++) {
+        const int b = sup_j[x], code = sup_code[x];
+        double Sx = 0.0, Sy = 0.0, Sz = 0.0;
+        if (g.periodic) {
+            Sx = (double)(code / 9 - 1 - (int)wrap_s[3 * b] + wa0);
+            Sy = (double)((code / 3) % 3 - 1 - (int)wrap_s[3 * b + 1] + wa1);
+            Sz = (double)(code % 3 - 1 - (int)wrap_s[3 * b + 2] + wa2);
+        }
+        double ex = __dsub_rn(__dadd_rn(pos_s[3 * b], __dmul_rn(Sx, g.box[0])), xa);
+        double ey = __dsub_rn(__dadd_rn(pos_s[3 * b + 1], __dmul_rn(Sy, g.box[1])), ya);
+        double ez = __dsub_rn(__dadd_rn(pos_s[3 * b + 2], __dmul_rn(Sz, g.box[2])), za);
+        double d2 = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
+        if (d2 < g.rc2) f(b, code, ex, ey, ez);
+    }
+}
+__global__ void __launch_bounds__(128) k_refilter_count(long long N, Grid g, const double* __restrict__ pos_s,
+                                                        const signed char* __restrict__ wrap_s, const int* __restrict__ sup_ptr,
+                                                        const int* __restrict__ sup_j, const unsigned char* __restrict__ sup_code,
+                                                        int* __restrict__ row_cnt, unsigned long long* __restrict__ real_total) {
+    long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    int cnt = 0;
+    if (a < N) {
+        visit_superset(a, g, pos_s, wrap_s, sup_ptr, sup_j, sup_code, [&](int, int, double, double, double) { cnt++; });
+        row_cnt[a] = (cnt + ROW_PAD - 1) & ~(ROW_PAD - 1);
+    }
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(real_total, (unsigned long long)cnt);
+}
+__global__ void __launch_bounds__(128) k_refilter_fill(long long N, Grid g, const double* __restrict__ pos_s,
+                                                       const signed char* __restrict__ wrap_s, const int* __restrict__ sup_ptr,
+                                                       const int* __restrict__ sup_j, const unsigned char* __restrict__ sup_code,
+                                                       const int* __restrict__ row_ptr, long long cap_edges, EdgeOut o,
+                                                       int* __restrict__ flags) {
+    long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (a >= N) return;
+    long long e = row_ptr[a];
+    if ((long long)row_ptr[a + 1] > cap_edges) { atomicOr(flags, FLAG_EDGE_OVERFLOW); return; }   // (cannot happen: bound reserved at build)
+    visit_superset(a, g, pos_s, wrap_s, sup_ptr, sup_j, sup_code, [&](int b, int code, double ex, double ey, double ez) {
+        emit_edge(o, e, b, code, ex, ey, ez);
+        e++;
+    });
+    emit_padding(o, e, row_ptr[a + 1], a);
+}
+void nbr_refilter_count(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s, const int* sup_ptr,
+                        const int* sup_j, const unsigned char* sup_code, int* row_cnt, unsigned long long* real_total) {
+    if (N == 0) return;
+    k_refilter_count<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, pos_s, wrap_s, sup_ptr, sup_j, sup_code, row_cnt, real_total);
+    KLAUNCH(L);
+}
+void nbr_refilter_fill(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s, const int* sup_ptr,
+                       const int* sup_j, const unsigned char* sup_code, const int* row_ptr, long long cap_edges, EdgeOut o, int* flags) {
+    if (N == 0) return;
+    if (N >= (1ll << 26)) o.key = nullptr;
+    k_refilter_fill<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, pos_s, wrap_s, sup_ptr, sup_j, sup_code, row_ptr, cap_edges, o, flags);
+    KLAUNCH(L);
+}
+// A step that reuses the list: current positions into the final order, wrap counts continued from the build
+// (wrap_now = wrap_build + whole box lengths the as-given coordinate jumped by since), and the validity test: no atom
+// further than skin / 2 from where it was at the build (minimum image), same species.  Sets FLAG_REBUILD otherwise.
+__global__ void k_reuse_prep(long long N, const int* __restrict__ perm, const double* __restrict__ pos, const int* __restrict__ types,
+                             const double* __restrict__ pos_ref_s, const signed char* __restrict__ wrap_ref_s,
+                             const int* __restrict__ types_s, Grid g, double half_skin2, double* __restrict__ pos_s,
+                             signed char* __restrict__ wrap_s, int* __restrict__ flags) {
+    long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (a >= N) return;
+    const long long i = perm[a];
+    int bad = 0;
+    double d2 = 0.0;
+    for (int d = 0; d < 3; d++) {
+        const double x = pos[3 * i + d];
+        if (!isfinite(x)) bad |= FLAG_NONFINITE;
+        double dx = x - pos_ref_s[3 * a + d], m = 0.0;
+        if (g.periodic) { m = rint(dx / g.box[d]); dx -= m * g.box[d]; }
+        if (fabs(m) > 100.0) { bad |= FLAG_REBUILD; m = 0.0; }
+        d2 += dx * dx;
+        pos_s[3 * a + d] = x;
+        wrap_s[3 * a + d] = (signed char)((int)wrap_ref_s[3 * a + d] + (int)m);
+    }
+    if (!(d2 <= half_skin2) || types[i] != types_s[a]) bad |= FLAG_REBUILD;
+    if (bad) atomicOr(flags, bad);
+}
+void nbr_reuse_prep(const Launch& L, long long N, const int* perm, const double* pos, const int* types, const double* pos_ref_s,
+                    const signed char* wrap_ref_s, const int* types_s, Grid g, double half_skin2, double* pos_s, signed char* wrap_s,
+                    int* flags) {
+    if (N == 0) return;
+    k_reuse_prep<<<(unsigned)((N + 255) / 256), 256, 0, L.stream>>>(N, perm, pos, types, pos_ref_s, wrap_ref_s, types_s, g, half_skin2,
+                                                                    pos_s, wrap_s, flags);
     KLAUNCH(L);
 }
 

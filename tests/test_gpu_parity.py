@@ -81,9 +81,30 @@ def _check(c, e, f, w, ref, label="", e_rel=0.0):
         assert dw <= W_TOL * wn, msg
 
 
-def _same_edges(m, c, rc=5.0):
+def reached_atoms(oi, oj, n_local, N, T):
+    """Atoms within T hops of a local atom over the oracle's edge list (Fig. 1e) -- plain breadth-first
+    search on the host.  The library's ghost-mode list is the sub-graph over these atoms (T-hop pruning)."""
+    level = np.full(N, 255, np.int64)
+    level[:n_local] = 0
+    for t in range(1, T + 1):
+        hit = np.zeros(N, bool)
+        hit[oi[level[oj] == t - 1]] = True
+        level[hit & (level == 255)] = t
+    return level <= T
+
+
+def _same_edges(m, c, rc=5.0, pruned=None):
+    """Bit-exact comparison of the neighbour set with the oracle's.  Ghost mode with T-hop pruning (the default): the
+    oracle's set restricted to the atoms a local atom reaches within T hops."""
     gi, gj, gim = m.neighbors()
     oi, oj, oim = oracle.neighbors(c["pos"], c["box"], rc, periodic=c["n_ghost"] == 0)
+    if pruned is None:
+        pruned = c["n_ghost"] > 0
+    if pruned:
+        keep = reached_atoms(oi, oj, c["n_local"], len(c["pos"]), c["model"]["T"])
+        sel = keep[oi] & keep[oj]
+        assert m.stats()["n_reached"] == int(keep.sum()), (m.stats()["n_reached"], int(keep.sum()))
+        oi, oj, oim = oi[sel], oj[sel], oim[sel]
     assert len(gi) == len(oi), (len(gi), len(oi))
     assert np.array_equal(gi, oi) and np.array_equal(gj, oj) and np.array_equal(gim, oim)
     return len(gi)
@@ -112,7 +133,7 @@ def test_parity_small_configs(case):
     m, e, f, w = _gpu_eval(c, blob)
     ne = _same_edges(m, c)
     ref = _oracle_eval(c, blob)
-    assert ref["n_edges"] == ne
+    assert ref["n_edges"] == ne or c["n_ghost"] > 0          # (ghost mode: the pruned sub-graph, checked by _same_edges)
     _check(c, e, f, w, ref, f"config {k} (reduced, N={len(c['pos'])}, E={ne})")
     st = m.stats()
     assert st["n_edges"] == ne and st["n_atoms"] == len(c["pos"]) and st["n_launches"] > 0
