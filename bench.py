@@ -76,19 +76,38 @@ def _cached_workload(k):
     return c, blob
 
 
+def _cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
 def _oracle_time(k, steps, warmup):
+    """The fp64 oracle, as it stands, on a bounded reduced sample of config k: the O(N^2) neighbour
+    search and the whole evaluation are timed separately, median of `steps` runs each; model = evaluation - search."""
     import oracle
     c, blob = _workload(k, small=True)
-    ts = []
+    rc = c["model"]["rc"]
+    tn, tt = [], []
     for it in range(warmup + steps):
         t0 = time.perf_counter()
+        oracle.neighbors(c["pos"], c["box"], rc, periodic=c["n_ghost"] == 0)
+        t1 = time.perf_counter()
         oracle.compute(blob, c["pos"], c["types"], c["box"], c["n_local"], c["n_ghost"], c["ghost_owner"])
+        t2 = time.perf_counter()
         if it >= warmup:
-            ts.append(time.perf_counter() - t0)
-    t = float(np.mean(ts))
-    return dict(value=c["n_local"] / t, unit=UNIT, cores=oracle.threads(), kind="oracle",
-                sample=f"config {k} recipe reduced to {c['n_local']} local atoms ({len(c['pos'])} total), "
-                       f"{steps} evaluation(s) of {t:.2f} s each, O(N^2) neighbour search included"), t
+            tn.append(t1 - t0); tt.append(t2 - t1)
+    t, t_n = float(np.median(tt)), float(np.median(tn))
+    return dict(value=c["n_local"] / t, unit=UNIT, cores=oracle.threads(), kind="oracle", cpu=_cpu_model(),
+                seconds=dict(evaluation=round(t, 3), neighbour_search=round(t_n, 3), model_forward_adjoint=round(max(t - t_n, 0.0), 3)),
+                atom_steps_per_s=dict(neighbour_search=c["n_local"] / t_n, model_forward_adjoint=c["n_local"] / max(t - t_n, 1e-9)),
+                sample=f"config {k} recipe reduced to {c['n_local']} local atoms ({len(c['pos'])} total), median of "
+                       f"{steps} evaluation(s) of {t:.2f} s each (O(N^2) neighbour search {t_n:.2f} s of it; the sample is "
+                       f"size-dependent: the search is quadratic)"), t
 
 
 class _ClockSampler:
@@ -189,6 +208,7 @@ def main():
     ap.add_argument("--config", type=int, default=5, help="BASELINE.json config (1-5); 5 = 1M-atom headline")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the list-reuse leg and the small configs 1-3")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -225,6 +245,9 @@ def main():
     model = c["model"]
     N, n_local = len(c["pos"]), c["n_local"]
     m = P.Model(blob, model["n_species"], model["rc"], N)
+    # The metric times one FULL mlp_compute, neighbour rebuild included: the Verlet-skin reuse of the
+    # library (default on) is switched off for the headline and measured as its own leg below (`list_reuse`).
+    m.set_option("skin_mA", 0)
     opts = os.environ.get("PAINN_OPTS", "")          # experiment knobs "name=value,..." (mlp_set_option); default: none
     for kv in filter(None, opts.split(",")):
         name, val = kv.split("=")
@@ -298,10 +321,11 @@ def main():
     dom = max(acc, key=acc.get)
     n_launch = n_launch_of.get(dom, 1)
     dur_ms = acc[dom] / n_launch
-    # DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/r01_traffic.json)
+    # DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/r02_traffic.json, else r01)
     traffic = None
     try:
-        tj = json.load(open(os.path.join(ROOT, "profiles", "r01_traffic.json")))
+        tp = os.path.join(ROOT, "profiles", "r02_traffic.json")
+        tj = json.load(open(tp if os.path.exists(tp) else os.path.join(ROOT, "profiles", "r01_traffic.json")))
         if k == tj.get("config"):
             traffic = tj["dram_bytes_per_launch"].get(dom)
     except Exception:
@@ -315,7 +339,8 @@ def main():
         per_edge = {"fwd_edge": 20.0 if split else (8.0 + 20.0 * (T - 1)) / T, "bwd_edge": 16.0}[dom] * model["F"]
         gb = stats["n_edges"] * per_edge / (dur_ms * 1e-3) / 1e9
         roofline["l2_gather"] = dict(achieved=gb, peak=16200.0, unit="GB/s", frac=gb / 16200.0,
-                                     peak_source="measured row-gather microbenchmark (512 B per warp request)")
+                                     peak_source="row-gather microbenchmark (512 B per warp request), measured ONCE in round 1 on "
+                                                 "another pod (profiles/r01_microbench.md); not re-measured in this run")
 
     # ---- end to end through the host-buffer entry point (pinned host memory, copies inside the timed region) ----
     hpos = torch.from_numpy(c["pos"]).pin_memory()
@@ -335,11 +360,57 @@ def main():
     e2e = dict(value=_job_value(world, n_local, te), unit=UNIT, ms_per_step=te * 1e3,
                h2d_bytes_per_step=N * 28 + (0 if hown is None else 4 * c["n_ghost"]), d2h_bytes_per_step=N * 24 + 56)
 
+    # ---- the same workload with the kept rc + skin list: static positions, so every step after the
+    # first re-filters the list and replays the captured graph -- the steady state of an MD run between rebuilds
+    def _time_mode(mm, cc, skin_mA, steps, warm):
+        mm.set_option("skin_mA", skin_mA)
+        NN = len(cc["pos"])
+        p_ = torch.from_numpy(cc["pos"]).to(dev); t_ = torch.from_numpy(cc["types"]).to(dev)
+        o_ = None if cc["ghost_owner"] is None else torch.from_numpy(np.ascontiguousarray(cc["ghost_owner"], np.int32)).to(dev)
+        out_ = (torch.empty(1, dtype=torch.float64, device=dev), torch.empty((NN, 3), dtype=torch.float64, device=dev),
+                torch.empty(6, dtype=torch.float64, device=dev))
+        for _ in range(warm):
+            mm.compute(p_, t_, cc["box"], cc["n_local"], cc["n_ghost"], o_, out=out_, stream=stream)
+        torch.cuda.synchronize(dev)
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record(stream)
+        for _ in range(steps):
+            mm.compute(p_, t_, cc["box"], cc["n_local"], cc["n_ghost"], o_, out=out_, stream=stream)
+        a1.record(stream)
+        torch.cuda.synchronize(dev)
+        return a0.elapsed_time(a1) / steps, mm.stats()
+
+    extra = {}
+    if rank == 0 and world == 1 and not args.no_extra:
+        ms_r, st_r = _time_mode(m, c, 1000, args.steps, max(args.warmup, 3))
+        extra["list_reuse"] = dict(skin_A=1.0, ms_per_step=ms_r, value=n_local / (ms_r * 1e-3), unit=UNIT,
+                                   graph_replays=st_r["n_graph_replays"], launches_per_step=st_r["n_launches"],
+                                   note="static positions: every timed step re-filters the kept list at rc and replays the "
+                                        "captured CUDA graph (no cell binning / sort / 27-cell scan, no host read)")
+        m.set_option("skin_mA", 0)
+        small = {}
+        for kk in (1, 2, 3):
+            if kk == k:
+                continue
+            cc, bb = _cached_workload(kk)
+            mk = cc["model"]
+            with P.Model(bb, mk["n_species"], mk["rc"], len(cc["pos"])) as mm:
+                ms0, st0 = _time_mode(mm, cc, 0, 20, 5)
+                ms1, st1 = _time_mode(mm, cc, 1000, 20, 5)
+                mm.set_option("prune", 0); ms2, _ = _time_mode(mm, cc, 0, 20, 5) if cc["n_ghost"] else (None, None)
+            small[f"config{kk}"] = dict(n_local=cc["n_local"], n_ghost=cc["n_ghost"], n_edges=st0["n_edges"],
+                                        ms_rebuild_every_step=ms0, ms_list_reuse_graph=ms1,
+                                        atom_steps_per_s_rebuild=cc["n_local"] / (ms0 * 1e-3),
+                                        atom_steps_per_s_reuse=cc["n_local"] / (ms1 * 1e-3),
+                                        launches_rebuild=st0["n_launches"], atoms_kept_by_pruning=st0["n_reached"],
+                                        **({"ms_rebuild_unpruned": ms2} if ms2 is not None else {}))
+        extra["other_configs"] = small
+
     if rank == 0:
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             try:
-                cpu, _ = _oracle_time(k, 1, 0)
+                cpu, _ = _oracle_time(k, 3, 0)
             except Exception as ex:      # never lose the GPU measurement to the CPU leg
                 cpu = dict(value=None, unit=UNIT, cores=os.cpu_count(), kind="oracle", sample=f"failed: {ex!r}")
         line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
@@ -349,9 +420,9 @@ def main():
                                          f"{stats['n_edges']} directed edges, PaiNN {model['T']}x{model['F']} K={model['K']} rc={model['rc']}",
                                 l2="working set (tens of GB) far larger than the 126 MB L2; no explicit flush",
                                 multi_gpu="replicas only (one evaluation does not shard; BASELINE.json fixes 1 GPU)",
-                                options=opts or "defaults",
+                                options="skin_mA=0 (list rebuilt in every step, as the metric demands)" + ("," + opts if opts else ""),
                                 precision="fp64 cutoff predicate, fp32 edge math and node state, forward GEMMs exact (fp16 integer slices on tcgen05), adjoint GEMMs 3xTF32"),
-                    clocks=clocks, e2e=e2e, gpu_launches=launches, roofline=roofline, cpu_baseline=cpu)
+                    clocks=clocks, e2e=e2e, gpu_launches=launches, roofline=roofline, cpu_baseline=cpu, **extra)
         print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of include/mlp.h: weight blob parsing, buffer management (fixed capacity, grow on
 // overflow: PAPER.md:84-86) and the per-timestep orchestration of the hot path.
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>      // header-only; ranges are no-ops unless a profiler injects its library
 
 #include <algorithm>
 #include <cmath>
@@ -44,6 +45,7 @@ struct mlp_model {
     GemmRegistry reg;                   // tensor-core operands of the GEMM weights (split planes, exact slices)
     void* filt_img[PAINN_MAX_T] = {};   // tcgen05 A-operand image of (bf | Wf), four fp16 planes (edge_v3.cu), K-major shared-memory layout
     void* filt_rows[PAINN_MAX_T] = {};  // same numbers as plain rows [3][F][96] fp16 (TMEM-resident A operand)
+    void* filt_rows_bwd[PAINN_MAX_T] = {};   // adjoint kernel: three product terms, rows [3][F][80] fp16
     int cell_strip = 6;                 // y-strip width of the cell order in cells (0: plain z, y, x order)
     int edge_path = 0;                  // 0: tensor-core edge kernels when F == 128, 1: plain fp32 kernels
     int apu_fwd = 12, apu_bwd = 16;     // atoms per work unit of the tensor-core edge kernels (option atoms_per_unit)
@@ -118,6 +120,7 @@ struct mlp_model {
     std::string err;
     // stage timing
     bool timing = false;
+    bool nvtx_open = false;
     std::vector<cudaEvent_t> ev_pool;
     std::vector<std::pair<int, cudaEvent_t>> marks;
     long long forced_edge_cap = 0;
@@ -276,7 +279,11 @@ struct Misc {
 constexpr size_t MISC_HEAD = offsetof(Misc, bbox);        // what the host reads
 constexpr size_t MISC_CLEAR = offsetof(Misc, prefix);     // what every call zeroes
 
+// Stage boundary: an NVTX range per stage (host-side, around the launches of the stage; visible in nsys / ncu --nvtx) and,
+// with stage timing enabled, a CUDA event on the stream.  stage < 0 closes the last range of the call.
 void mark(mlp_model* m, cudaStream_t st, int stage) {
+    if (m->nvtx_open) { nvtxRangePop(); m->nvtx_open = false; }
+    if (stage >= 0 && stage < ST_COUNT) { nvtxRangePushA(kStageNames[stage]); m->nvtx_open = true; }
     if (!m->timing) return;
     size_t k = m->marks.size();
     if (k >= m->ev_pool.size()) {
@@ -287,7 +294,6 @@ void mark(mlp_model* m, cudaStream_t st, int stage) {
     cudaEventRecord(m->ev_pool[k], st);
     m->marks.push_back({stage, m->ev_pool[k]});
 }
-
 
 void drop_graph(mlp_model* m) {
     if (m->graph_exec) { cudaGraphExecDestroy(m->graph_exec); m->graph_exec = nullptr; }
@@ -666,7 +672,7 @@ int run_model(StepCtx& cx) {
                                        P<int>(m->b_rev), m->filt_rows[0], P<float4>(m->b_G), first);
             if (!done)
                 done = message_bwd_v3(L, Ns, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<float>(m->b_phi[t]),
-                                      P<float>(m->b_V[t]), v1b, m->filt_img[t], m->filt_rows[t], phib, vb, P<float4>(m->b_G), first, t == 0);
+                                      P<float>(m->b_V[t]), v1b, m->filt_img[t], m->filt_rows_bwd[t], phib, vb, P<float4>(m->b_G), first, t == 0);
         }
         if (!done) {
             if (l0_table) return fail(m, MLP_ERR_CUDA, "layer-0 table path unavailable");
@@ -769,6 +775,12 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
                 if (rcode == MLP_OK && cudaMemcpy(b3.p, img.data(), img.size() * 2, cudaMemcpyHostToDevice) != cudaSuccess) rcode = MLP_ERR_CUDA;
                 m->wbufs.push_back(b3);
                 m->filt_rows[t] = b3.p;
+                edge_build_filter_rows_bwd(Wf_h.data(), bf_h.data(), K, img);
+                Buf b4;
+                if (rcode == MLP_OK) rcode = ensure(m, b4, img.size() * 2);
+                if (rcode == MLP_OK && cudaMemcpy(b4.p, img.data(), img.size() * 2, cudaMemcpyHostToDevice) != cudaSuccess) rcode = MLP_ERR_CUDA;
+                m->wbufs.push_back(b4);
+                m->filt_rows_bwd[t] = b4.p;
             }
         }
         up((size_t)3 * F * K, (float**)&l.Wf); up(3 * F, (float**)&l.bf);

@@ -186,6 +186,7 @@ bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
                     float* vb_out, float4* G, bool first, bool layer0);
 
 void edge_build_filter_rows(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img);
+void edge_build_filter_rows_bwd(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img);
 bool message_bwd0_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
                      const int* types_s, const float* tab, int n_tab, const int* rev, const void* A_img, float4* G, bool first);
 // ---- layer 0 with the channels contracted outside the edge loop (edge_l0.cu) ----

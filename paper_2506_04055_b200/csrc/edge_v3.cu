@@ -108,6 +108,19 @@ __device__ __forceinline__ void split4(const float (&v)[8], uint4& p_ll, uint4& 
     }
     p_hh = *(uint4*)a; p_hl = *(uint4*)b; p_lh = *(uint4*)c; p_ll = *(uint4*)d;
 }
+// the adjoint kernels' three planes (terms hl, lh, hh of split4, same scales)
+__device__ __forceinline__ void split3b(const float (&v)[8], uint4& p_hl, uint4& p_lh, uint4& p_hh) {
+    __half2 a[4], b[4], c[4];
+    const __half2 k = __floats2half2_rn(1.0f / 64.0f, 1.0f / 64.0f);
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+        a[i] = __floats2half2_rn(v[2 * i], v[2 * i + 1]);
+        const float2 f = __half22float2(a[i]);
+        b[i] = __floats2half2_rn((v[2 * i] - f.x) * 64.0f, (v[2 * i + 1] - f.y) * 64.0f);
+        c[i] = __hmul2(a[i], k);
+    }
+    p_hh = *(uint4*)a; p_hl = *(uint4*)b; p_lh = *(uint4*)c;
+}
 // byte offset of the 8-slot group h (basis slots 8h .. 8h+7) of product term t inside a B (or A) row block: K index
 // 24 t + 8 h + i, 12 groups of 8 = 96 = KP
 __device__ __forceinline__ int kgrp_off(int t, int h) { return (3 * t + h) * 128; }
@@ -159,7 +172,11 @@ constexpr int GW = 16;                                  // gather window (edges 
 constexpr int RING_BYTES = GW * F * 16;                 // 32768
 constexpr int G_OFF_B = 0, G_OFF_P = 2 * BB_BYTES, G_OFF_RING = G_OFF_P + 2 * P_BYTES, G_OFF_META = G_OFF_RING + RING_BYTES,
               G_OFF_BAR = G_OFF_META + 4 * NEB * 16, GROUP_BYTES = G_OFF_BAR + 128;
-constexpr int bwd_smem_bytes(int nch) { return (nch - 2) * A_CHUNK_BYTES + 2 * GROUP_BYTES + 128; }
+constexpr int bwd_smem_bytes(int) { return 2 * GROUP_BYTES + 128; }
+// adjoint kernel: three product terms (hl, lh, hh: forces carry a relative tolerance, the r r term is not needed) on
+// K = 3 x 24 + 8 zero slots = 80 = five k-steps; 40 TMEM columns per chunk, all chunks TMEM-resident
+constexpr int KB = 80, KB_COLS = KB / 2;
+constexpr int BWD_TMEM_A = 384;                         // TMEM columns of the filter operand (behind 2 x 2 x 96 accumulator columns)
 
 // two fp32 additions in one instruction (register pairs as they come out of a 16-byte shared-memory load): the reducer
 // warps sit on the critical path of their pipeline and are bound by instruction issue
@@ -179,6 +196,11 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16
         "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]),
         "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
         : "memory");
+}
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t (&r)[8]) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr), "r"(r[0]), "r"(r[1]),
+                 "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
+                 : "memory");
 }
 // A operand from TMEM (lane = row, 8 columns = 16 fp16 along K), B from shared memory
 __device__ __forceinline__ void umma_f16_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
@@ -529,10 +551,8 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
     constexpr int NCH = L0 ? 2 : 3;
     constexpr int TCOLS = NCH * 2 * NEB;            // TMEM columns per accumulator buffer
     extern __shared__ __align__(128) uint8_t smem[];
-    uint8_t* sA = smem;
     const int tid = threadIdx.x, grp = tid >> 8, ltid = tid & 255, lwarp = ltid >> 5, lane = tid & 31;
-    constexpr int NSM = NCH - 2;                    // chunks kept in shared memory (vv); s and vs live in TMEM
-    uint8_t* gbase = smem + NSM * A_CHUNK_BYTES + grp * GROUP_BYTES;
+    uint8_t* gbase = smem + grp * GROUP_BYTES;
     uint8_t* sB = gbase + G_OFF_B;
     uint8_t* sP = gbase + G_OFF_P;                 // [2][8] rows of P_ROW bytes: (db, ub_x, ub_y, ub_z) per channel
     float4* sMeta = (float4*)(gbase + G_OFF_META); // [4][NEB] (u of edge (i <- j), 1/d): ring of 4 tiles
@@ -543,12 +563,9 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
     const int NB_TE = 1 + grp * 6;    // consumers (128, arrive) -> producers (64, sync): tile buffer consumed
     const int NB_BF = NB_TE + 2;      // producers (64, arrive) -> MMA warp (32, sync): B operand written
     const int NB_PF = NB_TE + 4;      // consumers (128, arrive) -> reducer (32, sync): partials of one batch written
-    uint32_t* tmem_slot = (uint32_t*)(smem + NSM * A_CHUNK_BYTES + 2 * GROUP_BYTES);
+    uint32_t* tmem_slot = (uint32_t*)(smem + 2 * GROUP_BYTES);
 
     {
-        const uint4* src = p.A_img + 2 * (A_CHUNK_BYTES / 16);
-        uint4* dst = (uint4*)sA;
-        for (int i = tid; i < NSM * A_CHUNK_BYTES / 16; i += BWD_THREADS) dst[i] = src[i];
         uint4* zb = (uint4*)sB;
         for (int i = ltid; i < 2 * BB_BYTES / 16; i += 256) zb[i] = make_uint4(0, 0, 0, 0);
     }
@@ -561,28 +578,35 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    // chunks s and vs of the filter operand into TMEM (lane = channel row, 48 columns = 96 fp16 each): columns 192..239
-    // and 448..495, the gaps behind the two groups' accumulators (2 x 96 columns each)
+    // ALL chunks of the filter operand into TMEM (lane = channel row, KB_COLS = 40 columns = 80 fp16 per chunk, three
+    // product terms: edge_build_filter_rows_bwd): columns 384 .. 384 + 40 NCH behind the two groups' accumulators (2 x 2 x
+    // 96 columns).  The forward kernel keeps chunk vv in shared memory (its four terms need 48 columns per chunk, 16 more
+    // than TMEM has); here the tensor core re-read those 24 KB for every 16-edge tile: 12 of the kernel's 84 shared-memory
+    // wavefronts per edge on an LSU data pipe that is 75 % busy (profiles/r02_edge_ncu.md).
     if (tid < 128) {
 #pragma unroll
-        for (int c = 0; c < 2; c++) {
-            const uint32_t abase = *tmem_slot + 192 + c * 256 + ((uint32_t)((tid >> 5) * 32) << 16);
-            const uint4* src = p.A_rows + ((size_t)c * 128 + tid) * 12;
+        for (int c = 0; c < NCH; c++) {
+            const uint32_t abase = *tmem_slot + BWD_TMEM_A + c * KB_COLS + ((uint32_t)((tid >> 5) * 32) << 16);
+            const uint4* src = p.A_rows + ((size_t)c * 128 + tid) * (KB_COLS / 4);
 #pragma unroll
-            for (int j = 0; j < 3; j++) {
+            for (int j = 0; j < 2; j++) {
                 uint32_t r[16];
 #pragma unroll
                 for (int q = 0; q < 4; q++) { const uint4 v = src[j * 4 + q]; r[4 * q] = v.x; r[4 * q + 1] = v.y; r[4 * q + 2] = v.z; r[4 * q + 3] = v.w; }
                 tmem_st16(abase + j * 16, r);
             }
+            uint32_t r8[8];
+#pragma unroll
+            for (int q = 0; q < 2; q++) { const uint4 v = src[8 + q]; r8[4 * q] = v.x; r8[4 * q + 1] = v.y; r8[4 * q + 2] = v.z; r8[4 * q + 3] = v.w; }
+            tmem_st8(abase + 32, r8);
         }
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     }
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    const uint32_t tmem_base = *tmem_slot + grp * 256;
-    const uint32_t tmem_A = *tmem_slot + 192;
+    const uint32_t tmem_base = *tmem_slot + grp * 192;
+    const uint32_t tmem_A = *tmem_slot + BWD_TMEM_A;
     const long long N = p.N;
     const int apu = p.atoms_per_unit;
     const int* __restrict__ row_ptr = p.row_ptr;
@@ -780,7 +804,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
             float4 raw_n = load_edge_raw(p.ej, e_begin + e, h < 3 ? e_end : 0);
             for (int t = 0; t < ntiles; t++, it++) {
                 const int buf = it & 1;
-                uint4 q[8];
+                uint4 q[6];
                 float4 meta_v = make_float4(0.f, 0.f, 0.f, 0.f);
                 const float4 raw = raw_n;
                 if (t + 1 < ntiles) raw_n = load_edge_raw(p.ej, e_begin + (t + 1) * NEB + e, h < 3 ? e_end : 0);
@@ -805,8 +829,8 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                             sn_ = tt;
                         }
                     }
-                    split4(vals, q[0], q[1], q[2], q[3]);
-                    split4(dvals, q[4], q[5], q[6], q[7]);
+                    split3b(vals, q[0], q[1], q[2]);
+                    split3b(dvals, q[3], q[4], q[5]);
                     meta_v = make_float4(-g.r.x * g.inv_d, -g.r.y * g.inv_d, -g.r.z * g.inv_d, g.inv_d);   // u_e of edge (i <- j), 1/d
                 }
                 __syncwarp();
@@ -817,7 +841,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                         const int row = z * NEB + e;
                         uint8_t* bb = sB + buf * BB_BYTES + (row >> 3) * SBO + (row & 7) * 16;
 #pragma unroll
-                        for (int tm = 0; tm < 4; tm++) *(uint4*)(bb + kgrp_off(tm, h)) = q[4 * z + tm];
+                        for (int tm = 0; tm < 3; tm++) *(uint4*)(bb + kgrp_off(tm, h)) = q[3 * z + tm];
                     }
                     if (h == 0) sMeta[(it & 3) * NEB + e] = meta_v;
                 }
@@ -876,7 +900,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
     } else if (lwarp == 7) {
         // ===================== MMA issuer (lane 0; the whole warp waits on the producers' named barrier) =====================
         const uint32_t idesc = (1u << 4) | ((uint32_t)((2 * NEB) >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-        const uint32_t a_base = smem_u32(sA), b_base = smem_u32(sB);
+        const uint32_t b_base = smem_u32(sB);
         uint32_t it = 0;
         for (long long u = u0; u < n_units; u += ustride) {
             const long long a0 = u * apu;
@@ -892,11 +916,9 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                     for (int c = 0; c < NCH; c++) {
                         const uint32_t d = tmem_base + buf * TCOLS + c * 2 * NEB;
 #pragma unroll
-                        for (int o = 0; o < 6; o++) {
-                            const int kk = o;
+                        for (int kk = 0; kk < KB_COLS / 8; kk++) {     // ascending K: cross terms first, the hh term last
                             const uint64_t bd = make_desc_nosw(b_base + buf * BB_BYTES + kk * 2 * LBO, LBO, SBO);
-                            if (c < 2) umma_f16_ts(d, tmem_A + c * 256 + kk * 8, bd, idesc, o != 0);
-                            else umma_f16(d, make_desc_nosw(a_base + kk * 2 * LBO, LBO, SBO), bd, idesc, o != 0);
+                            umma_f16_ts(d, tmem_A + c * KB_COLS + kk * 8, bd, idesc, kk != 0);
                         }
                     }
                     umma_commit(&t_full[buf]);
@@ -1290,6 +1312,18 @@ void edge_build_filter_rows(const float* Wf, const float* bf, int K, std::vector
                 for (int t = 0; t < 4; t++) img[((size_t)c * ev3::F + r) * ev3::KP + t * 24 + b] = bits[t];
             }
 }
+// host: the adjoint kernel's operand, rows [3 chunks][128 channels][80 fp16]: terms (hl, lh, hh) at k = 24 t + b, k >= 72 zero
+void edge_build_filter_rows_bwd(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img) {
+    img.assign((size_t)3 * ev3::F * ev3::KB, 0);
+    for (int c = 0; c < 3; c++)
+        for (int r = 0; r < ev3::F; r++)
+            for (int b = 0; b <= K; b++) {
+                const float w = b == 0 ? bf[c * ev3::F + r] : Wf[(size_t)(c * ev3::F + r) * K + (b - 1)];
+                unsigned short bits[4];
+                filter_planes(w, bits);                         // (r, hi 2^-6, r 2^6, hi)
+                for (int t = 0; t < 3; t++) img[((size_t)c * ev3::F + r) * ev3::KB + t * 24 + b] = bits[t + 1];
+            }
+}
 // host: the same numbers as the K-major no-swizzle shared-memory image of the A operand (3 chunks of A_CHUNK_BYTES)
 void edge_build_filter_image(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img) {
     using namespace ev3;
@@ -1351,7 +1385,7 @@ bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
                     float* vb_out, float4* G, bool first, bool layer0) {
     using namespace ev3;
     if (N == 0) return true;
-    if (K > 23 || !A_rows || !A_img) return false;
+    if (K > 23 || !A_rows) return false;
     static bool attr = false;
     if (!attr) {
         if (cudaFuncSetAttribute(k_msg_bwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bwd_smem_bytes(2)) != cudaSuccess ||

@@ -10,6 +10,9 @@ O(N^2) and cannot evaluate 10^5 - 10^6 atoms, so above config 2 the check is mad
   * properties that hold at any size: Newton's third law (sum of forces = 0), neighbour count against the counted
     pairs of sampled atoms, finite outputs, bit-identical repeat.
 """
+import json
+import os
+
 import numpy as np
 import pytest
 
@@ -19,6 +22,42 @@ import oracle
 pytestmark = pytest.mark.gpu
 
 T_RC = 15.0          # T * rc of the 3-layer model with rc = 5 A
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def _golden(k):
+    """Whole-system fp64 oracle values of config k at full size (energy, virial, stratified force sample), written by
+    tests/golden/make_golden_fullsize.py from gen/ + oracle/ only (block sums with a T rc halo)."""
+    with open(os.path.join(GOLDEN, f"fullsize_config{k}.json")) as fh:
+        g = json.load(fh)
+    g["sample_idx"] = np.asarray(g["sample_idx"], np.int64)
+    g["sample_forces"] = np.asarray(g["sample_forces"], np.float64)
+    g["virial"] = np.asarray(g["virial"], np.float64)
+    return g
+
+
+def _check_against_golden(k, c, e, f, w, label):
+    """north_star's tolerances, bare, at the full size: |dE| / n_local <= 1e-4; over the stratified sample (>= 96 atoms
+    per stratum) rms(dF) <= 2e-3 F_rms and max|dF| <= 1e-2 F_rms with F_rms of ALL local atoms; ||dW|| <= 2e-3 ||W||."""
+    g = _golden(k)
+    assert g["meta"]["n_local"] == c["n_local"] and g["meta"]["n_total"] == len(c["pos"])
+    nl = c["n_local"]
+    de = abs(e - g["energy"]) / nl
+    idx = g["sample_idx"]
+    df = f[idx] - g["sample_forces"]
+    frms = g["f_rms"]
+    drms = np.sqrt((df ** 2).mean()) / frms
+    dmax = np.abs(df).max() / frms
+    dw = np.linalg.norm(w - g["virial"]) / np.linalg.norm(g["virial"])
+    strata = sorted(set(g["sample_strata"]))
+    print(f"{label}: E/atom = {g['energy'] / nl:.6f}  signed dE/atom = {(e - g['energy']) / nl:+.3e}  sample of {len(idx)} atoms "
+          f"({', '.join(strata)}): rel_rms_dF = {drms:.2e}  max_dF/rms = {dmax:.2e}  rel_dW = {dw:.2e}")
+    assert len(idx) >= 64
+    assert de <= 1e-4, (label, de)
+    assert drms <= 2e-3 and dmax <= 1e-2, (label, drms, dmax)
+    assert dw <= 2e-3, (label, dw)
+    # own force rms of the GPU result against the oracle's (all local atoms)
+    assert abs(np.sqrt((f[:nl] ** 2).mean()) / frms - 1.0) <= 1e-4
 
 
 def _cluster(pos, box, center, radius):
@@ -41,6 +80,7 @@ def test_config5_full_size_sampled_against_oracle():
     N = len(pos)
     assert N == 1029000 and c["n_ghost"] == 0
     with P.Model(blob, mdl["n_species"], mdl["rc"], N) as m:
+        m.set_option("skin_mA", 0)                                # bench.py's headline configuration: full rebuild per call
         dpos, dtyp = torch.from_numpy(pos).to(dev), torch.from_numpy(types).to(dev)
         e, f, w = m.compute(dpos, dtyp, box)
         torch.cuda.synchronize()
@@ -86,6 +126,8 @@ def test_config5_full_size_sampled_against_oracle():
         print(f"atom {a}: cluster {len(idx)} atoms, {n_nb} neighbours, |dF|max/rms = {df / frms:.2e}, "
               f"state err = {np.abs(s_gpu[:F] - s_ref[:F]).max() / scale:.2e}")
         assert df <= 1e-2 * frms, (a, f1[a], ref["forces"][ctr], frms)
+    # whole-system energy, virial and the stratified force sample against the full-size oracle golden
+    _check_against_golden(5, c, e1, f1, w1, "config 5 full size")
 
 
 # ------------------------------------------------------------------------------------------------------------------
@@ -152,6 +194,11 @@ def test_config2_full_size_whole_system_against_oracle():
     print(f"config 2 full: E={st['n_edges']} dE/atom={de:.2e} rel_rms_dF={drms:.2e} max_dF/rms={dmax:.2e} rel_dW={dw:.2e}")
     # north_star's tolerances, bare: energy per atom 1e-4, force rms 2e-3 and max 1e-2 of the force rms, virial 2e-3 (A16)
     assert de <= 1e-4 and drms <= 2e-3 and dmax <= 1e-2 and dw <= 2e-3
+    # the block-summed golden of the same system must be the whole-system oracle (pins the golden script at full size)
+    g = _golden(2)
+    assert abs(g["energy"] - ref["energy"]) <= 1e-9 * abs(ref["energy"])
+    assert np.abs(g["sample_forces"] - fr[g["sample_idx"]]).max() <= 1e-8 * rms
+    _check_against_golden(2, c, e, f, w, "config 2 full size")
 
 
 def test_config3_full_size_slab_with_ghosts():
@@ -177,6 +224,8 @@ def test_config3_full_size_slab_with_ghosts():
     face = np.asarray(c["ghost_owner"], np.int64)                         # atoms with images: next to the ghost halo
     samples = [int(rng.choice(nl)), int(rng.choice(surface)), int(rng.choice(face))]
     _check_sampled(c, blob, fp, state, samples, frms, minimum_image=False)
+    # whole system: energy, virial, partial forces on a stratified sample (bulk / surface / next to the halo / ghosts)
+    _check_against_golden(3, c, e, fp, w, "config 3 full size (partial forces on all rows)")
 
 
 def test_config4_full_size_crystal():
@@ -192,3 +241,4 @@ def test_config4_full_size_crystal():
     assert np.abs(f.sum(0)).max() <= 1e-5 * frms * np.sqrt(N), f.sum(0)
     rng = np.random.default_rng(20250602)
     _check_sampled(c, blob, f, state, [int(a) for a in rng.choice(N, size=2, replace=False)], frms, minimum_image=True)
+    _check_against_golden(4, c, e, f, w, "config 4 full size")

@@ -271,6 +271,53 @@ def test_row_length_stress_tensor_core_path(name):
     _check(c, e, f, w, ref, f"stress {name} (N={n}, E={ne}, {ne / n:.1f} neighbours per atom)", e_rel=3e-5)
 
 
+def test_sparse_system_with_more_cells_than_atoms():
+    """200,000 atoms at 0.002 / A^3: the periodic grid has ~4 cells per atom (capped at 4 N + 4096), so the exclusive scan
+    over the CELLS needs more block scratch than the scan over the atoms (the scratch was once sized by the atoms only).
+    The O(N^2) oracle cannot run this size: the directed edge count is checked against scipy's cKDTree pair count (a
+    library routine), forces against Newton's third law, and a repeat must be bit-identical."""
+    from scipy.spatial import cKDTree
+    import paper_2506_04055_b200 as P
+    torch = _torch()
+    dev = torch.device("cuda:0")
+    n, L = 200000, 464.0
+    pos, types, box = gen.random_gas(n, (L, L, L), 1.0, seed=4242, n_species=2)
+    model = dict(n_species=2, F=32, K=16, T=2, rc=5.0, wseed=5)
+    blob = _blob(model)
+    with P.Model(blob, 2, 5.0, n) as m:
+        m.set_option("skin_mA", 0)
+        dp, dt = torch.from_numpy(pos).to(dev), torch.from_numpy(types).to(dev)
+        e, f, w = m.compute(dp, dt, box)
+        torch.cuda.synchronize()
+        st = m.stats()
+        e1, f1 = float(e[0]), f.cpu().numpy().copy()
+        e, f, w = m.compute(dp, dt, box)
+        torch.cuda.synchronize()
+        assert float(e[0]) == e1 and np.abs(f.cpu().numpy() - f1).max() <= 1e-9 * max(np.abs(f1).max(), 1e-30)
+    ncell = st["n_cells"][0] * st["n_cells"][1] * st["n_cells"][2]
+    assert ncell > 3 * n, (st["n_cells"], n)
+    pairs = cKDTree(pos, boxsize=box).count_neighbors(cKDTree(pos, boxsize=box), 5.0 - 1e-12) - n
+    assert abs(st["n_edges"] - pairs) <= 2, (st["n_edges"], pairs)          # (pairs at d = rc +- 1e-12 may differ)
+    assert np.isfinite(e1) and np.isfinite(f1).all()
+    frms = np.sqrt((f1 ** 2).mean())
+    assert np.abs(f1.sum(0)).max() <= 1e-5 * max(frms, 1e-30) * np.sqrt(n)
+
+
+def test_ghost_owner_out_of_range_is_an_error():
+    import paper_2506_04055_b200 as P
+    torch = _torch()
+    dev = torch.device("cuda:0")
+    c = gen.make_config(3, **SMALL[3])
+    blob = _blob(c["model"])
+    own = np.ascontiguousarray(c["ghost_owner"], np.int32).copy()
+    own[5] = c["n_local"] + 3                                   # points at a ghost row: the fold would corrupt memory
+    with P.Model(blob, c["model"]["n_species"], c["model"]["rc"], len(c["pos"])) as m:
+        with pytest.raises(P.MLPError) as ei:
+            m.compute(torch.from_numpy(c["pos"]).to(dev), torch.from_numpy(c["types"]).to(dev), c["box"], c["n_local"],
+                      c["n_ghost"], torch.from_numpy(own).to(dev))
+        assert ei.value.code == 1
+
+
 def test_error_codes():
     import paper_2506_04055_b200 as P
     torch = _torch()
