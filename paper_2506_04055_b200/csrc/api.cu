@@ -43,9 +43,7 @@ struct mlp_model {
     LayerW lw[PAINN_MAX_T];
     float *Wr1 = nullptr, *br1 = nullptr, *wr2 = nullptr, *br2 = nullptr, *Wr1T = nullptr;
     GemmRegistry reg;                   // tensor-core operands of the GEMM weights (split planes, exact slices)
-    void* filt_img[PAINN_MAX_T] = {};   // tcgen05 A-operand image of (bf | Wf), four fp16 planes (edge_v3.cu), K-major shared-memory layout
-    void* filt_rows[PAINN_MAX_T] = {};  // same numbers as plain rows [3][F][96] fp16 (TMEM-resident A operand)
-    void* filt_rows_bwd[PAINN_MAX_T] = {};   // adjoint kernel: three product terms, rows [3][F][80] fp16
+    void* filt_rows[PAINN_MAX_T] = {};  // tcgen05 A operand (bf | Wf) of the edge kernels: three fp16 product-term planes, rows [3][F][80]
     int cell_strip = 6;                 // y-strip width of the cell order in cells (0: plain z, y, x order)
     int edge_path = 0;                  // 0: tensor-core edge kernels when F == 128, 1: plain fp32 kernels
     int apu_fwd = 12, apu_bwd = 16;     // atoms per work unit of the tensor-core edge kernels (option atoms_per_unit)
@@ -562,7 +560,7 @@ int run_model(StepCtx& cx) {
     // 32 gate-MLP out, 64 readout and layer-0 sums); 1 = all
     auto LfT = [&](int type) { Launch x = Lf; x.fwd_exact = m->gemm_fwd_exact == 1 ? 1 : ((m->gemm_fwd_exact >> (type + 1)) & 1); return x; };
     Lb.gemm_path = m->bwd_exact ? 1 : 0;
-    const bool tc_edges = m->edge_path == 0 && F == 128 && K <= 23 && m->filt_img[0] != nullptr;
+    const bool tc_edges = m->edge_path == 0 && F == 128 && K <= 23 && m->filt_rows[0] != nullptr;
     mark(m, st, ST_FWD_NODE);
     embed(L, Nreach, F, P<int>(m->b_types_s), m->Emb, P<float>(m->b_S[0]), P<float>(m->b_V[0]));
     float* h = P<float>(m->b_h);
@@ -600,8 +598,7 @@ int run_model(StepCtx& cx) {
         }
         if (!done && tc_edges && (t > 0 || l0_table)) {
             if (!l0_table) make_gather_rows(L, Ns, phi, V, P<float>(m->b_Q4), P<float>(m->b_Q1), t > 0);
-            done = message_fwd_v3(L, Nr, K, rcf, row_ptr, ej, S, V, P<float>(m->b_Q4), P<float>(m->b_Q1), m->filt_img[t],
-                                  m->filt_rows[t], sn, v1, t > 0, P<int>(m->b_types_s), m->tab0, m->n_species, xph);
+            done = message_fwd_v3(L, Nr, K, rcf, row_ptr, ej, S, V, P<float>(m->b_Q4), P<float>(m->b_Q1), m->filt_rows[t], sn, v1, t > 0, P<int>(m->b_types_s), m->tab0, m->n_species, xph);
         }
         if (!done) {
             if (l0_table) return fail(m, MLP_ERR_CUDA, "layer-0 table path unavailable");   // (phi was not computed)
@@ -672,7 +669,7 @@ int run_model(StepCtx& cx) {
                                        P<int>(m->b_rev), m->filt_rows[0], P<float4>(m->b_G), first);
             if (!done)
                 done = message_bwd_v3(L, Ns, K, rcf, row_ptr, ej, P<float>(m->b_Q4), P<float>(m->b_phi[t]),
-                                      P<float>(m->b_V[t]), v1b, m->filt_img[t], m->filt_rows_bwd[t], phib, vb, P<float4>(m->b_G), first, t == 0);
+                                      P<float>(m->b_V[t]), v1b, m->filt_rows[t], phib, vb, P<float4>(m->b_G), first, t == 0);
         }
         if (!done) {
             if (l0_table) return fail(m, MLP_ERR_CUDA, "layer-0 table path unavailable");
@@ -763,24 +760,12 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
             if (t == 0) { Wf0_h = Wf_h; bf0_h = bf_h; }
             if (F == 128 && K <= 23 && rcode == MLP_OK) {
                 std::vector<unsigned short> img;
-                edge_build_filter_image(Wf_h.data(), bf_h.data(), K, img);
-                Buf b;
-                rcode = ensure(m, b, img.size() * 2);
-                if (rcode == MLP_OK && cudaMemcpy(b.p, img.data(), img.size() * 2, cudaMemcpyHostToDevice) != cudaSuccess) rcode = MLP_ERR_CUDA;
-                m->wbufs.push_back(b);
-                m->filt_img[t] = b.p;
                 edge_build_filter_rows(Wf_h.data(), bf_h.data(), K, img);
                 Buf b3;
-                if (rcode == MLP_OK) rcode = ensure(m, b3, img.size() * 2);
+                rcode = ensure(m, b3, img.size() * 2);
                 if (rcode == MLP_OK && cudaMemcpy(b3.p, img.data(), img.size() * 2, cudaMemcpyHostToDevice) != cudaSuccess) rcode = MLP_ERR_CUDA;
                 m->wbufs.push_back(b3);
                 m->filt_rows[t] = b3.p;
-                edge_build_filter_rows_bwd(Wf_h.data(), bf_h.data(), K, img);
-                Buf b4;
-                if (rcode == MLP_OK) rcode = ensure(m, b4, img.size() * 2);
-                if (rcode == MLP_OK && cudaMemcpy(b4.p, img.data(), img.size() * 2, cudaMemcpyHostToDevice) != cudaSuccess) rcode = MLP_ERR_CUDA;
-                m->wbufs.push_back(b4);
-                m->filt_rows_bwd[t] = b4.p;
             }
         }
         up((size_t)3 * F * K, (float**)&l.Wf); up(3 * F, (float**)&l.bf);
@@ -808,7 +793,7 @@ __attribute__((visibility("default"))) int mlp_create(const void* weights, size_
     up((size_t)R * F, &m->Wr1, &Wr1); up(R, &m->br1); up(R, &m->wr2); up(1, &m->br2);
     if (rcode == MLP_OK) painn::gemm_register_exact(m->reg, m->Wr1, Wr1.data(), R, F);
     upT(Wr1, R, F, &m->Wr1T);
-    if (rcode == MLP_OK && F == 128 && m->filt_img[0] && ns <= 16) {
+    if (rcode == MLP_OK && F == 128 && m->filt_rows[0] && ns <= 16) {
         // layer-0 sender rows per species: phi(Emb[z]) through the same forward GEMM path as the per-atom rows
         Buf bh, bp;
         rcode = ensure(m, bh, (size_t)ns * F * 4);

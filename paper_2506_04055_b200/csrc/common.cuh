@@ -175,18 +175,16 @@ void unpermute_state(const Launch& L, long long N, int F, const int* perm, const
                      float* out);
 
 // ---- tensor-core edge kernels (edge_v3.cu), F = 128: per-edge filter on tcgen05, software-pipelined gathers ----
-void edge_build_filter_image(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img);
 void make_gather_rows(const Launch& L, long long N, const float* phi, const float* v, float* Q4, float* Q1, bool has_v);
 void make_gather_rows_bwd(const Launch& L, long long N, const float* s1b, const float* v1b, float* Gb);
 bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* s,
-                    const float* v, const float* Q4, const float* Q1, const void* A_img, const void* A_rows, float* sn, float* v1,
+                    const float* v, const float* Q4, const float* Q1, const void* A_rows, float* sn, float* v1,
                     bool has_v, const int* types_s, const float* tab, int n_tab, const float2* xph);
 bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
-                    const float* phi, const float* v_in, const float* v1b, const void* A_img, const void* A_rows, float* phib,
+                    const float* phi, const float* v_in, const float* v1b, const void* A_rows, float* phib,
                     float* vb_out, float4* G, bool first, bool layer0);
 
 void edge_build_filter_rows(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img);
-void edge_build_filter_rows_bwd(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img);
 bool message_bwd0_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
                      const int* types_s, const float* tab, int n_tab, const int* rev, const void* A_img, float4* G, bool first);
 // ---- layer 0 with the channels contracted outside the edge loop (edge_l0.cu) ----

@@ -8,13 +8,15 @@
 //   atomics, coalesced 512 B gathers of the sender rows.
 //
 // Precision: fp16 operands alone miss the force tolerance, so both operands are split
-// x = hi + r (hi = RN_fp16(x), r the exact remainder) and FOUR product terms are accumulated along K = 4 x 24 = 96:
-//   r(W) r(R)  +  [hi(W) 2^-6][r(R) 2^6]  +  [r(W) 2^6][hi(R) 2^-6]  +  hi(W) hi(R)
-// (split4 / filter_planes; K + 1 <= 24 basis slots per term).  The small terms come first in K and the MMAs are issued
+// x = hi + r (hi = RN_fp16(x), r the exact remainder) and THREE product terms are accumulated along K = 3 x 24 (+ 8 zero
+// slots) = 80, five k-steps:
+//   [hi(W) 2^-6][r(R) 2^6]  +  [r(W) 2^6][hi(R) 2^-6]  +  hi(W) hi(R)
+// (split3b / filter_planes; K + 1 <= 24 basis slots per term).  The cross terms come first in K and the MMAs are issued
 // in ascending K, so the fp32 accumulator (which truncates toward zero after every MMA, B3) sees only two
-// full-magnitude additions.  Round 1 used three terms with 2^+-11 scales on 32-slot terms: same MMA count, but the
-// hi 2^-11 planes were fp16 subnormals for most operands and the r r term was missing -- 3.6x the per-atom energy noise
-// of the plain fp32 kernels (B1).
+// full-magnitude additions.  Round 1 used 2^+-11 scales on 32-slot terms: the hi 2^-11 planes were fp16 subnormals for
+// most operands and a cross term lost its bits -- 3.6x the per-atom energy noise of the plain fp32 kernels (DESIGN.md
+// B1).  A fourth term r(W) r(R) was measured and changes nothing (2^-24 relative); without it the operand is 40 TMEM
+// columns per chunk and ALL chunks are TMEM-resident: the tensor core reads only the small B operand from shared memory.
 //
 // Kernel structure (from the ncu captures, profiles/r01_edge_ncu.md):
 //   * gathers are software-pipelined: two register banks of 8 edges (forward), a 16-row cp.async window per thread
@@ -86,29 +88,13 @@ __device__ __forceinline__ EdgeGeom edge_geom(const float4 raw, int E, int e_end
     g.s1 = ts;
     return g;
 }
-// Split 8 fp32 values x = hi + r (hi = RN_fp16(x), r exact in fp32) into the four fp16 planes of the B operand, one per
-// product term of (A_hi + A_lo)(B_hi + B_lo) (edge_build_filter_rows holds the matching A planes):
-//   term 0 (ll): r            term 1 (hl): r * 2^6  (against A_hi * 2^-6)
-//   term 2 (lh): hi * 2^-6    (against A_lo * 2^6)             term 3 (hh): hi
+// Split 8 fp32 values x = hi + r (hi = RN_fp16(x), r exact in fp32) into the three fp16 planes of the B operand, one per
+// product term of (A_hi + A_r)(B_hi + B_r) without the r r term (filter_planes holds the matching A planes):
+//   term 0 (hl): r * 2^6  (against A_hi * 2^-6)     term 1 (lh): hi * 2^-6  (against A_r * 2^6)     term 2 (hh): hi
 // The 2^+-6 scales keep both factors of the cross terms inside fp16's normal range for the magnitudes that occur
-// (|R| ~ 1e-3 .. 1, |W| ~ 1e-3 .. 2): with the earlier 2^+-11 scales hi * 2^-11 was a subnormal for |R| < 0.125 and the
+// (|R| ~ 1e-3 .. 1, |W| ~ 1e-3 .. 2): with the 2^+-11 scales of round 1 hi * 2^-11 was a subnormal for |R| < 0.125 and the
 // cross term lost most of its bits (B1).  What falls below the normal range only costs 2^-25 absolute times
 // the other factor.  Packed conversions: one F2FP per pair; the 2^-6 plane is an exact exponent shift done in half2.
-__device__ __forceinline__ void split4(const float (&v)[8], uint4& p_ll, uint4& p_hl, uint4& p_lh, uint4& p_hh) {
-    __half2 a[4], b[4], c[4], d[4];
-    const __half2 k = __floats2half2_rn(1.0f / 64.0f, 1.0f / 64.0f);
-#pragma unroll
-    for (int i = 0; i < 4; i++) {
-        a[i] = __floats2half2_rn(v[2 * i], v[2 * i + 1]);
-        const float2 f = __half22float2(a[i]);
-        const float r0 = v[2 * i] - f.x, r1 = v[2 * i + 1] - f.y;
-        b[i] = __floats2half2_rn(r0 * 64.0f, r1 * 64.0f);
-        c[i] = __hmul2(a[i], k);
-        d[i] = __floats2half2_rn(r0, r1);
-    }
-    p_hh = *(uint4*)a; p_hl = *(uint4*)b; p_lh = *(uint4*)c; p_ll = *(uint4*)d;
-}
-// the adjoint kernels' three planes (terms hl, lh, hh of split4, same scales)
 __device__ __forceinline__ void split3b(const float (&v)[8], uint4& p_hl, uint4& p_lh, uint4& p_hh) {
     __half2 a[4], b[4], c[4];
     const __half2 k = __floats2half2_rn(1.0f / 64.0f, 1.0f / 64.0f);
@@ -121,8 +107,8 @@ __device__ __forceinline__ void split3b(const float (&v)[8], uint4& p_hl, uint4&
     }
     p_hh = *(uint4*)a; p_hl = *(uint4*)b; p_lh = *(uint4*)c;
 }
-// byte offset of the 8-slot group h (basis slots 8h .. 8h+7) of product term t inside a B (or A) row block: K index
-// 24 t + 8 h + i, 12 groups of 8 = 96 = KP
+// byte offset of the 8-slot group h (basis slots 8h .. 8h+7) of product term t inside a B row block: K index 24 t + 8 h + i
+// (the row block keeps the 12-group stride of KP = 96; groups 9 .. 11 stay zero)
 __device__ __forceinline__ int kgrp_off(int t, int h) { return (3 * t + h) * 128; }
 
 // =============================================================================================================
@@ -140,8 +126,7 @@ struct FwdParams {
     const float4* Q4;
     const float* Q1;
     const float2* Q2;
-    const uint4* A_img;
-    const uint4* A_rows;   // [3][128][96] fp16 rows of the same operand (grouped kernel: TMEM-resident chunks s, vs)
+    const uint4* A_rows;   // [3][128][80] fp16 rows of the filter operand (edge_build_filter_rows), TMEM-resident
     float* sn;     // s' written with row stride 2F
     float* v1;
     float inv_rc;
@@ -156,6 +141,10 @@ struct FwdParams {
 };
 
 constexpr int TAB_MAX = 16;                             // species rows the shared-memory table can hold
+// three product terms (hl, lh, hh) on K = 3 x 24 + 8 zero slots = 80 = five k-steps; 40 TMEM columns per chunk, so all
+// three chunks are TMEM-resident (four terms would need 48 columns per chunk: 16 more than TMEM has)
+constexpr int KB = 80, KB_COLS = KB / 2;
+constexpr int BWD_TMEM_A = 384;                         // TMEM columns of the filter operand (behind 2 x 2 x 96 accumulator columns)
 
 // =============================================================================================================
 // adjoint message pass (sender-row gather form, painn_bwd.cu header): one 512-thread CTA per SM = two independent
@@ -173,10 +162,7 @@ constexpr int RING_BYTES = GW * F * 16;                 // 32768
 constexpr int G_OFF_B = 0, G_OFF_P = 2 * BB_BYTES, G_OFF_RING = G_OFF_P + 2 * P_BYTES, G_OFF_META = G_OFF_RING + RING_BYTES,
               G_OFF_BAR = G_OFF_META + 4 * NEB * 16, GROUP_BYTES = G_OFF_BAR + 128;
 constexpr int bwd_smem_bytes(int) { return 2 * GROUP_BYTES + 128; }
-// adjoint kernel: three product terms (hl, lh, hh: forces carry a relative tolerance, the r r term is not needed) on
-// K = 3 x 24 + 8 zero slots = 80 = five k-steps; 40 TMEM columns per chunk, all chunks TMEM-resident
-constexpr int KB = 80, KB_COLS = KB / 2;
-constexpr int BWD_TMEM_A = 384;                         // TMEM columns of the filter operand (behind 2 x 2 x 96 accumulator columns)
+
 
 // two fp32 additions in one instruction (register pairs as they come out of a 16-byte shared-memory load): the reducer
 // warps sit on the critical path of their pipeline and are bound by instruction issue
@@ -224,30 +210,25 @@ __device__ __forceinline__ void umma_f16_ts(uint32_t tmem_d, uint32_t tmem_a, ui
 constexpr int FWDG_THREADS = 512;
 constexpr int FWDG_GROUP_BYTES = ((2 * B_BYTES + 2 * NE * 16 + 64) + 127) / 128 * 128;
 constexpr int fwdg_smem_bytes(bool has_v) {
-    return (has_v ? 1 : 0) * A_CHUNK_BYTES + 2 * FWDG_GROUP_BYTES + 128 + (has_v ? 0 : TAB_MAX * F * 8);
+    return 2 * FWDG_GROUP_BYTES + 128 + (has_v ? 0 : TAB_MAX * F * 8);
 }
 template <bool HAS_V>
 __global__ void __launch_bounds__(FWDG_THREADS, 1) k_msg_fwd_g(const FwdParams p) {
     constexpr int NCH = HAS_V ? 3 : 2;
     constexpr int TCOLS = NCH * NE;                 // TMEM columns per buffer
     extern __shared__ __align__(128) uint8_t smem[];
-    constexpr int NSM = NCH - 2;                    // chunks kept in shared memory (vv); s and vs live in TMEM
-    uint8_t* sA = smem;
     const int tid = threadIdx.x, grp = tid >> 8, ltid = tid & 255, lwarp = ltid >> 5, lane = tid & 31;
-    uint8_t* gbase = smem + NSM * A_CHUNK_BYTES + grp * FWDG_GROUP_BYTES;
+    uint8_t* gbase = smem + grp * FWDG_GROUP_BYTES;
     uint8_t* sB = gbase;
     float4* sMeta = (float4*)(sB + 2 * B_BYTES);   // [2][NE] (u_e, sender index)
     uint64_t* bars = (uint64_t*)(sMeta + 2 * NE);
     uint64_t* b_full = bars;          // [2] producers -> MMA (and consumers: sender indices readable)  (count 96)
     uint64_t* t_full = bars + 2;      // [2] MMA commit -> consumers (count 1)
     const int NB = 1 + grp * 2;       // named barriers NB + buf of this group (consumers -> producers: tile consumed)
-    uint32_t* tmem_slot = (uint32_t*)(smem + NSM * A_CHUNK_BYTES + 2 * FWDG_GROUP_BYTES);
+    uint32_t* tmem_slot = (uint32_t*)(smem + 2 * FWDG_GROUP_BYTES);
     float2* sTab = (float2*)(tmem_slot + 32);          // [n_tab][F] species table (layer 0 only), shared by both groups
 
     {
-        const uint4* src = p.A_img + 2 * (A_CHUNK_BYTES / 16);        // chunk vv of the shared-memory image
-        uint4* dst = (uint4*)sA;
-        for (int i = tid; i < NSM * A_CHUNK_BYTES / 16; i += FWDG_THREADS) dst[i] = src[i];
         uint4* zb = (uint4*)sB;
         for (int i = ltid; i < 2 * B_BYTES / 16; i += 256) zb[i] = make_uint4(0, 0, 0, 0);
         if (!HAS_V)
@@ -262,28 +243,32 @@ __global__ void __launch_bounds__(FWDG_THREADS, 1) k_msg_fwd_g(const FwdParams p
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    // chunks s and vs of the filter operand into TMEM (lane = channel row, 48 columns = 96 fp16 each): columns 192..239
-    // and 448..495, the gaps behind the two groups' accumulators (2 buffers x TCOLS <= 192 columns each)
+    // all chunks of the filter operand into TMEM (lane = channel row, KB_COLS = 40 columns = 80 fp16 per chunk: three
+    // product terms, see KB): columns 384 .. behind the two groups' accumulators (2 x 2 x 96 columns)
     if (tid < 128) {
 #pragma unroll
-        for (int c = 0; c < 2; c++) {
-            const uint32_t abase = *tmem_slot + 192 + c * 256 + ((uint32_t)((tid >> 5) * 32) << 16);
-            const uint4* src = p.A_rows + ((size_t)c * 128 + tid) * 12;
+        for (int c = 0; c < NCH; c++) {
+            const uint32_t abase = *tmem_slot + BWD_TMEM_A + c * KB_COLS + ((uint32_t)((tid >> 5) * 32) << 16);
+            const uint4* src = p.A_rows + ((size_t)c * 128 + tid) * (KB_COLS / 4);
 #pragma unroll
-            for (int j = 0; j < 3; j++) {
+            for (int j = 0; j < 2; j++) {
                 uint32_t r[16];
 #pragma unroll
                 for (int q = 0; q < 4; q++) { const uint4 v = src[j * 4 + q]; r[4 * q] = v.x; r[4 * q + 1] = v.y; r[4 * q + 2] = v.z; r[4 * q + 3] = v.w; }
                 tmem_st16(abase + j * 16, r);
             }
+            uint32_t r8[8];
+#pragma unroll
+            for (int q = 0; q < 2; q++) { const uint4 v = src[8 + q]; r8[4 * q] = v.x; r8[4 * q + 1] = v.y; r8[4 * q + 2] = v.z; r8[4 * q + 3] = v.w; }
+            tmem_st8(abase + 32, r8);
         }
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     }
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    const uint32_t tmem_base = *tmem_slot + grp * 256;
-    const uint32_t tmem_A = *tmem_slot + 192;
+    const uint32_t tmem_base = *tmem_slot + grp * 192;
+    const uint32_t tmem_A = *tmem_slot + BWD_TMEM_A;
 
     const long long N = p.N;
     const int apu = p.atoms_per_unit;
@@ -467,14 +452,13 @@ __global__ void __launch_bounds__(FWDG_THREADS, 1) k_msg_fwd_g(const FwdParams p
                     }
                     vals[i] = R;
                 }
-                uint4 p0, p1, p2, p3;
-                split4(vals, p0, p1, p2, p3);
+                uint4 p0, p1, p2;
+                split3b(vals, p0, p1, p2);
                 if (it >= 2) bar_sync(NB + buf, 224);   // tile it - 2 consumed (hardware-blocking wait, no spin)
                 uint8_t* bb = sB + buf * B_BYTES + (e >> 3) * SBO + (e & 7) * 16;
-                *(uint4*)(bb + kgrp_off(0, h)) = p0;      // term 0: k = b        lo(R)
-                *(uint4*)(bb + kgrp_off(1, h)) = p1;      // term 1: k = 24 + b   lo(R) 2^6
-                *(uint4*)(bb + kgrp_off(2, h)) = p2;      // term 2: k = 48 + b   hi(R) 2^-6
-                *(uint4*)(bb + kgrp_off(3, h)) = p3;      // term 3: k = 72 + b   hi(R)
+                *(uint4*)(bb + kgrp_off(0, h)) = p0;      // term 0: k = b        lo(R) 2^6
+                *(uint4*)(bb + kgrp_off(1, h)) = p1;      // term 1: k = 24 + b   hi(R) 2^-6
+                *(uint4*)(bb + kgrp_off(2, h)) = p2;      // term 2: k = 48 + b   hi(R)
                 if (h == 0) {
                     float mw = g.r.w;                                             // sender index ...
                     if (!HAS_V) mw = __int_as_float(__ldg(p.types + __float_as_int(g.r.w)));   // ... or its species (layer 0)
@@ -488,7 +472,7 @@ __global__ void __launch_bounds__(FWDG_THREADS, 1) k_msg_fwd_g(const FwdParams p
         // ===================== MMA issuer: the warp stays converged, one elected lane issues (descriptors in uniform registers) =====================
         {
             const uint32_t idesc = (1u << 4) | ((uint32_t)(NE >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);   // f16 x f16 -> f32
-            const uint32_t a_base = smem_u32(sA), b_base = smem_u32(sB);
+            const uint32_t b_base = smem_u32(sB);
             uint32_t it = 0;
             for (long long u = u0; u < n_units; u += ustride) {
                 const long long a0 = u * apu;
@@ -504,11 +488,9 @@ __global__ void __launch_bounds__(FWDG_THREADS, 1) k_msg_fwd_g(const FwdParams p
                         for (int c = 0; c < NCH; c++) {
                             const uint32_t d = tmem_base + buf * TCOLS + c * NE;
 #pragma unroll
-                            for (int o = 0; o < 6; o++) {
-                                const int kk = o;                    // ascending K: the small terms (ll, hl, lh) first, the main term (hh) last
+                            for (int kk = 0; kk < KB_COLS / 8; kk++) {     // ascending K: the cross terms first, the main term (hh) last
                                 const uint64_t bd = make_desc_nosw(b_base + buf * B_BYTES + kk * 2 * LBO, LBO, SBO);
-                                if (c < 2) umma_f16_ts(d, tmem_A + c * 256 + kk * 8, bd, idesc, o != 0);
-                                else umma_f16(d, make_desc_nosw(a_base + kk * 2 * LBO, LBO, SBO), bd, idesc, o != 0);
+                                umma_f16_ts(d, tmem_A + c * KB_COLS + kk * 8, bd, idesc, kk != 0);
                             }
                         }
                         umma_commit(&t_full[buf]);
@@ -533,8 +515,7 @@ struct BwdParams {
     const float* phi;
     const float* v_in;
     const float* v1b;
-    const uint4* A_img;    // chunk vv of the no-swizzle K-major image (shared-memory A operand)
-    const uint4* A_rows;   // [3][128][96] fp16 rows: chunks s, vs become TMEM-resident A operands
+    const uint4* A_rows;   // [3][128][80] fp16 rows of the filter operand, TMEM-resident
     float* phib;
     float* vb_out;
     float4* G;
@@ -947,7 +928,7 @@ struct Bwd0Params {
     const int* types;
     const float2* tab;     // [n_tab][F] (phi^s, phi^vs) per species
     const int* rev;
-    const uint4* A_img;    // [2 chunks][128 rows][96 fp16] row-major (k = 24 term + basis slot): TMEM-resident A operand
+    const uint4* A_img;    // [>= 2 chunks][128 rows][80 fp16] rows (edge_build_filter_rows): TMEM-resident A operand
     float4* G;
     float inv_rc;
     int K;
@@ -957,7 +938,7 @@ struct Bwd0Params {
 };
 constexpr int G0_OFF_SPEC = G_OFF_BAR + 128, G0_OFF_TAB = G0_OFF_SPEC + 4 * NEB * 4, GROUP0_BYTES = G0_OFF_TAB;
 constexpr int bwd0_smem_bytes() { return 2 * GROUP0_BYTES + TAB_MAX * F * 8 + 128; }
-constexpr int BWD0_TMEM_A = 128;                        // TMEM columns 128..223: the filter operand (2 chunks x 48 columns)
+constexpr int BWD0_TMEM_A = 128;                        // TMEM columns 128..207: the filter operand (2 chunks x 40 columns)
 
 __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p) {
     constexpr int NCH = 2;
@@ -989,21 +970,24 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    // filter operand into TMEM (lane = channel row, 48 columns = 96 fp16 per chunk): the MMAs then read only the small B
-    // operand from shared memory -- the 72 KB image and its re-read by every MMA (ncu: 35 % of the shared-memory data
-    // pipe next to an LSU pipe that was 82 % busy) are gone
+    // filter operand into TMEM (lane = channel row, KB_COLS = 40 columns = 80 fp16 per chunk): the MMAs read only the small
+    // B operand from shared memory
     if (tid < 128) {
-        const uint32_t abase = *tmem_slot + BWD0_TMEM_A + ((uint32_t)((tid >> 5) * 32) << 16);
 #pragma unroll
         for (int c = 0; c < NCH; c++) {
-            const uint4* src = p.A_img + ((size_t)c * 128 + tid) * 12;       // 96 fp16 = 12 x 16 B
+            const uint32_t abase = *tmem_slot + BWD0_TMEM_A + c * KB_COLS + ((uint32_t)((tid >> 5) * 32) << 16);
+            const uint4* src = p.A_img + ((size_t)c * 128 + tid) * (KB_COLS / 4);
 #pragma unroll
-            for (int j = 0; j < 3; j++) {
+            for (int j = 0; j < 2; j++) {
                 uint32_t r[16];
 #pragma unroll
                 for (int q = 0; q < 4; q++) { const uint4 v = src[j * 4 + q]; r[4 * q] = v.x; r[4 * q + 1] = v.y; r[4 * q + 2] = v.z; r[4 * q + 3] = v.w; }
-                tmem_st16(abase + c * 48 + j * 16, r);
+                tmem_st16(abase + j * 16, r);
             }
+            uint32_t r8[8];
+#pragma unroll
+            for (int q = 0; q < 2; q++) { const uint4 v = src[8 + q]; r8[4 * q] = v.x; r8[4 * q + 1] = v.y; r8[4 * q + 2] = v.z; r8[4 * q + 3] = v.w; }
+            tmem_st8(abase + 32, r8);
         }
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     }
@@ -1102,7 +1086,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
             float4 raw_n = load_edge_raw(p.ej, e_begin + e, h < 3 ? e_end : 0);
             for (int t = 0; t < ntiles; t++, it++) {
                 const int buf = it & 1;
-                uint4 q[8];
+                uint4 q[6];
                 float4 meta_v = make_float4(0.f, 0.f, 0.f, 0.f);
                 const float4 raw = raw_n;
                 if (t + 1 < ntiles) raw_n = load_edge_raw(p.ej, e_begin + (t + 1) * NEB + e, h < 3 ? e_end : 0);
@@ -1129,8 +1113,8 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
                             sn_ = tt;
                         }
                     }
-                    split4(vals, q[0], q[1], q[2], q[3]);
-                    split4(dvals, q[4], q[5], q[6], q[7]);
+                    split3b(vals, q[0], q[1], q[2]);
+                    split3b(dvals, q[3], q[4], q[5]);
                     meta_v = make_float4(g.r.x * g.inv_d, g.r.y * g.inv_d, g.r.z * g.inv_d, g.inv_d);
                 }
                 __syncwarp();
@@ -1141,7 +1125,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
                         const int row = z * NEB + e;
                         uint8_t* bb = sB + buf * BB_BYTES + (row >> 3) * SBO + (row & 7) * 16;
 #pragma unroll
-                        for (int tm = 0; tm < 4; tm++) *(uint4*)(bb + kgrp_off(tm, h)) = q[4 * z + tm];
+                        for (int tm = 0; tm < 3; tm++) *(uint4*)(bb + kgrp_off(tm, h)) = q[3 * z + tm];
                     }
                     if (h == 0) { sMeta[(it & 3) * NEB + e] = meta_v; sSpec[(it & 3) * NEB + e] = spec_v; }
                 }
@@ -1234,10 +1218,9 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd0(const Bwd0Params p)
                     for (int c = 0; c < NCH; c++) {
                         const uint32_t d = tmem_base + buf * TCOLS + c * 2 * NEB;
 #pragma unroll
-                        for (int o = 0; o < 6; o++) {
-                            const int kk = o;
+                        for (int kk = 0; kk < KB_COLS / 8; kk++) {
                             const uint64_t bd = make_desc_nosw(b_base + buf * BB_BYTES + kk * 2 * LBO, LBO, SBO);
-                            umma_f16_ts(d, tmem_A + c * 48 + kk * 8, bd, idesc, o != 0);
+                            umma_f16_ts(d, tmem_A + c * KB_COLS + kk * 8, bd, idesc, kk != 0);
                         }
                     }
                     umma_commit(&t_full[buf]);
@@ -1291,54 +1274,24 @@ void make_gather_rows_bwd(const Launch& L, long long N, const float* s1b, const 
     KLAUNCH(L);
 }
 
-// host: the four fp16 planes of one filter weight w = hi + r (same split as split4() of the B operand; the term order
-// (ll, hl, lh, hh) pairs plane t of A with plane t of B):  r | hi 2^-6 | r 2^6 | hi
-static void filter_planes(float w, unsigned short (&bits)[4]) {
+// host: the three fp16 planes of one filter weight w = hi + r, term order (hl, lh, hh) as in split3b:  hi 2^-6 | r 2^6 | hi
+static void filter_planes(float w, unsigned short (&bits)[3]) {
     const __half hi = __float2half_rn(w);
     const float hif = __half2float(hi), r = w - hif;
-    const __half vals[4] = {__float2half_rn(r), __float2half_rn(hif * (1.0f / 64.0f)), __float2half_rn(r * 64.0f), hi};
-    for (int t = 0; t < 4; t++) memcpy(&bits[t], &vals[t], 2);
+    const __half vals[3] = {__float2half_rn(hif * (1.0f / 64.0f)), __float2half_rn(r * 64.0f), hi};
+    for (int t = 0; t < 3; t++) memcpy(&bits[t], &vals[t], 2);
 }
-// host: filter operand (bf | Wf) of one layer as plain rows [3 chunks][128 channels][96 fp16], k = 24 term + basis slot
-// (basis slot 0 = the bias bf) -- the TMEM-resident A operand
+// host: filter operand (bf | Wf) of one layer as plain rows [3 chunks][128 channels][80 fp16], k = 24 term + basis slot
+// (basis slot 0 = the bias bf), k >= 72 zero -- the TMEM-resident A operand of every tensor-core edge kernel
 void edge_build_filter_rows(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img) {
-    img.assign((size_t)3 * ev3::F * ev3::KP, 0);
-    for (int c = 0; c < 3; c++)
-        for (int r = 0; r < ev3::F; r++)
-            for (int b = 0; b <= K; b++) {
-                const float w = b == 0 ? bf[c * ev3::F + r] : Wf[(size_t)(c * ev3::F + r) * K + (b - 1)];
-                unsigned short bits[4];
-                filter_planes(w, bits);
-                for (int t = 0; t < 4; t++) img[((size_t)c * ev3::F + r) * ev3::KP + t * 24 + b] = bits[t];
-            }
-}
-// host: the adjoint kernel's operand, rows [3 chunks][128 channels][80 fp16]: terms (hl, lh, hh) at k = 24 t + b, k >= 72 zero
-void edge_build_filter_rows_bwd(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img) {
     img.assign((size_t)3 * ev3::F * ev3::KB, 0);
     for (int c = 0; c < 3; c++)
         for (int r = 0; r < ev3::F; r++)
             for (int b = 0; b <= K; b++) {
                 const float w = b == 0 ? bf[c * ev3::F + r] : Wf[(size_t)(c * ev3::F + r) * K + (b - 1)];
-                unsigned short bits[4];
-                filter_planes(w, bits);                         // (r, hi 2^-6, r 2^6, hi)
-                for (int t = 0; t < 3; t++) img[((size_t)c * ev3::F + r) * ev3::KB + t * 24 + b] = bits[t + 1];
-            }
-}
-// host: the same numbers as the K-major no-swizzle shared-memory image of the A operand (3 chunks of A_CHUNK_BYTES)
-void edge_build_filter_image(const float* Wf, const float* bf, int K, std::vector<unsigned short>& img) {
-    using namespace ev3;
-    img.assign(3 * A_CHUNK_BYTES / 2, 0);
-    for (int c = 0; c < 3; c++)
-        for (int r = 0; r < F; r++)
-            for (int b = 0; b <= K; b++) {
-                const float w = b == 0 ? bf[c * F + r] : Wf[(size_t)(c * F + r) * K + (b - 1)];
-                unsigned short bits[4];
+                unsigned short bits[3];
                 filter_planes(w, bits);
-                for (int t = 0; t < 4; t++) {
-                    const int k = t * 24 + b;
-                    const size_t off = (size_t)c * A_CHUNK_BYTES + (r / 8) * SBO + (k / 8) * LBO + (r % 8) * 16 + (k % 8) * 2;
-                    img[off / 2] = bits[t];
-                }
+                for (int t = 0; t < 3; t++) img[((size_t)c * ev3::F + r) * ev3::KB + t * 24 + b] = bits[t];
             }
 }
 
@@ -1352,14 +1305,14 @@ static int sm_count() {
     return n_sm;
 }
 
-// F = 128, K <= 23 only.  Q4/Q1 from make_gather_rows; A_img / A_rows from edge_build_filter_image / _rows.  has_v = false:
+// F = 128, K <= 23 only.  Q4/Q1 from make_gather_rows; A_rows from edge_build_filter_rows.  has_v = false:
 // layer 0 through the species table.
 bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* s,
-                    const float* v, const float* Q4, const float* Q1, const void* A_img, const void* A_rows, float* sn, float* v1,
+                    const float* v, const float* Q4, const float* Q1, const void* A_rows, float* sn, float* v1,
                     bool has_v, const int* types_s, const float* tab, int n_tab, const float2* xph) {
     using namespace ev3;
     if (N == 0) return true;
-    if (K > 23 || !A_rows || !A_img) return false;
+    if (K > 23 || !A_rows) return false;
     if (!has_v && (!tab || !types_s || n_tab > TAB_MAX)) return false;
     static bool attr = false;
     if (!attr) {
@@ -1368,7 +1321,7 @@ bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
             return false;
         attr = true;
     }
-    FwdParams p{N, row_ptr, ej, s, v, (const float4*)Q4, Q1, (const float2*)Q4, (const uint4*)A_img, (const uint4*)A_rows, sn, v1,
+    FwdParams p{N, row_ptr, ej, s, v, (const float4*)Q4, Q1, (const float2*)Q4, (const uint4*)A_rows, sn, v1,
                 1.0f / rc, K, L.apu_fwd, types_s, (const float2*)tab, n_tab, xph};
     const long long n_units = (N + p.atoms_per_unit - 1) / p.atoms_per_unit;
     // one CTA per SM, two 8-warp pipelines sharing the TMEM-resident filter operand
@@ -1381,7 +1334,7 @@ bool message_fwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
 
 // layer0: v_in = 0 and no sender adjoint wanted (phib / vb_out untouched)
 bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* row_ptr, const float4* ej, const float* Gb,
-                    const float* phi, const float* v_in, const float* v1b, const void* A_img, const void* A_rows, float* phib,
+                    const float* phi, const float* v_in, const float* v1b, const void* A_rows, float* phib,
                     float* vb_out, float4* G, bool first, bool layer0) {
     using namespace ev3;
     if (N == 0) return true;
@@ -1393,7 +1346,7 @@ bool message_bwd_v3(const Launch& L, long long N, int K, float rc, const int* ro
             return false;
         attr = true;
     }
-    BwdParams p{N, row_ptr, ej, (const float4*)Gb, phi, v_in, v1b, (const uint4*)A_img, (const uint4*)A_rows, phib, vb_out, G,
+    BwdParams p{N, row_ptr, ej, (const float4*)Gb, phi, v_in, v1b, (const uint4*)A_rows, phib, vb_out, G,
                 1.0f / rc, K, L.apu_bwd, first ? 1 : 0};
     const long long n_units = (N + p.atoms_per_unit - 1) / p.atoms_per_unit;
     const int grid = (int)std::min<long long>((n_units + 1) / 2, (long long)sm_count());

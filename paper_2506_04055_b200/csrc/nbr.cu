@@ -516,68 +516,93 @@ void nbr_sup_fill(const Launch& L, long long N, Grid g, const NbrSearch& S, cons
     k_sup_fill<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, S, n_rows_p, sup_ptr, sup_j, sup_code);
     KLAUNCH(L);
 }
-// candidates of row a from the superset list, tested with the SAME fp64 expression as visit_neighbors on the current
-// positions as given (pos_s / wrap_s in final order, refreshed by k_reuse_prep): identical edge sets, bit for bit
-template <class Fn>
-__device__ __forceinline__ void visit_superset(long long a, const Grid& g, const double* __restrict__ pos_s,
-                                               const signed char* __restrict__ wrap_s, const int* __restrict__ sup_ptr,
-                                               const int* __restrict__ sup_j, const unsigned char* __restrict__ sup_code, Fn f) {
-    const double xa = pos_s[3 * a], ya = pos_s[3 * a + 1], za = pos_s[3 * a + 2];
-    const int wa0 = wrap_s[3 * a], wa1 = wrap_s[3 * a + 1], wa2 = wrap_s[3 * a + 2];
-    for (int x = sup_ptr[a], x1 = sup_ptr[a + 1]; x < x1; x++) {
-        const int b = sup_j[x], code = sup_code[x];
-        double Sx = 0.0, Sy = 0.0, Sz = 0.0;
-        if (g.periodic) {
-            Sx = (double)(code / 9 - 1 - (int)wrap_s[3 * b] + wa0);
-            Sy = (double)((code / 3) % 3 - 1 - (int)wrap_s[3 * b + 1] + wa1);
-            Sz = (double)(code % 3 - 1 - (int)wrap_s[3 * b + 2] + wa2);
-        }
-        double ex = __dsub_rn(__dadd_rn(pos_s[3 * b], __dmul_rn(Sx, g.box[0])), xa);
-        double ey = __dsub_rn(__dadd_rn(pos_s[3 * b + 1], __dmul_rn(Sy, g.box[1])), ya);
-        double ez = __dsub_rn(__dadd_rn(pos_s[3 * b + 2], __dmul_rn(Sz, g.box[2])), za);
-        double d2 = __dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez));
-        if (d2 < g.rc2) f(b, code, ex, ey, ez);
+// One warp per row: lanes take the candidates of the superset row 32 at a time (coalesced reads of sup_j / sup_code, the
+// position gathers of a batch in flight together) and test them with the SAME fp64 expression as visit_neighbors on the
+// current positions as given (pos_s / wrap_s in final order, refreshed by k_reuse_prep): identical edge sets, bit for
+// bit.  Kept candidates are compacted in candidate order (ballot + prefix popcount), so count and fill agree.
+struct SupCand {
+    int b, code;
+    double ex, ey, ez;
+    bool keep;
+};
+__device__ __forceinline__ SupCand test_candidate(int x, int x1, long long a, const Grid& g, const double* __restrict__ pos_s,
+                                                  const signed char* __restrict__ wrap_s, const int* __restrict__ sup_j,
+                                                  const unsigned char* __restrict__ sup_code, double xa, double ya, double za,
+                                                  int wa0, int wa1, int wa2) {
+    SupCand c;
+    c.keep = false;
+    c.b = 0; c.code = 13; c.ex = c.ey = c.ez = 0.0;
+    if (x >= x1) return c;
+    const int b = sup_j[x], code = sup_code[x];
+    double Sx = 0.0, Sy = 0.0, Sz = 0.0;
+    if (g.periodic) {
+        Sx = (double)(code / 9 - 1 - (int)wrap_s[3 * b] + wa0);
+        Sy = (double)((code / 3) % 3 - 1 - (int)wrap_s[3 * b + 1] + wa1);
+        Sz = (double)(code % 3 - 1 - (int)wrap_s[3 * b + 2] + wa2);
     }
+    c.ex = __dsub_rn(__dadd_rn(pos_s[3 * b], __dmul_rn(Sx, g.box[0])), xa);
+    c.ey = __dsub_rn(__dadd_rn(pos_s[3 * b + 1], __dmul_rn(Sy, g.box[1])), ya);
+    c.ez = __dsub_rn(__dadd_rn(pos_s[3 * b + 2], __dmul_rn(Sz, g.box[2])), za);
+    const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(c.ex, c.ex), __dmul_rn(c.ey, c.ey)), __dmul_rn(c.ez, c.ez));
+    c.keep = d2 < g.rc2;
+    c.b = b; c.code = code;
+    (void)a;
+    return c;
 }
-__global__ void __launch_bounds__(128) k_refilter_count(long long N, Grid g, const double* __restrict__ pos_s,
+__global__ void __launch_bounds__(256) k_refilter_count(long long N, Grid g, const double* __restrict__ pos_s,
                                                         const signed char* __restrict__ wrap_s, const int* __restrict__ sup_ptr,
                                                         const int* __restrict__ sup_j, const unsigned char* __restrict__ sup_code,
                                                         int* __restrict__ row_cnt, unsigned long long* __restrict__ real_total) {
-    long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    const long long a = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (a >= N) return;
+    const double xa = pos_s[3 * a], ya = pos_s[3 * a + 1], za = pos_s[3 * a + 2];
+    const int wa0 = wrap_s[3 * a], wa1 = wrap_s[3 * a + 1], wa2 = wrap_s[3 * a + 2];
+    const int x0 = sup_ptr[a], x1 = sup_ptr[a + 1];
     int cnt = 0;
-    if (a < N) {
-        visit_superset(a, g, pos_s, wrap_s, sup_ptr, sup_j, sup_code, [&](int, int, double, double, double) { cnt++; });
-        row_cnt[a] = (cnt + ROW_PAD - 1) & ~(ROW_PAD - 1);
+    for (int x = x0; x < x1; x += 32) {
+        const SupCand c = test_candidate(x + lane, x1, a, g, pos_s, wrap_s, sup_j, sup_code, xa, ya, za, wa0, wa1, wa2);
+        cnt += __popc(__ballot_sync(0xffffffffu, c.keep));
     }
-    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
-    if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(real_total, (unsigned long long)cnt);
+    if (lane == 0) {
+        row_cnt[a] = (cnt + ROW_PAD - 1) & ~(ROW_PAD - 1);
+        if (cnt) atomicAdd(real_total, (unsigned long long)cnt);
+    }
 }
-__global__ void __launch_bounds__(128) k_refilter_fill(long long N, Grid g, const double* __restrict__ pos_s,
+__global__ void __launch_bounds__(256) k_refilter_fill(long long N, Grid g, const double* __restrict__ pos_s,
                                                        const signed char* __restrict__ wrap_s, const int* __restrict__ sup_ptr,
                                                        const int* __restrict__ sup_j, const unsigned char* __restrict__ sup_code,
                                                        const int* __restrict__ row_ptr, long long cap_edges, EdgeOut o,
                                                        int* __restrict__ flags) {
-    long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    const long long a = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
     if (a >= N) return;
     long long e = row_ptr[a];
-    if ((long long)row_ptr[a + 1] > cap_edges) { atomicOr(flags, FLAG_EDGE_OVERFLOW); return; }   // (cannot happen: bound reserved at build)
-    visit_superset(a, g, pos_s, wrap_s, sup_ptr, sup_j, sup_code, [&](int b, int code, double ex, double ey, double ez) {
-        emit_edge(o, e, b, code, ex, ey, ez);
-        e++;
-    });
-    emit_padding(o, e, row_ptr[a + 1], a);
+    const long long e1 = row_ptr[a + 1];
+    if (e1 > cap_edges) { if (lane == 0) atomicOr(flags, FLAG_EDGE_OVERFLOW); return; }   // (cannot happen: bound reserved at build)
+    const double xa = pos_s[3 * a], ya = pos_s[3 * a + 1], za = pos_s[3 * a + 2];
+    const int wa0 = wrap_s[3 * a], wa1 = wrap_s[3 * a + 1], wa2 = wrap_s[3 * a + 2];
+    const int x0 = sup_ptr[a], x1 = sup_ptr[a + 1];
+    for (int x = x0; x < x1; x += 32) {
+        const SupCand c = test_candidate(x + lane, x1, a, g, pos_s, wrap_s, sup_j, sup_code, xa, ya, za, wa0, wa1, wa2);
+        const unsigned m = __ballot_sync(0xffffffffu, c.keep);
+        if (c.keep) emit_edge(o, e + __popc(m & ((1u << lane) - 1u)), c.b, c.code, c.ex, c.ey, c.ez);
+        e += __popc(m);
+    }
+    // dummy slots of the padded row
+    for (long long k = e + lane; k < e1; k += 32) emit_padding(o, k, k + 1, a);
 }
 void nbr_refilter_count(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s, const int* sup_ptr,
                         const int* sup_j, const unsigned char* sup_code, int* row_cnt, unsigned long long* real_total) {
     if (N == 0) return;
-    k_refilter_count<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, pos_s, wrap_s, sup_ptr, sup_j, sup_code, row_cnt, real_total);
+    k_refilter_count<<<(unsigned)((N * 32 + 255) / 256), 256, 0, L.stream>>>(N, g, pos_s, wrap_s, sup_ptr, sup_j, sup_code, row_cnt, real_total);
     KLAUNCH(L);
 }
 void nbr_refilter_fill(const Launch& L, long long N, Grid g, const double* pos_s, const signed char* wrap_s, const int* sup_ptr,
                        const int* sup_j, const unsigned char* sup_code, const int* row_ptr, long long cap_edges, EdgeOut o, int* flags) {
     if (N == 0) return;
     if (N >= (1ll << 26)) o.key = nullptr;
-    k_refilter_fill<<<(unsigned)((N + 127) / 128), 128, 0, L.stream>>>(N, g, pos_s, wrap_s, sup_ptr, sup_j, sup_code, row_ptr, cap_edges, o, flags);
+    k_refilter_fill<<<(unsigned)((N * 32 + 255) / 256), 256, 0, L.stream>>>(N, g, pos_s, wrap_s, sup_ptr, sup_j, sup_code, row_ptr, cap_edges, o, flags);
     KLAUNCH(L);
 }
 // A step that reuses the list: current positions into the final order, wrap counts continued from the build
