@@ -88,8 +88,13 @@ int mlp_create(const void* weights, size_t nbytes, int n_species, double cutoff,
  *   virial       DEVICE fp64 [6]  xx, yy, zz, xy, xz, yz  (W_ab = -sum_e r_e,a g_e,b, off-diagonals symmetrised;
  *                not divided by the volume)
  *   cuda_stream  cudaStream_t (NULL = default stream)
- * Errors: MLP_ERR_ARG, MLP_ERR_BOX_TOO_SMALL, MLP_ERR_TYPE_RANGE, MLP_ERR_NONFINITE, MLP_ERR_NOMEM, MLP_ERR_CUDA.
- * MLP_ERR_TYPE_RANGE / MLP_ERR_NONFINITE are detected on the device and reported by this same call.
+ * Errors: MLP_ERR_ARG (also: a ghost_owner entry outside 0 .. n_local-1), MLP_ERR_BOX_TOO_SMALL, MLP_ERR_TYPE_RANGE,
+ * MLP_ERR_NONFINITE, MLP_ERR_NOMEM, MLP_ERR_CUDA.  MLP_ERR_TYPE_RANGE / MLP_ERR_NONFINITE / the owner range are detected on
+ * the device and reported by this same call.
+ * Host synchronisation: a call that builds the list reads flags and totals back once (twice in ghost mode: bounding box),
+ * the overflow check of PAPER.md:84; a call that reuses the kept list reads one flag word (displacement test) and is
+ * otherwise asynchronous.  Threads: one model must not be used from two threads at once; different models are independent
+ * (no process-wide state).
  */
 int mlp_compute(mlp_model* m, const double* pos, const int* types, const double* box, long long n_local,
                 long long n_ghost, const int* ghost_owner, double* energy, double* forces, double* virial,
@@ -98,7 +103,9 @@ int mlp_compute(mlp_model* m, const double* pos, const int* types, const double*
 /*
  * mlp_compute_host -- the same computation with HOST buffers for every argument (the end-to-end call an MD
  * engine with host-resident atoms makes; "transforms and copies data to the device ... copies
- * forces back").  Host<->device copies go through pinned staging buffers owned by the model; synchronous.
+ * forces back").  The copies are cudaMemcpyAsync on the model's own stream straight from / to the caller's buffers (pin
+ * them for full PCIe speed; pageable memory works and is staged by the driver); device staging buffers are owned by the
+ * model.  Synchronous: returns when the outputs are in the caller's buffers.
  */
 int mlp_compute_host(mlp_model* m, const double* pos, const int* types, const double* box, long long n_local,
                      long long n_ghost, const int* ghost_owner, double* energy, double* forces, double* virial);
@@ -123,13 +130,15 @@ int mlp_get_layer_state(mlp_model* m, int t, float* out);
 /*
  * mlp_debug_gemm -- test export of the per-atom linear-layer kernel:
  *   C[M x N] (+)= A[M x K] . W[N x K]^T + bias.   A, C: DEVICE fp32 row-major (ld = K resp. N); W [N x K], bias [N]
- *   (or NULL): HOST fp32.  path 0 = tensor-core (tcgen05 3xTF32) when the shape is covered, 1 = plain fp32 SIMT.
- *   *used_tc (may be NULL) receives 1 if the tensor-core kernel ran.  Synchronous.
+ *   (or NULL): HOST fp32.  path 0 = tcgen05 3xTF32 (the adjoint GEMMs) when the shape is covered, 1 = plain fp32
+ *   (FFMA / SIMT), 2 = tcgen05 exact integer slices (the forward GEMMs; MLP_ERR_ARG when the shape is not covered).
+ *   *used_tc (may be NULL) receives 1 if a tensor-core kernel ran.  Synchronous.
  */
 int mlp_debug_gemm(const float* A, const float* W, const float* bias, float* C, long long M, int N, int K,
                    int accumulate, int path, int* used_tc);
 
-/* mlp_get_stats -- copy the statistics of the last call. */
+/* mlp_get_stats -- copy the statistics of the last call (waits for that call when it was served by the kept list: its
+ * edge count is read back lazily). */
 int mlp_get_stats(mlp_model* m, mlp_stats* out);
 
 /*
@@ -139,20 +148,32 @@ int mlp_get_stats(mlp_model* m, mlp_stats* out);
  */
 int mlp_get_stage_ms(mlp_model* m, int max_stages, const char** names, float* ms);
 
-/* mlp_set_option -- integer knobs: "stage_timing" (0/1), "edge_capacity" (force an initial edge capacity,
- * test hook for the overflow / regrow path of PAPER.md:84-86), and experiment switches that select between
- * implementations of the same arithmetic (defaults are the shipped path; DESIGN.md sections 5-7b):
- *   "edge_path"       0 gen-3 tensor-core edge kernels (F = 128, K <= 23), 1 plain fp32 kernels, 2 / 3 earlier generations
- *   "l0_collapse"     1 layer-0 adjoint with the channel contraction hoisted into two GEMMs (n_species (K+1) <= 128),
- *                     0 per-edge channel sums (k_msg_bwd0)
- *   "gemm_fwd_exact"  1 forward GEMMs on tcgen05 with exact integer slices, 0 fp32 FFMA kernel
+/* mlp_set_option -- integer knobs of ONE model (nothing is process-wide; setting an option drops the kept neighbour list
+ * and the captured step of that model):
+ *   "skin_mA"         Verlet skin in 1e-3 Angstrom, default 1000.  > 0: the list is built at cutoff + skin
+ *                     and kept; a later call whose atoms have all moved less than skin / 2 (minimum image), with the same
+ *                     atom counts, species and box, only re-filters it at the cutoff (exact: same fp64 predicate, same edge
+ *                     set) and replays the captured CUDA graph.  0: every call rebuilds the list (the metric of bench.py)
+ *   "prune"           1 (default): ghost mode drops the atoms no local atom reaches within T hops and restricts layer t to
+ *                     the atoms within T - 1 - t hops (Fig. 1e; exact).  mlp_get_neighbors then returns the
+ *                     sub-graph over the reached atoms.  0: all given atoms are carried through all layers
+ *   "use_graph"       1 (default): steps that reuse the list are captured once and replayed with cudaGraphLaunch
+ *   "stage_timing"    0/1: CUDA-event stage timers for mlp_get_stage_ms (disables graph replay while on)
+ *   "edge_capacity"   TEST HOOK for the overflow / regrow path: drops the edge buffers and reallocates them
+ *                     at exactly this size -- the one place where a buffer may shrink (mlp_compute itself only grows them)
+ * and switches that select between implementations of the same arithmetic (defaults are the shipped path):
+ *   "edge_path"       0 tensor-core edge kernels (F = 128, K <= 23), 1 plain fp32 kernels
+ *   "l0_collapse"     1 layer-0 message passes with the channel contraction hoisted into GEMMs (n_species (K+1) <= 128),
+ *                     0 per-edge channel kernels through the species table
+ *   "gemm_fwd_exact"  1 forward GEMMs on tcgen05 with exact integer slices, 0 fp32 FFMA kernel (other values: bit mask over
+ *                     the forward GEMM types, a measurement aid)
  *   "gemm_bwd_exact"  0 adjoint GEMMs 3xTF32, 1 exact integer slices
  *   "gemm_fwd_tc"     1 forward GEMMs 3xTF32 (biased energy, B3)
+ *   "phase_comp"      1 (default) forward edge kernels take the radial phase d / rc as an fp32 pair from the fp64 build
  *   "cell_strip"      order of the cells (hence of the sorted atoms): y cut into strips of this many cells, inside a strip
  *                     (z, y, x); default 6, 0 = plain (z, y, x).  Keeps three z planes of gathered rows inside L2
  *   "atoms_per_unit"  1..31 consecutive cell-sorted atoms per work unit of the tensor-core edge kernels (default 12 forward,
  *                     16 adjoint; setting it sets both, 0 restores the defaults)
- *   "gemm_emulate", "filter_emulate", "gather_emulate", "gemm_path"  operand-precision emulation (measurements of section 5)
  * Unknown names return MLP_ERR_ARG. */
 int mlp_set_option(mlp_model* m, const char* name, long long value);
 
