@@ -133,7 +133,7 @@ def test_config5_full_size_sampled_against_oracle():
 # ------------------------------------------------------------------------------------------------------------------
 # configs 2, 3, 4 at full size (BASELINE.json `configs`; boxes of configs 2 / 3 as corrected in DESIGN.md section 4)
 
-def _gpu_run(c, blob, owner=False, want_state=True):
+def _gpu_run(c, blob, owner=False, want_state=True, opts=None):
     import torch
     import paper_2506_04055_b200 as P
     dev = torch.device("cuda:0")
@@ -143,6 +143,8 @@ def _gpu_run(c, blob, owner=False, want_state=True):
     if owner and c["ghost_owner"] is not None:
         go = torch.from_numpy(np.ascontiguousarray(c["ghost_owner"], np.int32)).to(dev)
     with P.Model(blob, mdl["n_species"], mdl["rc"], N) as m:
+        for name, v in (opts or {}).items():
+            m.set_option(name, v)
         e, f, w = m.compute(torch.from_numpy(c["pos"]).to(dev), torch.from_numpy(c["types"]).to(dev), c["box"],
                             c["n_local"], c["n_ghost"], go)
         torch.cuda.synchronize()
@@ -226,6 +228,14 @@ def test_config3_full_size_slab_with_ghosts():
     _check_sampled(c, blob, fp, state, samples, frms, minimum_image=False)
     # whole system: energy, virial, partial forces on a stratified sample (bulk / surface / next to the halo / ghosts)
     _check_against_golden(3, c, e, fp, w, "config 3 full size (partial forces on all rows)")
+    # T-hop pruning (the default above) does not change the result, only the cost: the same system with every
+    # given atom carried through all layers
+    e3, f3, w3, st3, _ = _gpu_run(c, blob, owner=False, want_state=False, opts=dict(prune=0))
+    assert st3["n_reached"] == N and st["n_reached"] < N and st3["n_edges"] >= st["n_edges"]
+    print(f"config 3 full size: pruning keeps {st['n_reached']} of {N} atoms ({nl} local; ghost overhead {N / nl:.3f} -> "
+          f"{st['n_reached'] / nl:.3f}), {st['n_edges']} of {st3['n_edges']} edges")
+    _check_against_golden(3, c, e3, f3, w3, "config 3 full size, un-pruned")
+    assert abs(e3 - e) <= 1e-4 * nl and np.abs(f3 - fp).max() <= 1e-2 * frms
 
 
 def test_config4_full_size_crystal():
