@@ -84,6 +84,7 @@ struct mlp_model {
     void* h_misc = nullptr;   // pinned mirror
     // host staging for mlp_compute_host
     Buf d_pos, d_types, d_owner, d_out;   // d_out: energy[1] virial[6] forces[3N]
+    Buf b_gout, b_gowner;                 // outputs / owner map of the captured step (same layout as d_out)
     cudaStream_t own_stream = nullptr;
     cudaStream_t side_stream = nullptr;            // reverse-edge index is built beside the forward pass
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_gin = nullptr, ev_gout = nullptr;
@@ -105,14 +106,8 @@ struct mlp_model {
     cudaStream_t stats_stream = nullptr;
     // captured reuse step
     cudaGraphExec_t graph_exec = nullptr;
-    struct GraphKey {
-        const void *pos = nullptr, *types = nullptr, *owner = nullptr, *energy = nullptr, *forces = nullptr, *virial = nullptr;
-        cudaStream_t st = nullptr;
-        bool operator==(const GraphKey& o) const {
-            return pos == o.pos && types == o.types && owner == o.owner && energy == o.energy && forces == o.forces &&
-                   virial == o.virial && st == o.st;
-        }
-    } graph_key;
+    bool graph_has_owner = false;         // what the captured step was built for
+    void *graph_out = nullptr, *graph_owner = nullptr;
     long long graph_launches = 0;         // kernels inside the captured step
     mlp_stats stats{};
     std::string err;
@@ -876,7 +871,7 @@ __attribute__((visibility("default"))) void mlp_destroy(mlp_model* m) {
                  &m->b_lvl_hist, &m->b_pos_ref, &m->b_wrap_ref, &m->b_sup_ptr, &m->b_h, &m->b_rpre,
                  &m->b_rb, &m->b_eatom, &m->b_sb, &m->b_s1b, &m->b_vb, &m->b_v1b, &m->b_ab, &m->b_pqb, &m->b_gb,
                  &m->b_snb, &m->b_phib, &m->b_hb, &m->b_Q4, &m->b_Q1, &m->b_epart, &m->b_wpart, &m->b_red, &m->b_misc, &m->d_pos, &m->d_types,
-                 &m->d_owner, &m->d_out};
+                 &m->d_owner, &m->d_out, &m->b_gout, &m->b_gowner};
     for (Buf* b : bs) free_buf(*b, nullptr);
     for (int t = 0; t <= PAINN_MAX_T; t++) { free_buf(m->b_S[t], nullptr); free_buf(m->b_V[t], nullptr); }
     for (int t = 0; t < PAINN_MAX_T; t++) {
@@ -1021,25 +1016,37 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
     if (reuse) {
         ls.n_reuse++;
         int r = MLP_OK;
-        mlp_model::GraphKey key{pos, types, ghost_owner, energy, forces, virial, nullptr};
         const bool want_graph = m->use_graph && !m->timing;
         // The captured step lives on the model's own stream (the caller's may be the legacy default stream, which cannot be
-        // captured) and is ordered after / before the caller's stream with two events.
+        // captured), ordered after / before the caller's stream with two events, and touches NO caller buffer: it reads the
+        // model's copy of the owner map and writes E, W, F into the model's staging buffer, both copied outside the graph.
+        // So one capture serves every later reuse step, whatever buffers the caller passes.
         cudaStream_t gs = m->own_stream;
-        if (want_graph && !(m->graph_exec && m->graph_key == key)) {
-            // capture this step once; later steps with the same buffers replay it (no launch overhead, no host read)
+        const bool has_owner = ghost_owner != nullptr && n_ghost > 0;
+        double* gout = nullptr;
+        int* gowner = nullptr;
+        if (want_graph) {
+            ENS(m, m->b_gout, (size_t)(7 + 3 * N) * 8);
+            if (has_owner) ENS(m, m->b_gowner, (size_t)n_ghost * 4);
+            gout = P<double>(m->b_gout);
+            gowner = has_owner ? P<int>(m->b_gowner) : nullptr;
+        }
+        if (want_graph && !(m->graph_exec && m->graph_has_owner == has_owner && m->graph_out == (void*)gout && m->graph_owner == (void*)gowner)) {
+            // capture this step once; later steps replay it (no launch overhead, no host read)
             drop_graph(m);
             cudaGraph_t graph = nullptr;
             const long long l0 = launches;
             if (cudaStreamBeginCapture(gs, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
                 Launch Lg = L;
                 Lg.stream = gs;
-                StepCtx cgx{m, Lg, gs, pos, types, box, n_local, n_ghost, ghost_owner, energy, forces, virial, N, periodic};
+                StepCtx cgx{m, Lg, gs, pos, types, box, n_local, n_ghost, gowner, gout, gout + 7, gout + 1, N, periodic};
                 r = step_from_list(cgx);
                 cudaError_t ce = cudaStreamEndCapture(gs, &graph);
                 if (r == MLP_OK && ce == cudaSuccess && graph &&
                     cudaGraphInstantiate(&m->graph_exec, graph, nullptr, nullptr, 0) == cudaSuccess) {
-                    m->graph_key = key;
+                    m->graph_has_owner = has_owner;
+                    m->graph_out = gout;
+                    m->graph_owner = gowner;
                     m->graph_launches = launches - l0;
                 } else
                     m->graph_exec = nullptr;
@@ -1055,7 +1062,11 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
         if (want_graph && m->graph_exec) {
             CU(m, cudaEventRecord(m->ev_gin, st));
             CU(m, cudaStreamWaitEvent(gs, m->ev_gin, 0));
+            if (has_owner) CU(m, cudaMemcpyAsync(gowner, ghost_owner, (size_t)n_ghost * 4, cudaMemcpyDeviceToDevice, gs));
             CU(m, cudaGraphLaunch(m->graph_exec, gs));
+            CU(m, cudaMemcpyAsync(energy, gout, 8, cudaMemcpyDeviceToDevice, gs));
+            CU(m, cudaMemcpyAsync(virial, gout + 1, 48, cudaMemcpyDeviceToDevice, gs));
+            if (N > 0) CU(m, cudaMemcpyAsync(forces, gout + 7, (size_t)N * 24, cudaMemcpyDeviceToDevice, gs));
             CU(m, cudaEventRecord(m->ev_gout, gs));
             CU(m, cudaStreamWaitEvent(st, m->ev_gout, 0));
             launches += m->graph_launches;
