@@ -177,6 +177,15 @@ int mlp_get_stage_ms(mlp_model* m, int max_stages, const char** names, float* ms
  * Unknown names return MLP_ERR_ARG. */
 int mlp_set_option(mlp_model* m, const char* name, long long value);
 
+/*
+ * mlp_measure_row_gather -- measurement utility ("L2 -> SM bandwidth is not in PEAKS: measure it
+ * first with a gather micro-benchmark, because it bounds the edge stages").  Runs the access pattern of the edge kernels --
+ * a warp reads one 512-byte row per request, rows chosen inside `window` neighbouring rows of a table of `table_bytes`
+ * (>= 1 MiB), 16 rows in flight per thread, 16 / 32 / 64 warps per SM -- on the current device and returns the best
+ * sustained rate in GB/s in *gb_per_s (HOST).  Allocates and frees its own buffers; synchronous.
+ */
+int mlp_measure_row_gather(long long table_bytes, int window, double* gb_per_s);
+
 /* mlp_last_error -- text of the last error on this model (static string when m == NULL). */
 const char* mlp_last_error(mlp_model* m);
 

@@ -12,6 +12,7 @@ _LIB_NAME = "libpainn_b200.so"
 EXPORTED_SYMBOLS = [
     "mlp_create", "mlp_compute", "mlp_compute_host", "mlp_destroy", "mlp_get_neighbors", "mlp_get_layer_state",
     "mlp_get_stats", "mlp_get_stage_ms", "mlp_set_option", "mlp_last_error", "mlp_version", "mlp_debug_gemm",
+    "mlp_measure_row_gather",
 ]
 
 ERR_NAMES = {0: "MLP_OK", 1: "MLP_ERR_ARG", 2: "MLP_ERR_WEIGHTS", 3: "MLP_ERR_BOX_TOO_SMALL", 4: "MLP_ERR_TYPE_RANGE",
@@ -65,6 +66,8 @@ def load_library(build_if_missing: bool = True):
     lib.mlp_set_option.argtypes = [vp, C.c_char_p, ll]
     lib.mlp_debug_gemm.argtypes = [vp, vp, vp, vp, ll, i32, i32, i32, i32, C.POINTER(i32)]
     lib.mlp_debug_gemm.restype = i32
+    lib.mlp_measure_row_gather.argtypes = [ll, i32, C.POINTER(dbl)]
+    lib.mlp_measure_row_gather.restype = i32
     lib.mlp_last_error.argtypes = [vp]
     lib.mlp_last_error.restype = C.c_char_p
     lib.mlp_version.restype = C.c_char_p
@@ -77,6 +80,16 @@ def load_library(build_if_missing: bool = True):
 
 def version() -> str:
     return load_library().mlp_version().decode()
+
+
+def measure_row_gather(table_bytes: int = 2 << 30, window: int = 400) -> float:
+    """GB/s the device sustains for the 512-byte row gather of the edge kernels (mlp_measure_row_gather)."""
+    lib = load_library()
+    out = C.c_double(0.0)
+    rc = lib.mlp_measure_row_gather(int(table_bytes), int(window), C.byref(out))
+    if rc != 0:
+        raise MLPError(rc, "mlp_measure_row_gather")
+    return out.value
 
 
 def debug_gemm(A, W, bias=None, C_out=None, accumulate=False, path=0):
