@@ -216,3 +216,55 @@ def test_two_models_two_threads_different_options():
     for k in range(2):
         _check(c, *out[k], ref, f"thread {k} options {opts[k]}")
     assert out[0][0] != out[1][0]                    # different kernels did run (plain fp32 edge path vs tensor-core path)
+
+
+def test_list_is_rebuilt_when_the_system_changes():
+    """The kept list serves a call only for the same atom counts, species and box, and only while no atom has moved further
+    than skin / 2: each of these changes must rebuild (and give the oracle's result)."""
+    import paper_2506_04055_b200 as P
+    c = gen.make_config(1)
+    blob = _blob(c["model"])
+    mdl = c["model"]
+    N = len(c["pos"])
+    with P.Model(blob, mdl["n_species"], mdl["rc"], N) as m:
+        m.set_option("skin_mA", 1500)
+        _run(m, c["pos"], c["types"], c["box"])
+        _run(m, c["pos"], c["types"], c["box"])
+        assert (m.stats()["n_list_rebuilds"], m.stats()["n_list_reuses"]) == (1, 1)
+        # (i) one atom jumps by 1 A > skin / 2
+        pos = c["pos"].copy(); pos[17, 1] += 1.0
+        e, f, w = _run(m, pos, c["types"], c["box"])
+        assert m.stats()["n_list_rebuilds"] == 2
+        _check(c, e, f, w, oracle.compute(blob, pos, c["types"], c["box"]), "jump > skin / 2")
+        # (ii) a species changes
+        types = c["types"].copy(); types[5] = 1 - types[5]
+        e, f, w = _run(m, pos, types, c["box"])
+        assert m.stats()["n_list_rebuilds"] == 3
+        _check(c, e, f, w, oracle.compute(blob, pos, types, c["box"]), "species change")
+        # (iii) the box changes (positions scaled with it)
+        box2 = np.asarray(c["box"]) * 1.01
+        e, f, w = _run(m, pos * 1.01, types, box2)
+        assert m.stats()["n_list_rebuilds"] == 4
+        _check(c, e, f, w, oracle.compute(blob, pos * 1.01, types, box2), "box change")
+        # (iv) fewer atoms
+        e, f, w = _run(m, pos[:150] * 1.01, types[:150], box2)
+        assert m.stats()["n_list_rebuilds"] == 5 and f.shape == (150, 3)
+        cc = dict(c); cc["n_local"] = 150
+        _check(cc, e, f, w, oracle.compute(blob, pos[:150] * 1.01, types[:150], box2), "fewer atoms")
+        # ... and then it is reused again
+        _run(m, pos[:150] * 1.01, types[:150], box2)
+        assert m.stats()["n_list_reuses"] == 2
+
+
+def test_host_entry_point_with_list_reuse():
+    import paper_2506_04055_b200 as P
+    c = gen.make_config(2, **SMALL[2])
+    blob = _blob(c["model"])
+    mdl = c["model"]
+    with P.Model(blob, mdl["n_species"], mdl["rc"], len(c["pos"])) as m:
+        out = [m.compute_host(c["pos"], c["types"], c["box"]) for _ in range(3)]
+        out = [(float(e[0]), f.copy(), w.copy()) for e, f, w in out]
+        st = m.stats()
+    assert st["n_list_rebuilds"] == 1 and st["n_list_reuses"] == 2 and st["n_graph_replays"] == 2
+    assert out[1][0] == out[0][0] == out[2][0] and np.abs(out[2][1] - out[0][1]).max() <= 1e-9 * np.abs(out[0][1]).max()
+    _check(c, *out[2], _oracle_eval(c, blob), "host entry point, third call (graph replay)")
