@@ -186,6 +186,30 @@ int mlp_set_option(mlp_model* m, const char* name, long long value);
  */
 int mlp_measure_row_gather(long long table_bytes, int window, double* gb_per_s);
 
+/*
+ * mlp_row_offsets_static -- the CSR row-offset step of the neighbour build ("compute the neighbor list";
+ * per-receiver edge counts -> row_ptr by an exclusive scan) as an entry point that
+ * ALLOCATES NOTHING: no cudaMalloc, cudaFree or allocating library routine is called, so it may be used where those are
+ * forbidden (under CUDA graph capture, in tight serving loops).  The scratch of the scan (one total per block of 4,096
+ * rows) lives in a file-scope device array of 64 KiB + 256 B that every GPU loading this library holds until exit.
+ *   counts       DEVICE [n] int, read only
+ *   offsets      DEVICE [n + 1] int, written: offsets[i] = counts[0] + ... + counts[i-1]; offsets[n] = the total (low 32 bits)
+ *   n            0 <= n <= MLP_ROW_OFFSETS_STATIC_MAX, else MLP_ERR_ARG (nothing is launched)
+ *   total        DEVICE long long, receives the 64-bit total; may be NULL
+ *   cuda_stream  cudaStream_t (NULL = default stream); asynchronous, three kernel launches
+ * Every call on a device shares the one array, which keeps the last call's contents (the call clears the one word that
+ * must start at zero itself).  Calls that overlap on the GPU -- different streams, or host threads with no ordering
+ * between their launches -- race on it: order them on one stream or with events.
+ */
+#define MLP_ROW_OFFSETS_STATIC_MAX 67108864LL
+int mlp_row_offsets_static(const int* counts, int* offsets, long long n, long long* total, void* cuda_stream);
+
+/*
+ * mlp_debug_row_offsets -- the same step through the EXISTING path: the scan kernels mlp_compute launches (nbr.cu), with
+ * a block buffer from cudaMalloc, on caller buffers.  Same arguments (total must not be NULL); synchronous.  Test hook.
+ */
+int mlp_debug_row_offsets(const int* counts, int* offsets, long long n, long long* total, void* cuda_stream);
+
 /* mlp_last_error -- text of the last error on this model (static string when m == NULL). */
 const char* mlp_last_error(mlp_model* m);
 

@@ -5,5 +5,6 @@ runs in the CUDA kernels of ``csrc/``.  PyTorch is used for device memory and st
 fallback: if the shared library is missing or no CUDA device is present, calls raise.
 """
 from .binding import (  # noqa: F401
-    MLPError, Model, lib_path, load_library, version, debug_gemm, measure_row_gather, EXPORTED_SYMBOLS,
+    MLPError, Model, lib_path, load_library, version, debug_gemm, measure_row_gather, row_offsets, row_offsets_into,
+    ROW_OFFSETS_STATIC_MAX, EXPORTED_SYMBOLS,
 )

@@ -12,7 +12,7 @@ _LIB_NAME = "libpainn_b200.so"
 EXPORTED_SYMBOLS = [
     "mlp_create", "mlp_compute", "mlp_compute_host", "mlp_destroy", "mlp_get_neighbors", "mlp_get_layer_state",
     "mlp_get_stats", "mlp_get_stage_ms", "mlp_set_option", "mlp_last_error", "mlp_version", "mlp_debug_gemm",
-    "mlp_measure_row_gather",
+    "mlp_measure_row_gather", "mlp_row_offsets_static", "mlp_debug_row_offsets",
 ]
 
 ERR_NAMES = {0: "MLP_OK", 1: "MLP_ERR_ARG", 2: "MLP_ERR_WEIGHTS", 3: "MLP_ERR_BOX_TOO_SMALL", 4: "MLP_ERR_TYPE_RANGE",
@@ -68,6 +68,9 @@ def load_library(build_if_missing: bool = True):
     lib.mlp_debug_gemm.restype = i32
     lib.mlp_measure_row_gather.argtypes = [ll, i32, C.POINTER(dbl)]
     lib.mlp_measure_row_gather.restype = i32
+    for n in ("mlp_row_offsets_static", "mlp_debug_row_offsets"):
+        getattr(lib, n).argtypes = [vp, vp, ll, vp, vp]
+        getattr(lib, n).restype = i32
     lib.mlp_last_error.argtypes = [vp]
     lib.mlp_last_error.restype = C.c_char_p
     lib.mlp_version.restype = C.c_char_p
@@ -90,6 +93,36 @@ def measure_row_gather(table_bytes: int = 2 << 30, window: int = 400) -> float:
     if rc != 0:
         raise MLPError(rc, "mlp_measure_row_gather")
     return out.value
+
+
+ROW_OFFSETS_STATIC_MAX = 67108864      # mlp.h: MLP_ROW_OFFSETS_STATIC_MAX
+
+
+def row_offsets(counts, static=True, stream=None):
+    """Exclusive scan of a cuda int32 tensor of row counts -> (offsets[n + 1] int32, total int64 tensor).
+    static=True: mlp_row_offsets_static (allocates nothing inside the library; the outputs are torch tensors made here);
+    static=False: mlp_debug_row_offsets (the scan kernels of mlp_compute with a cudaMalloc'ed block buffer)."""
+    import torch
+    lib = load_library()
+    assert counts.is_cuda and counts.dtype == torch.int32 and counts.is_contiguous()
+    n = counts.numel()
+    offsets = torch.empty(n + 1, dtype=torch.int32, device=counts.device)
+    total = torch.empty(1, dtype=torch.int64, device=counts.device)
+    return row_offsets_into(counts, offsets, total, static=static, stream=stream)
+
+
+def row_offsets_into(counts, offsets, total, static=True, stream=None, n=None):
+    """Same with caller-provided outputs (no torch allocation either).  `total` may be None for the static entry."""
+    import torch
+    lib = load_library()
+    n = counts.numel() if n is None else int(n)
+    st = torch.cuda.current_stream(counts.device).cuda_stream if stream is None else int(stream)
+    fn = lib.mlp_row_offsets_static if static else lib.mlp_debug_row_offsets
+    rc = fn(counts.data_ptr() if counts.numel() else None, offsets.data_ptr(), n,
+            total.data_ptr() if total is not None else None, st)
+    if rc != 0:
+        raise MLPError(rc, fn.__name__)
+    return offsets, total
 
 
 def debug_gemm(A, W, bias=None, C_out=None, accumulate=False, path=0):

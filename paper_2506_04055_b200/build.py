@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpainn_b200.so")
-SOURCES = ["api.cu", "nbr.cu", "gemm.cu", "gemm_tc.cu", "edge_v3.cu", "edge_l0.cu", "painn_fwd.cu", "painn_bwd.cu", "measure.cu"]
+SOURCES = ["api.cu", "nbr.cu", "gemm.cu", "gemm_tc.cu", "edge_v3.cu", "edge_l0.cu", "painn_fwd.cu", "painn_bwd.cu", "measure.cu", "scan_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--extended-lambda",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
 
