@@ -23,7 +23,8 @@
 //     (adjoint); the pipeline runs across tile and unit boundaries;
 //   * rows are padded to 8 slots with zero-weight dummies, so nothing is predicated per edge: one uniform
 //     row-boundary test per 8 edges; the receiver's own rows (residual / phi_j, v_j) are loaded one row ahead;
-//   * the adjoint reduces its per-edge sums over the 128 channels through shared-memory planes and a reducer warp;
+//   * the adjoint reduces its per-edge sums over the 128 channels through shared-memory planes and a reducer warp
+//     (four planes per edge: db and the vector beta' vb'; u, 1/d and the projection are applied once per edge);
 //   * one 512-thread CTA per SM = two independent 8-warp pipelines sharing one copy of the filter operand.
 #include <cuda_fp16.h>
 
@@ -161,7 +162,17 @@ constexpr int GW = 16;                                  // gather window (edges 
 constexpr int RING_BYTES = GW * F * 16;                 // 32768
 constexpr int G_OFF_B = 0, G_OFF_P = 2 * BB_BYTES, G_OFF_RING = G_OFF_P + 2 * P_BYTES, G_OFF_META = G_OFF_RING + RING_BYTES,
               G_OFF_BAR = G_OFF_META + 4 * NEB * 16, GROUP_BYTES = G_OFF_BAR + 128;
-constexpr int bwd_smem_bytes(int) { return 2 * GROUP_BYTES + 128; }
+// k_msg_bwd reduces FOUR planes per edge (db | beta' vb_x | beta' vb_y | beta' vb_z, see its consumer loop); the layer-0
+// species-table kernel k_msg_bwd0 keeps the three-plane layout above
+constexpr int P4_ROW = 4 * F * 4 + 64;
+constexpr int P4_BYTES = 8 * P4_ROW;
+// k_msg_bwd: gather window of 24 edges per thread = three 8-edge slot groups (A/B at config 5: 16 -> 24 edges 45.2 -> 44.2 ms
+// per step, 32 edges 44.9 ms)
+constexpr int GWH = 24, NSG = GWH / 8;
+constexpr int HRING_BYTES = GWH * F * 16;
+constexpr int H_OFF_B = 0, H_OFF_P = 2 * BB_BYTES, H_OFF_RING = H_OFF_P + 2 * P4_BYTES, H_OFF_META = H_OFF_RING + HRING_BYTES,
+              H_OFF_BAR = H_OFF_META + 4 * NEB * 16, HGROUP_BYTES = H_OFF_BAR + 128;
+constexpr int bwd_smem_bytes(int) { return 2 * HGROUP_BYTES + 128; }
 
 
 // two fp32 additions in one instruction (register pairs as they come out of a 16-byte shared-memory load): the reducer
@@ -533,18 +544,18 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
     constexpr int TCOLS = NCH * 2 * NEB;            // TMEM columns per accumulator buffer
     extern __shared__ __align__(128) uint8_t smem[];
     const int tid = threadIdx.x, grp = tid >> 8, ltid = tid & 255, lwarp = ltid >> 5, lane = tid & 31;
-    uint8_t* gbase = smem + grp * GROUP_BYTES;
-    uint8_t* sB = gbase + G_OFF_B;
-    uint8_t* sP = gbase + G_OFF_P;                 // [2][8] rows of P_ROW bytes: (db, ub_x, ub_y, ub_z) per channel
-    float4* sMeta = (float4*)(gbase + G_OFF_META); // [4][NEB] (u of edge (i <- j), 1/d): ring of 4 tiles
-    uint64_t* bars = (uint64_t*)(gbase + G_OFF_BAR);
+    uint8_t* gbase = smem + grp * HGROUP_BYTES;
+    uint8_t* sB = gbase + H_OFF_B;
+    uint8_t* sP = gbase + H_OFF_P;                 // [2][8] rows of P4_ROW bytes: four planes of 128 floats per edge
+    float4* sMeta = (float4*)(gbase + H_OFF_META); // [4][NEB] (u of edge (i <- j), 1/d): ring of 4 tiles
+    uint64_t* bars = (uint64_t*)(gbase + H_OFF_BAR);
     uint64_t* t_full = bars;          // [2] MMA commit -> consumers (mbarrier, count 1)
     uint64_t* p_empty = bars + 2;     // [2] reducer -> consumers: partials buffer read (mbarrier, count 1)
     // named barriers of this group (hardware-blocking waits): [2] each
-    const int NB_TE = 1 + grp * 6;    // consumers (128, arrive) -> producers (64, sync): tile buffer consumed
-    const int NB_BF = NB_TE + 2;      // producers (64, arrive) -> MMA warp (32, sync): B operand written
+    const int NB_TE = 1 + grp * 6;    // consumers (128, arrive) -> producer (32, sync): tile buffer consumed
+    const int NB_BF = NB_TE + 2;      // producer (32, arrive) -> MMA warp (32, sync): B operand written
     const int NB_PF = NB_TE + 4;      // consumers (128, arrive) -> reducer (32, sync): partials of one batch written
-    uint32_t* tmem_slot = (uint32_t*)(smem + 2 * GROUP_BYTES);
+    uint32_t* tmem_slot = (uint32_t*)(smem + 2 * HGROUP_BYTES);
 
     {
         uint4* zb = (uint4*)sB;
@@ -611,7 +622,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
         // cp.async copies into private 16-byte shared-memory slots (one commit group per edge, wait_group W-1 before
         // an edge is consumed).  ptxas tracks register-landing loads of different pipeline stages on one scoreboard
         // (measured: the "ping-pong" LDG banks serialised), cp.async groups complete in order by construction.
-        float4* ring = (float4*)(gbase + G_OFF_RING) + f;             // slot s of this thread: ring[s * F]
+        float4* ring = (float4*)(gbase + H_OFF_RING) + f;             // slot s of this thread: ring[s * F]
         const float4* __restrict__ ejp = p.ej;
         uint32_t it = 0, hc = 0;          // tile counter, active 8-edge batch counter (selects the partials buffer)
         for (long long u = u0; u < n_units; u += ustride) {
@@ -634,18 +645,20 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
             int idxn = 0;
             if (ntiles > 0) {
 #pragma unroll
-                for (int i = 0; i < GW; i++) {
+                for (int i = 0; i < GWH; i++) {
                     const int j = __shfl_sync(0xffffffffu, idx0, i);
                     if (i < n_e) cp_async16(ring + i * F, Gb + (size_t)j * F);
                     if ((i & 7) == 7) cp_async_commit();            // one commit group per 8-edge batch
                 }
             }
             int j_rel = 0;
+            int sg = 0;                       // ring slot group of the next batch (batch b of the unit lives in group b % NSG)
             int row_end = __shfl_sync(0xffffffffu, rp, 1);
             // own rows of sender j (current) and j + 1 (prefetched)
             float phS, phVS, phVV = 0.f, vj0 = 0.f, vj1 = 0.f, vj2 = 0.f, r0 = 0.f, r1 = 0.f, r2 = 0.f;
             float nphS = 0.f, nphVS = 0.f, nphVV = 0.f, nvj0 = 0.f, nvj1 = 0.f, nvj2 = 0.f, nr0 = 0.f, nr1 = 0.f, nr2 = 0.f;
             float pbS = 0.f, pbVS = 0.f, Y0 = 0.f, Y1 = 0.f, Y2 = 0.f;
+            float vp0 = 0.f, vp1 = 0.f, vp2 = 0.f;                     // phi^vv_j v_j: the vv share of db takes one dot product with it
             auto load_own = [&](long long j, float& a, float& b, float& c, float& x, float& y, float& z, float& q0, float& q1, float& q2) {
                 a = phi[j * 3 * F]; b = phi[j * 3 * F + F];
                 if (!L0) {
@@ -655,6 +668,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                 }
             };
             load_own(a0, phS, phVS, phVV, vj0, vj1, vj2, r0, r1, r2);
+            vp0 = phVV * vj0; vp1 = phVV * vj1; vp2 = phVV * vj2;
             if (na > 1) load_own(a0 + 1, nphS, nphVS, nphVV, nvj0, nvj1, nvj2, nr0, nr1, nr2);
             auto store_row = [&]() {
                 if (L0) return;
@@ -671,6 +685,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                 j_rel++;
                 row_end = __shfl_sync(0xffffffffu, rp, j_rel + 1);
                 phS = nphS; phVS = nphVS; phVV = nphVV; vj0 = nvj0; vj1 = nvj1; vj2 = nvj2; r0 = nr0; r1 = nr1; r2 = nr2;
+                vp0 = phVV * vj0; vp1 = phVV * vj1; vp2 = phVV * vj2;
                 pbS = pbVS = Y0 = Y1 = Y2 = 0.f;
                 if (j_rel + 1 < na) load_own(a0 + j_rel + 1, nphS, nphVS, nphVV, nvj0, nvj1, nvj2, nr0, nr1, nr2);
             };
@@ -681,13 +696,14 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
         if (E8_ < e_end) {                                                                                        \
             while (E8_ >= row_end) next_row();                                                                    \
             /* prefetch targets: edges k0 + 16 .. k0 + 23 of the unit, all in index block tb_ */                  \
-            const int tb_ = (k0_ + GW) >> 5, l0_ = (k0_ + GW) & 31;                                               \
+            const int tb_ = (k0_ + GWH) >> 5, l0_ = (k0_ + GWH) & 31;                                             \
             /* the next index block lands in its own register and is folded into idx0 / idx1 one batch later: */ \
             /* the select below then never reads a register with a load in flight                              */ \
             if (l0_ == 0) idxn = load_idx(tb_ + 1);                                                               \
             if (l0_ == 8) { if (tb_ & 1) idx0 = idxn ^ (idxn >> 31); else idx1 = idxn ^ (idxn >> 31); }           \
             const int isel_ = (tb_ & 1) ? idx1 : idx0;                                                            \
-            const bool pf_ = k0_ + GW < n_e;                                                                      \
+            const bool pf_ = k0_ + GWH < n_e;                                                                     \
+            float4* rslot_ = ring + sg * 8 * F;              /* slot group of this batch */                       \
             uint32_t wS_[8], wVS_[8], wVV_[8], dS_[8], dVS_[8], dVV_[8];                                          \
             tmem_ld8_nowait(lane_base + buf * TCOLS + (H) * 8, wS_);                                              \
             tmem_ld8_nowait(lane_base + buf * TCOLS + NEB + (H) * 8, dS_);                                        \
@@ -699,50 +715,53 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
             }                                                                                                     \
             mbar_wait(&p_empty[hc & 1], ((hc >> 1) & 1) ^ 1);           /* partials buffer free again */          \
             tmem_wait_ld();                                                                                       \
-            cp_async_wait<1>();              /* this batch's rows have landed; the next batch's stay in flight */ \
-            uint8_t* pdst_ = sP + (hc & 1) * P_BYTES;                                                             \
+            cp_async_wait<NSG - 1>();        /* this batch's rows have landed; the next batches' stay in flight */ \
+            uint8_t* pdst_ = sP + (hc & 1) * P4_BYTES;                                                             \
             /* the loads of edge i + BWD_PD are issued before the partials of edge i are stored: ptxas cannot */  \
             /* prove that the stores to sP do not alias the ring, and would otherwise expose the full LDS     */  \
             /* latency once per edge (measured: 25 % of the consumers' time)                                  */  \
             float4 mq_[8], gq_[8];                                                                                \
             _Pragma("unroll") for (int i_ = 0; i_ < BWD_PD; i_++) {                                               \
                 mq_[i_] = meta[(H) * 8 + i_];                                                                     \
-                gq_[i_] = ring[((H) * 8 + i_) * F];                                                               \
+                gq_[i_] = rslot_[i_ * F];                                                                         \
             }                                                                                                     \
             _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                                    \
                 if (i_ + BWD_PD < 8) {                                                                            \
                     mq_[i_ + BWD_PD] = meta[(H) * 8 + i_ + BWD_PD];                                               \
-                    gq_[i_ + BWD_PD] = ring[((H) * 8 + i_ + BWD_PD) * F];                                         \
+                    gq_[i_ + BWD_PD] = rslot_[(i_ + BWD_PD) * F];                                                 \
                 }                                                                                                 \
                 const float4 m_ = mq_[i_];                                                                        \
                 const float4 g_ = gq_[i_];                                                                        \
                 const float sb_ = g_.x, vb0_ = g_.y, vb1_ = g_.z, vb2_ = g_.w;                                    \
                 const float X_ = fmaf(vb0_, m_.x, fmaf(vb1_, m_.y, vb2_ * m_.z));                                 \
                 const float wVSf_ = __uint_as_float(wVS_[i_]);                                                    \
-                float db_ = phS * (sb_ * __uint_as_float(dS_[i_]));                                               \
-                db_ = fmaf(phVS, X_ * __uint_as_float(dVS_[i_]), db_);                                            \
+                float db_ = (phS * sb_) * __uint_as_float(dS_[i_]);                                               \
+                db_ = fmaf(phVS * X_, __uint_as_float(dVS_[i_]), db_);                                            \
                 if (!L0) {                                                                                        \
                     const float wVVf_ = __uint_as_float(wVV_[i_]);                                                \
-                    const float Z_ = fmaf(vb0_, vj0, fmaf(vb1_, vj1, vb2_ * vj2));                                \
-                    db_ = fmaf(phVV, Z_ * __uint_as_float(dVV_[i_]), db_);                                        \
+                    const float Z_ = fmaf(vb0_, vp0, fmaf(vb1_, vp1, vb2_ * vp2));      /* phi^vv (vb' . v_j) */  \
+                    db_ = fmaf(Z_, __uint_as_float(dVV_[i_]), db_);                                               \
                     pbS = fmaf(__uint_as_float(wS_[i_]), sb_, pbS);                                               \
                     pbVS = fmaf(wVSf_, X_, pbVS);                                                                 \
                     Y0 = fmaf(wVVf_, vb0_, Y0); Y1 = fmaf(wVVf_, vb1_, Y1); Y2 = fmaf(wVVf_, vb2_, Y2);           \
                 }                                                                                                 \
-                /* this channel's share of g_e = db u + (ub - (ub.u) u) / d, ub = tt vb':  alpha u + beta vb' */  \
-                const float beta_ = wVSf_ * phVS * m_.w;                                                          \
-                const float alpha_ = fmaf(-beta_, X_, db_);                                                       \
-                float* pd_ = (float*)(pdst_ + i_ * P_ROW) + f;          /* three planes of 128 floats per edge */ \
-                pd_[0] = fmaf(alpha_, m_.x, beta_ * vb0_);                                                        \
-                pd_[F] = fmaf(alpha_, m_.y, beta_ * vb1_);                                                        \
-                pd_[2 * F] = fmaf(alpha_, m_.z, beta_ * vb2_);                                                    \
+                /* this channel's share of g_e = db u + (ub - (ub.u) u) / d with ub = beta' vb', beta' = w^vs phi^vs: */ \
+                /* the planes (db, ub) are summed over the channels first; u, 1/d and the projection are applied   */ \
+                /* once per edge by the reducer (sum_c ub_c . u = u . sum_c ub_c)                                   */ \
+                const float bq_ = wVSf_ * phVS;                                                                   \
+                float* pd_ = (float*)(pdst_ + i_ * P4_ROW) + f;         /* four planes of 128 floats per edge */  \
+                pd_[0] = db_;                                                                                     \
+                pd_[F] = bq_ * vb0_;                                                                              \
+                pd_[2 * F] = bq_ * vb1_;                                                                          \
+                pd_[3 * F] = bq_ * vb2_;                                                                          \
             }                                                                                                     \
             /* re-arm the 8 slots with the rows of edges k0 + 16 .. k0 + 23 (one commit group, also when empty) */ \
             _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                                    \
                 const int jn_ = __shfl_sync(0xffffffffu, isel_, l0_ + i_);                                        \
-                if (pf_) cp_async16(ring + ((H) * 8 + i_) * F, Gb + (size_t)jn_ * F);                             \
+                if (pf_) cp_async16(rslot_ + i_ * F, Gb + (size_t)jn_ * F);                                       \
             }                                                                                                     \
             cp_async_commit();                                                                                    \
+            if (++sg == NSG) sg = 0;                                                                              \
             bar_arrive(NB_PF + (hc & 1), 160);                          /* hand the batch to the reducer warp */  \
             hc++;                                                                                                 \
         }                                                                                                         \
@@ -755,7 +774,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                 BWD_COMPUTE(0);
                 BWD_COMPUTE(1);
                 tc_fence_before();
-                bar_arrive(NB_TE + buf, 192);
+                bar_arrive(NB_TE + buf, 160);
             }
             cp_async_wait<0>();           // slots are re-armed by the next unit's prologue
             for (;;) {
@@ -769,69 +788,101 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
             }
         }
 #undef BWD_COMPUTE
-    } else if (lwarp < 6) {
-        // ===================== producers: rows 0..15 R_e, rows 16..31 R'_e =====================
-        // thread = (edge e, basis slots 8h .. 8h+7); the h == 3 quarter only takes part in the barriers
-        const int pt = ltid - 128, e = pt & 15, h = pt >> 4;
+    } else if (lwarp == 4 + grp) {
+        // ===================== producer: rows 0..15 R_e, rows 16..31 R'_e =====================
+        // (helper roles sit on different schedulers in the two pipelines: producer on 0 | 1, reducer on 2 | 3, MMA issuer on 3 | 2)
+        // ONE warp per pipeline: lane = (edge e of the tile, half hh): basis slots 12 hh .. 12 hh + 11 (slot 0 = bias).  The
+        // per-edge part (record, 1/d, sincospi, cutoff) is evaluated twice per edge instead of four times (round 1 / 2 used
+        // two warps with one 8-slot group per thread and an idle quarter), and R' comes from the closed form
+        //   R'_n = sin(n pi x) A + cos(n pi x) n B,   A = (fc' - fc / d) / d,   B = (pi / rc) fc / d,   R_n = sin(n pi x) fc / d
+        // (3 instructions per slot instead of 6): 330 instead of 740 warp instructions per 16-edge tile -- the producers were
+        // a sixth of all instructions this kernel issues (profiles/r02_edge_ncu.md).
+        const int e = lane & 15, hh = lane >> 4;
         const float inv_rc = p.inv_rc;
         const float a1c = 3.14159265358979323846f * inv_rc;
         const int K = p.K;
+        // the thread's 12 slots are three 8-byte pieces of a B row (4 fp16 each): piece j holds slots 12 hh + 4 j .. + 3,
+        // i.e. bytes ((12 hh + 4 j) & 7) * 2 .. of the 16-byte chunk (12 hh + 4 j) >> 3 of every product term
+        int poff[3];
+#pragma unroll
+        for (int j = 0; j < 3; j++) { const int sl = 12 * hh + 4 * j; poff[j] = (sl >> 3) * 128 + (sl & 7) * 2; }
         uint32_t it = 0;
         for (long long u = u0; u < n_units; u += ustride) {
             const long long a0 = u * apu;
             const long long a1 = min(N, a0 + (long long)apu);
             const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
             const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
-            float4 raw_n = load_edge_raw(p.ej, e_begin + e, h < 3 ? e_end : 0);
+            float4 raw_n = load_edge_raw(p.ej, e_begin + e, e_end);
             for (int t = 0; t < ntiles; t++, it++) {
                 const int buf = it & 1;
-                uint4 q[6];
-                float4 meta_v = make_float4(0.f, 0.f, 0.f, 0.f);
                 const float4 raw = raw_n;
-                if (t + 1 < ntiles) raw_n = load_edge_raw(p.ej, e_begin + (t + 1) * NEB + e, h < 3 ? e_end : 0);
-                if (h < 3) {
-                    const EdgeGeom g = edge_geom(raw, e_begin + t * NEB + e, e_end, inv_rc);
-                    const float fc = g.real ? 0.5f * (1.0f + g.c1) : 0.0f;
-                    const float dfc = g.real ? -0.5f * a1c * g.s1 : 0.0f;
-                    float sn_, cn_;
-                    if (h == 0) { sn_ = g.s1; cn_ = g.c1; } else sincospif((float)(8 * h) * g.x, &sn_, &cn_);
-                    float vals[8], dvals[8];
+                if (t + 1 < ntiles) raw_n = load_edge_raw(p.ej, e_begin + (t + 1) * NEB + e, e_end);
+                const EdgeGeom g = edge_geom(raw, e_begin + t * NEB + e, e_end, inv_rc);
+                const float fc = g.real ? 0.5f * (1.0f + g.c1) : 0.0f;
+                const float dfc = g.real ? -0.5f * a1c * g.s1 : 0.0f;
+                const float amp = fc * g.inv_d;                       // R_n = amp sin(n pi x)
+                const float cA = (dfc - amp) * g.inv_d, cB = a1c * amp;
+                float sn_, cn_;
+                sincospif(12.0f * g.x, &sn_, &cn_);                   // first slot of the upper half (the lower half starts at slot 1)
+                if (hh == 0) { sn_ = g.s1; cn_ = g.c1; }
+                float nB = hh == 0 ? cB : 12.0f * cB;                 // n B of the current slot
+                uint2 q[2][3][3];                                     // [R | R'][term][piece]
 #pragma unroll
-                    for (int i = 0; i < 8; i++) {
-                        const int b = h * 8 + i;
-                        if (b == 0) { vals[i] = fc; dvals[i] = dfc; }
-                        else {
-                            const float rho = sn_ * g.inv_d;
-                            const float drho = ((float)b * a1c * cn_ - rho) * g.inv_d;
-                            vals[i] = b <= K ? fc * rho : 0.0f;
-                            dvals[i] = b <= K ? dfc * rho + fc * drho : 0.0f;
-                            const float tt = sn_ * g.c1 + cn_ * g.s1;
-                            cn_ = cn_ * g.c1 - sn_ * g.s1;
-                            sn_ = tt;
+                for (int j = 0; j < 3; j++) {
+                    float vals[4], dvals[4];
+#pragma unroll
+                    for (int i = 0; i < 4; i++) {
+                        const int sl = 4 * j + i;                     // slot 12 hh + sl
+                        if (sl == 0) {                                // (hh == 0: the bias slot; hh == 1: slot 12, an ordinary one)
+                            const bool ok = 12 <= K;
+                            vals[i] = hh == 0 ? fc : (ok ? amp * sn_ : 0.0f);
+                            dvals[i] = hh == 0 ? dfc : (ok ? fmaf(sn_, cA, cn_ * nB) : 0.0f);
+                            if (hh == 0) continue;                    // (uniform per half-warp; the rotation below is skipped for the bias)
+                        } else {
+                            const bool ok = 12 * hh + sl <= K;
+                            vals[i] = ok ? amp * sn_ : 0.0f;
+                            dvals[i] = ok ? fmaf(sn_, cA, cn_ * nB) : 0.0f;
                         }
+                        const float tt = sn_ * g.c1 + cn_ * g.s1;
+                        cn_ = cn_ * g.c1 - sn_ * g.s1;
+                        sn_ = tt;
+                        nB += cB;
                     }
-                    split3b(vals, q[0], q[1], q[2]);
-                    split3b(dvals, q[3], q[4], q[5]);
-                    meta_v = make_float4(-g.r.x * g.inv_d, -g.r.y * g.inv_d, -g.r.z * g.inv_d, g.inv_d);   // u_e of edge (i <- j), 1/d
-                }
-                __syncwarp();
-                if (it >= 2) bar_sync(NB_TE + buf, 192);          // tile it - 2 consumed: B operand / TMEM buffer free
-                if (h < 3) {
 #pragma unroll
                     for (int z = 0; z < 2; z++) {
-                        const int row = z * NEB + e;
-                        uint8_t* bb = sB + buf * BB_BYTES + (row >> 3) * SBO + (row & 7) * 16;
+                        const float* v = z ? dvals : vals;
+                        const __half2 k64 = __floats2half2_rn(1.0f / 64.0f, 1.0f / 64.0f);
+                        __half2 h_hh[2], h_hl[2], h_lh[2];
 #pragma unroll
-                        for (int tm = 0; tm < 3; tm++) *(uint4*)(bb + kgrp_off(tm, h)) = q[3 * z + tm];
+                        for (int w = 0; w < 2; w++) {                 // split3b on two values at a time
+                            h_hh[w] = __floats2half2_rn(v[2 * w], v[2 * w + 1]);
+                            const float2 f = __half22float2(h_hh[w]);
+                            h_hl[w] = __floats2half2_rn((v[2 * w] - f.x) * 64.0f, (v[2 * w + 1] - f.y) * 64.0f);
+                            h_lh[w] = __hmul2(h_hh[w], k64);
+                        }
+                        q[z][0][j] = make_uint2(*(uint32_t*)&h_hl[0], *(uint32_t*)&h_hl[1]);     // term 0: r 2^6
+                        q[z][1][j] = make_uint2(*(uint32_t*)&h_lh[0], *(uint32_t*)&h_lh[1]);     // term 1: hi 2^-6
+                        q[z][2][j] = make_uint2(*(uint32_t*)&h_hh[0], *(uint32_t*)&h_hh[1]);     // term 2: hi
                     }
-                    if (h == 0) sMeta[(it & 3) * NEB + e] = meta_v;
                 }
+                __syncwarp();
+                if (it >= 2) bar_sync(NB_TE + buf, 160);          // tile it - 2 consumed: B operand / TMEM buffer free
+#pragma unroll
+                for (int z = 0; z < 2; z++) {
+                    const int row = z * NEB + e;
+                    uint8_t* bb = sB + buf * BB_BYTES + (row >> 3) * SBO + (row & 7) * 16;
+#pragma unroll
+                    for (int tm = 0; tm < 3; tm++)
+#pragma unroll
+                        for (int j = 0; j < 3; j++) *(uint2*)(bb + tm * 3 * 128 + poff[j]) = q[z][tm][j];
+                }
+                if (hh == 0) sMeta[(it & 3) * NEB + e] = make_float4(-g.r.x * g.inv_d, -g.r.y * g.inv_d, -g.r.z * g.inv_d, g.inv_d);   // u_e of edge (i <- j), 1/d
                 fence_async_smem();
                 __syncwarp();
-                bar_arrive(NB_BF + buf, 96);
+                bar_arrive(NB_BF + buf, 64);
             }
         }
-    } else if (lwarp == 6) {
+    } else if (lwarp == 6 + grp) {
         // ===================== reducer: sum the partials over the 128 channels, assemble g_e, accumulate G =====================
         // lane = (edge of the batch, quarter of the channels): 32 conflict-free LDS.128 + two shuffle stages per batch
         const int re = lane >> 2, rsub = lane & 3;
@@ -852,33 +903,42 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
                     float4 gold = make_float4(0.f, 0.f, 0.f, 0.f);
                     if (rsub == 0 && !first) gold = Gout[E];                  // running sum over layers, fetched early
                     bar_sync(NB_PF + (hc & 1), 160);
-                    // this lane adds a quarter (chunks rsub + 4 k) of each of the three 128-float planes of row re
-                    const uint8_t* src = sP + (hc & 1) * P_BYTES + re * P_ROW + rsub * 16;
-                    unsigned long long ax = 0ull, ay = 0ull, az = 0ull;      // packed (+0.f, +0.f)
+                    // this lane adds a quarter (chunks rsub + 4 k) of each of the four 128-float planes of row re
+                    const uint8_t* src = sP + (hc & 1) * P4_BYTES + re * P4_ROW + rsub * 16;
+                    const float4 mt = sMeta[(it & 3) * NEB + h * 8 + re];      // (u_e, 1 / d_e)
+                    unsigned long long ad = 0ull, ax = 0ull, ay = 0ull, az = 0ull;      // packed (+0.f, +0.f)
 #pragma unroll
                     for (int k = 0; k < 8; k++) {
-                        const ulonglong2 x = *(const ulonglong2*)(src + k * 64);
-                        const ulonglong2 y = *(const ulonglong2*)(src + F * 4 + k * 64);
-                        const ulonglong2 z = *(const ulonglong2*)(src + 2 * F * 4 + k * 64);
+                        const ulonglong2 d = *(const ulonglong2*)(src + k * 64);
+                        const ulonglong2 x = *(const ulonglong2*)(src + F * 4 + k * 64);
+                        const ulonglong2 y = *(const ulonglong2*)(src + 2 * F * 4 + k * 64);
+                        const ulonglong2 z = *(const ulonglong2*)(src + 3 * F * 4 + k * 64);
+                        ad = fadd2(ad, fadd2(d.x, d.y));
                         ax = fadd2(ax, fadd2(x.x, x.y));
                         ay = fadd2(ay, fadd2(y.x, y.y));
                         az = fadd2(az, fadd2(z.x, z.y));
                     }
-                    float3 acc = make_float3(hsum2(ax), hsum2(ay), hsum2(az));
+                    float db = hsum2(ad);
+                    float3 ub = make_float3(hsum2(ax), hsum2(ay), hsum2(az));
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&p_empty[hc & 1]);
                     hc++;
 #pragma unroll
                     for (int o = 2; o >= 1; o >>= 1) {
-                        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o);
-                        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
-                        acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o);
+                        db += __shfl_xor_sync(0xffffffffu, db, o);
+                        ub.x += __shfl_xor_sync(0xffffffffu, ub.x, o);
+                        ub.y += __shfl_xor_sync(0xffffffffu, ub.y, o);
+                        ub.z += __shfl_xor_sync(0xffffffffu, ub.z, o);
                     }
+                    // g_e = db u + (ub - (ub . u) u) / d
+                    ub.x *= mt.w; ub.y *= mt.w; ub.z *= mt.w;
+                    const float al = db - (ub.x * mt.x + ub.y * mt.y + ub.z * mt.z);
+                    const float3 acc = make_float3(fmaf(al, mt.x, ub.x), fmaf(al, mt.y, ub.y), fmaf(al, mt.z, ub.z));
                     if (rsub == 0) Gout[E] = make_float4(gold.x + acc.x, gold.y + acc.y, gold.z + acc.z, 0.f);
                 }
             }
         }
-    } else if (lwarp == 7) {
+    } else if (lwarp == 7 - grp) {
         // ===================== MMA issuer (lane 0; the whole warp waits on the producers' named barrier) =====================
         const uint32_t idesc = (1u << 4) | ((uint32_t)((2 * NEB) >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
         const uint32_t b_base = smem_u32(sB);
@@ -890,7 +950,7 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
             const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
             for (int t = 0; t < ntiles; t++, it++) {
                 const int buf = it & 1;
-                bar_sync(NB_BF + buf, 96);
+                bar_sync(NB_BF + buf, 64);
                 tc_fence_after();
                 if (elect_one()) {
 #pragma unroll
