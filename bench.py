@@ -345,6 +345,18 @@ def main():
         except Exception as ex:      # noqa: BLE001
             g_peak, g_src = 16200.0, f"round-1 figure of another pod (profiles/r01_microbench.md); live measurement failed: {ex!r}"
         roofline["l2_gather"] = dict(achieved=gb, peak=g_peak, unit="GB/s", frac=gb / g_peak, peak_source=g_src)
+    if split:
+        # third view of the edge stages (SURVEY.md 8(d) "edge products + segment sums: plain ALUs"): fp32 instructions the
+        # consumers execute per edge and channel (forward 9: 8 FFMA + 1 FMUL; adjoint 21) against the
+        # plain-ALU peak = SMs x 128 lanes x max SM clock (B200_PROFILING.md nominal table; one instruction = one lane-op)
+        alu_peak = 148 * 128 * peaks["sm_max"] * 1e6 / 1e12
+        roofline["alu"] = {}
+        for name, per in (("fwd_edge", 9.0), ("bwd_edge", 21.0)):
+            if acc.get(name, 0.0) > 0.0:
+                ops = stats["n_edges"] * model["F"] * per * (T - 1)
+                ach = ops / (acc[name] * 1e-3) / 1e12
+                roofline["alu"][name] = dict(achieved=ach, peak=alu_peak, unit="T-op/s (fp32 FMA/MUL lane-ops)", frac=ach / alu_peak,
+                                             ops_per_edge_channel=per)
 
     # ---- end to end through the host-buffer entry point (pinned host memory, copies inside the timed region) ----
     hpos = torch.from_numpy(c["pos"]).pin_memory()
