@@ -396,6 +396,40 @@ def main():
         torch.cuda.synchronize(dev)
         return a0.elapsed_time(a1) / steps, mm.stats()
 
+    def _md_protocol(mm, cc, n_equil, n_prod, skin_mA, drift_A):
+        """The paper's timing protocol (100 equilibration + 250 production steps, neighbour list with a skin,
+        rebuilt when needed) on synthetic motion: the whole configuration drifts rigidly by `drift_A` per step (0.03 A = a
+        hydrogen atom at thermal speed, 300 K, 1 fs), so every pair distance -- hence E, F, W -- stays put while the
+        displacement test fires after skin / 2 / drift steps: reuse steps replay the captured graph, rebuild steps run the
+        cell list; positions leave the box and are wrapped by the library.  (Forces of the random-weight models are not
+        physical: integrating them would say nothing about a real run's rebuild cadence.)"""
+        mm.set_option("skin_mA", skin_mA)
+        NN = len(cc["pos"])
+        p_ = torch.from_numpy(cc["pos"]).to(dev); t_ = torch.from_numpy(cc["types"]).to(dev)
+        o_ = None if cc["ghost_owner"] is None else torch.from_numpy(np.ascontiguousarray(cc["ghost_owner"], np.int32)).to(dev)
+        out_ = (torch.empty(1, dtype=torch.float64, device=dev), torch.empty((NN, 3), dtype=torch.float64, device=dev),
+                torch.empty(6, dtype=torch.float64, device=dev))
+        step_v = torch.tensor([drift_A * 0.6, drift_A * 0.64, drift_A * 0.48], dtype=torch.float64, device=dev)   # |v| = drift_A
+        # (stream is torch's current stream: the position update and the evaluation are ordered on it)
+        for _ in range(n_equil):
+            p_ += step_v
+            mm.compute(p_, t_, cc["box"], cc["n_local"], cc["n_ghost"], o_, out=out_, stream=stream)
+        torch.cuda.synchronize(dev)
+        s0 = mm.stats()
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record(stream)
+        for _ in range(n_prod):
+            p_ += step_v
+            mm.compute(p_, t_, cc["box"], cc["n_local"], cc["n_ghost"], o_, out=out_, stream=stream)
+        a1.record(stream)
+        torch.cuda.synchronize(dev)
+        s1 = mm.stats()
+        ms = a0.elapsed_time(a1) / n_prod
+        return dict(n_local=cc["n_local"], equilibration_steps=n_equil, production_steps=n_prod, skin_A=skin_mA / 1000.0,
+                    drift_A_per_step=drift_A, ms_per_step=ms, atom_steps_per_s=cc["n_local"] / (ms * 1e-3),
+                    list_rebuilds=s1["n_list_rebuilds"] - s0["n_list_rebuilds"], list_reuses=s1["n_list_reuses"] - s0["n_list_reuses"],
+                    graph_replays=s1["n_graph_replays"] - s0["n_graph_replays"])
+
     extra = {}
     if rank == 0 and world == 1 and not args.no_extra:
         ms_r, st_r = _time_mode(m, c, 1000, args.steps, max(args.warmup, 3))
@@ -421,6 +455,18 @@ def main():
                                         launches_rebuild=st0["n_launches"], atoms_kept_by_pruning=st0["n_reached"],
                                         **({"ms_rebuild_unpruned": ms2} if ms2 is not None else {}))
         extra["other_configs"] = small
+        # MD timing protocol of the paper (100 + 250 steps; at 1M atoms 10 + 40 to keep the default run short)
+        md = {}
+        for kk, (ne, npd) in ((1, (100, 250)), (2, (100, 250)), (k, (10, 40))):
+            cc, bb = (c, blob) if kk == k else _cached_workload(kk)
+            mk = cc["model"]
+            if kk == k:
+                md[f"config{kk}"] = _md_protocol(m, cc, ne, npd, 1000, 0.03)
+                m.set_option("skin_mA", 0)
+            else:
+                with P.Model(bb, mk["n_species"], mk["rc"], len(cc["pos"])) as mm:
+                    md[f"config{kk}"] = _md_protocol(mm, cc, ne, npd, 1000, 0.03)
+        extra["md_protocol"] = md
 
     if rank == 0:
         cpu = None
