@@ -980,8 +980,7 @@ __attribute__((visibility("default"))) int mlp_compute(mlp_model* m, const doubl
     L.apu_bwd = m->apu_bwd;
     m->marks.clear();
     m->stats.n_calls++;
-    const int F = m->F, K = m->K, T = m->T, R = m->R;
-    const float rcf = (float)m->rc;
+    const int T = m->T;
 
     // ---- capacity (atoms): buffers only grow ----
     if (N > m->cap_atoms) {

@@ -46,7 +46,6 @@ using namespace tc;
 constexpr int F = 128;
 constexpr int KP = 96;                        // 4 split terms x 24 basis slots
 constexpr int LBO = 128, SBO = (KP / 8) * 128;          // 1536
-constexpr int A_CHUNK_BYTES = (F / 8) * SBO;            // 24576
 
 // -------------------------------------------------------------------------------------------------------------
 // producer helper: R_e = fc (1, rho_1..rho_K) [and R'_e = d/dd of it] for basis slots 8h..8h+7 of one edge
@@ -161,7 +160,7 @@ constexpr int BWD_PD = 3;                               // consumer loop: shared
 constexpr int GW = 16;                                  // gather window (edges in flight per thread)
 constexpr int RING_BYTES = GW * F * 16;                 // 32768
 constexpr int G_OFF_B = 0, G_OFF_P = 2 * BB_BYTES, G_OFF_RING = G_OFF_P + 2 * P_BYTES, G_OFF_META = G_OFF_RING + RING_BYTES,
-              G_OFF_BAR = G_OFF_META + 4 * NEB * 16, GROUP_BYTES = G_OFF_BAR + 128;
+              G_OFF_BAR = G_OFF_META + 4 * NEB * 16;      // (layout of k_msg_bwd0's pipelines: GROUP0_BYTES below)
 // k_msg_bwd reduces FOUR planes per edge (db | beta' vb_x | beta' vb_y | beta' vb_z, see its consumer loop); the layer-0
 // species-table kernel k_msg_bwd0 keeps the three-plane layout above
 constexpr int P4_ROW = 4 * F * 4 + 64;
@@ -293,7 +292,6 @@ __global__ void __launch_bounds__(FWDG_THREADS, 1) k_msg_fwd_g(const FwdParams p
         const int f = ltid;
         const float4* __restrict__ Q4 = p.Q4 + f;
         const float* __restrict__ Q1 = p.Q1 + f;
-        const float2* __restrict__ Q2 = p.Q2 + f;
         const float* __restrict__ s_in = p.s + f;
         const float* __restrict__ v_in = p.v + f;
         float* __restrict__ sn = p.sn + f;
@@ -301,8 +299,7 @@ __global__ void __launch_bounds__(FWDG_THREADS, 1) k_msg_fwd_g(const FwdParams p
         const uint32_t lane_base = tmem_base + ((uint32_t)(lwarp * 32) << 16);
         float4 qa4[8], qb4[8];
         float qa1[8], qb1[8];
-        float2 qa2[8], qb2[8];
-#define FWD_ISSUE(Q4R, Q1R, Q2R, META8)                                                   \
+#define FWD_ISSUE(Q4R, Q1R, META8)                                                   \
     {                                                                                     \
         _Pragma("unroll") for (int i_ = 0; i_ < 8; i_++) {                                \
             const size_t row_ = (size_t)__float_as_int((META8)[i_].w) * F;                \
@@ -328,7 +325,7 @@ __global__ void __launch_bounds__(FWDG_THREADS, 1) k_msg_fwd_g(const FwdParams p
             if (HAS_V && ntiles > 0 && !pre) {
                 mbar_wait(&b_full[it & 1], (it >> 1) & 1);
                 const float4* m0 = sMeta + (it & 1) * NE;
-                FWD_ISSUE(qa4, qa1, qa2, m0);
+                FWD_ISSUE(qa4, qa1, m0);
             }
             pre = false;
             int a_rel = 0;
@@ -351,7 +348,7 @@ __global__ void __launch_bounds__(FWDG_THREADS, 1) k_msg_fwd_g(const FwdParams p
                 rs = s_in[a * F];
                 if (HAS_V) { rv0 = v_in[a * 3 * F]; rv1 = v_in[a * 3 * F + F]; rv2 = v_in[a * 3 * F + 2 * F]; }
             };
-#define FWD_COMPUTE(BI, Q4R, Q1R, Q2R)                                                                      \
+#define FWD_COMPUTE(BI, Q4R, Q1R)                                                                      \
     {                                                                                                       \
         const int E8_ = e_begin + t * NE + (BI) * 8;                                                        \
         if (E8_ < e_end) {                                                                                  \
@@ -385,21 +382,21 @@ __global__ void __launch_bounds__(FWDG_THREADS, 1) k_msg_fwd_g(const FwdParams p
             for (int t = 0; t < ntiles; t++, it++) {
                 const int buf = it & 1;
                 const float4* meta = sMeta + buf * NE;
-                FWD_ISSUE(qb4, qb1, qb2, meta + 8);
+                FWD_ISSUE(qb4, qb1, meta + 8);
                 mbar_wait(&t_full[buf], (it >> 1) & 1);
                 tc_fence_after();
-                FWD_COMPUTE(0, qa4, qa1, qa2);
-                FWD_ISSUE(qa4, qa1, qa2, meta + 16);
-                FWD_COMPUTE(1, qb4, qb1, qb2);
-                FWD_ISSUE(qb4, qb1, qb2, meta + 24);
-                FWD_COMPUTE(2, qa4, qa1, qa2);
+                FWD_COMPUTE(0, qa4, qa1);
+                FWD_ISSUE(qa4, qa1, meta + 16);
+                FWD_COMPUTE(1, qb4, qb1);
+                FWD_ISSUE(qb4, qb1, meta + 24);
+                FWD_COMPUTE(2, qa4, qa1);
                 if (HAS_V && (t + 1 < ntiles || next_has)) {       // first batch of the CTA's next tile
                     mbar_wait(&b_full[buf ^ 1], ((it + 1) >> 1) & 1);
                     const float4* mn = sMeta + (buf ^ 1) * NE;
-                    FWD_ISSUE(qa4, qa1, qa2, mn);
+                    FWD_ISSUE(qa4, qa1, mn);
                     pre = t + 1 == ntiles;
                 }
-                FWD_COMPUTE(3, qb4, qb1, qb2);
+                FWD_COMPUTE(3, qb4, qb1);
                 tc_fence_before();
                 bar_arrive(NB + buf, 224);              // tile consumed: 128 consumers arrive, 96 producers wait (named barrier)
             }
@@ -615,8 +612,6 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
         const float* __restrict__ v1b = p.v1b + f;
         float* __restrict__ phib = p.phib + f;
         float* __restrict__ vb_out = p.vb_out + f;
-        float4* __restrict__ Gout = p.G;
-        const bool first = p.first != 0;
         const uint32_t lane_base = tmem_base + ((uint32_t)(lwarp * 32) << 16);
         // Rolling gather window: the W = 16 next neighbour rows of this thread's channel are always in flight as
         // cp.async copies into private 16-byte shared-memory slots (one commit group per edge, wait_group W-1 before
@@ -895,7 +890,6 @@ __global__ void __launch_bounds__(BWD_THREADS, 1) k_msg_bwd(const BwdParams p) {
             const int e_begin = __ldg(row_ptr + a0), e_end = __ldg(row_ptr + a1);
             const int ntiles = (e_end - e_begin + NEB - 1) / NEB;
             for (int t = 0; t < ntiles; t++, it++) {
-                const int buf = it & 1;
                 for (int h = 0; h < 2; h++) {
                     const int E8 = e_begin + t * NEB + h * 8;
                     if (E8 >= e_end) continue;
