@@ -80,8 +80,11 @@ def test_random_systems_options_and_trajectories(seed):
                 assert np.isfinite(e) and np.isfinite(f).all() and np.isfinite(w).all(), (label, step)
                 assert de <= etol, (label, step, de, etol)
                 if rms > 0:
-                    assert np.sqrt(((f - fr) ** 2).mean()) <= 2e-3 * rms, (label, step)
-                    assert np.abs(f - fr).max() <= max(1e-2 * rms, 1e-3 * np.abs(fr).max()), (label, step)
+                    # A17d: absolute floor 1e-8 |E| per Angstrom -- a force that cancels to 1e-6 of its natural scale |E| / rc (one
+                    # pair near the cutoff, caught where dE/dd changes sign: extended fuzz, seed 37) has no relative accuracy in fp32
+                    ffloor = 1e-8 * abs(ref["energy"])
+                    assert np.sqrt(((f - fr) ** 2).mean()) <= max(2e-3 * rms, ffloor), (label, step)
+                    assert np.abs(f - fr).max() <= max(1e-2 * rms, 1e-3 * np.abs(fr).max(), 3 * ffloor), (label, step)
                 wn = np.linalg.norm(ref["virial"])
                 if wn > 0:
                     assert np.linalg.norm(w - ref["virial"]) <= 2e-3 * wn, (label, step)
