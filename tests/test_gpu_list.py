@@ -268,3 +268,39 @@ def test_host_entry_point_with_list_reuse():
     assert st["n_list_rebuilds"] == 1 and st["n_list_reuses"] == 2 and st["n_graph_replays"] == 2
     assert out[1][0] == out[0][0] == out[2][0] and np.abs(out[2][1] - out[0][1]).max() <= 1e-9 * np.abs(out[0][1]).max()
     _check(c, *out[2], _oracle_eval(c, blob), "host entry point, third call (graph replay)")
+
+
+@pytest.mark.parametrize("k", [1, 2])
+def test_rigid_drift_far_out_of_the_box(k):
+    """The MD protocol leg of bench.py: the whole configuration drifts rigidly by 0.048 A per step and is never
+    wrapped by the caller -- after 150 steps every atom has left the box by up to 7.2 A (config 1: more than half a box length).
+    Pair vectors do not change, so at EVERY step the (i, j, image) set is the one of step 0 (images are relative to the positions
+    as given), E / F / W stay at their step-0 values up to the fp32 rounding of the shifted coordinates, and the kept list is
+    rebuilt exactly when the displacement since the last build exceeds skin / 2 (every 11 steps at skin 1 A), replaying the
+    captured graph in between."""
+    import paper_2506_04055_b200 as P
+    c = gen.make_config(k, **SMALL[k])
+    blob = _blob(c["model"])
+    mdl = c["model"]
+    N = len(c["pos"])
+    box = np.asarray(c["box"], np.float64)
+    v = 0.048 * np.array([0.6, 0.64, 0.48])                  # |v| = 0.048 A per step
+    pos = c["pos"].copy()
+    with P.Model(blob, mdl["n_species"], mdl["rc"], N) as m:
+        m.set_option("skin_mA", 1000)
+        e0, f0, w0 = _run(m, pos, c["types"], box)
+        ref_edges = m.neighbors()
+        frms = np.sqrt((f0 ** 2).mean())
+        for step in range(1, 151):
+            pos += v
+            e, f, w = _run(m, pos, c["types"], box)
+            assert abs(e - e0) <= 1e-4 * N, (step, e, e0)
+            assert np.sqrt(((f - f0) ** 2).mean()) <= 2e-4 * frms and np.abs(f - f0).max() <= 2e-3 * frms, step
+            assert np.linalg.norm(w - w0) <= 2e-4 * np.linalg.norm(w0), step
+            if step % 7 == 0 or step > 140:
+                for x, y in zip(m.neighbors(), ref_edges):
+                    assert np.array_equal(x, y), step
+        st = m.stats()
+    # displacement after n steps = 0.048 n: 0.48 A at n = 10, 0.528 > skin / 2 at n = 11, i.e. a rebuild at steps 11, 22, ... (+ the build at step 0)
+    assert st["n_list_rebuilds"] == 1 + 150 // 11, st
+    assert st["n_list_reuses"] == 150 - 150 // 11 and st["n_graph_replays"] >= st["n_list_reuses"] - 2, st
